@@ -1,0 +1,505 @@
+/*
+ * orc.c -- fp64 CPU ORACLE (test infrastructure, NOT the product; see orc.h).
+ *
+ * Plain, slow, step-by-step restatement of the particle hot path of arXiv 2511.17710 in the
+ * paper's order and notation.  P:nnn = line nnn of PAPER.md.  No tiling, no sorting, no fusion,
+ * absolute coordinates, OpenMP over particles only.  Shares nothing with the CUDA path.
+ */
+#include "orc.h"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define NG ORC_NGHOST
+static const double PI = 3.14159265358979323846264338327950288;
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------------------------------
+ * array geometry: planar padded arrays, x1 fastest, N_GHOST = 2 each side.
+ * element (i,j,k) of the active grid sits at padded index (i+2, j+2, k+2).
+ * ------------------------------------------------------------------------------------------ */
+static inline int64_t pext(const orc_grid *g, int d) { return d < g->D ? (int64_t)g->N[d] + 2 * NG : 1; }
+int64_t orc_padded_size(const orc_grid *g) { return pext(g, 0) * pext(g, 1) * pext(g, 2); }
+static inline int64_t pidx(const orc_grid *g, int i, int j, int k) {
+    int64_t P0 = pext(g, 0), P1 = pext(g, 1);
+    if (g->D == 2) return (int64_t)(i + NG) + P0 * (int64_t)(j + NG);
+    return (int64_t)(i + NG) + P0 * ((int64_t)(j + NG) + P1 * (int64_t)(k + NG));
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O1  metric
+ * ------------------------------------------------------------------------------------------ */
+static inline double cell_size(const orc_grid *g, int d) { return (g->xmax[d] - g->xmin[d]) / (double)g->N[d]; }
+
+double orc_theta_of_T(double vt, double T) {
+    return T + 2.0 * vt * T * (1.0 - 2.0 * T / PI) * (1.0 - T / PI);
+}
+double orc_dtheta_dT(double vt, double T) {
+    return 1.0 + 2.0 * vt + 12.0 * vt * (T / PI) * (T / PI - 1.0);
+}
+
+/* quasi-spherical helpers */
+static inline double qs_Rmin(const orc_grid *g) { return log(g->xmin[0] - g->r0); }
+static inline double qs_dR(const orc_grid *g) { return (log(g->xmax[0] - g->r0) - log(g->xmin[0] - g->r0)) / (double)g->N[0]; }
+static inline double qs_dT(const orc_grid *g) { return PI / (double)g->N[1]; }
+
+/* (r, theta) of a code position for the two axisymmetric metrics */
+static void r_theta_of_code(const orc_grid *g, double x1, double x2, double *r, double *th) {
+    if (g->kind == ORC_SPH) {
+        *r = g->xmin[0] + x1 * cell_size(g, 0);
+        *th = x2 * (PI / (double)g->N[1]);
+    } else {
+        double R = qs_Rmin(g) + x1 * qs_dR(g);
+        double T = x2 * qs_dT(g);
+        *r = g->r0 + exp(R);
+        *th = orc_theta_of_T(g->vartheta, T);
+    }
+}
+
+void orc_metric_h(const orc_grid *g, const double x[3], double h[3]) {
+    if (g->kind == ORC_CART) {
+        for (int d = 0; d < 3; ++d) {
+            if (d < g->D) { double dx = cell_size(g, d); h[d] = dx * dx; }
+            else h[d] = 1.0;
+        }
+    } else if (g->kind == ORC_SPH) {
+        double dr = cell_size(g, 0), dth = PI / (double)g->N[1];
+        double r = g->xmin[0] + x[0] * dr, th = x[1] * dth;
+        h[0] = dr * dr;
+        h[1] = (r * dth) * (r * dth);
+        h[2] = (r * sin(th)) * (r * sin(th));
+    } else {
+        double dR = qs_dR(g), dT = qs_dT(g);
+        double R = qs_Rmin(g) + x[0] * dR, T = x[1] * dT;
+        double eR = exp(R), r = g->r0 + eR;
+        double th = orc_theta_of_T(g->vartheta, T), dthdT = orc_dtheta_dT(g->vartheta, T);
+        h[0] = (dR * eR) * (dR * eR);
+        h[1] = (dT * dthdT * r) * (dT * dthdT * r);
+        h[2] = (r * sin(th)) * (r * sin(th));
+    }
+}
+
+/* Eq. 8: min over cell centres of (sum_d 1/h_dd)^(-1/2), d < D */
+double orc_dx_min(const orc_grid *g) {
+    double best = INFINITY;
+    int K = g->D == 3 ? g->N[2] : 1;
+    for (int k = 0; k < K; ++k)
+        for (int j = 0; j < g->N[1]; ++j)
+            for (int i = 0; i < g->N[0]; ++i) {
+                double x[3] = { i + 0.5, j + 0.5, k + 0.5 }, h[3];
+                orc_metric_h(g, x, h);
+                double s = 0.0;
+                for (int d = 0; d < g->D; ++d) s += 1.0 / h[d];
+                double v = 1.0 / sqrt(s);
+                if (v < best) best = v;
+            }
+    return best;
+}
+
+/* App. B: inverse of theta(T).  With s = T/pi the cubic is
+ *   4 vt s^3 - 6 vt s^2 + (1 + 2 vt) s - theta/pi = 0,
+ * depressed with u = s - 1/2:  4 vt u^3 + (1 - vt) u + (1/2 - theta/pi) = 0  (one real root for 0 < vt < 1).
+ * Cardano on the depressed form, then two Newton steps on theta(T) - theta. */
+double orc_T_of_theta(double vt, double theta) {
+    if (vt == 0.0) return theta;                        /* "only performed when vartheta != 0" */
+    double p = (1.0 - vt) / (4.0 * vt);
+    double q = (0.5 - theta / PI) / (4.0 * vt);
+    double disc = sqrt(q * q / 4.0 + p * p * p / 27.0);
+    double u = cbrt(-q / 2.0 + disc) + cbrt(-q / 2.0 - disc);
+    double T = PI * (u + 0.5);
+    for (int it = 0; it < 2; ++it) T -= (orc_theta_of_T(vt, T) - theta) / orc_dtheta_dT(vt, T);
+    return T;
+}
+
+/* Eq. (B3) evaluated literally; `theta` and `vt` as printed.  The extracted text has the radicand
+ * pi^2 (4 - vt)(1 + 2 vt); the algebra requires (1 + 2 vt)^2.  The sign of vt selects:
+ * vt > 0 -> corrected radicand, vt < 0 -> |vt| with the radicand exactly as printed (for the pin test). */
+double orc_T_of_theta_printed_B3(double vt_signed, double theta) {
+    int printed = vt_signed < 0.0;
+    double vt = fabs(vt_signed);
+    double f = printed ? (1.0 + 2.0 * vt) : (1.0 + 2.0 * vt) * (1.0 + 2.0 * vt);
+    double rad = 108.0 * vt * theta * theta - 108.0 * vt * PI * theta + PI * PI * (4.0 - vt) * f;
+    double Theta = cbrt(sqrt(3.0 * vt * vt * vt) * sqrt(rad) - 9.0 * vt * vt * (PI - 2.0 * theta));
+    return pow(PI, 2.0 / 3.0) / 12.0 *
+           (6.0 * cbrt(PI) - pow(2.0, 4.0 / 3.0) * pow(3.0 * PI, 2.0 / 3.0) * (1.0 - vt) / Theta +
+            pow(2.0, 2.0 / 3.0) * cbrt(3.0) * Theta / vt);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O5 / O6  coordinate maps
+ * ------------------------------------------------------------------------------------------ */
+void orc_code_to_cart(const orc_grid *g, const double x[3], double X[3]) {
+    if (g->kind == ORC_CART) {
+        for (int d = 0; d < 3; ++d) X[d] = d < g->D ? g->xmin[d] + x[d] * cell_size(g, d) : x[d];
+        return;
+    }
+    double r, th, phi = x[2];
+    r_theta_of_code(g, x[0], x[1], &r, &th);            /* P:285 / P:305-310 */
+    X[0] = r * sin(th) * cos(phi);                      /* P:287-289 / P:311-315 */
+    X[1] = r * sin(th) * sin(phi);
+    X[2] = r * cos(th);
+}
+
+void orc_cart_to_code(const orc_grid *g, const double X[3], double x[3]) {
+    if (g->kind == ORC_CART) {
+        for (int d = 0; d < 3; ++d) x[d] = d < g->D ? (X[d] - g->xmin[d]) / cell_size(g, d) : X[d];
+        return;
+    }
+    double r = sqrt(X[0] * X[0] + X[1] * X[1] + X[2] * X[2]);          /* P:294 / P:320 */
+    double th = PI / 2.0 - atan2(X[2], sqrt(X[0] * X[0] + X[1] * X[1])); /* P:296 / P:322 */
+    double phi = PI - atan2(X[1], -X[0]);                                /* P:297 / P:323 */
+    if (phi >= 2.0 * PI) phi -= 2.0 * PI;               /* atan2 = -pi exactly (y = -0) would give 2 pi */
+    if (g->kind == ORC_SPH) {
+        x[0] = (r - g->xmin[0]) / cell_size(g, 0);
+        x[1] = th / (PI / (double)g->N[1]);
+    } else {
+        x[0] = (log(r - g->r0) - qs_Rmin(g)) / qs_dR(g);
+        x[1] = orc_T_of_theta(g->vartheta, th) / qs_dT(g);
+    }
+    x[2] = phi;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O2  gather, P:131-133 with the first-order (cloud-in-cell) shape, reading G1:
+ * direct multilinear interpolation of each component on its own staggered lattice.
+ * Yee staggering:  E1(i+1/2,j,k) E2(i,j+1/2,k) E3(i,j,k+1/2)
+ *                                      B1(i,j+1/2,k+1/2) B2(i+1/2,j,k+1/2) B3(i+1/2,j+1/2,k)
+ * ------------------------------------------------------------------------------------------ */
+static const int STAG[6][3] = { {1,0,0}, {0,1,0}, {0,0,1}, {0,1,1}, {1,0,1}, {1,1,0} };  /* 1 = half-cell shift */
+
+void orc_gather(const orc_grid *g, const float *const F[6], const int32_t i[3], const double d[3], double out[6]) {
+    for (int c = 0; c < 6; ++c) {
+        int b[3] = {0, 0, 0};
+        double f[3] = {0, 0, 0};
+        for (int a = 0; a < g->D; ++a) {
+            if (!STAG[c][a]) { b[a] = i[a]; f[a] = d[a]; }
+            else if (d[a] < 0.5) { b[a] = i[a] - 1; f[a] = d[a] + 0.5; }
+            else { b[a] = i[a]; f[a] = d[a] - 0.5; }
+        }
+        double acc = 0.0;
+        int nk = g->D == 3 ? 2 : 1;
+        for (int ck = 0; ck < nk; ++ck)
+            for (int cj = 0; cj < 2; ++cj)
+                for (int ci = 0; ci < 2; ++ci) {
+                    double wgt = (ci ? f[0] : 1.0 - f[0]) * (cj ? f[1] : 1.0 - f[1]);
+                    if (g->D == 3) wgt *= (ck ? f[2] : 1.0 - f[2]);
+                    acc += wgt * (double)F[c][pidx(g, b[0] + ci, b[1] + cj, g->D == 3 ? b[2] + ck : 0)];
+                }
+        out[c] = acc;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O3  basis change: tetrad A^hat{i} = sqrt(h_ii) A^i at the particle (G2, G5), then for the
+ * axisymmetric metrics the rotation (r,theta,phi)-hat -> (x,y,z)-hat, i.e. the normalised Jacobian
+ * of P:287-289.  x = (x1, x2, x3) code position, with x3 = phi for the axisymmetric metrics.
+ * ------------------------------------------------------------------------------------------ */
+void orc_to_cartesian_basis(const orc_grid *g, const double x[3], const double A[3], double out[3]) {
+    double h[3];
+    orc_metric_h(g, x, h);
+    double Ar = sqrt(h[0]) * A[0], At = sqrt(h[1]) * A[1], Ap = sqrt(h[2]) * A[2];
+    if (g->kind == ORC_CART) { out[0] = Ar; out[1] = At; out[2] = Ap; return; }
+    double r, th, phi = x[2];
+    r_theta_of_code(g, x[0], x[1], &r, &th);
+    double st = sin(th), ct = cos(th), sp = sin(phi), cp = cos(phi);
+    out[0] = Ar * st * cp + At * ct * cp - Ap * sp;
+    out[1] = Ar * st * sp + At * ct * sp + Ap * cp;
+    out[2] = Ar * ct - At * st;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O4  relativistic Boris (Eq. 3, reading G3): half electric kick, rotation, half kick.
+ * ------------------------------------------------------------------------------------------ */
+void orc_boris(double u[3], const double E[3], const double B[3], double qm, double dt) {
+    double eps = qm * dt / 2.0;
+    double um[3], t[3], s[3], up[3], uplus[3];
+    for (int a = 0; a < 3; ++a) um[a] = u[a] + eps * E[a];
+    double gm = sqrt(1.0 + um[0] * um[0] + um[1] * um[1] + um[2] * um[2]);
+    for (int a = 0; a < 3; ++a) t[a] = eps * B[a] / gm;
+    double t2 = t[0] * t[0] + t[1] * t[1] + t[2] * t[2];
+    for (int a = 0; a < 3; ++a) s[a] = 2.0 * t[a] / (1.0 + t2);
+    up[0] = um[0] + (um[1] * t[2] - um[2] * t[1]);
+    up[1] = um[1] + (um[2] * t[0] - um[0] * t[2]);
+    up[2] = um[2] + (um[0] * t[1] - um[1] * t[0]);
+    uplus[0] = um[0] + (up[1] * s[2] - up[2] * s[1]);
+    uplus[1] = um[1] + (up[2] * s[0] - up[0] * s[2]);
+    uplus[2] = um[2] + (up[0] * s[1] - up[1] * s[0]);
+    for (int a = 0; a < 3; ++a) u[a] = uplus[a] + eps * E[a];
+}
+
+/* ------------------------------------------------------------------------------------------
+ * steps 3-7 + O7 crossing bookkeeping (readings G9, G11)
+ * ------------------------------------------------------------------------------------------ */
+static inline int floor_mod(int a, int n) { int r = a % n; return r < 0 ? r + n : r; }
+
+int orc_gather_push(const orc_grid *g, const float *const F[6], const orc_particles *in, orc_particles *out,
+                    double qm, double dt) {
+    const int D = g->D, axisym = g->kind != ORC_CART;
+    if (axisym && D != 2) return -1;
+    int64_t n = in->n;
+#pragma omp parallel for schedule(static)
+    for (int64_t p = 0; p < n; ++p) {
+        int alive = in->tag ? in->tag[p] != 0 : 1;
+        int32_t ic[3] = {0, 0, 0};
+        double dc[3] = {0, 0, 0}, u[3];
+        for (int a = 0; a < D; ++a) { ic[a] = in->i[a][p]; dc[a] = in->d[a][p]; }
+        for (int a = 0; a < 3; ++a) u[a] = in->u[a][p];
+        double phi = axisym ? in->phi[p] : 0.0;
+        int tag = alive;
+        if (alive) {
+            /* step 3: interpolate */
+            double EB[6];
+            orc_gather(g, F, ic, dc, EB);
+            /* step 4: to the global Cartesian basis, at the particle position */
+            double x[3] = { ic[0] + dc[0], ic[1] + dc[1], axisym ? phi : (D == 3 ? ic[2] + dc[2] : 0.0) };
+            double E[3], B[3];
+            orc_to_cartesian_basis(g, x, EB, E);
+            orc_to_cartesian_basis(g, x, EB + 3, B);
+            /* step 5: u^(n-1/2) -> u^(n+1/2) */
+            orc_boris(u, E, B, qm, dt);
+            /* step 6: x^(n) -> x^(n+1) with u^(n+1/2) / gamma^(n+1/2), in the global Cartesian frame */
+            double gam = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+            double X[3], xn[3];
+            orc_code_to_cart(g, x, X);
+            if (g->kind == ORC_CART) { for (int a = 0; a < D; ++a) X[a] += u[a] / gam * dt; }
+            else { for (int a = 0; a < 3; ++a) X[a] += u[a] / gam * dt; }
+            /* step 7: back to code coordinates */
+            orc_cart_to_code(g, X, xn);
+            if (axisym) phi = xn[2];
+            /* O7: split into cell index and offset, apply the boundary rule of each dimension */
+            for (int a = 0; a < D; ++a) {
+                double fl = floor(xn[a]);
+                int inew = (int)fl;
+                double dnew = xn[a] - fl;
+                if (g->bc[a] == ORC_PERIODIC) inew = floor_mod(inew, g->N[a]);
+                else if (g->bc[a] == ORC_AXIS) {
+                    if (inew >= g->N[a]) { inew = g->N[a] - 1; dnew = nextafter(1.0, 0.0); }   /* theta = pi exactly, G11 */
+                    if (inew < 0) { inew = 0; dnew = 0.0; }
+                } else if (inew < 0 || inew >= g->N[a]) tag = 0;                               /* ABSORB, G9 */
+                ic[a] = inew; dc[a] = dnew;
+            }
+        }
+        for (int a = 0; a < D; ++a) { out->i[a][p] = ic[a]; out->d[a][p] = dc[a]; }
+        for (int a = 0; a < 3; ++a) out->u[a][p] = u[a];
+        if (axisym) out->phi[p] = phi;
+        if (out->w && in->w && out->w != in->w) out->w[p] = in->w[p];
+        if (out->tag) out->tag[p] = (int8_t)tag;
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O8  deposit (Eq. 6, P:155-157 step 8, "modified zig-zag"; readings G6-G8)
+ * ------------------------------------------------------------------------------------------ */
+static inline double omega(double W, int s) { return s ? W : 1.0 - W; }
+
+static inline void jadd(double *J, int64_t idx, double v) {
+#pragma omp atomic
+    J[idx] += v;
+}
+
+/* one straight segment inside cell c: displacement Dv, midpoint offset W (cell-local), Q = q w / dt */
+static void deposit_segment_3d(const orc_grid *g, double *const J[3], const int c[3], const double Dv[3], const double W[3], double Q) {
+    for (int comp = 0; comp < 3; ++comp) {
+        int a = (comp + 1) % 3, b = (comp + 2) % 3;       /* cyclic transverse pair */
+        for (int sb = 0; sb < 2; ++sb)
+            for (int sa = 0; sa < 2; ++sa) {
+                double sigma = (sa == sb) ? 1.0 : -1.0;
+                double wgt = omega(W[a], sa) * omega(W[b], sb) + sigma * Dv[a] * Dv[b] / 12.0;   /* F2 / G7 */
+                int n[3] = { c[0], c[1], c[2] };
+                n[a] += sa; n[b] += sb;
+                jadd(J[comp], pidx(g, n[0], n[1], n[2]), Q * Dv[comp] * wgt);
+            }
+    }
+}
+
+static void deposit_segment_2d(const orc_grid *g, double *const J[3], const int c[3], const double Dv[3], const double W[3],
+                               double Q, double half_qw_v3) {
+    for (int s = 0; s < 2; ++s) {
+        jadd(J[0], pidx(g, c[0], c[1] + s, 0), Q * Dv[0] * omega(W[1], s));       /* J1[c + (0,s2)] */
+        jadd(J[1], pidx(g, c[0] + s, c[1], 0), Q * Dv[1] * omega(W[0], s));       /* J2[c + (s1,0)] */
+    }
+    for (int s2 = 0; s2 < 2; ++s2)                                                  /* G8: out-of-plane, velocity form */
+        for (int s1 = 0; s1 < 2; ++s1)
+            jadd(J[2], pidx(g, c[0] + s1, c[1] + s2, 0), half_qw_v3 * omega(W[0], s1) * omega(W[1], s2));
+}
+
+int orc_deposit(const orc_grid *g, const orc_particles *po, const orc_particles *pn, double *const J[3], double q, double dt) {
+    const int D = g->D, axisym = g->kind != ORC_CART;
+    int64_t n = po->n;
+    int err = 0;
+#pragma omp parallel for schedule(static)
+    for (int64_t p = 0; p < n; ++p) {
+        int alive = (po->tag ? po->tag[p] != 0 : 1) && (pn->tag ? pn->tag[p] != 0 : 1);
+        if (!alive) continue;                              /* G9: absorbed particles deposit nothing */
+        int c1[3] = {0, 0, 0}, c2[3] = {0, 0, 0}, di[3] = {0, 0, 0};
+        double a[3] = {0, 0, 0}, b[3] = {0, 0, 0}, r[3] = {0, 0, 0};
+        for (int k = 0; k < D; ++k) {
+            int dd = pn->i[k][p] - po->i[k][p];
+            if (g->bc[k] == ORC_PERIODIC) dd -= g->N[k] * (int)lround((double)dd / (double)g->N[k]);
+            if (dd < -1 || dd > 1) {
+#pragma omp atomic write
+                err = -2;
+                dd = 0;
+            }
+            di[k] = dd;
+            a[k] = po->d[k][p];
+            b[k] = dd + pn->d[k][p];                       /* new position in the OLD cell's frame */
+            r[k] = dd == 0 ? 0.5 * (a[k] + b[k]) : (dd > 0 ? 1.0 : 0.0);   /* relay point, small numbers only */
+            c1[k] = po->i[k][p];
+            c2[k] = po->i[k][p] + dd;                      /* un-wrapped: may be -1 or N -> ghosts, folded later */
+        }
+        double D1[3] = {0, 0, 0}, W1[3] = {0, 0, 0}, D2[3] = {0, 0, 0}, W2[3] = {0, 0, 0};
+        for (int k = 0; k < D; ++k) {
+            D1[k] = r[k] - a[k];  W1[k] = 0.5 * (a[k] + r[k]);
+            D2[k] = b[k] - r[k];  W2[k] = 0.5 * (r[k] + b[k]) - di[k];
+        }
+        double Q = q * po->w[p] / dt;
+        if (D == 3) {
+            deposit_segment_3d(g, J, c1, D1, W1, Q);
+            deposit_segment_3d(g, J, c2, D2, W2, Q);
+        } else {
+            /* out-of-plane rate q w v3_code, half per segment (G8); v3_code = v^hat3 / sqrt(h33(x_mid)) */
+            double ux = pn->u[0][p], uy = pn->u[1][p], uz = pn->u[2][p];
+            double gam = sqrt(1.0 + ux * ux + uy * uy + uz * uz);
+            double v3;
+            if (!axisym) v3 = uz / gam;                    /* h33 = 1 */
+            else {
+                double dphi = pn->phi[p] - po->phi[p];
+                dphi -= 2.0 * PI * floor((dphi + PI) / (2.0 * PI));      /* shorter arc, (-pi, pi] up to rounding */
+                double phm = po->phi[p] + 0.5 * dphi;
+                double xm[3] = { c1[0] + 0.5 * (a[0] + b[0]), c1[1] + 0.5 * (a[1] + b[1]), phm }, h[3];
+                orc_metric_h(g, xm, h);
+                double sh = sqrt(h[2]);
+                v3 = sh < 1e-12 ? 0.0 : ((-ux * sin(phm) + uy * cos(phm)) / gam) / sh;
+            }
+            double hv = 0.5 * q * po->w[p] * v3;
+            deposit_segment_2d(g, J, c1, D1, W1, Q, hv);
+            deposit_segment_2d(g, J, c2, D2, W2, Q, hv);
+        }
+    }
+    return err;
+}
+
+/* "currents synchronization" for a single periodic box: add what landed in the ghost layers of a
+ * periodic dimension onto the opposite active layers, then refill those ghosts with the periodic image. */
+static void fold_one(const orc_grid *g, double *A) {
+    int64_t P[3] = { pext(g, 0), pext(g, 1), pext(g, 2) };
+    int64_t stride[3] = { 1, P[0], P[0] * P[1] };
+    for (int d = 0; d < g->D; ++d) {
+        if (g->bc[d] != ORC_PERIODIC) continue;
+        int N = g->N[d];
+        int a = (d + 1) % 3, b = (d + 2) % 3;
+        for (int64_t ib = 0; ib < P[b]; ++ib)
+            for (int64_t ia = 0; ia < P[a]; ++ia) {
+                double *line = A + ia * stride[a] + ib * stride[b];
+                for (int gi = 0; gi < NG; ++gi) {
+                    int lo = gi, hi = NG + N + gi;          /* padded indices of ghost layers */
+                    line[(int64_t)(lo + N) * stride[d]] += line[(int64_t)lo * stride[d]];
+                    line[(int64_t)(hi - N) * stride[d]] += line[(int64_t)hi * stride[d]];
+                    line[(int64_t)lo * stride[d]] = 0.0;
+                    line[(int64_t)hi * stride[d]] = 0.0;
+                }
+            }
+    }
+    for (int d = 0; d < g->D; ++d) {
+        if (g->bc[d] != ORC_PERIODIC) continue;
+        int N = g->N[d];
+        int a = (d + 1) % 3, b = (d + 2) % 3;
+        for (int64_t ib = 0; ib < P[b]; ++ib)
+            for (int64_t ia = 0; ia < P[a]; ++ia) {
+                double *line = A + ia * stride[a] + ib * stride[b];
+                for (int gi = 0; gi < NG; ++gi) {
+                    int lo = gi, hi = NG + N + gi;
+                    line[(int64_t)lo * stride[d]] = line[(int64_t)(lo + N) * stride[d]];
+                    line[(int64_t)hi * stride[d]] = line[(int64_t)(hi - N) * stride[d]];
+                }
+            }
+    }
+}
+void orc_fold_current(const orc_grid *g, double *const J[3]) { for (int c = 0; c < 3; ++c) fold_one(g, J[c]); }
+void orc_fold_scalar(const orc_grid *g, double *rho) { fold_one(g, rho); }
+
+int orc_step(const orc_grid *g, const float *const F[6], orc_particles *p, double *const J[3], double q, double m, double dt) {
+    const int D = g->D, axisym = g->kind != ORC_CART;
+    int64_t n = p->n;
+    orc_particles old = *p;
+    for (int a = 0; a < D; ++a) {
+        old.i[a] = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n ? n : 1));
+        old.d[a] = (double *)malloc(sizeof(double) * (size_t)(n ? n : 1));
+        memcpy(old.i[a], p->i[a], sizeof(int32_t) * (size_t)n);
+        memcpy(old.d[a], p->d[a], sizeof(double) * (size_t)n);
+    }
+    old.phi = NULL; old.tag = NULL;
+    if (axisym) { old.phi = (double *)malloc(sizeof(double) * (size_t)(n ? n : 1)); memcpy(old.phi, p->phi, sizeof(double) * (size_t)n); }
+    if (p->tag) { old.tag = (int8_t *)malloc((size_t)(n ? n : 1)); memcpy(old.tag, p->tag, (size_t)n); }
+    int rc = orc_gather_push(g, F, p, p, q / m, dt);
+    if (rc == 0) rc = orc_deposit(g, &old, p, J, q, dt);
+    for (int a = 0; a < D; ++a) { free(old.i[a]); free(old.d[a]); }
+    free(old.phi); free(old.tag);
+    return rc;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Eq. 6 checker.  Conformal nodal charge (no 1/sqrt(h)):  rho[n] = sum_p q w prod_d omega(delta_d, s_d)
+ * ------------------------------------------------------------------------------------------ */
+void orc_charge_density(const orc_grid *g, const orc_particles *p, const int8_t *mask, double q, double *rho) {
+    const int D = g->D;
+    for (int64_t k = 0; k < p->n; ++k) {
+        if (mask && !mask[k]) continue;
+        int nk = D == 3 ? 2 : 1;
+        for (int s3 = 0; s3 < nk; ++s3)
+            for (int s2 = 0; s2 < 2; ++s2)
+                for (int s1 = 0; s1 < 2; ++s1) {
+                    double wgt = omega(p->d[0][k], s1) * omega(p->d[1][k], s2);
+                    if (D == 3) wgt *= omega(p->d[2][k], s3);
+                    rho[pidx(g, p->i[0][k] + s1, p->i[1][k] + s2, D == 3 ? p->i[2][k] + s3 : 0)] += q * p->w[k] * wgt;
+                }
+    }
+}
+
+/* R[n] = sum_d (J^d[n] - J^d[n - e_d]) + (rho_new[n] - rho_old[n]) / dt over the valid nodes:
+ * periodic dimension 0..N-1 (ghosts hold the periodic image after the fold), otherwise 0..N. */
+double orc_continuity_residual(const orc_grid *g, double *const J[3], const double *rho_old, const double *rho_new,
+                               double dt, double *R_out) {
+    const int D = g->D;
+    int hi[3];
+    for (int d = 0; d < 3; ++d) hi[d] = d < D ? (g->bc[d] == ORC_PERIODIC ? g->N[d] - 1 : g->N[d]) : 0;
+    double worst = 0.0;
+    for (int k = 0; k <= hi[2]; ++k)
+        for (int j = 0; j <= hi[1]; ++j)
+            for (int i = 0; i <= hi[0]; ++i) {
+                int64_t n = pidx(g, i, j, k);
+                double R = (rho_new[n] - rho_old[n]) / dt;
+                R += J[0][n] - J[0][pidx(g, i - 1, j, k)];
+                R += J[1][n] - J[1][pidx(g, i, j - 1, k)];
+                if (D == 3) R += J[2][n] - J[2][pidx(g, i, j, k - 1)];
+                if (R_out) R_out[n] = R;
+                if (fabs(R) > worst) worst = fabs(R);
+            }
+    return worst;
+}
+
+/* S10 checker: keys non-decreasing; offsets[c] = number of keys < c (exclusive scan of the histogram) */
+int orc_sort_check(const int64_t n, const int32_t *keys, int64_t ncell, const int32_t *offsets) {
+    for (int64_t p = 1; p < n; ++p) if (keys[p] < keys[p - 1]) return 1;
+    for (int64_t p = 0; p < n; ++p) if (keys[p] < 0 || keys[p] >= ncell) return 2;
+    if (offsets) {
+        int64_t p = 0;
+        for (int64_t c = 0; c <= ncell; ++c) {
+            while (p < n && keys[p] < c) ++p;
+            if (offsets[c] != p) return 3;
+        }
+    }
+    return 0;
+}
