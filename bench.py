@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py -- ns/particle/timestep of the particle hot path (push + deposit) on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3] [--shrink 1] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over the synthetic plasma: zero J, ent_step for every species (serial host
+loop over species), periodic ghost fold, plus ent_sort every --sort-every steps (inside the timed region).
+N > 1: one process per GPU (torchrun), every rank pushes an independent replica of the workload ("replicas only",
+DESIGN.md): no data-path collective, weak scaling, time = max over ranks.
+Prints ONE JSON line (rank 0).  --impl reference times the fp64 CPU oracle on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "ns_per_particle_per_timestep_push_plus_deposit"
+UNIT = "ns/particle/step"
+# algorithmic bytes: read the full record + write the changed fields, fused and in place
+PARTICLE_BYTES = {("cart", 3): 60, ("cart", 2): 52, ("axisym", 2): 60}
+GRID_BYTES_PER_CELL = 24 + 24            # E,B read once; J read-modify-write (3 comps x (4 + 4) B)
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def _load_workload(name, shrink, device, rank=0):
+    from paper_2511_17710_b200 import synth
+    if name == "C4s":
+        return synth.config4(shrink, device=device, shuffled=True)
+    return synth.CONFIGS[name](shrink, device=device)
+
+
+class ClockSampler:
+    """nvidia-smi sampled every 100 ms during the timed region (B200_PROFILING.md clocks line)"""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        os.unlink(self.f.name)
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def _oracle_sample(name, target_particles=2_000_000):
+    """a bounded sample of the same recipe for the CPU oracle: the workload with every grid extent divided by `shrink`"""
+    from paper_2511_17710_b200 import synth
+    full = {"C1": 65536, "C2": 2097152, "C3": 134217728, "C4": 536870912, "C4s": 536870912, "C5": 268435456}[name]
+    D = 3 if name in ("C3", "C4", "C4s") else 2
+    shrink = 1
+    while full / (shrink ** D) > target_particles:
+        shrink *= 2
+    return shrink
+
+
+def time_oracle(name, steps, warmup):
+    """fp64 CPU oracle (oracle/orc.c, as it stands) on a bounded sample; returns (ns/particle/step, cores, sample text, ms/step)"""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import parity as P
+    from oracle import orc
+    shrink = _oracle_sample(name)
+    wl = _load_workload(name, shrink, "cpu")
+    og = P.grid_to_orc(orc, wl.grid)
+    F = P.fields_to_orc(wl.fields)
+    parts = [P.species_to_orc(orc, sp) for sp in wl.species]
+    J = orc.zeros_current(og)
+    npart = sum(p.n for p in parts)
+
+    def one():
+        for j in J:
+            j[...] = 0.0
+        for sp, p in zip(wl.species, parts):
+            orc.step(og, F, p, J, sp.q, sp.m, wl.dt)
+        orc.fold_current(og, J)
+    for _ in range(warmup):
+        one()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        one()
+    dt = time.perf_counter() - t0
+    sample = f"{name} recipe with every grid extent / {shrink}: grid {tuple(wl.grid.N)}, {npart} particles, {steps} steps"
+    return dt / (npart * steps) * 1e9, orc.num_threads(), sample, dt / steps * 1e3
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps, warmup = max(1, min(args.steps, 3)), min(args.warmup, 1)
+    v, cores, sample, ms = time_oracle(args.workload, steps, warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps, "warmup": warmup,
+            "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "note": "fp64 CPU oracle on a bounded sample of the workload"},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2511_17710_b200 import binding as bind, synth
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    peak, peak_src = _peaks()
+
+    # ---- inputs: generated on the device, resident in HBM before the timed region ----
+    wl = _load_workload(args.workload, args.shrink, dev, rank)
+    g = wl.grid
+    eg = bind.Grid(D=g.D, N=tuple(g.N), bc=tuple(g.bc), kind=g.kind, xmin=tuple(g.xmin), xmax=tuple(g.xmax), r0=g.r0,
+                   vartheta=g.vartheta)
+    stream = torch.cuda.current_stream()
+    ctx = bind.ent_create(local, stream)
+    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, args.step_impl)
+    bind.ent_set_grid(ctx, eg)
+    absorb = any(b == synth.ABSORB for b in g.bc)
+    parts, spare = [], []
+    for sp in wl.species:
+        p = bind.Particles(cell=synth.pack_cell(g, sp.i), d=sp.d, u=sp.u, w=sp.w, phi=sp.phi,
+                           tag=torch.ones(sp.n, dtype=torch.uint8, device=dev) if absorb else None, q=sp.q, m=sp.m)
+        parts.append(p); spare.append(p.empty_like())
+    wl.species = None
+    F = wl.fields
+    J = bind.zeros_current(eg, dev)
+    npart = sum(p.n for p in parts)
+    ncell = g.ncells
+    pbytes = PARTICLE_BYTES[("cart" if g.kind == synth.CART else "axisym", g.D)]
+
+    launches0 = [0]
+    step_ev = []                       # (start, end) CUDA events around each ent_step launch in the timed region
+    sort_ev = []
+
+    def do_sort(record):
+        for k in range(len(parts)):
+            if record:
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True); a.record(stream)
+            bind.ent_sort(ctx, parts[k], spare[k], None)
+            parts[k], spare[k] = spare[k], parts[k]
+            if record:
+                b.record(stream); sort_ev.append((a, b))
+
+    def one_step(it, record):
+        if args.sort_every > 0 and it > 0 and it % args.sort_every == 0:
+            do_sort(record)
+        bind.ent_zero_current(ctx, J)
+        for p in parts:
+            if record:
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True); a.record(stream)
+            bind.ent_step(ctx, F, p, J, wl.dt)
+            if record:
+                b.record(stream); step_ev.append((a, b))
+        bind.ent_fold_current(ctx, J)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    do_sort(False)                     # particles enter the timed region cell-sorted (BASELINE.json configs 3, 4)
+    it = 0
+    for _ in range(args.warmup):
+        one_step(it, False); it += 1
+    barrier()
+    launches0[0] = bind.ent_get_stat(ctx, bind.STAT_LAUNCHES)
+    clocks = ClockSampler(local) if rank == 0 else None
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record(stream)
+    for _ in range(args.steps):
+        one_step(it, True); it += 1
+    t1.record(stream)
+    barrier()
+    ms = t0.elapsed_time(t1)
+    launches = bind.ent_get_stat(ctx, bind.STAT_LAUNCHES) - launches0[0]
+    clk = clocks.stop() if clocks else None
+    tiled = bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED)
+    strays = bind.ent_get_stat(ctx, bind.STAT_STRAYS)
+    bad = bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES)
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_per_step = ms / args.steps
+    value = ms * 1e6 / (npart * world * args.steps)
+
+    # ---- roofline of the dominant kernel (the fused step kernel), per launch ----
+    k_ms = sum(a.elapsed_time(b) for a, b in step_ev) / max(1, len(step_ev))
+    n_launch_part = npart / len(parts)
+    alg_bytes = pbytes * n_launch_part + GRID_BYTES_PER_CELL * ncell
+    achieved = alg_bytes / (k_ms * 1e-3) / 1e9
+    sort_ms = (sum(a.elapsed_time(b) for a, b in sort_ev) / len(sort_ev)) if sort_ev else None
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": args.traffic,
+                "kernel": "ent_step (fused gather+push+move+deposit), one species per launch", "kernel_ms": k_ms,
+                "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
+                "step_share": k_ms * len(parts) / ms_per_step}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": f"{wl.name} ({wl.note})", "grid": list(g.N), "particles_per_gpu": npart, "species": len(parts),
+                       "dt": wl.dt, "shrink": args.shrink, "sorted_at_start": True, "sort_every": args.sort_every,
+                       "tiled_kernel": bool(tiled), "l2": "inputs larger than L2 (no flush needed)" if npart * pbytes > 4e8 else
+                       "inputs smaller than L2: see note", "parallelism": "replicas only" if world > 1 else "1 GPU"},
+            "clocks": clk, "gpu_launches": launches, "roofline": roofline,
+            "particles_per_second": npart * world * args.steps / (ms * 1e-3),
+            "sort_ms_per_species": sort_ms, "strays_last_step": strays, "bad_moves": bad}
+
+    # ---- end to end through the host-buffer C-ABI call: H2D of the step's inputs and D2H of its results inside ----
+    if not args.no_e2e and rank == 0 or (not args.no_e2e and world > 1):
+        hp = [p.to("cpu", pin=True) for p in parts]
+        hF = [f.cpu().pin_memory() for f in F]
+        hJ = [torch.zeros(eg.padded_shape, dtype=torch.float32).pin_memory() for _ in range(3)]
+        nst = max(1, min(args.steps, args.e2e_steps))
+        up = down = 0
+        for p in hp:
+            bind.ent_step_host(ctx, hF, p, hJ, wl.dt, 1)          # warm-up: staging allocation
+        barrier()
+        w0 = time.perf_counter()
+        for _ in range(nst):
+            up = down = 0
+            for p in hp:
+                u_, d_ = bind.ent_step_host(ctx, hF, p, hJ, wl.dt, 1)
+                up += u_; down += d_
+        barrier()
+        e_ms = (time.perf_counter() - w0) * 1e3
+        if world > 1:
+            t = torch.tensor([e_ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e_ms = float(t.item())
+        line["e2e"] = {"value": e_ms * 1e6 / (npart * world * nst), "unit": UNIT, "h2d_bytes_per_step": up, "d2h_bytes_per_step": down,
+                       "steps": nst, "ms_per_step": e_ms / nst, "call": "ent_step_host per species (pinned host buffers)"}
+        del hp, hF, hJ
+    bind.ent_destroy(ctx)
+
+    if rank == 0:
+        if not args.no_cpu and world == 1:
+            v, cores, sample, _ = time_oracle(args.workload, 2, 1)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C4s", "C5"])
+    ap.add_argument("--shrink", type=int, default=1)
+    ap.add_argument("--sort-every", type=int, default=0)
+    ap.add_argument("--step-impl", type=int, default=0, help="ENT_OPT_STEP_IMPL: 0 auto, 1 untiled, 2 two-kernel")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None, help="dram bytes per launch from an ncu --set full capture (profiles/)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,174 @@
+/*
+ * ent.h -- C ABI of the B200-native particle hot path of arXiv 2511.17710 ("Entity", curvilinear
+ *          special-relativistic PIC module).  P:nnn = line nnn of the paper text.
+ *
+ * The library runs sub-steps 3-8 of the paper's time step for one particle species:
+ *   gather E,B at the particle -> code basis to global Cartesian basis
+ *   -> relativistic Boris push (Eq. 3) -> move + back-map to code coordinates with
+ *   cell-crossing bookkeeping -> charge-conserving conformal-current deposit
+ *   (Eq. 6, "modified zig-zag" P:575), plus the cell/tile counting sort that keeps those stages
+ *   memory-coherent (not in the paper; BASELINE.json north_star (e)).
+ *
+ * Conventions common to every call
+ *   - every function returns 0 (ENT_OK) or a negative ent_status; it never throws, never exits and never
+ *     synchronises the stream (except the *_host calls, which say so).  Work is enqueued on the CUDA stream
+ *     given to ent_create.  ent_last_error(ctx) returns a NUL-terminated message owned by ctx.
+ *   - "device pointer" = memory allocated by the caller on the ctx's device (e.g. a torch tensor); the
+ *     library never allocates or frees caller-visible memory.  All particle/field device pointers must be
+ *     16-byte aligned (ENT_EINVAL otherwise).
+ *   - grids: D = 2 or 3 dimensions, N[d] active cells, N_GHOST = 2 ghost layers on each side.
+ *     A grid array ("padded planar array") has extents N[d] + 4, x1 fastest; active cell (i,j,k) is element
+ *     (i+2) + P0*((j+2) + P1*(k+2)), P_d = N[d] + 4.  In 2D the third extent is 1 (no ghosts).
+ *   - field components are contravariant code-basis components on the Yee lattice (P:181,
+ *     P:1044-1053): element (i,j,k) of E1 is E^1(i+1/2,j,k), E2 (i,j+1/2,k), E3 (i,j,k+1/2),
+ *     B1 (i,j+1/2,k+1/2), B2 (i+1/2,j,k+1/2), B3 (i+1/2,j+1/2,k).  Ghosts are filled by the caller.
+ *   - currents are conformal currents \mathcal{J}^d = sqrt(h) J^d staggered like E, units
+ *     charge * cells / time, written un-wrapped into the ghost layers (see ent_fold_current).
+ *   - particles: structure of arrays, one struct per species.  Position = cell index +
+ *     in-cell offset in [0,1); momentum u = gamma*v in the GLOBAL Cartesian basis, c = 1.
+ */
+#ifndef ENT_H
+#define ENT_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ENT_NGHOST 2
+
+typedef enum { ENT_OK = 0, ENT_EINVAL = -1, ENT_EUNSUPPORTED = -2, ENT_ECUDA = -3, ENT_ENOMEM = -4 } ent_status;
+enum { ENT_CART = 0, ENT_SPH = 1, ENT_QSPH = 2 };             /* metric kind */
+enum { ENT_PERIODIC = 0, ENT_ABSORB = 1, ENT_AXIS = 2 };      /* boundary rule of a dimension (both sides) */
+
+typedef struct ent_ctx ent_ctx;                                /* opaque; owns only scratch memory */
+
+/* Grid + metric parameters, exactly those of P:211 (Eq. 7) and P:227-267.  Host struct, passed by pointer,
+ * copied by the call.  CART: cell size (xmax-xmin)/N per dimension.  SPH: r = xmin[0] + x1*dr, theta = x2*pi/N[1].
+ * QSPH: r = r0 + exp(log(xmin[0]-r0) + x1*dR), theta = T + 2 vartheta T (1-2T/pi)(1-T/pi), T = x2*pi/N[1].
+ * SPH/QSPH require D == 2 (axisymmetric; the particle carries phi), bc = {ABSORB, AXIS}. */
+typedef struct {
+    int32_t D;
+    int32_t N[3];
+    int32_t bc[3];
+    int32_t kind;
+    double  xmin[3], xmax[3];
+    double  r0, vartheta;
+} ent_grid;
+
+/* Six padded planar fp32 arrays, order ex1,ex2,ex3,bx1,bx2,bx3.  Device pointers (host pointers
+ * for the *_host calls).  Read-only for the library. */
+typedef struct { const float *comp[6]; } ent_fields;
+
+/* Three padded planar fp32 arrays, conformal J^1,J^2,J^3.  Device pointers.  The library ACCUMULATES into them. */
+typedef struct { float *comp[3]; } ent_current;
+
+/* One species.  n may be any value >= 0 (ragged tails are handled).
+ *   cell  : int32[n]  linear ACTIVE cell index  i1 + N1*(i2 + N2*i3)   (2D: i1 + N1*i2)
+ *   d[a]  : fp32[n]   in-cell offset along dimension a, 0 <= d < 1; d[2] = NULL when D == 2
+ *   phi   : fp32[n]   azimuth in [0, 2 pi) for SPH/QSPH, NULL for CART
+ *   u[a]  : fp32[n]   gamma*v, global Cartesian basis
+ *   w     : fp32[n]   macro-particle weight (read-only for the library)
+ *   tag   : uint8[n]  1 = alive, 0 = dead; NULL = all alive and no absorbing side in the grid
+ *   q, m  : charge and mass of the species (q/m enters the push, q*w the deposit)
+ * A particle that leaves through an ABSORB side gets tag = 0, keeps the momentum it had when
+ * it left, its cell is clamped into the grid, and it deposits nothing for that step. */
+typedef struct {
+    int64_t  n;
+    int32_t *cell;
+    float   *d[3];
+    float   *phi;
+    float   *u[3];
+    float   *w;
+    uint8_t *tag;
+    float    q, m;
+} ent_particles;
+
+/* ---- context -------------------------------------------------------------------------------------------
+ * ent_create: device = CUDA ordinal; cuda_stream = a cudaStream_t (NULL = default stream) on which every call
+ * of this ctx enqueues its work.  Fails with ENT_ECUDA when no usable CUDA device exists: there is NO CPU
+ * fallback.  ent_destroy frees the ctx's scratch (synchronises the stream first). */
+int ent_create(ent_ctx **out, int device, void *cuda_stream);
+int ent_destroy(ent_ctx *ctx);
+const char *ent_last_error(const ent_ctx *ctx);               /* never NULL; "" when no error was recorded */
+
+/* Validates and installs the grid (D, N, bc, metric).  ENT_EINVAL: D not in {2,3}, N[d] < 3 on a periodic
+ * dimension (|delta i| <= 1 would be ambiguous), N1*N2*N3 >= 2^31, xmax <= xmin, QSPH with xmin[0] <= r0 or
+ * vartheta outside [0,1).  ENT_EUNSUPPORTED: SPH/QSPH with D != 2 or bc != {ABSORB, AXIS}; AXIS on a CART grid. */
+int ent_set_grid(ent_ctx *ctx, const ent_grid *grid);
+
+/* ---- the three calls of the problem statement ----------------------------------------------------------
+ * ent_gather_push: sub-steps 3-7 + crossing bookkeeping for every alive
+ * particle of `in`, result in `out` (same n; out may alias in array-by-array; out->w is not written).
+ * u^(n-1/2) -> u^(n+1/2) with fields at n; x^(n) -> x^(n+1) with u^(n+1/2)/gamma^(n+1/2) * dt.
+ * PERIODIC dimension: cell index wraps.  ABSORB: tag = 0 on leaving (needs out->tag != NULL, else ENT_EINVAL
+ * at call time if the grid has an ABSORB side).  AXIS: theta stays in [0, pi] by construction. */
+int ent_gather_push(ent_ctx *ctx, const ent_fields *EB, const ent_particles *in, ent_particles *out, float dt);
+
+/* ent_deposit: sub-step 8.  For every particle alive in both blocks, adds the conformal current of
+ * the move old -> new (two straight segments through the relay point of P:575; 3D per-segment weights
+ * (1-W_a)(1-W_b) + D_a D_b/12, which make Eq. 6 hold to round-off) times q*w/dt to J, un-wrapped: a particle
+ * that crossed a periodic face deposits into the ghost layer beyond it.  In 2D the out-of-plane J^3 is
+ * q w v^3 (code basis) at n+1/2 taken from new->u, half per segment.  Requires |delta i| <= 1 per dimension
+ * (violations are counted, see ENT_STAT_BAD_MOVES, and deposit nothing).  Uses old->w, old->q. */
+int ent_deposit(ent_ctx *ctx, const ent_particles *old_, const ent_particles *new_, ent_current *J, float dt);
+
+/* ent_sort: out-of-place counting sort of a species by sort key (S10).  key(cell) orders cells tile-major:
+ * with tile extents T_d (ENT_STAT_TILE_1..3) and nt_d = ceil(N_d / T_d) tiles per dimension,
+ *     tile  = t1 + nt1*(t2 + nt2*t3),  t_d = i_d / T_d
+ *     local = l1 + T1*(l2 + T2*l3),    l_d = i_d % T_d
+ *     key   = tile * (T1*T2*T3) + local          (0 <= key < ENT_STAT_NKEYS)
+ * Dead particles keep their key.  On return `out` holds a permutation of `in` with non-decreasing keys
+ * (order inside one cell unspecified) and, if key_offsets != NULL (device, int32[NKEYS+1]),
+ * key_offsets[k] = number of particles with key < k.  in and out must not overlap; out's arrays must exist
+ * wherever in's do.  The ctx remembers `out` as "sorted" so that ent_step may take its tiled path on it. */
+int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *out, int32_t *key_offsets);
+
+/* ---- fused hot path: the timed entry point ------------------------------------------------------------------
+ * ent_step = ent_gather_push (in place) + ent_deposit(old, new) in one pass over the particles: the old
+ * position stays in registers instead of the i_prev/dx_prev arrays of P:559.  Accumulates into J un-wrapped.
+ * If `p` is the block the last ent_sort produced (same pointers and n), the tiled kernel runs: one CTA per
+ * tile, E/B halo staged in shared memory by TMA, J accumulated in shared memory and flushed once; particles
+ * that drifted out of their tile's halo since the sort take the global-atomic path inside the same kernel.
+ * Otherwise the untiled kernel (global gathers, global atomics) runs.  Results agree up to fp32 summation order. */
+int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_current *J, float dt);
+
+/* J := 0 (all three padded arrays) */
+int ent_zero_current(ent_ctx *ctx, ent_current *J);
+/* "currents synchronization" for one periodic box: ghost layers of every PERIODIC dimension are added
+ * onto the opposite active layers, then refilled with the periodic image. */
+int ent_fold_current(ent_ctx *ctx, ent_current *J);
+
+/* ---- host-buffer variant (end-to-end measurement) --------------------------------------------------------------
+ * Same as `nsteps` x ent_step, but every pointer in EB, p and J is a HOST pointer (pinned memory recommended).
+ * Copies E,B and the particle block to ctx-owned device staging, zeroes the device J, runs the steps, copies the
+ * particle block and J back.  Synchronises the stream before returning.  *h2d_bytes / *d2h_bytes (may be NULL)
+ * receive the bytes copied in each direction. */
+int ent_step_host(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_current *J, float dt, int nsteps,
+                  int64_t *h2d_bytes, int64_t *d2h_bytes);
+
+/* ---- options and counters ----------------------------------------------------------------------------------- */
+enum {
+    ENT_OPT_STEP_IMPL = 1,     /* 0 = auto (tiled when the block is the sorted one), 1 = force untiled, 2 = two-kernel
+                                  (gather_push to scratch copy + deposit; the paper's structure) */
+    ENT_OPT_TILE_1 = 2, ENT_OPT_TILE_2 = 3, ENT_OPT_TILE_3 = 4    /* tile extents in cells; takes effect at the next ent_set_grid */
+};
+enum {
+    ENT_STAT_TILE_1 = 1, ENT_STAT_TILE_2 = 2, ENT_STAT_TILE_3 = 3, ENT_STAT_NKEYS = 4, ENT_STAT_NTILES = 5,
+    ENT_STAT_LAUNCHES = 6,     /* kernels launched by this ctx since creation */
+    ENT_STAT_BAD_MOVES = 7,    /* particles with |delta i| > 1 seen by deposit/step (synchronises the stream) */
+    ENT_STAT_STRAYS = 8,       /* particles that took the out-of-halo path in the last tiled ent_step (synchronises) */
+    ENT_STAT_SCRATCH_BYTES = 9,
+    ENT_STAT_LAST_STEP_TILED = 10
+};
+int ent_set_option(ent_ctx *ctx, int key, int64_t value);
+int ent_get_stat(ent_ctx *ctx, int key, int64_t *value);
+
+/* library version, "major.minor" */
+const char *ent_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ENT_H */

@@ -1,0 +1,456 @@
+// ent_api.cu -- the C ABI of include/ent.h: context, validation, kernel dispatch.  No torch types anywhere.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+
+#include "ent_kernels.cuh"
+#include "ent_tiled.cuh"
+
+using namespace ent;
+
+struct ent_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    char err[512] = {0};
+    bool have_grid = false;
+    ent_grid grid{};
+    GridDev g{};
+    int tile_opt[3] = {0, 0, 0};          // 0 = default
+    int step_impl = 0;
+    long long launches = 0;
+    // scratch
+    unsigned long long *counters = nullptr;   // [0] bad moves, [1] strays
+    int32_t *keys = nullptr;   long long keys_cap = 0;
+    int32_t *count = nullptr;  int32_t *offsets = nullptr; int32_t *cursor = nullptr; long long nkeys_cap = 0;
+    int32_t *chunk = nullptr;  long long chunk_cap = 0;
+    // "old" copy for the two-kernel step
+    void *oldbuf = nullptr; size_t oldbuf_cap = 0;
+    // host-call staging
+    void *hbuf = nullptr; size_t hbuf_cap = 0;
+    size_t scratch_bytes = 0;
+    // the block ent_sort produced last
+    const int32_t *sorted_cell = nullptr; long long sorted_n = -1;
+    int last_step_tiled = 0;
+    TiledState tiled{};
+};
+
+static int fail(ent_ctx *c, int code, const char *fmt, ...) {
+    if (c) {
+        va_list ap; va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+#define CK(call)                                                                                         \
+    do { cudaError_t e_ = (call);                                                                        \
+         if (e_ != cudaSuccess) return fail(ctx, ENT_ECUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); } while (0)
+
+static int launch_check(ent_ctx *ctx, const char *what) {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(ctx, ENT_ECUDA, "launch of %s failed: %s", what, cudaGetErrorString(e));
+    ctx->launches += 1;
+    return ENT_OK;
+}
+
+static int ensure(ent_ctx *ctx, void **ptr, size_t *cap_bytes, size_t need) {
+    if (*cap_bytes >= need && *ptr) return ENT_OK;
+    if (*ptr) { CK(cudaStreamSynchronize(ctx->stream)); CK(cudaFree(*ptr)); ctx->scratch_bytes -= *cap_bytes; *ptr = nullptr; *cap_bytes = 0; }
+    cudaError_t e = cudaMalloc(ptr, need ? need : 16);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(ctx, ENT_ENOMEM, "cudaMalloc of %zu scratch bytes failed: %s", need, cudaGetErrorString(e)); }
+    *cap_bytes = need; ctx->scratch_bytes += need;
+    return ENT_OK;
+}
+
+extern "C" const char *ent_version(void) { return "0.1"; }
+
+extern "C" const char *ent_last_error(const ent_ctx *ctx) { return ctx ? ctx->err : "null ctx"; }
+
+extern "C" int ent_create(ent_ctx **out, int device, void *cuda_stream) {
+    if (!out) return ENT_EINVAL;
+    *out = nullptr;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev <= 0 || device < 0 || device >= ndev) { cudaGetLastError(); return ENT_ECUDA; }   // no CPU fallback
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return ENT_ECUDA; }
+    ent_ctx *ctx = new (std::nothrow) ent_ctx();
+    if (!ctx) return ENT_ENOMEM;
+    ctx->device = device;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    if (cudaMalloc((void **)&ctx->counters, 4 * sizeof(unsigned long long)) != cudaSuccess ||
+        cudaMemsetAsync(ctx->counters, 0, 4 * sizeof(unsigned long long), ctx->stream) != cudaSuccess) {
+        cudaGetLastError(); delete ctx; return ENT_ECUDA;
+    }
+    *out = ctx;
+    return ENT_OK;
+}
+
+extern "C" int ent_destroy(ent_ctx *ctx) {
+    if (!ctx) return ENT_EINVAL;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    tiled_release(ctx->tiled);
+    cudaFree(ctx->counters); cudaFree(ctx->keys); cudaFree(ctx->count); cudaFree(ctx->offsets); cudaFree(ctx->cursor);
+    cudaFree(ctx->chunk); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf);
+    cudaGetLastError();
+    delete ctx;
+    return ENT_OK;
+}
+
+// ---- grid --------------------------------------------------------------------------------------------------
+extern "C" int ent_set_grid(ent_ctx *ctx, const ent_grid *gr) {
+    if (!ctx) return ENT_EINVAL;
+    if (!gr) return fail(ctx, ENT_EINVAL, "grid is NULL");
+    if (gr->D != 2 && gr->D != 3) return fail(ctx, ENT_EINVAL, "D = %d, must be 2 or 3", gr->D);
+    if (gr->kind != ENT_CART && gr->kind != ENT_SPH && gr->kind != ENT_QSPH) return fail(ctx, ENT_EINVAL, "unknown metric kind %d", gr->kind);
+    const int D = gr->D;
+    long long ncell = 1;
+    for (int a = 0; a < D; ++a) {
+        if (gr->N[a] < 1) return fail(ctx, ENT_EINVAL, "N[%d] = %d", a, gr->N[a]);
+        if (gr->bc[a] != ENT_PERIODIC && gr->bc[a] != ENT_ABSORB && gr->bc[a] != ENT_AXIS) return fail(ctx, ENT_EINVAL, "bc[%d] = %d", a, gr->bc[a]);
+        if (gr->bc[a] == ENT_PERIODIC && gr->N[a] < 3) return fail(ctx, ENT_EINVAL, "periodic dimension %d needs N >= 3 (|delta i| <= 1 would be ambiguous)", a);
+        if (!(gr->xmax[a] > gr->xmin[a])) return fail(ctx, ENT_EINVAL, "xmax[%d] <= xmin[%d]", a, a);
+        ncell *= gr->N[a];
+        if (ncell >= (1LL << 31)) return fail(ctx, ENT_EINVAL, "more than 2^31 - 1 cells: the packed int32 cell index would overflow");
+    }
+    if (gr->kind != ENT_CART) {
+        if (D != 2) return fail(ctx, ENT_EUNSUPPORTED, "SPH/QSPH metrics are axisymmetric: D must be 2");
+        if (gr->bc[0] != ENT_ABSORB || gr->bc[1] != ENT_AXIS) return fail(ctx, ENT_EUNSUPPORTED, "SPH/QSPH need bc = {ABSORB, AXIS}");
+        if (gr->kind == ENT_QSPH) {
+            if (!(gr->xmin[0] > gr->r0)) return fail(ctx, ENT_EINVAL, "QSPH needs xmin[0] > r0");
+            if (!(gr->vartheta >= 0.0 && gr->vartheta < 1.0)) return fail(ctx, ENT_EINVAL, "QSPH needs 0 <= vartheta < 1");
+        } else if (!(gr->xmin[0] >= 0.0)) return fail(ctx, ENT_EINVAL, "SPH needs rmin >= 0");
+    } else {
+        for (int a = 0; a < D; ++a) if (gr->bc[a] == ENT_AXIS) return fail(ctx, ENT_EUNSUPPORTED, "AXIS boundary on a Cartesian grid");
+    }
+    GridDev g{};
+    g.D = D; g.kind = gr->kind;
+    const int deft[2][3] = { {16, 16, 1}, {8, 8, 8} };
+    long long pad = 1;
+    for (int a = 0; a < 3; ++a) {
+        bool on = a < D;
+        g.N[a] = on ? gr->N[a] : 1;
+        g.P[a] = on ? gr->N[a] + 2 * NG : 1;
+        g.bc[a] = on ? gr->bc[a] : ENT_PERIODIC;
+        int T = on ? (ctx->tile_opt[a] > 0 ? ctx->tile_opt[a] : deft[D - 2][a]) : 1;
+        if (T > g.N[a]) T = g.N[a];
+        g.T[a] = T;
+        g.nt[a] = (g.N[a] + T - 1) / T;
+        double dx = on ? (gr->xmax[a] - gr->xmin[a]) / (double)gr->N[a] : 1.0;
+        g.dx[a] = (float)dx; g.inv_dx[a] = (float)(1.0 / dx);
+        pad *= g.P[a];
+    }
+    if (pad >= (1LL << 31)) return fail(ctx, ENT_EINVAL, "padded array has more than 2^31 - 1 elements");
+    g.tcells = g.T[0] * g.T[1] * g.T[2];
+    long long nkeys = (long long)g.nt[0] * g.nt[1] * g.nt[2] * g.tcells;
+    if (nkeys >= (1LL << 31)) return fail(ctx, ENT_EINVAL, "sort key space exceeds int32");
+    if (gr->kind == ENT_SPH) {
+        g.rmin = gr->xmin[0]; g.dr = (gr->xmax[0] - gr->xmin[0]) / gr->N[0]; g.dth = PI_D / gr->N[1];
+    } else if (gr->kind == ENT_QSPH) {
+        g.r0 = gr->r0; g.vt = gr->vartheta;
+        g.Rmin = log(gr->xmin[0] - gr->r0);
+        g.dR = (log(gr->xmax[0] - gr->r0) - g.Rmin) / gr->N[0];
+        g.dT = PI_D / gr->N[1];
+    }
+    ctx->grid = *gr; ctx->g = g; ctx->have_grid = true;
+    ctx->sorted_cell = nullptr; ctx->sorted_n = -1;
+    return tiled_set_grid(ctx->tiled, g, ctx->err, sizeof(ctx->err));
+}
+
+// ---- argument checks ---------------------------------------------------------------------------------------
+static bool al16(const void *p) { return (((uintptr_t)p) & 15u) == 0; }
+
+static int check_particles(ent_ctx *ctx, const ent_particles *p, const char *name, bool need_tag_if_absorb) {
+    if (!p) return fail(ctx, ENT_EINVAL, "%s is NULL", name);
+    if (p->n < 0) return fail(ctx, ENT_EINVAL, "%s->n < 0", name);
+    if (p->n >= (1LL << 31)) return fail(ctx, ENT_EINVAL, "%s->n >= 2^31 (sort offsets are int32)", name);
+    const GridDev &g = ctx->g;
+    if (!p->cell || !al16(p->cell)) return fail(ctx, ENT_EINVAL, "%s->cell NULL or not 16-byte aligned", name);
+    for (int a = 0; a < g.D; ++a) if (!p->d[a] || !al16(p->d[a])) return fail(ctx, ENT_EINVAL, "%s->d[%d] NULL or misaligned", name, a);
+    for (int a = 0; a < 3; ++a) if (!p->u[a] || !al16(p->u[a])) return fail(ctx, ENT_EINVAL, "%s->u[%d] NULL or misaligned", name, a);
+    if (!p->w || !al16(p->w)) return fail(ctx, ENT_EINVAL, "%s->w NULL or misaligned", name);
+    if (g.kind != ENT_CART && (!p->phi || !al16(p->phi))) return fail(ctx, ENT_EINVAL, "%s->phi NULL or misaligned on an axisymmetric grid", name);
+    if (p->tag && !al16(p->tag)) return fail(ctx, ENT_EINVAL, "%s->tag misaligned", name);
+    if (need_tag_if_absorb && !p->tag)
+        for (int a = 0; a < g.D; ++a) if (g.bc[a] == ENT_ABSORB) return fail(ctx, ENT_EINVAL, "%s->tag is NULL but dimension %d is ABSORB", name, a);
+    return ENT_OK;
+}
+static int check_fields(ent_ctx *ctx, const ent_fields *F) {
+    if (!F) return fail(ctx, ENT_EINVAL, "fields struct is NULL");
+    for (int c = 0; c < 6; ++c) if (!F->comp[c] || !al16(F->comp[c])) return fail(ctx, ENT_EINVAL, "field component %d NULL or misaligned", c);
+    return ENT_OK;
+}
+static int check_current(ent_ctx *ctx, const ent_current *J) {
+    if (!J) return fail(ctx, ENT_EINVAL, "current struct is NULL");
+    for (int c = 0; c < 3; ++c) if (!J->comp[c] || !al16(J->comp[c])) return fail(ctx, ENT_EINVAL, "current component %d NULL or misaligned", c);
+    return ENT_OK;
+}
+static PartPtrs pp(const ent_particles *p) {
+    PartPtrs r;
+    r.cell = p->cell; for (int a = 0; a < 3; ++a) { r.d[a] = p->d[a]; r.u[a] = p->u[a]; }
+    r.phi = p->phi; r.w = p->w; r.tag = p->tag;
+    return r;
+}
+static FieldPtrs fp(const ent_fields *F) { FieldPtrs r; for (int c = 0; c < 6; ++c) r.c[c] = F->comp[c]; return r; }
+static CurrentPtrs cp(const ent_current *J) { CurrentPtrs r; for (int c = 0; c < 3; ++c) r.c[c] = J->comp[c]; return r; }
+static unsigned nblk(long long n) { return (unsigned)((n + TPB - 1) / TPB); }
+
+#define ENTER()                                                                              \
+    if (!ctx) return ENT_EINVAL;                                                             \
+    if (!ctx->have_grid) return fail(ctx, ENT_EINVAL, "ent_set_grid has not been called");   \
+    CK(cudaSetDevice(ctx->device))
+
+// dispatch on (D, kind): the four supported combinations
+#define DISPATCH(KERNEL, GRID, ...)                                                                          \
+    do {                                                                                                     \
+        const GridDev &g_ = ctx->g;                                                                          \
+        if (g_.kind == ENT_CART && g_.D == 2) KERNEL<2, ENT_CART><<<GRID, TPB, 0, ctx->stream>>>(__VA_ARGS__); \
+        else if (g_.kind == ENT_CART) KERNEL<3, ENT_CART><<<GRID, TPB, 0, ctx->stream>>>(__VA_ARGS__);        \
+        else if (g_.kind == ENT_SPH) KERNEL<2, ENT_SPH><<<GRID, TPB, 0, ctx->stream>>>(__VA_ARGS__);          \
+        else KERNEL<2, ENT_QSPH><<<GRID, TPB, 0, ctx->stream>>>(__VA_ARGS__);                                 \
+    } while (0)
+
+// ---- the calls ---------------------------------------------------------------------------------------------
+extern "C" int ent_gather_push(ent_ctx *ctx, const ent_fields *EB, const ent_particles *in, ent_particles *out, float dt) {
+    ENTER();
+    int rc;
+    if ((rc = check_fields(ctx, EB)) || (rc = check_particles(ctx, in, "in", false)) || (rc = check_particles(ctx, out, "out", true))) return rc;
+    if (in->n != out->n) return fail(ctx, ENT_EINVAL, "in->n != out->n");
+    if (!(in->m != 0.f)) return fail(ctx, ENT_EINVAL, "mass is zero");
+    if (in->n == 0) return ENT_OK;
+    float eps = 0.5f * (in->q / in->m) * dt;
+    DISPATCH(gather_push_kernel, nblk(in->n), ctx->g, fp(EB), pp(in), pp(out), (long long)in->n, eps, dt);
+    return launch_check(ctx, "gather_push_kernel");
+}
+
+extern "C" int ent_deposit(ent_ctx *ctx, const ent_particles *po, const ent_particles *pn, ent_current *J, float dt) {
+    ENTER();
+    int rc;
+    if ((rc = check_current(ctx, J)) || (rc = check_particles(ctx, po, "old", false)) || (rc = check_particles(ctx, pn, "new", false))) return rc;
+    if (po->n != pn->n) return fail(ctx, ENT_EINVAL, "old->n != new->n");
+    if (!(dt > 0.f)) return fail(ctx, ENT_EINVAL, "dt must be positive");
+    if (po->n == 0) return ENT_OK;
+    DISPATCH(deposit_kernel, nblk(po->n), ctx->g, pp(po), pp(pn), cp(J), (long long)po->n, po->q, 1.0f / dt, ctx->counters + 0);
+    return launch_check(ctx, "deposit_kernel");
+}
+
+extern "C" int ent_zero_current(ent_ctx *ctx, ent_current *J) {
+    ENTER();
+    int rc;
+    if ((rc = check_current(ctx, J))) return rc;
+    size_t bytes = (size_t)padded_size(ctx->g) * sizeof(float);
+    for (int c = 0; c < 3; ++c) CK(cudaMemsetAsync(J->comp[c], 0, bytes, ctx->stream));
+    return ENT_OK;
+}
+
+extern "C" int ent_fold_current(ent_ctx *ctx, ent_current *J) {
+    ENTER();
+    int rc;
+    if ((rc = check_current(ctx, J))) return rc;
+    const GridDev &g = ctx->g;
+    for (int c = 0; c < 3; ++c)
+        for (int pass = 0; pass < 2; ++pass)
+            for (int d = 0; d < g.D; ++d) {
+                if (g.bc[d] != ENT_PERIODIC) continue;
+                long long nthreads = (long long)g.P[(d + 1) % 3] * g.P[(d + 2) % 3] * NG;
+                fold_kernel<<<nblk(nthreads), TPB, 0, ctx->stream>>>(g, J->comp[c], d, pass);
+                if ((rc = launch_check(ctx, "fold_kernel"))) return rc;
+            }
+    return ENT_OK;
+}
+
+static int step_two_kernel(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_current *J, float dt) {
+    // the paper's structure: keep a copy of the old position, push, then deposit old -> new
+    const GridDev &g = ctx->g;
+    const size_t n = (size_t)p->n, slot = (n * 4 + 255) & ~(size_t)255;
+    int rc;
+    if ((rc = ensure(ctx, &ctx->oldbuf, &ctx->oldbuf_cap, slot * 6))) return rc;
+    char *b = (char *)ctx->oldbuf;
+    ent_particles old = *p;
+    old.cell = (int32_t *)b;
+    CK(cudaMemcpyAsync(old.cell, p->cell, n * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+    for (int a = 0; a < g.D; ++a) {
+        old.d[a] = (float *)(b + slot * (1 + a));
+        CK(cudaMemcpyAsync(old.d[a], p->d[a], n * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    if (g.kind != ENT_CART) {
+        old.phi = (float *)(b + slot * 4);
+        CK(cudaMemcpyAsync(old.phi, p->phi, n * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    if (p->tag) {
+        old.tag = (uint8_t *)(b + slot * 5);
+        CK(cudaMemcpyAsync(old.tag, p->tag, n, cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    if ((rc = ent_gather_push(ctx, EB, p, p, dt))) return rc;
+    return ent_deposit(ctx, &old, p, J, dt);
+}
+
+extern "C" int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_current *J, float dt) {
+    ENTER();
+    int rc;
+    if ((rc = check_fields(ctx, EB)) || (rc = check_current(ctx, J)) || (rc = check_particles(ctx, p, "p", true))) return rc;
+    if (!(dt > 0.f)) return fail(ctx, ENT_EINVAL, "dt must be positive");
+    if (!(p->m != 0.f)) return fail(ctx, ENT_EINVAL, "mass is zero");
+    ctx->last_step_tiled = 0;
+    if (p->n == 0) return ENT_OK;
+    if (ctx->step_impl == 2) return step_two_kernel(ctx, EB, p, J, dt);
+    float eps = 0.5f * (p->q / p->m) * dt;
+    bool sorted = p->cell == ctx->sorted_cell && p->n == ctx->sorted_n;
+    if (ctx->step_impl == 0 && sorted && tiled_supported(ctx->tiled, ctx->g)) {
+        rc = tiled_step(ctx->tiled, ctx->g, ctx->stream, fp(EB), pp(p), cp(J), (long long)p->n, ctx->offsets, eps, dt, p->q,
+                        1.0f / dt, ctx->counters, &ctx->launches, ctx->err, sizeof(ctx->err));
+        if (rc == ENT_OK) ctx->last_step_tiled = 1;
+        return rc;
+    }
+    DISPATCH(step_untiled_kernel, nblk(p->n), ctx->g, fp(EB), pp(p), cp(J), (long long)p->n, eps, dt, p->q, 1.0f / dt, ctx->counters + 0);
+    return launch_check(ctx, "step_untiled_kernel");
+}
+
+extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *out, int32_t *key_offsets) {
+    ENTER();
+    int rc;
+    if ((rc = check_particles(ctx, in, "in", false)) || (rc = check_particles(ctx, out, "out", false))) return rc;
+    if (in->n != out->n) return fail(ctx, ENT_EINVAL, "in->n != out->n");
+    if (in->cell == out->cell || in->w == out->w) return fail(ctx, ENT_EINVAL, "ent_sort is out-of-place: in and out overlap");
+    if (in->tag && !out->tag) return fail(ctx, ENT_EINVAL, "in has tags but out->tag is NULL");
+    const GridDev &g = ctx->g;
+    const long long n = in->n;
+    const long long nkeys = (long long)g.nt[0] * g.nt[1] * g.nt[2] * g.tcells;
+    const long long m = nkeys;                                        // scan length; offsets has m + 1 entries
+    const int nchunks = (int)((m + SCAN_CHUNK - 1) / SCAN_CHUNK);
+    {   // scratch
+        size_t cap;
+        cap = (size_t)ctx->keys_cap * 4;
+        if ((rc = ensure(ctx, (void **)&ctx->keys, &cap, (size_t)(n ? n : 1) * 4))) return rc;
+        ctx->keys_cap = (long long)(cap / 4);
+        if (ctx->nkeys_cap < nkeys + 1) {
+            size_t c1 = (size_t)ctx->nkeys_cap * 4, c2 = c1, c3 = c1;
+            if ((rc = ensure(ctx, (void **)&ctx->count, &c1, (size_t)(nkeys + 1) * 4))) return rc;
+            if ((rc = ensure(ctx, (void **)&ctx->offsets, &c2, (size_t)(nkeys + 1) * 4))) return rc;
+            if ((rc = ensure(ctx, (void **)&ctx->cursor, &c3, (size_t)(nkeys + 1) * 4))) return rc;
+            ctx->nkeys_cap = nkeys + 1;
+        }
+        cap = (size_t)ctx->chunk_cap * 4;
+        if ((rc = ensure(ctx, (void **)&ctx->chunk, &cap, (size_t)nchunks * 4))) return rc;
+        ctx->chunk_cap = (long long)(cap / 4);
+    }
+    ctx->sorted_cell = nullptr; ctx->sorted_n = -1;
+    CK(cudaMemsetAsync(ctx->count, 0, (size_t)(nkeys + 1) * 4, ctx->stream));
+    if (n > 0) {
+        if (g.D == 2) sort_hist_kernel<2><<<nblk(n), TPB, 0, ctx->stream>>>(g, in->cell, n, ctx->keys, ctx->count);
+        else sort_hist_kernel<3><<<nblk(n), TPB, 0, ctx->stream>>>(g, in->cell, n, ctx->keys, ctx->count);
+        if ((rc = launch_check(ctx, "sort_hist_kernel"))) return rc;
+    }
+    scan_reduce_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, m, ctx->chunk);
+    if ((rc = launch_check(ctx, "scan_reduce_kernel"))) return rc;
+    scan_chunks_kernel<<<1, TPB, 0, ctx->stream>>>(ctx->chunk, nchunks);
+    if ((rc = launch_check(ctx, "scan_chunks_kernel"))) return rc;
+    scan_apply_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, m, ctx->chunk, ctx->offsets, ctx->cursor);
+    if ((rc = launch_check(ctx, "scan_apply_kernel"))) return rc;
+    if (n > 0) {
+        sort_scatter_kernel<<<nblk(n), TPB, 0, ctx->stream>>>(ctx->keys, ctx->cursor, pp(in), pp(out), n, g.D, g.kind != ENT_CART);
+        if ((rc = launch_check(ctx, "sort_scatter_kernel"))) return rc;
+    }
+    if (key_offsets) CK(cudaMemcpyAsync(key_offsets, ctx->offsets, (size_t)(nkeys + 1) * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+    out->q = in->q; out->m = in->m;
+    ctx->sorted_cell = out->cell; ctx->sorted_n = n;
+    return ENT_OK;
+}
+
+extern "C" int ent_set_option(ent_ctx *ctx, int key, int64_t value) {
+    if (!ctx) return ENT_EINVAL;
+    switch (key) {
+        case ENT_OPT_STEP_IMPL:
+            if (value < 0 || value > 2) return fail(ctx, ENT_EINVAL, "ENT_OPT_STEP_IMPL must be 0, 1 or 2");
+            ctx->step_impl = (int)value; return ENT_OK;
+        case ENT_OPT_TILE_1: case ENT_OPT_TILE_2: case ENT_OPT_TILE_3:
+            if (value < 0 || value > 64) return fail(ctx, ENT_EINVAL, "tile extent must be in 0..64 (0 = default)");
+            ctx->tile_opt[key - ENT_OPT_TILE_1] = (int)value; return ENT_OK;
+        default: return fail(ctx, ENT_EINVAL, "unknown option %d", key);
+    }
+}
+
+extern "C" int ent_get_stat(ent_ctx *ctx, int key, int64_t *value) {
+    if (!ctx) return ENT_EINVAL;
+    if (!value) return fail(ctx, ENT_EINVAL, "value is NULL");
+    const GridDev &g = ctx->g;
+    switch (key) {
+        case ENT_STAT_TILE_1: case ENT_STAT_TILE_2: case ENT_STAT_TILE_3:
+            if (!ctx->have_grid) return fail(ctx, ENT_EINVAL, "no grid"); *value = g.T[key - ENT_STAT_TILE_1]; return ENT_OK;
+        case ENT_STAT_NKEYS:
+            if (!ctx->have_grid) return fail(ctx, ENT_EINVAL, "no grid"); *value = (int64_t)g.nt[0] * g.nt[1] * g.nt[2] * g.tcells; return ENT_OK;
+        case ENT_STAT_NTILES:
+            if (!ctx->have_grid) return fail(ctx, ENT_EINVAL, "no grid"); *value = (int64_t)g.nt[0] * g.nt[1] * g.nt[2]; return ENT_OK;
+        case ENT_STAT_LAUNCHES: *value = ctx->launches; return ENT_OK;
+        case ENT_STAT_BAD_MOVES: case ENT_STAT_STRAYS: {
+            unsigned long long h[4];
+            CK(cudaSetDevice(ctx->device));
+            CK(cudaMemcpyAsync(h, ctx->counters, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+            CK(cudaStreamSynchronize(ctx->stream));
+            *value = (int64_t)h[key == ENT_STAT_BAD_MOVES ? 0 : 1]; return ENT_OK;
+        }
+        case ENT_STAT_SCRATCH_BYTES: *value = (int64_t)(ctx->scratch_bytes + tiled_scratch_bytes(ctx->tiled)); return ENT_OK;
+        case ENT_STAT_LAST_STEP_TILED: *value = ctx->last_step_tiled; return ENT_OK;
+        default: return fail(ctx, ENT_EINVAL, "unknown stat %d", key);
+    }
+}
+
+// ---- host-buffer variant: H2D, nsteps x ent_step, D2H, all inside the call (end-to-end measurement) ----
+extern "C" int ent_step_host(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_current *J, float dt, int nsteps,
+                             int64_t *h2d_bytes, int64_t *d2h_bytes) {
+    ENTER();
+    if (!EB || !p || !J) return fail(ctx, ENT_EINVAL, "NULL argument");
+    if (nsteps < 0) return fail(ctx, ENT_EINVAL, "nsteps < 0");
+    const GridDev &g = ctx->g;
+    const size_t n = (size_t)p->n, pad = (size_t)padded_size(g);
+    const size_t fslot = (pad * 4 + 255) & ~(size_t)255, pslot = (n * 4 + 255) & ~(size_t)255;
+    const bool axisym = g.kind != ENT_CART;
+    int rc;
+    if ((rc = ensure(ctx, &ctx->hbuf, &ctx->hbuf_cap, fslot * 9 + pslot * 10))) return rc;
+    char *b = (char *)ctx->hbuf;
+    int64_t up = 0, down = 0;
+    ent_fields dEB; ent_current dJ; ent_particles dp = *p;
+    for (int c = 0; c < 6; ++c) {
+        if (!EB->comp[c]) return fail(ctx, ENT_EINVAL, "host field component %d is NULL", c);
+        float *dst = (float *)(b + fslot * c);
+        CK(cudaMemcpyAsync(dst, EB->comp[c], pad * 4, cudaMemcpyHostToDevice, ctx->stream)); up += (int64_t)pad * 4;
+        dEB.comp[c] = dst;
+    }
+    for (int c = 0; c < 3; ++c) {
+        if (!J->comp[c]) return fail(ctx, ENT_EINVAL, "host current component %d is NULL", c);
+        dJ.comp[c] = (float *)(b + fslot * (6 + c));
+    }
+    char *pb = b + fslot * 9;
+    struct Arr { void **dev; void *host; size_t bytes; bool back; };
+    Arr arrs[10]; int na = 0;
+    dp.cell = (int32_t *)(pb + pslot * 0); arrs[na++] = { (void **)&dp.cell, p->cell, n * 4, true };
+    for (int a = 0; a < 3; ++a) {
+        if (a < g.D) { dp.d[a] = (float *)(pb + pslot * (1 + a)); arrs[na++] = { (void **)&dp.d[a], p->d[a], n * 4, true }; }
+        else dp.d[a] = nullptr;
+        dp.u[a] = (float *)(pb + pslot * (4 + a)); arrs[na++] = { (void **)&dp.u[a], p->u[a], n * 4, true };
+    }
+    dp.w = (float *)(pb + pslot * 7); arrs[na++] = { (void **)&dp.w, p->w, n * 4, false };
+    if (axisym) { dp.phi = (float *)(pb + pslot * 8); arrs[na++] = { (void **)&dp.phi, p->phi, n * 4, true }; } else dp.phi = nullptr;
+    if (p->tag) { dp.tag = (uint8_t *)(pb + pslot * 9); arrs[na++] = { (void **)&dp.tag, p->tag, n, true }; } else dp.tag = nullptr;
+    for (int k = 0; k < na; ++k) {
+        if (!arrs[k].host) return fail(ctx, ENT_EINVAL, "a required host particle array is NULL");
+        if (arrs[k].bytes) CK(cudaMemcpyAsync(*arrs[k].dev, arrs[k].host, arrs[k].bytes, cudaMemcpyHostToDevice, ctx->stream));
+        up += (int64_t)arrs[k].bytes;
+    }
+    if ((rc = ent_zero_current(ctx, &dJ))) return rc;
+    for (int s = 0; s < nsteps; ++s)
+        if ((rc = ent_step(ctx, &dEB, &dp, &dJ, dt))) return rc;
+    for (int k = 0; k < na; ++k) {
+        if (!arrs[k].back) continue;
+        if (arrs[k].bytes) CK(cudaMemcpyAsync(arrs[k].host, *arrs[k].dev, arrs[k].bytes, cudaMemcpyDeviceToHost, ctx->stream));
+        down += (int64_t)arrs[k].bytes;
+    }
+    for (int c = 0; c < 3; ++c) { CK(cudaMemcpyAsync(J->comp[c], dJ.comp[c], pad * 4, cudaMemcpyDeviceToHost, ctx->stream)); down += (int64_t)pad * 4; }
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (h2d_bytes) *h2d_bytes = up;
+    if (d2h_bytes) *d2h_bytes = down;
+    return ENT_OK;
+}

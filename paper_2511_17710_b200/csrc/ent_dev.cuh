@@ -1,0 +1,186 @@
+// ent_dev.cuh -- device-side building blocks of the particle hot path (arXiv 2511.17710; P:nnn = PAPER.md line).
+// Everything here is fp32 except the curvilinear coordinate maps, which are evaluated in fp64 (DESIGN.md
+// "precision of the curvilinear round trip": the fp32 code->xyz->code round trip loses the displacement).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/ent.h"
+
+namespace ent {
+
+constexpr int NG = ENT_NGHOST;
+constexpr double PI_D = 3.14159265358979323846264338327950288;
+constexpr float TWO_PI_F = 6.28318548202514648f;   // float nearest to 2*pi (slightly above it)
+
+// Grid + metric constants, passed to kernels by value (the paper passes its metric object by value too).
+struct GridDev {
+    int D, kind;
+    int N[3];          // active cells (N[2] = 1 in 2D)
+    int P[3];          // padded extents N + 2*NG (P[2] = 1 in 2D)
+    int bc[3];
+    int T[3];          // tile extents in cells (T[2] = 1 in 2D)
+    int nt[3];         // tiles per dimension
+    int tcells;        // T0*T1*T2
+    float dx[3];       // CART: sqrt(h_dd) = cell size (1 for dimensions >= D)
+    float inv_dx[3];
+    // SPH:  r = rmin + x1*dr, theta = x2*dth
+    // QSPH: r = r0 + exp(Rmin + x1*dR), theta = theta(T), T = x2*dT
+    double rmin, dr, dth;
+    double Rmin, dR, dT, r0, vt;
+};
+
+__host__ __device__ inline long long padded_size(const GridDev &g) { return (long long)g.P[0] * g.P[1] * g.P[2]; }
+
+template <int D>
+__device__ __forceinline__ void unpack_cell(const GridDev &g, int cell, int i[3]) {
+    if (D == 2) {
+        i[1] = cell / g.N[0]; i[0] = cell - i[1] * g.N[0]; i[2] = 0;
+    } else {
+        int n01 = g.N[0] * g.N[1];
+        i[2] = cell / n01; int r = cell - i[2] * n01;
+        i[1] = r / g.N[0]; i[0] = r - i[1] * g.N[0];
+    }
+}
+template <int D>
+__device__ __forceinline__ int pack_cell(const GridDev &g, const int i[3]) {
+    return D == 2 ? i[0] + g.N[0] * i[1] : i[0] + g.N[0] * (i[1] + g.N[1] * i[2]);
+}
+// padded linear index of active cell (i,j,k)
+template <int D>
+__device__ __forceinline__ long long pidx(const GridDev &g, int i, int j, int k) {
+    return D == 2 ? (long long)(i + NG) + (long long)g.P[0] * (j + NG)
+                  : (long long)(i + NG) + (long long)g.P[0] * ((long long)(j + NG) + (long long)g.P[1] * (k + NG));
+}
+// sort key of a cell (ent.h, ent_sort): tile-major
+template <int D>
+__device__ __forceinline__ int sort_key(const GridDev &g, const int i[3]) {
+    int t0 = i[0] / g.T[0], t1 = i[1] / g.T[1];
+    int l0 = i[0] - t0 * g.T[0], l1 = i[1] - t1 * g.T[1];
+    if (D == 2) return (t0 + g.nt[0] * t1) * g.tcells + (l0 + g.T[0] * l1);
+    int t2 = i[2] / g.T[2], l2 = i[2] - t2 * g.T[2];
+    return (t0 + g.nt[0] * (t1 + g.nt[1] * t2)) * g.tcells + (l0 + g.T[0] * (l1 + g.T[1] * l2));
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S1 gather (first-order shape, direct multilinear interpolation on each component's own staggered
+// lattice; Yee staggering P:181).  F[c] = padded planar arrays.  Loader abstracts where the
+// values come from (global memory here, a shared-memory tile in the tiled kernel).
+// ---------------------------------------------------------------------------------------------------------
+struct GlobalFieldLoader {
+    const float *const *F;   // 6 pointers (kernel-parameter copy)
+    __device__ __forceinline__ float operator()(int c, long long idx) const { return __ldg(F[c] + idx); }
+};
+
+template <int D, class Loader>
+__device__ __forceinline__ void gather(const GridDev &g, const Loader &ld, const int i[3], const float d[3], float EB[6]) {
+    // per dimension: node-centred (b0,f0) and half-shifted (bs,fs) base index and fraction
+    int bs[3]; float fs[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (a < D) {
+            bool lo = d[a] < 0.5f;
+            bs[a] = lo ? i[a] - 1 : i[a];
+            fs[a] = lo ? d[a] + 0.5f : d[a] - 0.5f;
+        } else { bs[a] = 0; fs[a] = 0.f; }
+    }
+    const long long s1 = g.P[0], s2 = (long long)g.P[0] * g.P[1];
+    // stagger pattern per component (1 = half-cell shift): E1 100, E2 010, E3 001, B1 011, B2 101, B3 110
+    const int ST[6][3] = { {1,0,0}, {0,1,0}, {0,0,1}, {0,1,1}, {1,0,1}, {1,1,0} };
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        int b0 = ST[c][0] ? bs[0] : i[0];
+        int b1 = ST[c][1] ? bs[1] : i[1];
+        int b2 = (D == 3) ? (ST[c][2] ? bs[2] : i[2]) : 0;
+        float f0 = ST[c][0] ? fs[0] : d[0];
+        float f1 = ST[c][1] ? fs[1] : d[1];
+        long long base = pidx<D>(g, b0, b1, b2);
+        float v00 = ld(c, base), v10 = ld(c, base + 1), v01 = ld(c, base + s1), v11 = ld(c, base + s1 + 1);
+        float lo = (v00 + f0 * (v10 - v00)) + f1 * ((v01 + f0 * (v11 - v01)) - (v00 + f0 * (v10 - v00)));
+        if (D == 3) {
+            float f2 = ST[c][2] ? fs[2] : d[2];
+            float w00 = ld(c, base + s2), w10 = ld(c, base + s2 + 1), w01 = ld(c, base + s2 + s1), w11 = ld(c, base + s2 + s1 + 1);
+            float hi = (w00 + f0 * (w10 - w00)) + f1 * ((w01 + f0 * (w11 - w01)) - (w00 + f0 * (w10 - w00)));
+            lo = lo + f2 * (hi - lo);
+        }
+        EB[c] = lo;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// O1 metric pieces for the axisymmetric grids, fp64
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double theta_of_T(double vt, double T) {
+    return T + 2.0 * vt * T * (1.0 - 2.0 * T / PI_D) * (1.0 - T / PI_D);
+}
+__device__ __forceinline__ double dtheta_dT(double vt, double T) {
+    double s = T / PI_D;
+    return 1.0 + 2.0 * vt + 12.0 * vt * s * (s - 1.0);
+}
+// inverse of theta(T) (App. B): theta(T) is a monotone cubic for 0 <= vartheta < 1, so Newton from
+// T = theta converges quadratically; no cube root on the device (differs from Eq. B3).
+__device__ __forceinline__ double T_of_theta(double vt, double th) {
+    if (vt == 0.0) return th;
+    double T = th;
+#pragma unroll 1
+    for (int it = 0; it < 8; ++it) {
+        double f = theta_of_T(vt, T) - th;
+        T -= f / dtheta_dT(vt, T);
+        if (fabs(f) < 1e-15) break;
+    }
+    return T;
+}
+
+struct Sph {            // spherical-polar description of a code position + sqrt(h_ii) there
+    double r, th;
+    double sh1, sh2, sh3;   // sqrt(h11), sqrt(h22), sqrt(h33)
+};
+template <int KIND>
+__device__ __forceinline__ Sph sph_of_code(const GridDev &g, double x1, double x2) {
+    Sph s;
+    if (KIND == ENT_SPH) {
+        s.r = g.rmin + x1 * g.dr;
+        s.th = x2 * g.dth;
+        s.sh1 = g.dr; s.sh2 = s.r * g.dth;
+    } else {
+        double eR = exp(g.Rmin + x1 * g.dR);
+        double T = x2 * g.dT;
+        s.r = g.r0 + eR;
+        s.th = theta_of_T(g.vt, T);
+        s.sh1 = g.dR * eR; s.sh2 = g.dT * dtheta_dT(g.vt, T) * s.r;
+    }
+    s.sh3 = s.r * sin(s.th);
+    return s;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S3 relativistic Boris (Eq. 3): half electric kick, rotation about B, half kick.  eps = (q/m) dt / 2
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void boris(float u[3], const float E[3], const float B[3], float eps) {
+    float um0 = u[0] + eps * E[0], um1 = u[1] + eps * E[1], um2 = u[2] + eps * E[2];
+    float ig = rsqrtf(1.0f + um0 * um0 + um1 * um1 + um2 * um2);
+    ig = ig * (1.5f - 0.5f * (1.0f + um0 * um0 + um1 * um1 + um2 * um2) * ig * ig);   // one Newton step: full fp32 accuracy
+    float t0 = eps * B[0] * ig, t1 = eps * B[1] * ig, t2 = eps * B[2] * ig;
+    float sc = 2.0f / (1.0f + t0 * t0 + t1 * t1 + t2 * t2);
+    float p0 = um0 + (um1 * t2 - um2 * t1);
+    float p1 = um1 + (um2 * t0 - um0 * t2);
+    float p2 = um2 + (um0 * t1 - um1 * t0);
+    float s0 = sc * t0, s1 = sc * t1, s2 = sc * t2;
+    u[0] = um0 + (p1 * s2 - p2 * s1) + eps * E[0];
+    u[1] = um1 + (p2 * s0 - p0 * s2) + eps * E[1];
+    u[2] = um2 + (p0 * s1 - p1 * s0) + eps * E[2];
+}
+__device__ __forceinline__ float inv_gamma(const float u[3]) {
+    float g2 = 1.0f + u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    float ig = rsqrtf(g2);
+    return ig * (1.5f - 0.5f * g2 * ig * ig);
+}
+
+// split x = (old offset + displacement) into a cell shift and an offset in [0,1) (G11)
+__device__ __forceinline__ void split_offset(float x, int &di, float &dn) {
+    float fl = floorf(x);
+    di = (int)fl;
+    dn = x - fl;
+    if (dn >= 1.0f) { dn = 0.0f; di += 1; }          // tiny negative x: x - floor(x) rounds to 1
+}
+
+}  // namespace ent

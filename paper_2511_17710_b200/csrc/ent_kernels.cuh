@@ -1,0 +1,239 @@
+// ent_kernels.cuh -- untiled kernels: one thread per particle, global gathers, global atomics.
+// This is the structure of the paper's own pusher and deposit functors and serves as the in-repo
+// baseline for the tiled kernel (ent_tiled.cuh) as well as the path for unsorted particle blocks.
+#pragma once
+#include "ent_particle.cuh"
+
+namespace ent {
+
+struct FieldPtrs { const float *c[6]; };
+struct CurrentPtrs { float *c[3]; };
+struct PartPtrs {
+    int32_t *cell; float *d[3]; float *phi; float *u[3]; float *w; uint8_t *tag;
+};
+
+constexpr int TPB = 256;
+
+// ---- S0-S5: ent_gather_push ----
+template <int D, int KIND>
+__global__ void __launch_bounds__(TPB) gather_push_kernel(GridDev g, FieldPtrs F, PartPtrs in, PartPtrs out, long long n,
+                                                          float eps, float dt) {
+    long long p = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (p >= n) return;
+    bool alive = in.tag ? in.tag[p] != 0 : true;
+    int i[3], di[3]; float d[3] = {0.f, 0.f, 0.f}, u[3], phi = 0.f;
+    int cell = in.cell[p];
+#pragma unroll
+    for (int a = 0; a < D; ++a) d[a] = in.d[a][p];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) u[a] = in.u[a][p];
+    if (KIND != ENT_CART) phi = in.phi[p];
+    if (alive) {
+        unpack_cell<D>(g, cell, i);
+        const float *const Fp[6] = { F.c[0], F.c[1], F.c[2], F.c[3], F.c[4], F.c[5] };
+        GlobalFieldLoader ld{Fp};
+        push_particle<D, KIND>(g, ld, i, d, phi, u, eps, dt, di, alive);
+        cell = pack_cell<D>(g, i);
+    }
+    out.cell[p] = cell;
+#pragma unroll
+    for (int a = 0; a < D; ++a) out.d[a][p] = d[a];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) out.u[a][p] = u[a];
+    if (KIND != ENT_CART) out.phi[p] = phi;
+    if (out.tag) out.tag[p] = alive ? 1 : 0;
+}
+
+// ---- S7: ent_deposit (old and new blocks in memory, the paper's i_prev/dx_prev structure) ----
+template <int D, int KIND>
+__global__ void __launch_bounds__(TPB) deposit_kernel(GridDev g, PartPtrs po, PartPtrs pn, CurrentPtrs J, long long n,
+                                                      float q, float inv_dt, unsigned long long *bad_moves) {
+    long long p = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (p >= n) return;
+    bool alive = (po.tag ? po.tag[p] != 0 : true) && (pn.tag ? pn.tag[p] != 0 : true);
+    if (!alive) return;                                                        // G9
+    int i0[3], i1[3], di[3] = {0, 0, 0};
+    unpack_cell<D>(g, po.cell[p], i0);
+    unpack_cell<D>(g, pn.cell[p], i1);
+    float a[3] = {0.f, 0.f, 0.f}, dn[3] = {0.f, 0.f, 0.f}, u[3];
+    bool bad = false;
+#pragma unroll
+    for (int k = 0; k < D; ++k) {
+        int dd = i1[k] - i0[k];
+        if (g.bc[k] == ENT_PERIODIC) {                                         // recover the un-wrapped shift
+            if (2 * dd > g.N[k]) dd -= g.N[k];
+            else if (2 * dd < -g.N[k]) dd += g.N[k];
+        }
+        if (dd < -1 || dd > 1) bad = true;
+        di[k] = dd;
+        a[k] = po.d[k][p];
+        dn[k] = pn.d[k][p];
+    }
+    if (bad) { atomicAdd(bad_moves, 1ULL); return; }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) u[k] = pn.u[k][p];
+    float phi0 = 0.f, phi1 = 0.f;
+    if (KIND != ENT_CART) { phi0 = po.phi[p]; phi1 = pn.phi[p]; }
+    float *const Jp[3] = { J.c[0], J.c[1], J.c[2] };
+    GlobalAcc acc{Jp};
+    deposit_particle<D, KIND>(g, acc, i0, a, di, dn, phi0, phi1, u, q * po.w[p], inv_dt);
+}
+
+// ---- fused S0-S7, in place, untiled ----
+template <int D, int KIND>
+__global__ void __launch_bounds__(TPB) step_untiled_kernel(GridDev g, FieldPtrs F, PartPtrs P, CurrentPtrs J, long long n,
+                                                           float eps, float dt, float q, float inv_dt,
+                                                           unsigned long long *bad_moves) {
+    long long p = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (p >= n) return;
+    bool alive = P.tag ? P.tag[p] != 0 : true;
+    if (!alive) return;                                                        // dead particles are left untouched
+    int i[3], i0[3], di[3]; float d[3] = {0.f, 0.f, 0.f}, a[3], u[3], phi = 0.f;
+    unpack_cell<D>(g, P.cell[p], i);
+#pragma unroll
+    for (int k = 0; k < D; ++k) d[k] = P.d[k][p];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { u[k] = P.u[k][p]; a[k] = d[k]; i0[k] = i[k]; }
+    if (KIND != ENT_CART) phi = P.phi[p];
+    float phi0 = phi;
+    const float *const Fp[6] = { F.c[0], F.c[1], F.c[2], F.c[3], F.c[4], F.c[5] };
+    GlobalFieldLoader ld{Fp};
+    push_particle<D, KIND>(g, ld, i, d, phi, u, eps, dt, di, alive);
+    P.cell[p] = pack_cell<D>(g, i);
+#pragma unroll
+    for (int k = 0; k < D; ++k) P.d[k][p] = d[k];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) P.u[k][p] = u[k];
+    if (KIND != ENT_CART) P.phi[p] = phi;
+    if (!alive) { P.tag[p] = 0; return; }
+    bool bad = false;
+#pragma unroll
+    for (int k = 0; k < D; ++k) bad |= (di[k] < -1 || di[k] > 1);
+    if (bad) { atomicAdd(bad_moves, 1ULL); return; }
+    float *const Jp[3] = { J.c[0], J.c[1], J.c[2] };
+    GlobalAcc acc{Jp};
+    deposit_particle<D, KIND>(g, acc, i0, a, di, d, phi0, phi, u, q * P.w[p], inv_dt);
+}
+
+// ---- S9: periodic ghost fold of one padded array along dimension dim ----
+// pass 0: active += ghost on the opposite side, ghost = 0;  pass 1: ghost = periodic image.
+// One thread per (ghost layer gi, transverse point); the transverse range covers the whole padded extent so that
+// edges and corners are folded dimension after dimension.
+__global__ void fold_kernel(GridDev g, float *A, int dim, int pass) {
+    int a = (dim + 1) % 3, b = (dim + 2) % 3;
+    long long na = g.P[a], nb = g.P[b];
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= na * nb * NG) return;
+    int gi = (int)(t % NG); t /= NG;
+    long long ia = t % na, ib = t / na;
+    long long stride[3] = { 1, g.P[0], (long long)g.P[0] * g.P[1] };
+    float *line = A + ia * stride[a] + ib * stride[b];
+    int N = g.N[dim];
+    long long lo = gi, hi = NG + N + gi;
+    long long sd = stride[dim];
+    if (pass == 0) {
+        atomicAdd(&line[(lo + N) * sd], line[lo * sd]);      // atomics: for N < 4 two ghost layers fold onto one cell
+        atomicAdd(&line[(hi - N) * sd], line[hi * sd]);
+        line[lo * sd] = 0.f;
+        line[hi * sd] = 0.f;
+    } else {
+        line[lo * sd] = line[(lo + N) * sd];
+        line[hi * sd] = line[(hi - N) * sd];
+    }
+}
+
+// ---- S10: counting sort by tile-major key ----
+template <int D>
+__global__ void __launch_bounds__(TPB) sort_hist_kernel(GridDev g, const int32_t *cell, long long n, int32_t *keys, int32_t *count) {
+    long long p = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (p >= n) return;
+    int i[3];
+    unpack_cell<D>(g, cell[p], i);
+    int k = sort_key<D>(g, i);
+    keys[p] = k;
+    atomicAdd(count + k, 1);
+}
+
+constexpr int SCAN_ITEMS = 8;
+constexpr int SCAN_CHUNK = TPB * SCAN_ITEMS;
+
+__device__ __forceinline__ int block_exclusive_scan(int v, int &total) {      // TPB threads
+    __shared__ int wsum[TPB / 32];
+    int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (lane == 31) wsum[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+        int s = lane < TPB / 32 ? wsum[lane] : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += y; }
+        if (lane < TPB / 32) wsum[lane] = s;
+    }
+    __syncthreads();
+    int base = wid ? wsum[wid - 1] : 0;
+    total = wsum[TPB / 32 - 1];
+    __syncthreads();
+    return base + x - v;
+}
+
+// pass 1: per-chunk totals
+__global__ void __launch_bounds__(TPB) scan_reduce_kernel(const int32_t *in, long long m, int32_t *chunk_sum) {
+    long long base = (long long)blockIdx.x * SCAN_CHUNK + (long long)threadIdx.x * SCAN_ITEMS;
+    int s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) if (base + k < m) s += in[base + k];
+    int total;
+    block_exclusive_scan(s, total);
+    if (threadIdx.x == 0) chunk_sum[blockIdx.x] = total;
+}
+// pass 2: exclusive scan of the chunk totals, one block
+__global__ void __launch_bounds__(TPB) scan_chunks_kernel(int32_t *chunk_sum, int nchunks) {
+    __shared__ int carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < nchunks; b0 += TPB) {
+        int idx = b0 + threadIdx.x;
+        int v = idx < nchunks ? chunk_sum[idx] : 0;
+        int total;
+        int ex = block_exclusive_scan(v, total);
+        int c = carry;
+        if (idx < nchunks) chunk_sum[idx] = c + ex;
+        __syncthreads();
+        if (threadIdx.x == 0) carry = c + total;
+        __syncthreads();
+    }
+}
+// pass 3: exclusive scan inside each chunk + chunk offset; out[m] = grand total is written by the last chunk.
+// `cursor` (may alias nothing) receives a second copy used as the scatter cursor.
+__global__ void __launch_bounds__(TPB) scan_apply_kernel(const int32_t *in, long long m, const int32_t *chunk_off,
+                                                         int32_t *out, int32_t *cursor) {
+    long long base = (long long)blockIdx.x * SCAN_CHUNK + (long long)threadIdx.x * SCAN_ITEMS;
+    int v[SCAN_ITEMS]; int s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = base + k < m ? in[base + k] : 0; s += v[k]; }
+    int total;
+    int ex = block_exclusive_scan(s, total) + chunk_off[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        if (base + k < m) { out[base + k] = ex; cursor[base + k] = ex; }
+        ex += v[k];
+        if (base + k == m - 1) out[m] = ex;
+    }
+}
+
+__global__ void __launch_bounds__(TPB) sort_scatter_kernel(const int32_t *keys, int32_t *cursor, PartPtrs in, PartPtrs out,
+                                                           long long n, int D, int axisym) {
+    long long p = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (p >= n) return;
+    long long dst = atomicAdd(cursor + keys[p], 1);
+    out.cell[dst] = in.cell[p];
+    for (int a = 0; a < D; ++a) out.d[a][dst] = in.d[a][p];
+    for (int a = 0; a < 3; ++a) out.u[a][dst] = in.u[a][p];
+    out.w[dst] = in.w[p];
+    if (axisym) out.phi[dst] = in.phi[p];
+    if (in.tag) out.tag[dst] = in.tag[p];
+}
+
+}  // namespace ent

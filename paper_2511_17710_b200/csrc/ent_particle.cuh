@@ -1,0 +1,183 @@
+// ent_particle.cuh -- one particle through sub-steps 3-8.  Used by the untiled and the tiled kernels.
+#pragma once
+#include "ent_dev.cuh"
+
+namespace ent {
+
+// ---------------------------------------------------------------------------------------------------------
+// S1-S5 for one particle.  In: cell indices i[], offsets d[], phi, u[].  Out: the same, advanced by one step;
+// di[] = un-wrapped cell shift per dimension (for the deposit), alive = false if it left through an ABSORB side.
+// eps = (q/m) dt / 2.
+// ---------------------------------------------------------------------------------------------------------
+template <int D, int KIND, class Loader>
+__device__ __forceinline__ void push_particle(const GridDev &g, const Loader &ld, int i[3], float d[3], float &phi,
+                                              float u[3], float eps, float dt, int di[3], bool &alive) {
+    float EB[6];
+    gather<D>(g, ld, i, d, EB);                                               // step 3
+    float E[3], B[3];
+    if (KIND == ENT_CART) {
+        // step 4: A^hat = sqrt(h_ii) A^i; Cartesian code basis is already aligned with x,y,z
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { E[a] = g.dx[a] * EB[a]; B[a] = g.dx[a] * EB[3 + a]; }
+        boris(u, E, B, eps);                                                  // step 5, Eq. 3
+        float ig = inv_gamma(u);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {                                         // steps 6-7
+            if (a < D) {
+                float x = d[a] + (u[a] * ig) * (dt * g.inv_dx[a]);
+                split_offset(x, di[a], d[a]);
+            } else di[a] = 0;
+        }
+    } else {
+        // axisymmetric: particle at (x1, x2, phi); fp64 geometry
+        double x1 = (double)i[0] + (double)d[0], x2 = (double)i[1] + (double)d[1], ph = (double)phi;
+        Sph s = sph_of_code<KIND>(g, x1, x2);
+        double st, ct, sp, cp;
+        sincos(s.th, &st, &ct);
+        sincos(ph, &sp, &cp);
+        {   // step 4: tetrad (at the particle, G2) then rotation (r,th,phi)-hat -> (x,y,z)-hat
+            float fst = (float)st, fct = (float)ct, fsp = (float)sp, fcp = (float)cp;
+            float h1 = (float)s.sh1, h2 = (float)s.sh2, h3 = (float)s.sh3;
+            float Ar = h1 * EB[0], At = h2 * EB[1], Ap = h3 * EB[2];
+            E[0] = Ar * fst * fcp + At * fct * fcp - Ap * fsp;
+            E[1] = Ar * fst * fsp + At * fct * fsp + Ap * fcp;
+            E[2] = Ar * fct - At * fst;
+            Ar = h1 * EB[3]; At = h2 * EB[4]; Ap = h3 * EB[5];
+            B[0] = Ar * fst * fcp + At * fct * fcp - Ap * fsp;
+            B[1] = Ar * fst * fsp + At * fct * fsp + Ap * fcp;
+            B[2] = Ar * fct - At * fst;
+        }
+        boris(u, E, B, eps);
+        float ig = inv_gamma(u);
+        // step 6: x^X += u/gamma dt in the global Cartesian frame
+        double X = s.r * st * cp + (double)(u[0] * ig) * (double)dt;
+        double Y = s.r * st * sp + (double)(u[1] * ig) * (double)dt;
+        double Z = s.r * ct + (double)(u[2] * ig) * (double)dt;
+        // step 7: back to code coordinates
+        double rho2 = X * X + Y * Y;
+        double rn = sqrt(rho2 + Z * Z);
+        double thn = 0.5 * PI_D - atan2(Z, sqrt(rho2));
+        double phn = PI_D - atan2(Y, -X);
+        double y1, y2;
+        if (KIND == ENT_SPH) { y1 = (rn - g.rmin) / g.dr; y2 = thn / g.dth; }
+        else { y1 = (log(rn - g.r0) - g.Rmin) / g.dR; y2 = T_of_theta(g.vt, thn) / g.dT; }
+        float phf = (float)phn;
+        if (phf >= TWO_PI_F) phf -= TWO_PI_F;
+        if (phf < 0.f) phf = 0.f;
+        phi = phf;
+        double f1 = floor(y1), f2 = floor(y2);
+        int n1 = (int)f1, n2 = (int)f2;
+        float e1 = (float)(y1 - f1), e2 = (float)(y2 - f2);
+        if (e1 >= 1.0f) { e1 = 0.f; n1 += 1; }                                // rounding to fp32 reached the upper face
+        if (e2 >= 1.0f) { e2 = 0.f; n2 += 1; }
+        di[0] = n1 - i[0]; di[1] = n2 - i[1]; di[2] = 0;
+        d[0] = e1; d[1] = e2;
+    }
+    // O7 crossing bookkeeping
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (a >= D) continue;
+        int in = i[a] + di[a];
+        if (g.bc[a] == ENT_PERIODIC) {
+            if (in < 0) in += g.N[a];
+            if (in >= g.N[a]) in -= g.N[a];
+        } else if (g.bc[a] == ENT_AXIS) {
+            if (in >= g.N[a]) { in = g.N[a] - 1; d[a] = 0.99999994f; di[a] = in - i[a]; }   // theta = pi exactly (G11)
+            if (in < 0) { in = 0; d[a] = 0.f; di[a] = in - i[a]; }
+        } else {                                                              // ABSORB (G9)
+            if (in < 0) { alive = false; in = 0; }
+            if (in >= g.N[a]) { alive = false; in = g.N[a] - 1; }
+        }
+        i[a] = in;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S7 deposit for one particle (Eq. 6, step 8 P:155-157, "modified zig-zag" P:575).
+// i0[], a[] = old cell and offset; di[] = un-wrapped cell shift in {-1,0,1}; dn[] = new offset;
+// Q = q w / dt; qw = q w.  Acc::add(comp, padded_index, value) accumulates one contribution.
+// All arithmetic is in the old cell's frame (small numbers only: "(real)(i+delta) is never necessary").
+// ---------------------------------------------------------------------------------------------------------
+struct GlobalAcc {
+    float *const *J;
+    __device__ __forceinline__ void add(int comp, long long idx, float v) const { atomicAdd(J[comp] + idx, v); }
+};
+
+template <int D, class Acc>
+__device__ __forceinline__ void deposit_segment(const Acc &acc, long long base, long long s1, long long s2,
+                                                const float Dv[3], const float W[3], float Q, float hv) {
+    if (D == 3) {
+        // J^comp at the 4 transverse nodes: Q D_comp [ w(W_a,s_a) w(W_b,s_b) +- D_a D_b / 12 ]  (reading G7)
+        const long long st[3] = { 1, s1, s2 };
+#pragma unroll
+        for (int comp = 0; comp < 3; ++comp) {
+            const int a = (comp + 1) % 3, b = (comp + 2) % 3;
+            float c = Dv[a] * Dv[b] * (1.0f / 12.0f);
+            float QD = Q * Dv[comp];
+            float w11 = W[a] * W[b] + c;
+            float w10 = W[a] - w11;           // W_a (1 - W_b) - c
+            float w01 = W[b] - w11;           // (1 - W_a) W_b - c
+            float w00 = 1.0f - W[a] - w01;    // (1 - W_a)(1 - W_b) + c
+            acc.add(comp, base, QD * w00);
+            acc.add(comp, base + st[a], QD * w10);
+            acc.add(comp, base + st[b], QD * w01);
+            acc.add(comp, base + st[a] + st[b], QD * w11);
+        }
+    } else {
+        float q0 = Q * Dv[0], q1 = Q * Dv[1];
+        acc.add(0, base, q0 * (1.0f - W[1]));
+        acc.add(0, base + s1, q0 * W[1]);
+        acc.add(1, base, q1 * (1.0f - W[0]));
+        acc.add(1, base + 1, q1 * W[0]);
+        float h1 = hv * W[1], h0 = hv - h1;                                   // out-of-plane, velocity form (G8)
+        acc.add(2, base, h0 * (1.0f - W[0]));
+        acc.add(2, base + 1, h0 * W[0]);
+        acc.add(2, base + s1, h1 * (1.0f - W[0]));
+        acc.add(2, base + s1 + 1, h1 * W[0]);
+    }
+}
+
+// out-of-plane rate q w v^3_code / 2 per segment for the 2D grids (G8); u = momentum at n+1/2
+template <int KIND>
+__device__ __forceinline__ float half_qw_v3(const GridDev &g, const int i0[3], const float a[3], const float b[3],
+                                            float phi0, float phi1, const float u[3], float qw) {
+    float ig = inv_gamma(u);
+    if (KIND == ENT_CART) return 0.5f * qw * (u[2] * ig);                     // h33 = 1
+    double dphi = (double)phi1 - (double)phi0;
+    dphi -= 2.0 * PI_D * floor((dphi + PI_D) / (2.0 * PI_D));                 // shorter arc
+    double phm = (double)phi0 + 0.5 * dphi;
+    double x1 = (double)i0[0] + 0.5 * ((double)a[0] + (double)b[0]);
+    double x2 = (double)i0[1] + 0.5 * ((double)a[1] + (double)b[1]);
+    Sph s = sph_of_code<KIND>(g, x1, x2);
+    if (s.sh3 < 1e-12) return 0.f;
+    double sp, cp;
+    sincos(phm, &sp, &cp);
+    double v3 = ((-(double)u[0] * sp + (double)u[1] * cp) * (double)ig) / s.sh3;
+    return (float)(0.5 * (double)qw * v3);
+}
+
+template <int D, int KIND, class Acc>
+__device__ __forceinline__ void deposit_particle(const GridDev &g, const Acc &acc, const int i0[3], const float a[3],
+                                                 const int di[3], const float dn[3], float phi0, float phi1,
+                                                 const float u[3], float qw, float inv_dt) {
+    float D1[3], W1[3], D2[3], W2[3], b[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        if (k < D) {
+            b[k] = (float)di[k] + dn[k];                                      // new position in the old cell's frame
+            float r = di[k] == 0 ? 0.5f * (a[k] + b[k]) : (di[k] > 0 ? 1.0f : 0.0f);   // relay point
+            D1[k] = r - a[k];  W1[k] = 0.5f * (a[k] + r);
+            D2[k] = b[k] - r;  W2[k] = 0.5f * (r + b[k]) - (float)di[k];
+        } else { b[k] = 0.f; D1[k] = W1[k] = D2[k] = W2[k] = 0.f; }
+    }
+    const long long s1 = g.P[0], s2 = (long long)g.P[0] * g.P[1];
+    long long base1 = pidx<D>(g, i0[0], i0[1], i0[2]);
+    long long base2 = base1 + di[0] + s1 * di[1] + (D == 3 ? s2 * di[2] : 0);   // un-wrapped: may point into the ghosts
+    float Q = qw * inv_dt;
+    float hv = 0.f;
+    if (D == 2) hv = half_qw_v3<KIND>(g, i0, a, b, phi0, phi1, u, qw);
+    deposit_segment<D>(acc, base1, s1, s2, D1, W1, Q, hv);
+    deposit_segment<D>(acc, base2, s1, s2, D2, W2, Q, hv);
+}
+
+}  // namespace ent

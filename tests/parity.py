@@ -1,0 +1,139 @@
+"""Parity plumbing shared by the GPU tests, smoke() and nothing else: packs one seeded synthetic workload for the CUDA
+library (binding.Particles, fp32 on the device) and for the fp64 oracle (orc.Particles, numpy), and compares results
+with the rules of DESIGN.md "parity definition".  No arithmetic of the method lives here.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+POS_TOL = 1e-5          # |delta(i + d)| in cells (BASELINE.json: positions within 1e-5)
+MOM_TOL = 1e-5          # |delta u| / max(|u|_2, U_FLOOR)  (BASELINE.json: momenta within a relative error of 1e-5)
+U_FLOOR = 1e-2
+J_TOL = 1e-5            # max|J_gpu - J_orc| / max|J_orc|
+CONT_TOL = 1e-6         # continuity residual / normaliser
+FACE_EPS = 1e-5         # oracle offsets closer than this to a face are "straddlers" (G12)
+
+
+def species_to_ent(bind, synth, grid, sp, device, with_tag=True):
+    """synth.Species -> binding.Particles on `device` (packed linear cell index, fp32)"""
+    dev = torch.device(device)
+    mv = lambda t: t.to(dev).contiguous()
+    return bind.Particles(cell=mv(synth.pack_cell(grid, sp.i)), d=[mv(t) for t in sp.d], u=[mv(t) for t in sp.u], w=mv(sp.w),
+                          phi=None if sp.phi is None else mv(sp.phi),
+                          tag=torch.ones(sp.n, dtype=torch.uint8, device=dev) if with_tag else None, q=sp.q, m=sp.m)
+
+
+def species_to_orc(orc, sp):
+    """synth.Species -> orc.Particles (int32 indices per dimension, float64 copies of the SAME fp32 values)"""
+    f64 = lambda t: np.ascontiguousarray(t.detach().cpu().numpy().astype(np.float64))
+    return orc.Particles(i=[np.ascontiguousarray(t.detach().cpu().numpy().astype(np.int32)) for t in sp.i],
+                         d=[f64(t) for t in sp.d], u=[f64(t) for t in sp.u], w=f64(sp.w),
+                         phi=None if sp.phi is None else f64(sp.phi), tag=np.ones(sp.n, dtype=np.int8))
+
+
+def grid_to_ent(bind, g):
+    return bind.Grid(D=g.D, N=tuple(g.N), bc=tuple(g.bc), kind=g.kind, xmin=tuple(g.xmin), xmax=tuple(g.xmax), r0=g.r0,
+                     vartheta=g.vartheta)
+
+
+def grid_to_orc(orc, g):
+    return orc.Grid(D=g.D, N=tuple(g.N), bc=tuple(g.bc), kind=g.kind, xmin=tuple(g.xmin), xmax=tuple(g.xmax), r0=g.r0,
+                    vartheta=g.vartheta)
+
+
+def fields_to_orc(fields):
+    return [np.ascontiguousarray(f.detach().cpu().numpy()) for f in fields]
+
+
+def unpack_cell_np(grid, cell):
+    c = cell.astype(np.int64)
+    N0, N1 = int(grid.N[0]), int(grid.N[1])
+    if grid.D == 2:
+        return [c % N0, c // N0]
+    return [c % N0, (c // N0) % N1, c // (N0 * N1)]
+
+
+def compare_particles(grid, pe, po, order=None):
+    """pe: binding.Particles (any device), po: orc.Particles.  `order`: optional index array such that GPU particle k is
+    oracle particle order[k] (after a sort).  Returns a dict of maxima and counts; raises AssertionError on a violation."""
+    cell = pe.cell.detach().cpu().numpy()
+    ig = unpack_cell_np(grid, cell)
+    sel = (lambda a: a) if order is None else (lambda a: a[order])
+    tag_g = np.ones(cell.shape[0], dtype=bool) if pe.tag is None else pe.tag.detach().cpu().numpy() != 0
+    tag_o = np.ones(cell.shape[0], dtype=bool) if po.tag is None else sel(po.tag) != 0
+    both = tag_g & tag_o
+    stats = {"n": int(cell.shape[0]), "alive": int(both.sum()), "tag_mismatch": int((tag_g != tag_o).sum()), "straddlers": 0,
+             "max_pos_err": 0.0, "max_u_rel": 0.0, "max_phi_err": 0.0}
+    strad_any = np.zeros(cell.shape[0], dtype=bool)
+    PERIODIC = 0
+    for a in range(grid.D):
+        dg = pe.d[a].detach().cpu().numpy().astype(np.float64)
+        io, do = sel(po.i[a]).astype(np.int64), sel(po.d[a])
+        assert np.all((dg >= 0.0) & (dg < 1.0)), f"GPU offset outside [0,1) in dimension {a}"
+        strad = np.minimum(do, 1.0 - do) <= FACE_EPS
+        strad_any |= strad & both
+        ok = both & ~strad
+        assert np.array_equal(ig[a][ok], io[ok]), (
+            f"cell index mismatch in dimension {a} for {int((ig[a][ok] != io[ok]).sum())} non-straddling particles")
+        diff = (ig[a] + dg) - (io + do)
+        if grid.bc[a] == PERIODIC:
+            N = int(grid.N[a])
+            diff = diff - N * np.round(diff / N)
+        err = np.abs(diff[both])
+        if err.size:
+            stats["max_pos_err"] = max(stats["max_pos_err"], float(err.max()))
+    stats["straddlers"] = int(strad_any.sum())
+    ug = np.stack([t.detach().cpu().numpy().astype(np.float64) for t in pe.u])
+    uo = np.stack([sel(t) for t in po.u])
+    rel = np.abs(ug - uo).max(axis=0) / np.maximum(np.sqrt((uo * uo).sum(axis=0)), U_FLOOR)
+    if rel.size:
+        stats["max_u_rel"] = float(rel.max())
+    if pe.phi is not None:
+        dphi = pe.phi.detach().cpu().numpy().astype(np.float64) - sel(po.phi)
+        dphi = dphi - 2.0 * np.pi * np.round(dphi / (2.0 * np.pi))
+        if both.any():
+            stats["max_phi_err"] = float(np.abs(dphi[both]).max())
+    assert stats["max_pos_err"] <= POS_TOL, stats
+    assert stats["max_u_rel"] <= MOM_TOL, stats
+    assert stats["max_phi_err"] <= 2e-6 * 2.0 * np.pi + POS_TOL, stats      # fp32 storage of phi in [0, 2 pi)
+    # a tag can only differ for a particle that straddles an absorbing face
+    assert stats["tag_mismatch"] <= stats["straddlers"], stats
+    return stats
+
+
+def compare_current(Jg, Jo):
+    """Jg: list of 3 torch tensors (after fold), Jo: list of 3 float64 numpy arrays (after fold)"""
+    scale = max(float(np.abs(j).max()) for j in Jo)
+    err = max(float(np.abs(g.detach().cpu().numpy().astype(np.float64) - o).max()) for g, o in zip(Jg, Jo))
+    rel = err / scale if scale > 0 else err
+    assert rel <= J_TOL, f"max|J_gpu - J_orc| / max|J_orc| = {rel:.3e} (scale {scale:.3e})"
+    return rel
+
+
+def continuity_of_gpu_step(orc, og, p_before, p_after, Jg_folded, q, dt):
+    """Eq. 6 on the GPU's own output: the oracle's CHECKER is applied to the GPU positions and currents.
+    p_before / p_after: orc.Particles built from the GPU arrays (fp32 values up-cast).  Returns residual / normaliser."""
+    alive = np.ones(p_before.n, dtype=np.int8)
+    if p_before.tag is not None:
+        alive &= (p_before.tag != 0).astype(np.int8)
+    if p_after.tag is not None:
+        alive &= (p_after.tag != 0).astype(np.int8)
+    rho0 = orc.charge_density(og, p_before, q, mask=alive)
+    rho1 = orc.charge_density(og, p_after, q, mask=alive)
+    norm = orc.charge_density(og, p_before, abs(q), mask=alive)
+    J = [np.ascontiguousarray(j.detach().cpu().numpy().astype(np.float64)) for j in Jg_folded]
+    orc.fold_scalar(og, rho0); orc.fold_scalar(og, rho1); orc.fold_scalar(og, norm)
+    res = orc.continuity_residual(og, J, rho0, rho1, dt)
+    scale = float(np.abs(norm).max()) / dt
+    return res / scale if scale > 0 else res
+
+
+def ent_to_orc(orc, grid, pe):
+    """binding.Particles (GPU result) -> orc.Particles holding the same values (for the continuity checker)"""
+    cell = pe.cell.detach().cpu().numpy()
+    i = [np.ascontiguousarray(a.astype(np.int32)) for a in unpack_cell_np(grid, cell)]
+    f64 = lambda t: np.ascontiguousarray(t.detach().cpu().numpy().astype(np.float64))
+    return orc.Particles(i=i, d=[f64(t) for t in pe.d], u=[f64(t) for t in pe.u], w=f64(pe.w),
+                         phi=None if pe.phi is None else f64(pe.phi),
+                         tag=None if pe.tag is None else np.ascontiguousarray(pe.tag.detach().cpu().numpy().astype(np.int8)))

@@ -1,0 +1,107 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the fp64 oracle, element by element, on
+the same seeded synthetic inputs.  Sizes: the oracle finishes each case in seconds; every case spans several tiles and a
+ragged tail.  Tolerances are BASELINE.json's (north_star), written in tests/parity.py.
+"""
+import numpy as np
+import pytest
+import torch
+
+import parity as P
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env(orc):
+    from paper_2511_17710_b200 import binding as bind, synth
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device: there is no CPU fallback for the product path")
+    ctx = bind.ent_create(0, None)
+    yield bind, synth, ctx, orc
+    bind.ent_destroy(ctx)
+
+
+def _workloads(synth):
+    return {
+        "C1": lambda: synth.config1(1),                 # full size: 64x64, 65,536 particles
+        "C2/4": lambda: synth.config2(4),               # 64x64 log-spherical, ~131k particles, density ~ r^-2
+        "C3/8": lambda: synth.config3(8),               # 32^3, 262,144 particles
+        "C4/16": lambda: synth.config4(16),             # 32^3, 131,072 particles, counter-streaming beams
+        "C4/16-shuffled": lambda: synth.config4(16, shuffled=True),
+        "C5/32": lambda: synth.config5(32),             # 64x64 quasi-spherical vartheta = 0.4, ~262k particles
+        "SPH": lambda: synth.sph_small(48),             # linear-r spherical metric
+    }
+
+
+def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True):
+    bind, synth, ctx, orc = env
+    g = wl.grid
+    eg, og = P.grid_to_ent(bind, g), P.grid_to_orc(orc, g)
+    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, impl)
+    bind.ent_set_grid(ctx, eg)
+    F_dev = [f.cuda() for f in wl.fields]
+    F_orc = P.fields_to_orc(wl.fields)
+    steps = wl.steps if steps is None else steps
+    out = {}
+    for si, sp in enumerate(wl.species):                       # species loop is serial on the host
+        pe = P.species_to_ent(bind, synth, g, sp, "cuda")
+        po = P.species_to_orc(orc, sp)
+        order = None
+        if sort_first:
+            # carry the original index through the sort as the bit pattern of the weight array (the order inside a cell
+            # is unspecified, G18), then put the real weights back in sorted order
+            scratch = pe.clone()
+            scratch.w = torch.arange(pe.n, device="cuda", dtype=torch.int32).view(torch.float32).clone()
+            ps = scratch.empty_like()
+            bind.ent_sort(ctx, scratch, ps, None)
+            order_t = ps.w.view(torch.int32).to(torch.int64)
+            assert torch.equal(torch.sort(order_t).values, torch.arange(pe.n, device="cuda")), "ent_sort lost particles"
+            ps.w.copy_(pe.w[order_t])
+            order = order_t.cpu().numpy()
+            pe = ps
+        Jg = bind.zeros_current(eg, "cuda")
+        worstJ = worstC = 0.0
+        for s in range(steps):
+            before = P.ent_to_orc(orc, g, pe) if check_every_step else None
+            bind.ent_zero_current(ctx, Jg)
+            bind.ent_step(ctx, F_dev, pe, Jg, wl.dt)
+            bind.ent_fold_current(ctx, Jg)
+            torch.cuda.synchronize()
+            Jo = orc.zeros_current(og)
+            orc.step(og, F_orc, po, Jo, sp.q, sp.m, wl.dt)
+            orc.fold_current(og, Jo)
+            if check_every_step or s == steps - 1:
+                worstJ = max(worstJ, P.compare_current(Jg, Jo))
+            if check_every_step:
+                after = P.ent_to_orc(orc, g, pe)
+                c = P.continuity_of_gpu_step(orc, og, before, after, Jg, sp.q, wl.dt)
+                assert c <= P.CONT_TOL, f"continuity residual {c:.3e} at step {s}"
+                worstC = max(worstC, c)
+        stats = P.compare_particles(g, pe, po, order)
+        assert bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES) == 0
+        stats.update(worstJ=worstJ, worstC=worstC)
+        out[si] = stats
+    return out
+
+
+@pytest.mark.parametrize("name", ["C1", "C2/4", "C3/8", "C4/16", "C4/16-shuffled", "C5/32", "SPH"])
+def test_fused_step_untiled_matches_oracle(env, name):
+    wl = _workloads(env[1])[name]()
+    stats = _run_case(env, wl, impl=1)
+    print(name, stats)
+
+
+@pytest.mark.parametrize("name", ["C1", "C3/8", "C5/32"])
+def test_two_kernel_step_matches_oracle(env, name):
+    """ent_gather_push + ent_deposit with the old block kept in memory (the paper's structure)"""
+    wl = _workloads(env[1])[name]()
+    stats = _run_case(env, wl, impl=2, steps=3)
+    print(name, stats)
+
+
+@pytest.mark.parametrize("name", ["C1", "C2/4", "C3/8", "C4/16-shuffled", "C5/32"])
+def test_sorted_step_auto_path_matches_oracle(env, name):
+    """ent_sort, then ent_step on the sorted block (auto: the tiled kernel where it is supported)"""
+    wl = _workloads(env[1])[name]()
+    stats = _run_case(env, wl, impl=0, sort_first=True)
+    print(name, stats)
