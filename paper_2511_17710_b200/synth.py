@@ -421,7 +421,9 @@ def config2(shrink: int = 1, device="cpu") -> Workload:
     """C2: axisymmetric log-spherical (QSPH r0 = 0, vartheta = 0; reading G15) 256x256, r in [1,20], static dipole plus
     corotation E (Omega = 0.1), pair plasma 32 ppc ~ r^-2, theta_T = 0.05, |q/m| = 100, 20 steps."""
     N = max(16, 256 // shrink)
-    return _axisym_workload("C2", 1, N, 20.0, 0.0, 16.0, 0.05, 100.0, _dipole_corotation(0.1), 20, device,
+    # |q/m| = 100 at full size puts omega_c dt = |q/m| B dt at ~0.8 at the pole of the stellar surface (B = 2); dt grows with the
+    # cell size, so the shrunk variants scale |q/m| by N/256 to keep that number (and with it the conditioning of the push)
+    return _axisym_workload("C2", 1, N, 20.0, 0.0, 16.0, 0.05, 100.0 * N / 256.0, _dipole_corotation(0.1), 20, device,
                             "magnetosphere shape (sect. 5.2), log-r uniform-theta grid (P:993)")
 
 
@@ -429,7 +431,7 @@ def config5(shrink: int = 1, device="cpu") -> Workload:
     """C5: quasi-spherical 2048x2048 (r0 = 0, vartheta = 0.4; reading G16), r in [1,50], rotating-dipole magnetosphere with
     an equatorial Harris-type current sheet (Omega = 0.2), pair plasma 64 ppc ~ r^-2, theta_T = 0.1, |q/m| = 1000, 20 steps."""
     N = max(16, 2048 // shrink)
-    return _axisym_workload("C5", 4, N, 50.0, 0.4, 32.0, 0.1, 1000.0, _magnetosphere(0.2), 20, device,
+    return _axisym_workload("C5", 4, N, 50.0, 0.4, 32.0, 0.1, 1000.0 * N / 2048.0, _magnetosphere(0.2), 20, device,
                             "pulsar-magnetosphere shape (sect. 5.2, P:993), theta stretched toward the equator")
 
 
@@ -439,7 +441,7 @@ def sph_small(N: int = 64, device="cpu") -> Workload:
     grid = GridSpec(D=2, N=(N, N), bc=(ABSORB, AXIS), kind=SPH, xmin=(1.0, 0.0), xmax=(10.0, math.pi))
     fields = axisym_fields(grid, _dipole_corotation(0.1), device)
     counts = torch.full((N * N,), 4, dtype=torch.int64)
-    sp = load_pairs(grid, seed, counts, 0.05, 1.0, 1.0 / 50.0, device)
+    sp = load_pairs(grid, seed, counts, 0.05, 1.0, 1.0 / 12.0, device)       # omega_c dt ~ 0.8 at the pole
     return Workload("SPH-small", grid, 0.5 * cfl_dx_min(grid), 20, fields, sp, seed, "linear-r spherical metric")
 
 

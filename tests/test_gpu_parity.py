@@ -71,13 +71,14 @@ def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True
             orc.step(og, F_orc, po, Jo, sp.q, sp.m, wl.dt)
             orc.fold_current(og, Jo)
             if check_every_step or s == steps - 1:
-                worstJ = max(worstJ, P.compare_current(Jg, Jo))
+                bound = P.offset_format_bound(orc, g, og, before, sp.q, wl.dt) if (eg.axisym and before is not None) else None
+                worstJ = max(worstJ, P.compare_current(Jg, Jo, bound))
             if check_every_step:
                 after = P.ent_to_orc(orc, g, pe)
                 c = P.continuity_of_gpu_step(orc, og, before, after, Jg, sp.q, wl.dt)
                 assert c <= P.CONT_TOL, f"continuity residual {c:.3e} at step {s}"
                 worstC = max(worstC, c)
-        stats = P.compare_particles(g, pe, po, order)
+        stats = P.compare_particles(g, pe, po, order, steps=steps)
         assert bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES) == 0
         stats.update(worstJ=worstJ, worstC=worstC)
         out[si] = stats
