@@ -31,8 +31,11 @@ struct ent_ctx {
     // host-call staging
     void *hbuf = nullptr; size_t hbuf_cap = 0;
     size_t scratch_bytes = 0;
-    // the block ent_sort produced last
-    const int32_t *sorted_cell = nullptr; long long sorted_n = -1;
+    // the blocks ent_sort produced (most recent first): each keeps its own tile offsets so that several species
+    // can stay "sorted" at the same time
+    struct SortedBlock { const int32_t *cell = nullptr; long long n = -1; int32_t *tile_off = nullptr; size_t cap = 0; unsigned long long stamp = 0; };
+    SortedBlock sorted[8];
+    unsigned long long sort_stamp = 0;
     int last_step_tiled = 0;
     TiledState tiled{};
 };
@@ -95,6 +98,7 @@ extern "C" int ent_destroy(ent_ctx *ctx) {
     tiled_release(ctx->tiled);
     cudaFree(ctx->counters); cudaFree(ctx->keys); cudaFree(ctx->count); cudaFree(ctx->offsets); cudaFree(ctx->cursor);
     cudaFree(ctx->chunk); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf);
+    for (auto &b : ctx->sorted) cudaFree(b.tile_off);
     cudaGetLastError();
     delete ctx;
     return ENT_OK;
@@ -156,7 +160,7 @@ extern "C" int ent_set_grid(ent_ctx *ctx, const ent_grid *gr) {
         g.dT = PI_D / gr->N[1];
     }
     ctx->grid = *gr; ctx->g = g; ctx->have_grid = true;
-    ctx->sorted_cell = nullptr; ctx->sorted_n = -1;
+    for (auto &b : ctx->sorted) { b.cell = nullptr; b.n = -1; }
     return tiled_set_grid(ctx->tiled, g, ctx->err, sizeof(ctx->err));
 }
 
@@ -298,9 +302,11 @@ extern "C" int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, en
     if (p->n == 0) return ENT_OK;
     if (ctx->step_impl == 2) return step_two_kernel(ctx, EB, p, J, dt);
     float eps = 0.5f * (p->q / p->m) * dt;
-    bool sorted = p->cell == ctx->sorted_cell && p->n == ctx->sorted_n;
-    if (ctx->step_impl == 0 && sorted && tiled_supported(ctx->tiled, ctx->g)) {
-        rc = tiled_step(ctx->tiled, ctx->g, ctx->stream, fp(EB), pp(p), cp(J), (long long)p->n, ctx->offsets, eps, dt, p->q,
+    const int32_t *tile_off = nullptr;
+    for (auto &b : ctx->sorted) if (b.cell == p->cell && b.n == p->n) tile_off = b.tile_off;
+    if (ctx->step_impl == 0 && tile_off && tiled_supported(ctx->tiled, ctx->g)) {
+        CK(cudaMemsetAsync(ctx->counters + 1, 0, sizeof(unsigned long long), ctx->stream));      // strays of THIS step
+        rc = tiled_step(ctx->tiled, ctx->g, ctx->stream, fp(EB), pp(p), cp(J), (long long)p->n, tile_off, eps, dt, p->q,
                         1.0f / dt, ctx->counters, &ctx->launches, ctx->err, sizeof(ctx->err));
         if (rc == ENT_OK) ctx->last_step_tiled = 1;
         return rc;
@@ -337,7 +343,7 @@ extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *ou
         if ((rc = ensure(ctx, (void **)&ctx->chunk, &cap, (size_t)nchunks * 4))) return rc;
         ctx->chunk_cap = (long long)(cap / 4);
     }
-    ctx->sorted_cell = nullptr; ctx->sorted_n = -1;
+    for (auto &b : ctx->sorted) if (b.cell == out->cell || b.cell == in->cell) { b.cell = nullptr; b.n = -1; }
     CK(cudaMemsetAsync(ctx->count, 0, (size_t)(nkeys + 1) * 4, ctx->stream));
     if (n > 0) {
         if (g.D == 2) sort_hist_kernel<2><<<nblk(n), TPB, 0, ctx->stream>>>(g, in->cell, n, ctx->keys, ctx->count);
@@ -356,7 +362,16 @@ extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *ou
     }
     if (key_offsets) CK(cudaMemcpyAsync(key_offsets, ctx->offsets, (size_t)(nkeys + 1) * 4, cudaMemcpyDeviceToDevice, ctx->stream));
     out->q = in->q; out->m = in->m;
-    ctx->sorted_cell = out->cell; ctx->sorted_n = n;
+    {   // remember `out` as sorted, with its own copy of the tile offsets (tile t = particles [tile_off[t], tile_off[t+1]))
+        ent_ctx::SortedBlock *slot = &ctx->sorted[0];
+        for (auto &b : ctx->sorted) { if (!b.cell) { slot = &b; break; } if (b.stamp < slot->stamp) slot = &b; }
+        const long long ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
+        slot->cell = nullptr; slot->n = -1;
+        if ((rc = ensure(ctx, (void **)&slot->tile_off, &slot->cap, (size_t)(ntiles + 1) * 4))) return rc;
+        tile_offsets_kernel<<<nblk(ntiles + 1), TPB, 0, ctx->stream>>>(ctx->offsets, g.tcells, ntiles, slot->tile_off);
+        if ((rc = launch_check(ctx, "tile_offsets_kernel"))) return rc;
+        slot->cell = out->cell; slot->n = n; slot->stamp = ++ctx->sort_stamp;
+    }
     return ENT_OK;
 }
 

@@ -223,6 +223,12 @@ __global__ void __launch_bounds__(TPB) scan_apply_kernel(const int32_t *in, long
     }
 }
 
+// tile_off[t] = key_offsets[t * tcells], t = 0..ntiles
+__global__ void tile_offsets_kernel(const int32_t *key_off, int tcells, long long ntiles, int32_t *tile_off) {
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t <= ntiles) tile_off[t] = key_off[t * tcells];
+}
+
 __global__ void __launch_bounds__(TPB) sort_scatter_kernel(const int32_t *keys, int32_t *cursor, PartPtrs in, PartPtrs out,
                                                            long long n, int D, int axisym) {
     long long p = (long long)blockIdx.x * TPB + threadIdx.x;

@@ -1,17 +1,484 @@
-// ent_tiled.cuh -- tiled fused step (placeholder until the tiled kernel lands: reports "unsupported" so that
-// ent_step takes the untiled kernel).
+// ent_tiled.cuh -- tiled fused step for the Cartesian grids (sub-steps 3-8), sm_100a.
+//
+// One CTA per tile of TX x TY x TZ cells.  The block handed to ent_step is the one ent_sort produced, so the
+// particles of a tile are one contiguous range of the SoA arrays (tile-major key, ent.h).
+//   * E,B: the tile's box of the six padded planar arrays, [o-2, o+T+2) per dimension, lands in shared memory by
+//     TMA (cp.async.bulk.tensor, one box per component, one mbarrier);
+//   * particles: 128-bit loads/stores, four consecutive particles per thread.  Consecutive lanes are therefore
+//     four particles (~ one cell) apart: gathers of a warp hit neighbouring words, deposits of a warp hit
+//     different words;
+//   * deposit: into a shared-memory tile of J covering nodes [o-2, o+T+3), then ONE flush per CTA with the TMA
+//     reduce-add (cp.reduce.async.bulk.tensor .add.f32) into the un-wrapped padded J arrays;
+//   * a particle whose cell has drifted more than one cell out of the tile since the sort (or whose deposit could
+//     leave the padded array) takes the global path (stray_step): global gathers, global atomics.
+// Arithmetic per particle is the same as ent_particle.cuh (same Boris, same split_offset, same segment weights); a
+// particle that crosses no face deposits its straight move as one segment (the two half segments of P:575 are
+// collinear then, and the weights (1-W_a)(1-W_b) + D_a D_b/12 are the exact line integral, so the sum is identical).
 #pragma once
+#include <cuda.h>
 #include "ent_kernels.cuh"
 
 namespace ent {
 
-struct TiledState { size_t scratch = 0; };
+// ---------------------------------------------------------------------------------------------------------
+// PTX wrappers: mbarrier + TMA (cp.async.bulk.tensor), sm_90+/sm_100a
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!ok);
+}
+template <int D>
+__device__ __forceinline__ void tma_load_box(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2) {
+    if (D == 3)
+        asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                     ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+    else
+        asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                     ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
+}
+template <int D>
+__device__ __forceinline__ void tma_reduce_add_box(const CUtensorMap *map, const void *src, int c0, int c1, int c2) {
+    if (D == 3)
+        asm volatile("cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4}], [%1];"
+                     ::"l"(map), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+    else
+        asm volatile("cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3}], [%1];"
+                     ::"l"(map), "r"(smem_u32(src)), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+
+// ---------------------------------------------------------------------------------------------------------
+// geometry of a tile in shared memory (compile time)
+// ---------------------------------------------------------------------------------------------------------
+template <int D, int TX, int TY, int TZ>
+struct TileGeom {
+    static constexpr int FX = TX + 4, FY = TY + 4, FZ = (D == 3) ? TZ + 4 : 1;                 // E,B box: cells [o-2, o+T+2)
+    static constexpr int JX = ((TX + 5 + 3) / 4) * 4, JY = TY + 5, JZ = (D == 3) ? TZ + 5 : 1; // J box: nodes [o-2, o+T+3), x padded to 16 B
+    static constexpr int FN = FX * FY * FZ, JN = JX * JY * JZ;
+    static constexpr int FNP = ((FN + 31) / 32) * 32, JNP = ((JN + 31) / 32) * 32;              // 128-byte aligned component slabs
+    static constexpr int SMEM_BYTES = (6 * FNP + 3 * JNP) * 4;
+    static constexpr int TCELLS = TX * TY * TZ;
+};
+
+struct TileMaps { CUtensorMap F[6]; CUtensorMap J[3]; };
+
+struct FastDiv {                  // n / d for 0 <= n < 2^31, d >= 1
+    uint32_t mul, shr, d;
+    __device__ __forceinline__ int div(int n) const { return d == 1 ? n : (int)(__umulhi((uint32_t)n, mul) >> shr); }
+};
+inline FastDiv make_fastdiv(uint32_t d) {
+    FastDiv f{0, 0, d};
+    if (d <= 1) return f;
+    uint32_t lg = 0; while ((1ull << lg) < d) ++lg;
+    uint32_t p = 31 + lg;
+    f.mul = (uint32_t)(((1ull << p) + d - 1) / d);
+    f.shr = p - 32;
+    return f;
+}
+
+struct TiledArgs {
+    GridDev g;
+    FieldPtrs F;
+    CurrentPtrs J;
+    PartPtrs P;
+    const int32_t *key_off;       // tile offsets: tile t owns particles [key_off[t], key_off[t+1]) (ent_sort)
+    long long n;
+    float eps, dt, q, inv_dt;
+    float cdt[3];                 // dt / dx_d
+    unsigned long long *counters; // [0] bad moves, [1] strays
+    FastDiv divN0, divN01;
+};
+
+// the global path for one particle (same code as step_untiled_kernel); kept out of line so that the tile loop stays lean
+template <int D>
+__device__ __noinline__ void stray_step(const TiledArgs &A, long long p) {
+    const GridDev &g = A.g;
+    int i[3], i0[3], di[3]; float d[3] = {0.f, 0.f, 0.f}, a[3], u[3], phi = 0.f;
+    unpack_cell<D>(g, A.P.cell[p], i);
+#pragma unroll
+    for (int k = 0; k < D; ++k) d[k] = A.P.d[k][p];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { u[k] = A.P.u[k][p]; a[k] = d[k]; i0[k] = i[k]; }
+    GlobalFieldLoader ld{A.F.c};
+    bool alive = true;
+    push_particle<D, ENT_CART>(g, ld, i, d, phi, u, A.eps, A.dt, di, alive);
+    A.P.cell[p] = pack_cell<D>(g, i);
+#pragma unroll
+    for (int k = 0; k < D; ++k) A.P.d[k][p] = d[k];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) A.P.u[k][p] = u[k];
+    atomicAdd(A.counters + 1, 1ULL);
+    if (!alive) { A.P.tag[p] = 0; return; }
+    bool bad = false;
+#pragma unroll
+    for (int k = 0; k < D; ++k) bad |= (di[k] < -1 || di[k] > 1);
+    if (bad) { atomicAdd(A.counters + 0, 1ULL); return; }
+    GlobalAcc acc{A.J.c};
+    deposit_particle<D, ENT_CART>(g, acc, i0, a, di, d, 0.f, 0.f, u, A.q * A.P.w[p], A.inv_dt);
+}
+
+constexpr int TILED_TPB = 256;
+
+template <int D, int TX, int TY, int TZ>
+__global__ void __launch_bounds__(TILED_TPB, 2)
+step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ TiledArgs A) {
+    using G = TileGeom<D, TX, TY, TZ>;
+    extern __shared__ __align__(128) float smem[];
+    float *sF = smem;                     // [6][FNP]
+    float *sJ = smem + 6 * G::FNP;        // [3][JNP]
+    __shared__ uint64_t bar;
+    const GridDev &g = A.g;
+    const int tid = threadIdx.x;
+
+    // tile origin (active cell coordinates)
+    int tile = blockIdx.x;
+    int t0 = tile % g.nt[0], t12 = tile / g.nt[0];
+    int t1 = (D == 3) ? t12 % g.nt[1] : t12, t2 = (D == 3) ? t12 / g.nt[1] : 0;
+    const int o0 = t0 * TX, o1 = t1 * TY, o2 = t2 * TZ;
+
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        fence_mbar_init();
+        mbar_expect_tx(&bar, 6u * G::FN * 4u);
+#pragma unroll
+        for (int c = 0; c < 6; ++c) tma_load_box<D>(sF + c * G::FNP, &maps.F[c], &bar, o0, o1, o2);   // padded coords of active o-2
+    }
+    for (int k = tid; k < 3 * G::JNP; k += TILED_TPB) sJ[k] = 0.f;
+    __syncthreads();
+
+    const long long p0 = A.key_off[tile], p1 = A.key_off[tile + 1];
+    const long long G0 = p0 >> 2, G1 = (p1 + 3) >> 2;
+    const float sx = g.dx[0], sy = g.dx[1], sz = g.dx[2];
+    bool waited = false;
+
+    for (long long grp = G0 + tid; grp < G1; grp += TILED_TPB) {
+        const long long pb = grp * 4;
+        const bool full = pb >= p0 && pb + 4 <= p1;
+        int4 vc; float4 vd0, vd1, vd2, vu0, vu1, vu2, vw;
+        vd2 = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (pb + 4 <= A.n) {
+            vc = *reinterpret_cast<const int4 *>(A.P.cell + pb);
+            vd0 = *reinterpret_cast<const float4 *>(A.P.d[0] + pb);
+            vd1 = *reinterpret_cast<const float4 *>(A.P.d[1] + pb);
+            if (D == 3) vd2 = *reinterpret_cast<const float4 *>(A.P.d[2] + pb);
+            vu0 = *reinterpret_cast<const float4 *>(A.P.u[0] + pb);
+            vu1 = *reinterpret_cast<const float4 *>(A.P.u[1] + pb);
+            vu2 = *reinterpret_cast<const float4 *>(A.P.u[2] + pb);
+            vw = *reinterpret_cast<const float4 *>(A.P.w + pb);
+        } else {
+            int *c = &vc.x; float *d0 = &vd0.x, *d1 = &vd1.x, *d2 = &vd2.x, *u0 = &vu0.x, *u1 = &vu1.x, *u2 = &vu2.x, *w = &vw.x;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                bool in = pb + k < A.n;
+                c[k] = in ? A.P.cell[pb + k] : 0;
+                d0[k] = in ? A.P.d[0][pb + k] : 0.f; d1[k] = in ? A.P.d[1][pb + k] : 0.f;
+                d2[k] = (D == 3 && in) ? A.P.d[2][pb + k] : 0.f;
+                u0[k] = in ? A.P.u[0][pb + k] : 0.f; u1[k] = in ? A.P.u[1][pb + k] : 0.f; u2[k] = in ? A.P.u[2][pb + k] : 0.f;
+                w[k] = in ? A.P.w[pb + k] : 0.f;
+            }
+        }
+        unsigned valid = 0, tagv = 0xf;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) valid |= (pb + k >= p0 && pb + k < p1) ? (1u << k) : 0u;
+        if (A.P.tag) {
+            tagv = 0;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) if ((valid >> k) & 1u) tagv |= A.P.tag[pb + k] ? (1u << k) : 0u;
+        }
+        unsigned store = 0, died = 0;         // particles whose record this thread writes back / that left through ABSORB
+        if (!waited) { mbar_wait(&bar, 0); waited = true; }
+
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            // component k of every vector (the unrolled loop turns these into plain register names)
+            const int cell = (&vc.x)[k];
+            float d[3] = { (&vd0.x)[k], (&vd1.x)[k], (&vd2.x)[k] };
+            float u[3] = { (&vu0.x)[k], (&vu1.x)[k], (&vu2.x)[k] };
+            const float wgt = (&vw.x)[k];
+            if (!(((valid & tagv) >> k) & 1u)) continue;                       // not ours, or dead (left untouched)
+            // ---- where is the cell relative to the tile box?  b = cell index in box coordinates (box origin = o-2)
+            int i[3];
+            if (D == 2) { i[1] = A.divN0.div(cell); i[0] = cell - i[1] * g.N[0]; i[2] = 0; }
+            else { i[2] = A.divN01.div(cell); int r = cell - i[2] * (g.N[0] * g.N[1]); i[1] = A.divN0.div(r); i[0] = r - i[1] * g.N[0]; }
+            int b[3] = { i[0] - o0 + 2, i[1] - o1 + 2, (D == 3) ? i[2] - o2 + 2 : 0 };
+            const int TT[3] = { TX, TY, TZ }, OO[3] = { o0, o1, o2 };
+            bool local = true;
+#pragma unroll
+            for (int a = 0; a < D; ++a) {
+                if (g.bc[a] == ENT_PERIODIC) { if (b[a] < 1) b[a] += g.N[a]; else if (b[a] > g.N[a]) b[a] -= g.N[a]; }
+                // inside the box with one cell of margin, and the un-wrapped cell o-2+b <= N-1 so that the deposit of a
+                // +1 crossing (nodes up to cell+2) stays inside the padded array
+                local &= (b[a] >= 1) & (b[a] < TT[a] + 3) & (OO[a] - 2 + b[a] <= g.N[a] - 1);
+            }
+            if (!local) { stray_step<D>(A, pb + k); continue; }
+            store |= 1u << k;
+            // ---- S1 gather from the shared-memory box (same stencil as ent_dev.cuh gather)
+            float EBv[6];
+            {
+                int xs[2], ys[2], zs[2]; float fx[2], fy[2], fz[2];              // [0] node-centred, [1] half-shifted
+                { bool lo = d[0] < 0.5f; xs[0] = b[0]; xs[1] = lo ? b[0] - 1 : b[0]; fx[0] = d[0]; fx[1] = lo ? d[0] + 0.5f : d[0] - 0.5f; }
+                { bool lo = d[1] < 0.5f; ys[0] = b[1] * G::FX; ys[1] = lo ? ys[0] - G::FX : ys[0]; fy[0] = d[1]; fy[1] = lo ? d[1] + 0.5f : d[1] - 0.5f; }
+                if (D == 3) { bool lo = d[2] < 0.5f; zs[0] = b[2] * (G::FX * G::FY); zs[1] = lo ? zs[0] - G::FX * G::FY : zs[0]; fz[0] = d[2]; fz[1] = lo ? d[2] + 0.5f : d[2] - 0.5f; }
+                else { zs[0] = zs[1] = 0; fz[0] = fz[1] = 0.f; }
+                const int ST[6][3] = { {1,0,0}, {0,1,0}, {0,0,1}, {0,1,1}, {1,0,1}, {1,1,0} };
+#pragma unroll
+                for (int c = 0; c < 6; ++c) {
+                    const float *Fc = sF + c * G::FNP + (xs[ST[c][0]] + ys[ST[c][1]] + zs[ST[c][2]]);
+                    const float f0 = fx[ST[c][0]], f1 = fy[ST[c][1]];
+                    float v00 = Fc[0], v10 = Fc[1], v01 = Fc[G::FX], v11 = Fc[G::FX + 1];
+                    float l0 = v00 + f0 * (v10 - v00), l1 = v01 + f0 * (v11 - v01);
+                    float lo = l0 + f1 * (l1 - l0);
+                    if (D == 3) {
+                        const float f2 = fz[ST[c][2]];
+                        const float *Fh = Fc + G::FX * G::FY;
+                        float w00 = Fh[0], w10 = Fh[1], w01 = Fh[G::FX], w11 = Fh[G::FX + 1];
+                        float h0 = w00 + f0 * (w10 - w00), h1 = w01 + f0 * (w11 - w01);
+                        float hi = h0 + f1 * (h1 - h0);
+                        lo = lo + f2 * (hi - lo);
+                    }
+                    EBv[c] = lo;
+                }
+            }
+            // ---- S2 tetrad (A^hat = sqrt(h_ii) A^i), S3 Boris (Eq. 3), S4-S5 move + crossing
+            float E[3] = { sx * EBv[0], sy * EBv[1], sz * EBv[2] }, B[3] = { sx * EBv[3], sy * EBv[4], sz * EBv[5] };
+            boris(u, E, B, A.eps);
+            const float ig = inv_gamma(u);
+            const float a0[3] = { d[0], d[1], d[2] };
+            int di[3] = {0, 0, 0};
+            bool alive = true;
+#pragma unroll
+            for (int a = 0; a < D; ++a) {
+                float x = d[a] + (u[a] * ig) * A.cdt[a];
+                split_offset(x, di[a], d[a]);
+                int in = i[a] + di[a];
+                if (g.bc[a] == ENT_PERIODIC) { if (in < 0) in += g.N[a]; if (in >= g.N[a]) in -= g.N[a]; }
+                else { if (in < 0) { alive = false; in = 0; } if (in >= g.N[a]) { alive = false; in = g.N[a] - 1; } }
+                i[a] = in;
+            }
+            (&vc.x)[k] = (D == 2) ? i[0] + g.N[0] * i[1] : i[0] + g.N[0] * (i[1] + g.N[1] * i[2]);
+            (&vd0.x)[k] = d[0]; (&vd1.x)[k] = d[1]; if (D == 3) (&vd2.x)[k] = d[2];
+            (&vu0.x)[k] = u[0]; (&vu1.x)[k] = u[1]; (&vu2.x)[k] = u[2];
+            if (!alive) { died |= 1u << k; continue; }
+            bool bad = false;
+#pragma unroll
+            for (int a = 0; a < D; ++a) bad |= (di[a] < -1) | (di[a] > 1);
+            if (bad) { atomicAdd(A.counters + 0, 1ULL); continue; }
+            // ---- S7 deposit into the shared-memory J tile (Eq. 6); node (b) of the box = element b of the J tile
+            {
+                const float qw = A.q * wgt, Q = qw * A.inv_dt;
+                // 3D: one straight segment unless a face is crossed.  2D: always the two segments of P:575, because the
+                // out-of-plane weights (bilinear, G8) of two half segments do not sum to those of the whole one
+                const bool cross = (D == 2) || (di[0] | di[1] | di[2]) != 0;
+                float s[3], e[3], r[3];
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    if (a < D) {
+                        float bn = (float)di[a] + d[a];                          // new position in the old cell's frame
+                        r[a] = di[a] == 0 ? (cross ? 0.5f * (a0[a] + bn) : bn) : (di[a] > 0 ? 1.0f : 0.0f);
+                        s[a] = a0[a]; e[a] = r[a];
+                    } else { r[a] = s[a] = e[a] = 0.f; }
+                }
+                int base = b[0] + G::JX * (b[1] + G::JY * b[2]);
+                const int dbase = di[0] + G::JX * (di[1] + G::JY * di[2]);
+                float hv = 0.f;
+                if (D == 2) hv = 0.5f * qw * (u[2] * ig);       // out-of-plane rate per segment (G8), h33 = 1
+                const int nseg = cross ? 2 : 1;
+#pragma unroll 1
+                for (int seg = 0; seg < nseg; ++seg) {
+                    float Dv[3], W[3];
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) { Dv[a] = e[a] - s[a]; W[a] = 0.5f * (e[a] + s[a]); }
+                    if (D == 3) {
+                        const int st[3] = { 1, G::JX, G::JX * G::JY };
+#pragma unroll
+                        for (int comp = 0; comp < 3; ++comp) {
+                            const int a = (comp + 1) % 3, bb = (comp + 2) % 3;
+                            float c = Dv[a] * Dv[bb] * (1.0f / 12.0f);
+                            float QD = Q * Dv[comp];
+                            float w11 = W[a] * W[bb] + c, w10 = W[a] - w11, w01 = W[bb] - w11, w00 = 1.0f - W[a] - w01;
+                            float *Jc = sJ + comp * G::JNP + base;
+                            atomicAdd(Jc, QD * w00);
+                            atomicAdd(Jc + st[a], QD * w10);
+                            atomicAdd(Jc + st[bb], QD * w01);
+                            atomicAdd(Jc + st[a] + st[bb], QD * w11);
+                        }
+                    } else {
+                        float q0 = Q * Dv[0], q1 = Q * Dv[1];
+                        float *J0 = sJ + base, *J1 = sJ + G::JNP + base, *J2 = sJ + 2 * G::JNP + base;
+                        atomicAdd(J0, q0 * (1.0f - W[1])); atomicAdd(J0 + G::JX, q0 * W[1]);
+                        atomicAdd(J1, q1 * (1.0f - W[0])); atomicAdd(J1 + 1, q1 * W[0]);
+                        float h1 = hv * W[1], h0 = hv - h1;
+                        atomicAdd(J2, h0 * (1.0f - W[0])); atomicAdd(J2 + 1, h0 * W[0]);
+                        atomicAdd(J2 + G::JX, h1 * (1.0f - W[0])); atomicAdd(J2 + G::JX + 1, h1 * W[0]);
+                    }
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) { s[a] = r[a] - (float)di[a]; e[a] = d[a]; }
+                    base += dbase;
+                }
+            }
+        }
+        // ---- write back (cell, offsets, momentum; the weight is read-only)
+        if (full && store == 0xf) {
+            *reinterpret_cast<int4 *>(A.P.cell + pb) = vc;
+            *reinterpret_cast<float4 *>(A.P.d[0] + pb) = vd0;
+            *reinterpret_cast<float4 *>(A.P.d[1] + pb) = vd1;
+            if (D == 3) *reinterpret_cast<float4 *>(A.P.d[2] + pb) = vd2;
+            *reinterpret_cast<float4 *>(A.P.u[0] + pb) = vu0;
+            *reinterpret_cast<float4 *>(A.P.u[1] + pb) = vu1;
+            *reinterpret_cast<float4 *>(A.P.u[2] + pb) = vu2;
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                if (!((store >> k) & 1u)) continue;
+                A.P.cell[pb + k] = (&vc.x)[k];
+                A.P.d[0][pb + k] = (&vd0.x)[k]; A.P.d[1][pb + k] = (&vd1.x)[k];
+                if (D == 3) A.P.d[2][pb + k] = (&vd2.x)[k];
+                A.P.u[0][pb + k] = (&vu0.x)[k]; A.P.u[1][pb + k] = (&vu1.x)[k]; A.P.u[2][pb + k] = (&vu2.x)[k];
+            }
+        }
+        if (died) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) if ((died >> k) & 1u) A.P.tag[pb + k] = 0;
+        }
+    }
+    if (!waited) mbar_wait(&bar, 0);          // never leave with a TMA load still in flight into this CTA's shared memory
+    // ---- S8 flush: one TMA reduce-add per component into the un-wrapped padded J (ghost fold = ent_fold_current)
+    fence_proxy_async_smem();
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) tma_reduce_add_box<D>(&maps.J[c], sJ + c * G::JNP, o0, o1, o2);
+        tma_commit();
+        tma_wait_read0();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct TiledState {
+    size_t scratch = 0;
+    EncodeTiledFn encode = nullptr;
+    bool tried_encode = false;
+    int shape = -1;                         // index into the instantiated tile shapes, -1 = none fits
+    const void *ptrF[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    const void *ptrJ[3] = {nullptr, nullptr, nullptr};
+    TileMaps maps;
+    bool attr_set[8] = {false, false, false, false, false, false, false, false};
+};
 
 inline void tiled_release(TiledState &) {}
 inline size_t tiled_scratch_bytes(const TiledState &t) { return t.scratch; }
-inline int tiled_set_grid(TiledState &, const GridDev &, char *, size_t) { return ENT_OK; }
-inline bool tiled_supported(const TiledState &, const GridDev &) { return false; }
-inline int tiled_step(TiledState &, const GridDev &, cudaStream_t, FieldPtrs, PartPtrs, CurrentPtrs, long long, const int32_t *,
-                      float, float, float, float, unsigned long long *, long long *, char *, size_t) { return ENT_EUNSUPPORTED; }
+
+// instantiated tile shapes: index -> (D, TX, TY, TZ)
+#define ENT_TILE_SHAPES(X) X(0, 3, 8, 8, 8) X(1, 3, 16, 8, 4) X(2, 3, 32, 4, 4) X(3, 3, 16, 8, 8) X(4, 2, 16, 16, 1) X(5, 2, 32, 8, 1)
+
+inline int tiled_find_shape(const GridDev &g) {
+#define X(IDX, DD, A, B, C) if (g.D == DD && g.T[0] == A && g.T[1] == B && g.T[2] == C) return IDX;
+    ENT_TILE_SHAPES(X)
+#undef X
+    return -1;
+}
+
+inline int tiled_set_grid(TiledState &t, const GridDev &g, char *, size_t) {
+    t.shape = -1;
+    for (int c = 0; c < 6; ++c) t.ptrF[c] = nullptr;
+    for (int c = 0; c < 3; ++c) t.ptrJ[c] = nullptr;
+    if (!t.tried_encode) {
+        t.tried_encode = true;
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess && qres == cudaDriverEntryPointSuccess)
+            t.encode = (EncodeTiledFn)fn;
+        else cudaGetLastError();
+    }
+    // TMA needs 16-byte global strides: padded row length (N0 + 4) * 4 bytes, i.e. N0 % 4 == 0.  Cartesian grids only.
+    if (g.kind != ENT_CART || !t.encode || (g.P[0] % 4) != 0) return ENT_OK;
+    t.shape = tiled_find_shape(g);
+    return ENT_OK;
+}
+inline bool tiled_supported(const TiledState &t, const GridDev &) { return t.shape >= 0; }
+
+template <int D, int TX, int TY, int TZ>
+inline int tiled_encode(TiledState &t, const GridDev &g, const FieldPtrs &F, const CurrentPtrs &J, char *err, size_t errn) {
+    using G = TileGeom<D, TX, TY, TZ>;
+    cuuint64_t dims[3] = { (cuuint64_t)g.P[0], (cuuint64_t)g.P[1], (cuuint64_t)g.P[2] };
+    cuuint64_t strides[2] = { (cuuint64_t)g.P[0] * 4, (cuuint64_t)g.P[0] * g.P[1] * 4 };
+    cuuint32_t estr[3] = { 1, 1, 1 };
+    for (int c = 0; c < 6; ++c) {
+        if (t.ptrF[c] == F.c[c]) continue;
+        cuuint32_t box[3] = { G::FX, G::FY, G::FZ };
+        CUresult r = t.encode(&t.maps.F[c], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, D, (void *)F.c[c], dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { snprintf(err, errn, "cuTensorMapEncodeTiled(field %d) failed: %d", c, (int)r); return ENT_ECUDA; }
+        t.ptrF[c] = F.c[c];
+    }
+    for (int c = 0; c < 3; ++c) {
+        if (t.ptrJ[c] == J.c[c]) continue;
+        cuuint32_t box[3] = { G::JX, G::JY, G::JZ };
+        CUresult r = t.encode(&t.maps.J[c], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, D, (void *)J.c[c], dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { snprintf(err, errn, "cuTensorMapEncodeTiled(current %d) failed: %d", c, (int)r); return ENT_ECUDA; }
+        t.ptrJ[c] = J.c[c];
+    }
+    return ENT_OK;
+}
+
+template <int IDX, int D, int TX, int TY, int TZ>
+inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, char *err, size_t errn) {
+    using G = TileGeom<D, TX, TY, TZ>;
+    int rc = tiled_encode<D, TX, TY, TZ>(t, A.g, A.F, A.J, err, errn);
+    if (rc) return rc;
+    auto kern = step_tiled_kernel<D, TX, TY, TZ>;
+    if (!t.attr_set[IDX]) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM_BYTES);
+        if (e != cudaSuccess) { snprintf(err, errn, "cudaFuncSetAttribute(smem %d) failed: %s", G::SMEM_BYTES, cudaGetErrorString(e)); return ENT_ECUDA; }
+        t.attr_set[IDX] = true;
+    }
+    const int ntiles = A.g.nt[0] * A.g.nt[1] * A.g.nt[2];
+    kern<<<ntiles, TILED_TPB, G::SMEM_BYTES, stream>>>(t.maps, A);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { snprintf(err, errn, "launch of step_tiled_kernel failed: %s", cudaGetErrorString(e)); return ENT_ECUDA; }
+    return ENT_OK;
+}
+
+inline int tiled_step(TiledState &t, const GridDev &g, cudaStream_t stream, FieldPtrs F, PartPtrs P, CurrentPtrs J, long long n,
+                      const int32_t *key_off, float eps, float dt, float q, float inv_dt, unsigned long long *counters,
+                      long long *launches, char *err, size_t errn) {
+    TiledArgs A;
+    A.g = g; A.F = F; A.J = J; A.P = P; A.key_off = key_off; A.n = n;
+    A.eps = eps; A.dt = dt; A.q = q; A.inv_dt = inv_dt; A.counters = counters;
+    for (int a = 0; a < 3; ++a) A.cdt[a] = dt * g.inv_dx[a];
+    A.divN0 = make_fastdiv((uint32_t)g.N[0]);
+    A.divN01 = make_fastdiv((uint32_t)(g.N[0] * g.N[1]));
+    int rc = ENT_EUNSUPPORTED;
+    switch (t.shape) {
+#define X(IDX, DD, A_, B_, C_) case IDX: rc = tiled_launch<IDX, DD, A_, B_, C_>(t, A, stream, err, errn); break;
+        ENT_TILE_SHAPES(X)
+#undef X
+        default: snprintf(err, errn, "no tiled kernel for this tile shape"); break;
+    }
+    if (rc == ENT_OK) *launches += 1;
+    return rc;
+}
 
 }  // namespace ent

@@ -80,6 +80,8 @@ def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True
                 worstC = max(worstC, c)
         stats = P.compare_particles(g, pe, po, order, steps=steps)
         assert bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES) == 0
+        stats["tiled"] = bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED)
+        stats["strays"] = bind.ent_get_stat(ctx, bind.STAT_STRAYS)
         stats.update(worstJ=worstJ, worstC=worstC)
         out[si] = stats
     return out
@@ -106,3 +108,5 @@ def test_sorted_step_auto_path_matches_oracle(env, name):
     wl = _workloads(env[1])[name]()
     stats = _run_case(env, wl, impl=0, sort_first=True)
     print(name, stats)
+    if wl.grid.kind == env[1].CART:
+        assert all(st["tiled"] == 1 for st in stats.values()), "the tiled kernel did not run on a sorted Cartesian block"
