@@ -56,7 +56,7 @@ def lib():
     """Loads libent.so (building it if the sources are newer).  Raises if it cannot be built or loaded."""
     global _lib
     if _lib is None:
-        path = _build.build()
+        path = os.environ.get("ENT_LIBENT") or _build.build()      # ENT_LIBENT: load a specific build (A/B timing of variants)
         if not os.path.exists(path):
             raise RuntimeError("libent.so is missing: the CUDA library is the product, there is no fallback")
         L = C.CDLL(path)

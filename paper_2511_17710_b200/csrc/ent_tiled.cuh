@@ -130,16 +130,59 @@ __device__ __noinline__ void stray_step(const TiledArgs &A, long long p) {
     deposit_particle<D, ENT_CART>(g, acc, i0, a, di, d, 0.f, 0.f, u, A.q * A.P.w[p], A.inv_dt);
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Shared-memory accumulation of J.  fp32 atomicAdd on shared memory is a compare-and-swap loop on sm_100a
+// (SASS: LDS + FADD + ATOMS.CAST.SPIN + branch, several passes under contention); 32-bit integer add is native
+// (ATOMS.ADD).  The J tile is therefore accumulated in fixed point: value * 2^k rounded to nearest, k chosen per tile
+// from the largest |q w|/dt of the tile's particles so that one contribution uses at most 24 bits.  Integer sums are
+// exact and order-independent.  A signed wrap of the 32-bit accumulator (|J_node| * 2^k >= 2^31: hundreds of
+// particles' worth of current on one node) is detected from the value the atomic returns and carried straight into
+// the global array as +-2^32 / 2^k, so the sum stays exact for any input.
+// ---------------------------------------------------------------------------------------------------------
+struct CarryCtx { float *const *J; long long gbase; int P0, P01; float unit; int JX, JY, JNP; };
+
+__device__ __noinline__ void carry_fix(const CarryCtx &c, int comp, int off, int positive) {
+    int bx = off % c.JX, r = off / c.JX, by = r % c.JY, bz = r / c.JY;
+    long long idx = c.gbase + bx + (long long)c.P0 * by + (long long)c.P01 * bz;
+    atomicAdd(c.J[comp] + idx, positive ? c.unit : -c.unit);
+}
+__device__ __forceinline__ void acc_fixed(int *sJ, const CarryCtx &cc, int comp, int off, float scaled) {
+    int v = __float2int_rn(scaled);
+    int old = atomicAdd(sJ + comp * cc.JNP + off, v);
+    int nw = old + v;
+    if (((old ^ nw) & (v ^ nw)) < 0) carry_fix(cc, comp, off, v > 0);
+}
+// four contributions of one component: all four atomics are issued before the first returned value is looked at, and
+// one test covers the four carries
+__device__ __forceinline__ void acc_fixed4(int *sJ, const CarryCtx &cc, int comp, int o0, int o1, int o2, int o3,
+                                           float s0, float s1, float s2, float s3) {
+    int *Jc = sJ + comp * cc.JNP;
+    int v0 = __float2int_rn(s0), v1 = __float2int_rn(s1), v2 = __float2int_rn(s2), v3 = __float2int_rn(s3);
+    int a0 = atomicAdd(Jc + o0, v0), a1 = atomicAdd(Jc + o1, v1), a2 = atomicAdd(Jc + o2, v2), a3 = atomicAdd(Jc + o3, v3);
+    int n0 = a0 + v0, n1 = a1 + v1, n2 = a2 + v2, n3 = a3 + v3;
+    int t0 = (a0 ^ n0) & (v0 ^ n0), t1 = (a1 ^ n1) & (v1 ^ n1), t2 = (a2 ^ n2) & (v2 ^ n2), t3 = (a3 ^ n3) & (v3 ^ n3);
+    if ((t0 | t1 | t2 | t3) < 0) {
+        if (t0 < 0) carry_fix(cc, comp, o0, v0 > 0);
+        if (t1 < 0) carry_fix(cc, comp, o1, v1 > 0);
+        if (t2 < 0) carry_fix(cc, comp, o2, v2 > 0);
+        if (t3 < 0) carry_fix(cc, comp, o3, v3 > 0);
+    }
+}
+#ifndef ENT_TILED_MINB
+#define ENT_TILED_MINB 2
+#endif
+
 constexpr int TILED_TPB = 256;
 
-template <int D, int TX, int TY, int TZ>
-__global__ void __launch_bounds__(TILED_TPB, 2)
+template <int D, int TX, int TY, int TZ, bool ALLPER>     // ALLPER: every dimension periodic (no ABSORB bookkeeping)
+__global__ void __launch_bounds__(TILED_TPB, ENT_TILED_MINB)
 step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ TiledArgs A) {
     using G = TileGeom<D, TX, TY, TZ>;
     extern __shared__ __align__(128) float smem[];
     float *sF = smem;                     // [6][FNP]
-    float *sJ = smem + 6 * G::FNP;        // [3][JNP]
+    int *sJ = reinterpret_cast<int *>(smem + 6 * G::FNP);        // [3][JNP], fixed point (see acc_fixed)
     __shared__ uint64_t bar;
+    __shared__ float s_wmax[TILED_TPB / 32];
     const GridDev &g = A.g;
     const int tid = threadIdx.x;
 
@@ -156,13 +199,37 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
 #pragma unroll
         for (int c = 0; c < 6; ++c) tma_load_box<D>(sF + c * G::FNP, &maps.F[c], &bar, o0, o1, o2);   // padded coords of active o-2
     }
-    for (int k = tid; k < 3 * G::JNP; k += TILED_TPB) sJ[k] = 0.f;
-    __syncthreads();
+    for (int k = tid; k < 3 * G::JNP; k += TILED_TPB) sJ[k] = 0;
+
 
     const long long p0 = A.key_off[tile], p1 = A.key_off[tile + 1];
     const long long G0 = p0 >> 2, G1 = (p1 + 3) >> 2;
     const float sx = g.dx[0], sy = g.dx[1], sz = g.dx[2];
     bool waited = false;
+    // fixed-point scale of this tile: 2^k with 2^k * (13/12) |q| wmax / dt < 2^23 (wmax over the tile's particles)
+    float Sc, invSc;
+    {
+        float wm = 0.f;
+        for (long long p = p0 + tid; p < p1; p += TILED_TPB) wm = fmaxf(wm, fabsf(A.P.w[p]));
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) wm = fmaxf(wm, __shfl_xor_sync(0xffffffffu, wm, o));
+        if ((tid & 31) == 0) s_wmax[tid >> 5] = wm;
+        __syncthreads();                       // also: sJ zeroed, mbarrier initialised
+#pragma unroll
+        for (int k = 0; k < TILED_TPB / 32; ++k) wm = fmaxf(wm, s_wmax[k]);
+        // largest contribution: |q| wmax / dt * |D| * weight, |D| <= 1, weight <= 13/12 (2D: J^3 = q w v^3 has no 1/dt).
+        // It gets `bits` bits; fewer in a dense tile, so that ~8x the mean nodal current still fits the 32-bit accumulator.
+        float qmax = fabsf(A.q) * wm * ((D == 2) ? fmaxf(A.inv_dt, 0.5f) : A.inv_dt) * 1.0834f;
+        float dens = (float)(p1 - p0) / (float)G::TCELLS;
+        float top = fminf(16777000.0f, 2.6e8f / fmaxf(dens, 1.0f));
+        Sc = (qmax > 0.f && qmax < 1e37f) ? top / qmax : 0.f;
+        if (!(Sc > 1e-30f && Sc < 1e30f)) Sc = 0.f;
+        invSc = Sc > 0.f ? 1.0f / Sc : 0.f;
+    }
+    CarryCtx cc;
+    cc.J = A.J.c; cc.P0 = g.P[0]; cc.P01 = g.P[0] * g.P[1]; cc.unit = 4294967296.0f * invSc;
+    cc.JX = G::JX; cc.JY = G::JY; cc.JNP = G::JNP;
+    cc.gbase = (long long)o0 + (long long)g.P[0] * o1 + (D == 3 ? (long long)g.P[0] * g.P[1] * o2 : 0);
 
     for (long long grp = G0 + tid; grp < G1; grp += TILED_TPB) {
         const long long pb = grp * 4;
@@ -218,7 +285,9 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
             bool local = true;
 #pragma unroll
             for (int a = 0; a < D; ++a) {
-                if (g.bc[a] == ENT_PERIODIC) { if (b[a] < 1) b[a] += g.N[a]; else if (b[a] > g.N[a]) b[a] -= g.N[a]; }
+                const int wrapN = (ALLPER || g.bc[a] == ENT_PERIODIC) ? g.N[a] : 0;
+                b[a] += (b[a] < 1) ? wrapN : 0;
+                b[a] -= (b[a] > g.N[a]) ? wrapN : 0;
                 // inside the box with one cell of margin, and the un-wrapped cell o-2+b <= N-1 so that the deposit of a
                 // +1 crossing (nodes up to cell+2) stays inside the padded array
                 local &= (b[a] >= 1) & (b[a] < TT[a] + 3) & (OO[a] - 2 + b[a] <= g.N[a] - 1);
@@ -264,8 +333,10 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
                 float x = d[a] + (u[a] * ig) * A.cdt[a];
                 split_offset(x, di[a], d[a]);
                 int in = i[a] + di[a];
-                if (g.bc[a] == ENT_PERIODIC) { if (in < 0) in += g.N[a]; if (in >= g.N[a]) in -= g.N[a]; }
-                else { if (in < 0) { alive = false; in = 0; } if (in >= g.N[a]) { alive = false; in = g.N[a] - 1; } }
+                const int wrapN = (ALLPER || g.bc[a] == ENT_PERIODIC) ? g.N[a] : 0;
+                in += (in < 0) ? wrapN : 0;
+                in -= (in >= g.N[a]) ? wrapN : 0;
+                if (!ALLPER) { if (in < 0) { alive = false; in = 0; } if (in >= g.N[a]) { alive = false; in = g.N[a] - 1; } }
                 i[a] = in;
             }
             (&vc.x)[k] = (D == 2) ? i[0] + g.N[0] * i[1] : i[0] + g.N[0] * (i[1] + g.N[1] * i[2]);
@@ -278,7 +349,7 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
             if (bad) { atomicAdd(A.counters + 0, 1ULL); continue; }
             // ---- S7 deposit into the shared-memory J tile (Eq. 6); node (b) of the box = element b of the J tile
             {
-                const float qw = A.q * wgt, Q = qw * A.inv_dt;
+                const float qw = A.q * wgt, Q = qw * A.inv_dt * Sc;                 // Q in fixed-point units
                 // 3D: one straight segment unless a face is crossed.  2D: always the two segments of P:575, because the
                 // out-of-plane weights (bilinear, G8) of two half segments do not sum to those of the whole one
                 const bool cross = (D == 2) || (di[0] | di[1] | di[2]) != 0;
@@ -294,7 +365,7 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
                 int base = b[0] + G::JX * (b[1] + G::JY * b[2]);
                 const int dbase = di[0] + G::JX * (di[1] + G::JY * di[2]);
                 float hv = 0.f;
-                if (D == 2) hv = 0.5f * qw * (u[2] * ig);       // out-of-plane rate per segment (G8), h33 = 1
+                if (D == 2) hv = 0.5f * qw * Sc * (u[2] * ig);       // out-of-plane rate per segment (G8), h33 = 1
                 const int nseg = cross ? 2 : 1;
 #pragma unroll 1
                 for (int seg = 0; seg < nseg; ++seg) {
@@ -309,20 +380,16 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
                             float c = Dv[a] * Dv[bb] * (1.0f / 12.0f);
                             float QD = Q * Dv[comp];
                             float w11 = W[a] * W[bb] + c, w10 = W[a] - w11, w01 = W[bb] - w11, w00 = 1.0f - W[a] - w01;
-                            float *Jc = sJ + comp * G::JNP + base;
-                            atomicAdd(Jc, QD * w00);
-                            atomicAdd(Jc + st[a], QD * w10);
-                            atomicAdd(Jc + st[bb], QD * w01);
-                            atomicAdd(Jc + st[a] + st[bb], QD * w11);
+                            acc_fixed4(sJ, cc, comp, base, base + st[a], base + st[bb], base + st[a] + st[bb],
+                                       QD * w00, QD * w10, QD * w01, QD * w11);
                         }
                     } else {
                         float q0 = Q * Dv[0], q1 = Q * Dv[1];
-                        float *J0 = sJ + base, *J1 = sJ + G::JNP + base, *J2 = sJ + 2 * G::JNP + base;
-                        atomicAdd(J0, q0 * (1.0f - W[1])); atomicAdd(J0 + G::JX, q0 * W[1]);
-                        atomicAdd(J1, q1 * (1.0f - W[0])); atomicAdd(J1 + 1, q1 * W[0]);
+                        acc_fixed(sJ, cc, 0, base, q0 * (1.0f - W[1])); acc_fixed(sJ, cc, 0, base + G::JX, q0 * W[1]);
+                        acc_fixed(sJ, cc, 1, base, q1 * (1.0f - W[0])); acc_fixed(sJ, cc, 1, base + 1, q1 * W[0]);
                         float h1 = hv * W[1], h0 = hv - h1;
-                        atomicAdd(J2, h0 * (1.0f - W[0])); atomicAdd(J2 + 1, h0 * W[0]);
-                        atomicAdd(J2 + G::JX, h1 * (1.0f - W[0])); atomicAdd(J2 + G::JX + 1, h1 * W[0]);
+                        acc_fixed(sJ, cc, 2, base, h0 * (1.0f - W[0])); acc_fixed(sJ, cc, 2, base + 1, h0 * W[0]);
+                        acc_fixed(sJ, cc, 2, base + G::JX, h1 * (1.0f - W[0])); acc_fixed(sJ, cc, 2, base + G::JX + 1, h1 * W[0]);
                     }
 #pragma unroll
                     for (int a = 0; a < 3; ++a) { s[a] = r[a] - (float)di[a]; e[a] = d[a]; }
@@ -356,6 +423,8 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     }
     if (!waited) mbar_wait(&bar, 0);          // never leave with a TMA load still in flight into this CTA's shared memory
     // ---- S8 flush: one TMA reduce-add per component into the un-wrapped padded J (ghost fold = ent_fold_current)
+    __syncthreads();
+    for (int k = tid; k < 3 * G::JNP; k += TILED_TPB) reinterpret_cast<float *>(sJ)[k] = (float)sJ[k] * invSc;   // fixed point -> fp32, in place
     fence_proxy_async_smem();
     __syncthreads();
     if (tid == 0) {
@@ -381,7 +450,7 @@ struct TiledState {
     const void *ptrF[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     const void *ptrJ[3] = {nullptr, nullptr, nullptr};
     TileMaps maps;
-    bool attr_set[8] = {false, false, false, false, false, false, false, false};
+    bool attr_set[16] = {};
 };
 
 inline void tiled_release(TiledState &) {}
@@ -448,11 +517,14 @@ inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, 
     using G = TileGeom<D, TX, TY, TZ>;
     int rc = tiled_encode<D, TX, TY, TZ>(t, A.g, A.F, A.J, err, errn);
     if (rc) return rc;
-    auto kern = step_tiled_kernel<D, TX, TY, TZ>;
-    if (!t.attr_set[IDX]) {
+    bool allper = true;
+    for (int a = 0; a < D; ++a) allper &= A.g.bc[a] == ENT_PERIODIC;
+    auto kern = allper ? step_tiled_kernel<D, TX, TY, TZ, true> : step_tiled_kernel<D, TX, TY, TZ, false>;
+    const int slot = 2 * IDX + (allper ? 1 : 0);
+    if (!t.attr_set[slot]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM_BYTES);
         if (e != cudaSuccess) { snprintf(err, errn, "cudaFuncSetAttribute(smem %d) failed: %s", G::SMEM_BYTES, cudaGetErrorString(e)); return ENT_ECUDA; }
-        t.attr_set[IDX] = true;
+        t.attr_set[slot] = true;
     }
     const int ntiles = A.g.nt[0] * A.g.nt[1] * A.g.nt[2];
     kern<<<ntiles, TILED_TPB, G::SMEM_BYTES, stream>>>(t.maps, A);
