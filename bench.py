@@ -306,7 +306,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C4s", "C5"])
     ap.add_argument("--shrink", type=int, default=1)
-    ap.add_argument("--sort-every", type=int, default=0)
+    ap.add_argument("--sort-every", type=int, default=3, help="ent_sort every k steps inside the timed region (0 = never)")
     ap.add_argument("--step-impl", type=int, default=0, help="ENT_OPT_STEP_IMPL: 0 auto, 1 untiled, 2 two-kernel")
     ap.add_argument("--tile", default="", help="tile extents in cells, e.g. 8,8,8 (ENT_OPT_TILE_*; default: the library's)")
     ap.add_argument("--e2e-steps", type=int, default=3)

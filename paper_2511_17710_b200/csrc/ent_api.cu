@@ -33,7 +33,8 @@ struct ent_ctx {
     size_t scratch_bytes = 0;
     // the blocks ent_sort produced (most recent first): each keeps its own tile offsets so that several species
     // can stay "sorted" at the same time
-    struct SortedBlock { const int32_t *cell = nullptr; long long n = -1; int32_t *tile_off = nullptr; size_t cap = 0; unsigned long long stamp = 0; };
+    struct SortedBlock { const int32_t *cell = nullptr; long long n = -1; int32_t *tile_off = nullptr; size_t cap = 0;
+                         float *tile_wmax = nullptr; size_t wcap = 0; unsigned long long stamp = 0; };
     SortedBlock sorted[8];
     unsigned long long sort_stamp = 0;
     int last_step_tiled = 0;
@@ -98,7 +99,7 @@ extern "C" int ent_destroy(ent_ctx *ctx) {
     tiled_release(ctx->tiled);
     cudaFree(ctx->counters); cudaFree(ctx->keys); cudaFree(ctx->count); cudaFree(ctx->offsets); cudaFree(ctx->cursor);
     cudaFree(ctx->chunk); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf);
-    for (auto &b : ctx->sorted) cudaFree(b.tile_off);
+    for (auto &b : ctx->sorted) { cudaFree(b.tile_off); cudaFree(b.tile_wmax); }
     cudaGetLastError();
     delete ctx;
     return ENT_OK;
@@ -302,11 +303,11 @@ extern "C" int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, en
     if (p->n == 0) return ENT_OK;
     if (ctx->step_impl == 2) return step_two_kernel(ctx, EB, p, J, dt);
     float eps = 0.5f * (p->q / p->m) * dt;
-    const int32_t *tile_off = nullptr;
-    for (auto &b : ctx->sorted) if (b.cell == p->cell && b.n == p->n) tile_off = b.tile_off;
+    const int32_t *tile_off = nullptr; const float *tile_wmax = nullptr;
+    for (auto &b : ctx->sorted) if (b.cell == p->cell && b.n == p->n) { tile_off = b.tile_off; tile_wmax = b.tile_wmax; }
     if (ctx->step_impl == 0 && tile_off && tiled_supported(ctx->tiled, ctx->g)) {
         CK(cudaMemsetAsync(ctx->counters + 1, 0, sizeof(unsigned long long), ctx->stream));      // strays of THIS step
-        rc = tiled_step(ctx->tiled, ctx->g, ctx->stream, fp(EB), pp(p), cp(J), (long long)p->n, tile_off, eps, dt, p->q,
+        rc = tiled_step(ctx->tiled, ctx->g, ctx->stream, fp(EB), pp(p), cp(J), (long long)p->n, tile_off, tile_wmax, eps, dt, p->q,
                         1.0f / dt, ctx->counters, &ctx->launches, ctx->err, sizeof(ctx->err));
         if (rc == ENT_OK) ctx->last_step_tiled = 1;
         return rc;
@@ -370,6 +371,9 @@ extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *ou
         if ((rc = ensure(ctx, (void **)&slot->tile_off, &slot->cap, (size_t)(ntiles + 1) * 4))) return rc;
         tile_offsets_kernel<<<nblk(ntiles + 1), TPB, 0, ctx->stream>>>(ctx->offsets, g.tcells, ntiles, slot->tile_off);
         if ((rc = launch_check(ctx, "tile_offsets_kernel"))) return rc;
+        if ((rc = ensure(ctx, (void **)&slot->tile_wmax, &slot->wcap, (size_t)ntiles * 4))) return rc;
+        tile_wmax_kernel<<<(unsigned)ntiles, 128, 0, ctx->stream>>>(slot->tile_off, out->w, slot->tile_wmax);
+        if ((rc = launch_check(ctx, "tile_wmax_kernel"))) return rc;
         slot->cell = out->cell; slot->n = n; slot->stamp = ++ctx->sort_stamp;
     }
     return ENT_OK;

@@ -229,6 +229,19 @@ __global__ void tile_offsets_kernel(const int32_t *key_off, int tcells, long lon
     if (t <= ntiles) tile_off[t] = key_off[t * tcells];
 }
 
+// tile_wmax[t] = max |w| over the particles of tile t (scale of the tile's fixed-point J accumulation)
+__global__ void __launch_bounds__(128) tile_wmax_kernel(const int32_t *tile_off, const float *w, float *tile_wmax) {
+    __shared__ float red[4];
+    const long long p0 = tile_off[blockIdx.x], p1 = tile_off[blockIdx.x + 1];
+    float m = 0.f;
+    for (long long p = p0 + threadIdx.x; p < p1; p += 128) m = fmaxf(m, fabsf(w[p]));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) tile_wmax[blockIdx.x] = fmaxf(fmaxf(red[0], red[1]), fmaxf(red[2], red[3]));
+}
+
 __global__ void __launch_bounds__(TPB) sort_scatter_kernel(const int32_t *keys, int32_t *cursor, PartPtrs in, PartPtrs out,
                                                            long long n, int D, int axisym) {
     long long p = (long long)blockIdx.x * TPB + threadIdx.x;

@@ -95,6 +95,7 @@ struct TiledArgs {
     CurrentPtrs J;
     PartPtrs P;
     const int32_t *key_off;       // tile offsets: tile t owns particles [key_off[t], key_off[t+1]) (ent_sort)
+    const float *tile_wmax;       // max |w| over the particles of each tile (ent_sort)
     long long n;
     float eps, dt, q, inv_dt;
     float cdt[3];                 // dt / dx_d
@@ -174,69 +175,222 @@ __device__ __forceinline__ void acc_fixed4(int *sJ, const CarryCtx &cc, int comp
 
 constexpr int TILED_TPB = 256;
 
+// deposit of one particle through global atomics (ent_particle.cuh), out of line: used by the few particles of a tile that
+// cannot deposit into its shared-memory J tile
+template <int D>
+__device__ __noinline__ void edge_deposit(const TiledArgs &A, int i0, int i1, int i2, float a0, float a1, float a2, int di0, int di1, int di2,
+                                          float d0, float d1, float d2, float u0, float u1, float u2, float qw) {
+    const int i[3] = { i0, i1, i2 }, di[3] = { di0, di1, di2 };
+    const float a[3] = { a0, a1, a2 }, dn[3] = { d0, d1, d2 }, u[3] = { u0, u1, u2 };
+    GlobalAcc acc{A.J.c};
+    deposit_particle<D, ENT_CART>(A.g, acc, i, a, di, dn, 0.f, 0.f, u, qw, A.inv_dt);
+}
+
+// per-CTA constants of the tile loop
+template <int D>
+struct TileCtx {
+    const float *sF;      // [6][FNP] E,B box
+    int *sJ;              // [3][JNP] fixed-point J tile
+    int o[3];             // tile origin (active cell coordinates)
+    float sx[3];          // sqrt(h_ii) = cell sizes
+    float Sc;             // fixed-point scale of this tile
+    float wguard;         // weights above this deposit through the global path (contribution would not fit 2^30)
+    CarryCtx cc;
+};
+
+// One particle through sub-steps 3-8 inside a tile.  cell, d[], u[] are updated in place.
+// Returns 0: advanced (write the record back), 1: taken by the global path (already written), 2: advanced and left
+// through an ABSORB side (write back, tag = 0), 3: dead or not ours (untouched).
+template <int D, int TX, int TY, int TZ, bool ALLPER>
+__device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D> &T, long long p, int &cell, float d[3], float u[3],
+                                             float wgt) {
+    using G = TileGeom<D, TX, TY, TZ>;
+    const GridDev &g = A.g;
+    // ---- where is the cell relative to the tile box?  b = cell index in box coordinates (box origin = o-2)
+    int i[3];
+    if (D == 2) { i[1] = A.divN0.div(cell); i[0] = cell - i[1] * g.N[0]; i[2] = 0; }
+    else { i[2] = A.divN01.div(cell); int r = cell - i[2] * (g.N[0] * g.N[1]); i[1] = A.divN0.div(r); i[0] = r - i[1] * g.N[0]; }
+    const int iold[3] = { i[0], i[1], i[2] };
+    int b[3] = { i[0] - T.o[0] + 2, i[1] - T.o[1] + 2, (D == 3) ? i[2] - T.o[2] + 2 : 0 };
+    const int TT[3] = { TX, TY, TZ };
+    bool local = true, edge = false;
+#pragma unroll
+    for (int a = 0; a < D; ++a) {
+        const int wrapN = (ALLPER || g.bc[a] == ENT_PERIODIC) ? g.N[a] : 0;
+        b[a] += (b[a] < 1) ? wrapN : 0;
+        b[a] -= (b[a] > g.N[a]) ? wrapN : 0;
+        local &= (unsigned)(b[a] - 1) < (unsigned)(TT[a] + 2);           // inside the box with one cell of margin
+        // un-wrapped cell N (a particle that crossed the upper periodic face since the sort): its +1 crossing would deposit
+        // at node N+2, outside the padded array -> it gathers from the box but deposits through the global path
+        edge |= (T.o[a] - 2 + b[a] > g.N[a] - 1);
+    }
+    if (!local) { stray_step<D>(A, p); return 1; }
+    // ---- S1 gather from the shared-memory box (same stencil as ent_dev.cuh gather)
+    float EBv[6];
+    {
+        int xs[2], ys[2], zs[2]; float fx[2], fy[2], fz[2];              // [0] node-centred, [1] half-shifted
+        { bool lo = d[0] < 0.5f; xs[0] = b[0]; xs[1] = lo ? b[0] - 1 : b[0]; fx[0] = d[0]; fx[1] = lo ? d[0] + 0.5f : d[0] - 0.5f; }
+        { bool lo = d[1] < 0.5f; ys[0] = b[1] * G::FX; ys[1] = lo ? ys[0] - G::FX : ys[0]; fy[0] = d[1]; fy[1] = lo ? d[1] + 0.5f : d[1] - 0.5f; }
+        if (D == 3) { bool lo = d[2] < 0.5f; zs[0] = b[2] * (G::FX * G::FY); zs[1] = lo ? zs[0] - G::FX * G::FY : zs[0]; fz[0] = d[2]; fz[1] = lo ? d[2] + 0.5f : d[2] - 0.5f; }
+        else { zs[0] = zs[1] = 0; fz[0] = fz[1] = 0.f; }
+        const int ST[6][3] = { {1,0,0}, {0,1,0}, {0,0,1}, {0,1,1}, {1,0,1}, {1,1,0} };
+#pragma unroll
+        for (int c = 0; c < 6; ++c) {
+            const float *Fc = T.sF + c * G::FNP + (xs[ST[c][0]] + ys[ST[c][1]] + zs[ST[c][2]]);
+            const float f0 = fx[ST[c][0]], f1 = fy[ST[c][1]];
+            float v00 = Fc[0], v10 = Fc[1], v01 = Fc[G::FX], v11 = Fc[G::FX + 1];
+            float l0 = v00 + f0 * (v10 - v00), l1 = v01 + f0 * (v11 - v01);
+            float lo = l0 + f1 * (l1 - l0);
+            if (D == 3) {
+                const float f2 = fz[ST[c][2]];
+                const float *Fh = Fc + G::FX * G::FY;
+                float w00 = Fh[0], w10 = Fh[1], w01 = Fh[G::FX], w11 = Fh[G::FX + 1];
+                float h0 = w00 + f0 * (w10 - w00), h1 = w01 + f0 * (w11 - w01);
+                float hi = h0 + f1 * (h1 - h0);
+                lo = lo + f2 * (hi - lo);
+            }
+            EBv[c] = lo;
+        }
+    }
+    // ---- S2 tetrad (A^hat = sqrt(h_ii) A^i), S3 Boris (Eq. 3), S4-S5 move + crossing
+    float E[3] = { T.sx[0] * EBv[0], T.sx[1] * EBv[1], T.sx[2] * EBv[2] }, B[3] = { T.sx[0] * EBv[3], T.sx[1] * EBv[4], T.sx[2] * EBv[5] };
+    boris(u, E, B, A.eps);
+    const float ig = inv_gamma(u);
+    const float a0[3] = { d[0], d[1], d[2] };
+    int di[3] = {0, 0, 0};
+    bool alive = true;
+#pragma unroll
+    for (int a = 0; a < D; ++a) {
+        float x = d[a] + (u[a] * ig) * A.cdt[a];
+        split_offset(x, di[a], d[a]);
+        int in = i[a] + di[a];
+        const int wrapN = (ALLPER || g.bc[a] == ENT_PERIODIC) ? g.N[a] : 0;
+        in += (in < 0) ? wrapN : 0;
+        in -= (in >= g.N[a]) ? wrapN : 0;
+        if (!ALLPER) { if (in < 0) { alive = false; in = 0; } if (in >= g.N[a]) { alive = false; in = g.N[a] - 1; } }
+        i[a] = in;
+    }
+    cell = (D == 2) ? i[0] + g.N[0] * i[1] : i[0] + g.N[0] * (i[1] + g.N[1] * i[2]);
+    if (!alive) return 2;
+    bool bad = false;
+#pragma unroll
+    for (int a = 0; a < D; ++a) bad |= (di[a] < -1) | (di[a] > 1);
+    if (bad) { atomicAdd(A.counters + 0, 1ULL); return 0; }
+    const float qw = A.q * wgt;
+    edge |= !(fabsf(wgt) <= T.wguard);        // a weight far above the tile's recorded maximum (changed since the sort) cannot use the tile's scale
+    if (edge) { edge_deposit<D>(A, iold[0], iold[1], iold[2], a0[0], a0[1], a0[2], di[0], di[1], di[2], d[0], d[1], d[2], u[0], u[1], u[2], qw); return 0; }     // rare: global atomics, un-wrapped from the true cell
+    // ---- S7 deposit into the shared-memory J tile (Eq. 6); node (b) of the box = element b of the J tile
+    {
+        const float Q = qw * A.inv_dt * T.Sc;                                // Q in fixed-point units
+        // 3D: one straight segment unless a face is crossed.  2D: always the two segments of P:575, because the
+        // out-of-plane weights (bilinear, G8) of two half segments do not sum to those of the whole one
+        const bool cross = (D == 2) || (di[0] | di[1] | di[2]) != 0;
+        float s[3], e[3], r[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            if (a < D) {
+                float bn = (float)di[a] + d[a];                              // new position in the old cell's frame
+                r[a] = di[a] == 0 ? (cross ? 0.5f * (a0[a] + bn) : bn) : (di[a] > 0 ? 1.0f : 0.0f);
+                s[a] = a0[a]; e[a] = r[a];
+            } else { r[a] = s[a] = e[a] = 0.f; }
+        }
+        int base = b[0] + G::JX * (b[1] + G::JY * b[2]);
+        const int dbase = di[0] + G::JX * (di[1] + G::JY * di[2]);
+        float hv = 0.f;
+        if (D == 2) hv = 0.5f * qw * T.Sc * (u[2] * ig);                     // out-of-plane rate per segment (G8), h33 = 1
+        const int nseg = cross ? 2 : 1;
+#pragma unroll 1
+        for (int seg = 0; seg < nseg; ++seg) {
+            float Dv[3], W[3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { Dv[a] = e[a] - s[a]; W[a] = 0.5f * (e[a] + s[a]); }
+            if (D == 3) {
+                const int st[3] = { 1, G::JX, G::JX * G::JY };
+#pragma unroll
+                for (int comp = 0; comp < 3; ++comp) {
+                    const int a = (comp + 1) % 3, bb = (comp + 2) % 3;
+                    float c = Dv[a] * Dv[bb] * (1.0f / 12.0f);
+                    float QD = Q * Dv[comp];
+                    float w11 = W[a] * W[bb] + c, w10 = W[a] - w11, w01 = W[bb] - w11, w00 = 1.0f - W[a] - w01;
+                    acc_fixed4(T.sJ, T.cc, comp, base, base + st[a], base + st[bb], base + st[a] + st[bb],
+                               QD * w00, QD * w10, QD * w01, QD * w11);
+                }
+            } else {
+                float q0 = Q * Dv[0], q1 = Q * Dv[1];
+                float h1 = hv * W[1], h0 = hv - h1;
+                acc_fixed4(T.sJ, T.cc, 0, base, base + G::JX, base, base + G::JX, q0 * (1.0f - W[1]), q0 * W[1], 0.f, 0.f);
+                acc_fixed4(T.sJ, T.cc, 1, base, base + 1, base, base + 1, q1 * (1.0f - W[0]), q1 * W[0], 0.f, 0.f);
+                acc_fixed4(T.sJ, T.cc, 2, base, base + 1, base + G::JX, base + G::JX + 1,
+                           h0 * (1.0f - W[0]), h0 * W[0], h1 * (1.0f - W[0]), h1 * W[0]);
+            }
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { s[a] = r[a] - (float)di[a]; e[a] = d[a]; }
+            base += dbase;
+        }
+    }
+    return 0;
+}
+
 template <int D, int TX, int TY, int TZ, bool ALLPER>     // ALLPER: every dimension periodic (no ABSORB bookkeeping)
 __global__ void __launch_bounds__(TILED_TPB, ENT_TILED_MINB)
 step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ TiledArgs A) {
     using G = TileGeom<D, TX, TY, TZ>;
     extern __shared__ __align__(128) float smem[];
-    float *sF = smem;                     // [6][FNP]
+    float *sF = smem;                                            // [6][FNP]
     int *sJ = reinterpret_cast<int *>(smem + 6 * G::FNP);        // [3][JNP], fixed point (see acc_fixed)
     __shared__ uint64_t bar;
-    __shared__ float s_wmax[TILED_TPB / 32];
     const GridDev &g = A.g;
     const int tid = threadIdx.x;
 
-    // tile origin (active cell coordinates)
-    int tile = blockIdx.x;
-    int t0 = tile % g.nt[0], t12 = tile / g.nt[0];
-    int t1 = (D == 3) ? t12 % g.nt[1] : t12, t2 = (D == 3) ? t12 / g.nt[1] : 0;
-    const int o0 = t0 * TX, o1 = t1 * TY, o2 = t2 * TZ;
+    const int tile = blockIdx.x;
+    const int t0 = tile % g.nt[0], t12 = tile / g.nt[0];
+    const int t1 = (D == 3) ? t12 % g.nt[1] : t12, t2 = (D == 3) ? t12 / g.nt[1] : 0;
+    TileCtx<D> T;
+    T.sF = sF; T.sJ = sJ;
+    T.o[0] = t0 * TX; T.o[1] = t1 * TY; T.o[2] = t2 * TZ;
+    T.sx[0] = g.dx[0]; T.sx[1] = g.dx[1]; T.sx[2] = g.dx[2];
 
     if (tid == 0) {
         mbar_init(&bar, 1);
         fence_mbar_init();
         mbar_expect_tx(&bar, 6u * G::FN * 4u);
 #pragma unroll
-        for (int c = 0; c < 6; ++c) tma_load_box<D>(sF + c * G::FNP, &maps.F[c], &bar, o0, o1, o2);   // padded coords of active o-2
+        for (int c = 0; c < 6; ++c) tma_load_box<D>(sF + c * G::FNP, &maps.F[c], &bar, T.o[0], T.o[1], T.o[2]);   // padded coords of active o-2
     }
-    for (int k = tid; k < 3 * G::JNP; k += TILED_TPB) sJ[k] = 0;
-
+    for (int k = tid; k < 3 * G::JNP / 4; k += TILED_TPB) reinterpret_cast<int4 *>(sJ)[k] = make_int4(0, 0, 0, 0);
 
     const long long p0 = A.key_off[tile], p1 = A.key_off[tile + 1];
-    const long long G0 = p0 >> 2, G1 = (p1 + 3) >> 2;
-    const float sx = g.dx[0], sy = g.dx[1], sz = g.dx[2];
-    bool waited = false;
-    // fixed-point scale of this tile: 2^k with 2^k * (13/12) |q| wmax / dt < 2^23 (wmax over the tile's particles)
-    float Sc, invSc;
+    float invSc;
     {
-        float wm = 0.f;
-        for (long long p = p0 + tid; p < p1; p += TILED_TPB) wm = fmaxf(wm, fabsf(A.P.w[p]));
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) wm = fmaxf(wm, __shfl_xor_sync(0xffffffffu, wm, o));
-        if ((tid & 31) == 0) s_wmax[tid >> 5] = wm;
-        __syncthreads();                       // also: sJ zeroed, mbarrier initialised
-#pragma unroll
-        for (int k = 0; k < TILED_TPB / 32; ++k) wm = fmaxf(wm, s_wmax[k]);
-        // largest contribution: |q| wmax / dt * |D| * weight, |D| <= 1, weight <= 13/12 (2D: J^3 = q w v^3 has no 1/dt).
-        // It gets `bits` bits; fewer in a dense tile, so that ~8x the mean nodal current still fits the 32-bit accumulator.
+        // fixed-point scale of this tile.  Largest contribution: |q| wmax / dt * |D| * weight with |D| <= 1, weight <= 13/12
+        // (2D: J^3 = q w v^3 has no 1/dt); wmax = max |w| over the tile's particles (ent_sort).  It gets 24 bits, fewer in
+        // a dense tile so that ~8x the mean nodal current still fits the 32-bit accumulator (beyond that: carry_fix).
+        const float wm = A.tile_wmax[tile];
         float qmax = fabsf(A.q) * wm * ((D == 2) ? fmaxf(A.inv_dt, 0.5f) : A.inv_dt) * 1.0834f;
         float dens = (float)(p1 - p0) / (float)G::TCELLS;
         float top = fminf(16777000.0f, 2.6e8f / fmaxf(dens, 1.0f));
-        Sc = (qmax > 0.f && qmax < 1e37f) ? top / qmax : 0.f;
+        float Sc = (qmax > 0.f && qmax < 1e37f) ? top / qmax : 0.f;
         if (!(Sc > 1e-30f && Sc < 1e30f)) Sc = 0.f;
         invSc = Sc > 0.f ? 1.0f / Sc : 0.f;
+        T.Sc = Sc; T.wguard = Sc > 0.f ? 60.0f * wm : -1.0f;
     }
-    CarryCtx cc;
-    cc.J = A.J.c; cc.P0 = g.P[0]; cc.P01 = g.P[0] * g.P[1]; cc.unit = 4294967296.0f * invSc;
-    cc.JX = G::JX; cc.JY = G::JY; cc.JNP = G::JNP;
-    cc.gbase = (long long)o0 + (long long)g.P[0] * o1 + (D == 3 ? (long long)g.P[0] * g.P[1] * o2 : 0);
+    T.cc.J = A.J.c; T.cc.P0 = g.P[0]; T.cc.P01 = g.P[0] * g.P[1]; T.cc.unit = 4294967296.0f * invSc;
+    T.cc.JX = G::JX; T.cc.JY = G::JY; T.cc.JNP = G::JNP;
+    T.cc.gbase = (long long)T.o[0] + (long long)g.P[0] * T.o[1] + (D == 3 ? (long long)g.P[0] * g.P[1] * T.o[2] : 0);
+    __syncthreads();                                             // sJ zeroed, mbarrier initialised
+    bool waited = false;
 
+    // ---- groups of four consecutive particles per thread (128-bit accesses; consecutive lanes are four particles apart).
+    // A group that straddles the ends of the tile's range [p0, p1) is shared with the neighbouring tile's CTA: each side
+    // touches only its own particles, with scalar accesses.
+    const long long G0 = p0 >> 2, G1 = (p1 + 3) >> 2;
     for (long long grp = G0 + tid; grp < G1; grp += TILED_TPB) {
         const long long pb = grp * 4;
         const bool full = pb >= p0 && pb + 4 <= p1;
         int4 vc; float4 vd0, vd1, vd2, vu0, vu1, vu2, vw;
+        uchar4 vt = make_uchar4(1, 1, 1, 1);
         vd2 = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (pb + 4 <= A.n) {
+        if (full) {
             vc = *reinterpret_cast<const int4 *>(A.P.cell + pb);
             vd0 = *reinterpret_cast<const float4 *>(A.P.d[0] + pb);
             vd1 = *reinterpret_cast<const float4 *>(A.P.d[1] + pb);
@@ -245,160 +399,34 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
             vu1 = *reinterpret_cast<const float4 *>(A.P.u[1] + pb);
             vu2 = *reinterpret_cast<const float4 *>(A.P.u[2] + pb);
             vw = *reinterpret_cast<const float4 *>(A.P.w + pb);
+            if (A.P.tag) vt = *reinterpret_cast<const uchar4 *>(A.P.tag + pb);
         } else {
-            int *c = &vc.x; float *d0 = &vd0.x, *d1 = &vd1.x, *d2 = &vd2.x, *u0 = &vu0.x, *u1 = &vu1.x, *u2 = &vu2.x, *w = &vw.x;
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                bool in = pb + k < A.n;
-                c[k] = in ? A.P.cell[pb + k] : 0;
-                d0[k] = in ? A.P.d[0][pb + k] : 0.f; d1[k] = in ? A.P.d[1][pb + k] : 0.f;
-                d2[k] = (D == 3 && in) ? A.P.d[2][pb + k] : 0.f;
-                u0[k] = in ? A.P.u[0][pb + k] : 0.f; u1[k] = in ? A.P.u[1][pb + k] : 0.f; u2[k] = in ? A.P.u[2][pb + k] : 0.f;
-                w[k] = in ? A.P.w[pb + k] : 0.f;
+                const bool in = pb + k >= p0 && pb + k < p1;
+                (&vc.x)[k] = in ? A.P.cell[pb + k] : 0;
+                (&vd0.x)[k] = in ? A.P.d[0][pb + k] : 0.f; (&vd1.x)[k] = in ? A.P.d[1][pb + k] : 0.f;
+                (&vd2.x)[k] = (D == 3 && in) ? A.P.d[2][pb + k] : 0.f;
+                (&vu0.x)[k] = in ? A.P.u[0][pb + k] : 0.f; (&vu1.x)[k] = in ? A.P.u[1][pb + k] : 0.f; (&vu2.x)[k] = in ? A.P.u[2][pb + k] : 0.f;
+                (&vw.x)[k] = in ? A.P.w[pb + k] : 0.f;
+                (&vt.x)[k] = in ? (A.P.tag ? A.P.tag[pb + k] : 1) : 0;
             }
         }
-        unsigned valid = 0, tagv = 0xf;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) valid |= (pb + k >= p0 && pb + k < p1) ? (1u << k) : 0u;
-        if (A.P.tag) {
-            tagv = 0;
-#pragma unroll
-            for (int k = 0; k < 4; ++k) if ((valid >> k) & 1u) tagv |= A.P.tag[pb + k] ? (1u << k) : 0u;
-        }
-        unsigned store = 0, died = 0;         // particles whose record this thread writes back / that left through ABSORB
         if (!waited) { mbar_wait(&bar, 0); waited = true; }
-
+        int code[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            // component k of every vector (the unrolled loop turns these into plain register names)
-            const int cell = (&vc.x)[k];
+        for (int k = 0; k < 4; ++k) {                      // component k of every vector: plain register names after unrolling
             float d[3] = { (&vd0.x)[k], (&vd1.x)[k], (&vd2.x)[k] };
             float u[3] = { (&vu0.x)[k], (&vu1.x)[k], (&vu2.x)[k] };
-            const float wgt = (&vw.x)[k];
-            if (!(((valid & tagv) >> k) & 1u)) continue;                       // not ours, or dead (left untouched)
-            // ---- where is the cell relative to the tile box?  b = cell index in box coordinates (box origin = o-2)
-            int i[3];
-            if (D == 2) { i[1] = A.divN0.div(cell); i[0] = cell - i[1] * g.N[0]; i[2] = 0; }
-            else { i[2] = A.divN01.div(cell); int r = cell - i[2] * (g.N[0] * g.N[1]); i[1] = A.divN0.div(r); i[0] = r - i[1] * g.N[0]; }
-            int b[3] = { i[0] - o0 + 2, i[1] - o1 + 2, (D == 3) ? i[2] - o2 + 2 : 0 };
-            const int TT[3] = { TX, TY, TZ }, OO[3] = { o0, o1, o2 };
-            bool local = true;
-#pragma unroll
-            for (int a = 0; a < D; ++a) {
-                const int wrapN = (ALLPER || g.bc[a] == ENT_PERIODIC) ? g.N[a] : 0;
-                b[a] += (b[a] < 1) ? wrapN : 0;
-                b[a] -= (b[a] > g.N[a]) ? wrapN : 0;
-                // inside the box with one cell of margin, and the un-wrapped cell o-2+b <= N-1 so that the deposit of a
-                // +1 crossing (nodes up to cell+2) stays inside the padded array
-                local &= (b[a] >= 1) & (b[a] < TT[a] + 3) & (OO[a] - 2 + b[a] <= g.N[a] - 1);
-            }
-            if (!local) { stray_step<D>(A, pb + k); continue; }
-            store |= 1u << k;
-            // ---- S1 gather from the shared-memory box (same stencil as ent_dev.cuh gather)
-            float EBv[6];
-            {
-                int xs[2], ys[2], zs[2]; float fx[2], fy[2], fz[2];              // [0] node-centred, [1] half-shifted
-                { bool lo = d[0] < 0.5f; xs[0] = b[0]; xs[1] = lo ? b[0] - 1 : b[0]; fx[0] = d[0]; fx[1] = lo ? d[0] + 0.5f : d[0] - 0.5f; }
-                { bool lo = d[1] < 0.5f; ys[0] = b[1] * G::FX; ys[1] = lo ? ys[0] - G::FX : ys[0]; fy[0] = d[1]; fy[1] = lo ? d[1] + 0.5f : d[1] - 0.5f; }
-                if (D == 3) { bool lo = d[2] < 0.5f; zs[0] = b[2] * (G::FX * G::FY); zs[1] = lo ? zs[0] - G::FX * G::FY : zs[0]; fz[0] = d[2]; fz[1] = lo ? d[2] + 0.5f : d[2] - 0.5f; }
-                else { zs[0] = zs[1] = 0; fz[0] = fz[1] = 0.f; }
-                const int ST[6][3] = { {1,0,0}, {0,1,0}, {0,0,1}, {0,1,1}, {1,0,1}, {1,1,0} };
-#pragma unroll
-                for (int c = 0; c < 6; ++c) {
-                    const float *Fc = sF + c * G::FNP + (xs[ST[c][0]] + ys[ST[c][1]] + zs[ST[c][2]]);
-                    const float f0 = fx[ST[c][0]], f1 = fy[ST[c][1]];
-                    float v00 = Fc[0], v10 = Fc[1], v01 = Fc[G::FX], v11 = Fc[G::FX + 1];
-                    float l0 = v00 + f0 * (v10 - v00), l1 = v01 + f0 * (v11 - v01);
-                    float lo = l0 + f1 * (l1 - l0);
-                    if (D == 3) {
-                        const float f2 = fz[ST[c][2]];
-                        const float *Fh = Fc + G::FX * G::FY;
-                        float w00 = Fh[0], w10 = Fh[1], w01 = Fh[G::FX], w11 = Fh[G::FX + 1];
-                        float h0 = w00 + f0 * (w10 - w00), h1 = w01 + f0 * (w11 - w01);
-                        float hi = h0 + f1 * (h1 - h0);
-                        lo = lo + f2 * (hi - lo);
-                    }
-                    EBv[c] = lo;
-                }
-            }
-            // ---- S2 tetrad (A^hat = sqrt(h_ii) A^i), S3 Boris (Eq. 3), S4-S5 move + crossing
-            float E[3] = { sx * EBv[0], sy * EBv[1], sz * EBv[2] }, B[3] = { sx * EBv[3], sy * EBv[4], sz * EBv[5] };
-            boris(u, E, B, A.eps);
-            const float ig = inv_gamma(u);
-            const float a0[3] = { d[0], d[1], d[2] };
-            int di[3] = {0, 0, 0};
-            bool alive = true;
-#pragma unroll
-            for (int a = 0; a < D; ++a) {
-                float x = d[a] + (u[a] * ig) * A.cdt[a];
-                split_offset(x, di[a], d[a]);
-                int in = i[a] + di[a];
-                const int wrapN = (ALLPER || g.bc[a] == ENT_PERIODIC) ? g.N[a] : 0;
-                in += (in < 0) ? wrapN : 0;
-                in -= (in >= g.N[a]) ? wrapN : 0;
-                if (!ALLPER) { if (in < 0) { alive = false; in = 0; } if (in >= g.N[a]) { alive = false; in = g.N[a] - 1; } }
-                i[a] = in;
-            }
-            (&vc.x)[k] = (D == 2) ? i[0] + g.N[0] * i[1] : i[0] + g.N[0] * (i[1] + g.N[1] * i[2]);
-            (&vd0.x)[k] = d[0]; (&vd1.x)[k] = d[1]; if (D == 3) (&vd2.x)[k] = d[2];
-            (&vu0.x)[k] = u[0]; (&vu1.x)[k] = u[1]; (&vu2.x)[k] = u[2];
-            if (!alive) { died |= 1u << k; continue; }
-            bool bad = false;
-#pragma unroll
-            for (int a = 0; a < D; ++a) bad |= (di[a] < -1) | (di[a] > 1);
-            if (bad) { atomicAdd(A.counters + 0, 1ULL); continue; }
-            // ---- S7 deposit into the shared-memory J tile (Eq. 6); node (b) of the box = element b of the J tile
-            {
-                const float qw = A.q * wgt, Q = qw * A.inv_dt * Sc;                 // Q in fixed-point units
-                // 3D: one straight segment unless a face is crossed.  2D: always the two segments of P:575, because the
-                // out-of-plane weights (bilinear, G8) of two half segments do not sum to those of the whole one
-                const bool cross = (D == 2) || (di[0] | di[1] | di[2]) != 0;
-                float s[3], e[3], r[3];
-#pragma unroll
-                for (int a = 0; a < 3; ++a) {
-                    if (a < D) {
-                        float bn = (float)di[a] + d[a];                          // new position in the old cell's frame
-                        r[a] = di[a] == 0 ? (cross ? 0.5f * (a0[a] + bn) : bn) : (di[a] > 0 ? 1.0f : 0.0f);
-                        s[a] = a0[a]; e[a] = r[a];
-                    } else { r[a] = s[a] = e[a] = 0.f; }
-                }
-                int base = b[0] + G::JX * (b[1] + G::JY * b[2]);
-                const int dbase = di[0] + G::JX * (di[1] + G::JY * di[2]);
-                float hv = 0.f;
-                if (D == 2) hv = 0.5f * qw * Sc * (u[2] * ig);       // out-of-plane rate per segment (G8), h33 = 1
-                const int nseg = cross ? 2 : 1;
-#pragma unroll 1
-                for (int seg = 0; seg < nseg; ++seg) {
-                    float Dv[3], W[3];
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) { Dv[a] = e[a] - s[a]; W[a] = 0.5f * (e[a] + s[a]); }
-                    if (D == 3) {
-                        const int st[3] = { 1, G::JX, G::JX * G::JY };
-#pragma unroll
-                        for (int comp = 0; comp < 3; ++comp) {
-                            const int a = (comp + 1) % 3, bb = (comp + 2) % 3;
-                            float c = Dv[a] * Dv[bb] * (1.0f / 12.0f);
-                            float QD = Q * Dv[comp];
-                            float w11 = W[a] * W[bb] + c, w10 = W[a] - w11, w01 = W[bb] - w11, w00 = 1.0f - W[a] - w01;
-                            acc_fixed4(sJ, cc, comp, base, base + st[a], base + st[bb], base + st[a] + st[bb],
-                                       QD * w00, QD * w10, QD * w01, QD * w11);
-                        }
-                    } else {
-                        float q0 = Q * Dv[0], q1 = Q * Dv[1];
-                        acc_fixed(sJ, cc, 0, base, q0 * (1.0f - W[1])); acc_fixed(sJ, cc, 0, base + G::JX, q0 * W[1]);
-                        acc_fixed(sJ, cc, 1, base, q1 * (1.0f - W[0])); acc_fixed(sJ, cc, 1, base + 1, q1 * W[0]);
-                        float h1 = hv * W[1], h0 = hv - h1;
-                        acc_fixed(sJ, cc, 2, base, h0 * (1.0f - W[0])); acc_fixed(sJ, cc, 2, base + 1, h0 * W[0]);
-                        acc_fixed(sJ, cc, 2, base + G::JX, h1 * (1.0f - W[0])); acc_fixed(sJ, cc, 2, base + G::JX + 1, h1 * W[0]);
-                    }
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) { s[a] = r[a] - (float)di[a]; e[a] = d[a]; }
-                    base += dbase;
-                }
+            code[k] = 3;
+            if ((&vt.x)[k]) {
+                code[k] = tile_particle<D, TX, TY, TZ, ALLPER>(A, T, pb + k, (&vc.x)[k], d, u, (&vw.x)[k]);
+                (&vd0.x)[k] = d[0]; (&vd1.x)[k] = d[1]; (&vd2.x)[k] = d[2];
+                (&vu0.x)[k] = u[0]; (&vu1.x)[k] = u[1]; (&vu2.x)[k] = u[2];
             }
         }
         // ---- write back (cell, offsets, momentum; the weight is read-only)
-        if (full && store == 0xf) {
+        if (full && ((code[0] | code[1] | code[2] | code[3]) & 1) == 0) {        // nobody dead or taken by the global path
             *reinterpret_cast<int4 *>(A.P.cell + pb) = vc;
             *reinterpret_cast<float4 *>(A.P.d[0] + pb) = vd0;
             *reinterpret_cast<float4 *>(A.P.d[1] + pb) = vd1;
@@ -409,27 +437,30 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
         } else {
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                if (!((store >> k) & 1u)) continue;
+                if (code[k] & 1) continue;
                 A.P.cell[pb + k] = (&vc.x)[k];
                 A.P.d[0][pb + k] = (&vd0.x)[k]; A.P.d[1][pb + k] = (&vd1.x)[k];
                 if (D == 3) A.P.d[2][pb + k] = (&vd2.x)[k];
                 A.P.u[0][pb + k] = (&vu0.x)[k]; A.P.u[1][pb + k] = (&vu1.x)[k]; A.P.u[2][pb + k] = (&vu2.x)[k];
             }
         }
-        if (died) {
+        if (!ALLPER) {
 #pragma unroll
-            for (int k = 0; k < 4; ++k) if ((died >> k) & 1u) A.P.tag[pb + k] = 0;
+            for (int k = 0; k < 4; ++k) if (code[k] == 2) A.P.tag[pb + k] = 0;
         }
     }
     if (!waited) mbar_wait(&bar, 0);          // never leave with a TMA load still in flight into this CTA's shared memory
     // ---- S8 flush: one TMA reduce-add per component into the un-wrapped padded J (ghost fold = ent_fold_current)
     __syncthreads();
-    for (int k = tid; k < 3 * G::JNP; k += TILED_TPB) reinterpret_cast<float *>(sJ)[k] = (float)sJ[k] * invSc;   // fixed point -> fp32, in place
+    for (int k = tid; k < 3 * G::JNP / 4; k += TILED_TPB) {      // fixed point -> fp32, in place
+        int4 v = reinterpret_cast<int4 *>(sJ)[k];
+        reinterpret_cast<float4 *>(sJ)[k] = make_float4((float)v.x * invSc, (float)v.y * invSc, (float)v.z * invSc, (float)v.w * invSc);
+    }
     fence_proxy_async_smem();
     __syncthreads();
     if (tid == 0) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) tma_reduce_add_box<D>(&maps.J[c], sJ + c * G::JNP, o0, o1, o2);
+        for (int c = 0; c < 3; ++c) tma_reduce_add_box<D>(&maps.J[c], sJ + c * G::JNP, T.o[0], T.o[1], T.o[2]);
         tma_commit();
         tma_wait_read0();
     }
@@ -534,10 +565,10 @@ inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, 
 }
 
 inline int tiled_step(TiledState &t, const GridDev &g, cudaStream_t stream, FieldPtrs F, PartPtrs P, CurrentPtrs J, long long n,
-                      const int32_t *key_off, float eps, float dt, float q, float inv_dt, unsigned long long *counters,
+                      const int32_t *key_off, const float *tile_wmax, float eps, float dt, float q, float inv_dt, unsigned long long *counters,
                       long long *launches, char *err, size_t errn) {
     TiledArgs A;
-    A.g = g; A.F = F; A.J = J; A.P = P; A.key_off = key_off; A.n = n;
+    A.g = g; A.F = F; A.J = J; A.P = P; A.key_off = key_off; A.tile_wmax = tile_wmax; A.n = n;
     A.eps = eps; A.dt = dt; A.q = q; A.inv_dt = inv_dt; A.counters = counters;
     for (int a = 0; a < 3; ++a) A.cdt[a] = dt * g.inv_dx[a];
     A.divN0 = make_fastdiv((uint32_t)g.N[0]);

@@ -48,16 +48,20 @@ def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True
         po = P.species_to_orc(orc, sp)
         order = None
         if sort_first:
-            # carry the original index through the sort as the bit pattern of the weight array (the order inside a cell
-            # is unspecified, G18), then put the real weights back in sorted order
-            scratch = pe.clone()
-            scratch.w = torch.arange(pe.n, device="cuda", dtype=torch.int32).view(torch.float32).clone()
-            ps = scratch.empty_like()
-            bind.ent_sort(ctx, scratch, ps, None)
-            order_t = ps.w.view(torch.int32).to(torch.int64)
-            assert torch.equal(torch.sort(order_t).values, torch.arange(pe.n, device="cuda")), "ent_sort lost particles"
-            ps.w.copy_(pe.w[order_t])
-            order = order_t.cpu().numpy()
+            # ent_sort permutes every array alike; the order inside a cell is unspecified (G18), so the permutation is
+            # recovered by matching records: (cell, offsets, momentum) is unique per particle in these workloads
+            ps = pe.empty_like()
+            bind.ent_sort(ctx, pe, ps, None)
+
+            def rank(p):
+                cols = [p.u[0], p.d[1], p.d[0], p.cell] if g.D == 2 else [p.u[0], p.d[2], p.d[1], p.d[0], p.cell]
+                return np.lexsort([c.detach().cpu().numpy() for c in cols])
+            r_in, r_out = rank(pe), rank(ps)
+            order = np.empty(pe.n, dtype=np.int64)
+            order[r_out] = r_in                                   # sorted particle k is original particle order[k]
+            ot = torch.from_numpy(order).cuda()
+            assert torch.equal(ps.cell, pe.cell[ot]) and torch.equal(ps.u[2], pe.u[2][ot]) and torch.equal(ps.w, pe.w[ot]), \
+                "ent_sort is not a permutation of the records"
             pe = ps
         Jg = bind.zeros_current(eg, "cuda")
         worstJ = worstC = 0.0
