@@ -122,7 +122,11 @@ int ent_deposit(ent_ctx *ctx, const ent_particles *old_, const ent_particles *ne
  * Dead particles keep their key.  On return `out` holds a permutation of `in` with non-decreasing keys
  * (order inside one cell unspecified) and, if key_offsets != NULL (device, int32[NKEYS+1]),
  * key_offsets[k] = number of particles with key < k.  in and out must not overlap; out's arrays must exist
- * wherever in's do.  The ctx remembers `out` as "sorted" so that ent_step may take its tiled path on it. */
+ * wherever in's do.  The ctx remembers `out` as "sorted" so that ent_step may take its tiled path on it.
+ * Incremental form (ENT_OPT_SORT_MODE = 0, the default): when `in` is itself a block a previous ent_sort of this ctx
+ * produced (same pointers and n; its particles have drifted since) and key_offsets is NULL, only tile contiguity is
+ * re-established: `out` is a permutation of `in` in which tile(key) is non-decreasing; the order inside a tile is
+ * unspecified (the tiled ent_step does not depend on it).  ENT_STAT_LAST_SORT_REBIN tells which form ran. */
 int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *out, int32_t *key_offsets);
 
 /* ---- fused hot path: the timed entry point ------------------------------------------------------------------
@@ -152,7 +156,9 @@ int ent_step_host(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_curr
 enum {
     ENT_OPT_STEP_IMPL = 1,     /* 0 = auto (tiled when the block is the sorted one), 1 = force untiled, 2 = two-kernel
                                   (gather_push to scratch copy + deposit; the paper's structure) */
-    ENT_OPT_TILE_1 = 2, ENT_OPT_TILE_2 = 3, ENT_OPT_TILE_3 = 4    /* tile extents in cells; takes effect at the next ent_set_grid */
+    ENT_OPT_TILE_1 = 2, ENT_OPT_TILE_2 = 3, ENT_OPT_TILE_3 = 4,   /* tile extents in cells; takes effect at the next ent_set_grid */
+    ENT_OPT_SORT_MODE = 5      /* 0 = auto (incremental re-bin when `in` is itself a block ent_sort produced and key_offsets is NULL),
+                                  1 = always the full cell-level counting sort */
 };
 enum {
     ENT_STAT_TILE_1 = 1, ENT_STAT_TILE_2 = 2, ENT_STAT_TILE_3 = 3, ENT_STAT_NKEYS = 4, ENT_STAT_NTILES = 5,
@@ -160,7 +166,8 @@ enum {
     ENT_STAT_BAD_MOVES = 7,    /* particles with |delta i| > 1 seen by deposit/step (synchronises the stream) */
     ENT_STAT_STRAYS = 8,       /* particles that took the out-of-halo path in the last tiled ent_step (synchronises) */
     ENT_STAT_SCRATCH_BYTES = 9,
-    ENT_STAT_LAST_STEP_TILED = 10
+    ENT_STAT_LAST_STEP_TILED = 10,
+    ENT_STAT_LAST_SORT_REBIN = 11   /* 1 if the last ent_sort took the incremental re-bin path */
 };
 int ent_set_option(ent_ctx *ctx, int key, int64_t value);
 int ent_get_stat(ent_ctx *ctx, int key, int64_t *value);

@@ -20,6 +20,9 @@ struct ent_ctx {
     GridDev g{};
     int tile_opt[3] = {0, 0, 0};          // 0 = default
     int step_impl = 0;
+    int sort_mode = 0;                    // 0 auto (re-bin when the input is a sorted block), 1 always the full cell-level sort
+    int last_sort_rebin = 0;
+    int32_t *class_count = nullptr; size_t class_cap = 0;
     long long launches = 0;
     // scratch
     unsigned long long *counters = nullptr;   // [0] bad moves, [1] strays
@@ -98,7 +101,7 @@ extern "C" int ent_destroy(ent_ctx *ctx) {
     cudaStreamSynchronize(ctx->stream);
     tiled_release(ctx->tiled);
     cudaFree(ctx->counters); cudaFree(ctx->keys); cudaFree(ctx->count); cudaFree(ctx->offsets); cudaFree(ctx->cursor);
-    cudaFree(ctx->chunk); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf);
+    cudaFree(ctx->chunk); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf); cudaFree(ctx->class_count);
     for (auto &b : ctx->sorted) { cudaFree(b.tile_off); cudaFree(b.tile_wmax); }
     cudaGetLastError();
     delete ctx;
@@ -316,6 +319,49 @@ extern "C" int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, en
     return launch_check(ctx, "step_untiled_kernel");
 }
 
+// claims a SortedBlock slot for `out` (never the one in `keep`), sized for ntiles
+static int claim_slot(ent_ctx *ctx, const ent_ctx::SortedBlock *keep, long long ntiles, ent_ctx::SortedBlock **res) {
+    ent_ctx::SortedBlock *slot = nullptr;
+    for (auto &b : ctx->sorted) { if (&b == keep) continue; if (!b.cell) { slot = &b; break; } if (!slot || b.stamp < slot->stamp) slot = &b; }
+    slot->cell = nullptr; slot->n = -1;
+    int rc;
+    if ((rc = ensure(ctx, (void **)&slot->tile_off, &slot->cap, (size_t)(ntiles + 1) * 4))) return rc;
+    if ((rc = ensure(ctx, (void **)&slot->tile_wmax, &slot->wcap, (size_t)ntiles * 4))) return rc;
+    *res = slot;
+    return ENT_OK;
+}
+
+// incremental ent_sort: `in` is tile-contiguous (src), particles have drifted; re-establish tile contiguity in `out`
+static int sort_rebin(ent_ctx *ctx, const ent_ctx::SortedBlock *src, const ent_particles *in, ent_particles *out) {
+    const GridDev &g = ctx->g;
+    const long long ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
+    const int nchunks = (int)((ntiles + SCAN_CHUNK - 1) / SCAN_CHUNK);
+    int rc;
+    if ((rc = ensure(ctx, (void **)&ctx->class_count, &ctx->class_cap, (size_t)ntiles * REBIN_CLASSES * 4))) return rc;
+    ent_ctx::SortedBlock *slot;
+    if ((rc = claim_slot(ctx, src, ntiles, &slot))) return rc;
+    RebinGeom G;
+    G.D = g.D;
+    for (int a = 0; a < 3; ++a) { G.N[a] = g.N[a]; G.T[a] = g.T[a]; G.nt[a] = g.nt[a]; G.per[a] = g.bc[a] == ENT_PERIODIC; }
+    CK(cudaMemsetAsync(ctx->count, 0, (size_t)(ntiles + 1) * 4, ctx->stream));
+    CK(cudaMemsetAsync(slot->tile_wmax, 0, (size_t)ntiles * 4, ctx->stream));
+    rebin_count_kernel<<<(unsigned)ntiles, REBIN_TPB, 0, ctx->stream>>>(G, in->cell, src->tile_off, ctx->class_count, ctx->count);
+    if ((rc = launch_check(ctx, "rebin_count_kernel"))) return rc;
+    scan_reduce_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, ntiles, ctx->chunk);
+    if ((rc = launch_check(ctx, "scan_reduce_kernel"))) return rc;
+    scan_chunks_kernel<<<1, TPB, 0, ctx->stream>>>(ctx->chunk, nchunks);
+    if ((rc = launch_check(ctx, "scan_chunks_kernel"))) return rc;
+    scan_apply_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, ntiles, ctx->chunk, slot->tile_off, ctx->cursor);
+    if ((rc = launch_check(ctx, "scan_apply_kernel"))) return rc;
+    rebin_scatter_kernel<<<(unsigned)ntiles, REBIN_TPB, 0, ctx->stream>>>(G, src->tile_off, ctx->class_count, ctx->cursor, pp(in), pp(out),
+                                                                        g.kind != ENT_CART, (unsigned *)slot->tile_wmax);
+    if ((rc = launch_check(ctx, "rebin_scatter_kernel"))) return rc;
+    out->q = in->q; out->m = in->m;
+    slot->cell = out->cell; slot->n = in->n; slot->stamp = ++ctx->sort_stamp;
+    ctx->last_sort_rebin = 1;
+    return ENT_OK;
+}
+
 extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *out, int32_t *key_offsets) {
     ENTER();
     int rc;
@@ -344,7 +390,13 @@ extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *ou
         if ((rc = ensure(ctx, (void **)&ctx->chunk, &cap, (size_t)nchunks * 4))) return rc;
         ctx->chunk_cap = (long long)(cap / 4);
     }
-    for (auto &b : ctx->sorted) if (b.cell == out->cell || b.cell == in->cell) { b.cell = nullptr; b.n = -1; }
+    for (auto &b : ctx->sorted) if (b.cell == out->cell) { b.cell = nullptr; b.n = -1; }
+    ctx->last_sort_rebin = 0;
+    if (ctx->sort_mode == 0 && !key_offsets && n > 0) {
+        const ent_ctx::SortedBlock *src = nullptr;
+        for (auto &b : ctx->sorted) if (b.cell == in->cell && b.n == n) src = &b;
+        if (src) return sort_rebin(ctx, src, in, out);
+    }
     CK(cudaMemsetAsync(ctx->count, 0, (size_t)(nkeys + 1) * 4, ctx->stream));
     if (n > 0) {
         if (g.D == 2) sort_hist_kernel<2><<<nblk(n), TPB, 0, ctx->stream>>>(g, in->cell, n, ctx->keys, ctx->count);
@@ -364,14 +416,11 @@ extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *ou
     if (key_offsets) CK(cudaMemcpyAsync(key_offsets, ctx->offsets, (size_t)(nkeys + 1) * 4, cudaMemcpyDeviceToDevice, ctx->stream));
     out->q = in->q; out->m = in->m;
     {   // remember `out` as sorted, with its own copy of the tile offsets (tile t = particles [tile_off[t], tile_off[t+1]))
-        ent_ctx::SortedBlock *slot = &ctx->sorted[0];
-        for (auto &b : ctx->sorted) { if (!b.cell) { slot = &b; break; } if (b.stamp < slot->stamp) slot = &b; }
         const long long ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
-        slot->cell = nullptr; slot->n = -1;
-        if ((rc = ensure(ctx, (void **)&slot->tile_off, &slot->cap, (size_t)(ntiles + 1) * 4))) return rc;
+        ent_ctx::SortedBlock *slot;
+        if ((rc = claim_slot(ctx, nullptr, ntiles, &slot))) return rc;
         tile_offsets_kernel<<<nblk(ntiles + 1), TPB, 0, ctx->stream>>>(ctx->offsets, g.tcells, ntiles, slot->tile_off);
         if ((rc = launch_check(ctx, "tile_offsets_kernel"))) return rc;
-        if ((rc = ensure(ctx, (void **)&slot->tile_wmax, &slot->wcap, (size_t)ntiles * 4))) return rc;
         tile_wmax_kernel<<<(unsigned)ntiles, 128, 0, ctx->stream>>>(slot->tile_off, out->w, slot->tile_wmax);
         if ((rc = launch_check(ctx, "tile_wmax_kernel"))) return rc;
         slot->cell = out->cell; slot->n = n; slot->stamp = ++ctx->sort_stamp;
@@ -385,6 +434,9 @@ extern "C" int ent_set_option(ent_ctx *ctx, int key, int64_t value) {
         case ENT_OPT_STEP_IMPL:
             if (value < 0 || value > 2) return fail(ctx, ENT_EINVAL, "ENT_OPT_STEP_IMPL must be 0, 1 or 2");
             ctx->step_impl = (int)value; return ENT_OK;
+        case ENT_OPT_SORT_MODE:
+            if (value < 0 || value > 1) return fail(ctx, ENT_EINVAL, "ENT_OPT_SORT_MODE must be 0 or 1");
+            ctx->sort_mode = (int)value; return ENT_OK;
         case ENT_OPT_TILE_1: case ENT_OPT_TILE_2: case ENT_OPT_TILE_3:
             if (value < 0 || value > 64) return fail(ctx, ENT_EINVAL, "tile extent must be in 0..64 (0 = default)");
             ctx->tile_opt[key - ENT_OPT_TILE_1] = (int)value; return ENT_OK;
@@ -413,6 +465,7 @@ extern "C" int ent_get_stat(ent_ctx *ctx, int key, int64_t *value) {
         }
         case ENT_STAT_SCRATCH_BYTES: *value = (int64_t)(ctx->scratch_bytes + tiled_scratch_bytes(ctx->tiled)); return ENT_OK;
         case ENT_STAT_LAST_STEP_TILED: *value = ctx->last_step_tiled; return ENT_OK;
+        case ENT_STAT_LAST_SORT_REBIN: *value = ctx->last_sort_rebin; return ENT_OK;
         default: return fail(ctx, ENT_EINVAL, "unknown stat %d", key);
     }
 }

@@ -255,4 +255,121 @@ __global__ void __launch_bounds__(TPB) sort_scatter_kernel(const int32_t *keys, 
     if (in.tag) out.tag[dst] = in.tag[p];
 }
 
+
+// ---------------------------------------------------------------------------------------------------------
+// S10, incremental form ("re-bin"): the input block is tile-contiguous already (a previous ent_sort produced it) and its
+// particles have drifted a few cells, so almost all of them stay in their tile and the rest go to one of the 3^D - 1
+// neighbouring tiles.  One CTA per SOURCE tile: class counts per destination in shared memory, one global reservation per
+// (source tile, destination), particles of a warp that share a destination get consecutive slots in lane order (so the
+// ~90 % that stay are written fully coalesced).  Order inside a destination tile: unspecified.
+// ---------------------------------------------------------------------------------------------------------
+constexpr int REBIN_TPB = 256;
+constexpr int REBIN_CLASSES = 28;            // 27 neighbours (3^D used) + "far"
+
+struct RebinGeom {
+    int D, N[3], T[3], nt[3], per[3];
+    __device__ __forceinline__ void tile_of_cell(int cell, int t[3]) const {
+        int i0, i1, i2 = 0;
+        if (D == 2) { i1 = cell / N[0]; i0 = cell - i1 * N[0]; }
+        else { int n01 = N[0] * N[1]; i2 = cell / n01; int r = cell - i2 * n01; i1 = r / N[0]; i0 = r - i1 * N[0]; }
+        t[0] = i0 / T[0]; t[1] = i1 / T[1]; t[2] = (D == 3) ? i2 / T[2] : 0;
+    }
+    // class of destination tile t seen from source tile s: 0..26 = neighbour (dz+1)*9 + (dy+1)*3 + (dx+1), 27 = far
+    __device__ __forceinline__ int classify(const int s[3], const int t[3]) const {
+        int rel = 0, mul = 1;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            int dlt = t[a] - s[a];
+            if (per[a]) { if (2 * dlt > nt[a]) dlt -= nt[a]; else if (2 * dlt < -nt[a]) dlt += nt[a]; }
+            if (dlt < -1 || dlt > 1) return 27;
+            rel += (dlt + 1) * mul; mul *= 3;
+        }
+        return rel;
+    }
+    __device__ __forceinline__ int dest_tile(const int s[3], int rel) const {      // -1 if the neighbour does not exist
+        int t[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            int dlt = rel % 3 - 1; rel /= 3;
+            int v = s[a] + dlt;
+            if (per[a]) { if (v < 0) v += nt[a]; if (v >= nt[a]) v -= nt[a]; }
+            if (v < 0 || v >= nt[a]) return -1;
+            t[a] = v;
+        }
+        return t[0] + nt[0] * (t[1] + nt[1] * t[2]);
+    }
+};
+
+__global__ void __launch_bounds__(REBIN_TPB) rebin_count_kernel(RebinGeom G, const int32_t *cell, const int32_t *tile_off,
+                                                                int32_t *class_count /* [ntiles][28] */, int32_t *tile_count) {
+    __shared__ int cnt[REBIN_CLASSES];
+    const int src = blockIdx.x;
+    int s[3] = { src % G.nt[0], (src / G.nt[0]) % G.nt[1], src / (G.nt[0] * G.nt[1]) };
+    if (threadIdx.x < REBIN_CLASSES) cnt[threadIdx.x] = 0;
+    __syncthreads();
+    const long long p0 = tile_off[src], p1 = tile_off[src + 1];
+    for (long long base = p0; base < p1; base += REBIN_TPB) {
+        long long p = base + threadIdx.x;
+        int rel = -1, td = 0;
+        if (p < p1) { int t[3]; G.tile_of_cell(cell[p], t); rel = G.classify(s, t); td = t[0] + G.nt[0] * (t[1] + G.nt[1] * t[2]); }
+        unsigned m = __match_any_sync(0xffffffffu, rel);
+        if (rel >= 0) {
+            if (rel == 27) atomicAdd(tile_count + td, 1);
+            else if ((int)(__ffs(m) - 1) == (int)(threadIdx.x & 31)) atomicAdd(&cnt[rel], __popc(m));
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < REBIN_CLASSES) {
+        int c = cnt[threadIdx.x];
+        class_count[(long long)src * REBIN_CLASSES + threadIdx.x] = c;
+        if (threadIdx.x < 27 && c > 0) { int d = G.dest_tile(s, threadIdx.x); atomicAdd(tile_count + d, c); }
+    }
+}
+
+__global__ void __launch_bounds__(REBIN_TPB) rebin_scatter_kernel(RebinGeom G, const int32_t *tile_off, const int32_t *class_count,
+                                                                  int32_t *cursor, PartPtrs in, PartPtrs out, int axisym,
+                                                                  unsigned *tile_wmax_bits) {
+    __shared__ int base_s[REBIN_CLASSES], fill[REBIN_CLASSES], dest_s[REBIN_CLASSES];
+    __shared__ unsigned wmx[REBIN_CLASSES];
+    const int src = blockIdx.x;
+    int s[3] = { src % G.nt[0], (src / G.nt[0]) % G.nt[1], src / (G.nt[0] * G.nt[1]) };
+    if (threadIdx.x < REBIN_CLASSES) {
+        int c = class_count[(long long)src * REBIN_CLASSES + threadIdx.x];
+        int d = threadIdx.x < 27 ? G.dest_tile(s, threadIdx.x) : -1;
+        dest_s[threadIdx.x] = d;
+        base_s[threadIdx.x] = (threadIdx.x < 27 && c > 0) ? atomicAdd(cursor + d, c) : 0;
+        fill[threadIdx.x] = 0; wmx[threadIdx.x] = 0u;
+    }
+    __syncthreads();
+    const long long p0 = tile_off[src], p1 = tile_off[src + 1];
+    const int lane = threadIdx.x & 31;
+    for (long long base = p0; base < p1; base += REBIN_TPB) {
+        long long p = base + threadIdx.x;
+        int rel = -1, td = 0, c = 0;
+        if (p < p1) { c = in.cell[p]; int t[3]; G.tile_of_cell(c, t); rel = G.classify(s, t); td = t[0] + G.nt[0] * (t[1] + G.nt[1] * t[2]); }
+        unsigned m = __match_any_sync(0xffffffffu, rel);
+        if (rel < 0) continue;
+        const float w = in.w[p];
+        long long dst;
+        if (rel == 27) {
+            dst = atomicAdd(cursor + td, 1);
+            atomicMax(tile_wmax_bits + td, __float_as_uint(fabsf(w)));
+        } else {
+            int leader = __ffs(m) - 1, r0 = 0;
+            if (lane == leader) r0 = atomicAdd(&fill[rel], __popc(m));
+            r0 = __shfl_sync(m, r0, leader);
+            dst = (long long)base_s[rel] + r0 + __popc(m & ((1u << lane) - 1u));
+            atomicMax(&wmx[rel], __float_as_uint(fabsf(w)));
+        }
+        out.cell[dst] = c;
+        for (int a = 0; a < G.D; ++a) out.d[a][dst] = in.d[a][p];
+        for (int a = 0; a < 3; ++a) out.u[a][dst] = in.u[a][p];
+        out.w[dst] = w;
+        if (axisym) out.phi[dst] = in.phi[p];
+        if (in.tag) out.tag[dst] = in.tag[p];
+    }
+    __syncthreads();
+    if (threadIdx.x < 27 && dest_s[threadIdx.x] >= 0 && wmx[threadIdx.x]) atomicMax(tile_wmax_bits + dest_s[threadIdx.x], wmx[threadIdx.x]);
+}
+
 }  // namespace ent

@@ -33,7 +33,24 @@ def _workloads(synth):
     }
 
 
-def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True):
+def _match_perm(g, p_from, p_to):
+    """ent_sort permutes every array alike and leaves the order inside a cell (or, re-binning, inside a tile) unspecified
+    (G18): the permutation is recovered by matching records -- (cell, offsets, momentum) is unique per particle in these
+    workloads.  Returns perm with p_to[k] == p_from[perm[k]], and checks that every array was permuted alike."""
+    def rank(p):
+        cols = [p.u[0], p.d[1], p.d[0], p.cell] if g.D == 2 else [p.u[0], p.d[2], p.d[1], p.d[0], p.cell]
+        return np.lexsort([c.detach().cpu().numpy() for c in cols])
+    r_from, r_to = rank(p_from), rank(p_to)
+    perm = np.empty(p_from.n, dtype=np.int64)
+    perm[r_to] = r_from
+    pt = torch.from_numpy(perm).to(p_from.cell.device)
+    same = lambda a, b: (a is None and b is None) or torch.equal(b, a[pt])
+    assert same(p_from.cell, p_to.cell) and same(p_from.w, p_to.w) and same(p_from.phi, p_to.phi) and same(p_from.tag, p_to.tag)
+    assert all(same(a, b) for a, b in zip(p_from.d + p_from.u, p_to.d + p_to.u)), "ent_sort is not a permutation of the records"
+    return perm
+
+
+def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True, resort_every=0):
     bind, synth, ctx, orc = env
     g = wl.grid
     eg, og = P.grid_to_ent(bind, g), P.grid_to_orc(orc, g)
@@ -48,24 +65,27 @@ def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True
         po = P.species_to_orc(orc, sp)
         order = None
         if sort_first:
-            # ent_sort permutes every array alike; the order inside a cell is unspecified (G18), so the permutation is
-            # recovered by matching records: (cell, offsets, momentum) is unique per particle in these workloads
             ps = pe.empty_like()
-            bind.ent_sort(ctx, pe, ps, None)
-
-            def rank(p):
-                cols = [p.u[0], p.d[1], p.d[0], p.cell] if g.D == 2 else [p.u[0], p.d[2], p.d[1], p.d[0], p.cell]
-                return np.lexsort([c.detach().cpu().numpy() for c in cols])
-            r_in, r_out = rank(pe), rank(ps)
-            order = np.empty(pe.n, dtype=np.int64)
-            order[r_out] = r_in                                   # sorted particle k is original particle order[k]
-            ot = torch.from_numpy(order).cuda()
-            assert torch.equal(ps.cell, pe.cell[ot]) and torch.equal(ps.u[2], pe.u[2][ot]) and torch.equal(ps.w, pe.w[ot]), \
-                "ent_sort is not a permutation of the records"
+            bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 1)       # full cell-level sort (a fresh tensor may reuse the address of
+            bind.ent_sort(ctx, pe, ps, None)                      # a block sorted earlier, which would select the re-bin form)
+            bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 0)
+            assert bind.ent_get_stat(ctx, bind.STAT_LAST_SORT_REBIN) == 0
+            order = _match_perm(g, pe, ps)
             pe = ps
         Jg = bind.zeros_current(eg, "cuda")
         worstJ = worstC = 0.0
         for s in range(steps):
+            if resort_every and s > 0 and s % resort_every == 0:
+                # incremental ent_sort (re-bin) of the drifted block: tile contiguity only
+                ps = pe.empty_like()
+                bind.ent_sort(ctx, pe, ps, None)
+                assert bind.ent_get_stat(ctx, bind.STAT_LAST_SORT_REBIN) == 1
+                perm = _match_perm(g, pe, ps)
+                order = order[perm]
+                T = [bind.ent_get_stat(ctx, k) for k in (bind.STAT_TILE_1, bind.STAT_TILE_2, bind.STAT_TILE_3)][:g.D]
+                tile = (synth.sort_key(g, synth.unpack_cell(g, ps.cell.cpu()), tuple(T)) // int(np.prod(T))).numpy()
+                assert np.all(np.diff(tile) >= 0), "re-binned block is not tile-contiguous"
+                pe = ps
             before = P.ent_to_orc(orc, g, pe) if check_every_step else None
             bind.ent_zero_current(ctx, Jg)
             bind.ent_step(ctx, F_dev, pe, Jg, wl.dt)
@@ -114,3 +134,13 @@ def test_sorted_step_auto_path_matches_oracle(env, name):
     print(name, stats)
     if wl.grid.kind == env[1].CART:
         assert all(st["tiled"] == 1 for st in stats.values()), "the tiled kernel did not run on a sorted Cartesian block"
+
+
+@pytest.mark.parametrize("name", ["C1", "C3/8", "C4/16-shuffled", "C5/32"])
+def test_rebinned_block_matches_oracle(env, name):
+    """ent_sort, steps, incremental ent_sort (re-bin) every 3 steps, steps: the tiled kernel on re-binned blocks"""
+    wl = _workloads(env[1])[name]()
+    stats = _run_case(env, wl, impl=0, sort_first=True, resort_every=3)
+    print(name, stats)
+    if wl.grid.kind == env[1].CART:
+        assert all(st["tiled"] == 1 and st["strays"] == 0 for st in stats.values())
