@@ -40,6 +40,22 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed ncu --set full capture
+# (profiles/r1_step_kernel_C3.md, section 2, current build); None where no capture exists
+NCU_TRAFFIC_BYTES = {"C3": 5.30e9}
+
+
+def max_over_ranks(value: float, device) -> float:
+    """time-like quantities are reduced with MAX over the ranks of the job (no-op for a single process)"""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def _load_workload(name, shrink, device, rank=0):
     from paper_2511_17710_b200 import synth
     if name == "C4s":
@@ -89,7 +105,7 @@ class ClockSampler:
         return out
 
 
-def _oracle_sample(name, target_particles=2_000_000):
+def _oracle_sample(name, target_particles=20_000_000):
     """a bounded sample of the same recipe for the CPU oracle: the workload with every grid extent divided by `shrink`"""
     from paper_2511_17710_b200 import synth
     full = {"C1": 65536, "C2": 2097152, "C3": 134217728, "C4": 536870912, "C4s": 536870912, "C5": 268435456}[name]
@@ -126,7 +142,7 @@ def time_oracle(name, steps, warmup):
         one()
     dt = time.perf_counter() - t0
     sample = f"{name} recipe with every grid extent / {shrink}: grid {tuple(wl.grid.N)}, {npart} particles, {steps} steps"
-    return dt / (npart * steps) * 1e9, orc.num_threads(), sample, dt / steps * 1e3
+    return dt / (npart * steps) * 1e9, orc.num_threads(), sample, dt / steps * 1e3, f"{wl.name} ({wl.note})"
 
 
 def run_reference(args):
@@ -134,10 +150,10 @@ def run_reference(args):
     if rank != 0:
         return
     steps, warmup = max(1, min(args.steps, 3)), min(args.warmup, 1)
-    v, cores, sample, ms = time_oracle(args.workload, steps, warmup)
+    v, cores, sample, ms, wname = time_oracle(args.workload, steps, warmup)
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps, "warmup": warmup,
             "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "note": "fp64 CPU oracle on a bounded sample of the workload"},
+            "config": {"workload": wname, "note": "fp64 CPU oracle (oracle/orc.c, as it stands) on a bounded sample of the workload"},
             "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line))
@@ -233,10 +249,7 @@ def run_ours(args):
     tiled = bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED)
     strays = bind.ent_get_stat(ctx, bind.STAT_STRAYS)
     bad = bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES)
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dev)
     ms_per_step = ms / args.steps
     value = ms * 1e6 / (npart * world * args.steps)
 
@@ -246,7 +259,8 @@ def run_ours(args):
     alg_bytes = pbytes * n_launch_part + GRID_BYTES_PER_CELL * ncell
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
     sort_ms = (sum(a.elapsed_time(b) for a, b in sort_ev) / len(sort_ev)) if sort_ev else None
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": args.traffic,
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": args.traffic if args.traffic is not None else (NCU_TRAFFIC_BYTES.get(args.workload) if args.shrink == 1 else None),
                 "kernel": "ent_step (fused gather+push+move+deposit), one species per launch", "kernel_ms": k_ms,
                 "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
                 "step_share": k_ms * len(parts) / ms_per_step}
@@ -280,10 +294,7 @@ def run_ours(args):
                 up += u_; down += d_
         barrier()
         e_ms = (time.perf_counter() - w0) * 1e3
-        if world > 1:
-            t = torch.tensor([e_ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e_ms = float(t.item())
+        e_ms = max_over_ranks(e_ms, dev)
         line["e2e"] = {"value": e_ms * 1e6 / (npart * world * nst), "unit": UNIT, "h2d_bytes_per_step": up, "d2h_bytes_per_step": down,
                        "steps": nst, "ms_per_step": e_ms / nst, "call": "ent_step_host per species (pinned host buffers)"}
         del hp, hF, hJ
@@ -291,7 +302,7 @@ def run_ours(args):
 
     if rank == 0:
         if not args.no_cpu and world == 1:
-            v, cores, sample, _ = time_oracle(args.workload, 2, 1)
+            v, cores, sample, _, _ = time_oracle(args.workload, 2, 1)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
         print(json.dumps(line))
     if world > 1:
@@ -312,7 +323,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--traffic", type=float, default=None, help="dram bytes per launch from an ncu --set full capture (profiles/)")
+    ap.add_argument("--traffic", type=float, default=None, help="dram bytes per launch of the dominant kernel from an ncu --set full capture (default: the committed one in profiles/)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -346,10 +346,18 @@ __global__ void __launch_bounds__(REBIN_TPB) rebin_scatter_kernel(RebinGeom G, c
     for (long long base = p0; base < p1; base += REBIN_TPB) {
         long long p = base + threadIdx.x;
         int rel = -1, td = 0, c = 0;
-        if (p < p1) { c = in.cell[p]; int t[3]; G.tile_of_cell(c, t); rel = G.classify(s, t); td = t[0] + G.nt[0] * (t[1] + G.nt[1] * t[2]); }
+        // the whole record is loaded before the destination is known (the loads do not depend on it): one round trip
+        float rd[3] = {0.f, 0.f, 0.f}, ru[3] = {0.f, 0.f, 0.f}, w = 0.f, rphi = 0.f; uint8_t rtag = 1;
+        if (p < p1) {
+            c = in.cell[p];
+            for (int a = 0; a < 3; ++a) { if (a < G.D) rd[a] = in.d[a][p]; ru[a] = in.u[a][p]; }
+            w = in.w[p];
+            if (axisym) rphi = in.phi[p];
+            if (in.tag) rtag = in.tag[p];
+            int t[3]; G.tile_of_cell(c, t); rel = G.classify(s, t); td = t[0] + G.nt[0] * (t[1] + G.nt[1] * t[2]);
+        }
         unsigned m = __match_any_sync(0xffffffffu, rel);
         if (rel < 0) continue;
-        const float w = in.w[p];
         long long dst;
         if (rel == 27) {
             dst = atomicAdd(cursor + td, 1);
@@ -359,14 +367,14 @@ __global__ void __launch_bounds__(REBIN_TPB) rebin_scatter_kernel(RebinGeom G, c
             if (lane == leader) r0 = atomicAdd(&fill[rel], __popc(m));
             r0 = __shfl_sync(m, r0, leader);
             dst = (long long)base_s[rel] + r0 + __popc(m & ((1u << lane) - 1u));
-            atomicMax(&wmx[rel], __float_as_uint(fabsf(w)));
+            unsigned wb = __reduce_max_sync(m, __float_as_uint(fabsf(w)));
+            if (lane == leader) atomicMax(&wmx[rel], wb);
         }
         out.cell[dst] = c;
-        for (int a = 0; a < G.D; ++a) out.d[a][dst] = in.d[a][p];
-        for (int a = 0; a < 3; ++a) out.u[a][dst] = in.u[a][p];
+        for (int a = 0; a < 3; ++a) { if (a < G.D) out.d[a][dst] = rd[a]; out.u[a][dst] = ru[a]; }
         out.w[dst] = w;
-        if (axisym) out.phi[dst] = in.phi[p];
-        if (in.tag) out.tag[dst] = in.tag[p];
+        if (axisym) out.phi[dst] = rphi;
+        if (in.tag) out.tag[dst] = rtag;
     }
     __syncthreads();
     if (threadIdx.x < 27 && dest_s[threadIdx.x] >= 0 && wmx[threadIdx.x]) atomicMax(tile_wmax_bits + dest_s[threadIdx.x], wmx[threadIdx.x]);
