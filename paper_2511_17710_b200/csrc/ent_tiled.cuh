@@ -170,7 +170,10 @@ __device__ __forceinline__ void acc_fixed4(int *sJ, const CarryCtx &cc, int comp
     }
 }
 #ifndef ENT_TILED_MINB
-#define ENT_TILED_MINB 2
+#define ENT_TILED_MINB 3
+#endif
+#ifndef ENT_TILED_VEC4
+#define ENT_TILED_VEC4 0
 #endif
 
 constexpr int TILED_TPB = 256;
@@ -380,6 +383,7 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     __syncthreads();                                             // sJ zeroed, mbarrier initialised
     bool waited = false;
 
+#if ENT_TILED_VEC4
     // ---- groups of four consecutive particles per thread (128-bit accesses; consecutive lanes are four particles apart).
     // A group that straddles the ends of the tile's range [p0, p1) is shared with the neighbouring tile's CTA: each side
     // touches only its own particles, with scalar accesses.
@@ -449,6 +453,26 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
             for (int k = 0; k < 4; ++k) if (code[k] == 2) A.P.tag[pb + k] = 0;
         }
     }
+#else
+    // ---- one particle per thread and iteration, consecutive lanes on consecutive particles: every access is a fully
+    // coalesced 128-byte line per warp, the work of a tile is balanced to within one particle per thread, and the order of the
+    // particles inside the tile's range does not matter (the incremental ent_sort does not keep one)
+    for (long long p = p0 + tid; p < p1; p += TILED_TPB) {
+        int cell = A.P.cell[p];
+        float d[3] = { A.P.d[0][p], A.P.d[1][p], (D == 3) ? A.P.d[2][p] : 0.f };
+        float u[3] = { A.P.u[0][p], A.P.u[1][p], A.P.u[2][p] };
+        const float wgt = A.P.w[p];
+        const bool live = A.P.tag ? A.P.tag[p] != 0 : true;
+        if (!waited) { mbar_wait(&bar, 0); waited = true; }
+        if (!live) continue;
+        const int code = tile_particle<D, TX, TY, TZ, ALLPER>(A, T, p, cell, d, u, wgt);
+        if (code & 1) continue;
+        A.P.cell[p] = cell;
+        A.P.d[0][p] = d[0]; A.P.d[1][p] = d[1]; if (D == 3) A.P.d[2][p] = d[2];
+        A.P.u[0][p] = u[0]; A.P.u[1][p] = u[1]; A.P.u[2][p] = u[2];
+        if (!ALLPER && code == 2) A.P.tag[p] = 0;
+    }
+#endif
     if (!waited) mbar_wait(&bar, 0);          // never leave with a TMA load still in flight into this CTA's shared memory
     // ---- S8 flush: one TMA reduce-add per component into the un-wrapped padded J (ghost fold = ent_fold_current)
     __syncthreads();
