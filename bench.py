@@ -182,6 +182,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     ctx = bind.ent_create(local, stream)
     bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, args.step_impl)
+    bind.ent_set_option(ctx, bind.OPT_SORT_MODE, args.sort_mode)
     if args.tile:
         for k, t in zip((bind.OPT_TILE_1, bind.OPT_TILE_2, bind.OPT_TILE_3), (int(x) for x in args.tile.split(","))):
             bind.ent_set_option(ctx, k, t)
@@ -319,6 +320,7 @@ def main():
     ap.add_argument("--shrink", type=int, default=1)
     ap.add_argument("--sort-every", type=int, default=3, help="ent_sort every k steps inside the timed region (0 = never)")
     ap.add_argument("--step-impl", type=int, default=0, help="ENT_OPT_STEP_IMPL: 0 auto, 1 untiled, 2 two-kernel")
+    ap.add_argument("--sort-mode", type=int, default=0, help="ENT_OPT_SORT_MODE: 0 auto (incremental re-bin), 1 always the full sort")
     ap.add_argument("--tile", default="", help="tile extents in cells, e.g. 8,8,8 (ENT_OPT_TILE_*; default: the library's)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")

@@ -172,6 +172,9 @@ __device__ __forceinline__ void acc_fixed4(int *sJ, const CarryCtx &cc, int comp
 #ifndef ENT_TILED_MINB
 #define ENT_TILED_MINB 3
 #endif
+#ifndef ENT_TILED_PREFETCH
+#define ENT_TILED_PREFETCH 1
+#endif
 #ifndef ENT_TILED_VEC4
 #define ENT_TILED_VEC4 0
 #endif
@@ -457,6 +460,35 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     // ---- one particle per thread and iteration, consecutive lanes on consecutive particles: every access is a fully
     // coalesced 128-byte line per warp, the work of a tile is balanced to within one particle per thread, and the order of the
     // particles inside the tile's range does not matter (the incremental ent_sort does not keep one)
+#if ENT_TILED_PREFETCH
+    // software pipeline: the record of the thread's next particle is requested before the current one is advanced
+    long long p = p0 + tid;
+    int ncell = 0; float nd0 = 0.f, nd1 = 0.f, nd2 = 0.f, nu0 = 0.f, nu1 = 0.f, nu2 = 0.f, nw = 0.f; bool nlive = true;
+    if (p < p1) {
+        ncell = A.P.cell[p]; nd0 = A.P.d[0][p]; nd1 = A.P.d[1][p]; if (D == 3) nd2 = A.P.d[2][p];
+        nu0 = A.P.u[0][p]; nu1 = A.P.u[1][p]; nu2 = A.P.u[2][p]; nw = A.P.w[p];
+        if (A.P.tag) nlive = A.P.tag[p] != 0;
+    }
+    for (; p < p1; p += TILED_TPB) {
+        int cell = ncell;
+        float d[3] = { nd0, nd1, nd2 }, u[3] = { nu0, nu1, nu2 };
+        const float wgt = nw; const bool live = nlive;
+        const long long pn = p + TILED_TPB;
+        if (pn < p1) {
+            ncell = A.P.cell[pn]; nd0 = A.P.d[0][pn]; nd1 = A.P.d[1][pn]; if (D == 3) nd2 = A.P.d[2][pn];
+            nu0 = A.P.u[0][pn]; nu1 = A.P.u[1][pn]; nu2 = A.P.u[2][pn]; nw = A.P.w[pn];
+            if (A.P.tag) nlive = A.P.tag[pn] != 0;
+        }
+        if (!waited) { mbar_wait(&bar, 0); waited = true; }
+        if (!live) continue;
+        const int code = tile_particle<D, TX, TY, TZ, ALLPER>(A, T, p, cell, d, u, wgt);
+        if (code & 1) continue;
+        A.P.cell[p] = cell;
+        A.P.d[0][p] = d[0]; A.P.d[1][p] = d[1]; if (D == 3) A.P.d[2][p] = d[2];
+        A.P.u[0][p] = u[0]; A.P.u[1][p] = u[1]; A.P.u[2][p] = u[2];
+        if (!ALLPER && code == 2) A.P.tag[p] = 0;
+    }
+#else
     for (long long p = p0 + tid; p < p1; p += TILED_TPB) {
         int cell = A.P.cell[p];
         float d[3] = { A.P.d[0][p], A.P.d[1][p], (D == 3) ? A.P.d[2][p] : 0.f };
@@ -472,6 +504,7 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
         A.P.u[0][p] = u[0]; A.P.u[1][p] = u[1]; A.P.u[2][p] = u[2];
         if (!ALLPER && code == 2) A.P.tag[p] = 0;
     }
+#endif
 #endif
     if (!waited) mbar_wait(&bar, 0);          // never leave with a TMA load still in flight into this CTA's shared memory
     // ---- S8 flush: one TMA reduce-add per component into the un-wrapped padded J (ghost fold = ent_fold_current)
