@@ -7,7 +7,7 @@
 #include <new>
 
 #include "ent_kernels.cuh"
-#include "ent_tiled.cuh"
+#include "ent_tiled_axisym.cuh"
 
 using namespace ent;
 
@@ -37,7 +37,7 @@ struct ent_ctx {
     // the blocks ent_sort produced (most recent first): each keeps its own tile offsets so that several species
     // can stay "sorted" at the same time
     struct SortedBlock { const int32_t *cell = nullptr; long long n = -1; int32_t *tile_off = nullptr; size_t cap = 0;
-                         float *tile_wmax = nullptr; size_t wcap = 0; unsigned long long stamp = 0; };
+                         float *tile_wmax = nullptr; size_t wcap = 0; int32_t *chunk_off = nullptr; size_t ccap = 0; unsigned long long stamp = 0; };
     SortedBlock sorted[8];
     unsigned long long sort_stamp = 0;
     int last_step_tiled = 0;
@@ -102,7 +102,7 @@ extern "C" int ent_destroy(ent_ctx *ctx) {
     tiled_release(ctx->tiled);
     cudaFree(ctx->counters); cudaFree(ctx->keys); cudaFree(ctx->count); cudaFree(ctx->offsets); cudaFree(ctx->cursor);
     cudaFree(ctx->chunk); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf); cudaFree(ctx->class_count);
-    for (auto &b : ctx->sorted) { cudaFree(b.tile_off); cudaFree(b.tile_wmax); }
+    for (auto &b : ctx->sorted) { cudaFree(b.tile_off); cudaFree(b.tile_wmax); cudaFree(b.chunk_off); }
     cudaGetLastError();
     delete ctx;
     return ENT_OK;
@@ -306,11 +306,11 @@ extern "C" int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, en
     if (p->n == 0) return ENT_OK;
     if (ctx->step_impl == 2) return step_two_kernel(ctx, EB, p, J, dt);
     float eps = 0.5f * (p->q / p->m) * dt;
-    const int32_t *tile_off = nullptr; const float *tile_wmax = nullptr;
-    for (auto &b : ctx->sorted) if (b.cell == p->cell && b.n == p->n) { tile_off = b.tile_off; tile_wmax = b.tile_wmax; }
+    const int32_t *tile_off = nullptr, *chunk_off = nullptr; const float *tile_wmax = nullptr;
+    for (auto &b : ctx->sorted) if (b.cell == p->cell && b.n == p->n) { tile_off = b.tile_off; tile_wmax = b.tile_wmax; chunk_off = b.chunk_off; }
     if (ctx->step_impl == 0 && tile_off && tiled_supported(ctx->tiled, ctx->g)) {
         CK(cudaMemsetAsync(ctx->counters + 1, 0, sizeof(unsigned long long), ctx->stream));      // strays of THIS step
-        rc = tiled_step(ctx->tiled, ctx->g, ctx->stream, fp(EB), pp(p), cp(J), (long long)p->n, tile_off, tile_wmax, eps, dt, p->q,
+        rc = tiled_step(ctx->tiled, ctx->g, ctx->stream, fp(EB), pp(p), cp(J), (long long)p->n, tile_off, tile_wmax, chunk_off, eps, dt, p->q,
                         1.0f / dt, ctx->counters, &ctx->launches, ctx->err, sizeof(ctx->err));
         if (rc == ENT_OK) ctx->last_step_tiled = 1;
         return rc;
@@ -327,8 +327,23 @@ static int claim_slot(ent_ctx *ctx, const ent_ctx::SortedBlock *keep, long long 
     int rc;
     if ((rc = ensure(ctx, (void **)&slot->tile_off, &slot->cap, (size_t)(ntiles + 1) * 4))) return rc;
     if ((rc = ensure(ctx, (void **)&slot->tile_wmax, &slot->wcap, (size_t)ntiles * 4))) return rc;
+    if ((rc = ensure(ctx, (void **)&slot->chunk_off, &slot->ccap, (size_t)(ntiles + 1) * 4))) return rc;
     *res = slot;
     return ENT_OK;
+}
+
+// work list of the tiled step for a sorted block: chunk_off = exclusive scan of ceil(tile count / TILE_CHUNK)
+static int build_work_list(ent_ctx *ctx, ent_ctx::SortedBlock *slot, long long ntiles) {
+    const int nchunks = (int)((ntiles + SCAN_CHUNK - 1) / SCAN_CHUNK);
+    int rc;
+    tile_chunks_kernel<<<nblk(ntiles), TPB, 0, ctx->stream>>>(slot->tile_off, ntiles, TILE_CHUNK, ctx->count);
+    if ((rc = launch_check(ctx, "tile_chunks_kernel"))) return rc;
+    scan_reduce_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, ntiles, ctx->chunk);
+    if ((rc = launch_check(ctx, "scan_reduce_kernel"))) return rc;
+    scan_chunks_kernel<<<1, TPB, 0, ctx->stream>>>(ctx->chunk, nchunks);
+    if ((rc = launch_check(ctx, "scan_chunks_kernel"))) return rc;
+    scan_apply_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, ntiles, ctx->chunk, slot->chunk_off, ctx->cursor);
+    return launch_check(ctx, "scan_apply_kernel");
 }
 
 // incremental ent_sort: `in` is tile-contiguous (src), particles have drifted; re-establish tile contiguity in `out`
@@ -356,6 +371,7 @@ static int sort_rebin(ent_ctx *ctx, const ent_ctx::SortedBlock *src, const ent_p
     rebin_scatter_kernel<<<(unsigned)ntiles, REBIN_TPB, 0, ctx->stream>>>(G, src->tile_off, ctx->class_count, ctx->cursor, pp(in), pp(out),
                                                                         g.kind != ENT_CART, (unsigned *)slot->tile_wmax);
     if ((rc = launch_check(ctx, "rebin_scatter_kernel"))) return rc;
+    if ((rc = build_work_list(ctx, slot, ntiles))) return rc;
     out->q = in->q; out->m = in->m;
     slot->cell = out->cell; slot->n = in->n; slot->stamp = ++ctx->sort_stamp;
     ctx->last_sort_rebin = 1;
@@ -423,6 +439,7 @@ extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *ou
         if ((rc = launch_check(ctx, "tile_offsets_kernel"))) return rc;
         tile_wmax_kernel<<<(unsigned)ntiles, 128, 0, ctx->stream>>>(slot->tile_off, out->w, slot->tile_wmax);
         if ((rc = launch_check(ctx, "tile_wmax_kernel"))) return rc;
+        if ((rc = build_work_list(ctx, slot, ntiles))) return rc;
         slot->cell = out->cell; slot->n = n; slot->stamp = ++ctx->sort_stamp;
     }
     return ENT_OK;

@@ -229,6 +229,12 @@ __global__ void tile_offsets_kernel(const int32_t *key_off, int tcells, long lon
     if (t <= ntiles) tile_off[t] = key_off[t * tcells];
 }
 
+// chunks[t] = ceil(count of tile t / chunk): the number of CTAs the tiled step gives to tile t
+__global__ void tile_chunks_kernel(const int32_t *tile_off, long long ntiles, int chunk, int32_t *chunks) {
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < ntiles) chunks[t] = (tile_off[t + 1] - tile_off[t] + chunk - 1) / chunk;
+}
+
 // tile_wmax[t] = max |w| over the particles of tile t (scale of the tile's fixed-point J accumulation)
 __global__ void __launch_bounds__(128) tile_wmax_kernel(const int32_t *tile_off, const float *w, float *tile_wmax) {
     __shared__ float red[4];

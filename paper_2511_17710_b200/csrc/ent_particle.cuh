@@ -9,11 +9,10 @@ namespace ent {
 // di[] = un-wrapped cell shift per dimension (for the deposit), alive = false if it left through an ABSORB side.
 // eps = (q/m) dt / 2.
 // ---------------------------------------------------------------------------------------------------------
-template <int D, int KIND, class Loader>
-__device__ __forceinline__ void push_particle(const GridDev &g, const Loader &ld, int i[3], float d[3], float &phi,
-                                              float u[3], float eps, float dt, int di[3], bool &alive) {
-    float EB[6];
-    gather<D>(g, ld, i, d, EB);                                               // step 3, P:131-133
+// push_from_fields: everything after the gather (EB = the six interpolated contravariant components).
+template <int D, int KIND>
+__device__ __forceinline__ void push_from_fields(const GridDev &g, const float EB[6], int i[3], float d[3], float &phi,
+                                                 float u[3], float eps, float dt, int di[3], bool &alive) {
     float E[3], B[3];
     if (KIND == ENT_CART) {
         // step 4: A^hat = sqrt(h_ii) A^i; Cartesian code basis is already aligned with x,y,z
@@ -92,6 +91,14 @@ __device__ __forceinline__ void push_particle(const GridDev &g, const Loader &ld
     }
 }
 
+template <int D, int KIND, class Loader>
+__device__ __forceinline__ void push_particle(const GridDev &g, const Loader &ld, int i[3], float d[3], float &phi,
+                                              float u[3], float eps, float dt, int di[3], bool &alive) {
+    float EB[6];
+    gather<D>(g, ld, i, d, EB);                                               // step 3, P:131-133
+    push_from_fields<D, KIND>(g, EB, i, d, phi, u, eps, dt, di, alive);
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // S7 deposit for one particle (Eq. 6, step 8 P:155-157, "modified zig-zag" P:575).
 // i0[], a[] = old cell and offset; di[] = un-wrapped cell shift in {-1,0,1}; dn[] = new offset;
@@ -156,10 +163,12 @@ __device__ __forceinline__ float half_qw_v3(const GridDev &g, const int i0[3], c
     return (float)(0.5 * (double)qw * v3);
 }
 
+// gi / ii: the array the contributions are indexed in and the old cell's index in it (the padded global arrays and i0
+// itself for the global path; a shared-memory J tile and the cell's box coordinates for the tiled path).
 template <int D, int KIND, class Acc>
-__device__ __forceinline__ void deposit_particle(const GridDev &g, const Acc &acc, const int i0[3], const float a[3],
-                                                 const int di[3], const float dn[3], float phi0, float phi1,
-                                                 const float u[3], float qw, float inv_dt) {
+__device__ __forceinline__ void deposit_particle_at(const GridDev &g, const Acc &acc, const int i0[3], const float a[3],
+                                                    const int di[3], const float dn[3], float phi0, float phi1,
+                                                    const float u[3], float qw, float inv_dt, const GridDev &gi, const int ii[3]) {
     float D1[3], W1[3], D2[3], W2[3], b[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
@@ -170,14 +179,21 @@ __device__ __forceinline__ void deposit_particle(const GridDev &g, const Acc &ac
             D2[k] = b[k] - r;  W2[k] = 0.5f * (r + b[k]) - (float)di[k];
         } else { b[k] = 0.f; D1[k] = W1[k] = D2[k] = W2[k] = 0.f; }
     }
-    const long long s1 = g.P[0], s2 = (long long)g.P[0] * g.P[1];
-    long long base1 = pidx<D>(g, i0[0], i0[1], i0[2]);
+    const long long s1 = gi.P[0], s2 = (long long)gi.P[0] * gi.P[1];
+    long long base1 = pidx<D>(gi, ii[0], ii[1], ii[2]);
     long long base2 = base1 + di[0] + s1 * di[1] + (D == 3 ? s2 * di[2] : 0);   // un-wrapped: may point into the ghosts
     float Q = qw * inv_dt;
     float hv = 0.f;
     if (D == 2) hv = half_qw_v3<KIND>(g, i0, a, b, phi0, phi1, u, qw);
     deposit_segment<D>(acc, base1, s1, s2, D1, W1, Q, hv);
     deposit_segment<D>(acc, base2, s1, s2, D2, W2, Q, hv);
+}
+
+template <int D, int KIND, class Acc>
+__device__ __forceinline__ void deposit_particle(const GridDev &g, const Acc &acc, const int i0[3], const float a[3],
+                                                 const int di[3], const float dn[3], float phi0, float phi1,
+                                                 const float u[3], float qw, float inv_dt) {
+    deposit_particle_at<D, KIND>(g, acc, i0, a, di, dn, phi0, phi1, u, qw, inv_dt, g, i0);
 }
 
 }  // namespace ent

@@ -96,6 +96,8 @@ struct TiledArgs {
     PartPtrs P;
     const int32_t *key_off;       // tile offsets: tile t owns particles [key_off[t], key_off[t+1]) (ent_sort)
     const float *tile_wmax;       // max |w| over the particles of each tile (ent_sort)
+    const int32_t *chunk_off;     // work list: tile t is processed by CTAs [chunk_off[t], chunk_off[t+1]), TILE_CHUNK particles each
+    int ntiles;
     long long n;
     float eps, dt, q, inv_dt;
     float cdt[3];                 // dt / dx_d
@@ -180,6 +182,19 @@ __device__ __forceinline__ void acc_fixed4(int *sJ, const CarryCtx &cc, int comp
 #endif
 
 constexpr int TILED_TPB = 256;
+constexpr int TILE_CHUNK = 4096;              // particles per CTA: a heavy tile is shared by several CTAs, each with its own J tile
+
+// work-list lookup: the tile whose chunk range contains CTA `vb` (binary search in the exclusive scan), or -1
+__device__ __forceinline__ int find_tile(const int32_t *chunk_off, int ntiles, int vb) {
+    if (vb < ntiles) {                        // uniform plasma: one chunk per tile, chunk_off[t] == t (two independent loads)
+        int a = chunk_off[vb], b = chunk_off[vb + 1];
+        if (a == vb && b == vb + 1) return vb;
+    }
+    if (vb >= chunk_off[ntiles]) return -1;
+    int lo = 0, hi = ntiles;                  // invariant: chunk_off[lo] <= vb < chunk_off[hi]
+    while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (chunk_off[mid] <= vb) lo = mid; else hi = mid; }
+    return lo;
+}
 
 // deposit of one particle through global atomics (ent_particle.cuh), out of line: used by the few particles of a tile that
 // cannot deposit into its shared-memory J tile
@@ -348,7 +363,8 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     const GridDev &g = A.g;
     const int tid = threadIdx.x;
 
-    const int tile = blockIdx.x;
+    const int tile = find_tile(A.chunk_off, A.ntiles, blockIdx.x);
+    if (tile < 0) return;                                        // the grid is an upper bound of the work list
     const int t0 = tile % g.nt[0], t12 = tile / g.nt[0];
     const int t1 = (D == 3) ? t12 % g.nt[1] : t12, t2 = (D == 3) ? t12 / g.nt[1] : 0;
     TileCtx<D> T;
@@ -365,17 +381,20 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     }
     for (int k = tid; k < 3 * G::JNP / 4; k += TILED_TPB) reinterpret_cast<int4 *>(sJ)[k] = make_int4(0, 0, 0, 0);
 
-    const long long p0 = A.key_off[tile], p1 = A.key_off[tile + 1];
+    long long p0 = A.key_off[tile], p1 = A.key_off[tile + 1];
+    p0 += (long long)(blockIdx.x - A.chunk_off[tile]) * TILE_CHUNK;
+    if (p1 > p0 + TILE_CHUNK) p1 = p0 + TILE_CHUNK;
     float invSc;
     {
         // fixed-point scale of this tile.  Largest contribution: |q| wmax / dt * |D| * weight with |D| <= 1, weight <= 13/12
-        // (2D: J^3 = q w v^3 has no 1/dt); wmax = max |w| over the tile's particles (ent_sort).  It gets 24 bits, fewer in
-        // a dense tile so that ~8x the mean nodal current still fits the 32-bit accumulator (beyond that: carry_fix).
+        // (2D: J^3 = q w v^3 has no 1/dt); wmax = max |w| over the tile's particles (ent_sort).  It gets 24 bits; a nodal sum
+        // beyond 2^31 (128 such contributions adding coherently) wraps and is carried exactly (carry_fix).
         const float wm = A.tile_wmax[tile];
-        float qmax = fabsf(A.q) * wm * ((D == 2) ? fmaxf(A.inv_dt, 0.5f) : A.inv_dt) * 1.0834f;
-        float dens = (float)(p1 - p0) / (float)G::TCELLS;
-        float top = fminf(16777000.0f, 2.6e8f / fmaxf(dens, 1.0f));
-        float Sc = (qmax > 0.f && qmax < 1e37f) ? top / qmax : 0.f;
+        // |D_a| <= min(1, dt / dx_a): the rate q w D / dt is at most q w / min dx (2D: J^3 = q w v^3, |v^3| < 1, h33 = 1)
+        float rate = fminf(A.inv_dt, 1.02f * fmaxf(g.inv_dx[0], fmaxf(g.inv_dx[1], (D == 3) ? g.inv_dx[2] : 0.f)));
+        if (D == 2) rate = fmaxf(rate, 0.5f);
+        float qmax = fabsf(A.q) * wm * rate * 1.0834f;
+        float Sc = (qmax > 0.f && qmax < 1e37f) ? 16777000.0f / qmax : 0.f;
         if (!(Sc > 1e-30f && Sc < 1e30f)) Sc = 0.f;
         invSc = Sc > 0.f ? 1.0f / Sc : 0.f;
         T.Sc = Sc; T.wguard = Sc > 0.f ? 60.0f * wm : -1.0f;
@@ -566,8 +585,8 @@ inline int tiled_set_grid(TiledState &t, const GridDev &g, char *, size_t) {
             t.encode = (EncodeTiledFn)fn;
         else cudaGetLastError();
     }
-    // TMA needs 16-byte global strides: padded row length (N0 + 4) * 4 bytes, i.e. N0 % 4 == 0.  Cartesian grids only.
-    if (g.kind != ENT_CART || !t.encode || (g.P[0] % 4) != 0) return ENT_OK;
+    // TMA needs 16-byte global strides: padded row length (N0 + 4) * 4 bytes, i.e. N0 % 4 == 0.
+    if (!t.encode || (g.P[0] % 4) != 0) return ENT_OK;
     t.shape = tiled_find_shape(g);
     return ENT_OK;
 }
@@ -600,6 +619,9 @@ inline int tiled_encode(TiledState &t, const GridDev &g, const FieldPtrs &F, con
     return ENT_OK;
 }
 
+template <int KIND, int TX, int TY>
+__global__ void step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ TiledArgs A);   // ent_tiled_axisym.cuh
+
 template <int IDX, int D, int TX, int TY, int TZ>
 inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, char *err, size_t errn) {
     using G = TileGeom<D, TX, TY, TZ>;
@@ -607,25 +629,30 @@ inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, 
     if (rc) return rc;
     bool allper = true;
     for (int a = 0; a < D; ++a) allper &= A.g.bc[a] == ENT_PERIODIC;
-    auto kern = allper ? step_tiled_kernel<D, TX, TY, TZ, true> : step_tiled_kernel<D, TX, TY, TZ, false>;
-    const int slot = 2 * IDX + (allper ? 1 : 0);
+    void (*kern)(const TileMaps, const TiledArgs) = allper ? step_tiled_kernel<D, TX, TY, TZ, true> : step_tiled_kernel<D, TX, TY, TZ, false>;
+    int slot = 2 * IDX + (allper ? 1 : 0);
+    if constexpr (D == 2) {
+        if (A.g.kind == ENT_SPH) { kern = step_tiled_axisym_kernel<ENT_SPH, TX, TY>; slot = 12 + 2 * (IDX - 4); }
+        else if (A.g.kind == ENT_QSPH) { kern = step_tiled_axisym_kernel<ENT_QSPH, TX, TY>; slot = 13 + 2 * (IDX - 4); }
+    } else if (A.g.kind != ENT_CART) { snprintf(err, errn, "no 3D tiled kernel for this metric"); return ENT_EUNSUPPORTED; }
     if (!t.attr_set[slot]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM_BYTES);
         if (e != cudaSuccess) { snprintf(err, errn, "cudaFuncSetAttribute(smem %d) failed: %s", G::SMEM_BYTES, cudaGetErrorString(e)); return ENT_ECUDA; }
         t.attr_set[slot] = true;
     }
     const int ntiles = A.g.nt[0] * A.g.nt[1] * A.g.nt[2];
-    kern<<<ntiles, TILED_TPB, G::SMEM_BYTES, stream>>>(t.maps, A);
+    const long long grid = (long long)ntiles + A.n / TILE_CHUNK + 1;        // upper bound of the number of chunks
+    kern<<<(unsigned)grid, TILED_TPB, G::SMEM_BYTES, stream>>>(t.maps, A);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { snprintf(err, errn, "launch of step_tiled_kernel failed: %s", cudaGetErrorString(e)); return ENT_ECUDA; }
     return ENT_OK;
 }
 
 inline int tiled_step(TiledState &t, const GridDev &g, cudaStream_t stream, FieldPtrs F, PartPtrs P, CurrentPtrs J, long long n,
-                      const int32_t *key_off, const float *tile_wmax, float eps, float dt, float q, float inv_dt, unsigned long long *counters,
+                      const int32_t *key_off, const float *tile_wmax, const int32_t *chunk_off, float eps, float dt, float q, float inv_dt, unsigned long long *counters,
                       long long *launches, char *err, size_t errn) {
     TiledArgs A;
-    A.g = g; A.F = F; A.J = J; A.P = P; A.key_off = key_off; A.tile_wmax = tile_wmax; A.n = n;
+    A.g = g; A.F = F; A.J = J; A.P = P; A.key_off = key_off; A.tile_wmax = tile_wmax; A.chunk_off = chunk_off; A.ntiles = g.nt[0] * g.nt[1] * g.nt[2]; A.n = n;
     A.eps = eps; A.dt = dt; A.q = q; A.inv_dt = inv_dt; A.counters = counters;
     for (int a = 0; a < 3; ++a) A.cdt[a] = dt * g.inv_dx[a];
     A.divN0 = make_fastdiv((uint32_t)g.N[0]);

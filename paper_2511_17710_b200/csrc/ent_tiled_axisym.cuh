@@ -1,0 +1,164 @@
+// ent_tiled_axisym.cuh -- tiled fused step for the axisymmetric grids (SPH, QSPH), sm_100a.
+// Same structure as ent_tiled.cuh (TMA-staged E,B box, fixed-point shared-memory J tile, TMA reduce-add flush, one particle
+// per thread and iteration); the per-particle arithmetic is the one of ent_particle.cuh (fp64 coordinate maps, fp32 fields,
+// Boris and deposit), with the gather reading the box and the deposit writing the tile.  Boundaries: ABSORB in x1, AXIS in x2
+// (no periodic wrap), so a particle is local iff its cell lies within one cell of the tile.
+#pragma once
+#include "ent_tiled.cuh"
+
+namespace ent {
+
+struct BoxLoader {                       // gather() hands over the index inside a (FX x FY) box addressed like a padded array
+    const float *sF; int fnp;
+    __device__ __forceinline__ float operator()(int c, long long idx) const { return sF[c * fnp + (int)idx]; }
+};
+
+// a contribution that does not fit the tile's fixed-point range goes straight to the global array (J^3 = q w v^phi / (r sin theta)
+// is unbounded towards the axis, reading G8)
+__device__ __noinline__ void global_add(const CarryCtx &c, int comp, int off, float v) {
+    int bx = off % c.JX, r = off / c.JX, by = r % c.JY, bz = r / c.JY;
+    long long idx = c.gbase + bx + (long long)c.P0 * by + (long long)c.P01 * bz;
+    atomicAdd(c.J[comp] + idx, v);
+}
+struct TileAcc {                         // Acc of deposit_particle_at: fixed-point add into the shared J tile
+    int *sJ; const CarryCtx *cc; float Sc;
+    __device__ __forceinline__ void add(int comp, long long idx, float v) const {
+        float sv = v * Sc;
+        if (fabsf(sv) < 1.0e9f) acc_fixed(sJ, *cc, comp, (int)idx, sv);
+        else if (sv == sv) global_add(*cc, comp, (int)idx, v);
+    }
+};
+
+template <int KIND>
+__device__ __noinline__ void stray_step_axisym(const TiledArgs &A, long long p) {
+    const GridDev &g = A.g;
+    int i[3], i0[3], di[3]; float d[3] = {0.f, 0.f, 0.f}, a[3], u[3];
+    unpack_cell<2>(g, A.P.cell[p], i);
+    d[0] = A.P.d[0][p]; d[1] = A.P.d[1][p];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { u[k] = A.P.u[k][p]; a[k] = d[k]; i0[k] = i[k]; }
+    float phi = A.P.phi[p];
+    const float phi0 = phi;
+    GlobalFieldLoader ld{A.F.c};
+    bool alive = true;
+    push_particle<2, KIND>(g, ld, i, d, phi, u, A.eps, A.dt, di, alive);
+    A.P.cell[p] = pack_cell<2>(g, i);
+    A.P.d[0][p] = d[0]; A.P.d[1][p] = d[1];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) A.P.u[k][p] = u[k];
+    A.P.phi[p] = phi;
+    atomicAdd(A.counters + 1, 1ULL);
+    if (!alive) { A.P.tag[p] = 0; return; }
+    if (di[0] < -1 || di[0] > 1 || di[1] < -1 || di[1] > 1) { atomicAdd(A.counters + 0, 1ULL); return; }
+    GlobalAcc acc{A.J.c};
+    deposit_particle<2, KIND>(g, acc, i0, a, di, d, phi0, phi, u, A.q * A.P.w[p], A.inv_dt);
+}
+
+template <int KIND, int TX, int TY>
+__global__ void __launch_bounds__(TILED_TPB, 2)
+step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ TiledArgs A) {
+    using G = TileGeom<2, TX, TY, 1>;
+    extern __shared__ __align__(128) float smem[];
+    float *sF = smem;
+    int *sJ = reinterpret_cast<int *>(smem + 6 * G::FNP);
+    __shared__ uint64_t bar;
+    __shared__ CarryCtx s_cc;
+    const GridDev &g = A.g;
+    const int tid = threadIdx.x;
+    const int tile = find_tile(A.chunk_off, A.ntiles, blockIdx.x);
+    if (tile < 0) return;
+    const int o0 = (tile % g.nt[0]) * TX, o1 = (tile / g.nt[0]) * TY;
+
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        fence_mbar_init();
+        mbar_expect_tx(&bar, 6u * G::FN * 4u);
+#pragma unroll
+        for (int c = 0; c < 6; ++c) tma_load_box<2>(sF + c * G::FNP, &maps.F[c], &bar, o0, o1, 0);
+    }
+    for (int k = tid; k < 3 * G::JNP / 4; k += TILED_TPB) reinterpret_cast<int4 *>(sJ)[k] = make_int4(0, 0, 0, 0);
+
+    long long p0 = A.key_off[tile], p1 = A.key_off[tile + 1];
+    p0 += (long long)(blockIdx.x - A.chunk_off[tile]) * TILE_CHUNK;
+    if (p1 > p0 + TILE_CHUNK) p1 = p0 + TILE_CHUNK;
+    float Sc, invSc;
+    {   // fixed-point scale of this CTA's J tile.  A contribution is q w / dt * D * weight with |D_a| <= dt / sqrt(h_aa) (|v| < 1), i.e.
+        // at most |q| wmax / min sqrt(h_aa) over the tile (x 13/12); bounding |D| by 1 instead would waste ~10 bits on the
+        // log-r grids, where a particle moves ~1e-3 cells per step.  J^3 = q w v^phi / sqrt(h33) is of the same size except next
+        // to the axis, where the contributions that do not fit go to the global array (TileAcc).
+        const float wm = A.tile_wmax[tile];
+        double x1a = fmax(0.0, (double)o0 - 1.0), x1b = fmin((double)g.N[0], (double)(o0 + TX) + 1.0);
+        double x2a = fmax(0.0, (double)o1 - 1.0), x2b = fmin((double)g.N[1], (double)(o1 + TY) + 1.0);
+        double hmin = 1e300;
+        for (int c = 0; c < 6; ++c) {
+            Sph sp = sph_of_code<KIND>(g, (c & 1) ? x1b : x1a, c < 2 ? x2a : (c < 4 ? x2b : 0.5 * (x2a + x2b)));
+            hmin = fmin(hmin, fmin(sp.sh1, sp.sh2));
+        }
+        float rate = fminf(A.inv_dt, (float)(1.25 / hmin));              // 1/dt: |D| <= 1 always
+        float qmax = fabsf(A.q) * wm * fmaxf(rate, 1e-30f) * 1.0834f;
+        Sc = (qmax > 0.f && qmax < 1e37f) ? 16777000.0f / qmax : 0.f;
+        if (!(Sc > 1e-30f && Sc < 1e30f)) Sc = 0.f;
+        invSc = Sc > 0.f ? 1.0f / Sc : 0.f;
+    }
+    if (tid == 0) {
+        s_cc.J = A.J.c; s_cc.P0 = g.P[0]; s_cc.P01 = g.P[0] * g.P[1]; s_cc.unit = 4294967296.0f * invSc;
+        s_cc.JX = G::JX; s_cc.JY = G::JY; s_cc.JNP = G::JNP;
+        s_cc.gbase = (long long)o0 + (long long)g.P[0] * o1;
+    }
+    __syncthreads();
+    const TileAcc acc{sJ, &s_cc, Sc};
+    const BoxLoader ld{sF, G::FNP};
+    const float wguard = Sc > 0.f ? 60.0f * A.tile_wmax[tile] : -1.0f;
+    bool waited = false;
+
+    for (long long p = p0 + tid; p < p1; p += TILED_TPB) {
+        const int cell = A.P.cell[p];
+        float d[3] = { A.P.d[0][p], A.P.d[1][p], 0.f };
+        float u[3] = { A.P.u[0][p], A.P.u[1][p], A.P.u[2][p] };
+        float phi = A.P.phi[p];
+        const float wgt = A.P.w[p];
+        const bool live = A.P.tag[p] != 0;
+        if (!waited) { mbar_wait(&bar, 0); waited = true; }
+        if (!live) continue;
+        int i[3];
+        i[1] = A.divN0.div(cell); i[0] = cell - i[1] * g.N[0]; i[2] = 0;
+        const int b0 = i[0] - o0 + 2, b1 = i[1] - o1 + 2;
+        const bool local = ((unsigned)(b0 - 1) < (unsigned)(TX + 2)) & ((unsigned)(b1 - 1) < (unsigned)(TY + 2)) & (fabsf(wgt) <= wguard);
+        if (!local) { stray_step_axisym<KIND>(A, p); continue; }
+        // gather from the box: the box is addressed like a padded array of extents FX x FY whose "active" origin is the tile
+        // origin, so the cell's coordinates in it are (b - 2)
+        GridDev gb = g; gb.P[0] = G::FX; gb.P[1] = G::FY; gb.P[2] = 1;
+        const int ib[3] = { b0 - NG, b1 - NG, 0 };
+        float EB[6];
+        gather<2>(gb, ld, ib, d, EB);
+        const int i0[3] = { i[0], i[1], 0 };
+        const float a[3] = { d[0], d[1], 0.f };
+        const float phi0 = phi;
+        int di[3]; bool alive = true;
+        push_from_fields<2, KIND>(g, EB, i, d, phi, u, A.eps, A.dt, di, alive);
+        A.P.cell[p] = i[0] + g.N[0] * i[1];
+        A.P.d[0][p] = d[0]; A.P.d[1][p] = d[1];
+        A.P.u[0][p] = u[0]; A.P.u[1][p] = u[1]; A.P.u[2][p] = u[2];
+        A.P.phi[p] = phi;
+        if (!alive) { A.P.tag[p] = 0; continue; }
+        if (di[0] < -1 || di[0] > 1 || di[1] < -1 || di[1] > 1) { atomicAdd(A.counters + 0, 1ULL); continue; }
+        GridDev gj = g; gj.P[0] = G::JX; gj.P[1] = G::JY; gj.P[2] = 1;
+        deposit_particle_at<2, KIND>(g, acc, i0, a, di, d, phi0, phi, u, A.q * wgt, A.inv_dt, gj, ib);
+    }
+    if (!waited) mbar_wait(&bar, 0);
+    __syncthreads();
+    for (int k = tid; k < 3 * G::JNP / 4; k += TILED_TPB) {
+        int4 v = reinterpret_cast<int4 *>(sJ)[k];
+        reinterpret_cast<float4 *>(sJ)[k] = make_float4((float)v.x * invSc, (float)v.y * invSc, (float)v.z * invSc, (float)v.w * invSc);
+    }
+    fence_proxy_async_smem();
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) tma_reduce_add_box<2>(&maps.J[c], sJ + c * G::JNP, o0, o1, 0);
+        tma_commit();
+        tma_wait_read0();
+    }
+}
+
+}  // namespace ent

@@ -126,21 +126,19 @@ def test_two_kernel_step_matches_oracle(env, name):
     print(name, stats)
 
 
-@pytest.mark.parametrize("name", ["C1", "C2/4", "C3/8", "C4/16-shuffled", "C5/32"])
+@pytest.mark.parametrize("name", ["C1", "C2/4", "C3/8", "C4/16-shuffled", "C5/32", "SPH"])
 def test_sorted_step_auto_path_matches_oracle(env, name):
     """ent_sort, then ent_step on the sorted block (auto: the tiled kernel where it is supported)"""
     wl = _workloads(env[1])[name]()
     stats = _run_case(env, wl, impl=0, sort_first=True)
     print(name, stats)
-    if wl.grid.kind == env[1].CART:
-        assert all(st["tiled"] == 1 for st in stats.values()), "the tiled kernel did not run on a sorted Cartesian block"
+    assert all(st["tiled"] == 1 for st in stats.values()), "the tiled kernel did not run on a sorted block"
 
 
-@pytest.mark.parametrize("name", ["C1", "C3/8", "C4/16-shuffled", "C5/32"])
+@pytest.mark.parametrize("name", ["C1", "C2/4", "C3/8", "C4/16-shuffled", "C5/32", "SPH"])
 def test_rebinned_block_matches_oracle(env, name):
     """ent_sort, steps, incremental ent_sort (re-bin) every 3 steps, steps: the tiled kernel on re-binned blocks"""
     wl = _workloads(env[1])[name]()
     stats = _run_case(env, wl, impl=0, sort_first=True, resort_every=3)
     print(name, stats)
-    if wl.grid.kind == env[1].CART:
-        assert all(st["tiled"] == 1 and st["strays"] == 0 for st in stats.values())
+    assert all(st["tiled"] == 1 and st["strays"] == 0 for st in stats.values())
