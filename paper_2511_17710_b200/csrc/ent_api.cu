@@ -309,7 +309,7 @@ extern "C" int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, en
     const int32_t *tile_off = nullptr, *chunk_off = nullptr; const float *tile_wmax = nullptr;
     for (auto &b : ctx->sorted) if (b.cell == p->cell && b.n == p->n) { tile_off = b.tile_off; tile_wmax = b.tile_wmax; chunk_off = b.chunk_off; }
     if (ctx->step_impl == 0 && tile_off && tiled_supported(ctx->tiled, ctx->g)) {
-        CK(cudaMemsetAsync(ctx->counters + 1, 0, sizeof(unsigned long long), ctx->stream));      // strays of THIS step
+        CK(cudaMemsetAsync(ctx->counters + 1, 0, 2 * sizeof(unsigned long long), ctx->stream));  // strays of THIS step, stray-list length
         rc = tiled_step(ctx->tiled, ctx->g, ctx->stream, fp(EB), pp(p), cp(J), (long long)p->n, tile_off, tile_wmax, chunk_off, eps, dt, p->q,
                         1.0f / dt, ctx->counters, &ctx->launches, ctx->err, sizeof(ctx->err));
         if (rc == ENT_OK) ctx->last_step_tiled = 1;
@@ -357,7 +357,8 @@ static int sort_rebin(ent_ctx *ctx, const ent_ctx::SortedBlock *src, const ent_p
     if ((rc = claim_slot(ctx, src, ntiles, &slot))) return rc;
     RebinGeom G;
     G.D = g.D;
-    for (int a = 0; a < 3; ++a) { G.N[a] = g.N[a]; G.T[a] = g.T[a]; G.nt[a] = g.nt[a]; G.per[a] = g.bc[a] == ENT_PERIODIC; }
+    for (int a = 0; a < 3; ++a) { G.N[a] = g.N[a]; G.T[a] = g.T[a]; G.nt[a] = g.nt[a]; G.per[a] = g.bc[a] == ENT_PERIODIC; G.dT[a] = make_magicdiv((uint32_t)g.T[a]); }
+    G.dN0 = make_magicdiv((uint32_t)g.N[0]); G.dN01 = make_magicdiv((uint32_t)(g.N[0] * g.N[1]));
     CK(cudaMemsetAsync(ctx->count, 0, (size_t)(ntiles + 1) * 4, ctx->stream));
     CK(cudaMemsetAsync(slot->tile_wmax, 0, (size_t)ntiles * 4, ctx->stream));
     rebin_count_kernel<<<(unsigned)ntiles, REBIN_TPB, 0, ctx->stream>>>(G, in->cell, src->tile_off, ctx->class_count, ctx->count);

@@ -272,13 +272,28 @@ __global__ void __launch_bounds__(TPB) sort_scatter_kernel(const int32_t *keys, 
 constexpr int REBIN_TPB = 256;
 constexpr int REBIN_CLASSES = 28;            // 27 neighbours (3^D used) + "far"
 
+struct MagicDiv {                 // n / d for 0 <= n < 2^31, d >= 1 (multiply-high + shift)
+    uint32_t mul, shr, d;
+    __device__ __forceinline__ int div(int n) const { return d == 1 ? n : (int)(__umulhi((uint32_t)n, mul) >> shr); }
+};
+inline MagicDiv make_magicdiv(uint32_t d) {
+    MagicDiv f{0, 0, d};
+    if (d <= 1) return f;
+    uint32_t lg = 0; while ((1ull << lg) < d) ++lg;
+    uint32_t p = 31 + lg;
+    f.mul = (uint32_t)(((1ull << p) + d - 1) / d);
+    f.shr = p - 32;
+    return f;
+}
+
 struct RebinGeom {
     int D, N[3], T[3], nt[3], per[3];
+    MagicDiv dN0, dN01, dT[3];
     __device__ __forceinline__ void tile_of_cell(int cell, int t[3]) const {
         int i0, i1, i2 = 0;
-        if (D == 2) { i1 = cell / N[0]; i0 = cell - i1 * N[0]; }
-        else { int n01 = N[0] * N[1]; i2 = cell / n01; int r = cell - i2 * n01; i1 = r / N[0]; i0 = r - i1 * N[0]; }
-        t[0] = i0 / T[0]; t[1] = i1 / T[1]; t[2] = (D == 3) ? i2 / T[2] : 0;
+        if (D == 2) { i1 = dN0.div(cell); i0 = cell - i1 * N[0]; }
+        else { int n01 = N[0] * N[1]; i2 = dN01.div(cell); int r = cell - i2 * n01; i1 = dN0.div(r); i0 = r - i1 * N[0]; }
+        t[0] = dT[0].div(i0); t[1] = dT[1].div(i1); t[2] = (D == 3) ? dT[2].div(i2) : 0;
     }
     // class of destination tile t seen from source tile s: 0..26 = neighbour (dz+1)*9 + (dy+1)*3 + (dx+1), 27 = far
     __device__ __forceinline__ int classify(const int s[3], const int t[3]) const {

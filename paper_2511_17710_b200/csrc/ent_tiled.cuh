@@ -101,7 +101,8 @@ struct TiledArgs {
     long long n;
     float eps, dt, q, inv_dt;
     float cdt[3];                 // dt / dx_d
-    unsigned long long *counters; // [0] bad moves, [1] strays
+    unsigned long long *counters; // [0] bad moves, [1] strays, [2] length of stray_list
+    int32_t *stray_list; long long stray_cap;   // particles left to stray_kernel (all lanes busy there instead of one per warp here)
     FastDiv divN0, divN01;
 };
 
@@ -207,6 +208,13 @@ __device__ __noinline__ void edge_deposit(const TiledArgs &A, int i0, int i1, in
     deposit_particle<D, ENT_CART>(A.g, acc, i, a, di, dn, 0.f, 0.f, u, qw, A.inv_dt);
 }
 
+// a particle the tile cannot take: hand it to stray_kernel through the list, or advance it right here if the list is full
+template <class F>
+__device__ __forceinline__ void defer_stray(const TiledArgs &A, long long p, F &&fallback) {
+    unsigned long long k = atomicAdd(A.counters + 2, 1ULL);
+    if ((long long)k < A.stray_cap) A.stray_list[k] = (int32_t)p; else fallback();
+}
+
 // per-CTA constants of the tile loop
 template <int D>
 struct TileCtx {
@@ -245,7 +253,7 @@ __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D
         // at node N+2, outside the padded array -> it gathers from the box but deposits through the global path
         edge |= (T.o[a] - 2 + b[a] > g.N[a] - 1);
     }
-    if (!local) { stray_step<D>(A, p); return 1; }
+    if (!local) { defer_stray(A, p, [&] { stray_step<D>(A, p); }); return 1; }
     // ---- S1 gather from the shared-memory box (same stencil as ent_dev.cuh gather)
     float EBv[6];
     {
@@ -542,6 +550,15 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     }
 }
 
+// the strays of the last tiled launch, one per thread (global gathers, global atomics)
+template <int D>
+__global__ void __launch_bounds__(256) stray_kernel(const __grid_constant__ TiledArgs A) {
+    const unsigned long long cnt = A.counters[2];
+    const long long m = (long long)cnt < A.stray_cap ? (long long)cnt : A.stray_cap;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < m; k += (long long)gridDim.x * blockDim.x)
+        stray_step<D>(A, A.stray_list[k]);
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------
@@ -554,14 +571,15 @@ struct TiledState {
     EncodeTiledFn encode = nullptr;
     bool tried_encode = false;
     int shape = -1;                         // index into the instantiated tile shapes, -1 = none fits
+    int32_t *stray_list = nullptr; long long stray_cap = 0;
     const void *ptrF[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     const void *ptrJ[3] = {nullptr, nullptr, nullptr};
     TileMaps maps;
     bool attr_set[16] = {};
 };
 
-inline void tiled_release(TiledState &) {}
-inline size_t tiled_scratch_bytes(const TiledState &t) { return t.scratch; }
+inline void tiled_release(TiledState &t) { cudaFree(t.stray_list); t.stray_list = nullptr; t.stray_cap = 0; }
+inline size_t tiled_scratch_bytes(const TiledState &t) { return t.scratch + (size_t)t.stray_cap * 4; }
 
 // instantiated tile shapes: index -> (D, TX, TY, TZ)
 #define ENT_TILE_SHAPES(X) X(0, 3, 8, 8, 8) X(1, 3, 16, 8, 4) X(2, 3, 32, 4, 4) X(3, 3, 16, 8, 8) X(4, 2, 16, 16, 1) X(5, 2, 32, 8, 1)
@@ -622,6 +640,8 @@ inline int tiled_encode(TiledState &t, const GridDev &g, const FieldPtrs &F, con
 template <int KIND, int TX, int TY>
 __global__ void step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ TiledArgs A);   // ent_tiled_axisym.cuh
 
+template <int D> inline void launch_strays(const TiledArgs &A, cudaStream_t stream);      // after the axisymmetric kernels are known
+
 template <int IDX, int D, int TX, int TY, int TZ>
 inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, char *err, size_t errn) {
     using G = TileGeom<D, TX, TY, TZ>;
@@ -645,6 +665,9 @@ inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, 
     kern<<<(unsigned)grid, TILED_TPB, G::SMEM_BYTES, stream>>>(t.maps, A);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { snprintf(err, errn, "launch of step_tiled_kernel failed: %s", cudaGetErrorString(e)); return ENT_ECUDA; }
+    launch_strays<D>(A, stream);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) { snprintf(err, errn, "launch of stray_kernel failed: %s", cudaGetErrorString(e)); return ENT_ECUDA; }
     return ENT_OK;
 }
 
@@ -654,6 +677,15 @@ inline int tiled_step(TiledState &t, const GridDev &g, cudaStream_t stream, Fiel
     TiledArgs A;
     A.g = g; A.F = F; A.J = J; A.P = P; A.key_off = key_off; A.tile_wmax = tile_wmax; A.chunk_off = chunk_off; A.ntiles = g.nt[0] * g.nt[1] * g.nt[2]; A.n = n;
     A.eps = eps; A.dt = dt; A.q = q; A.inv_dt = inv_dt; A.counters = counters;
+    {   // stray list: room for 1/16 of the block (beyond that the tile kernel advances strays itself)
+        long long want = n / 16 + 4096;
+        if (t.stray_cap < want) {
+            if (t.stray_list) { cudaStreamSynchronize(stream); cudaFree(t.stray_list); t.stray_list = nullptr; t.stray_cap = 0; }
+            if (cudaMalloc((void **)&t.stray_list, (size_t)want * 4) != cudaSuccess) { cudaGetLastError(); snprintf(err, errn, "cudaMalloc of the stray list failed"); return ENT_ENOMEM; }
+            t.stray_cap = want;
+        }
+        A.stray_list = t.stray_list; A.stray_cap = t.stray_cap;
+    }
     for (int a = 0; a < 3; ++a) A.cdt[a] = dt * g.inv_dx[a];
     A.divN0 = make_fastdiv((uint32_t)g.N[0]);
     A.divN01 = make_fastdiv((uint32_t)(g.N[0] * g.N[1]));
@@ -664,7 +696,7 @@ inline int tiled_step(TiledState &t, const GridDev &g, cudaStream_t stream, Fiel
 #undef X
         default: snprintf(err, errn, "no tiled kernel for this tile shape"); break;
     }
-    if (rc == ENT_OK) *launches += 1;
+    if (rc == ENT_OK) *launches += 2;
     return rc;
 }
 

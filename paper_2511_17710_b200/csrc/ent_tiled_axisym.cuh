@@ -124,7 +124,7 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
         i[1] = A.divN0.div(cell); i[0] = cell - i[1] * g.N[0]; i[2] = 0;
         const int b0 = i[0] - o0 + 2, b1 = i[1] - o1 + 2;
         const bool local = ((unsigned)(b0 - 1) < (unsigned)(TX + 2)) & ((unsigned)(b1 - 1) < (unsigned)(TY + 2)) & (fabsf(wgt) <= wguard);
-        if (!local) { stray_step_axisym<KIND>(A, p); continue; }
+        if (!local) { defer_stray(A, p, [&] { stray_step_axisym<KIND>(A, p); }); continue; }
         // gather from the box: the box is addressed like a padded array of extents FX x FY whose "active" origin is the tile
         // origin, so the cell's coordinates in it are (b - 2)
         GridDev gb = g; gb.P[0] = G::FX; gb.P[1] = G::FY; gb.P[2] = 1;
@@ -159,6 +159,21 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
         tma_commit();
         tma_wait_read0();
     }
+}
+
+template <int KIND>
+__global__ void __launch_bounds__(256) stray_axisym_kernel(const __grid_constant__ TiledArgs A) {
+    const unsigned long long cnt = A.counters[2];
+    const long long m = (long long)cnt < A.stray_cap ? (long long)cnt : A.stray_cap;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < m; k += (long long)gridDim.x * blockDim.x)
+        stray_step_axisym<KIND>(A, A.stray_list[k]);
+}
+
+template <int D> inline void launch_strays(const TiledArgs &A, cudaStream_t stream) {
+    const int grid = 148 * 4;
+    if (A.g.kind == ENT_CART) stray_kernel<D><<<grid, 256, 0, stream>>>(A);
+    else if (A.g.kind == ENT_SPH) stray_axisym_kernel<ENT_SPH><<<grid, 256, 0, stream>>>(A);
+    else stray_axisym_kernel<ENT_QSPH><<<grid, 256, 0, stream>>>(A);
 }
 
 }  // namespace ent
