@@ -42,7 +42,7 @@ def _peaks():
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed ncu --set full capture
 # (profiles/r1_step_kernel_C3.md, section 2, current build); None where no capture exists
-NCU_TRAFFIC_BYTES = {"C3": 5.30e9}
+NCU_TRAFFIC_BYTES = {"C3": 5.33e9}
 
 
 def max_over_ranks(value: float, device) -> float:
