@@ -175,6 +175,7 @@ static int check_particles(ent_ctx *ctx, const ent_particles *p, const char *nam
     if (!p) return fail(ctx, ENT_EINVAL, "%s is NULL", name);
     if (p->n < 0) return fail(ctx, ENT_EINVAL, "%s->n < 0", name);
     if (p->n >= (1LL << 31)) return fail(ctx, ENT_EINVAL, "%s->n >= 2^31 (sort offsets are int32)", name);
+    if (p->n == 0) return ENT_OK;                         // an empty block needs no arrays
     const GridDev &g = ctx->g;
     if (!p->cell || !al16(p->cell)) return fail(ctx, ENT_EINVAL, "%s->cell NULL or not 16-byte aligned", name);
     for (int a = 0; a < g.D; ++a) if (!p->d[a] || !al16(p->d[a])) return fail(ctx, ENT_EINVAL, "%s->d[%d] NULL or misaligned", name, a);

@@ -445,4 +445,24 @@ def sph_small(N: int = 64, device="cpu") -> Workload:
     return Workload("SPH-small", grid, 0.5 * cfl_dx_min(grid), 20, fields, sp, seed, "linear-r spherical metric")
 
 
+def cart_absorb_small(D: int = 3, device="cpu") -> Workload:
+    """parity-only edge case: Cartesian box with ABSORB sides in x1 (and x3), periodic in x2, extents that are not multiples
+    of the tile (partial tiles), a particle count that is not a multiple of 4, hot plasma so that particles do leave"""
+    seed = 6
+    N = (20, 16, 12) if D == 3 else (36, 24)
+    bc = (ABSORB, PERIODIC, ABSORB) if D == 3 else (ABSORB, PERIODIC)
+    grid = GridSpec(D=D, N=N, bc=bc, kind=CART, xmin=(0.0,) * D, xmax=tuple(0.5 * n for n in N))
+    Um = uniform(seed, 8, 6 * 4 * 4, "cpu", dtype=torch.float64).view(6, 4, 4)
+    modes = [[(0.2, (int(Um[c, k, 0] * 3) + 1, int(Um[c, k, 1] * 3), int(Um[c, k, 2] * 3) if D == 3 else 0),
+               2.0 * math.pi * float(Um[c, k, 3])) for k in range(4)] for c in range(6)]
+    fields = _cart_fields_from_modes(grid, modes, (0, 0, 0, 0, 0, 1.0), device)
+    counts = torch.full((grid.ncells,), 3, dtype=torch.int64)
+    sp = load_pairs(grid, seed, counts, 0.5, 1.0, 1.0, device)
+    for s_ in sp:                                            # ragged tail: n % 4 == 1
+        keep = s_.n - 3
+        s_.i = [t[:keep].contiguous() for t in s_.i]; s_.d = [t[:keep].contiguous() for t in s_.d]
+        s_.u = [t[:keep].contiguous() for t in s_.u]; s_.w = s_.w[:keep].contiguous()
+    return Workload(f"CART-absorb-{D}D", grid, 0.45 * 0.5, 12, fields, sp, seed, "absorbing Cartesian box, partial tiles, ragged n")
+
+
 CONFIGS = {"C1": config1, "C2": config2, "C3": config3, "C4": config4, "C5": config5}

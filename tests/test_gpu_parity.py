@@ -30,6 +30,8 @@ def _workloads(synth):
         "C4/16-shuffled": lambda: synth.config4(16, shuffled=True),
         "C5/32": lambda: synth.config5(32),             # 64x64 quasi-spherical vartheta = 0.4, ~262k particles
         "SPH": lambda: synth.sph_small(48),             # linear-r spherical metric
+        "ABS3": lambda: synth.cart_absorb_small(3),     # absorbing Cartesian box, partial tiles, n % 4 != 0
+        "ABS2": lambda: synth.cart_absorb_small(2),
     }
 
 
@@ -111,7 +113,7 @@ def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True
     return out
 
 
-@pytest.mark.parametrize("name", ["C1", "C2/4", "C3/8", "C4/16", "C4/16-shuffled", "C5/32", "SPH"])
+@pytest.mark.parametrize("name", ["C1", "C2/4", "C3/8", "C4/16", "C4/16-shuffled", "C5/32", "SPH", "ABS3", "ABS2"])
 def test_fused_step_untiled_matches_oracle(env, name):
     wl = _workloads(env[1])[name]()
     stats = _run_case(env, wl, impl=1)
@@ -135,10 +137,54 @@ def test_sorted_step_auto_path_matches_oracle(env, name):
     assert all(st["tiled"] == 1 for st in stats.values()), "the tiled kernel did not run on a sorted block"
 
 
-@pytest.mark.parametrize("name", ["C1", "C2/4", "C3/8", "C4/16-shuffled", "C5/32", "SPH"])
+@pytest.mark.parametrize("name", ["C1", "C2/4", "C3/8", "C4/16-shuffled", "C5/32", "SPH", "ABS3", "ABS2"])
 def test_rebinned_block_matches_oracle(env, name):
     """ent_sort, steps, incremental ent_sort (re-bin) every 3 steps, steps: the tiled kernel on re-binned blocks"""
     wl = _workloads(env[1])[name]()
     stats = _run_case(env, wl, impl=0, sort_first=True, resort_every=3)
     print(name, stats)
     assert all(st["tiled"] == 1 and st["strays"] == 0 for st in stats.values())
+
+
+def test_empty_block_is_accepted(env):
+    """n = 0: every call returns ENT_OK and touches nothing (ent.h: n may be any value >= 0)"""
+    bind, synth, ctx, orc = env
+    wl = synth.config3(16)
+    eg = P.grid_to_ent(bind, wl.grid)
+    bind.ent_set_grid(ctx, eg)
+    F = [f.cuda() for f in wl.fields]
+    e = lambda dt: torch.empty(0, dtype=dt, device="cuda")
+    mk = lambda: bind.Particles(cell=e(torch.int32), d=[e(torch.float32) for _ in range(3)], u=[e(torch.float32) for _ in range(3)],
+                                w=e(torch.float32), q=-1.0, m=1.0)
+    p, p2 = mk(), mk()
+    J = bind.zeros_current(eg, "cuda")
+    bind.ent_step(ctx, F, p, J, wl.dt)
+    bind.ent_gather_push(ctx, F, p, p2, wl.dt)
+    bind.ent_deposit(ctx, p, p2, J, wl.dt)
+    torch.cuda.synchronize()
+    assert all(float(j.abs().max()) == 0.0 for j in J)
+
+
+def test_error_paths_on_device(env):
+    """misaligned / missing arrays and mismatched sizes are refused with ENT_EINVAL, nothing is launched"""
+    bind, synth, ctx, orc = env
+    wl = synth.config3(16)
+    g = wl.grid
+    eg = P.grid_to_ent(bind, g)
+    bind.ent_set_grid(ctx, eg)
+    F = [f.cuda() for f in wl.fields]
+    pe = P.species_to_ent(bind, synth, g, wl.species[0], "cuda", with_tag=False)
+    J = bind.zeros_current(eg, "cuda")
+    before = bind.ent_get_stat(ctx, bind.STAT_LAUNCHES)
+    bad = pe.clone(); bad.d[1] = torch.zeros(pe.n + 1, dtype=torch.float32, device="cuda")[1:]          # 4-byte aligned only
+    with pytest.raises(bind.EntError) as ei:
+        bind.ent_step(ctx, F, bad, J, wl.dt)
+    assert ei.value.code == bind.EINVAL
+    out = pe.empty_like(); out.cell = out.cell[:-1]
+    with pytest.raises(bind.EntError):
+        bind.ent_sort(ctx, pe, out, None)                                                               # in->n != out->n
+    with pytest.raises(bind.EntError):
+        bind.ent_sort(ctx, pe, pe, None)                                                                # not out of place
+    with pytest.raises(bind.EntError):
+        bind.ent_step(ctx, F, pe, J, -1.0)                                                              # dt <= 0
+    assert bind.ent_get_stat(ctx, bind.STAT_LAUNCHES) == before
