@@ -96,7 +96,7 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
         }
         float rate = fminf(A.inv_dt, (float)(1.25 / hmin));              // 1/dt: |D| <= 1 always
         float qmax = fabsf(A.q) * wm * fmaxf(rate, 1e-30f) * 1.0834f;
-        Sc = (qmax > 0.f && qmax < 1e37f) ? 16777000.0f / qmax : 0.f;
+        Sc = (qmax > 0.f && qmax < 1e37f) ? 67100000.0f / qmax : 0.f;       // 26 bits: weights vary strongly inside a tile of a coarse grid
         if (!(Sc > 1e-30f && Sc < 1e30f)) Sc = 0.f;
         invSc = Sc > 0.f ? 1.0f / Sc : 0.f;
     }
