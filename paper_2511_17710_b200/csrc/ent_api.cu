@@ -260,14 +260,15 @@ extern "C" int ent_fold_current(ent_ctx *ctx, ent_current *J) {
     int rc;
     if ((rc = check_current(ctx, J))) return rc;
     const GridDev &g = ctx->g;
-    for (int c = 0; c < 3; ++c)
-        for (int pass = 0; pass < 2; ++pass)
-            for (int d = 0; d < g.D; ++d) {
-                if (g.bc[d] != ENT_PERIODIC) continue;
-                long long nthreads = (long long)g.P[(d + 1) % 3] * g.P[(d + 2) % 3] * NG;
-                fold_kernel<<<nblk(nthreads), TPB, 0, ctx->stream>>>(g, J->comp[c], d, pass);
-                if ((rc = launch_check(ctx, "fold_kernel"))) return rc;
-            }
+    // all ghost layers are added onto the active cells (dimension after dimension, so that edges and corners arrive), then
+    // all ghost layers are refilled; the three components are independent and share a launch
+    for (int pass = 0; pass < 2; ++pass)
+        for (int d = 0; d < g.D; ++d) {
+            if (g.bc[d] != ENT_PERIODIC) continue;
+            long long nthreads = (long long)g.P[(d + 1) % 3] * g.P[(d + 2) % 3] * NG;
+            fold_kernel<<<dim3(nblk(nthreads), 3), TPB, 0, ctx->stream>>>(g, cp(J), d, pass);
+            if ((rc = launch_check(ctx, "fold_kernel"))) return rc;
+        }
     return ENT_OK;
 }
 

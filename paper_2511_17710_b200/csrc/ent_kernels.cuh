@@ -119,7 +119,8 @@ __global__ void __launch_bounds__(TPB) step_untiled_kernel(GridDev g, FieldPtrs 
 // pass 0: active += ghost on the opposite side, ghost = 0;  pass 1: ghost = periodic image.
 // One thread per (ghost layer gi, transverse point); the transverse range covers the whole padded extent so that
 // edges and corners are folded dimension after dimension.
-__global__ void fold_kernel(GridDev g, float *A, int dim, int pass) {
+__global__ void fold_kernel(GridDev g, CurrentPtrs J, int dim, int pass) {      // blockIdx.y = component
+    float *A = J.c[blockIdx.y];
     int a = (dim + 1) % 3, b = (dim + 2) % 3;
     long long na = g.P[a], nb = g.P[b];
     long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
