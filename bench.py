@@ -64,7 +64,8 @@ def _load_workload(name, shrink, device, rank=0):
 
 
 class ClockSampler:
-    """nvidia-smi sampled every 100 ms during the timed region (B200_PROFILING.md clocks line)"""
+    """nvidia-smi sampled every 10 ms during the timed region (B200_PROFILING.md clocks line); the default timed region is
+    only ~60 ms long"""
     Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
 
@@ -72,7 +73,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "-lms", "10"], stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
 

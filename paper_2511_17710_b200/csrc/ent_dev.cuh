@@ -118,9 +118,11 @@ __device__ __forceinline__ double dtheta_dT(double vt, double T) {            //
 }
 // inverse of theta(T) (App. B): theta(T) is a monotone cubic for 0 <= vartheta < 1, so Newton from
 // T = theta converges quadratically; no cube root on the device (differs from Eq. B3).
-__device__ __forceinline__ double T_of_theta(double vt, double th) {
+// T0 = starting point: the particle's previous T plus the linearised change is within a fraction of a cell of the root,
+// so two or three steps reach 1e-15.
+__device__ __forceinline__ double T_of_theta(double vt, double th, double T0) {
     if (vt == 0.0) return th;
-    double T = th;
+    double T = T0;
 #pragma unroll 1
     for (int it = 0; it < 8; ++it) {
         double f = theta_of_T(vt, T) - th;

@@ -59,7 +59,7 @@ __device__ __forceinline__ void push_from_fields(const GridDev &g, const float E
         double phn = PI_D - atan2(Y, -X);
         double y1, y2;
         if (KIND == ENT_SPH) { y1 = (rn - g.rmin) / g.dr; y2 = thn / g.dth; }
-        else { y1 = (log(rn - g.r0) - g.Rmin) / g.dR; y2 = T_of_theta(g.vt, thn) / g.dT; }
+        else { y1 = (log(rn - g.r0) - g.Rmin) / g.dR; double T_old = x2 * g.dT; y2 = T_of_theta(g.vt, thn, T_old + (thn - s.th) / dtheta_dT(g.vt, T_old)) / g.dT; }
         float phf = (float)phn;
         if (phf >= TWO_PI_F) phf -= TWO_PI_F;
         if (phf < 0.f) phf = 0.f;

@@ -54,8 +54,11 @@ __device__ __noinline__ void stray_step_axisym(const TiledArgs &A, long long p) 
     deposit_particle<2, KIND>(g, acc, i0, a, di, d, phi0, phi, u, A.q * A.P.w[p], A.inv_dt);
 }
 
+#ifndef ENT_AXISYM_MINB
+#define ENT_AXISYM_MINB 4
+#endif
 template <int KIND, int TX, int TY>
-__global__ void __launch_bounds__(TILED_TPB, 2)
+__global__ void __launch_bounds__(TILED_TPB, ENT_AXISYM_MINB)
 step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ TiledArgs A) {
     using G = TileGeom<2, TX, TY, 1>;
     extern __shared__ __align__(128) float smem[];
