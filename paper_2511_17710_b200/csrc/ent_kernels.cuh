@@ -334,11 +334,11 @@ __global__ void __launch_bounds__(REBIN_TPB) rebin_count_kernel(RebinGeom G, con
         long long p = base + threadIdx.x;
         int rel = -1, td = 0;
         if (p < p1) { int t[3]; G.tile_of_cell(cell[p], t); rel = G.classify(s, t); td = t[0] + G.nt[0] * (t[1] + G.nt[1] * t[2]); }
-        unsigned m = __match_any_sync(0xffffffffu, rel);
-        if (rel >= 0) {
-            if (rel == 27) atomicAdd(tile_count + td, 1);
-            else if ((int)(__ffs(m) - 1) == (int)(threadIdx.x & 31)) atomicAdd(&cnt[rel], __popc(m));
-        }
+        // the ~90 % that stay (class 13 = the source tile itself) are counted with one ballot; the few others one by one
+        const unsigned stay = __ballot_sync(0xffffffffu, rel == 13);
+        if (rel == 13) { if ((int)(__ffs(stay) - 1) == (int)(threadIdx.x & 31)) atomicAdd(&cnt[13], __popc(stay)); }
+        else if (rel == 27) atomicAdd(tile_count + td, 1);
+        else if (rel >= 0) atomicAdd(&cnt[rel], 1);
     }
     __syncthreads();
     if (threadIdx.x < REBIN_CLASSES) {
@@ -378,19 +378,23 @@ __global__ void __launch_bounds__(REBIN_TPB) rebin_scatter_kernel(RebinGeom G, c
             if (in.tag) rtag = in.tag[p];
             int t[3]; G.tile_of_cell(c, t); rel = G.classify(s, t); td = t[0] + G.nt[0] * (t[1] + G.nt[1] * t[2]);
         }
-        unsigned m = __match_any_sync(0xffffffffu, rel);
+        // stayers (class 13): one ballot, one reservation per warp, slots in lane order; the few others one by one
+        const unsigned stay = __ballot_sync(0xffffffffu, rel == 13);
+        const unsigned wbits = __float_as_uint(fabsf(w));
+        const unsigned wstay = __reduce_max_sync(0xffffffffu, rel == 13 ? wbits : 0u);
+        int r0 = 0;
+        const int leader = __ffs(stay) - 1;
+        if (stay && lane == leader) { r0 = atomicAdd(&fill[13], __popc(stay)); atomicMax(&wmx[13], wstay); }
+        r0 = __shfl_sync(0xffffffffu, r0, leader < 0 ? 0 : leader);
         if (rel < 0) continue;
         long long dst;
-        if (rel == 27) {
+        if (rel == 13) dst = (long long)base_s[13] + r0 + __popc(stay & ((1u << lane) - 1u));
+        else if (rel == 27) {
             dst = atomicAdd(cursor + td, 1);
-            atomicMax(tile_wmax_bits + td, __float_as_uint(fabsf(w)));
+            atomicMax(tile_wmax_bits + td, wbits);
         } else {
-            int leader = __ffs(m) - 1, r0 = 0;
-            if (lane == leader) r0 = atomicAdd(&fill[rel], __popc(m));
-            r0 = __shfl_sync(m, r0, leader);
-            dst = (long long)base_s[rel] + r0 + __popc(m & ((1u << lane) - 1u));
-            unsigned wb = __reduce_max_sync(m, __float_as_uint(fabsf(w)));
-            if (lane == leader) atomicMax(&wmx[rel], wb);
+            dst = (long long)base_s[rel] + atomicAdd(&fill[rel], 1);
+            atomicMax(&wmx[rel], wbits);
         }
         out.cell[dst] = c;
         for (int a = 0; a < 3; ++a) { if (a < G.D) out.d[a][dst] = rd[a]; out.u[a][dst] = ru[a]; }
