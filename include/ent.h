@@ -158,7 +158,8 @@ enum {
                                   (gather_push to scratch copy + deposit; the paper's structure) */
     ENT_OPT_TILE_1 = 2, ENT_OPT_TILE_2 = 3, ENT_OPT_TILE_3 = 4,   /* tile extents in cells; takes effect at the next ent_set_grid */
     ENT_OPT_SORT_MODE = 5      /* 0 = auto (incremental re-bin when `in` is itself a block ent_sort produced and key_offsets is NULL),
-                                  1 = always the full cell-level counting sort */
+                                  1 = always the full cell-level counting sort,
+                                  2 = like 0, but the re-bin does not order the particles that stay in a tile by cell */
 };
 enum {
     ENT_STAT_TILE_1 = 1, ENT_STAT_TILE_2 = 2, ENT_STAT_TILE_3 = 3, ENT_STAT_NKEYS = 4, ENT_STAT_NTILES = 5,

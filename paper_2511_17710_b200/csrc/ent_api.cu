@@ -22,6 +22,8 @@ struct ent_ctx {
     int step_impl = 0;
     int sort_mode = 0;                    // 0 auto (re-bin when the input is a sorted block), 1 always the full cell-level sort
     int last_sort_rebin = 0;
+    int rebin_ordered = 1;                // re-bin keeps the particles that stay in a tile ordered by cell (Cartesian grids)
+    bool ord_attr_set = false;
     int32_t *class_count = nullptr; size_t class_cap = 0;
     long long launches = 0;
     // scratch
@@ -371,9 +373,21 @@ static int sort_rebin(ent_ctx *ctx, const ent_ctx::SortedBlock *src, const ent_p
     if ((rc = launch_check(ctx, "scan_chunks_kernel"))) return rc;
     scan_apply_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, ntiles, ctx->chunk, slot->tile_off, ctx->cursor);
     if ((rc = launch_check(ctx, "scan_apply_kernel"))) return rc;
-    rebin_scatter_kernel<<<(unsigned)ntiles, REBIN_TPB, 0, ctx->stream>>>(G, src->tile_off, ctx->class_count, ctx->cursor, pp(in), pp(out),
-                                                                        g.kind != ENT_CART, (unsigned *)slot->tile_wmax);
-    if ((rc = launch_check(ctx, "rebin_scatter_kernel"))) return rc;
+    if (g.kind == ENT_CART && g.tcells <= ORD_BINS && ctx->rebin_ordered) {
+        if (!ctx->ord_attr_set) { CK(cudaFuncSetAttribute(rebin_scatter_ordered_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ORD_CAP_MAX * 33)); ctx->ord_attr_set = true; }
+        // staging capacity: 25 % above the mean tile population (a fuller tile is placed unordered), as small as possible so
+        // that several CTAs fit an SM
+        long long cap = ((in->n / ntiles) * 5 / 4 + 64 + 3) & ~3LL;
+        if (cap < 256) cap = 256;
+        if (cap > ORD_CAP_MAX) cap = ORD_CAP_MAX;
+        rebin_scatter_ordered_kernel<<<(unsigned)ntiles, ORD_TPB, (size_t)cap * 33, ctx->stream>>>(G, g.tcells, (int)cap, src->tile_off, ctx->class_count,
+                                                                                                 ctx->cursor, pp(in), pp(out), (unsigned *)slot->tile_wmax);
+        if ((rc = launch_check(ctx, "rebin_scatter_ordered_kernel"))) return rc;
+    } else {
+        rebin_scatter_kernel<<<(unsigned)ntiles, REBIN_TPB, 0, ctx->stream>>>(G, src->tile_off, ctx->class_count, ctx->cursor, pp(in), pp(out),
+                                                                            g.kind != ENT_CART, (unsigned *)slot->tile_wmax);
+        if ((rc = launch_check(ctx, "rebin_scatter_kernel"))) return rc;
+    }
     if ((rc = build_work_list(ctx, slot, ntiles))) return rc;
     out->q = in->q; out->m = in->m;
     slot->cell = out->cell; slot->n = in->n; slot->stamp = ++ctx->sort_stamp;
@@ -455,8 +469,8 @@ extern "C" int ent_set_option(ent_ctx *ctx, int key, int64_t value) {
             if (value < 0 || value > 2) return fail(ctx, ENT_EINVAL, "ENT_OPT_STEP_IMPL must be 0, 1 or 2");
             ctx->step_impl = (int)value; return ENT_OK;
         case ENT_OPT_SORT_MODE:
-            if (value < 0 || value > 1) return fail(ctx, ENT_EINVAL, "ENT_OPT_SORT_MODE must be 0 or 1");
-            ctx->sort_mode = (int)value; return ENT_OK;
+            if (value < 0 || value > 2) return fail(ctx, ENT_EINVAL, "ENT_OPT_SORT_MODE must be 0, 1 or 2");
+            ctx->sort_mode = value == 1 ? 1 : 0; ctx->rebin_ordered = value != 2; return ENT_OK;
         case ENT_OPT_TILE_1: case ENT_OPT_TILE_2: case ENT_OPT_TILE_3:
             if (value < 0 || value > 64) return fail(ctx, ENT_EINVAL, "tile extent must be in 0..64 (0 = default)");
             ctx->tile_opt[key - ENT_OPT_TILE_1] = (int)value; return ENT_OK;

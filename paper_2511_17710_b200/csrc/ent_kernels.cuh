@@ -296,6 +296,14 @@ struct RebinGeom {
         else { int n01 = N[0] * N[1]; i2 = dN01.div(cell); int r = cell - i2 * n01; i1 = dN0.div(r); i0 = r - i1 * N[0]; }
         t[0] = dT[0].div(i0); t[1] = dT[1].div(i1); t[2] = (D == 3) ? dT[2].div(i2) : 0;
     }
+    // index of the cell inside its own tile: l0 + T0*(l1 + T1*l2)
+    __device__ __forceinline__ int local_cell(int cell) const {
+        int i0, i1, i2 = 0;
+        if (D == 2) { i1 = dN0.div(cell); i0 = cell - i1 * N[0]; }
+        else { int n01 = N[0] * N[1]; i2 = dN01.div(cell); int r = cell - i2 * n01; i1 = dN0.div(r); i0 = r - i1 * N[0]; }
+        int l0 = i0 - dT[0].div(i0) * T[0], l1 = i1 - dT[1].div(i1) * T[1], l2 = (D == 3) ? i2 - dT[2].div(i2) * T[2] : 0;
+        return l0 + T[0] * (l1 + T[1] * l2);
+    }
     // class of destination tile t seen from source tile s: 0..26 = neighbour (dz+1)*9 + (dy+1)*3 + (dx+1), 27 = far
     __device__ __forceinline__ int classify(const int s[3], const int t[3]) const {
         int rel = 0, mul = 1;
@@ -404,6 +412,119 @@ __global__ void __launch_bounds__(REBIN_TPB) rebin_scatter_kernel(RebinGeom G, c
     }
     __syncthreads();
     if (threadIdx.x < 27 && dest_s[threadIdx.x] >= 0 && wmx[threadIdx.x]) atomicMax(tile_wmax_bits + dest_s[threadIdx.x], wmx[threadIdx.x]);
+}
+
+
+// ---------------------------------------------------------------------------------------------------------
+// Re-bin with the particles that stay ORDERED BY CELL (Cartesian grids).  The tiled step's shared-memory accesses are
+// conflict-free when the lanes of a warp sit in the same or neighbouring cells and cost 3-4 wavefronts each when they sit in
+// unrelated cells, and writing particles straight to cell-ordered global slots costs 8x the L2 write transactions (that is
+// what makes the full counting sort slow).  So the stayers of a tile (~90 %) are counting-sorted by local cell INTO SHARED
+// MEMORY and copied out coalesced; the few that leave are written one by one as in rebin_scatter_kernel.  A tile with more
+// than `cap` stayers falls back to the unordered placement.
+// ---------------------------------------------------------------------------------------------------------
+constexpr int ORD_TPB = 512;
+constexpr int ORD_CAP_MAX = 2560;        // staged records per CTA at most: 8 arrays x 4 B + tag = 33 B each
+constexpr int ORD_BINS = 1024;           // cells per tile, at most
+
+__global__ void __launch_bounds__(ORD_TPB) rebin_scatter_ordered_kernel(RebinGeom G, int tcells, int cap /* staged records, multiple of 4 */, const int32_t *tile_off, const int32_t *class_count,
+                                                                        int32_t *cursor, PartPtrs in, PartPtrs out, unsigned *tile_wmax_bits) {
+    extern __shared__ __align__(16) unsigned char ord_smem[];
+    int *st_cell = reinterpret_cast<int *>(ord_smem);
+    float *st_f = reinterpret_cast<float *>(ord_smem) + cap;               // [7][cap]: d0,d1,d2,u0,u1,u2,w
+    uint8_t *st_tag = ord_smem + cap * 32;
+    __shared__ int hist[ORD_BINS], wsum[ORD_TPB / 32];
+    __shared__ int base_s[REBIN_CLASSES], fill[REBIN_CLASSES], dest_s[REBIN_CLASSES];
+    __shared__ unsigned wmx[REBIN_CLASSES];
+    const int src = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+    int s[3] = { src % G.nt[0], (src / G.nt[0]) % G.nt[1], src / (G.nt[0] * G.nt[1]) };
+    if (tid < REBIN_CLASSES) {
+        int c = class_count[(long long)src * REBIN_CLASSES + tid];
+        int d = tid < 27 ? G.dest_tile(s, tid) : -1;
+        dest_s[tid] = d;
+        base_s[tid] = (tid < 27 && c > 0) ? atomicAdd(cursor + d, c) : 0;
+        fill[tid] = 0; wmx[tid] = 0u;
+    }
+    for (int k = tid; k < ORD_BINS; k += ORD_TPB) hist[k] = 0;
+    __syncthreads();
+    const long long p0 = tile_off[src], p1 = tile_off[src + 1];
+    const int nstay = class_count[(long long)src * REBIN_CLASSES + 13];
+    const bool ordered = nstay <= cap;                                    // uniform over the CTA
+    if (ordered) {
+        // pass A: histogram of the stayers' local cells (only the cell array is read)
+        for (long long p = p0 + tid; p < p1; p += ORD_TPB) {
+            const int c = in.cell[p];
+            int t[3]; G.tile_of_cell(c, t);
+            if (G.classify(s, t) == 13) atomicAdd(&hist[G.local_cell(c)], 1);
+        }
+        __syncthreads();
+        // exclusive scan of hist[0..tcells): two bins per thread
+        const int b0 = 2 * tid, h0 = b0 < tcells ? hist[b0] : 0, h1 = b0 + 1 < tcells ? hist[b0 + 1] : 0;
+        int x = h0 + h1;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+        if (lane == 31) wsum[tid >> 5] = x;
+        __syncthreads();
+        if (tid < 32) {
+            int v = tid < ORD_TPB / 32 ? wsum[tid] : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v += y; }
+            if (tid < ORD_TPB / 32) wsum[tid] = v;
+        }
+        __syncthreads();
+        const int excl = x - (h0 + h1) + ((tid >> 5) ? wsum[(tid >> 5) - 1] : 0);
+        if (b0 < tcells) hist[b0] = excl;
+        if (b0 + 1 < tcells) hist[b0 + 1] = excl + h0;
+        __syncthreads();                                                        // hist[] = first staged slot of every cell
+    }
+    // pass B: every record once
+    for (long long base = p0; base < p1; base += ORD_TPB) {
+        const long long p = base + tid;
+        int rel = -1, td = 0, c = 0;
+        float rd[3] = {0.f, 0.f, 0.f}, ru[3] = {0.f, 0.f, 0.f}, w = 0.f; uint8_t rtag = 1;
+        if (p < p1) {
+            c = in.cell[p];
+            for (int a = 0; a < 3; ++a) { if (a < G.D) rd[a] = in.d[a][p]; ru[a] = in.u[a][p]; }
+            w = in.w[p];
+            if (in.tag) rtag = in.tag[p];
+            int t[3]; G.tile_of_cell(c, t); rel = G.classify(s, t); td = t[0] + G.nt[0] * (t[1] + G.nt[1] * t[2]);
+        }
+        const unsigned wbits = __float_as_uint(fabsf(w));
+        const unsigned stay = __ballot_sync(0xffffffffu, rel == 13);
+        const unsigned wstay = __reduce_max_sync(0xffffffffu, rel == 13 ? wbits : 0u);
+        int r0 = 0;
+        const int leader = __ffs(stay) - 1;
+        if (stay && lane == leader) { if (!ordered) r0 = atomicAdd(&fill[13], __popc(stay)); atomicMax(&wmx[13], wstay); }
+        r0 = __shfl_sync(0xffffffffu, r0, leader < 0 ? 0 : leader);
+        if (rel < 0) continue;
+        if (rel == 13 && ordered) {                                             // staged at its cell's next slot
+            const int slot = atomicAdd(&hist[G.local_cell(c)], 1);
+            st_cell[slot] = c;
+            for (int a = 0; a < 3; ++a) { st_f[a * cap + slot] = rd[a]; st_f[(3 + a) * cap + slot] = ru[a]; }
+            st_f[6 * cap + slot] = w;
+            st_tag[slot] = rtag;
+            continue;
+        }
+        long long dst;
+        if (rel == 13) dst = (long long)base_s[13] + r0 + __popc(stay & ((1u << lane) - 1u));
+        else if (rel == 27) { dst = atomicAdd(cursor + td, 1); atomicMax(tile_wmax_bits + td, wbits); }
+        else { dst = (long long)base_s[rel] + atomicAdd(&fill[rel], 1); atomicMax(&wmx[rel], wbits); }
+        out.cell[dst] = c;
+        for (int a = 0; a < 3; ++a) { if (a < G.D) out.d[a][dst] = rd[a]; out.u[a][dst] = ru[a]; }
+        out.w[dst] = w;
+        if (in.tag) out.tag[dst] = rtag;
+    }
+    __syncthreads();
+    if (ordered) {                                                              // coalesced copy-out of the staged stayers
+        const long long b13 = base_s[13];
+        for (int k = tid; k < nstay; k += ORD_TPB) {
+            out.cell[b13 + k] = st_cell[k];
+            for (int a = 0; a < 3; ++a) { if (a < G.D) out.d[a][b13 + k] = st_f[a * cap + k]; out.u[a][b13 + k] = st_f[(3 + a) * cap + k]; }
+            out.w[b13 + k] = st_f[6 * cap + k];
+            if (in.tag) out.tag[b13 + k] = st_tag[k];
+        }
+    }
+    if (tid < 27 && dest_s[tid] >= 0 && wmx[tid]) atomicMax(tile_wmax_bits + dest_s[tid], wmx[tid]);
 }
 
 }  // namespace ent
