@@ -374,13 +374,13 @@ static int sort_rebin(ent_ctx *ctx, const ent_ctx::SortedBlock *src, const ent_p
     scan_apply_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, ntiles, ctx->chunk, slot->tile_off, ctx->cursor);
     if ((rc = launch_check(ctx, "scan_apply_kernel"))) return rc;
     if (g.kind == ENT_CART && g.tcells <= ORD_BINS && ctx->rebin_ordered) {
-        if (!ctx->ord_attr_set) { CK(cudaFuncSetAttribute(rebin_scatter_ordered_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ORD_CAP_MAX * 33)); ctx->ord_attr_set = true; }
+        if (!ctx->ord_attr_set) { CK(cudaFuncSetAttribute(rebin_scatter_ordered_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ORD_CAP_MAX * ORD_REC_BYTES)); ctx->ord_attr_set = true; }
         // staging capacity: 25 % above the mean tile population (a fuller tile is placed unordered), as small as possible so
         // that several CTAs fit an SM
         long long cap = ((in->n / ntiles) * 5 / 4 + 64 + 3) & ~3LL;
         if (cap < 256) cap = 256;
         if (cap > ORD_CAP_MAX) cap = ORD_CAP_MAX;
-        rebin_scatter_ordered_kernel<<<(unsigned)ntiles, ORD_TPB, (size_t)cap * 33, ctx->stream>>>(G, g.tcells, (int)cap, src->tile_off, ctx->class_count,
+        rebin_scatter_ordered_kernel<<<(unsigned)ntiles, ORD_TPB, (size_t)cap * ORD_REC_BYTES, ctx->stream>>>(G, g.tcells, (int)cap, src->tile_off, ctx->class_count,
                                                                                                  ctx->cursor, pp(in), pp(out), (unsigned *)slot->tile_wmax);
         if ((rc = launch_check(ctx, "rebin_scatter_ordered_kernel"))) return rc;
     } else {

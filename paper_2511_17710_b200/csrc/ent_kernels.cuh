@@ -420,19 +420,23 @@ __global__ void __launch_bounds__(REBIN_TPB) rebin_scatter_kernel(RebinGeom G, c
 // conflict-free when the lanes of a warp sit in the same or neighbouring cells and cost 3-4 wavefronts each when they sit in
 // unrelated cells, and writing particles straight to cell-ordered global slots costs 8x the L2 write transactions (that is
 // what makes the full counting sort slow).  So the stayers of a tile (~90 %) are counting-sorted by local cell INTO SHARED
-// MEMORY and copied out coalesced; the few that leave are written one by one as in rebin_scatter_kernel.  A tile with more
-// than `cap` stayers falls back to the unordered placement.
+// MEMORY (staged in arrival order, then a cell histogram, a scan and a permutation, all on chip) and copied out coalesced;
+// the few that leave are written one by one as in rebin_scatter_kernel.  A tile with more than `cap` stayers is placed unordered.
 // ---------------------------------------------------------------------------------------------------------
 constexpr int ORD_TPB = 512;
-constexpr int ORD_CAP_MAX = 2560;        // staged records per CTA at most: 8 arrays x 4 B + tag = 33 B each
+constexpr int ORD_CAP_MAX = 2560;        // staged records per CTA at most: 8 arrays x 4 B + tag + local cell + permutation = 37 B each
+constexpr int ORD_REC_BYTES = 37;
 constexpr int ORD_BINS = 1024;           // cells per tile, at most
 
-__global__ void __launch_bounds__(ORD_TPB) rebin_scatter_ordered_kernel(RebinGeom G, int tcells, int cap /* staged records, multiple of 4 */, const int32_t *tile_off, const int32_t *class_count,
-                                                                        int32_t *cursor, PartPtrs in, PartPtrs out, unsigned *tile_wmax_bits) {
+__global__ void __launch_bounds__(ORD_TPB) rebin_scatter_ordered_kernel(RebinGeom G, int tcells, int cap /* staged records, multiple of 4 */,
+                                                                        const int32_t *tile_off, const int32_t *class_count, int32_t *cursor,
+                                                                        PartPtrs in, PartPtrs out, unsigned *tile_wmax_bits) {
     extern __shared__ __align__(16) unsigned char ord_smem[];
     int *st_cell = reinterpret_cast<int *>(ord_smem);
-    float *st_f = reinterpret_cast<float *>(ord_smem) + cap;               // [7][cap]: d0,d1,d2,u0,u1,u2,w
-    uint8_t *st_tag = ord_smem + cap * 32;
+    float *st_f = reinterpret_cast<float *>(ord_smem) + cap;                   // [7][cap]: d0,d1,d2,u0,u1,u2,w
+    unsigned short *st_lc = reinterpret_cast<unsigned short *>(ord_smem + (size_t)cap * 32);   // local cell of every staged record
+    unsigned short *perm = st_lc + cap;                                         // staged slot of the k-th record in cell order
+    uint8_t *st_tag = ord_smem + (size_t)cap * 36;
     __shared__ int hist[ORD_BINS], wsum[ORD_TPB / 32];
     __shared__ int base_s[REBIN_CLASSES], fill[REBIN_CLASSES], dest_s[REBIN_CLASSES];
     __shared__ unsigned wmx[REBIN_CLASSES];
@@ -449,35 +453,8 @@ __global__ void __launch_bounds__(ORD_TPB) rebin_scatter_ordered_kernel(RebinGeo
     __syncthreads();
     const long long p0 = tile_off[src], p1 = tile_off[src + 1];
     const int nstay = class_count[(long long)src * REBIN_CLASSES + 13];
-    const bool ordered = nstay <= cap;                                    // uniform over the CTA
-    if (ordered) {
-        // pass A: histogram of the stayers' local cells (only the cell array is read)
-        for (long long p = p0 + tid; p < p1; p += ORD_TPB) {
-            const int c = in.cell[p];
-            int t[3]; G.tile_of_cell(c, t);
-            if (G.classify(s, t) == 13) atomicAdd(&hist[G.local_cell(c)], 1);
-        }
-        __syncthreads();
-        // exclusive scan of hist[0..tcells): two bins per thread
-        const int b0 = 2 * tid, h0 = b0 < tcells ? hist[b0] : 0, h1 = b0 + 1 < tcells ? hist[b0 + 1] : 0;
-        int x = h0 + h1;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-        if (lane == 31) wsum[tid >> 5] = x;
-        __syncthreads();
-        if (tid < 32) {
-            int v = tid < ORD_TPB / 32 ? wsum[tid] : 0;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v += y; }
-            if (tid < ORD_TPB / 32) wsum[tid] = v;
-        }
-        __syncthreads();
-        const int excl = x - (h0 + h1) + ((tid >> 5) ? wsum[(tid >> 5) - 1] : 0);
-        if (b0 < tcells) hist[b0] = excl;
-        if (b0 + 1 < tcells) hist[b0 + 1] = excl + h0;
-        __syncthreads();                                                        // hist[] = first staged slot of every cell
-    }
-    // pass B: every record once
+    const bool ordered = nstay <= cap;                                          // uniform over the CTA
+    // every record is read once; a stayer is staged in arrival order (ordered tile) or placed at once (too full a tile)
     for (long long base = p0; base < p1; base += ORD_TPB) {
         const long long p = base + tid;
         int rel = -1, td = 0, c = 0;
@@ -494,19 +471,22 @@ __global__ void __launch_bounds__(ORD_TPB) rebin_scatter_ordered_kernel(RebinGeo
         const unsigned wstay = __reduce_max_sync(0xffffffffu, rel == 13 ? wbits : 0u);
         int r0 = 0;
         const int leader = __ffs(stay) - 1;
-        if (stay && lane == leader) { if (!ordered) r0 = atomicAdd(&fill[13], __popc(stay)); atomicMax(&wmx[13], wstay); }
+        if (stay && lane == leader) { r0 = atomicAdd(&fill[13], __popc(stay)); atomicMax(&wmx[13], wstay); }
         r0 = __shfl_sync(0xffffffffu, r0, leader < 0 ? 0 : leader);
         if (rel < 0) continue;
-        if (rel == 13 && ordered) {                                             // staged at its cell's next slot
-            const int slot = atomicAdd(&hist[G.local_cell(c)], 1);
-            st_cell[slot] = c;
-            for (int a = 0; a < 3; ++a) { st_f[a * cap + slot] = rd[a]; st_f[(3 + a) * cap + slot] = ru[a]; }
-            st_f[6 * cap + slot] = w;
-            st_tag[slot] = rtag;
+        const int mine = r0 + __popc(stay & ((1u << lane) - 1u));              // stayers: slot in arrival order
+        if (rel == 13 && ordered) {
+            const int lc = G.local_cell(c);
+            st_cell[mine] = c;
+            for (int a = 0; a < 3; ++a) { st_f[a * cap + mine] = rd[a]; st_f[(3 + a) * cap + mine] = ru[a]; }
+            st_f[6 * cap + mine] = w;
+            st_tag[mine] = rtag;
+            st_lc[mine] = (unsigned short)lc;
+            atomicAdd(&hist[lc], 1);
             continue;
         }
         long long dst;
-        if (rel == 13) dst = (long long)base_s[13] + r0 + __popc(stay & ((1u << lane) - 1u));
+        if (rel == 13) dst = (long long)base_s[13] + mine;
         else if (rel == 27) { dst = atomicAdd(cursor + td, 1); atomicMax(tile_wmax_bits + td, wbits); }
         else { dst = (long long)base_s[rel] + atomicAdd(&fill[rel], 1); atomicMax(&wmx[rel], wbits); }
         out.cell[dst] = c;
@@ -515,13 +495,34 @@ __global__ void __launch_bounds__(ORD_TPB) rebin_scatter_ordered_kernel(RebinGeo
         if (in.tag) out.tag[dst] = rtag;
     }
     __syncthreads();
-    if (ordered) {                                                              // coalesced copy-out of the staged stayers
+    if (ordered) {
+        // exclusive scan of the cell histogram (two bins per thread), permutation, coalesced copy-out in cell order
+        const int b0 = 2 * tid, h0 = b0 < tcells ? hist[b0] : 0, h1 = b0 + 1 < tcells ? hist[b0 + 1] : 0;
+        int x = h0 + h1;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+        if (lane == 31) wsum[tid >> 5] = x;
+        __syncthreads();
+        if (tid < 32) {
+            int v = tid < ORD_TPB / 32 ? wsum[tid] : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v += y; }
+            if (tid < ORD_TPB / 32) wsum[tid] = v;
+        }
+        __syncthreads();
+        const int excl = x - (h0 + h1) + ((tid >> 5) ? wsum[(tid >> 5) - 1] : 0);
+        if (b0 < tcells) hist[b0] = excl;
+        if (b0 + 1 < tcells) hist[b0 + 1] = excl + h0;
+        __syncthreads();
+        for (int k = tid; k < nstay; k += ORD_TPB) perm[atomicAdd(&hist[st_lc[k]], 1)] = (unsigned short)k;
+        __syncthreads();
         const long long b13 = base_s[13];
         for (int k = tid; k < nstay; k += ORD_TPB) {
-            out.cell[b13 + k] = st_cell[k];
-            for (int a = 0; a < 3; ++a) { if (a < G.D) out.d[a][b13 + k] = st_f[a * cap + k]; out.u[a][b13 + k] = st_f[(3 + a) * cap + k]; }
-            out.w[b13 + k] = st_f[6 * cap + k];
-            if (in.tag) out.tag[b13 + k] = st_tag[k];
+            const int q = perm[k];
+            out.cell[b13 + k] = st_cell[q];
+            for (int a = 0; a < 3; ++a) { if (a < G.D) out.d[a][b13 + k] = st_f[a * cap + q]; out.u[a][b13 + k] = st_f[(3 + a) * cap + q]; }
+            out.w[b13 + k] = st_f[6 * cap + q];
+            if (in.tag) out.tag[b13 + k] = st_tag[q];
         }
     }
     if (tid < 27 && dest_s[tid] >= 0 && wmx[tid]) atomicMax(tile_wmax_bits + dest_s[tid], wmx[tid]);
