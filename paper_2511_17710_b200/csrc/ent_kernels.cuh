@@ -496,9 +496,13 @@ __global__ void __launch_bounds__(ORD_TPB) rebin_scatter_ordered_kernel(RebinGeo
     }
     __syncthreads();
     if (ordered) {
-        // exclusive scan of the cell histogram (two bins per thread), permutation, coalesced copy-out in cell order
-        const int b0 = 2 * tid, h0 = b0 < tcells ? hist[b0] : 0, h1 = b0 + 1 < tcells ? hist[b0 + 1] : 0;
-        int x = h0 + h1;
+        // exclusive scan of the cell histogram (ORD_BINS / ORD_TPB consecutive bins per thread), permutation, coalesced
+        // copy-out in cell order
+        constexpr int BPT = ORD_BINS / ORD_TPB;
+        int hb[BPT], x = 0;
+#pragma unroll
+        for (int j = 0; j < BPT; ++j) { int b = BPT * tid + j; hb[j] = b < tcells ? hist[b] : 0; x += hb[j]; }
+        const int mysum = x;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
         if (lane == 31) wsum[tid >> 5] = x;
@@ -510,9 +514,9 @@ __global__ void __launch_bounds__(ORD_TPB) rebin_scatter_ordered_kernel(RebinGeo
             if (tid < ORD_TPB / 32) wsum[tid] = v;
         }
         __syncthreads();
-        const int excl = x - (h0 + h1) + ((tid >> 5) ? wsum[(tid >> 5) - 1] : 0);
-        if (b0 < tcells) hist[b0] = excl;
-        if (b0 + 1 < tcells) hist[b0 + 1] = excl + h0;
+        int excl = x - mysum + ((tid >> 5) ? wsum[(tid >> 5) - 1] : 0);
+#pragma unroll
+        for (int j = 0; j < BPT; ++j) { int b = BPT * tid + j; if (b < tcells) hist[b] = excl; excl += hb[j]; }
         __syncthreads();
         for (int k = tid; k < nstay; k += ORD_TPB) perm[atomicAdd(&hist[st_lc[k]], 1)] = (unsigned short)k;
         __syncthreads();
