@@ -1,16 +1,16 @@
 // ent_tiled.cuh -- tiled fused step for the Cartesian grids (sub-steps 3-8), sm_100a.
 //
-// One CTA per tile of TX x TY x TZ cells.  The block handed to ent_step is the one ent_sort produced, so the
-// particles of a tile are one contiguous range of the SoA arrays (tile-major key, ent.h).
+// A CTA works on one tile of TX x TY x TZ cells (a tile with more than TILE_CHUNK particles is shared by several CTAs: work
+// list built by ent_sort).  The block handed to ent_step is the one ent_sort produced, so the particles of a tile are one
+// contiguous range of the SoA arrays (tile-major key, ent.h).
 //   * E,B: the tile's box of the six padded planar arrays, [o-2, o+T+2) per dimension, lands in shared memory by
 //     TMA (cp.async.bulk.tensor, one box per component, one mbarrier);
-//   * particles: 128-bit loads/stores, four consecutive particles per thread.  Consecutive lanes are therefore
-//     four particles (~ one cell) apart: gathers of a warp hit neighbouring words, deposits of a warp hit
-//     different words;
-//   * deposit: into a shared-memory tile of J covering nodes [o-2, o+T+3), then ONE flush per CTA with the TMA
-//     reduce-add (cp.reduce.async.bulk.tensor .add.f32) into the un-wrapped padded J arrays;
-//   * a particle whose cell has drifted more than one cell out of the tile since the sort (or whose deposit could
-//     leave the padded array) takes the global path (stray_step): global gathers, global atomics.
+//   * particles: one per thread and iteration, consecutive lanes on consecutive particles (fully coalesced lines), the
+//     next record requested before the current one is advanced;
+//   * deposit: fixed-point adds into a shared-memory tile of J covering nodes [o-2, o+T+3), then ONE flush per CTA with
+//     the TMA reduce-add (cp.reduce.async.bulk.tensor .add.f32) into the un-wrapped padded J arrays;
+//   * a particle whose cell has drifted more than one cell out of the tile since the sort goes to a list for stray_kernel
+//     (global gathers, global atomics); one whose deposit could leave the padded array deposits through global atomics.
 // Arithmetic per particle is the same as ent_particle.cuh (same Boris, same split_offset, same segment weights); a
 // particle that crosses no face deposits its straight move as one segment (the two half segments of P:575 are
 // collinear then, and the weights (1-W_a)(1-W_b) + D_a D_b/12 are the exact line integral, so the sum is identical).
@@ -177,9 +177,6 @@ __device__ __forceinline__ void acc_fixed4(int *sJ, const CarryCtx &cc, int comp
 #endif
 #ifndef ENT_TILED_PREFETCH
 #define ENT_TILED_PREFETCH 1
-#endif
-#ifndef ENT_TILED_VEC4
-#define ENT_TILED_VEC4 0
 #endif
 
 constexpr int TILED_TPB = 256;
@@ -413,77 +410,6 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     __syncthreads();                                             // sJ zeroed, mbarrier initialised
     bool waited = false;
 
-#if ENT_TILED_VEC4
-    // ---- groups of four consecutive particles per thread (128-bit accesses; consecutive lanes are four particles apart).
-    // A group that straddles the ends of the tile's range [p0, p1) is shared with the neighbouring tile's CTA: each side
-    // touches only its own particles, with scalar accesses.
-    const long long G0 = p0 >> 2, G1 = (p1 + 3) >> 2;
-    for (long long grp = G0 + tid; grp < G1; grp += TILED_TPB) {
-        const long long pb = grp * 4;
-        const bool full = pb >= p0 && pb + 4 <= p1;
-        int4 vc; float4 vd0, vd1, vd2, vu0, vu1, vu2, vw;
-        uchar4 vt = make_uchar4(1, 1, 1, 1);
-        vd2 = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (full) {
-            vc = *reinterpret_cast<const int4 *>(A.P.cell + pb);
-            vd0 = *reinterpret_cast<const float4 *>(A.P.d[0] + pb);
-            vd1 = *reinterpret_cast<const float4 *>(A.P.d[1] + pb);
-            if (D == 3) vd2 = *reinterpret_cast<const float4 *>(A.P.d[2] + pb);
-            vu0 = *reinterpret_cast<const float4 *>(A.P.u[0] + pb);
-            vu1 = *reinterpret_cast<const float4 *>(A.P.u[1] + pb);
-            vu2 = *reinterpret_cast<const float4 *>(A.P.u[2] + pb);
-            vw = *reinterpret_cast<const float4 *>(A.P.w + pb);
-            if (A.P.tag) vt = *reinterpret_cast<const uchar4 *>(A.P.tag + pb);
-        } else {
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const bool in = pb + k >= p0 && pb + k < p1;
-                (&vc.x)[k] = in ? A.P.cell[pb + k] : 0;
-                (&vd0.x)[k] = in ? A.P.d[0][pb + k] : 0.f; (&vd1.x)[k] = in ? A.P.d[1][pb + k] : 0.f;
-                (&vd2.x)[k] = (D == 3 && in) ? A.P.d[2][pb + k] : 0.f;
-                (&vu0.x)[k] = in ? A.P.u[0][pb + k] : 0.f; (&vu1.x)[k] = in ? A.P.u[1][pb + k] : 0.f; (&vu2.x)[k] = in ? A.P.u[2][pb + k] : 0.f;
-                (&vw.x)[k] = in ? A.P.w[pb + k] : 0.f;
-                (&vt.x)[k] = in ? (A.P.tag ? A.P.tag[pb + k] : 1) : 0;
-            }
-        }
-        if (!waited) { mbar_wait(&bar, 0); waited = true; }
-        int code[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {                      // component k of every vector: plain register names after unrolling
-            float d[3] = { (&vd0.x)[k], (&vd1.x)[k], (&vd2.x)[k] };
-            float u[3] = { (&vu0.x)[k], (&vu1.x)[k], (&vu2.x)[k] };
-            code[k] = 3;
-            if ((&vt.x)[k]) {
-                code[k] = tile_particle<D, TX, TY, TZ, ALLPER>(A, T, pb + k, (&vc.x)[k], d, u, (&vw.x)[k]);
-                (&vd0.x)[k] = d[0]; (&vd1.x)[k] = d[1]; (&vd2.x)[k] = d[2];
-                (&vu0.x)[k] = u[0]; (&vu1.x)[k] = u[1]; (&vu2.x)[k] = u[2];
-            }
-        }
-        // ---- write back (cell, offsets, momentum; the weight is read-only)
-        if (full && ((code[0] | code[1] | code[2] | code[3]) & 1) == 0) {        // nobody dead or taken by the global path
-            *reinterpret_cast<int4 *>(A.P.cell + pb) = vc;
-            *reinterpret_cast<float4 *>(A.P.d[0] + pb) = vd0;
-            *reinterpret_cast<float4 *>(A.P.d[1] + pb) = vd1;
-            if (D == 3) *reinterpret_cast<float4 *>(A.P.d[2] + pb) = vd2;
-            *reinterpret_cast<float4 *>(A.P.u[0] + pb) = vu0;
-            *reinterpret_cast<float4 *>(A.P.u[1] + pb) = vu1;
-            *reinterpret_cast<float4 *>(A.P.u[2] + pb) = vu2;
-        } else {
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                if (code[k] & 1) continue;
-                A.P.cell[pb + k] = (&vc.x)[k];
-                A.P.d[0][pb + k] = (&vd0.x)[k]; A.P.d[1][pb + k] = (&vd1.x)[k];
-                if (D == 3) A.P.d[2][pb + k] = (&vd2.x)[k];
-                A.P.u[0][pb + k] = (&vu0.x)[k]; A.P.u[1][pb + k] = (&vu1.x)[k]; A.P.u[2][pb + k] = (&vu2.x)[k];
-            }
-        }
-        if (!ALLPER) {
-#pragma unroll
-            for (int k = 0; k < 4; ++k) if (code[k] == 2) A.P.tag[pb + k] = 0;
-        }
-    }
-#else
     // ---- one particle per thread and iteration, consecutive lanes on consecutive particles: every access is a fully
     // coalesced 128-byte line per warp, the work of a tile is balanced to within one particle per thread, and the order of the
     // particles inside the tile's range does not matter (the incremental ent_sort does not keep one)
@@ -531,7 +457,6 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
         A.P.u[0][p] = u[0]; A.P.u[1][p] = u[1]; A.P.u[2][p] = u[2];
         if (!ALLPER && code == 2) A.P.tag[p] = 0;
     }
-#endif
 #endif
     if (!waited) mbar_wait(&bar, 0);          // never leave with a TMA load still in flight into this CTA's shared memory
     // ---- S8 flush: one TMA reduce-add per component into the un-wrapped padded J (ghost fold = ent_fold_current)
