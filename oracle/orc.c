@@ -89,6 +89,11 @@ void orc_metric_h(const orc_grid *g, const double x[3], double h[3]) {
     }
 }
 
+/* the same at n positions (x1[k], x2[k], 0): h[3*k + d]; a loop over orc_metric_h, for the test helpers */
+void orc_metric_h_many(const orc_grid *g, int64_t n, const double *x1, const double *x2, double *h) {
+    for (int64_t k = 0; k < n; ++k) { double x[3] = { x1[k], x2[k], 0.0 }; orc_metric_h(g, x, h + 3 * k); }
+}
+
 /* Eq. 8: min over cell centres of (sum_d 1/h_dd)^(-1/2), d < D */
 double orc_dx_min(const orc_grid *g) {
     double best = INFINITY;

@@ -16,8 +16,12 @@
  * plus the discrete continuity checker of Eq. 6 and a sort checker.
  * Readings of silent / garbled passages are those of SURVEY.md section 8(c) (G1..G19), listed in DESIGN.md.
  *
- * Parity pins: tests/test_oracle_*.py (every function below is pinned except the 2D out-of-plane
- * current J^3, which the paper does not constrain: "parity unpinned" beyond sum + symmetry).
+ * Parity pins: tests/test_oracle_pins_*.py; tests/oracle_mutants.py lists the one-line misreadings those pins kill
+ * (gamma^- in the Boris rotation, gamma^(n+1/2) in the move, time level / azimuth midpoint / evaluation point of the
+ * out-of-plane current, the theta = pi clamp, the D_a D_b / 12 term, ...).  One choice stays a READING the paper does
+ * not fix: the FORM of the 2D out-of-plane current J^3 (velocity form, half per segment, bilinear weights at the
+ * segment midpoints, reading G8) -- "parity unpinned" by the paper beyond its nodal sum, time level and evaluation
+ * point, which are pinned; see DESIGN.md.
  *
  * All arithmetic is double.  Field arrays are the fp32 arrays handed to the GPU (up-cast on load).
  */
@@ -57,6 +61,7 @@ typedef struct {
 /* ---- O1 metric ---- */
 void   orc_metric_h(const orc_grid *g, const double x[3], double h[3]);   /* h11,h22,h33 at code coords */
 double orc_theta_of_T(double vartheta, double T);
+void   orc_metric_h_many(const orc_grid *g, int64_t n, const double *x1, const double *x2, double *h /* [n][3] */);
 double orc_dtheta_dT(double vartheta, double T);
 double orc_T_of_theta(double vartheta, double theta);                      /* App. B, corrected (F1) */
 double orc_T_of_theta_printed_B3(double vartheta, double theta);           /* App. B exactly as printed + F1 fix flag; for the pin */

@@ -15,7 +15,8 @@ from dataclasses import dataclass, field
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "liborc.so")
+# ORC_LIBORC: load a prebuilt copy instead (tests/oracle_mutants.py points the pin tests at deliberately broken builds)
+_LIB_PATH = os.environ.get("ORC_LIBORC") or os.path.join(_HERE, "liborc.so")
 
 CART, SPH, QSPH = 0, 1, 2
 PERIODIC, ABSORB, AXIS = 0, 1, 2
@@ -24,6 +25,8 @@ NGHOST = 2
 
 def build(force: bool = False) -> str:
     """Compile oracle/orc.c -> oracle/liborc.so with gcc (no fast-math: the oracle must stay IEEE)."""
+    if os.environ.get("ORC_LIBORC"):
+        return _LIB_PATH
     src = os.path.join(_HERE, "orc.c")
     hdr = os.path.join(_HERE, "orc.h")
     if (not force and os.path.exists(_LIB_PATH)
@@ -54,6 +57,7 @@ def lib():
         L = C.CDLL(_LIB_PATH)
         dp = C.POINTER(C.c_double)
         L.orc_metric_h.argtypes = [C.POINTER(_Grid), dp, dp]
+        L.orc_metric_h_many.argtypes = [C.POINTER(_Grid), C.c_int64, dp, dp, dp]
         L.orc_theta_of_T.restype = C.c_double; L.orc_theta_of_T.argtypes = [C.c_double, C.c_double]
         L.orc_dtheta_dT.restype = C.c_double; L.orc_dtheta_dT.argtypes = [C.c_double, C.c_double]
         L.orc_T_of_theta.restype = C.c_double; L.orc_T_of_theta.argtypes = [C.c_double, C.c_double]
@@ -194,6 +198,14 @@ def _jptrs(J):
 # ---- thin wrappers (argument marshalling only) ----
 def metric_h(g: Grid, x) -> np.ndarray:
     xa, xp = _vec(x); h = np.zeros(3); lib().orc_metric_h(C.byref(g.c()), xp, h.ctypes.data_as(C.POINTER(C.c_double)))
+    return h
+
+
+def metric_h_many(g: Grid, x1, x2) -> np.ndarray:
+    """h_11, h_22, h_33 at many code positions (x1[k], x2[k]): orc_metric_h called in a loop; returns shape (n, 3)."""
+    a1, p1 = _vec(x1); a2, p2 = _vec(x2)
+    h = np.zeros((a1.shape[0], 3))
+    lib().orc_metric_h_many(C.byref(g.c()), a1.shape[0], p1, p2, h.ctypes.data_as(C.POINTER(C.c_double)))
     return h
 
 

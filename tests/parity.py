@@ -56,10 +56,11 @@ def unpack_cell_np(grid, cell):
     return [c % N0, (c // N0) % N1, c // (N0 * N1)]
 
 
-def compare_particles(grid, pe, po, order=None, steps=1):
+def compare_particles(grid, pe, po, order=None, steps=1, orc_metric=None):
     """pe: binding.Particles (any device), po: orc.Particles.  `order`: optional index array such that GPU particle k is
     oracle particle order[k] (after a sort).  `steps`: steps taken since the two states were equal (enters only the
-    fp32-storage allowance of phi).  Returns a dict of maxima and counts; raises AssertionError on a violation."""
+    fp32-storage allowance of phi).  `orc_metric`: (orc module, orc grid), needed on the axisymmetric grids (the azimuth error is
+    measured as an arc with the ORACLE's metric).  Returns a dict of maxima and counts; raises AssertionError on a violation."""
     cell = pe.cell.detach().cpu().numpy()
     ig = unpack_cell_np(grid, cell)
     sel = (lambda a: a) if order is None else (lambda a: a[order])
@@ -98,13 +99,12 @@ def compare_particles(grid, pe, po, order=None, steps=1):
         # azimuth: phi is ill-conditioned near the axis (d phi = d x / (r sin theta)), so its
         # error is measured as the ARC it spans in units of the theta-cell, sqrt(h33) |d phi| / sqrt(h22) <= POS_TOL like the
         # other two coordinates, on top of what storing phi as an fp32 in [0, 2 pi) costs (half an ulp per step).
-        from paper_2511_17710_b200 import synth
+        assert orc_metric is not None, "compare_particles on an axisymmetric grid needs orc_metric=(orc, og)"
         dphi = pe.phi.detach().cpu().numpy().astype(np.float64) - sel(po.phi)
         dphi = dphi - 2.0 * np.pi * np.round(dphi / (2.0 * np.pi))
-        x1 = torch.from_numpy(sel(po.i[0]).astype(np.float64) + sel(po.d[0]))
-        x2 = torch.from_numpy(sel(po.i[1]).astype(np.float64) + sel(po.d[1]))
-        _, _, _, h2, h3 = synth.sph_geometry(grid, x1, x2)
-        arc = (np.abs(dphi) - steps * PHI_ULP).clip(min=0.0) * (h3 / h2).numpy()
+        h = orc_metric[0].metric_h_many(orc_metric[1], sel(po.i[0]).astype(np.float64) + sel(po.d[0]),
+                                        sel(po.i[1]).astype(np.float64) + sel(po.d[1]))
+        arc = (np.abs(dphi) - steps * PHI_ULP).clip(min=0.0) * np.sqrt(h[:, 2] / h[:, 1])
         if both.any():
             stats["max_phi_err"] = float(np.abs(dphi[both]).max())
             stats["max_phi_arc_cells"] = float(arc[both].max())
@@ -120,17 +120,34 @@ def compare_current(Jg, Jo, fmt_bound=None):
     """Jg: list of 3 torch tensors (after fold), Jo: list of 3 float64 numpy arrays (after fold).
     BASELINE.json's bar: |J_gpu - J_orc| <= 1e-5 max|J| at every element.  fmt_bound (optional, 3 padded arrays): what the
     fp32 particle FORMAT itself allows at each element (see offset_format_bound); an element may exceed the bar by that.
-    Returns max over elements of (error - allowance) / max|J|, asserted <= J_TOL."""
+    Returns max over elements of (error - allowance) / max|J|, asserted <= J_TOL; compare_current.last_raw holds the RAW
+    max|J_gpu - J_orc| / max|J_orc| of the same call (no allowance subtracted), which the tests print beside it."""
     scale = max(float(np.abs(j).max()) for j in Jo)
-    worst = 0.0
+    worst = raw = 0.0
     for c, (g, o) in enumerate(zip(Jg, Jo)):
-        e = np.abs(g.detach().cpu().numpy().astype(np.float64) - o)
+        e = np.abs((g.detach().cpu().numpy().astype(np.float64) if torch.is_tensor(g) else g) - o)
+        raw = max(raw, float(e.max()))
         if fmt_bound is not None:
             e = (e - fmt_bound[c]).clip(min=0.0)
         worst = max(worst, float(e.max()))
     rel = worst / scale if scale > 0 else worst
-    assert rel <= J_TOL, f"max|J_gpu - J_orc| / max|J_orc| = {rel:.3e} (scale {scale:.3e})"
+    compare_current.last_raw = raw / scale if scale > 0 else raw
+    assert rel <= J_TOL, f"max|J_gpu - J_orc| / max|J_orc| = {rel:.3e} (raw {compare_current.last_raw:.3e}, scale {scale:.3e})"
     return rel
+
+
+compare_current.last_raw = 0.0
+
+
+def deposit_of_gpu_positions(orc, og, p_before, p_after, q, dt, fold=True):
+    """The STRICT current check (no allowance): the oracle's deposit fed with the GPU's own stored positions before and after the
+    step (fp32 values up-cast) and the GPU's new momenta.  Whatever the push did, the GPU's J must equal this to J_TOL * max|J|:
+    it isolates sub-step 8 from the conditioning of sub-steps 3-7.  Returns 3 padded float64 arrays."""
+    J = orc.zeros_current(og)
+    orc.deposit(og, p_before, p_after, J, q, dt)
+    if fold:
+        orc.fold_current(og, J)
+    return J
 
 
 def _box3(a):
@@ -152,13 +169,15 @@ def offset_format_bound(orc, grid, og, p_before, q, dt):
         |d ln sin(theta) / d x2| * OFFSET_ULP = |cos theta| sqrt(h22)/sqrt(h33) * OFFSET_ULP, unbounded toward the axis.
     The allowance at an element is that figure summed over the particles within one cell of it (3x3 box sum of a nodal
     deposit; the in-plane one is the oracle's charge_density of |q| w)."""
-    from paper_2511_17710_b200 import synth
     inplane = _box3(orc.charge_density(og, p_before, abs(q))) * (OFFSET_ULP / dt)
-    x1 = torch.from_numpy(p_before.i[0].astype(np.float64) + p_before.d[0])
-    x2 = torch.from_numpy(p_before.i[1].astype(np.float64) + p_before.d[1])
-    _, th, _, h2, h3 = synth.sph_geometry(grid, x1, x2)
-    h2, h3, th = h2.numpy(), np.maximum(h3.numpy(), 1e-300), th.numpy()
-    per = abs(q) * p_before.w / h3 * (np.abs(np.cos(th)) * h2 / h3) * OFFSET_ULP          # |v^phi-hat| <= 1
+    x1 = p_before.i[0].astype(np.float64) + p_before.d[0]
+    x2 = p_before.i[1].astype(np.float64) + p_before.d[1]
+    h = orc.metric_h_many(og, x1, x2)                                    # the ORACLE's metric (P:233-267)
+    # d sqrt(h33) / d x2 by a centred difference of the oracle's own h33: no second statement of the metric in the tests
+    eps = 1e-4
+    dh3 = (np.sqrt(orc.metric_h_many(og, x1, x2 + eps)[:, 2]) - np.sqrt(orc.metric_h_many(og, x1, x2 - eps)[:, 2])) / (2 * eps)
+    h3 = np.maximum(np.sqrt(h[:, 2]), 1e-300)
+    per = abs(q) * p_before.w / h3 * (np.abs(dh3) / h3) * OFFSET_ULP     # |v^phi-hat| <= 1; |d ln sqrt(h33) / d x2| per offset ulp
     if p_before.tag is not None:
         per = per * (p_before.tag != 0)
     out3 = np.zeros(inplane.shape, dtype=np.float64)
