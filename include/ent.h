@@ -129,6 +129,11 @@ int ent_deposit(ent_ctx *ctx, const ent_particles *old_, const ent_particles *ne
  * unspecified (the tiled ent_step does not depend on it).  ENT_STAT_LAST_SORT_REBIN tells which form ran. */
 int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *out, int32_t *key_offsets);
 
+/* Copies the tile offsets the ctx keeps for a sorted block (the `out` of an ent_sort of this ctx) to tile_offsets (device,
+ * int32[ENT_STAT_NTILES + 1]): tile t owns particles [tile_offsets[t], tile_offsets[t+1]) of the block.  ENT_EINVAL if the
+ * block is not a sorted block of this ctx.  Enqueued on the ctx's stream. */
+int ent_tile_offsets(ent_ctx *ctx, const ent_particles *block, int32_t *tile_offsets);
+
 /* ---- fused hot path: the timed entry point ------------------------------------------------------------------
  * ent_step = ent_gather_push (in place) + ent_deposit(old, new) in one pass over the particles: the old
  * position stays in registers instead of the i_prev/dx_prev arrays of P:559.  Accumulates into J un-wrapped.

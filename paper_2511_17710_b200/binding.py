@@ -22,7 +22,7 @@ OPT_STEP_IMPL, OPT_TILE_1, OPT_TILE_2, OPT_TILE_3, OPT_SORT_MODE = 1, 2, 3, 4, 5
  STAT_SCRATCH_BYTES, STAT_LAST_STEP_TILED, STAT_LAST_SORT_REBIN) = range(1, 12)
 
 SYMBOLS = ["ent_create", "ent_destroy", "ent_last_error", "ent_set_grid", "ent_gather_push", "ent_deposit", "ent_sort",
-           "ent_step", "ent_zero_current", "ent_fold_current", "ent_step_host", "ent_set_option", "ent_get_stat", "ent_version"]
+           "ent_step", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_step_host", "ent_set_option", "ent_get_stat", "ent_version"]
 
 
 class EntError(RuntimeError):
@@ -69,6 +69,7 @@ def lib():
         L.ent_gather_push.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Particles), C.c_float]
         L.ent_deposit.argtypes = [vp, C.POINTER(_Particles), C.POINTER(_Particles), C.POINTER(_Current), C.c_float]
         L.ent_sort.argtypes = [vp, C.POINTER(_Particles), C.POINTER(_Particles), vp]
+        L.ent_tile_offsets.argtypes = [vp, C.POINTER(_Particles), vp]
         L.ent_step.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Current), C.c_float]
         L.ent_zero_current.argtypes = [vp, C.POINTER(_Current)]
         L.ent_fold_current.argtypes = [vp, C.POINTER(_Current)]
@@ -253,6 +254,13 @@ def ent_deposit(ctx: Ctx, pold: Particles, pnew: Particles, J, dt: float) -> Non
 def ent_sort(ctx: Ctx, pin: Particles, pout: Particles, key_offsets: torch.Tensor | None = None) -> None:
     ko = _ptr(key_offsets, torch.int32, "key_offsets")
     ctx._ck(lib().ent_sort(ctx._h, C.byref(pin.c()), C.byref(pout.c()), ko))
+
+
+def ent_tile_offsets(ctx: Ctx, block: Particles) -> torch.Tensor:
+    """int32[ntiles + 1] device tensor: the tile offsets the ctx keeps for a sorted block"""
+    out = torch.empty(ent_get_stat(ctx, STAT_NTILES) + 1, dtype=torch.int32, device=block.cell.device)
+    ctx._ck(lib().ent_tile_offsets(ctx._h, C.byref(block.c()), out.data_ptr()))
+    return out
 
 
 def ent_step(ctx: Ctx, EB, p: Particles, J, dt: float) -> None:

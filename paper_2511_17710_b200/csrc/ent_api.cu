@@ -462,6 +462,19 @@ extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *ou
     return ENT_OK;
 }
 
+extern "C" int ent_tile_offsets(ent_ctx *ctx, const ent_particles *block, int32_t *tile_offsets) {
+    ENTER();
+    if (!block || !tile_offsets) return fail(ctx, ENT_EINVAL, "NULL argument");
+    const GridDev &g = ctx->g;
+    const long long ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
+    for (auto &b : ctx->sorted)
+        if (b.cell && b.cell == block->cell && b.n == block->n) {
+            CK(cudaMemcpyAsync(tile_offsets, b.tile_off, (size_t)(ntiles + 1) * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+            return ENT_OK;
+        }
+    return fail(ctx, ENT_EINVAL, "the block is not one ent_sort of this ctx produced");
+}
+
 extern "C" int ent_set_option(ent_ctx *ctx, int key, int64_t value) {
     if (!ctx) return ENT_EINVAL;
     switch (key) {

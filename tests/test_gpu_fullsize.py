@@ -79,7 +79,7 @@ def test_full_size_last_step(orc, name):
         idx = torch.randint(0, pe.n, (NSAMPLE,), device="cuda", generator=gen)
         pb = P.ent_to_orc(orc, g, _subset(bind, before, idx))
         po = orc.gather_push(og, F_orc, pb, before.q / before.m, wl.dt)
-        stats = P.compare_particles(g, _subset(bind, pe, idx), po, steps=1)
+        stats = P.compare_particles(g, _subset(bind, pe, idx), po, steps=1, orc_metric=(orc, og))
         print("sample:", stats)
 
         # ---- (2) current in two sub-boxes: every particle that can reach a node of the box goes through the oracle
@@ -157,7 +157,7 @@ def test_c5_full_size_last_step(orc):
         idx = torch.randint(0, pe.n, (NSAMPLE,), device="cuda", generator=gen)
         pb = P.ent_to_orc(orc, g, _subset(bind, before, idx))
         po = orc.gather_push(og, F_orc, pb, before.q / before.m, wl.dt)
-        stats = P.compare_particles(g, _subset(bind, pe, idx), po, steps=1)
+        stats = P.compare_particles(g, _subset(bind, pe, idx), po, steps=1, orc_metric=(orc, og))
         print("sample:", stats)
 
         Jscale = max(float(j.abs().max()) for j in J)

@@ -75,7 +75,7 @@ def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True
             order = _match_perm(g, pe, ps)
             pe = ps
         Jg = bind.zeros_current(eg, "cuda")
-        worstJ = worstC = 0.0
+        worstJ = worstC = rawJ = strictJ = 0.0
         for s in range(steps):
             if resort_every and s > 0 and s % resort_every == 0:
                 # incremental ent_sort (re-bin) of the drifted block: tile contiguity only
@@ -99,16 +99,19 @@ def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True
             if check_every_step or s == steps - 1:
                 bound = P.offset_format_bound(orc, g, og, before, sp.q, wl.dt) if (eg.axisym and before is not None) else None
                 worstJ = max(worstJ, P.compare_current(Jg, Jo, bound))
+                rawJ = max(rawJ, P.compare_current.last_raw)
             if check_every_step:
                 after = P.ent_to_orc(orc, g, pe)
+                # STRICT current check, no allowance: the oracle's deposit of the GPU's own stored move (isolates sub-step 8)
+                strictJ = max(strictJ, P.compare_current(Jg, P.deposit_of_gpu_positions(orc, og, before, after, sp.q, wl.dt)))
                 c = P.continuity_of_gpu_step(orc, og, before, after, Jg, sp.q, wl.dt)
                 assert c <= P.CONT_TOL, f"continuity residual {c:.3e} at step {s}"
                 worstC = max(worstC, c)
-        stats = P.compare_particles(g, pe, po, order, steps=steps)
+        stats = P.compare_particles(g, pe, po, order, steps=steps, orc_metric=(orc, og))
         assert bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES) == 0
         stats["tiled"] = bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED)
         stats["strays"] = bind.ent_get_stat(ctx, bind.STAT_STRAYS)
-        stats.update(worstJ=worstJ, worstC=worstC)
+        stats.update(worstJ=worstJ, rawJ=rawJ, strictJ=strictJ, worstC=worstC)
         out[si] = stats
     return out
 
@@ -144,6 +147,71 @@ def test_rebinned_block_matches_oracle(env, name):
     stats = _run_case(env, wl, impl=0, sort_first=True, resort_every=3)
     print(name, stats)
     assert all(st["tiled"] == 1 and st["strays"] == 0 for st in stats.values())
+
+
+def _host_keys(synth, bind, ctx, g, cell):
+    """sort keys recomputed on the host from the cell indices with the formula of include/ent.h (ent_sort)"""
+    T = tuple(bind.ent_get_stat(ctx, k) for k in (bind.STAT_TILE_1, bind.STAT_TILE_2, bind.STAT_TILE_3))[:g.D]
+    return synth.sort_key(g, synth.unpack_cell(g, cell.cpu()), T).numpy().astype(np.int32), T
+
+
+@pytest.mark.parametrize("name", ["C1", "C3/8", "C4/16-shuffled", "C5/32", "ABS3", "ABS2"])
+def test_full_sort_passes_the_oracle_checker(env, name):
+    """S10: ent_sort (full form) with a key_offsets output.  Keys are recomputed on the host from out.cell; the ORACLE's checker
+    (orc_sort_check: non-decreasing keys, offsets = exclusive scan of the key histogram) must accept them, and the records must
+    be a permutation of the input (every array permuted alike)."""
+    bind, synth, ctx, orc = env
+    wl = _workloads(synth)[name]()
+    g = wl.grid
+    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, 0)
+    bind.ent_set_grid(ctx, P.grid_to_ent(bind, g))
+    nkeys = bind.ent_get_stat(ctx, bind.STAT_NKEYS)
+    for sp in wl.species:
+        pe = P.species_to_ent(bind, synth, g, sp, "cuda")
+        ps = pe.empty_like()
+        ko = torch.full((nkeys + 1,), -7, dtype=torch.int32, device="cuda")
+        bind.ent_sort(ctx, pe, ps, ko)
+        torch.cuda.synchronize()
+        assert bind.ent_get_stat(ctx, bind.STAT_LAST_SORT_REBIN) == 0
+        _match_perm(g, pe, ps)
+        keys, T = _host_keys(synth, bind, ctx, g, ps.cell)
+        assert orc.sort_check(keys, nkeys, ko.cpu().numpy()) == 0, "ent_sort output rejected by orc_sort_check"
+        tcells = int(np.prod(T))
+        toff = bind.ent_tile_offsets(ctx, ps).cpu().numpy()
+        assert np.array_equal(toff, ko.cpu().numpy()[::tcells]), "tile offsets != key offsets at the tile boundaries"
+
+
+@pytest.mark.parametrize("name", ["C1", "C3/8", "C4/16-shuffled", "C5/32", "ABS3"])
+def test_rebin_tile_offsets_are_the_scan_of_the_tile_histogram(env, name):
+    """S10, incremental form: after steps + re-bin, the block is tile-contiguous and the ctx's tile offsets equal the exclusive scan
+    of the histogram of tile(key) recomputed on the host (checked with the oracle's checker on the TILE keys)."""
+    bind, synth, ctx, orc = env
+    wl = _workloads(synth)[name]()
+    g = wl.grid
+    eg = P.grid_to_ent(bind, g)
+    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, 0)
+    bind.ent_set_grid(ctx, eg)
+    ntiles = bind.ent_get_stat(ctx, bind.STAT_NTILES)
+    F = [f.cuda() for f in wl.fields]
+    J = bind.zeros_current(eg, "cuda")
+    sp = wl.species[0]
+    pe = P.species_to_ent(bind, synth, g, sp, "cuda")
+    ps = pe.empty_like()
+    bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 1)
+    bind.ent_sort(ctx, pe, ps, None)
+    bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 0)
+    pe, ps = ps, pe
+    for _ in range(3):
+        bind.ent_step(ctx, F, pe, J, wl.dt)
+    bind.ent_sort(ctx, pe, ps, None)
+    torch.cuda.synchronize()
+    assert bind.ent_get_stat(ctx, bind.STAT_LAST_SORT_REBIN) == 1
+    _match_perm(g, pe, ps)
+    keys, T = _host_keys(synth, bind, ctx, g, ps.cell)
+    tile_keys = (keys // int(np.prod(T))).astype(np.int32)
+    toff = bind.ent_tile_offsets(ctx, ps).cpu().numpy()
+    assert toff.shape[0] == ntiles + 1
+    assert orc.sort_check(tile_keys, ntiles, toff) == 0, "re-binned block / tile offsets rejected by orc_sort_check"
 
 
 def test_empty_block_is_accepted(env):
