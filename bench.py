@@ -214,14 +214,20 @@ def run_ours(args):
             if record:
                 b.record(stream); sort_ev.append((a, b))
 
+    fused = args.mode == "sorted" or (args.mode == "auto" and g.kind == synth.CART and args.step_impl == 0 and not args.tile)
+
     def one_step(it, record):
-        if args.sort_every > 0 and it > 0 and it % args.sort_every == 0:
+        if not fused and args.sort_every > 0 and it > 0 and it % args.sort_every == 0:
             do_sort(record)
         bind.ent_zero_current(ctx, J)
-        for p in parts:
+        for k in range(len(parts)):
             if record:
                 a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True); a.record(stream)
-            bind.ent_step(ctx, F, p, J, wl.dt)
+            if fused:                                    # fused step + re-bin, ping-pong between the two blocks: no ent_sort at all
+                bind.ent_step_sorted(ctx, F, parts[k], spare[k], J, wl.dt)
+                parts[k], spare[k] = spare[k], parts[k]
+            else:
+                bind.ent_step(ctx, F, parts[k], J, wl.dt)
             if record:
                 b.record(stream); step_ev.append((a, b))
         bind.ent_fold_current(ctx, J)
@@ -232,6 +238,7 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
+    bind.ent_reserve(ctx, max(p.n for p in parts))
     do_sort(False)                     # particles enter the timed region cell-sorted (BASELINE.json configs 3, 4)
     it = 0
     for _ in range(args.warmup):
@@ -271,7 +278,7 @@ def run_ours(args):
             "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
             "config": {"workload": f"{wl.name} ({wl.note})", "grid": list(g.N), "particles_per_gpu": npart, "species": len(parts),
-                       "dt": wl.dt, "shrink": args.shrink, "sorted_at_start": True, "sort_every": args.sort_every,
+                       "dt": wl.dt, "shrink": args.shrink, "sorted_at_start": True, "sort_every": 0 if fused else args.sort_every, "step_call": "ent_step_sorted" if fused else "ent_step",
                        "tiled_kernel": bool(tiled), "l2": "inputs larger than L2 (no flush needed)" if npart * pbytes > 4e8 else
                        "inputs smaller than L2: see note", "parallelism": "replicas only" if world > 1 else "1 GPU"},
             "clocks": clk, "gpu_launches": launches, "roofline": roofline,
@@ -323,6 +330,8 @@ def main():
     ap.add_argument("--step-impl", type=int, default=0, help="ENT_OPT_STEP_IMPL: 0 auto, 1 untiled, 2 two-kernel")
     ap.add_argument("--sort-mode", type=int, default=0, help="ENT_OPT_SORT_MODE: 0 auto (incremental re-bin), 1 always the full sort")
     ap.add_argument("--tile", default="", help="tile extents in cells, e.g. 8,8,8 (ENT_OPT_TILE_*; default: the library's)")
+    ap.add_argument("--mode", default="auto", choices=["auto", "sorted", "inplace"],
+                    help="sorted: ent_step_sorted (fused step + re-bin, out of place); inplace: ent_step + ent_sort every --sort-every steps; auto: sorted on Cartesian grids")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

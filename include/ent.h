@@ -11,7 +11,8 @@
  *
  * Conventions common to every call
  *   - every function returns 0 (ENT_OK) or a negative ent_status; it never throws, never exits and never
- *     synchronises the stream (except the *_host calls, which say so).  Work is enqueued on the CUDA stream
+ *     synchronises the stream (except the *_host calls, ent_reserve and the counters of ent_get_stat, which say so; a call that
+ *     has to grow the scratch pool because ent_reserve was not used also does).  Work is enqueued on the CUDA stream
  *     given to ent_create.  ent_last_error(ctx) returns a NUL-terminated message owned by ctx.
  *   - "device pointer" = memory allocated by the caller on the ctx's device (e.g. a torch tensor); the
  *     library never allocates or frees caller-visible memory.  All particle/field device pointers must be
@@ -122,7 +123,8 @@ int ent_deposit(ent_ctx *ctx, const ent_particles *old_, const ent_particles *ne
  * Dead particles keep their key.  On return `out` holds a permutation of `in` with non-decreasing keys
  * (order inside one cell unspecified) and, if key_offsets != NULL (device, int32[NKEYS+1]),
  * key_offsets[k] = number of particles with key < k.  in and out must not overlap; out's arrays must exist
- * wherever in's do.  The ctx remembers `out` as "sorted" so that ent_step may take its tiled path on it.
+ * wherever in's do (if only out has tags they are set to 1).  The ctx remembers `out` as "sorted" so that ent_step may take its
+ * tiled path on it and ent_step_sorted accepts it.
  * Incremental form (ENT_OPT_SORT_MODE = 0, the default): when `in` is itself a block a previous ent_sort of this ctx
  * produced (same pointers and n; its particles have drifted since) and key_offsets is NULL, only tile contiguity is
  * re-established: `out` is a permutation of `in` in which tile(key) is non-decreasing; the order inside a tile is
@@ -142,6 +144,32 @@ int ent_tile_offsets(ent_ctx *ctx, const ent_particles *block, int32_t *tile_off
  * that drifted out of their tile's halo since the sort take the global-atomic path inside the same kernel.
  * Otherwise the untiled kernel (global gathers, global atomics) runs.  Results agree up to fp32 summation order. */
 int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_current *J, float dt);
+
+/* ent_step_sorted = ent_step + the tile sort in ONE pass, out of place: every particle of `in` is advanced exactly as by
+ * ent_step (accumulating into J un-wrapped) and written to `out`, in the range of the tile its cell lay in BEFORE the step.
+ * `in` must be a sorted block of this ctx (the `out` of ent_sort or of a previous ent_step_sorted); `out` becomes one, ordered
+ * by positions that are one step stale -- every particle lies within one cell of the tile whose range holds it, which is the
+ * halo the kernel stages.  Calling it back and forth between two blocks (ping-pong) therefore never needs ent_sort again.
+ * `in` is not modified; in and out must not overlap; out->tag must exist if in->tag does or the grid has an ABSORB side.
+ * out->w, out->q, out->m are written.  Order of the particles inside a tile's range: unspecified.
+ * Contract: between the call that produced a sorted block and the call that consumes it, the caller must not change its
+ * cell / tag arrays (or must call ent_forget / ent_sort): the output layout is computed from per-tile populations recorded when
+ * the block was written.  Particles that contradict it are counted in ENT_STAT_SLOT_ERRORS and dropped; particles found more
+ * than one cell outside their tile take a slow global path (ENT_STAT_STRAYS) and are still placed correctly.
+ * ENT_EUNSUPPORTED: SPH / QSPH grids, N1 % 4 != 0, non-default tile shapes (use ent_step + ent_sort there). */
+int ent_step_sorted(ent_ctx *ctx, const ent_fields *EB, const ent_particles *in, ent_particles *out, ent_current *J, float dt);
+
+/* ---- scratch memory ------------------------------------------------------------------------------------------
+ * The ctx owns one device allocation ("pool") for sort keys, histograms, work lists and the layouts of up to 8 sorted blocks.
+ * ent_workspace_bytes: size of that pool for blocks of up to npart particles on the current grid (host-side arithmetic only).
+ * ent_reserve: allocates it now (may synchronise the stream).  Afterwards ent_sort / ent_step / ent_step_sorted on blocks of
+ * at most npart particles never allocate and never synchronise.  Without it the pool is (re)allocated by the first call that
+ * needs more, which synchronises and forgets every sorted block.  ent_set_grid releases the pool. */
+int ent_workspace_bytes(ent_ctx *ctx, int64_t npart, size_t *bytes);
+int ent_reserve(ent_ctx *ctx, int64_t npart);
+/* The ctx recognises a sorted block by (cell pointer, n).  ent_forget drops that record: call it before re-using the memory of
+ * a sorted block for something else, or after editing its cell / tag arrays (ent_gather_push does it for its `out`). */
+int ent_forget(ent_ctx *ctx, const ent_particles *block);
 
 /* J := 0 (all three padded arrays) */
 int ent_zero_current(ent_ctx *ctx, ent_current *J);
@@ -173,7 +201,9 @@ enum {
     ENT_STAT_STRAYS = 8,       /* particles that took the out-of-halo path in the last tiled ent_step (synchronises) */
     ENT_STAT_SCRATCH_BYTES = 9,
     ENT_STAT_LAST_STEP_TILED = 10,
-    ENT_STAT_LAST_SORT_REBIN = 11   /* 1 if the last ent_sort took the incremental re-bin path */
+    ENT_STAT_LAST_SORT_REBIN = 11,  /* 1 if the last ent_sort took the incremental re-bin path */
+    ENT_STAT_SLOT_ERRORS = 12       /* particles ent_step_sorted could not place (layout counts contradicted by the block: the caller
+                                       edited the cell arrays of a sorted block without ent_forget / ent_sort); synchronises */
 };
 int ent_set_option(ent_ctx *ctx, int key, int64_t value);
 int ent_get_stat(ent_ctx *ctx, int key, int64_t *value);

@@ -19,10 +19,10 @@ NGHOST = 2
 OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM = 0, -1, -2, -3, -4
 OPT_STEP_IMPL, OPT_TILE_1, OPT_TILE_2, OPT_TILE_3, OPT_SORT_MODE = 1, 2, 3, 4, 5
 (STAT_TILE_1, STAT_TILE_2, STAT_TILE_3, STAT_NKEYS, STAT_NTILES, STAT_LAUNCHES, STAT_BAD_MOVES, STAT_STRAYS,
- STAT_SCRATCH_BYTES, STAT_LAST_STEP_TILED, STAT_LAST_SORT_REBIN) = range(1, 12)
+ STAT_SCRATCH_BYTES, STAT_LAST_STEP_TILED, STAT_LAST_SORT_REBIN, STAT_SLOT_ERRORS) = range(1, 13)
 
 SYMBOLS = ["ent_create", "ent_destroy", "ent_last_error", "ent_set_grid", "ent_gather_push", "ent_deposit", "ent_sort",
-           "ent_step", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_step_host", "ent_set_option", "ent_get_stat", "ent_version"]
+           "ent_step", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_step_host", "ent_set_option", "ent_get_stat", "ent_version"]
 
 
 class EntError(RuntimeError):
@@ -56,7 +56,7 @@ def lib():
     """Loads libent.so (building it if the sources are newer).  Raises if it cannot be built or loaded."""
     global _lib
     if _lib is None:
-        path = os.environ.get("ENT_LIBENT") or _build.build()      # ENT_LIBENT: load a specific build (A/B timing of variants)
+        path = _build.build()
         if not os.path.exists(path):
             raise RuntimeError("libent.so is missing: the CUDA library is the product, there is no fallback")
         L = C.CDLL(path)
@@ -70,6 +70,10 @@ def lib():
         L.ent_deposit.argtypes = [vp, C.POINTER(_Particles), C.POINTER(_Particles), C.POINTER(_Current), C.c_float]
         L.ent_sort.argtypes = [vp, C.POINTER(_Particles), C.POINTER(_Particles), vp]
         L.ent_tile_offsets.argtypes = [vp, C.POINTER(_Particles), vp]
+        L.ent_step_sorted.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Particles), C.POINTER(_Current), C.c_float]
+        L.ent_workspace_bytes.argtypes = [vp, C.c_int64, C.POINTER(C.c_size_t)]
+        L.ent_reserve.argtypes = [vp, C.c_int64]
+        L.ent_forget.argtypes = [vp, C.POINTER(_Particles)]
         L.ent_step.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Current), C.c_float]
         L.ent_zero_current.argtypes = [vp, C.POINTER(_Current)]
         L.ent_fold_current.argtypes = [vp, C.POINTER(_Current)]
@@ -265,6 +269,24 @@ def ent_tile_offsets(ctx: Ctx, block: Particles) -> torch.Tensor:
 
 def ent_step(ctx: Ctx, EB, p: Particles, J, dt: float) -> None:
     ctx._ck(lib().ent_step(ctx._h, C.byref(_fields(EB)), C.byref(p.c()), C.byref(_current(J)), dt))
+
+
+def ent_step_sorted(ctx: Ctx, EB, pin: Particles, pout: Particles, J, dt: float) -> None:
+    ctx._ck(lib().ent_step_sorted(ctx._h, C.byref(_fields(EB)), C.byref(pin.c()), C.byref(pout.c()), C.byref(_current(J)), dt))
+
+
+def ent_workspace_bytes(ctx: Ctx, npart: int) -> int:
+    b = C.c_size_t(0)
+    ctx._ck(lib().ent_workspace_bytes(ctx._h, npart, C.byref(b)))
+    return b.value
+
+
+def ent_reserve(ctx: Ctx, npart: int) -> None:
+    ctx._ck(lib().ent_reserve(ctx._h, npart))
+
+
+def ent_forget(ctx: Ctx, block: Particles) -> None:
+    ctx._ck(lib().ent_forget(ctx._h, C.byref(block.c())))
 
 
 def ent_zero_current(ctx: Ctx, J) -> None:

@@ -8,6 +8,7 @@
 
 #include "ent_kernels.cuh"
 #include "ent_tiled_axisym.cuh"
+#include "ent_sorted.cuh"
 
 using namespace ent;
 
@@ -24,22 +25,22 @@ struct ent_ctx {
     int last_sort_rebin = 0;
     int rebin_ordered = 1;                // re-bin keeps the particles that stay in a tile ordered by cell (Cartesian grids)
     bool ord_attr_set = false;
-    int32_t *class_count = nullptr; size_t class_cap = 0;
     long long launches = 0;
-    // scratch
-    unsigned long long *counters = nullptr;   // [0] bad moves, [1] strays
-    int32_t *keys = nullptr;   long long keys_cap = 0;
-    int32_t *count = nullptr;  int32_t *offsets = nullptr; int32_t *cursor = nullptr; long long nkeys_cap = 0;
-    int32_t *chunk = nullptr;  long long chunk_cap = 0;
-    // "old" copy for the two-kernel step
+    // ---- scratch pool: ONE device allocation carved by reserve_pool(); hot calls never allocate once it is large enough (ent_reserve)
+    void *pool = nullptr; size_t pool_bytes = 0;
+    long long pool_n = -1;                    // particle count the pool was carved for (-1: none)
+    unsigned long long *counters = nullptr;   // [0] bad moves, [1] strays, [2] stray-list length, [3] slot errors (own tiny allocation)
+    int32_t *keys = nullptr, *count = nullptr, *offsets = nullptr, *cursor = nullptr, *chunk = nullptr, *class_count = nullptr;
+    // side buffers of the non-hot paths (two-kernel step, host-buffer step): allocated on first use
     void *oldbuf = nullptr; size_t oldbuf_cap = 0;
-    // host-call staging
     void *hbuf = nullptr; size_t hbuf_cap = 0;
-    size_t scratch_bytes = 0;
-    // the blocks ent_sort produced (most recent first): each keeps its own tile offsets so that several species
-    // can stay "sorted" at the same time
-    struct SortedBlock { const int32_t *cell = nullptr; long long n = -1; int32_t *tile_off = nullptr; size_t cap = 0;
-                         float *tile_wmax = nullptr; size_t wcap = 0; int32_t *chunk_off = nullptr; size_t ccap = 0; unsigned long long stamp = 0; };
+    size_t side_bytes = 0;
+    // the blocks ent_sort / ent_step_sorted produced: each keeps its own layout so that several species stay sorted at a time
+    struct SortedBlock { const int32_t *cell = nullptr; long long n = -1; int32_t *tile_off = nullptr; float *tile_wmax = nullptr;
+                         int32_t *chunk_off = nullptr;      // work list of the in-place tiled kernel (TILE_CHUNK particles per CTA)
+                         int32_t *chunk_off2 = nullptr;     // work list of the fused step + re-bin kernel (SORTED_CAP per CTA)
+                         int32_t *next_count = nullptr;     // particles per tile by their CURRENT cell (layout of the next ent_step_sorted output)
+                         bool wmax_valid = false, counts_valid = false; unsigned long long stamp = 0; };
     SortedBlock sorted[8];
     unsigned long long sort_stamp = 0;
     int last_step_tiled = 0;
@@ -65,16 +66,70 @@ static int launch_check(ent_ctx *ctx, const char *what) {
     return ENT_OK;
 }
 
+// side buffers (non-hot paths): grown on demand; may synchronise the stream
 static int ensure(ent_ctx *ctx, void **ptr, size_t *cap_bytes, size_t need) {
     if (*cap_bytes >= need && *ptr) return ENT_OK;
-    if (*ptr) { CK(cudaStreamSynchronize(ctx->stream)); CK(cudaFree(*ptr)); ctx->scratch_bytes -= *cap_bytes; *ptr = nullptr; *cap_bytes = 0; }
+    if (*ptr) { CK(cudaStreamSynchronize(ctx->stream)); CK(cudaFree(*ptr)); ctx->side_bytes -= *cap_bytes; *ptr = nullptr; *cap_bytes = 0; }
     cudaError_t e = cudaMalloc(ptr, need ? need : 16);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(ctx, ENT_ENOMEM, "cudaMalloc of %zu scratch bytes failed: %s", need, cudaGetErrorString(e)); }
-    *cap_bytes = need; ctx->scratch_bytes += need;
+    *cap_bytes = need; ctx->side_bytes += need;
     return ENT_OK;
 }
 
-extern "C" const char *ent_version(void) { return "0.1"; }
+// ---- scratch pool --------------------------------------------------------------------------------------------
+// Everything ent_sort / ent_step / ent_step_sorted need for blocks of up to n particles on the current grid, in ONE allocation.
+struct PoolLayout {
+    size_t keys, count, offsets, cursor, chunk, class_count, stray, slots, slot_stride, total;
+    long long nkeys, ntiles, stray_cap;
+};
+static size_t al256(size_t b) { return (b + 255) & ~(size_t)255; }
+static PoolLayout pool_layout(const GridDev &g, long long n) {
+    PoolLayout L{};
+    L.ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
+    L.nkeys = L.ntiles * g.tcells;
+    L.stray_cap = n / 16 + 4096;
+    const size_t nchunks = (size_t)((L.nkeys + 1 + SCAN_CHUNK - 1) / SCAN_CHUNK) + 1;
+    size_t off = 0;
+    L.keys = off;        off += al256((size_t)(n > 0 ? n : 1) * 4);
+    L.count = off;       off += al256((size_t)(L.nkeys + 1) * 4);
+    L.offsets = off;     off += al256((size_t)(L.nkeys + 1) * 4);
+    L.cursor = off;      off += al256((size_t)(L.nkeys + 1) * 4);
+    L.chunk = off;       off += al256(nchunks * 4);
+    L.class_count = off; off += al256((size_t)L.ntiles * REBIN_CLASSES * 4);
+    L.stray = off;       off += al256((size_t)L.stray_cap * 4);
+    L.slots = off;
+    L.slot_stride = 5 * al256((size_t)(L.ntiles + 1) * 4);       // tile_off, tile_wmax, chunk_off, chunk_off2, next_count
+    off += 8 * L.slot_stride;
+    L.total = off;
+    return L;
+}
+static void forget_all(ent_ctx *ctx) { for (auto &b : ctx->sorted) { b.cell = nullptr; b.n = -1; } }
+
+// makes the pool large enough for blocks of n particles.  Growing it synchronises the stream, frees and re-allocates (the
+// sorted-block registry is lost): call ent_reserve once with the largest block to keep that out of the hot calls.
+static int reserve_pool(ent_ctx *ctx, long long n) {
+    if (ctx->pool && ctx->pool_n >= n) return ENT_OK;
+    const PoolLayout L = pool_layout(ctx->g, n);
+    if (ctx->pool) { CK(cudaStreamSynchronize(ctx->stream)); CK(cudaFree(ctx->pool)); ctx->pool = nullptr; ctx->pool_bytes = 0; ctx->pool_n = -1; }
+    forget_all(ctx);
+    cudaError_t e = cudaMalloc(&ctx->pool, L.total);
+    if (e != cudaSuccess) { cudaGetLastError(); ctx->pool = nullptr; return fail(ctx, ENT_ENOMEM, "cudaMalloc of the %zu-byte scratch pool failed: %s", L.total, cudaGetErrorString(e)); }
+    ctx->pool_bytes = L.total; ctx->pool_n = n;
+    char *b = (char *)ctx->pool;
+    ctx->keys = (int32_t *)(b + L.keys); ctx->count = (int32_t *)(b + L.count); ctx->offsets = (int32_t *)(b + L.offsets);
+    ctx->cursor = (int32_t *)(b + L.cursor); ctx->chunk = (int32_t *)(b + L.chunk); ctx->class_count = (int32_t *)(b + L.class_count);
+    ctx->tiled.stray_list = (int32_t *)(b + L.stray); ctx->tiled.stray_cap = L.stray_cap;
+    const size_t part = L.slot_stride / 5;
+    for (int k = 0; k < 8; ++k) {
+        char *sb = b + L.slots + (size_t)k * L.slot_stride;
+        auto &S = ctx->sorted[k];
+        S.tile_off = (int32_t *)sb; S.tile_wmax = (float *)(sb + part); S.chunk_off = (int32_t *)(sb + 2 * part);
+        S.chunk_off2 = (int32_t *)(sb + 3 * part); S.next_count = (int32_t *)(sb + 4 * part);
+    }
+    return ENT_OK;
+}
+
+extern "C" const char *ent_version(void) { return "0.2"; }
 
 extern "C" const char *ent_last_error(const ent_ctx *ctx) { return ctx ? ctx->err : "null ctx"; }
 
@@ -101,10 +156,7 @@ extern "C" int ent_destroy(ent_ctx *ctx) {
     if (!ctx) return ENT_EINVAL;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    tiled_release(ctx->tiled);
-    cudaFree(ctx->counters); cudaFree(ctx->keys); cudaFree(ctx->count); cudaFree(ctx->offsets); cudaFree(ctx->cursor);
-    cudaFree(ctx->chunk); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf); cudaFree(ctx->class_count);
-    for (auto &b : ctx->sorted) { cudaFree(b.tile_off); cudaFree(b.tile_wmax); cudaFree(b.chunk_off); }
+    cudaFree(ctx->counters); cudaFree(ctx->pool); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf);
     cudaGetLastError();
     delete ctx;
     return ENT_OK;
@@ -138,7 +190,7 @@ extern "C" int ent_set_grid(ent_ctx *ctx, const ent_grid *gr) {
     }
     GridDev g{};
     g.D = D; g.kind = gr->kind;
-    const int deft[2][3] = { {16, 16, 1}, {8, 8, 8} };
+    const int deft[2][3] = { {16, 16, 1}, {8, 8, 4} };
     long long pad = 1;
     for (int a = 0; a < 3; ++a) {
         bool on = a < D;
@@ -166,7 +218,11 @@ extern "C" int ent_set_grid(ent_ctx *ctx, const ent_grid *gr) {
         g.dT = PI_D / gr->N[1];
     }
     ctx->grid = *gr; ctx->g = g; ctx->have_grid = true;
-    for (auto &b : ctx->sorted) { b.cell = nullptr; b.n = -1; }
+    forget_all(ctx);
+    if (ctx->pool) {                                            // the pool was carved for the previous grid
+        CK(cudaStreamSynchronize(ctx->stream)); CK(cudaFree(ctx->pool));
+        ctx->pool = nullptr; ctx->pool_bytes = 0; ctx->pool_n = -1; ctx->tiled.stray_list = nullptr; ctx->tiled.stray_cap = 0;
+    }
     return tiled_set_grid(ctx->tiled, g, ctx->err, sizeof(ctx->err));
 }
 
@@ -198,6 +254,12 @@ static int check_current(ent_ctx *ctx, const ent_current *J) {
     if (!J) return fail(ctx, ENT_EINVAL, "current struct is NULL");
     for (int c = 0; c < 3; ++c) if (!J->comp[c] || !al16(J->comp[c])) return fail(ctx, ENT_EINVAL, "current component %d NULL or misaligned", c);
     return ENT_OK;
+}
+static void forget_block(ent_ctx *ctx, const int32_t *cell) { for (auto &b : ctx->sorted) if (b.cell == cell) { b.cell = nullptr; b.n = -1; } }
+static ent_ctx::SortedBlock *find_block(ent_ctx *ctx, const ent_particles *p) {
+    if (!p->cell || p->n <= 0) return nullptr;
+    for (auto &b : ctx->sorted) if (b.cell == p->cell && b.n == p->n) return &b;
+    return nullptr;
 }
 static PartPtrs pp(const ent_particles *p) {
     PartPtrs r;
@@ -232,6 +294,7 @@ extern "C" int ent_gather_push(ent_ctx *ctx, const ent_fields *EB, const ent_par
     if (in->n != out->n) return fail(ctx, ENT_EINVAL, "in->n != out->n");
     if (!(in->m != 0.f)) return fail(ctx, ENT_EINVAL, "mass is zero");
     if (in->n == 0) return ENT_OK;
+    forget_block(ctx, out->cell);                             // `out` is overwritten: it is no longer a sorted block
     float eps = 0.5f * (in->q / in->m) * dt;
     DISPATCH(gather_push_kernel, nblk(in->n), ctx->g, fp(EB), pp(in), pp(out), (long long)in->n, eps, dt);
     return launch_check(ctx, "gather_push_kernel");
@@ -300,6 +363,27 @@ static int step_two_kernel(ent_ctx *ctx, const ent_fields *EB, ent_particles *p,
     return ent_deposit(ctx, &old, p, J, dt);
 }
 
+extern "C" int ent_workspace_bytes(ent_ctx *ctx, int64_t npart, size_t *bytes) {
+    if (!ctx) return ENT_EINVAL;
+    if (!ctx->have_grid) return fail(ctx, ENT_EINVAL, "ent_set_grid has not been called");
+    if (!bytes || npart < 0) return fail(ctx, ENT_EINVAL, "bad argument");
+    *bytes = pool_layout(ctx->g, npart).total;
+    return ENT_OK;
+}
+
+extern "C" int ent_reserve(ent_ctx *ctx, int64_t npart) {
+    ENTER();
+    if (npart < 0 || npart >= (1LL << 31)) return fail(ctx, ENT_EINVAL, "npart out of range");
+    return reserve_pool(ctx, npart);
+}
+
+extern "C" int ent_forget(ent_ctx *ctx, const ent_particles *block) {
+    if (!ctx) return ENT_EINVAL;
+    if (!block) return fail(ctx, ENT_EINVAL, "block is NULL");
+    forget_block(ctx, block->cell);
+    return ENT_OK;
+}
+
 extern "C" int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_current *J, float dt) {
     ENTER();
     int rc;
@@ -310,69 +394,88 @@ extern "C" int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, en
     if (p->n == 0) return ENT_OK;
     if (ctx->step_impl == 2) return step_two_kernel(ctx, EB, p, J, dt);
     float eps = 0.5f * (p->q / p->m) * dt;
-    const int32_t *tile_off = nullptr, *chunk_off = nullptr; const float *tile_wmax = nullptr;
-    for (auto &b : ctx->sorted) if (b.cell == p->cell && b.n == p->n) { tile_off = b.tile_off; tile_wmax = b.tile_wmax; chunk_off = b.chunk_off; }
-    if (ctx->step_impl == 0 && tile_off && tiled_supported(ctx->tiled, ctx->g)) {
+    ent_ctx::SortedBlock *sb = find_block(ctx, p);
+    if (ctx->step_impl == 0 && sb && tiled_supported(ctx->tiled, ctx->g)) {
+        if (!sb->wmax_valid) {                                   // a block ent_step_sorted produced: its per-tile max |w| was never needed
+            tile_wmax_kernel<<<(unsigned)((long long)ctx->g.nt[0] * ctx->g.nt[1] * ctx->g.nt[2]), 128, 0, ctx->stream>>>(sb->tile_off, p->w, sb->tile_wmax);
+            if ((rc = launch_check(ctx, "tile_wmax_kernel"))) return rc;
+            sb->wmax_valid = true;
+        }
         CK(cudaMemsetAsync(ctx->counters + 1, 0, 2 * sizeof(unsigned long long), ctx->stream));  // strays of THIS step, stray-list length
-        rc = tiled_step(ctx->tiled, ctx->g, ctx->stream, fp(EB), pp(p), cp(J), (long long)p->n, tile_off, tile_wmax, chunk_off, eps, dt, p->q,
+        rc = tiled_step(ctx->tiled, ctx->g, ctx->stream, fp(EB), pp(p), cp(J), (long long)p->n, sb->tile_off, sb->tile_wmax, sb->chunk_off, eps, dt, p->q,
                         1.0f / dt, ctx->counters, &ctx->launches, ctx->err, sizeof(ctx->err));
         if (rc == ENT_OK) ctx->last_step_tiled = 1;
+        sb->counts_valid = false;          // the particles moved inside their ranges: next_count no longer describes their current tiles
         return rc;
     }
     DISPATCH(step_untiled_kernel, nblk(p->n), ctx->g, fp(EB), pp(p), cp(J), (long long)p->n, eps, dt, p->q, 1.0f / dt, ctx->counters + 0);
     return launch_check(ctx, "step_untiled_kernel");
 }
 
-// claims a SortedBlock slot for `out` (never the one in `keep`), sized for ntiles
-static int claim_slot(ent_ctx *ctx, const ent_ctx::SortedBlock *keep, long long ntiles, ent_ctx::SortedBlock **res) {
+// claims a SortedBlock slot for `out` (never the one in `keep`)
+static ent_ctx::SortedBlock *claim_slot(ent_ctx *ctx, const ent_ctx::SortedBlock *keep, const int32_t *out_cell) {
+    forget_block(ctx, out_cell);
     ent_ctx::SortedBlock *slot = nullptr;
     for (auto &b : ctx->sorted) { if (&b == keep) continue; if (!b.cell) { slot = &b; break; } if (!slot || b.stamp < slot->stamp) slot = &b; }
-    slot->cell = nullptr; slot->n = -1;
-    int rc;
-    if ((rc = ensure(ctx, (void **)&slot->tile_off, &slot->cap, (size_t)(ntiles + 1) * 4))) return rc;
-    if ((rc = ensure(ctx, (void **)&slot->tile_wmax, &slot->wcap, (size_t)ntiles * 4))) return rc;
-    if ((rc = ensure(ctx, (void **)&slot->chunk_off, &slot->ccap, (size_t)(ntiles + 1) * 4))) return rc;
-    *res = slot;
-    return ENT_OK;
+    slot->cell = nullptr; slot->n = -1; slot->wmax_valid = false; slot->counts_valid = false;
+    return slot;
 }
 
-// work list of the tiled step for a sorted block: chunk_off = exclusive scan of ceil(tile count / TILE_CHUNK)
-static int build_work_list(ent_ctx *ctx, ent_ctx::SortedBlock *slot, long long ntiles) {
-    const int nchunks = (int)((ntiles + SCAN_CHUNK - 1) / SCAN_CHUNK);
+static int exclusive_scan(ent_ctx *ctx, const int32_t *in, long long m, int32_t *out, int32_t *copy) {
+    const int nchunks = (int)((m + SCAN_CHUNK - 1) / SCAN_CHUNK);
     int rc;
-    tile_chunks_kernel<<<nblk(ntiles), TPB, 0, ctx->stream>>>(slot->tile_off, ntiles, TILE_CHUNK, ctx->count);
-    if ((rc = launch_check(ctx, "tile_chunks_kernel"))) return rc;
-    scan_reduce_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, ntiles, ctx->chunk);
+    scan_reduce_kernel<<<nchunks, TPB, 0, ctx->stream>>>(in, m, ctx->chunk);
     if ((rc = launch_check(ctx, "scan_reduce_kernel"))) return rc;
     scan_chunks_kernel<<<1, TPB, 0, ctx->stream>>>(ctx->chunk, nchunks);
     if ((rc = launch_check(ctx, "scan_chunks_kernel"))) return rc;
-    scan_apply_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, ntiles, ctx->chunk, slot->chunk_off, ctx->cursor);
+    scan_apply_kernel<<<nchunks, TPB, 0, ctx->stream>>>(in, m, ctx->chunk, out, copy);
     return launch_check(ctx, "scan_apply_kernel");
 }
 
-// incremental ent_sort: `in` is tile-contiguous (src), particles have drifted; re-establish tile contiguity in `out`
-static int sort_rebin(ent_ctx *ctx, const ent_ctx::SortedBlock *src, const ent_particles *in, ent_particles *out) {
-    const GridDev &g = ctx->g;
-    const long long ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
-    const int nchunks = (int)((ntiles + SCAN_CHUNK - 1) / SCAN_CHUNK);
+// work lists of a sorted block: exclusive scans of ceil(tile population / chunk) for the two chunk sizes.  Scratch: ctx->count,
+// ctx->offsets (second copy of a scan, unused), both idle between the phases of ent_sort / ent_step_sorted.
+static int build_work_lists(ent_ctx *ctx, ent_ctx::SortedBlock *slot, long long ntiles) {
     int rc;
-    if ((rc = ensure(ctx, (void **)&ctx->class_count, &ctx->class_cap, (size_t)ntiles * REBIN_CLASSES * 4))) return rc;
-    ent_ctx::SortedBlock *slot;
-    if ((rc = claim_slot(ctx, src, ntiles, &slot))) return rc;
+    tile_chunks_kernel<<<nblk(ntiles), TPB, 0, ctx->stream>>>(slot->tile_off, ntiles, TILE_CHUNK, ctx->count);
+    if ((rc = launch_check(ctx, "tile_chunks_kernel"))) return rc;
+    if ((rc = exclusive_scan(ctx, ctx->count, ntiles, slot->chunk_off, ctx->offsets))) return rc;
+    tile_chunks_kernel<<<nblk(ntiles), TPB, 0, ctx->stream>>>(slot->tile_off, ntiles, SORTED_CAP, ctx->count);
+    if ((rc = launch_check(ctx, "tile_chunks_kernel"))) return rc;
+    return exclusive_scan(ctx, ctx->count, ntiles, slot->chunk_off2, ctx->offsets);
+}
+
+static RebinGeom rebin_geom(const GridDev &g) {
     RebinGeom G;
     G.D = g.D;
     for (int a = 0; a < 3; ++a) { G.N[a] = g.N[a]; G.T[a] = g.T[a]; G.nt[a] = g.nt[a]; G.per[a] = g.bc[a] == ENT_PERIODIC; G.dT[a] = make_magicdiv((uint32_t)g.T[a]); }
     G.dN0 = make_magicdiv((uint32_t)g.N[0]); G.dN01 = make_magicdiv((uint32_t)(g.N[0] * g.N[1]));
+    return G;
+}
+
+// next_count of a block whose particles drifted inside their ranges: population per tile by the CURRENT cells
+static int recount_tiles(ent_ctx *ctx, ent_ctx::SortedBlock *sb, const ent_particles *p) {
+    const GridDev &g = ctx->g;
+    const long long ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
+    CK(cudaMemsetAsync(sb->next_count, 0, (size_t)(ntiles + 1) * 4, ctx->stream));
+    rebin_count_kernel<<<(unsigned)ntiles, REBIN_TPB, 0, ctx->stream>>>(rebin_geom(g), p->cell, sb->tile_off, ctx->class_count, sb->next_count);
+    int rc = launch_check(ctx, "rebin_count_kernel");
+    if (rc == ENT_OK) sb->counts_valid = true;
+    return rc;
+}
+
+// incremental ent_sort: `in` is tile-contiguous (src), particles have drifted; re-establish tile contiguity in `out`
+static int sort_rebin(ent_ctx *ctx, ent_ctx::SortedBlock *src, const ent_particles *in, ent_particles *out) {
+    const GridDev &g = ctx->g;
+    const long long ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
+    int rc;
+    ent_ctx::SortedBlock *slot = claim_slot(ctx, src, out->cell);
+    const RebinGeom G = rebin_geom(g);
     CK(cudaMemsetAsync(ctx->count, 0, (size_t)(ntiles + 1) * 4, ctx->stream));
     CK(cudaMemsetAsync(slot->tile_wmax, 0, (size_t)ntiles * 4, ctx->stream));
     rebin_count_kernel<<<(unsigned)ntiles, REBIN_TPB, 0, ctx->stream>>>(G, in->cell, src->tile_off, ctx->class_count, ctx->count);
     if ((rc = launch_check(ctx, "rebin_count_kernel"))) return rc;
-    scan_reduce_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, ntiles, ctx->chunk);
-    if ((rc = launch_check(ctx, "scan_reduce_kernel"))) return rc;
-    scan_chunks_kernel<<<1, TPB, 0, ctx->stream>>>(ctx->chunk, nchunks);
-    if ((rc = launch_check(ctx, "scan_chunks_kernel"))) return rc;
-    scan_apply_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, ntiles, ctx->chunk, slot->tile_off, ctx->cursor);
-    if ((rc = launch_check(ctx, "scan_apply_kernel"))) return rc;
+    CK(cudaMemcpyAsync(slot->next_count, ctx->count, (size_t)ntiles * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+    if ((rc = exclusive_scan(ctx, ctx->count, ntiles, slot->tile_off, ctx->cursor))) return rc;
     if (g.kind == ENT_CART && g.tcells <= ORD_BINS && ctx->rebin_ordered) {
         if (!ctx->ord_attr_set) { CK(cudaFuncSetAttribute(rebin_scatter_ordered_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ORD_CAP_MAX * ORD_REC_BYTES)); ctx->ord_attr_set = true; }
         // staging capacity: 25 % above the mean tile population (a fuller tile is placed unordered), as small as possible so
@@ -388,9 +491,9 @@ static int sort_rebin(ent_ctx *ctx, const ent_ctx::SortedBlock *src, const ent_p
                                                                             g.kind != ENT_CART, (unsigned *)slot->tile_wmax);
         if ((rc = launch_check(ctx, "rebin_scatter_kernel"))) return rc;
     }
-    if ((rc = build_work_list(ctx, slot, ntiles))) return rc;
+    if ((rc = build_work_lists(ctx, slot, ntiles))) return rc;
     out->q = in->q; out->m = in->m;
-    slot->cell = out->cell; slot->n = in->n; slot->stamp = ++ctx->sort_stamp;
+    slot->cell = out->cell; slot->n = in->n; slot->stamp = ++ctx->sort_stamp; slot->wmax_valid = true; slot->counts_valid = true;
     ctx->last_sort_rebin = 1;
     return ENT_OK;
 }
@@ -400,65 +503,80 @@ extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *ou
     int rc;
     if ((rc = check_particles(ctx, in, "in", false)) || (rc = check_particles(ctx, out, "out", false))) return rc;
     if (in->n != out->n) return fail(ctx, ENT_EINVAL, "in->n != out->n");
-    if (in->cell == out->cell || in->w == out->w) return fail(ctx, ENT_EINVAL, "ent_sort is out-of-place: in and out overlap");
+    if (in->n > 0 && (in->cell == out->cell || in->w == out->w)) return fail(ctx, ENT_EINVAL, "ent_sort is out-of-place: in and out overlap");
     if (in->tag && !out->tag) return fail(ctx, ENT_EINVAL, "in has tags but out->tag is NULL");
     const GridDev &g = ctx->g;
     const long long n = in->n;
     const long long nkeys = (long long)g.nt[0] * g.nt[1] * g.nt[2] * g.tcells;
-    const long long m = nkeys;                                        // scan length; offsets has m + 1 entries
-    const int nchunks = (int)((m + SCAN_CHUNK - 1) / SCAN_CHUNK);
-    {   // scratch
-        size_t cap;
-        cap = (size_t)ctx->keys_cap * 4;
-        if ((rc = ensure(ctx, (void **)&ctx->keys, &cap, (size_t)(n ? n : 1) * 4))) return rc;
-        ctx->keys_cap = (long long)(cap / 4);
-        if (ctx->nkeys_cap < nkeys + 1) {
-            size_t c1 = (size_t)ctx->nkeys_cap * 4, c2 = c1, c3 = c1;
-            if ((rc = ensure(ctx, (void **)&ctx->count, &c1, (size_t)(nkeys + 1) * 4))) return rc;
-            if ((rc = ensure(ctx, (void **)&ctx->offsets, &c2, (size_t)(nkeys + 1) * 4))) return rc;
-            if ((rc = ensure(ctx, (void **)&ctx->cursor, &c3, (size_t)(nkeys + 1) * 4))) return rc;
-            ctx->nkeys_cap = nkeys + 1;
-        }
-        cap = (size_t)ctx->chunk_cap * 4;
-        if ((rc = ensure(ctx, (void **)&ctx->chunk, &cap, (size_t)nchunks * 4))) return rc;
-        ctx->chunk_cap = (long long)(cap / 4);
-    }
-    for (auto &b : ctx->sorted) if (b.cell == out->cell) { b.cell = nullptr; b.n = -1; }
+    const long long ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
+    if ((rc = reserve_pool(ctx, n))) return rc;
     ctx->last_sort_rebin = 0;
     if (ctx->sort_mode == 0 && !key_offsets && n > 0) {
-        const ent_ctx::SortedBlock *src = nullptr;
-        for (auto &b : ctx->sorted) if (b.cell == in->cell && b.n == n) src = &b;
+        ent_ctx::SortedBlock *src = find_block(ctx, in);
         if (src) return sort_rebin(ctx, src, in, out);
     }
+    forget_block(ctx, out->cell);
     CK(cudaMemsetAsync(ctx->count, 0, (size_t)(nkeys + 1) * 4, ctx->stream));
     if (n > 0) {
         if (g.D == 2) sort_hist_kernel<2><<<nblk(n), TPB, 0, ctx->stream>>>(g, in->cell, n, ctx->keys, ctx->count);
         else sort_hist_kernel<3><<<nblk(n), TPB, 0, ctx->stream>>>(g, in->cell, n, ctx->keys, ctx->count);
         if ((rc = launch_check(ctx, "sort_hist_kernel"))) return rc;
     }
-    scan_reduce_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, m, ctx->chunk);
-    if ((rc = launch_check(ctx, "scan_reduce_kernel"))) return rc;
-    scan_chunks_kernel<<<1, TPB, 0, ctx->stream>>>(ctx->chunk, nchunks);
-    if ((rc = launch_check(ctx, "scan_chunks_kernel"))) return rc;
-    scan_apply_kernel<<<nchunks, TPB, 0, ctx->stream>>>(ctx->count, m, ctx->chunk, ctx->offsets, ctx->cursor);
-    if ((rc = launch_check(ctx, "scan_apply_kernel"))) return rc;
+    if ((rc = exclusive_scan(ctx, ctx->count, nkeys, ctx->offsets, ctx->cursor))) return rc;
     if (n > 0) {
         sort_scatter_kernel<<<nblk(n), TPB, 0, ctx->stream>>>(ctx->keys, ctx->cursor, pp(in), pp(out), n, g.D, g.kind != ENT_CART);
         if ((rc = launch_check(ctx, "sort_scatter_kernel"))) return rc;
+        // in has no tags but out has: every particle is alive (ent.h)
+        if (!in->tag && out->tag) CK(cudaMemsetAsync(out->tag, 1, (size_t)n, ctx->stream));
     }
     if (key_offsets) CK(cudaMemcpyAsync(key_offsets, ctx->offsets, (size_t)(nkeys + 1) * 4, cudaMemcpyDeviceToDevice, ctx->stream));
     out->q = in->q; out->m = in->m;
-    {   // remember `out` as sorted, with its own copy of the tile offsets (tile t = particles [tile_off[t], tile_off[t+1]))
-        const long long ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
-        ent_ctx::SortedBlock *slot;
-        if ((rc = claim_slot(ctx, nullptr, ntiles, &slot))) return rc;
-        tile_offsets_kernel<<<nblk(ntiles + 1), TPB, 0, ctx->stream>>>(ctx->offsets, g.tcells, ntiles, slot->tile_off);
+    if (n > 0) {   // remember `out` as sorted, with its own layout (tile t = particles [tile_off[t], tile_off[t+1]))
+        ent_ctx::SortedBlock *slot = claim_slot(ctx, nullptr, out->cell);
+        tile_offsets_kernel<<<nblk(ntiles + 1), TPB, 0, ctx->stream>>>(ctx->offsets, g.tcells, ntiles, slot->tile_off, slot->next_count);
         if ((rc = launch_check(ctx, "tile_offsets_kernel"))) return rc;
         tile_wmax_kernel<<<(unsigned)ntiles, 128, 0, ctx->stream>>>(slot->tile_off, out->w, slot->tile_wmax);
         if ((rc = launch_check(ctx, "tile_wmax_kernel"))) return rc;
-        if ((rc = build_work_list(ctx, slot, ntiles))) return rc;
-        slot->cell = out->cell; slot->n = n; slot->stamp = ++ctx->sort_stamp;
+        if ((rc = build_work_lists(ctx, slot, ntiles))) return rc;
+        slot->cell = out->cell; slot->n = n; slot->stamp = ++ctx->sort_stamp; slot->wmax_valid = true; slot->counts_valid = true;
     }
+    return ENT_OK;
+}
+
+// ---- fused step + re-bin: the timed entry point on Cartesian grids ----------------------------------------------
+extern "C" int ent_step_sorted(ent_ctx *ctx, const ent_fields *EB, const ent_particles *in, ent_particles *out, ent_current *J, float dt) {
+    ENTER();
+    int rc;
+    if ((rc = check_fields(ctx, EB)) || (rc = check_current(ctx, J)) || (rc = check_particles(ctx, in, "in", false)) ||
+        (rc = check_particles(ctx, out, "out", true))) return rc;
+    if (in->n != out->n) return fail(ctx, ENT_EINVAL, "in->n != out->n");
+    if (!(dt > 0.f)) return fail(ctx, ENT_EINVAL, "dt must be positive");
+    if (!(in->m != 0.f)) return fail(ctx, ENT_EINVAL, "mass is zero");
+    if (in->tag && !out->tag) return fail(ctx, ENT_EINVAL, "in has tags but out->tag is NULL");
+    ctx->last_step_tiled = 0;
+    out->q = in->q; out->m = in->m;
+    if (in->n == 0) return ENT_OK;
+    if (in->cell == out->cell || in->w == out->w || in->u[0] == out->u[0]) return fail(ctx, ENT_EINVAL, "ent_step_sorted is out-of-place: in and out overlap");
+    if (!sorted_supported(ctx->tiled, ctx->g)) return fail(ctx, ENT_EUNSUPPORTED, "ent_step_sorted: Cartesian grids with N1 %% 4 == 0 and the default tile shape only");
+    ent_ctx::SortedBlock *src = find_block(ctx, in);
+    if (!src) return fail(ctx, ENT_EINVAL, "ent_step_sorted: `in` is not a sorted block of this ctx (call ent_sort first)");
+    const GridDev &g = ctx->g;
+    const long long ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
+    if (!src->counts_valid && (rc = recount_tiles(ctx, src, in))) return rc;
+    ent_ctx::SortedBlock *dst = claim_slot(ctx, src, out->cell);
+    // layout of `out`: exclusive scan of the populations by current tile; cursor = second copy, consumed by the kernel's reservations
+    if ((rc = exclusive_scan(ctx, src->next_count, ntiles, dst->tile_off, ctx->cursor))) return rc;
+    CK(cudaMemsetAsync(dst->next_count, 0, (size_t)(ntiles + 1) * 4, ctx->stream));
+    CK(cudaMemsetAsync(ctx->counters + 1, 0, sizeof(unsigned long long), ctx->stream));         // strays of THIS step
+    SortedArgs A;
+    A.g = g; A.F = fp(EB); A.J = cp(J); A.in = pp(in); A.out = pp(out);
+    A.tile_off = src->tile_off; A.chunk_off = src->chunk_off2; A.cursor = ctx->cursor; A.next_count = dst->next_count;
+    A.n = in->n; A.eps = 0.5f * (in->q / in->m) * dt; A.dt = dt; A.q = in->q; A.inv_dt = 1.0f / dt; A.counters = ctx->counters;
+    if ((rc = sorted_step(ctx->tiled, A, dt, ctx->stream, ctx->err, sizeof(ctx->err)))) return rc;
+    ctx->launches += 1;
+    if ((rc = build_work_lists(ctx, dst, ntiles))) return rc;
+    dst->cell = out->cell; dst->n = in->n; dst->stamp = ++ctx->sort_stamp; dst->wmax_valid = false; dst->counts_valid = true;
+    ctx->last_step_tiled = 1;
     return ENT_OK;
 }
 
@@ -467,12 +585,10 @@ extern "C" int ent_tile_offsets(ent_ctx *ctx, const ent_particles *block, int32_
     if (!block || !tile_offsets) return fail(ctx, ENT_EINVAL, "NULL argument");
     const GridDev &g = ctx->g;
     const long long ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
-    for (auto &b : ctx->sorted)
-        if (b.cell && b.cell == block->cell && b.n == block->n) {
-            CK(cudaMemcpyAsync(tile_offsets, b.tile_off, (size_t)(ntiles + 1) * 4, cudaMemcpyDeviceToDevice, ctx->stream));
-            return ENT_OK;
-        }
-    return fail(ctx, ENT_EINVAL, "the block is not one ent_sort of this ctx produced");
+    ent_ctx::SortedBlock *b = find_block(ctx, block);
+    if (!b) return fail(ctx, ENT_EINVAL, "the block is not a sorted block of this ctx");
+    CK(cudaMemcpyAsync(tile_offsets, b->tile_off, (size_t)(ntiles + 1) * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+    return ENT_OK;
 }
 
 extern "C" int ent_set_option(ent_ctx *ctx, int key, int64_t value) {
@@ -503,14 +619,14 @@ extern "C" int ent_get_stat(ent_ctx *ctx, int key, int64_t *value) {
         case ENT_STAT_NTILES:
             if (!ctx->have_grid) return fail(ctx, ENT_EINVAL, "no grid"); *value = (int64_t)g.nt[0] * g.nt[1] * g.nt[2]; return ENT_OK;
         case ENT_STAT_LAUNCHES: *value = ctx->launches; return ENT_OK;
-        case ENT_STAT_BAD_MOVES: case ENT_STAT_STRAYS: {
+        case ENT_STAT_BAD_MOVES: case ENT_STAT_STRAYS: case ENT_STAT_SLOT_ERRORS: {
             unsigned long long h[4];
             CK(cudaSetDevice(ctx->device));
             CK(cudaMemcpyAsync(h, ctx->counters, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
             CK(cudaStreamSynchronize(ctx->stream));
-            *value = (int64_t)h[key == ENT_STAT_BAD_MOVES ? 0 : 1]; return ENT_OK;
+            *value = (int64_t)h[key == ENT_STAT_BAD_MOVES ? 0 : (key == ENT_STAT_STRAYS ? 1 : 3)]; return ENT_OK;
         }
-        case ENT_STAT_SCRATCH_BYTES: *value = (int64_t)(ctx->scratch_bytes + tiled_scratch_bytes(ctx->tiled)); return ENT_OK;
+        case ENT_STAT_SCRATCH_BYTES: *value = (int64_t)(ctx->pool_bytes + ctx->side_bytes); return ENT_OK;
         case ENT_STAT_LAST_STEP_TILED: *value = ctx->last_step_tiled; return ENT_OK;
         case ENT_STAT_LAST_SORT_REBIN: *value = ctx->last_sort_rebin; return ENT_OK;
         default: return fail(ctx, ENT_EINVAL, "unknown stat %d", key);

@@ -14,6 +14,21 @@ struct PartPtrs {
 
 constexpr int TPB = 256;
 
+struct MagicDiv {                 // n / d for 0 <= n < 2^31, d >= 1 (multiply-high + shift)
+    uint32_t mul, shr, d;
+    __device__ __forceinline__ int div(int n) const { return d == 1 ? n : (int)(__umulhi((uint32_t)n, mul) >> shr); }
+};
+inline MagicDiv make_magicdiv(uint32_t d) {
+    MagicDiv f{0, 0, d};
+    if (d <= 1) return f;
+    uint32_t lg = 0; while ((1ull << lg) < d) ++lg;
+    uint32_t p = 31 + lg;
+    f.mul = (uint32_t)(((1ull << p) + d - 1) / d);
+    f.shr = p - 32;
+    return f;
+}
+
+
 // ---- S0-S5: ent_gather_push ----
 template <int D, int KIND>
 __global__ void __launch_bounds__(TPB) gather_push_kernel(GridDev g, FieldPtrs F, PartPtrs in, PartPtrs out, long long n,
@@ -224,10 +239,11 @@ __global__ void __launch_bounds__(TPB) scan_apply_kernel(const int32_t *in, long
     }
 }
 
-// tile_off[t] = key_offsets[t * tcells], t = 0..ntiles
-__global__ void tile_offsets_kernel(const int32_t *key_off, int tcells, long long ntiles, int32_t *tile_off) {
+// tile_off[t] = key_offsets[t * tcells], t = 0..ntiles; tile_count[t] = population of tile t
+__global__ void tile_offsets_kernel(const int32_t *key_off, int tcells, long long ntiles, int32_t *tile_off, int32_t *tile_count) {
     long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t <= ntiles) tile_off[t] = key_off[t * tcells];
+    if (t < ntiles) tile_count[t] = key_off[(t + 1) * tcells] - key_off[t * tcells];
 }
 
 // chunks[t] = ceil(count of tile t / chunk): the number of CTAs the tiled step gives to tile t
@@ -272,20 +288,6 @@ __global__ void __launch_bounds__(TPB) sort_scatter_kernel(const int32_t *keys, 
 // ---------------------------------------------------------------------------------------------------------
 constexpr int REBIN_TPB = 256;
 constexpr int REBIN_CLASSES = 28;            // 27 neighbours (3^D used) + "far"
-
-struct MagicDiv {                 // n / d for 0 <= n < 2^31, d >= 1 (multiply-high + shift)
-    uint32_t mul, shr, d;
-    __device__ __forceinline__ int div(int n) const { return d == 1 ? n : (int)(__umulhi((uint32_t)n, mul) >> shr); }
-};
-inline MagicDiv make_magicdiv(uint32_t d) {
-    MagicDiv f{0, 0, d};
-    if (d <= 1) return f;
-    uint32_t lg = 0; while ((1ull << lg) < d) ++lg;
-    uint32_t p = 31 + lg;
-    f.mul = (uint32_t)(((1ull << p) + d - 1) / d);
-    f.shr = p - 32;
-    return f;
-}
 
 struct RebinGeom {
     int D, N[3], T[3], nt[3], per[3];

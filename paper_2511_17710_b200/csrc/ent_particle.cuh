@@ -105,9 +105,14 @@ __device__ __forceinline__ void push_particle(const GridDev &g, const Loader &ld
 // Q = q w / dt; qw = q w.  Acc::add(comp, padded_index, value) accumulates one contribution.
 // All arithmetic is in the old cell's frame (small numbers only: "(real)(i+delta) is never necessary").
 // ---------------------------------------------------------------------------------------------------------
+// fp32 add to GLOBAL memory without a return value.  The pointers come out of structs handed to out-of-line functions, where the
+// compiler no longer knows their state space and would emit the generic atomic (with its shared-memory compare-and-swap branch).
+__device__ __forceinline__ void red_global_f32(float *p, float v) {
+    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(__cvta_generic_to_global(p)), "f"(v) : "memory");
+}
 struct GlobalAcc {
     float *const *J;
-    __device__ __forceinline__ void add(int comp, long long idx, float v) const { atomicAdd(J[comp] + idx, v); }
+    __device__ __forceinline__ void add(int comp, long long idx, float v) const { red_global_f32(J[comp] + idx, v); }
 };
 
 template <int D, class Acc>

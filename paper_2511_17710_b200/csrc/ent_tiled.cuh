@@ -75,20 +75,6 @@ struct TileGeom {
 
 struct TileMaps { CUtensorMap F[6]; CUtensorMap J[3]; };
 
-struct FastDiv {                  // n / d for 0 <= n < 2^31, d >= 1
-    uint32_t mul, shr, d;
-    __device__ __forceinline__ int div(int n) const { return d == 1 ? n : (int)(__umulhi((uint32_t)n, mul) >> shr); }
-};
-inline FastDiv make_fastdiv(uint32_t d) {
-    FastDiv f{0, 0, d};
-    if (d <= 1) return f;
-    uint32_t lg = 0; while ((1ull << lg) < d) ++lg;
-    uint32_t p = 31 + lg;
-    f.mul = (uint32_t)(((1ull << p) + d - 1) / d);
-    f.shr = p - 32;
-    return f;
-}
-
 struct TiledArgs {
     GridDev g;
     FieldPtrs F;
@@ -103,7 +89,7 @@ struct TiledArgs {
     float cdt[3];                 // dt / dx_d
     unsigned long long *counters; // [0] bad moves, [1] strays, [2] length of stray_list
     int32_t *stray_list; long long stray_cap;   // particles left to stray_kernel (all lanes busy there instead of one per warp here)
-    FastDiv divN0, divN01;
+    MagicDiv divN0, divN01;
 };
 
 // the global path for one particle (same code as step_untiled_kernel); kept out of line so that the tile loop stays lean
@@ -148,7 +134,7 @@ struct CarryCtx { float *const *J; long long gbase; int P0, P01; float unit; int
 __device__ __noinline__ void carry_fix(const CarryCtx &c, int comp, int off, int positive) {
     int bx = off % c.JX, r = off / c.JX, by = r % c.JY, bz = r / c.JY;
     long long idx = c.gbase + bx + (long long)c.P0 * by + (long long)c.P01 * bz;
-    atomicAdd(c.J[comp] + idx, positive ? c.unit : -c.unit);
+    red_global_f32(c.J[comp] + idx, positive ? c.unit : -c.unit);
 }
 __device__ __forceinline__ void acc_fixed(int *sJ, const CarryCtx &cc, int comp, int off, float scaled) {
     int v = __float2int_rn(scaled);
@@ -174,9 +160,6 @@ __device__ __forceinline__ void acc_fixed4(int *sJ, const CarryCtx &cc, int comp
 }
 #ifndef ENT_TILED_MINB
 #define ENT_TILED_MINB 3
-#endif
-#ifndef ENT_TILED_PREFETCH
-#define ENT_TILED_PREFETCH 1
 #endif
 
 constexpr int TILED_TPB = 256;
@@ -413,7 +396,6 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     // ---- one particle per thread and iteration, consecutive lanes on consecutive particles: every access is a fully
     // coalesced 128-byte line per warp, the work of a tile is balanced to within one particle per thread, and the order of the
     // particles inside the tile's range does not matter (the incremental ent_sort does not keep one)
-#if ENT_TILED_PREFETCH
     // software pipeline: the record of the thread's next particle is requested before the current one is advanced
     long long p = p0 + tid;
     int ncell = 0; float nd0 = 0.f, nd1 = 0.f, nd2 = 0.f, nu0 = 0.f, nu1 = 0.f, nu2 = 0.f, nw = 0.f; bool nlive = true;
@@ -441,23 +423,6 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
         A.P.u[0][p] = u[0]; A.P.u[1][p] = u[1]; A.P.u[2][p] = u[2];
         if (!ALLPER && code == 2) A.P.tag[p] = 0;
     }
-#else
-    for (long long p = p0 + tid; p < p1; p += TILED_TPB) {
-        int cell = A.P.cell[p];
-        float d[3] = { A.P.d[0][p], A.P.d[1][p], (D == 3) ? A.P.d[2][p] : 0.f };
-        float u[3] = { A.P.u[0][p], A.P.u[1][p], A.P.u[2][p] };
-        const float wgt = A.P.w[p];
-        const bool live = A.P.tag ? A.P.tag[p] != 0 : true;
-        if (!waited) { mbar_wait(&bar, 0); waited = true; }
-        if (!live) continue;
-        const int code = tile_particle<D, TX, TY, TZ, ALLPER>(A, T, p, cell, d, u, wgt);
-        if (code & 1) continue;
-        A.P.cell[p] = cell;
-        A.P.d[0][p] = d[0]; A.P.d[1][p] = d[1]; if (D == 3) A.P.d[2][p] = d[2];
-        A.P.u[0][p] = u[0]; A.P.u[1][p] = u[1]; A.P.u[2][p] = u[2];
-        if (!ALLPER && code == 2) A.P.tag[p] = 0;
-    }
-#endif
     if (!waited) mbar_wait(&bar, 0);          // never leave with a TMA load still in flight into this CTA's shared memory
     // ---- S8 flush: one TMA reduce-add per component into the un-wrapped padded J (ghost fold = ent_fold_current)
     __syncthreads();
@@ -496,18 +461,16 @@ struct TiledState {
     EncodeTiledFn encode = nullptr;
     bool tried_encode = false;
     int shape = -1;                         // index into the instantiated tile shapes, -1 = none fits
-    int32_t *stray_list = nullptr; long long stray_cap = 0;
+    int32_t *stray_list = nullptr; long long stray_cap = 0;     // ctx scratch (ent_reserve)
     const void *ptrF[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     const void *ptrJ[3] = {nullptr, nullptr, nullptr};
     TileMaps maps;
     bool attr_set[16] = {};
 };
 
-inline void tiled_release(TiledState &t) { cudaFree(t.stray_list); t.stray_list = nullptr; t.stray_cap = 0; }
-inline size_t tiled_scratch_bytes(const TiledState &t) { return t.scratch + (size_t)t.stray_cap * 4; }
 
 // instantiated tile shapes: index -> (D, TX, TY, TZ)
-#define ENT_TILE_SHAPES(X) X(0, 3, 8, 8, 8) X(1, 3, 16, 8, 4) X(2, 3, 32, 4, 4) X(3, 3, 16, 8, 8) X(4, 2, 16, 16, 1) X(5, 2, 32, 8, 1)
+#define ENT_TILE_SHAPES(X) X(0, 3, 8, 8, 4) X(1, 3, 8, 8, 8) X(2, 2, 16, 16, 1)
 
 inline int tiled_find_shape(const GridDev &g) {
 #define X(IDX, DD, A, B, C) if (g.D == DD && g.T[0] == A && g.T[1] == B && g.T[2] == C) return IDX;
@@ -577,8 +540,8 @@ inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, 
     void (*kern)(const TileMaps, const TiledArgs) = allper ? step_tiled_kernel<D, TX, TY, TZ, true> : step_tiled_kernel<D, TX, TY, TZ, false>;
     int slot = 2 * IDX + (allper ? 1 : 0);
     if constexpr (D == 2) {
-        if (A.g.kind == ENT_SPH) { kern = step_tiled_axisym_kernel<ENT_SPH, TX, TY>; slot = 12 + 2 * (IDX - 4); }
-        else if (A.g.kind == ENT_QSPH) { kern = step_tiled_axisym_kernel<ENT_QSPH, TX, TY>; slot = 13 + 2 * (IDX - 4); }
+        if (A.g.kind == ENT_SPH) { kern = step_tiled_axisym_kernel<ENT_SPH, TX, TY>; slot = 6; }
+        else if (A.g.kind == ENT_QSPH) { kern = step_tiled_axisym_kernel<ENT_QSPH, TX, TY>; slot = 7; }
     } else if (A.g.kind != ENT_CART) { snprintf(err, errn, "no 3D tiled kernel for this metric"); return ENT_EUNSUPPORTED; }
     if (!t.attr_set[slot]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM_BYTES);
@@ -602,18 +565,10 @@ inline int tiled_step(TiledState &t, const GridDev &g, cudaStream_t stream, Fiel
     TiledArgs A;
     A.g = g; A.F = F; A.J = J; A.P = P; A.key_off = key_off; A.tile_wmax = tile_wmax; A.chunk_off = chunk_off; A.ntiles = g.nt[0] * g.nt[1] * g.nt[2]; A.n = n;
     A.eps = eps; A.dt = dt; A.q = q; A.inv_dt = inv_dt; A.counters = counters;
-    {   // stray list: room for 1/16 of the block (beyond that the tile kernel advances strays itself)
-        long long want = n / 16 + 4096;
-        if (t.stray_cap < want) {
-            if (t.stray_list) { cudaStreamSynchronize(stream); cudaFree(t.stray_list); t.stray_list = nullptr; t.stray_cap = 0; }
-            if (cudaMalloc((void **)&t.stray_list, (size_t)want * 4) != cudaSuccess) { cudaGetLastError(); snprintf(err, errn, "cudaMalloc of the stray list failed"); return ENT_ENOMEM; }
-            t.stray_cap = want;
-        }
-        A.stray_list = t.stray_list; A.stray_cap = t.stray_cap;
-    }
+    A.stray_list = t.stray_list; A.stray_cap = t.stray_cap;
     for (int a = 0; a < 3; ++a) A.cdt[a] = dt * g.inv_dx[a];
-    A.divN0 = make_fastdiv((uint32_t)g.N[0]);
-    A.divN01 = make_fastdiv((uint32_t)(g.N[0] * g.N[1]));
+    A.divN0 = make_magicdiv((uint32_t)g.N[0]);
+    A.divN01 = make_magicdiv((uint32_t)(g.N[0] * g.N[1]));
     int rc = ENT_EUNSUPPORTED;
     switch (t.shape) {
 #define X(IDX, DD, A_, B_, C_) case IDX: rc = tiled_launch<IDX, DD, A_, B_, C_>(t, A, stream, err, errn); break;

@@ -18,7 +18,7 @@ struct BoxLoader {                       // gather() hands over the index inside
 __device__ __noinline__ void global_add(const CarryCtx &c, int comp, int off, float v) {
     int bx = off % c.JX, r = off / c.JX, by = r % c.JY, bz = r / c.JY;
     long long idx = c.gbase + bx + (long long)c.P0 * by + (long long)c.P01 * bz;
-    atomicAdd(c.J[comp] + idx, v);
+    red_global_f32(c.J[comp] + idx, v);
 }
 struct TileAcc {                         // Acc of deposit_particle_at: fixed-point add into the shared J tile
     int *sJ; const CarryCtx *cc; float Sc;

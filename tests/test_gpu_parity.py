@@ -149,6 +149,132 @@ def test_rebinned_block_matches_oracle(env, name):
     assert all(st["tiled"] == 1 and st["strays"] == 0 for st in stats.values())
 
 
+def _ids(p):
+    """particle identity carried by the weights of _with_id_weights"""
+    return torch.round((p.w.double() - 1.0) * 2.0 ** 20).long().cpu().numpy()
+
+
+def _with_id_weights(sp):
+    """w_k = 1 + k 2^-20 (exact in fp32): the weight doubles as a particle id, so that the permutation ent_step_sorted applies can
+    be followed without assuming anything about it.  Changes the recipe's uniform weights by < 26 %; both sides get the same w."""
+    assert sp.n < (1 << 18)
+    sp.w = (1.0 + torch.arange(sp.n, dtype=torch.float64) * 2.0 ** -20).to(torch.float32)
+    return sp
+
+
+def _take(orc, p, idx):
+    f = lambda a: None if a is None else np.ascontiguousarray(a[idx])
+    return orc.Particles(i=[f(a) for a in p.i], d=[f(a) for a in p.d], u=[f(a) for a in p.u], w=f(p.w), phi=f(p.phi), tag=f(p.tag))
+
+
+@pytest.mark.parametrize("name", ["C1", "C3/8", "C4/16", "C4/16-shuffled", "ABS3", "ABS2"])
+def test_step_sorted_matches_oracle(env, name):
+    """ent_step_sorted (fused step + re-bin, ping-pong between two blocks, no ent_sort after the first): every step is compared
+    with the oracle -- positions, momenta, current (end to end and the strict deposit check), continuity -- and the layout of
+    the output block is checked: tile offsets = exclusive scan of the histogram of the tiles of the INPUT positions (oracle's
+    sort checker), every particle in the range of the tile it started the step in, no strays, no slot errors."""
+    bind, synth, ctx, orc = env
+    wl = _workloads(synth)[name]()
+    g = wl.grid
+    eg, og = P.grid_to_ent(bind, g), P.grid_to_orc(orc, g)
+    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, 0)
+    bind.ent_set_grid(ctx, eg)
+    ntiles = bind.ent_get_stat(ctx, bind.STAT_NTILES)
+    F_dev, F_orc = [f.cuda() for f in wl.fields], P.fields_to_orc(wl.fields)
+    for sp in wl.species:
+        sp = _with_id_weights(sp)
+        pe0 = P.species_to_ent(bind, synth, g, sp, "cuda")
+        po = P.species_to_orc(orc, sp)
+        a, b = pe0.empty_like(), pe0.empty_like()
+        bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 1)
+        bind.ent_sort(ctx, pe0, a, None)
+        bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 0)
+        Jg = bind.zeros_current(eg, "cuda")
+        worstJ = worstC = strictJ = 0.0
+        for s in range(wl.steps):
+            ida = _ids(a)
+            before = P.ent_to_orc(orc, g, a)
+            keys, T = _host_keys(synth, bind, ctx, g, a.cell)
+            tile_before = keys // int(np.prod(T))
+            bind.ent_zero_current(ctx, Jg)
+            bind.ent_step_sorted(ctx, F_dev, a, b, Jg, wl.dt)
+            bind.ent_fold_current(ctx, Jg)
+            torch.cuda.synchronize()
+            assert bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED) == 1
+            assert bind.ent_get_stat(ctx, bind.STAT_SLOT_ERRORS) == 0 and bind.ent_get_stat(ctx, bind.STAT_STRAYS) == 0
+            assert bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES) == 0
+            idb = _ids(b)
+            assert np.array_equal(np.sort(idb), np.arange(sp.n)), "ent_step_sorted lost or duplicated particles"
+            # layout of the output block
+            toff = bind.ent_tile_offsets(ctx, b).cpu().numpy()
+            inv = np.empty(sp.n, dtype=np.int64); inv[ida] = np.arange(sp.n)          # slot in a of particle id
+            tile_of_slot_b = tile_before[inv[idb]].astype(np.int32)                   # tile each output slot's particle started in
+            assert orc.sort_check(tile_of_slot_b, ntiles, toff) == 0, "output block is not contiguous by the tiles of the input positions"
+            # oracle step, same particles in the oracle's own (original) order
+            Jo = orc.zeros_current(og)
+            orc.step(og, F_orc, po, Jo, sp.q, sp.m, wl.dt)
+            orc.fold_current(og, Jo)
+            worstJ = max(worstJ, P.compare_current(Jg, Jo))
+            after_slots = P.ent_to_orc(orc, g, b)
+            after = _take(orc, after_slots, np.argsort(idb)[ida])                     # the output in the order of `before`
+            strictJ = max(strictJ, P.compare_current(Jg, P.deposit_of_gpu_positions(orc, og, before, after, sp.q, wl.dt)))
+            c = P.continuity_of_gpu_step(orc, og, before, after, Jg, sp.q, wl.dt)
+            assert c <= P.CONT_TOL, f"continuity residual {c:.3e} at step {s}"
+            worstC = max(worstC, c)
+            st = P.compare_particles(g, b, po, idb, steps=s + 1)
+            a, b = b, a
+        print(name, sp.q, st, dict(worstJ=worstJ, strictJ=strictJ, worstC=worstC))
+
+
+def test_step_sorted_after_in_place_steps_and_error_paths(env):
+    """mixing calls: ent_step (in place, tiled) moves the particles inside their ranges, so ent_step_sorted must recount the tile
+    populations before it lays out its output; an unsorted input, overlapping blocks and axisymmetric grids are refused."""
+    bind, synth, ctx, orc = env
+    wl = synth.config3(8)
+    g = wl.grid
+    eg, og = P.grid_to_ent(bind, g), P.grid_to_orc(orc, g)
+    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, 0)
+    bind.ent_set_grid(ctx, eg)
+    F_dev, F_orc = [f.cuda() for f in wl.fields], P.fields_to_orc(wl.fields)
+    sp = _with_id_weights(wl.species[0])
+    pe0 = P.species_to_ent(bind, synth, g, sp, "cuda")
+    po = P.species_to_orc(orc, sp)
+    a, b = pe0.empty_like(), pe0.empty_like()
+    Jg = bind.zeros_current(eg, "cuda")
+    with pytest.raises(bind.EntError) as ei:
+        bind.ent_step_sorted(ctx, F_dev, pe0, b, Jg, wl.dt)                           # not a sorted block
+    assert ei.value.code == bind.EINVAL
+    bind.ent_sort(ctx, pe0, a, None)
+    with pytest.raises(bind.EntError):
+        bind.ent_step_sorted(ctx, F_dev, a, a, Jg, wl.dt)                             # overlap
+    for s in range(4):
+        Jo = orc.zeros_current(og)
+        orc.step(og, F_orc, po, Jo, sp.q, sp.m, wl.dt)
+        bind.ent_zero_current(ctx, Jg)
+        if s % 2 == 0:
+            bind.ent_step(ctx, F_dev, a, Jg, wl.dt)                                   # in place, tiled
+        else:
+            bind.ent_step_sorted(ctx, F_dev, a, b, Jg, wl.dt)
+            a, b = b, a
+        assert bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED) == 1
+    bind.ent_fold_current(ctx, Jg); orc.fold_current(og, Jo)
+    torch.cuda.synchronize()
+    assert bind.ent_get_stat(ctx, bind.STAT_SLOT_ERRORS) == 0
+    P.compare_current(Jg, Jo)
+    P.compare_particles(g, a, po, _ids(a), steps=4)
+    bind.ent_forget(ctx, a)
+    with pytest.raises(bind.EntError):
+        bind.ent_step_sorted(ctx, F_dev, a, b, Jg, wl.dt)                             # forgotten
+    wl5 = synth.config5(32)
+    bind.ent_set_grid(ctx, P.grid_to_ent(bind, wl5.grid))
+    p5 = P.species_to_ent(bind, synth, wl5.grid, wl5.species[0], "cuda")
+    q5, r5 = p5.empty_like(), p5.empty_like()
+    bind.ent_sort(ctx, p5, q5, None)
+    with pytest.raises(bind.EntError) as ei:
+        bind.ent_step_sorted(ctx, [f.cuda() for f in wl5.fields], q5, r5, bind.zeros_current(P.grid_to_ent(bind, wl5.grid), "cuda"), wl5.dt)
+    assert ei.value.code == bind.EUNSUPPORTED
+
+
 def _host_keys(synth, bind, ctx, g, cell):
     """sort keys recomputed on the host from the cell indices with the formula of include/ent.h (ent_sort)"""
     T = tuple(bind.ent_get_stat(ctx, k) for k in (bind.STAT_TILE_1, bind.STAT_TILE_2, bind.STAT_TILE_3))[:g.D]
