@@ -37,8 +37,7 @@ struct ent_ctx {
     size_t side_bytes = 0;
     // the blocks ent_sort / ent_step_sorted produced: each keeps its own layout so that several species stay sorted at a time
     struct SortedBlock { const int32_t *cell = nullptr; long long n = -1; int32_t *tile_off = nullptr; float *tile_wmax = nullptr;
-                         int32_t *chunk_off = nullptr;      // work list of the in-place tiled kernel (TILE_CHUNK particles per CTA)
-                         int32_t *chunk_off2 = nullptr;     // work list of the fused step + re-bin kernel (SORTED_CAP per CTA)
+                         int32_t *chunk_off = nullptr;      // work list of the tiled kernels (TILE_CHUNK particles per CTA)
                          int32_t *next_count = nullptr;     // particles per tile by their CURRENT cell (layout of the next ent_step_sorted output)
                          bool wmax_valid = false, counts_valid = false; unsigned long long stamp = 0; };
     SortedBlock sorted[8];
@@ -98,7 +97,7 @@ static PoolLayout pool_layout(const GridDev &g, long long n) {
     L.class_count = off; off += al256((size_t)L.ntiles * REBIN_CLASSES * 4);
     L.stray = off;       off += al256((size_t)L.stray_cap * 4);
     L.slots = off;
-    L.slot_stride = 5 * al256((size_t)(L.ntiles + 1) * 4);       // tile_off, tile_wmax, chunk_off, chunk_off2, next_count
+    L.slot_stride = 4 * al256((size_t)(L.ntiles + 1) * 4);       // tile_off, tile_wmax, chunk_off, next_count
     off += 8 * L.slot_stride;
     L.total = off;
     return L;
@@ -119,12 +118,12 @@ static int reserve_pool(ent_ctx *ctx, long long n) {
     ctx->keys = (int32_t *)(b + L.keys); ctx->count = (int32_t *)(b + L.count); ctx->offsets = (int32_t *)(b + L.offsets);
     ctx->cursor = (int32_t *)(b + L.cursor); ctx->chunk = (int32_t *)(b + L.chunk); ctx->class_count = (int32_t *)(b + L.class_count);
     ctx->tiled.stray_list = (int32_t *)(b + L.stray); ctx->tiled.stray_cap = L.stray_cap;
-    const size_t part = L.slot_stride / 5;
+    const size_t part = L.slot_stride / 4;
     for (int k = 0; k < 8; ++k) {
         char *sb = b + L.slots + (size_t)k * L.slot_stride;
         auto &S = ctx->sorted[k];
         S.tile_off = (int32_t *)sb; S.tile_wmax = (float *)(sb + part); S.chunk_off = (int32_t *)(sb + 2 * part);
-        S.chunk_off2 = (int32_t *)(sb + 3 * part); S.next_count = (int32_t *)(sb + 4 * part);
+        S.next_count = (int32_t *)(sb + 3 * part);
     }
     return ENT_OK;
 }
@@ -432,16 +431,13 @@ static int exclusive_scan(ent_ctx *ctx, const int32_t *in, long long m, int32_t 
     return launch_check(ctx, "scan_apply_kernel");
 }
 
-// work lists of a sorted block: exclusive scans of ceil(tile population / chunk) for the two chunk sizes.  Scratch: ctx->count,
-// ctx->offsets (second copy of a scan, unused), both idle between the phases of ent_sort / ent_step_sorted.
+// work list of a sorted block: exclusive scan of ceil(tile population / TILE_CHUNK).  Scratch: ctx->count, ctx->offsets (second
+// copy of the scan, unused), both idle between the phases of ent_sort / ent_step_sorted.
 static int build_work_lists(ent_ctx *ctx, ent_ctx::SortedBlock *slot, long long ntiles) {
     int rc;
     tile_chunks_kernel<<<nblk(ntiles), TPB, 0, ctx->stream>>>(slot->tile_off, ntiles, TILE_CHUNK, ctx->count);
     if ((rc = launch_check(ctx, "tile_chunks_kernel"))) return rc;
-    if ((rc = exclusive_scan(ctx, ctx->count, ntiles, slot->chunk_off, ctx->offsets))) return rc;
-    tile_chunks_kernel<<<nblk(ntiles), TPB, 0, ctx->stream>>>(slot->tile_off, ntiles, SORTED_CAP, ctx->count);
-    if ((rc = launch_check(ctx, "tile_chunks_kernel"))) return rc;
-    return exclusive_scan(ctx, ctx->count, ntiles, slot->chunk_off2, ctx->offsets);
+    return exclusive_scan(ctx, ctx->count, ntiles, slot->chunk_off, ctx->offsets);
 }
 
 static RebinGeom rebin_geom(const GridDev &g) {
@@ -557,25 +553,32 @@ extern "C" int ent_step_sorted(ent_ctx *ctx, const ent_fields *EB, const ent_par
     out->q = in->q; out->m = in->m;
     if (in->n == 0) return ENT_OK;
     if (in->cell == out->cell || in->w == out->w || in->u[0] == out->u[0]) return fail(ctx, ENT_EINVAL, "ent_step_sorted is out-of-place: in and out overlap");
-    if (!sorted_supported(ctx->tiled, ctx->g)) return fail(ctx, ENT_EUNSUPPORTED, "ent_step_sorted: Cartesian grids with N1 %% 4 == 0 and the default tile shape only");
+    if (!sorted_supported(ctx->tiled, ctx->g)) return fail(ctx, ENT_EUNSUPPORTED, "ent_step_sorted: Cartesian grids with N1 %% 4 == 0 only");
     ent_ctx::SortedBlock *src = find_block(ctx, in);
     if (!src) return fail(ctx, ENT_EINVAL, "ent_step_sorted: `in` is not a sorted block of this ctx (call ent_sort first)");
     const GridDev &g = ctx->g;
     const long long ntiles = (long long)g.nt[0] * g.nt[1] * g.nt[2];
     if (!src->counts_valid && (rc = recount_tiles(ctx, src, in))) return rc;
+    if (!src->wmax_valid) {
+        tile_wmax_kernel<<<(unsigned)ntiles, 128, 0, ctx->stream>>>(src->tile_off, in->w, src->tile_wmax);
+        if ((rc = launch_check(ctx, "tile_wmax_kernel"))) return rc;
+        src->wmax_valid = true;
+    }
     ent_ctx::SortedBlock *dst = claim_slot(ctx, src, out->cell);
     // layout of `out`: exclusive scan of the populations by current tile; cursor = second copy, consumed by the kernel's reservations
     if ((rc = exclusive_scan(ctx, src->next_count, ntiles, dst->tile_off, ctx->cursor))) return rc;
     CK(cudaMemsetAsync(dst->next_count, 0, (size_t)(ntiles + 1) * 4, ctx->stream));
+    CK(cudaMemsetAsync(dst->tile_wmax, 0, (size_t)(ntiles + 1) * 4, ctx->stream));
     CK(cudaMemsetAsync(ctx->counters + 1, 0, sizeof(unsigned long long), ctx->stream));         // strays of THIS step
     SortedArgs A;
     A.g = g; A.F = fp(EB); A.J = cp(J); A.in = pp(in); A.out = pp(out);
-    A.tile_off = src->tile_off; A.chunk_off = src->chunk_off2; A.cursor = ctx->cursor; A.next_count = dst->next_count;
+    A.tile_off = src->tile_off; A.chunk_off = src->chunk_off; A.tile_wmax = src->tile_wmax; A.cursor = ctx->cursor;
+    A.next_count = dst->next_count; A.wmax_out = (unsigned *)dst->tile_wmax;
     A.n = in->n; A.eps = 0.5f * (in->q / in->m) * dt; A.dt = dt; A.q = in->q; A.inv_dt = 1.0f / dt; A.counters = ctx->counters;
     if ((rc = sorted_step(ctx->tiled, A, dt, ctx->stream, ctx->err, sizeof(ctx->err)))) return rc;
     ctx->launches += 1;
     if ((rc = build_work_lists(ctx, dst, ntiles))) return rc;
-    dst->cell = out->cell; dst->n = in->n; dst->stamp = ++ctx->sort_stamp; dst->wmax_valid = false; dst->counts_valid = true;
+    dst->cell = out->cell; dst->n = in->n; dst->stamp = ++ctx->sort_stamp; dst->wmax_valid = true; dst->counts_valid = true;
     ctx->last_step_tiled = 1;
     return ENT_OK;
 }

@@ -60,6 +60,48 @@ __device__ __forceinline__ void tma_reduce_add_box(const CUtensorMap *map, const
 __device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 
+// ---- packed fp32 pairs (FFMA2 / FADD2 on sm_100a): two independent lerps per instruction ----
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void upk2(f32x2 v, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+// a + f * (b - a), per half (the same FADD, FFMA sequence as the scalar gather of ent_dev.cuh: identical results)
+__device__ __forceinline__ f32x2 lerp2(f32x2 a, f32x2 b, f32x2 f) {
+    f32x2 d, r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(b), "l"(a));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(f), "l"(d), "l"(a));
+    return r;
+}
+
+// S1 gather of the six components from a shared-memory box (stencil and arithmetic of ent_dev.cuh gather): b = cell in
+// box coordinates, d = in-cell offsets.  The seven lerps of a component run as packed pairs (z and z+1 planes together in 3D).
+template <int D, int FX, int FY, int FNP>
+__device__ __forceinline__ void gather_box(const float *sF, const int b[3], const float d[3], float EBv[6]) {
+    int xs[2], ys[2], zs[2]; float fx[2], fy[2], fz[2];              // [0] node-centred, [1] half-shifted
+    { bool lo = d[0] < 0.5f; xs[0] = b[0]; xs[1] = lo ? b[0] - 1 : b[0]; fx[0] = d[0]; fx[1] = lo ? d[0] + 0.5f : d[0] - 0.5f; }
+    { bool lo = d[1] < 0.5f; ys[0] = b[1] * FX; ys[1] = lo ? ys[0] - FX : ys[0]; fy[0] = d[1]; fy[1] = lo ? d[1] + 0.5f : d[1] - 0.5f; }
+    if (D == 3) { bool lo = d[2] < 0.5f; zs[0] = b[2] * (FX * FY); zs[1] = lo ? zs[0] - FX * FY : zs[0]; fz[0] = d[2]; fz[1] = lo ? d[2] + 0.5f : d[2] - 0.5f; }
+    else { zs[0] = zs[1] = 0; fz[0] = fz[1] = 0.f; }
+    const f32x2 FX2[2] = { pk2(fx[0], fx[0]), pk2(fx[1], fx[1]) }, FY2[2] = { pk2(fy[0], fy[0]), pk2(fy[1], fy[1]) };
+    const int ST[6][3] = { {1,0,0}, {0,1,0}, {0,0,1}, {0,1,1}, {1,0,1}, {1,1,0} };
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        const float *Fc = sF + c * FNP + (xs[ST[c][0]] + ys[ST[c][1]] + zs[ST[c][2]]);
+        if (D == 3) {
+            const float *Fh = Fc + FX * FY;
+            const f32x2 P00 = pk2(Fc[0], Fh[0]), P10 = pk2(Fc[1], Fh[1]), P01 = pk2(Fc[FX], Fh[FX]), P11 = pk2(Fc[FX + 1], Fh[FX + 1]);
+            const f32x2 L0 = lerp2(P00, P10, FX2[ST[c][0]]), L1 = lerp2(P01, P11, FX2[ST[c][0]]);
+            float lo, hi;
+            upk2(lerp2(L0, L1, FY2[ST[c][1]]), lo, hi);
+            EBv[c] = lo + fz[ST[c][2]] * (hi - lo);
+        } else {
+            const f32x2 P0 = pk2(Fc[0], Fc[FX]), P1 = pk2(Fc[1], Fc[FX + 1]);
+            float l0, l1;
+            upk2(lerp2(P0, P1, FX2[ST[c][0]]), l0, l1);
+            EBv[c] = l0 + fy[ST[c][1]] * (l1 - l0);
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // geometry of a tile in shared memory (compile time)
 // ---------------------------------------------------------------------------------------------------------
@@ -142,20 +184,20 @@ __device__ __forceinline__ void acc_fixed(int *sJ, const CarryCtx &cc, int comp,
     int nw = old + v;
     if (((old ^ nw) & (v ^ nw)) < 0) carry_fix(cc, comp, off, v > 0);
 }
-// four contributions of one component: all four atomics are issued before the first returned value is looked at, and
-// one test covers the four carries
+// four contributions of one component: all four atomics are issued before the first returned value is looked at.  One cheap,
+// conservative test covers the four carries: a contribution is below 2^25 in magnitude, so an accumulator can only wrap if its
+// old value is outside [-2^30, 2^30); only then the exact per-add test runs.
 __device__ __forceinline__ void acc_fixed4(int *sJ, const CarryCtx &cc, int comp, int o0, int o1, int o2, int o3,
                                            float s0, float s1, float s2, float s3) {
     int *Jc = sJ + comp * cc.JNP;
     int v0 = __float2int_rn(s0), v1 = __float2int_rn(s1), v2 = __float2int_rn(s2), v3 = __float2int_rn(s3);
     int a0 = atomicAdd(Jc + o0, v0), a1 = atomicAdd(Jc + o1, v1), a2 = atomicAdd(Jc + o2, v2), a3 = atomicAdd(Jc + o3, v3);
-    int n0 = a0 + v0, n1 = a1 + v1, n2 = a2 + v2, n3 = a3 + v3;
-    int t0 = (a0 ^ n0) & (v0 ^ n0), t1 = (a1 ^ n1) & (v1 ^ n1), t2 = (a2 ^ n2) & (v2 ^ n2), t3 = (a3 ^ n3) & (v3 ^ n3);
-    if ((t0 | t1 | t2 | t3) < 0) {
-        if (t0 < 0) carry_fix(cc, comp, o0, v0 > 0);
-        if (t1 < 0) carry_fix(cc, comp, o1, v1 > 0);
-        if (t2 < 0) carry_fix(cc, comp, o2, v2 > 0);
-        if (t3 < 0) carry_fix(cc, comp, o3, v3 > 0);
+    if ((((a0 + 0x40000000) | (a1 + 0x40000000)) | ((a2 + 0x40000000) | (a3 + 0x40000000))) < 0) {
+        int n0 = a0 + v0, n1 = a1 + v1, n2 = a2 + v2, n3 = a3 + v3;
+        if (((a0 ^ n0) & (v0 ^ n0)) < 0) carry_fix(cc, comp, o0, v0 > 0);
+        if (((a1 ^ n1) & (v1 ^ n1)) < 0) carry_fix(cc, comp, o1, v1 > 0);
+        if (((a2 ^ n2) & (v2 ^ n2)) < 0) carry_fix(cc, comp, o2, v2 > 0);
+        if (((a3 ^ n3) & (v3 ^ n3)) < 0) carry_fix(cc, comp, o3, v3 > 0);
     }
 }
 #ifndef ENT_TILED_MINB
@@ -179,8 +221,8 @@ __device__ __forceinline__ int find_tile(const int32_t *chunk_off, int ntiles, i
 
 // deposit of one particle through global atomics (ent_particle.cuh), out of line: used by the few particles of a tile that
 // cannot deposit into its shared-memory J tile
-template <int D>
-__device__ __noinline__ void edge_deposit(const TiledArgs &A, int i0, int i1, int i2, float a0, float a1, float a2, int di0, int di1, int di2,
+template <int D, class ARGS>
+__device__ __noinline__ void edge_deposit(const ARGS &A, int i0, int i1, int i2, float a0, float a1, float a2, int di0, int di1, int di2,
                                           float d0, float d1, float d2, float u0, float u1, float u2, float qw) {
     const int i[3] = { i0, i1, i2 }, di[3] = { di0, di1, di2 };
     const float a[3] = { a0, a1, a2 }, dn[3] = { d0, d1, d2 }, u[3] = { u0, u1, u2 };
@@ -236,31 +278,7 @@ __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D
     if (!local) { defer_stray(A, p, [&] { stray_step<D>(A, p); }); return 1; }
     // ---- S1 gather from the shared-memory box (same stencil as ent_dev.cuh gather)
     float EBv[6];
-    {
-        int xs[2], ys[2], zs[2]; float fx[2], fy[2], fz[2];              // [0] node-centred, [1] half-shifted
-        { bool lo = d[0] < 0.5f; xs[0] = b[0]; xs[1] = lo ? b[0] - 1 : b[0]; fx[0] = d[0]; fx[1] = lo ? d[0] + 0.5f : d[0] - 0.5f; }
-        { bool lo = d[1] < 0.5f; ys[0] = b[1] * G::FX; ys[1] = lo ? ys[0] - G::FX : ys[0]; fy[0] = d[1]; fy[1] = lo ? d[1] + 0.5f : d[1] - 0.5f; }
-        if (D == 3) { bool lo = d[2] < 0.5f; zs[0] = b[2] * (G::FX * G::FY); zs[1] = lo ? zs[0] - G::FX * G::FY : zs[0]; fz[0] = d[2]; fz[1] = lo ? d[2] + 0.5f : d[2] - 0.5f; }
-        else { zs[0] = zs[1] = 0; fz[0] = fz[1] = 0.f; }
-        const int ST[6][3] = { {1,0,0}, {0,1,0}, {0,0,1}, {0,1,1}, {1,0,1}, {1,1,0} };
-#pragma unroll
-        for (int c = 0; c < 6; ++c) {
-            const float *Fc = T.sF + c * G::FNP + (xs[ST[c][0]] + ys[ST[c][1]] + zs[ST[c][2]]);
-            const float f0 = fx[ST[c][0]], f1 = fy[ST[c][1]];
-            float v00 = Fc[0], v10 = Fc[1], v01 = Fc[G::FX], v11 = Fc[G::FX + 1];
-            float l0 = v00 + f0 * (v10 - v00), l1 = v01 + f0 * (v11 - v01);
-            float lo = l0 + f1 * (l1 - l0);
-            if (D == 3) {
-                const float f2 = fz[ST[c][2]];
-                const float *Fh = Fc + G::FX * G::FY;
-                float w00 = Fh[0], w10 = Fh[1], w01 = Fh[G::FX], w11 = Fh[G::FX + 1];
-                float h0 = w00 + f0 * (w10 - w00), h1 = w01 + f0 * (w11 - w01);
-                float hi = h0 + f1 * (h1 - h0);
-                lo = lo + f2 * (hi - lo);
-            }
-            EBv[c] = lo;
-        }
-    }
+    gather_box<D, G::FX, G::FY, G::FNP>(T.sF, b, d, EBv);
     // ---- S2 tetrad (A^hat = sqrt(h_ii) A^i), S3 Boris (Eq. 3), S4-S5 move + crossing
     float E[3] = { T.sx[0] * EBv[0], T.sx[1] * EBv[1], T.sx[2] * EBv[2] }, B[3] = { T.sx[0] * EBv[3], T.sx[1] * EBv[4], T.sx[2] * EBv[5] };
     boris(u, E, B, A.eps);
@@ -287,7 +305,7 @@ __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D
     if (bad) { atomicAdd(A.counters + 0, 1ULL); return 0; }
     const float qw = A.q * wgt;
     edge |= !(fabsf(wgt) <= T.wguard);        // a weight far above the tile's recorded maximum (changed since the sort) cannot use the tile's scale
-    if (edge) { edge_deposit<D>(A, iold[0], iold[1], iold[2], a0[0], a0[1], a0[2], di[0], di[1], di[2], d[0], d[1], d[2], u[0], u[1], u[2], qw); return 0; }     // rare: global atomics, un-wrapped from the true cell
+    if (edge) { edge_deposit<D, TiledArgs>(A, iold[0], iold[1], iold[2], a0[0], a0[1], a0[2], di[0], di[1], di[2], d[0], d[1], d[2], u[0], u[1], u[2], qw); return 0; }     // rare: global atomics, un-wrapped from the true cell
     // ---- S7 deposit into the shared-memory J tile (Eq. 6); node (b) of the box = element b of the J tile
     {
         const float Q = qw * A.inv_dt * T.Sc;                                // Q in fixed-point units
@@ -318,11 +336,12 @@ __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D
 #pragma unroll
                 for (int comp = 0; comp < 3; ++comp) {
                     const int a = (comp + 1) % 3, bb = (comp + 2) % 3;
-                    float c = Dv[a] * Dv[bb] * (1.0f / 12.0f);
-                    float QD = Q * Dv[comp];
-                    float w11 = W[a] * W[bb] + c, w10 = W[a] - w11, w01 = W[bb] - w11, w00 = 1.0f - W[a] - w01;
-                    acc_fixed4(T.sJ, T.cc, comp, base, base + st[a], base + st[bb], base + st[a] + st[bb],
-                               QD * w00, QD * w10, QD * w01, QD * w11);
+                    // the four products Q D_comp [w(W_a) w(W_b) +- D_a D_b / 12] directly: v11 = QD (W_a W_b + c), v10 = QD W_a - v11, ...
+                    const float QD = Q * Dv[comp];
+                    const float ta = QD * W[a], tb = QD * W[bb];
+                    const float v11 = fmaf(ta, W[bb], QD * (Dv[a] * Dv[bb] * (1.0f / 12.0f)));
+                    const float v10 = ta - v11, v01 = tb - v11, v00 = (QD - ta) - v01;
+                    acc_fixed4(T.sJ, T.cc, comp, base, base + st[a], base + st[bb], base + st[a] + st[bb], v00, v10, v01, v11);
                 }
             } else {
                 float q0 = Q * Dv[0], q1 = Q * Dv[1];
