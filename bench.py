@@ -5,6 +5,8 @@
 
 One "step" = one pass of the whole hot path over the synthetic plasma: zero J, ent_step for every species (serial host
 loop over species), periodic ghost fold, plus ent_sort every --sort-every steps (inside the timed region).
+The top-level numbers are the workload of --workload (default C3, the configuration BASELINE.json's metric is quoted on);
+without --workload the same line carries `per_config`: C4 sorted, C4 shuffled (its first ent_sort timed alone), C5, C2, C1.
 N > 1: one process per GPU (torchrun), every rank pushes an independent replica of the workload ("replicas only",
 DESIGN.md): no data-path collective, weak scaling, time = max over ranks.
 Prints ONE JSON line (rank 0).  --impl reference times the fp64 CPU oracle on a bounded sample of the same workload.
@@ -40,9 +42,6 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed ncu --set full capture
-# (profiles/r1_step_kernel_C3.md, section 2, current build); None where no capture exists
-NCU_TRAFFIC_BYTES = {"C3": 5.33e9}
 
 
 def max_over_ranks(value: float, device) -> float:
@@ -64,8 +63,8 @@ def _load_workload(name, shrink, device, rank=0):
 
 
 class ClockSampler:
-    """nvidia-smi sampled every 10 ms during the timed region (B200_PROFILING.md clocks line); the default timed region is
-    only ~60 ms long"""
+    """nvidia-smi sampled every 10 ms during the timed region (B200_PROFILING.md clocks line); short workloads repeat their timed
+    region until it lasts >= 0.5 s so that the sampler sees it"""
     Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
 
@@ -108,7 +107,6 @@ class ClockSampler:
 
 def _oracle_sample(name, target_particles=20_000_000):
     """a bounded sample of the same recipe for the CPU oracle: the workload with every grid extent divided by `shrink`"""
-    from paper_2511_17710_b200 import synth
     full = {"C1": 65536, "C2": 2097152, "C3": 134217728, "C4": 536870912, "C4s": 536870912, "C5": 268435456}[name]
     D = 3 if name in ("C3", "C4", "C4s") else 2
     shrink = 1
@@ -117,8 +115,18 @@ def _oracle_sample(name, target_particles=20_000_000):
     return shrink
 
 
-def time_oracle(name, steps, warmup):
-    """fp64 CPU oracle (oracle/orc.c, as it stands) on a bounded sample; returns (ns/particle/step, cores, sample text, ms/step)"""
+def _cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def time_oracle(name, steps, warmup, single_thread_too=False):
+    """fp64 CPU oracle (oracle/orc.c, as it stands) on a bounded sample; returns a dict"""
     sys.path.insert(0, os.path.join(ROOT, "tests"))
     import parity as P
     from oracle import orc
@@ -130,20 +138,33 @@ def time_oracle(name, steps, warmup):
     J = orc.zeros_current(og)
     npart = sum(p.n for p in parts)
 
-    def one():
+    def one(ps):
         for j in J:
             j[...] = 0.0
-        for sp, p in zip(wl.species, parts):
+        for sp, p in zip(wl.species, ps):
             orc.step(og, F, p, J, sp.q, sp.m, wl.dt)
         orc.fold_current(og, J)
     for _ in range(warmup):
-        one()
+        one(parts)
     t0 = time.perf_counter()
     for _ in range(steps):
-        one()
+        one(parts)
     dt = time.perf_counter() - t0
-    sample = f"{name} recipe with every grid extent / {shrink}: grid {tuple(wl.grid.N)}, {npart} particles, {steps} steps"
-    return dt / (npart * steps) * 1e9, orc.num_threads(), sample, dt / steps * 1e3, f"{wl.name} ({wl.note})"
+    out = {"value": dt / (npart * steps) * 1e9, "cores": orc.num_threads(), "ms_per_step": dt / steps * 1e3, "cpu_model": _cpu_model(),
+           "host_cores_available": len(os.sched_getaffinity(0)),
+           "sample": f"{name} recipe with every grid extent / {shrink}: grid {tuple(wl.grid.N)}, {npart} particles, {steps} steps",
+           "workload": f"{wl.name} ({wl.note})"}
+    if single_thread_too:                                     # one thread, 1/64 of the sample's particles, one step
+        sub = [orc.Particles(i=[a[::64].copy() for a in p.i], d=[a[::64].copy() for a in p.d], u=[a[::64].copy() for a in p.u],
+                             w=p.w[::64].copy(), phi=None if p.phi is None else p.phi[::64].copy(), tag=None if p.tag is None else p.tag[::64].copy())
+               for p in parts]
+        prev = orc.set_num_threads(1)
+        t0 = time.perf_counter()
+        one(sub)
+        out["single_thread_value"] = (time.perf_counter() - t0) / sum(p.n for p in sub) * 1e9
+        out["single_thread_sample"] = "every 64th particle of the sample, one step, 1 thread"
+        orc.set_num_threads(prev)
+    return out
 
 
 def run_reference(args):
@@ -151,32 +172,23 @@ def run_reference(args):
     if rank != 0:
         return
     steps, warmup = max(1, min(args.steps, 3)), min(args.warmup, 1)
-    v, cores, sample, ms, wname = time_oracle(args.workload, steps, warmup)
+    r = time_oracle(args.workload or "C3", steps, warmup)
+    v = r["value"]
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps, "warmup": warmup,
-            "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wname, "note": "fp64 CPU oracle (oracle/orc.c, as it stands) on a bounded sample of the workload"},
-            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "ms_per_step": r["ms_per_step"], "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": r["workload"], "note": "fp64 CPU oracle (oracle/orc.c, as it stands) on a bounded sample of the workload"},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"], "cpu_model": r["cpu_model"]},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line))
 
 
-def run_ours(args):
+def measure(args, name, env, want_e2e):
+    """times one workload on this rank's GPU; returns the dict of its numbers"""
     import torch
     import torch.distributed as dist
     from paper_2511_17710_b200 import binding as bind, synth
-    sys.path.insert(0, os.path.join(ROOT, "tests"))
-    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback (use --impl reference for the oracle)")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-    peak, peak_src = _peaks()
-
-    # ---- inputs: generated on the device, resident in HBM before the timed region ----
-    wl = _load_workload(args.workload, args.shrink, dev, rank)
+    rank, world, local, dev, peak, peak_src = env
+    wl = _load_workload(name, args.shrink, dev, rank)
     g = wl.grid
     eg = bind.Grid(D=g.D, N=tuple(g.N), bc=tuple(g.bc), kind=g.kind, xmin=tuple(g.xmin), xmax=tuple(g.xmax), r0=g.r0,
                    vartheta=g.vartheta)
@@ -200,36 +212,31 @@ def run_ours(args):
     npart = sum(p.n for p in parts)
     ncell = g.ncells
     pbytes = PARTICLE_BYTES[("cart" if g.kind == synth.CART else "axisym", g.D)]
+    fused = args.mode == "sorted"
+    step_ev, sort_ev = [], []          # (start, end) CUDA events around each ent_step / ent_sort call in the timed region
 
-    launches0 = [0]
-    step_ev = []                       # (start, end) CUDA events around each ent_step launch in the timed region
-    sort_ev = []
+    def timed(fn, store):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream); fn(); b.record(stream); store.append((a, b))
 
     def do_sort(record):
         for k in range(len(parts)):
-            if record:
-                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True); a.record(stream)
-            bind.ent_sort(ctx, parts[k], spare[k], None)
+            f = lambda: bind.ent_sort(ctx, parts[k], spare[k], None)
+            timed(f, sort_ev) if record else f()
             parts[k], spare[k] = spare[k], parts[k]
-            if record:
-                b.record(stream); sort_ev.append((a, b))
-
-    fused = args.mode == "sorted" or (args.mode == "auto" and g.kind == synth.CART and args.step_impl == 0 and not args.tile)
 
     def one_step(it, record):
         if not fused and args.sort_every > 0 and it > 0 and it % args.sort_every == 0:
             do_sort(record)
         bind.ent_zero_current(ctx, J)
         for k in range(len(parts)):
-            if record:
-                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True); a.record(stream)
             if fused:                                    # fused step + re-bin, ping-pong between the two blocks: no ent_sort at all
-                bind.ent_step_sorted(ctx, F, parts[k], spare[k], J, wl.dt)
-                parts[k], spare[k] = spare[k], parts[k]
+                def f():
+                    bind.ent_step_sorted(ctx, F, parts[k], spare[k], J, wl.dt)
+                    parts[k], spare[k] = spare[k], parts[k]
             else:
-                bind.ent_step(ctx, F, parts[k], J, wl.dt)
-            if record:
-                b.record(stream); step_ev.append((a, b))
+                f = lambda: bind.ent_step(ctx, F, parts[k], J, wl.dt)
+            timed(f, step_ev) if record else f()
         bind.ent_fold_current(ctx, J)
 
     def barrier():
@@ -239,61 +246,63 @@ def run_ours(args):
             torch.cuda.synchronize()
 
     bind.ent_reserve(ctx, max(p.n for p in parts))
-    do_sort(False)                     # particles enter the timed region cell-sorted (BASELINE.json configs 3, 4)
+    first_sort = []
+    for k in range(len(parts)):        # the particles enter the timed region tile-sorted (BASELINE.json configs 3, 4); timed alone
+        timed(lambda: bind.ent_sort(ctx, parts[k], spare[k], None), first_sort)
+        parts[k], spare[k] = spare[k], parts[k]
     it = 0
+    w0 = time.perf_counter()
     for _ in range(args.warmup):
         one_step(it, False); it += 1
     barrier()
-    launches0[0] = bind.ent_get_stat(ctx, bind.STAT_LAUNCHES)
+    est = (time.perf_counter() - w0) / max(1, args.warmup)
+    reps = max(1, min(2000, int(0.6 / max(est * args.steps, 1e-6)) + 1)) if est * args.steps < 0.5 else 1
+    launches0 = bind.ent_get_stat(ctx, bind.STAT_LAUNCHES)
     clocks = ClockSampler(local) if rank == 0 else None
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0.record(stream)
-    for _ in range(args.steps):
-        one_step(it, True); it += 1
+    for r in range(reps):              # the K steps, repeated so that a short workload is sampled by nvidia-smi too
+        for _ in range(args.steps):
+            one_step(it, r == 0); it += 1
     t1.record(stream)
     barrier()
-    ms = t0.elapsed_time(t1)
-    launches = bind.ent_get_stat(ctx, bind.STAT_LAUNCHES) - launches0[0]
+    ms = t0.elapsed_time(t1) / reps
+    launches = (bind.ent_get_stat(ctx, bind.STAT_LAUNCHES) - launches0) // reps
     clk = clocks.stop() if clocks else None
     tiled = bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED)
     strays = bind.ent_get_stat(ctx, bind.STAT_STRAYS)
     bad = bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES)
     ms = max_over_ranks(ms, dev)
     ms_per_step = ms / args.steps
-    value = ms * 1e6 / (npart * world * args.steps)
+    value = ms * 1e6 / (npart * world * args.steps)         # whole job: every rank advances its own replica (weak scaling)
 
-    # ---- roofline of the dominant kernel (the fused step kernel), per launch ----
+    # ---- roofline of the dominant kernel (the fused gather+push+move+deposit kernel), per launch ----
     k_ms = sum(a.elapsed_time(b) for a, b in step_ev) / max(1, len(step_ev))
-    n_launch_part = npart / len(parts)
-    alg_bytes = pbytes * n_launch_part + GRID_BYTES_PER_CELL * ncell
+    alg_bytes = pbytes * npart / len(parts) + GRID_BYTES_PER_CELL * ncell
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
-    sort_ms = (sum(a.elapsed_time(b) for a, b in sort_ev) / len(sort_ev)) if sort_ev else None
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": args.traffic if args.traffic is not None else (NCU_TRAFFIC_BYTES.get(args.workload) if args.shrink == 1 else None),
-                "kernel": "ent_step (fused gather+push+move+deposit), one species per launch", "kernel_ms": k_ms,
-                "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
-                "step_share": k_ms * len(parts) / ms_per_step}
-
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-            "data": "synthetic",
-            "config": {"workload": f"{wl.name} ({wl.note})", "grid": list(g.N), "particles_per_gpu": npart, "species": len(parts),
-                       "dt": wl.dt, "shrink": args.shrink, "sorted_at_start": True, "sort_every": 0 if fused else args.sort_every, "step_call": "ent_step_sorted" if fused else "ent_step",
-                       "tiled_kernel": bool(tiled), "l2": "inputs larger than L2 (no flush needed)" if npart * pbytes > 4e8 else
-                       "inputs smaller than L2: see note", "parallelism": "replicas only" if world > 1 else "1 GPU"},
-            "clocks": clk, "gpu_launches": launches, "roofline": roofline,
-            "particles_per_second": npart * world * args.steps / (ms * 1e-3),
-            "sort_ms_per_species": sort_ms, "strays_last_step": strays, "bad_moves": bad}
+    mean = lambda ev: (sum(a.elapsed_time(b) for a, b in ev) / len(ev)) if ev else None
+    out = {"name": name, "value": value, "ms_per_step": ms_per_step, "ms_timed": ms, "reps": reps, "npart": npart, "launches": launches,
+           "clocks": clk, "tiled": bool(tiled), "strays": strays, "bad_moves": bad, "kernel_ms": k_ms,
+           "sort_ms_per_species": mean(sort_ev), "first_sort_ms_per_species": mean(first_sort), "fused": fused,
+           "workload": f"{wl.name} ({wl.note})", "grid": list(g.N), "species": len(parts), "dt": wl.dt, "pbytes": pbytes,
+           "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                        "traffic": args.traffic, "traffic_source": args.traffic_source if args.traffic is not None else None,
+                        "kernel": ("ent_step_sorted" if fused else "ent_step") + " (fused gather+push+move+deposit), one species per launch",
+                        "kernel_ms": k_ms, "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
+                        "step_share": k_ms * len(parts) / ms_per_step}}
 
     # ---- end to end through the host-buffer C-ABI call: H2D of the step's inputs and D2H of its results inside ----
-    if not args.no_e2e and rank == 0 or (not args.no_e2e and world > 1):
+    if want_e2e:
         hp = [p.to("cpu", pin=True) for p in parts]
         hF = [f.cpu().pin_memory() for f in F]
         hJ = [torch.zeros(eg.padded_shape, dtype=torch.float32).pin_memory() for _ in range(3)]
+        del parts, spare
+        torch.cuda.empty_cache()
         nst = max(1, min(args.steps, args.e2e_steps))
         up = down = 0
         for p in hp:
             bind.ent_step_host(ctx, hF, p, hJ, wl.dt, 1)          # warm-up: staging allocation
+        tiled_e2e = bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED)
         barrier()
         w0 = time.perf_counter()
         for _ in range(nst):
@@ -302,17 +311,69 @@ def run_ours(args):
                 u_, d_ = bind.ent_step_host(ctx, hF, p, hJ, wl.dt, 1)
                 up += u_; down += d_
         barrier()
-        e_ms = (time.perf_counter() - w0) * 1e3
-        e_ms = max_over_ranks(e_ms, dev)
-        line["e2e"] = {"value": e_ms * 1e6 / (npart * world * nst), "unit": UNIT, "h2d_bytes_per_step": up, "d2h_bytes_per_step": down,
-                       "steps": nst, "ms_per_step": e_ms / nst, "call": "ent_step_host per species (pinned host buffers)"}
+        e_ms = max_over_ranks((time.perf_counter() - w0) * 1e3, dev)
+        out["e2e"] = {"value": e_ms * 1e6 / (npart * world * nst), "unit": UNIT, "h2d_bytes_per_step": up, "d2h_bytes_per_step": down,
+                      "steps": nst, "ms_per_step": e_ms / nst, "tiled_kernel": bool(tiled_e2e),
+                      "call": "ent_step_host per species: pinned host buffers -> H2D, ent_sort, ent_step (tiled), D2H"}
         del hp, hF, hJ
     bind.ent_destroy(ctx)
+    del F, J, wl
+    torch.cuda.empty_cache()
+    return out
 
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    peak, peak_src = _peaks()
+    env = (rank, world, local, dev, peak, peak_src)
+    main_wl = args.workload or "C3"
+    m = measure(args, main_wl, env, want_e2e=not args.no_e2e)
+    npart = m["npart"]
+    line = {"metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": m["ms_per_step"], "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": m["workload"], "grid": m["grid"], "particles_per_gpu": npart, "species": m["species"],
+                       "dt": m["dt"], "shrink": args.shrink, "sorted_at_start": True, "sort_every": 0 if m["fused"] else args.sort_every,
+                       "step_call": "ent_step_sorted" if m["fused"] else "ent_step", "tiled_kernel": m["tiled"],
+                       "timed_region_repeats": m["reps"],
+                       "l2": "inputs larger than L2 (no flush needed)" if npart * m["pbytes"] > 4e8 else
+                       "inputs smaller than L2: the workload itself is L2-resident (BASELINE.json's size), no flush",
+                       "parallelism": "replicas only" if world > 1 else "1 GPU"},
+            "clocks": m["clocks"], "gpu_launches": m["launches"], "roofline": m["roofline"],
+            "particles_per_second": npart * world * args.steps / (m["ms_timed"] * 1e-3),
+            "sort_ms_per_species": m["sort_ms_per_species"], "first_sort_ms_per_species": m["first_sort_ms_per_species"],
+            "strays_last_step": m["strays"], "bad_moves": m["bad_moves"]}
+    if "e2e" in m:
+        line["e2e"] = m["e2e"]
+    if args.workload is None and not args.no_per_config and world == 1:
+        per = []
+        for name in ("C4", "C4s", "C5", "C2", "C1"):
+            try:
+                r = measure(args, name, env, want_e2e=False)
+                per.append({"workload": r["workload"], "name": name, "particles": r["npart"], "value": r["value"], "unit": UNIT,
+                            "ms_per_step": r["ms_per_step"], "kernel_ms": r["kernel_ms"], "roofline_frac": r["roofline"]["frac"],
+                            "achieved_gbs": r["roofline"]["achieved"], "sort_ms_per_species": r["sort_ms_per_species"],
+                            "first_sort_ms_per_species": r["first_sort_ms_per_species"], "tiled_kernel": r["tiled"],
+                            "timed_region_repeats": r["reps"], "gpu_launches": r["launches"], "clocks": r["clocks"]})
+            except Exception as e:                            # e.g. not enough free memory on a smaller part: say so, keep the line
+                per.append({"name": name, "error": f"{type(e).__name__}: {e}"})
+        line["per_config"] = per
     if rank == 0:
         if not args.no_cpu and world == 1:
-            v, cores, sample, _, _ = time_oracle(args.workload, 2, 1)
-            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+            r = time_oracle(main_wl, 2, 1, single_thread_too=True)
+            line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
+                                    "cpu_model": r["cpu_model"], "host_cores_available": r["host_cores_available"],
+                                    "single_thread_value": r["single_thread_value"], "single_thread_sample": r["single_thread_sample"]}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -324,18 +385,22 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C4s", "C5"])
+    ap.add_argument("--workload", default=None, choices=["C1", "C2", "C3", "C4", "C4s", "C5"],
+                    help="default: C3 as the headline plus the per_config list of the other configurations")
     ap.add_argument("--shrink", type=int, default=1)
     ap.add_argument("--sort-every", type=int, default=3, help="ent_sort every k steps inside the timed region (0 = never)")
     ap.add_argument("--step-impl", type=int, default=0, help="ENT_OPT_STEP_IMPL: 0 auto, 1 untiled, 2 two-kernel")
     ap.add_argument("--sort-mode", type=int, default=0, help="ENT_OPT_SORT_MODE: 0 auto (incremental re-bin), 1 always the full sort")
-    ap.add_argument("--tile", default="", help="tile extents in cells, e.g. 8,8,8 (ENT_OPT_TILE_*; default: the library's)")
-    ap.add_argument("--mode", default="auto", choices=["auto", "sorted", "inplace"],
-                    help="sorted: ent_step_sorted (fused step + re-bin, out of place); inplace: ent_step + ent_sort every --sort-every steps; auto: sorted on Cartesian grids")
+    ap.add_argument("--tile", default="", help="tile extents in cells, e.g. 8,8,4 (ENT_OPT_TILE_*; default: the library's)")
+    ap.add_argument("--mode", default="inplace", choices=["sorted", "inplace"],
+                    help="inplace (default): ent_step + ent_sort every --sort-every steps; sorted: ent_step_sorted (fused step + re-bin, out of place)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--traffic", type=float, default=None, help="dram bytes per launch of the dominant kernel from an ncu --set full capture (default: the committed one in profiles/)")
+    ap.add_argument("--no-per-config", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel from an ncu --set full capture of THIS build")
+    ap.add_argument("--traffic-source", default=None, help="the capture --traffic comes from (file under profiles/, commit)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -178,10 +178,11 @@ int ent_zero_current(ent_ctx *ctx, ent_current *J);
 int ent_fold_current(ent_ctx *ctx, ent_current *J);
 
 /* ---- host-buffer variant (end-to-end measurement) --------------------------------------------------------------
- * Same as `nsteps` x ent_step, but every pointer in EB, p and J is a HOST pointer (pinned memory recommended).
- * Copies E,B and the particle block to ctx-owned device staging, zeroes the device J, runs the steps, copies the
- * particle block and J back.  Synchronises the stream before returning.  *h2d_bytes / *d2h_bytes (may be NULL)
- * receive the bytes copied in each direction. */
+ * Every pointer in EB, p and J is a HOST pointer (pinned memory recommended).  Copies E,B and the particle block to ctx-owned
+ * device staging, zeroes the device J, sorts the block by tile (ent_sort, full form), runs `nsteps` x ent_step on the sorted
+ * block (the tiled kernel where the grid supports it), copies the particle block and J back.  The block comes back PERMUTED
+ * (tile-sorted order; every array alike, w included).  Synchronises the stream before returning.  *h2d_bytes / *d2h_bytes
+ * (may be NULL) receive the bytes copied in each direction. */
 int ent_step_host(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_current *J, float dt, int nsteps,
                   int64_t *h2d_bytes, int64_t *d2h_bytes);
 

@@ -24,6 +24,14 @@ int orc_num_threads(void) {
 #endif
 }
 
+int orc_set_num_threads(int n) {
+    int prev = orc_num_threads();
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#endif
+    return prev;
+}
+
 /* ------------------------------------------------------------------------------------------
  * array geometry: planar padded arrays, x1 fastest, N_GHOST = 2 each side.
  * element (i,j,k) of the active grid sits at padded index (i+2, j+2, k+2).

@@ -107,6 +107,7 @@ int orc_sort_check(const int64_t n, const int32_t *keys_sorted, int64_t ncell, c
 
 int64_t orc_padded_size(const orc_grid *g);
 int     orc_num_threads(void);
+int     orc_set_num_threads(int n);                                         /* returns the previous count */
 
 #ifdef __cplusplus
 }

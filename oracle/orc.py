@@ -86,6 +86,7 @@ def lib():
         L.orc_sort_check.argtypes = [C.c_int64, C.c_void_p, C.c_int64, C.c_void_p]
         L.orc_padded_size.restype = C.c_int64; L.orc_padded_size.argtypes = [C.POINTER(_Grid)]
         L.orc_num_threads.restype = C.c_int
+        L.orc_set_num_threads.restype = C.c_int; L.orc_set_num_threads.argtypes = [C.c_int]
         _lib = L
     return _lib
 
@@ -308,3 +309,8 @@ def sort_check(keys_sorted, ncell, offsets=None) -> int:
 
 def num_threads() -> int:
     return lib().orc_num_threads()
+
+
+def set_num_threads(n: int) -> int:
+    """OpenMP thread count of the following oracle calls; returns the previous one (bench.py's single-thread figure)"""
+    return lib().orc_set_num_threads(int(n))

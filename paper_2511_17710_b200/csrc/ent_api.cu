@@ -189,7 +189,7 @@ extern "C" int ent_set_grid(ent_ctx *ctx, const ent_grid *gr) {
     }
     GridDev g{};
     g.D = D; g.kind = gr->kind;
-    const int deft[2][3] = { {16, 16, 1}, {8, 8, 4} };
+    const int deft[2][3] = { {16, 16, 1}, {8, 8, 8} };
     long long pad = 1;
     for (int a = 0; a < 3; ++a) {
         bool on = a < D;
@@ -636,7 +636,7 @@ extern "C" int ent_get_stat(ent_ctx *ctx, int key, int64_t *value) {
     }
 }
 
-// ---- host-buffer variant: H2D, nsteps x ent_step, D2H, all inside the call (end-to-end measurement) ----
+// ---- host-buffer variant: H2D, ent_sort, nsteps x ent_step (tiled kernel), D2H, all inside the call (end-to-end measurement) ----
 extern "C" int ent_step_host(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_current *J, float dt, int nsteps,
                              int64_t *h2d_bytes, int64_t *d2h_bytes) {
     ENTER();
@@ -647,10 +647,11 @@ extern "C" int ent_step_host(ent_ctx *ctx, const ent_fields *EB, ent_particles *
     const size_t fslot = (pad * 4 + 255) & ~(size_t)255, pslot = (n * 4 + 255) & ~(size_t)255;
     const bool axisym = g.kind != ENT_CART;
     int rc;
-    if ((rc = ensure(ctx, &ctx->hbuf, &ctx->hbuf_cap, fslot * 9 + pslot * 10))) return rc;
+    if ((rc = ensure(ctx, &ctx->hbuf, &ctx->hbuf_cap, fslot * 9 + pslot * 20))) return rc;      // fields, J, two particle blocks
+    if ((rc = reserve_pool(ctx, (long long)n))) return rc;
     char *b = (char *)ctx->hbuf;
     int64_t up = 0, down = 0;
-    ent_fields dEB; ent_current dJ; ent_particles dp = *p;
+    ent_fields dEB; ent_current dJ; ent_particles dp = *p, ds = *p;
     for (int c = 0; c < 6; ++c) {
         if (!EB->comp[c]) return fail(ctx, ENT_EINVAL, "host field component %d is NULL", c);
         float *dst = (float *)(b + fslot * c);
@@ -661,29 +662,39 @@ extern "C" int ent_step_host(ent_ctx *ctx, const ent_fields *EB, ent_particles *
         if (!J->comp[c]) return fail(ctx, ENT_EINVAL, "host current component %d is NULL", c);
         dJ.comp[c] = (float *)(b + fslot * (6 + c));
     }
-    char *pb = b + fslot * 9;
-    struct Arr { void **dev; void *host; size_t bytes; bool back; };
+    char *pb = b + fslot * 9, *sb = pb + pslot * 10;          // staged block (as uploaded) and its sorted copy
+    struct Arr { void **dev; void **srt; void *host; size_t bytes; bool back; };
     Arr arrs[10]; int na = 0;
-    dp.cell = (int32_t *)(pb + pslot * 0); arrs[na++] = { (void **)&dp.cell, p->cell, n * 4, true };
+    dp.cell = (int32_t *)(pb + pslot * 0); ds.cell = (int32_t *)(sb + pslot * 0); arrs[na++] = { (void **)&dp.cell, (void **)&ds.cell, p->cell, n * 4, true };
     for (int a = 0; a < 3; ++a) {
-        if (a < g.D) { dp.d[a] = (float *)(pb + pslot * (1 + a)); arrs[na++] = { (void **)&dp.d[a], p->d[a], n * 4, true }; }
-        else dp.d[a] = nullptr;
-        dp.u[a] = (float *)(pb + pslot * (4 + a)); arrs[na++] = { (void **)&dp.u[a], p->u[a], n * 4, true };
+        if (a < g.D) { dp.d[a] = (float *)(pb + pslot * (1 + a)); ds.d[a] = (float *)(sb + pslot * (1 + a)); arrs[na++] = { (void **)&dp.d[a], (void **)&ds.d[a], p->d[a], n * 4, true }; }
+        else dp.d[a] = ds.d[a] = nullptr;
+        dp.u[a] = (float *)(pb + pslot * (4 + a)); ds.u[a] = (float *)(sb + pslot * (4 + a)); arrs[na++] = { (void **)&dp.u[a], (void **)&ds.u[a], p->u[a], n * 4, true };
     }
-    dp.w = (float *)(pb + pslot * 7); arrs[na++] = { (void **)&dp.w, p->w, n * 4, false };
-    if (axisym) { dp.phi = (float *)(pb + pslot * 8); arrs[na++] = { (void **)&dp.phi, p->phi, n * 4, true }; } else dp.phi = nullptr;
-    if (p->tag) { dp.tag = (uint8_t *)(pb + pslot * 9); arrs[na++] = { (void **)&dp.tag, p->tag, n, true }; } else dp.tag = nullptr;
+    dp.w = (float *)(pb + pslot * 7); ds.w = (float *)(sb + pslot * 7); arrs[na++] = { (void **)&dp.w, (void **)&ds.w, p->w, n * 4, true };
+    if (axisym) { dp.phi = (float *)(pb + pslot * 8); ds.phi = (float *)(sb + pslot * 8); arrs[na++] = { (void **)&dp.phi, (void **)&ds.phi, p->phi, n * 4, true }; }
+    else dp.phi = ds.phi = nullptr;
+    if (p->tag) { dp.tag = (uint8_t *)(pb + pslot * 9); ds.tag = (uint8_t *)(sb + pslot * 9); arrs[na++] = { (void **)&dp.tag, (void **)&ds.tag, p->tag, n, true }; }
+    else dp.tag = ds.tag = nullptr;
     for (int k = 0; k < na; ++k) {
         if (!arrs[k].host) return fail(ctx, ENT_EINVAL, "a required host particle array is NULL");
         if (arrs[k].bytes) CK(cudaMemcpyAsync(*arrs[k].dev, arrs[k].host, arrs[k].bytes, cudaMemcpyHostToDevice, ctx->stream));
         up += (int64_t)arrs[k].bytes;
     }
     if ((rc = ent_zero_current(ctx, &dJ))) return rc;
+    // tile sort of the uploaded block, so that the steps run the tiled kernel (the block comes back in that order)
+    forget_block(ctx, dp.cell);
+    const int saved_mode = ctx->sort_mode;
+    ctx->sort_mode = 1;
+    rc = n ? ent_sort(ctx, &dp, &ds, nullptr) : ENT_OK;
+    ctx->sort_mode = saved_mode;
+    if (rc) return rc;
     for (int s = 0; s < nsteps; ++s)
-        if ((rc = ent_step(ctx, &dEB, &dp, &dJ, dt))) return rc;
+        if ((rc = ent_step(ctx, &dEB, &ds, &dJ, dt))) return rc;
+    forget_block(ctx, ds.cell);                               // the staging memory is reused by the next call
     for (int k = 0; k < na; ++k) {
         if (!arrs[k].back) continue;
-        if (arrs[k].bytes) CK(cudaMemcpyAsync(arrs[k].host, *arrs[k].dev, arrs[k].bytes, cudaMemcpyDeviceToHost, ctx->stream));
+        if (arrs[k].bytes) CK(cudaMemcpyAsync(arrs[k].host, *arrs[k].srt, arrs[k].bytes, cudaMemcpyDeviceToHost, ctx->stream));
         down += (int64_t)arrs[k].bytes;
     }
     for (int c = 0; c < 3; ++c) { CK(cudaMemcpyAsync(J->comp[c], dJ.comp[c], pad * 4, cudaMemcpyDeviceToHost, ctx->stream)); down += (int64_t)pad * 4; }
