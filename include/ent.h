@@ -203,8 +203,12 @@ enum {
     ENT_STAT_SCRATCH_BYTES = 9,
     ENT_STAT_LAST_STEP_TILED = 10,
     ENT_STAT_LAST_SORT_REBIN = 11,  /* 1 if the last ent_sort took the incremental re-bin path */
-    ENT_STAT_SLOT_ERRORS = 12       /* particles ent_step_sorted could not place (layout counts contradicted by the block: the caller
+    ENT_STAT_SLOT_ERRORS = 12,      /* particles ent_step_sorted could not place (layout counts contradicted by the block: the caller
                                        edited the cell arrays of a sorted block without ent_forget / ent_sort); synchronises */
+    ENT_STAT_CARRIES = 13,          /* since ent_create: signed wraps of a fixed-point J-tile accumulator carried into the global array
+                                       (a node received > ~128 coherent contributions of the largest size); synchronises */
+    ENT_STAT_GLOBAL_ADDS = 14       /* since ent_create: contributions of the axisymmetric tiled kernel too large for the tile's
+                                       fixed-point range (J^3 next to the axis), added to the global array directly; synchronises */
 };
 int ent_set_option(ent_ctx *ctx, int key, int64_t value);
 int ent_get_stat(ent_ctx *ctx, int key, int64_t *value);

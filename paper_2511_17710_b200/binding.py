@@ -19,7 +19,7 @@ NGHOST = 2
 OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM = 0, -1, -2, -3, -4
 OPT_STEP_IMPL, OPT_TILE_1, OPT_TILE_2, OPT_TILE_3, OPT_SORT_MODE = 1, 2, 3, 4, 5
 (STAT_TILE_1, STAT_TILE_2, STAT_TILE_3, STAT_NKEYS, STAT_NTILES, STAT_LAUNCHES, STAT_BAD_MOVES, STAT_STRAYS,
- STAT_SCRATCH_BYTES, STAT_LAST_STEP_TILED, STAT_LAST_SORT_REBIN, STAT_SLOT_ERRORS) = range(1, 13)
+ STAT_SCRATCH_BYTES, STAT_LAST_STEP_TILED, STAT_LAST_SORT_REBIN, STAT_SLOT_ERRORS, STAT_CARRIES, STAT_GLOBAL_ADDS) = range(1, 15)
 
 SYMBOLS = ["ent_create", "ent_destroy", "ent_last_error", "ent_set_grid", "ent_gather_push", "ent_deposit", "ent_sort",
            "ent_step", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_step_host", "ent_set_option", "ent_get_stat", "ent_version"]

@@ -29,7 +29,7 @@ struct ent_ctx {
     // ---- scratch pool: ONE device allocation carved by reserve_pool(); hot calls never allocate once it is large enough (ent_reserve)
     void *pool = nullptr; size_t pool_bytes = 0;
     long long pool_n = -1;                    // particle count the pool was carved for (-1: none)
-    unsigned long long *counters = nullptr;   // [0] bad moves, [1] strays, [2] stray-list length, [3] slot errors (own tiny allocation)
+    unsigned long long *counters = nullptr;   // [0] bad moves, [1] strays, [2] stray-list length, [3] slot errors, [4] carries, [5] direct global adds
     int32_t *keys = nullptr, *count = nullptr, *offsets = nullptr, *cursor = nullptr, *chunk = nullptr, *class_count = nullptr;
     // side buffers of the non-hot paths (two-kernel step, host-buffer step): allocated on first use
     void *oldbuf = nullptr; size_t oldbuf_cap = 0;
@@ -143,8 +143,8 @@ extern "C" int ent_create(ent_ctx **out, int device, void *cuda_stream) {
     if (!ctx) return ENT_ENOMEM;
     ctx->device = device;
     ctx->stream = (cudaStream_t)cuda_stream;
-    if (cudaMalloc((void **)&ctx->counters, 4 * sizeof(unsigned long long)) != cudaSuccess ||
-        cudaMemsetAsync(ctx->counters, 0, 4 * sizeof(unsigned long long), ctx->stream) != cudaSuccess) {
+    if (cudaMalloc((void **)&ctx->counters, 8 * sizeof(unsigned long long)) != cudaSuccess ||
+        cudaMemsetAsync(ctx->counters, 0, 8 * sizeof(unsigned long long), ctx->stream) != cudaSuccess) {
         cudaGetLastError(); delete ctx; return ENT_ECUDA;
     }
     *out = ctx;
@@ -622,12 +622,12 @@ extern "C" int ent_get_stat(ent_ctx *ctx, int key, int64_t *value) {
         case ENT_STAT_NTILES:
             if (!ctx->have_grid) return fail(ctx, ENT_EINVAL, "no grid"); *value = (int64_t)g.nt[0] * g.nt[1] * g.nt[2]; return ENT_OK;
         case ENT_STAT_LAUNCHES: *value = ctx->launches; return ENT_OK;
-        case ENT_STAT_BAD_MOVES: case ENT_STAT_STRAYS: case ENT_STAT_SLOT_ERRORS: {
-            unsigned long long h[4];
+        case ENT_STAT_BAD_MOVES: case ENT_STAT_STRAYS: case ENT_STAT_SLOT_ERRORS: case ENT_STAT_CARRIES: case ENT_STAT_GLOBAL_ADDS: {
+            unsigned long long h[8];
             CK(cudaSetDevice(ctx->device));
             CK(cudaMemcpyAsync(h, ctx->counters, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
             CK(cudaStreamSynchronize(ctx->stream));
-            *value = (int64_t)h[key == ENT_STAT_BAD_MOVES ? 0 : (key == ENT_STAT_STRAYS ? 1 : 3)]; return ENT_OK;
+            *value = (int64_t)h[key == ENT_STAT_BAD_MOVES ? 0 : key == ENT_STAT_STRAYS ? 1 : key == ENT_STAT_SLOT_ERRORS ? 3 : key == ENT_STAT_CARRIES ? 4 : 5]; return ENT_OK;
         }
         case ENT_STAT_SCRATCH_BYTES: *value = (int64_t)(ctx->pool_bytes + ctx->side_bytes); return ENT_OK;
         case ENT_STAT_LAST_STEP_TILED: *value = ctx->last_step_tiled; return ENT_OK;

@@ -172,7 +172,7 @@ step_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
         T.Sc = Sc; T.wguard = Sc > 0.f ? 60.0f * wm : -1.0f;
     }
     T.cc.J = A.J.c; T.cc.P0 = g.P[0]; T.cc.P01 = g.P[0] * g.P[1]; T.cc.unit = 4294967296.0f * invSc;
-    T.cc.JX = G::JX; T.cc.JY = G::JY; T.cc.JNP = G::JNP;
+    T.cc.JX = G::JX; T.cc.JY = G::JY; T.cc.JNP = G::JNP; T.cc.carries = A.counters + 4;
     T.cc.gbase = (long long)o[0] + (long long)g.P[0] * o[1] + (D == 3 ? (long long)g.P[0] * g.P[1] * o[2] : 0);
     __syncthreads();                                             // sJ zeroed, mbarrier initialised, dest_s ready
     bool waited = false;

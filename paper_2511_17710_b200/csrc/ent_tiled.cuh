@@ -129,7 +129,7 @@ struct TiledArgs {
     long long n;
     float eps, dt, q, inv_dt;
     float cdt[3];                 // dt / dx_d
-    unsigned long long *counters; // [0] bad moves, [1] strays, [2] length of stray_list
+    unsigned long long *counters; // [0] bad moves, [1] strays, [2] length of stray_list, [4] carries of the fixed-point J tile
     int32_t *stray_list; long long stray_cap;   // particles left to stray_kernel (all lanes busy there instead of one per warp here)
     MagicDiv divN0, divN01;
 };
@@ -171,12 +171,13 @@ __device__ __noinline__ void stray_step(const TiledArgs &A, long long p) {
 // particles' worth of current on one node) is detected from the value the atomic returns and carried straight into
 // the global array as +-2^32 / 2^k, so the sum stays exact for any input.
 // ---------------------------------------------------------------------------------------------------------
-struct CarryCtx { float *const *J; long long gbase; int P0, P01; float unit; int JX, JY, JNP; };
+struct CarryCtx { float *const *J; long long gbase; int P0, P01; float unit; int JX, JY, JNP; unsigned long long *carries; };
 
 __device__ __noinline__ void carry_fix(const CarryCtx &c, int comp, int off, int positive) {
     int bx = off % c.JX, r = off / c.JX, by = r % c.JY, bz = r / c.JY;
     long long idx = c.gbase + bx + (long long)c.P0 * by + (long long)c.P01 * bz;
     red_global_f32(c.J[comp] + idx, positive ? c.unit : -c.unit);
+    atomicAdd(c.carries, 1ULL);
 }
 __device__ __forceinline__ void acc_fixed(int *sJ, const CarryCtx &cc, int comp, int off, float scaled) {
     int v = __float2int_rn(scaled);
@@ -407,7 +408,7 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
         T.Sc = Sc; T.wguard = Sc > 0.f ? 60.0f * wm : -1.0f;
     }
     T.cc.J = A.J.c; T.cc.P0 = g.P[0]; T.cc.P01 = g.P[0] * g.P[1]; T.cc.unit = 4294967296.0f * invSc;
-    T.cc.JX = G::JX; T.cc.JY = G::JY; T.cc.JNP = G::JNP;
+    T.cc.JX = G::JX; T.cc.JY = G::JY; T.cc.JNP = G::JNP; T.cc.carries = A.counters + 4;
     T.cc.gbase = (long long)T.o[0] + (long long)g.P[0] * T.o[1] + (D == 3 ? (long long)g.P[0] * g.P[1] * T.o[2] : 0);
     __syncthreads();                                             // sJ zeroed, mbarrier initialised
     bool waited = false;

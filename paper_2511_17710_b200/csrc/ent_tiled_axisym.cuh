@@ -19,6 +19,7 @@ __device__ __noinline__ void global_add(const CarryCtx &c, int comp, int off, fl
     int bx = off % c.JX, r = off / c.JX, by = r % c.JY, bz = r / c.JY;
     long long idx = c.gbase + bx + (long long)c.P0 * by + (long long)c.P01 * bz;
     red_global_f32(c.J[comp] + idx, v);
+    atomicAdd(c.carries + 1, 1ULL);                          // counters[5]: contributions too large for the tile's fixed-point range
 }
 struct TileAcc {                         // Acc of deposit_particle_at: fixed-point add into the shared J tile
     int *sJ; const CarryCtx *cc; float Sc;
@@ -105,7 +106,7 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
     }
     if (tid == 0) {
         s_cc.J = A.J.c; s_cc.P0 = g.P[0]; s_cc.P01 = g.P[0] * g.P[1]; s_cc.unit = 4294967296.0f * invSc;
-        s_cc.JX = G::JX; s_cc.JY = G::JY; s_cc.JNP = G::JNP;
+        s_cc.JX = G::JX; s_cc.JY = G::JY; s_cc.JNP = G::JNP; s_cc.carries = A.counters + 4;
         s_cc.gbase = (long long)o0 + (long long)g.P[0] * o1;
     }
     __syncthreads();

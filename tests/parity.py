@@ -150,6 +150,38 @@ def deposit_of_gpu_positions(orc, og, p_before, p_after, q, dt, fold=True):
     return J
 
 
+def straddler_correction(orc, grid, og, po_before, po_after, pe_before, pe_after, q, dt, order=None):
+    """The zig-zag path of P:575 is DISCONTINUOUS in the crossing decision: a particle that starts or ends within rounding of a cell
+    face is routed through the face (relay on the face) if it crossed and through the midpoint if it did not, and the two paths
+    put a single-particle-sized amount of current on different nodes (both conserve charge).  fp32 and fp64 take that decision
+    differently for a few particles per million per step (the straddlers of reading G12 / F3).  For exactly those particles --
+    cell index before or after the step differing between the GPU and the oracle while the real positions agree (compare_particles
+    checks that) -- the oracle's current is re-evaluated on the GPU's stored positions; returns (number of such particles,
+    3 padded arrays to ADD to the oracle's folded current, or None).  pe_before / pe_after: orc.Particles built from the GPU arrays
+    (ent_to_orc), in GPU slot order; order[k] = oracle index of GPU slot k."""
+    n = po_before.n
+    sel = np.arange(n) if order is None else np.asarray(order)
+    inv = np.empty(n, dtype=np.int64); inv[sel] = np.arange(n)          # oracle particle j sits in GPU slot inv[j]
+    mism = np.zeros(n, dtype=bool)
+    for a in range(grid.D):
+        mism |= (pe_after.i[a][inv] != po_after.i[a]) | (pe_before.i[a][inv] != po_before.i[a])
+    alive = np.ones(n, dtype=bool)
+    for p, g in ((po_after, False), (po_before, False), (pe_after, True), (pe_before, True)):
+        if p.tag is not None:
+            alive &= (p.tag[inv] if g else p.tag) != 0
+    idx = np.nonzero(mism & alive)[0]
+    if idx.size == 0:
+        return 0, None
+    take = lambda p, ii: orc.Particles(i=[np.ascontiguousarray(a[ii]) for a in p.i], d=[np.ascontiguousarray(a[ii]) for a in p.d],
+                                       u=[np.ascontiguousarray(a[ii]) for a in p.u], w=np.ascontiguousarray(p.w[ii]),
+                                       phi=None if p.phi is None else np.ascontiguousarray(p.phi[ii]), tag=None)
+    Jp, Jm = orc.zeros_current(og), orc.zeros_current(og)
+    orc.deposit(og, take(pe_before, inv[idx]), take(pe_after, inv[idx]), Jp, q, dt)
+    orc.deposit(og, take(po_before, idx), take(po_after, idx), Jm, q, dt)
+    orc.fold_current(og, Jp); orc.fold_current(og, Jm)
+    return int(idx.size), [a - b for a, b in zip(Jp, Jm)]
+
+
 def _box3(a):
     b = np.zeros_like(a)
     for s2 in (-1, 0, 1):

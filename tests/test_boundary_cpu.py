@@ -95,3 +95,28 @@ def test_workload_recipes_have_the_stated_shape():
     assert float(ux[0::2].mean()) > 0.3 and float(ux[1::2].mean()) < -0.3   # two counter-streaming beams
     for f in synth.config5(64).fields:
         assert torch.isfinite(f).all()
+
+
+def _build_abi_check(tmp_path):
+    """tests/c/abi_check.c compiled with gcc against include/ent.h and linked with libent.so: the ABI is usable from plain C"""
+    import subprocess
+    from paper_2511_17710_b200 import build
+    lib = build.build()
+    exe = str(tmp_path / "abi_check")
+    subprocess.check_call(["gcc", "-std=c11", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), os.path.join(ROOT, "tests", "c", "abi_check.c"),
+                           "-o", exe, lib, "-Wl,-rpath," + os.path.dirname(lib)])
+    return exe
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU behaviour")
+def test_c_program_against_the_abi_without_a_device(tmp_path):
+    import subprocess
+    r = subprocess.run([_build_abi_check(tmp_path)], capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0 and "no device" in r.stdout, (r.stdout, r.stderr)
+
+
+@pytest.mark.gpu
+def test_c_program_against_the_abi_on_the_gpu(tmp_path):
+    import subprocess
+    r = subprocess.run([_build_abi_check(tmp_path)], capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0 and "abi ok" in r.stdout, (r.stdout, r.stderr)

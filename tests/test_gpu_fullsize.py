@@ -185,3 +185,22 @@ def test_c5_full_size_last_step(orc):
         assert c <= P.CONT_TOL
     finally:
         bind.ent_destroy(ctx)
+
+
+def test_c2_full_size_every_step(orc):
+    """C2 at BASELINE.json's size (log-spherical 256 x 256, ~1 M particles per species, 20 steps): the oracle follows EVERY particle
+    for all 20 steps; sorted block, tiled axisymmetric kernel, incremental re-sort every 3 steps; every step checks the current (end
+    to end with the format allowance, raw value printed; strict deposit check without allowance) and continuity."""
+    from paper_2511_17710_b200 import binding as bind, synth
+    import test_gpu_parity as T
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    ctx = bind.ent_create(0, None)
+    try:
+        wl = synth.config2(1)
+        assert tuple(wl.grid.N) == (256, 256) and wl.steps == 20
+        stats = T._run_case((bind, synth, ctx, orc), wl, impl=0, sort_first=True, resort_every=3)
+        print("C2 full size:", stats)
+        assert all(st["tiled"] == 1 and st["strays"] == 0 for st in stats.values())
+    finally:
+        bind.ent_destroy(ctx)

@@ -76,6 +76,7 @@ def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True
             pe = ps
         Jg = bind.zeros_current(eg, "cuda")
         worstJ = worstC = rawJ = strictJ = 0.0
+        zz = 0
         for s in range(steps):
             if resort_every and s > 0 and s % resort_every == 0:
                 # incremental ent_sort (re-bin) of the drifted block: tile contiguity only
@@ -94,14 +95,20 @@ def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True
             bind.ent_fold_current(ctx, Jg)
             torch.cuda.synchronize()
             Jo = orc.zeros_current(og)
+            po_before = po.copy()
             orc.step(og, F_orc, po, Jo, sp.q, sp.m, wl.dt)
             orc.fold_current(og, Jo)
+            if check_every_step:
+                after = P.ent_to_orc(orc, g, pe)
+                nz, corr = P.straddler_correction(orc, g, og, po_before, po, before, after, sp.q, wl.dt, order)    # zig-zag relay of face straddlers (G12)
+                zz += nz
+                if corr is not None:
+                    Jo = [a + b for a, b in zip(Jo, corr)]
             if check_every_step or s == steps - 1:
                 bound = P.offset_format_bound(orc, g, og, before, sp.q, wl.dt) if (eg.axisym and before is not None) else None
                 worstJ = max(worstJ, P.compare_current(Jg, Jo, bound))
                 rawJ = max(rawJ, P.compare_current.last_raw)
             if check_every_step:
-                after = P.ent_to_orc(orc, g, pe)
                 # STRICT current check, no allowance: the oracle's deposit of the GPU's own stored move (isolates sub-step 8)
                 strictJ = max(strictJ, P.compare_current(Jg, P.deposit_of_gpu_positions(orc, og, before, after, sp.q, wl.dt)))
                 c = P.continuity_of_gpu_step(orc, og, before, after, Jg, sp.q, wl.dt)
@@ -111,7 +118,7 @@ def _run_case(env, wl, impl, steps=None, sort_first=False, check_every_step=True
         assert bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES) == 0
         stats["tiled"] = bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED)
         stats["strays"] = bind.ent_get_stat(ctx, bind.STAT_STRAYS)
-        stats.update(worstJ=worstJ, rawJ=rawJ, strictJ=strictJ, worstC=worstC)
+        stats.update(worstJ=worstJ, rawJ=rawJ, strictJ=strictJ, worstC=worstC, zigzag_straddlers=zz)
         out[si] = stats
     return out
 
@@ -212,11 +219,15 @@ def test_step_sorted_matches_oracle(env, name):
             assert orc.sort_check(tile_of_slot_b, ntiles, toff) == 0, "output block is not contiguous by the tiles of the input positions"
             # oracle step, same particles in the oracle's own (original) order
             Jo = orc.zeros_current(og)
+            po_before = po.copy()
             orc.step(og, F_orc, po, Jo, sp.q, sp.m, wl.dt)
             orc.fold_current(og, Jo)
-            worstJ = max(worstJ, P.compare_current(Jg, Jo))
             after_slots = P.ent_to_orc(orc, g, b)
             after = _take(orc, after_slots, np.argsort(idb)[ida])                     # the output in the order of `before`
+            nz, corr = P.straddler_correction(orc, g, og, po_before, po, before, after, sp.q, wl.dt, ida)
+            if corr is not None:
+                Jo = [x + y for x, y in zip(Jo, corr)]
+            worstJ = max(worstJ, P.compare_current(Jg, Jo))
             strictJ = max(strictJ, P.compare_current(Jg, P.deposit_of_gpu_positions(orc, og, before, after, sp.q, wl.dt)))
             c = P.continuity_of_gpu_step(orc, og, before, after, Jg, sp.q, wl.dt)
             assert c <= P.CONT_TOL, f"continuity residual {c:.3e} at step {s}"
