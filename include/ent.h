@@ -191,6 +191,10 @@ enum {
     ENT_OPT_STEP_IMPL = 1,     /* 0 = auto (tiled when the block is the sorted one), 1 = force untiled, 2 = two-kernel
                                   (gather_push to scratch copy + deposit; the paper's structure) */
     ENT_OPT_TILE_1 = 2, ENT_OPT_TILE_2 = 3, ENT_OPT_TILE_3 = 4,   /* tile extents in cells; takes effect at the next ent_set_grid */
+    ENT_OPT_CURV_FP64 = 6,     /* SPH / QSPH grids: 0 (default) = the move is evaluated in fp32 as a DISPLACEMENT in the local frame at the
+                                  particle (increments of the code coordinates added to the in-cell offsets; same mathematics as
+                                  P:147-153 + P:285-327); 1 = fp64 coordinate maps through the global Cartesian frame (the literal
+                                  round trip; slower, kept for comparison).  Takes effect at once. */
     ENT_OPT_SORT_MODE = 5      /* 0 = auto (incremental re-bin when `in` is itself a block ent_sort produced and key_offsets is NULL),
                                   1 = always the full cell-level counting sort,
                                   2 = like 0, but the re-bin does not order the particles that stay in a tile by cell */

@@ -27,6 +27,9 @@ struct GridDev {
     // QSPH: r = r0 + exp(Rmin + x1*dR), theta = theta(T), T = x2*dT
     double rmin, dr, dth;
     double Rmin, dR, dT, r0, vt;
+    // fp32 copies for the displacement form of the curvilinear move (ent_particle.cuh) and its switch
+    float rminf, drf, dthf, Rminf, dRf, dTf, r0f, vtf;
+    int curv_f64;      // 1: coordinate maps of the axisymmetric grids in fp64 through the global Cartesian frame (round-1 form)
 };
 
 __host__ __device__ inline long long padded_size(const GridDev &g) { return (long long)g.P[0] * g.P[1] * g.P[2]; }
@@ -130,6 +133,81 @@ __device__ __forceinline__ double T_of_theta(double vt, double th, double T0) {
         if (fabs(f) < 1e-15) break;
     }
     return T;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// fp32 description of a code position on the axisymmetric grids, for the DISPLACEMENT form of the move.
+// The transcendental part of the metric lives at the grid NODES: exp(R_i) (or r_i) per x1 node, sin/cos(theta_j), d theta/dT and
+// half the second derivative of theta(T) per x2 node, evaluated in fp64 and rounded once ("metric factors", BASELINE.json
+// north_star (b)).  The tiled kernel stages them per tile in shared memory (TileGeo, ent_tiled_axisym.cuh); the untiled kernels
+// evaluate them per particle (GlobalGeo) -- the same function, hence the same values.  At the particle only short polynomials in
+// the in-cell offset remain: exp(x), x < dR, and sin/cos of the angle to the NEARER node, so sin(theta) keeps its relative
+// accuracy next to either pole and (i + d) is never formed (the offset would lose its low bits).
+// ---------------------------------------------------------------------------------------------------------
+struct NodeY { float st, ct, th1, c2; };   // sin, cos of theta_j; d theta / dT and (d2 theta / dT2) / 2 at T_j (SPH: 1, 0)
+template <int KIND>
+__device__ __forceinline__ float node_x(const GridDev &g, int i) {            // P:243 / P:261: r_i (SPH) or exp(R_i) (QSPH)
+    return KIND == ENT_SPH ? (float)(g.rmin + (double)i * g.dr) : (float)exp(g.Rmin + (double)i * g.dR);
+}
+template <int KIND>
+__device__ __forceinline__ NodeY node_y(const GridDev &g, int j) {            // P:243 / P:265-267
+    NodeY y;
+    double th, s_, c_;
+    if (KIND == ENT_SPH) { th = (double)j * g.dth; y.th1 = 1.f; y.c2 = 0.f; }
+    else {
+        const double T = (double)j * g.dT, s = T / PI_D;
+        th = T + 2.0 * g.vt * T * (1.0 - 2.0 * s) * (1.0 - s);
+        y.th1 = (float)(1.0 + 2.0 * g.vt + 12.0 * g.vt * s * (s - 1.0));
+        y.c2 = (float)(6.0 * g.vt * (2.0 * s - 1.0) / PI_D);
+    }
+    sincos(th, &s_, &c_);
+    y.st = (float)s_; y.ct = (float)c_;
+    return y;
+}
+template <int KIND>
+struct GlobalGeo {                       // node factors evaluated on the spot (untiled kernels, stray path)
+    const GridDev &g;
+    __device__ __forceinline__ float x(int i) const { return node_x<KIND>(g, i); }
+    __device__ __forceinline__ NodeY y(int j) const { return node_y<KIND>(g, j); }
+};
+
+struct SphF {
+    float r, rr0;           // r and r - r0
+    float st, ct;           // sin(theta), cos(theta)
+    float sh1, sh2, sh3;    // sqrt(h11), sqrt(h22), sqrt(h33)
+    float th1, c2;          // QSPH: d theta / dT and (d2 theta / dT2) / 2 at the particle
+};
+// d1, d2 may lie a little outside [0, 1) (midpoint of a move)
+template <int KIND, class GEO>
+__device__ __forceinline__ SphF sphf_of_code(const GridDev &g, const GEO &geo, int i1, float d1, int i2, float d2) {
+    SphF s;
+    const int rnd = (int)floorf(d2 + 0.5f);                    // nearer x2 node
+    const NodeY y = geo.y(i2 + rnd);
+    float eps;                                                 // theta - theta_node
+    if (KIND == ENT_SPH) {
+        s.r = fmaf(d1, g.drf, geo.x(i1));
+        s.rr0 = s.r;
+        eps = (d2 - (float)rnd) * g.dthf;
+        s.th1 = 1.f; s.c2 = 0.f;
+        s.sh1 = g.drf; s.sh2 = s.r * g.dthf;
+    } else {
+        const float x = d1 * g.dRf;                            // exp(R_i + x) = exp(R_i) (1 + x + x^2/2 + x^3/6 + x^4/24), x < 2 dR
+        const float eR = geo.x(i1) * fmaf(x, fmaf(x, fmaf(x, fmaf(x, 1.0f / 24.0f, 1.0f / 6.0f), 0.5f), 1.0f), 1.0f);
+        s.r = g.r0f + eR; s.rr0 = eR;
+        const float eT = (d2 - (float)rnd) * g.dTf;
+        const float c3 = 4.0f * g.vtf * 0.101321183642337771f;                 // third derivative / 6 = 4 vt / pi^2: theta(T) is a cubic
+        eps = ((c3 * eT + y.c2) * eT + y.th1) * eT;
+        s.th1 = (3.0f * c3 * eT + 2.0f * y.c2) * eT + y.th1;
+        s.c2 = y.c2 + 3.0f * c3 * eT;
+        s.sh1 = g.dRf * eR; s.sh2 = g.dTf * s.th1 * s.r;
+    }
+    const float e2 = eps * eps;                                // |eps| <= half a cell
+    const float se = eps * fmaf(e2, fmaf(e2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
+    const float ce = fmaf(e2, fmaf(e2, fmaf(e2, -1.0f / 720.0f, 1.0f / 24.0f), -0.5f), 1.0f);
+    s.st = y.st * ce + y.ct * se;
+    s.ct = y.ct * ce - y.st * se;
+    s.sh3 = s.r * s.st;
+    return s;
 }
 
 struct Sph {            // spherical-polar description of a code position + sqrt(h_ii) there

@@ -10,9 +10,10 @@ namespace ent {
 // eps = (q/m) dt / 2.
 // ---------------------------------------------------------------------------------------------------------
 // push_from_fields: everything after the gather (EB = the six interpolated contravariant components).
-template <int D, int KIND>
-__device__ __forceinline__ void push_from_fields(const GridDev &g, const float EB[6], int i[3], float d[3], float &phi,
-                                                 float u[3], float eps, float dt, int di[3], bool &alive) {
+struct NoGeo {};                          // Cartesian grids need no node factors
+template <int D, int KIND, class GEO>
+__device__ __forceinline__ void push_from_fields_geo(const GridDev &g, const GEO &geo, const float EB[6], int i[3], float d[3], float &phi,
+                                                     float u[3], float eps, float dt, int di[3], bool &alive) {
     float E[3], B[3];
     if (KIND == ENT_CART) {
         // step 4: A^hat = sqrt(h_ii) A^i; Cartesian code basis is already aligned with x,y,z
@@ -27,8 +28,68 @@ __device__ __forceinline__ void push_from_fields(const GridDev &g, const float E
                 split_offset(x, di[a], d[a]);
             } else di[a] = 0;
         }
+    } else if (!g.curv_f64) {
+        // axisymmetric, fp32 DISPLACEMENT form: the step v dt is projected on the local frame
+        // (r, theta, phi)-hat at the old point and turned into increments of the code coordinates, which are added to the in-cell
+        // offsets exactly as on the Cartesian grids; no absolute position is ever formed in fp32.  Same mathematics as the
+        // global-Cartesian round trip of P:147-153, P:285-327 (the oracle's), which in fp32 would lose the displacement.
+        SphF s;
+        if constexpr (KIND != ENT_CART) s = sphf_of_code<KIND>(g, geo, i[0], d[0], i[1], d[1]);
+        float sp, cp;
+        sincosf(phi, &sp, &cp);
+        {   // step 4: tetrad (at the particle, G2) then rotation (r,th,phi)-hat -> (x,y,z)-hat
+            float Ar = s.sh1 * EB[0], At = s.sh2 * EB[1], Ap = s.sh3 * EB[2];
+            E[0] = Ar * s.st * cp + At * s.ct * cp - Ap * sp;
+            E[1] = Ar * s.st * sp + At * s.ct * sp + Ap * cp;
+            E[2] = Ar * s.ct - At * s.st;
+            Ar = s.sh1 * EB[3]; At = s.sh2 * EB[4]; Ap = s.sh3 * EB[5];
+            B[0] = Ar * s.st * cp + At * s.ct * cp - Ap * sp;
+            B[1] = Ar * s.st * sp + At * s.ct * sp + Ap * cp;
+            B[2] = Ar * s.ct - At * s.st;
+        }
+        boris(u, E, B, eps);
+        const float ig = inv_gamma(u);
+        const float Dx = (u[0] * ig) * dt, Dy = (u[1] * ig) * dt, Dz = (u[2] * ig) * dt;
+        const float Dh = Dx * cp + Dy * sp;                                   // component along the old cylindrical radius
+        const float dr_ = Dh * s.st + Dz * s.ct, dth_ = Dh * s.ct - Dz * s.st, dph_ = Dy * cp - Dx * sp;
+        const float rp = s.r + dr_;
+        const float d2 = dr_ * dr_ + dth_ * dth_ + dph_ * dph_;
+        const float rn = sqrtf(rp * rp + dth_ * dth_ + dph_ * dph_);
+        const float Dr = (2.0f * s.r * dr_ + d2) / (rn + s.r);                 // r' - r without cancellation
+        const float a = rp * s.st + dth_ * s.ct;                               // new cylindrical radius vector in the old meridional plane
+        const float rho = sqrtf(a * a + dph_ * dph_);
+        const float zn = rp * s.ct - dth_ * s.st;
+        const float rma = a > 0.f ? (dph_ * dph_) / (rho + a) : rho - a;       // rho' - a
+        const float Dth = atan2f(dth_ + rma * s.ct, zn * s.ct + rho * s.st);   // theta' - theta
+        const float Dph = atan2f(dph_, a);
+        float x1n, x2n;
+        if (KIND == ENT_SPH) { x1n = Dr / g.drf; x2n = Dth / g.dthf; }
+        else {
+            x1n = log1pf(Dr / s.rr0) / g.dRf;
+            float DT = Dth;
+            if (g.vtf != 0.f) {                                               // theta(T + DT) - theta(T) = Dth: theta is a cubic, so its
+                const float c3 = 4.0f * g.vtf * 0.101321183642337771f;        // Taylor series ends: th1 DT + c2 DT^2 + c3 DT^3, c3 = 4 vt / pi^2
+                DT = Dth / s.th1;
+#pragma unroll
+                for (int it = 0; it < 2; ++it) {                              // two Newton steps from the linear guess (no cube root, cf. App. B)
+                    const float f = ((c3 * DT + s.c2) * DT + s.th1) * DT - Dth;
+                    const float fp = (3.0f * c3 * DT + 2.0f * s.c2) * DT + s.th1;
+                    DT -= f / fp;
+                }
+            }
+            x2n = DT / g.dTf;
+        }
+        split_offset(d[0] + x1n, di[0], d[0]);
+        split_offset(d[1] + x2n, di[1], d[1]);
+        di[2] = 0;
+        float phn = phi + Dph;
+        if (phn >= TWO_PI_F) phn -= TWO_PI_F;
+        if (phn < 0.f) phn += TWO_PI_F;
+        if (phn >= TWO_PI_F) phn = 0.f;
+        phi = phn;
     } else {
-        // axisymmetric: particle at (x1, x2, phi); fp64 geometry
+        // axisymmetric, fp64 maps through the global Cartesian frame (ENT_OPT_CURV_FP64 = 1; the round-1 form, kept for A/B)
+        // particle at (x1, x2, phi)
         double x1 = (double)i[0] + (double)d[0], x2 = (double)i[1] + (double)d[1], ph = (double)phi;
         Sph s = sph_of_code<KIND>(g, x1, x2);
         double st, ct, sp, cp;
@@ -91,6 +152,13 @@ __device__ __forceinline__ void push_from_fields(const GridDev &g, const float E
     }
 }
 
+template <int D, int KIND>
+__device__ __forceinline__ void push_from_fields(const GridDev &g, const float EB[6], int i[3], float d[3], float &phi,
+                                                 float u[3], float eps, float dt, int di[3], bool &alive) {
+    if constexpr (KIND == ENT_CART) push_from_fields_geo<D, KIND>(g, NoGeo{}, EB, i, d, phi, u, eps, dt, di, alive);
+    else push_from_fields_geo<D, KIND>(g, GlobalGeo<KIND>{g}, EB, i, d, phi, u, eps, dt, di, alive);
+}
+
 template <int D, int KIND, class Loader>
 __device__ __forceinline__ void push_particle(const GridDev &g, const Loader &ld, int i[3], float d[3], float &phi,
                                               float u[3], float eps, float dt, int di[3], bool &alive) {
@@ -150,11 +218,22 @@ __device__ __forceinline__ void deposit_segment(const Acc &acc, long long base, 
 }
 
 // out-of-plane rate q w v^3_code / 2 per segment for the 2D grids (G8); u = momentum at n+1/2
-template <int KIND>
-__device__ __forceinline__ float half_qw_v3(const GridDev &g, const int i0[3], const float a[3], const float b[3],
+template <int KIND, class GEO>
+__device__ __forceinline__ float half_qw_v3(const GridDev &g, const GEO &geo, const int i0[3], const float a[3], const float b[3],
                                             float phi0, float phi1, const float u[3], float qw) {
     float ig = inv_gamma(u);
     if (KIND == ENT_CART) return 0.5f * qw * (u[2] * ig);                     // h33 = 1
+    if (!g.curv_f64) {
+        float dphi = phi1 - phi0;                                             // shorter arc
+        if (dphi > 3.14159265358979f) dphi -= TWO_PI_F;
+        if (dphi <= -3.14159265358979f) dphi += TWO_PI_F;
+        SphF s;
+        if constexpr (KIND != ENT_CART) s = sphf_of_code<KIND>(g, geo, i0[0], 0.5f * (a[0] + b[0]), i0[1], 0.5f * (a[1] + b[1]));
+        if (s.sh3 < 1e-12f) return 0.f;
+        float sp, cp;
+        sincosf(phi0 + 0.5f * dphi, &sp, &cp);
+        return 0.5f * qw * (((u[1] * cp - u[0] * sp) * ig) / s.sh3);
+    }
     double dphi = (double)phi1 - (double)phi0;
     dphi -= 2.0 * PI_D * floor((dphi + PI_D) / (2.0 * PI_D));                 // shorter arc
     double phm = (double)phi0 + 0.5 * dphi;
@@ -170,8 +249,8 @@ __device__ __forceinline__ float half_qw_v3(const GridDev &g, const int i0[3], c
 
 // gi / ii: the array the contributions are indexed in and the old cell's index in it (the padded global arrays and i0
 // itself for the global path; a shared-memory J tile and the cell's box coordinates for the tiled path).
-template <int D, int KIND, class Acc>
-__device__ __forceinline__ void deposit_particle_at(const GridDev &g, const Acc &acc, const int i0[3], const float a[3],
+template <int D, int KIND, class Acc, class GEO>
+__device__ __forceinline__ void deposit_particle_at(const GridDev &g, const GEO &geo, const Acc &acc, const int i0[3], const float a[3],
                                                     const int di[3], const float dn[3], float phi0, float phi1,
                                                     const float u[3], float qw, float inv_dt, const GridDev &gi, const int ii[3]) {
     float D1[3], W1[3], D2[3], W2[3], b[3];
@@ -189,7 +268,7 @@ __device__ __forceinline__ void deposit_particle_at(const GridDev &g, const Acc 
     long long base2 = base1 + di[0] + s1 * di[1] + (D == 3 ? s2 * di[2] : 0);   // un-wrapped: may point into the ghosts
     float Q = qw * inv_dt;
     float hv = 0.f;
-    if (D == 2) hv = half_qw_v3<KIND>(g, i0, a, b, phi0, phi1, u, qw);
+    if (D == 2) hv = half_qw_v3<KIND>(g, geo, i0, a, b, phi0, phi1, u, qw);
     deposit_segment<D>(acc, base1, s1, s2, D1, W1, Q, hv);
     deposit_segment<D>(acc, base2, s1, s2, D2, W2, Q, hv);
 }
@@ -198,7 +277,8 @@ template <int D, int KIND, class Acc>
 __device__ __forceinline__ void deposit_particle(const GridDev &g, const Acc &acc, const int i0[3], const float a[3],
                                                  const int di[3], const float dn[3], float phi0, float phi1,
                                                  const float u[3], float qw, float inv_dt) {
-    deposit_particle_at<D, KIND>(g, acc, i0, a, di, dn, phi0, phi1, u, qw, inv_dt, g, i0);
+    if constexpr (KIND == ENT_CART) deposit_particle_at<D, KIND>(g, NoGeo{}, acc, i0, a, di, dn, phi0, phi1, u, qw, inv_dt, g, i0);
+    else deposit_particle_at<D, KIND>(g, GlobalGeo<KIND>{g}, acc, i0, a, di, dn, phi0, phi1, u, qw, inv_dt, g, i0);
 }
 
 }  // namespace ent

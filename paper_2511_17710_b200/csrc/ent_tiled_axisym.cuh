@@ -21,6 +21,13 @@ __device__ __noinline__ void global_add(const CarryCtx &c, int comp, int off, fl
     red_global_f32(c.J[comp] + idx, v);
     atomicAdd(c.carries + 1, 1ULL);                          // counters[5]: contributions too large for the tile's fixed-point range
 }
+// node factors of the metric staged per tile in shared memory (ent_dev.cuh sphf_of_code): x1 nodes o1 - 1 .. o1 + TX + 2,
+// x2 nodes o2 - 1 .. o2 + TY + 2
+struct TileGeo {
+    const float *gx; const NodeY *gy; int o1, o2;
+    __device__ __forceinline__ float x(int i) const { return gx[i - o1 + 1]; }
+    __device__ __forceinline__ NodeY y(int j) const { return gy[j - o2 + 1]; }
+};
 struct TileAcc {                         // Acc of deposit_particle_at: fixed-point add into the shared J tile
     int *sJ; const CarryCtx *cc; float Sc;
     __device__ __forceinline__ void add(int comp, long long idx, float v) const {
@@ -67,11 +74,15 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
     int *sJ = reinterpret_cast<int *>(smem + 6 * G::FNP);
     __shared__ uint64_t bar;
     __shared__ CarryCtx s_cc;
+    __shared__ float s_gx[TX + 4];
+    __shared__ NodeY s_gy[TY + 4];
     const GridDev &g = A.g;
     const int tid = threadIdx.x;
     const int tile = find_tile(A.chunk_off, A.ntiles, blockIdx.x);
     if (tile < 0) return;
     const int o0 = (tile % g.nt[0]) * TX, o1 = (tile / g.nt[0]) * TY;
+    if (tid < TX + 4) s_gx[tid] = node_x<KIND>(g, o0 - 1 + tid);                 // metric factors at the nodes of this tile, fp64 -> fp32
+    else if (tid >= 32 && tid < 32 + TY + 4) s_gy[tid - 32] = node_y<KIND>(g, o1 - 1 + tid - 32);
 
     if (tid == 0) {
         mbar_init(&bar, 1);
@@ -112,6 +123,7 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
     __syncthreads();
     const TileAcc acc{sJ, &s_cc, Sc};
     const BoxLoader ld{sF, G::FNP};
+    const TileGeo geo{s_gx, s_gy, o0, o1};
     const float wguard = Sc > 0.f ? 60.0f * A.tile_wmax[tile] : -1.0f;
     bool waited = false;
 
@@ -139,7 +151,7 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
         const float a[3] = { d[0], d[1], 0.f };
         const float phi0 = phi;
         int di[3]; bool alive = true;
-        push_from_fields<2, KIND>(g, EB, i, d, phi, u, A.eps, A.dt, di, alive);
+        push_from_fields_geo<2, KIND>(g, geo, EB, i, d, phi, u, A.eps, A.dt, di, alive);
         A.P.cell[p] = i[0] + g.N[0] * i[1];
         A.P.d[0][p] = d[0]; A.P.d[1][p] = d[1];
         A.P.u[0][p] = u[0]; A.P.u[1][p] = u[1]; A.P.u[2][p] = u[2];
@@ -147,7 +159,7 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
         if (!alive) { A.P.tag[p] = 0; continue; }
         if (di[0] < -1 || di[0] > 1 || di[1] < -1 || di[1] > 1) { atomicAdd(A.counters + 0, 1ULL); continue; }
         GridDev gj = g; gj.P[0] = G::JX; gj.P[1] = G::JY; gj.P[2] = 1;
-        deposit_particle_at<2, KIND>(g, acc, i0, a, di, d, phi0, phi, u, A.q * wgt, A.inv_dt, gj, ib);
+        deposit_particle_at<2, KIND>(g, geo, acc, i0, a, di, d, phi0, phi, u, A.q * wgt, A.inv_dt, gj, ib);
     }
     if (!waited) mbar_wait(&bar, 0);
     __syncthreads();
