@@ -11,6 +11,20 @@ namespace ent {
 // ---------------------------------------------------------------------------------------------------------
 // push_from_fields: everything after the gather (EB = the six interpolated contravariant components).
 struct NoGeo {};                          // Cartesian grids need no node factors
+
+// atan2(y, x) and log1p(x) with a short series where the argument is small (the displacement of one step is a small fraction
+// of r), the library routine otherwise; truncation error below 2e-12
+__device__ __forceinline__ float atan2_step(float y, float x) {
+    if (x > 0.f && fabsf(y) < 0.0625f * x) {
+        const float t = __fdividef(y, x), t2 = t * t;
+        return t * fmaf(t2, fmaf(t2, fmaf(t2, -1.0f / 7.0f, 0.2f), -1.0f / 3.0f), 1.0f);
+    }
+    return atan2f(y, x);
+}
+__device__ __forceinline__ float log1p_step(float x) {
+    if (fabsf(x) < 0.015f) return x * fmaf(x, fmaf(x, fmaf(x, fmaf(x, 0.2f, -0.25f), 1.0f / 3.0f), -0.5f), 1.0f);
+    return log1pf(x);
+}
 template <int D, int KIND, class GEO>
 __device__ __forceinline__ void push_from_fields_geo(const GridDev &g, const GEO &geo, const float EB[6], int i[3], float d[3], float &phi,
                                                      float u[3], float eps, float dt, int di[3], bool &alive) {
@@ -60,12 +74,12 @@ __device__ __forceinline__ void push_from_fields_geo(const GridDev &g, const GEO
         const float rho = sqrtf(a * a + dph_ * dph_);
         const float zn = rp * s.ct - dth_ * s.st;
         const float rma = a > 0.f ? (dph_ * dph_) / (rho + a) : rho - a;       // rho' - a
-        const float Dth = atan2f(dth_ + rma * s.ct, zn * s.ct + rho * s.st);   // theta' - theta
-        const float Dph = atan2f(dph_, a);
+        const float Dth = atan2_step(dth_ + rma * s.ct, zn * s.ct + rho * s.st);   // theta' - theta
+        const float Dph = atan2_step(dph_, a);
         float x1n, x2n;
         if (KIND == ENT_SPH) { x1n = Dr / g.drf; x2n = Dth / g.dthf; }
         else {
-            x1n = log1pf(Dr / s.rr0) / g.dRf;
+            x1n = log1p_step(Dr / s.rr0) / g.dRf;
             float DT = Dth;
             if (g.vtf != 0.f) {                                               // theta(T + DT) - theta(T) = Dth: theta is a cubic, so its
                 const float c3 = 4.0f * g.vtf * 0.101321183642337771f;        // Taylor series ends: th1 DT + c2 DT^2 + c3 DT^3, c3 = 4 vt / pi^2

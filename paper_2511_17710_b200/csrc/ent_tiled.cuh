@@ -182,8 +182,10 @@ __device__ __noinline__ void carry_fix(const CarryCtx &c, int comp, int off, int
 __device__ __forceinline__ void acc_fixed(int *sJ, const CarryCtx &cc, int comp, int off, float scaled) {
     int v = __float2int_rn(scaled);
     int old = atomicAdd(sJ + comp * cc.JNP + off, v);
-    int nw = old + v;
-    if (((old ^ nw) & (v ^ nw)) < 0) carry_fix(cc, comp, off, v > 0);
+    if ((old + 0x40000000) < 0) {             // |old| >= 2^30: only then can |v| < 2^27 wrap the accumulator (conservative, cheap)
+        int nw = old + v;
+        if (((old ^ nw) & (v ^ nw)) < 0) carry_fix(cc, comp, off, v > 0);
+    }
 }
 // four contributions of one component: all four atomics are issued before the first returned value is looked at.  One cheap,
 // conservative test covers the four carries: a contribution is below 2^25 in magnitude, so an accumulator can only wrap if its
@@ -547,6 +549,7 @@ inline int tiled_encode(TiledState &t, const GridDev &g, const FieldPtrs &F, con
 
 template <int KIND, int TX, int TY>
 __global__ void step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ TiledArgs A);   // ent_tiled_axisym.cuh
+template <int TX, int TY> struct AxiGeom;
 
 template <int D> inline void launch_strays(const TiledArgs &A, cudaStream_t stream);      // after the axisymmetric kernels are known
 
@@ -559,18 +562,20 @@ inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, 
     for (int a = 0; a < D; ++a) allper &= A.g.bc[a] == ENT_PERIODIC;
     void (*kern)(const TileMaps, const TiledArgs) = allper ? step_tiled_kernel<D, TX, TY, TZ, true> : step_tiled_kernel<D, TX, TY, TZ, false>;
     int slot = 2 * IDX + (allper ? 1 : 0);
+    int smem_bytes = G::SMEM_BYTES;
     if constexpr (D == 2) {
         if (A.g.kind == ENT_SPH) { kern = step_tiled_axisym_kernel<ENT_SPH, TX, TY>; slot = 6; }
         else if (A.g.kind == ENT_QSPH) { kern = step_tiled_axisym_kernel<ENT_QSPH, TX, TY>; slot = 7; }
+        if (A.g.kind != ENT_CART) smem_bytes = AxiGeom<TX, TY>::SMEM_BYTES;
     } else if (A.g.kind != ENT_CART) { snprintf(err, errn, "no 3D tiled kernel for this metric"); return ENT_EUNSUPPORTED; }
     if (!t.attr_set[slot]) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM_BYTES);
-        if (e != cudaSuccess) { snprintf(err, errn, "cudaFuncSetAttribute(smem %d) failed: %s", G::SMEM_BYTES, cudaGetErrorString(e)); return ENT_ECUDA; }
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+        if (e != cudaSuccess) { snprintf(err, errn, "cudaFuncSetAttribute(smem %d) failed: %s", smem_bytes, cudaGetErrorString(e)); return ENT_ECUDA; }
         t.attr_set[slot] = true;
     }
     const int ntiles = A.g.nt[0] * A.g.nt[1] * A.g.nt[2];
     const long long grid = (long long)ntiles + A.n / TILE_CHUNK + 1;        // upper bound of the number of chunks
-    kern<<<(unsigned)grid, TILED_TPB, G::SMEM_BYTES, stream>>>(t.maps, A);
+    kern<<<(unsigned)grid, TILED_TPB, smem_bytes, stream>>>(t.maps, A);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { snprintf(err, errn, "launch of step_tiled_kernel failed: %s", cudaGetErrorString(e)); return ENT_ECUDA; }
     launch_strays<D>(A, stream);

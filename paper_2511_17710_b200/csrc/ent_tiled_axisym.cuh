@@ -65,13 +65,32 @@ __device__ __noinline__ void stray_step_axisym(const TiledArgs &A, long long p) 
 #ifndef ENT_AXISYM_MINB
 #define ENT_AXISYM_MINB 4
 #endif
+// On these grids the inner cells hold hundreds of particles (density ~ r^-2), so the 32 lanes of a warp usually sit in ONE cell and
+// every shared atomic serialises 32 ways on one address (measured on C5: 16 wavefronts per ATOMS, 84 % of all shared-memory
+// wavefronts).  The J tile is therefore kept in AXI_NCOPY copies, lane L adding into copy L mod AXI_NCOPY; the copies are one word
+// apart modulo the 32 banks, so the same node in different copies sits in different banks: a one-cell warp costs
+// 32 / AXI_NCOPY wavefronts per ATOMS.  The copies are summed in the flush pass.  Measured on C5 (ms per species; copies x CTAs/SM):
+// 1x4 6.30, 2x4 6.21, 4x4 6.07, 4x3 6.65, 8x3 6.84 -- shared-memory wavefronts fall 1295 M -> 553 M with 8 copies, but the kernel is
+// then bound by instruction issue, so the fourth resident CTA is worth more than the last copies.  (Grouping equal-cell lanes with
+// __match_any_sync + __reduce_add_sync was measured 1.6 x SLOWER than no grouping at all: the per-group masks serialise.)
+#ifndef ENT_AXI_NCOPY
+#define ENT_AXI_NCOPY 4
+#endif
+constexpr int AXI_NCOPY = ENT_AXI_NCOPY;
+template <int TX, int TY> struct AxiGeom {
+    using G = TileGeom<2, TX, TY, 1>;
+    static constexpr int CSTRIDE = 3 * G::JNP + 1;                        // words between copies: 1 modulo 32
+    static constexpr int JWORDS = ((AXI_NCOPY * CSTRIDE + 3) / 4) * 4;
+    static constexpr int SMEM_BYTES = (6 * G::FNP + JWORDS) * 4;
+};
 template <int KIND, int TX, int TY>
 __global__ void __launch_bounds__(TILED_TPB, ENT_AXISYM_MINB)
 step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ TiledArgs A) {
     using G = TileGeom<2, TX, TY, 1>;
+    using X = AxiGeom<TX, TY>;
     extern __shared__ __align__(128) float smem[];
     float *sF = smem;
-    int *sJ = reinterpret_cast<int *>(smem + 6 * G::FNP);
+    int *sJ = reinterpret_cast<int *>(smem + 6 * G::FNP);          // AXI_NCOPY copies of [3][JNP], X::CSTRIDE words apart
     __shared__ uint64_t bar;
     __shared__ CarryCtx s_cc;
     __shared__ float s_gx[TX + 4];
@@ -91,7 +110,7 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
 #pragma unroll
         for (int c = 0; c < 6; ++c) tma_load_box<2>(sF + c * G::FNP, &maps.F[c], &bar, o0, o1, 0);
     }
-    for (int k = tid; k < 3 * G::JNP / 4; k += TILED_TPB) reinterpret_cast<int4 *>(sJ)[k] = make_int4(0, 0, 0, 0);
+    for (int k = tid; k < X::JWORDS / 4; k += TILED_TPB) reinterpret_cast<int4 *>(sJ)[k] = make_int4(0, 0, 0, 0);
 
     long long p0 = A.key_off[tile], p1 = A.key_off[tile + 1];
     p0 += (long long)(blockIdx.x - A.chunk_off[tile]) * TILE_CHUNK;
@@ -121,7 +140,7 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
         s_cc.gbase = (long long)o0 + (long long)g.P[0] * o1;
     }
     __syncthreads();
-    const TileAcc acc{sJ, &s_cc, Sc};
+    const TileAcc acc{sJ + (tid & (AXI_NCOPY - 1)) * X::CSTRIDE, &s_cc, Sc};
     const BoxLoader ld{sF, G::FNP};
     const TileGeo geo{s_gx, s_gy, o0, o1};
     const float wguard = Sc > 0.f ? 60.0f * A.tile_wmax[tile] : -1.0f;
@@ -163,9 +182,11 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
     }
     if (!waited) mbar_wait(&bar, 0);
     __syncthreads();
-    for (int k = tid; k < 3 * G::JNP / 4; k += TILED_TPB) {
-        int4 v = reinterpret_cast<int4 *>(sJ)[k];
-        reinterpret_cast<float4 *>(sJ)[k] = make_float4((float)v.x * invSc, (float)v.y * invSc, (float)v.z * invSc, (float)v.w * invSc);
+    for (int k = tid; k < 3 * G::JNP; k += TILED_TPB) {            // sum of the copies, fixed point -> fp32, into copy 0 (dense: the TMA box)
+        long long v = sJ[k];                                       // each copy may hold up to +-2^31: the sum needs more than 32 bits
+#pragma unroll
+        for (int c = 1; c < AXI_NCOPY; ++c) v += sJ[k + c * X::CSTRIDE];
+        reinterpret_cast<float *>(sJ)[k] = (float)v * invSc;
     }
     fence_proxy_async_smem();
     __syncthreads();
