@@ -182,7 +182,8 @@ __device__ __noinline__ void carry_fix(const CarryCtx &c, int comp, int off, int
 __device__ __forceinline__ void acc_fixed(int *sJ, const CarryCtx &cc, int comp, int off, float scaled) {
     int v = __float2int_rn(scaled);
     int old = atomicAdd(sJ + comp * cc.JNP + off, v);
-    if ((old + 0x40000000) < 0) {             // |old| >= 2^30: only then can |v| < 2^27 wrap the accumulator (conservative, cheap)
+    if ((int)((unsigned)old + 0x40000000u) < 0) {     // |old| >= 2^30: only then can |v| < 2^30 wrap the accumulator (conservative, cheap;
+                                                      // unsigned: a signed overflow here would be undefined and was optimised away)
         int nw = old + v;
         if (((old ^ nw) & (v ^ nw)) < 0) carry_fix(cc, comp, off, v > 0);
     }
@@ -195,7 +196,7 @@ __device__ __forceinline__ void acc_fixed4(int *sJ, const CarryCtx &cc, int comp
     int *Jc = sJ + comp * cc.JNP;
     int v0 = __float2int_rn(s0), v1 = __float2int_rn(s1), v2 = __float2int_rn(s2), v3 = __float2int_rn(s3);
     int a0 = atomicAdd(Jc + o0, v0), a1 = atomicAdd(Jc + o1, v1), a2 = atomicAdd(Jc + o2, v2), a3 = atomicAdd(Jc + o3, v3);
-    if ((((a0 + 0x40000000) | (a1 + 0x40000000)) | ((a2 + 0x40000000) | (a3 + 0x40000000))) < 0) {
+    if ((int)((((unsigned)a0 + 0x40000000u) | ((unsigned)a1 + 0x40000000u)) | (((unsigned)a2 + 0x40000000u) | ((unsigned)a3 + 0x40000000u))) < 0) {
         int n0 = a0 + v0, n1 = a1 + v1, n2 = a2 + v2, n3 = a3 + v3;
         if (((a0 ^ n0) & (v0 ^ n0)) < 0) carry_fix(cc, comp, o0, v0 > 0);
         if (((a1 ^ n1) & (v1 ^ n1)) < 0) carry_fix(cc, comp, o1, v1 > 0);
