@@ -464,6 +464,91 @@ int orc_step(const orc_grid *g, const float *const F[6], orc_particles *p, doubl
 }
 
 /* ------------------------------------------------------------------------------------------
+ * N1  step 9 of the loop: digital filter passes on the conformal currents, Eqs. 9-11, then the
+ * recovery of the current density J^i = conformal J^i / sqrt(h).
+ * One pass = the (1/4, 1/2, 1/4) convolution along every dimension of the grid, f = (1/2)^(D + |di| + |dj| + |dk|), applied to
+ * each component on its OWN staggered lattice ("we disregard the staggering ... when denoting the indices").
+ * Values beyond the lattice of a component (readings):
+ *   PERIODIC dimension: the periodic image;
+ *   AXIS (theta) dimension: J^1(i+1/2, -1) = J^1(i+1/2, +1), J^2(i, -1/2) = -J^2(i, +1/2), J^3(i, 0) = 0, and the
+ *     mirror image of the same at theta = pi (j = N_2);
+ *   ABSORB dimension: zero (the paper is silent; what leaves through an absorbing side is discarded, G20).
+ * Lattice of component c along dimension d: N_d points (0 .. N_d - 1) if d is periodic; otherwise the half-integer lattice of a
+ * component staggered along d has N_d points (i + 1/2, i = 0 .. N_d - 1) and the integer lattice N_d + 1 (0 .. N_d).
+ * J staggering = E staggering: J^1 (1,0,0), J^2 (0,1,0), J^3 (0,0,1); in 2D J^3 sits on the nodes.
+ * divide != 0: afterwards J^c /= sqrt(h) at the component's own position, except on the polar axis itself (sqrt(h) = 0 there:
+ * J^3 = 0 by Eq. 12 and E^1 is advanced with the conformal J^1 through Eq. 13, so those nodes keep the conformal value).
+ * ------------------------------------------------------------------------------------------ */
+static int lattice_extent(const orc_grid *g, int comp, int d) {
+    if (d >= g->D) return 1;
+    if (g->bc[d] == ORC_PERIODIC) return g->N[d];
+    int stag = (comp == d);                                   /* J^c is staggered along its own direction only */
+    return stag ? g->N[d] : g->N[d] + 1;
+}
+/* value of component comp at lattice index (i0,i1,i2), with the boundary rules above; *sign receives the parity factor */
+static double filt_fetch(const orc_grid *g, const double *A, int comp, int i[3]) {
+    double sign = 1.0;
+    int q[3] = { i[0], i[1], i[2] };
+    for (int d = 0; d < g->D; ++d) {
+        int n = lattice_extent(g, comp, d);
+        if (q[d] >= 0 && q[d] < n) continue;
+        if (g->bc[d] == ORC_PERIODIC) { q[d] = ((q[d] % n) + n) % n; continue; }
+        if (g->bc[d] == ORC_AXIS) {
+            int stag = (comp == d);
+            if (stag) { q[d] = q[d] < 0 ? -1 - q[d] : 2 * n - 1 - q[d]; sign = -sign; }      /* (j + 1/2) -> -(j + 1/2): odd */
+            else { q[d] = q[d] < 0 ? -q[d] : 2 * (n - 1) - q[d]; }                            /* node j -> -j: even */
+            continue;
+        }
+        return 0.0;                                            /* ABSORB */
+    }
+    return sign * A[pidx(g, q[0], q[1], g->D == 3 ? q[2] : 0)];
+}
+static int on_axis_node(const orc_grid *g, int comp, const int i[3]) {
+    for (int d = 0; d < g->D; ++d)
+        if (g->bc[d] == ORC_AXIS && comp != d && (i[d] == 0 || i[d] == g->N[d])) return 1;
+    return 0;
+}
+void orc_filter_current(const orc_grid *g, double *const J[3], int npasses, int divide) {
+    int64_t total = orc_padded_size(g);
+    double *tmp = (double *)malloc(sizeof(double) * (size_t)total);
+    for (int comp = 0; comp < 3; ++comp) {
+        int n[3] = { lattice_extent(g, comp, 0), lattice_extent(g, comp, 1), lattice_extent(g, comp, 2) };
+        for (int pass = 0; pass < npasses; ++pass) {
+            memcpy(tmp, J[comp], sizeof(double) * (size_t)total);
+            if (comp == 2 && g->D == 2)                        /* J^3(i, 0) = 0 is a condition on the INPUT of the convolution */
+                for (int j = 0; j < n[1]; ++j)
+                    for (int i = 0; i < n[0]; ++i) { int c[3] = { i, j, 0 }; if (on_axis_node(g, comp, c)) tmp[pidx(g, i, j, 0)] = 0.0; }
+            for (int k = 0; k < n[2]; ++k)
+                for (int j = 0; j < n[1]; ++j)
+                    for (int i = 0; i < n[0]; ++i) {
+                        int c[3] = { i, j, k };
+                        double acc = 0.0;
+                        if (comp == 2 && g->D == 2 && on_axis_node(g, comp, c)) { J[comp][pidx(g, i, j, 0)] = 0.0; continue; }   /* J^3(i, 0) = 0 */
+                        for (int dk = (g->D == 3 ? -1 : 0); dk <= (g->D == 3 ? 1 : 0); ++dk)
+                            for (int dj = -1; dj <= 1; ++dj)
+                                for (int di = -1; di <= 1; ++di) {
+                                    int q[3] = { i + di, j + dj, k + dk };
+                                    double f = pow(0.5, g->D + abs(di) + abs(dj) + abs(dk));     /* Eqs. 9-11 */
+                                    acc += f * filt_fetch(g, tmp, comp, q);
+                                }
+                        J[comp][pidx(g, i, j, g->D == 3 ? k : 0)] = acc;
+                    }
+        }
+        if (divide)
+            for (int k = 0; k < n[2]; ++k)
+                for (int j = 0; j < n[1]; ++j)
+                    for (int i = 0; i < n[0]; ++i) {
+                        int c[3] = { i, j, k };
+                        if (on_axis_node(g, comp, c)) continue;
+                        double x[3] = { i + (comp == 0 ? 0.5 : 0.0), j + (comp == 1 ? 0.5 : 0.0), g->D == 3 ? k + (comp == 2 ? 0.5 : 0.0) : 0.0 }, h[3];
+                        orc_metric_h(g, x, h);
+                        J[comp][pidx(g, i, j, g->D == 3 ? k : 0)] /= sqrt(h[0] * h[1] * h[2]);
+                    }
+    }
+    free(tmp);
+}
+
+/* ------------------------------------------------------------------------------------------
  * Eq. 6 checker.  Conformal nodal charge (no 1/sqrt(h)):  rho[n] = sum_p q w prod_d omega(delta_d, s_d)
  * ------------------------------------------------------------------------------------------ */
 void orc_charge_density(const orc_grid *g, const orc_particles *p, const int8_t *mask, double q, double *rho) {

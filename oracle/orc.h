@@ -92,6 +92,11 @@ int orc_deposit(const orc_grid *g, const orc_particles *pold, const orc_particle
 void orc_fold_current(const orc_grid *g, double *const J[3]);
 void orc_fold_scalar(const orc_grid *g, double *rho);
 
+/* ---- step 9: npasses digital filter passes (Eqs. 9-11) with the periodic / axis / absorbing rules,
+ *      then (divide != 0) J^i = conformal J^i / sqrt(h) at each component's own position.  In place; J must already be
+ *      folded (orc_fold_current).  Ghost layers of the arrays are not touched. ---- */
+void orc_filter_current(const orc_grid *g, double *const J[3], int npasses, int divide);
+
 /* fused: gather_push then deposit (no fold) */
 int orc_step(const orc_grid *g, const float *const F[6], orc_particles *p, double *const J[3],
              double q, double m, double dt);

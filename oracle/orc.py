@@ -76,6 +76,7 @@ def lib():
                                   C.c_double, C.c_double]
         L.orc_fold_current.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p)]
         L.orc_fold_scalar.argtypes = [C.POINTER(_Grid), C.c_void_p]
+        L.orc_filter_current.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p), C.c_int, C.c_int]
         L.orc_step.restype = C.c_int
         L.orc_step.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p), C.POINTER(_Particles), C.POINTER(C.c_void_p),
                                C.c_double, C.c_double, C.c_double]
@@ -275,6 +276,11 @@ def fold_current(g: Grid, J) -> None:
 
 def fold_scalar(g: Grid, rho) -> None:
     lib().orc_fold_scalar(C.byref(g.c()), rho.ctypes.data)
+
+
+def filter_current(g: Grid, J, npasses: int, divide: bool = False) -> None:
+    """step 9: digital filter passes (Eqs. 9-11) in place, then optionally J = conformal J / sqrt(h)"""
+    lib().orc_filter_current(C.byref(g.c()), _jptrs(J), int(npasses), 1 if divide else 0)
 
 
 def step(g: Grid, F, p: Particles, J, q: float, m: float, dt: float) -> None:
