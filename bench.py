@@ -291,6 +291,18 @@ def measure(args, name, env, want_e2e):
                         "kernel_ms": k_ms, "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
                         "step_share": k_ms * len(parts) / ms_per_step}}
 
+    # ---- step 9: 4 digital filter passes (the count of the paper's magnetosphere runs) + J = conformal J / sqrt(h)
+    npass = 4
+    bind.ent_filter_current(ctx, J, npass, True)
+    fev = []
+    for _ in range(5):
+        timed(lambda: bind.ent_filter_current(ctx, J, npass, True), fev)
+    torch.cuda.synchronize()
+    f_ms = mean(fev)
+    f_bytes = 24.0 * ncell * npass                           # every pass reads and writes the three components once
+    out["current_filter"] = {"passes": npass, "ms": f_ms, "algorithmic_bytes": f_bytes, "achieved_gbs": f_bytes / (f_ms * 1e-3) / 1e9,
+                             "frac_of_hbm_peak": f_bytes / (f_ms * 1e-3) / 1e9 / peak, "note": "not part of `value` (sub-steps 3-8 only)"}
+
     # ---- end to end through the host-buffer C-ABI call: H2D of the step's inputs and D2H of its results inside ----
     if want_e2e:
         hp = [p.to("cpu", pin=True) for p in parts]
@@ -355,6 +367,7 @@ def run_ours(args):
             "strays_last_step": m["strays"], "bad_moves": m["bad_moves"]}
     if "e2e" in m:
         line["e2e"] = m["e2e"]
+    line["current_filter"] = m["current_filter"]
     if args.workload is None and not args.no_per_config and world == 1:
         per = []
         for name in ("C4", "C4s", "C5", "C2", "C1"):

@@ -177,6 +177,17 @@ int ent_zero_current(ent_ctx *ctx, ent_current *J);
  * onto the opposite active layers, then refilled with the periodic image. */
 int ent_fold_current(ent_ctx *ctx, ent_current *J);
 
+/* ---- step 9 of the loop: current post-processing ------------------------------------------------------------
+ * ent_filter_current: `npasses` digital filter passes on the conformal currents (Eqs. 9-11: the (1/4, 1/2, 1/4)
+ * kernel along every grid dimension, each component on its own staggered lattice) and then, if divide_by_sqrt_h != 0, the
+ * current density J^i = conformal J^i / sqrt(h) at each component's own position.  Values beyond a component's lattice:
+ * periodic image (PERIODIC); J^1 even, J^2 odd about the polar axis and J^3 = 0 on it (AXIS); zero (ABSORB).  On the
+ * axis itself (sqrt(h) = 0) the conformal value is kept (Eqs. 12-13 use it).  In place; J must have been folded
+ * (ent_fold_current).  Only the lattice points of each component are written (periodic dimension: 0 .. N-1; otherwise N points
+ * for the component staggered along that dimension, N + 1 for the others); ghost layers keep what they held.  A second set of
+ * current arrays is allocated in the ctx on first use (may synchronise). */
+int ent_filter_current(ent_ctx *ctx, ent_current *J, int npasses, int divide_by_sqrt_h);
+
 /* ---- host-buffer variant (end-to-end measurement) --------------------------------------------------------------
  * Every pointer in EB, p and J is a HOST pointer (pinned memory recommended).  Copies E,B and the particle block to ctx-owned
  * device staging, zeroes the device J, sorts the block by tile (ent_sort, full form), runs `nsteps` x ent_step on the sorted

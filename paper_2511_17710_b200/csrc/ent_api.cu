@@ -35,6 +35,7 @@ struct ent_ctx {
     // side buffers of the non-hot paths (two-kernel step, host-buffer step): allocated on first use
     void *oldbuf = nullptr; size_t oldbuf_cap = 0;
     void *hbuf = nullptr; size_t hbuf_cap = 0;
+    void *fbuf = nullptr; size_t fbuf_cap = 0;          // second set of current arrays for the filter passes
     size_t side_bytes = 0;
     // the blocks ent_sort / ent_step_sorted produced: each keeps its own layout so that several species stay sorted at a time
     struct SortedBlock { const int32_t *cell = nullptr; long long n = -1; int32_t *tile_off = nullptr; float *tile_wmax = nullptr;
@@ -156,7 +157,7 @@ extern "C" int ent_destroy(ent_ctx *ctx) {
     if (!ctx) return ENT_EINVAL;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    cudaFree(ctx->counters); cudaFree(ctx->pool); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf);
+    cudaFree(ctx->counters); cudaFree(ctx->pool); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf); cudaFree(ctx->fbuf);
     cudaGetLastError();
     delete ctx;
     return ENT_OK;
@@ -336,6 +337,43 @@ extern "C" int ent_fold_current(ent_ctx *ctx, ent_current *J) {
             fold_kernel<<<dim3(nblk(nthreads), 3), TPB, 0, ctx->stream>>>(g, cp(J), d, pass);
             if ((rc = launch_check(ctx, "fold_kernel"))) return rc;
         }
+    return ENT_OK;
+}
+
+// step 9: npasses digital filter passes (Eqs. 9-11) + optional J = conformal J / sqrt(h)
+extern "C" int ent_filter_current(ent_ctx *ctx, ent_current *J, int npasses, int divide_by_sqrt_h) {
+    ENTER();
+    int rc;
+    if ((rc = check_current(ctx, J))) return rc;
+    if (npasses < 0 || npasses > 1024) return fail(ctx, ENT_EINVAL, "npasses out of range");
+    if (npasses == 0 && !divide_by_sqrt_h) return ENT_OK;
+    const GridDev &g = ctx->g;
+    const size_t slot = ((size_t)padded_size(g) * 4 + 255) & ~(size_t)255;
+    if ((rc = ensure(ctx, &ctx->fbuf, &ctx->fbuf_cap, 3 * slot))) return rc;
+    FilterGeom L;
+    long long maxpts = 1;
+    for (int d = 0; d < 3; ++d) L.rule[d] = d < g.D ? g.bc[d] : ENT_PERIODIC;
+    for (int c = 0; c < 3; ++c) {
+        long long pts = 1;
+        for (int d = 0; d < 3; ++d) {
+            int n = 1;
+            if (d < g.D) n = g.bc[d] == ENT_PERIODIC ? g.N[d] : (c == d ? g.N[d] : g.N[d] + 1);       // half-integer / integer lattice
+            L.n[c][d] = n; pts *= n;
+        }
+        if (pts > maxpts) maxpts = pts;
+    }
+    CurrentPtrs a = cp(J), b;
+    for (int c = 0; c < 3; ++c) b.c[c] = (float *)((char *)ctx->fbuf + slot * c);
+    const int total = npasses ? npasses : 1;
+    for (int pass = 0; pass < total; ++pass) {
+        const bool last = pass == total - 1;
+        filter_pass_kernel<<<dim3(nblk(maxpts), 3), TPB, 0, ctx->stream>>>(g, L, (pass & 1) ? b : a, (pass & 1) ? a : b, npasses == 0, last && divide_by_sqrt_h);
+        if ((rc = launch_check(ctx, "filter_pass_kernel"))) return rc;
+    }
+    if (total & 1) {                                         // the result sits in the scratch arrays: copy the lattice points back
+        filter_pass_kernel<<<dim3(nblk(maxpts), 3), TPB, 0, ctx->stream>>>(g, L, b, a, 2, 0);
+        if ((rc = launch_check(ctx, "filter_pass_kernel"))) return rc;
+    }
     return ENT_OK;
 }
 

@@ -158,6 +158,70 @@ __global__ void fold_kernel(GridDev g, CurrentPtrs J, int dim, int pass) {      
     }
 }
 
+// ---- N1, step 9 of the loop: one digital filter pass on the conformal currents, Eqs. 9-11 ----
+// Each component is convolved with (1/4, 1/2, 1/4) along every grid dimension on its own staggered lattice.  Values beyond the
+// lattice: periodic image; polar axis: J^1 even, J^2 odd about the axis, J^3 = 0 on it; ABSORB side: zero.
+// `divide`: the pass also turns its result into J^i = conformal J^i / sqrt(h) at the component's own position, except on
+// the axis itself (sqrt(h) = 0: Eq. 12-13 use the conformal value there).  `identity`: no convolution (scaling pass only).
+// One thread per lattice point, blockIdx.y = component; src and dst are different arrays.
+struct FilterGeom {
+    int n[3][3];       // lattice extent of component c along dimension d
+    int rule[3];       // boundary rule of dimension d (ENT_PERIODIC / ENT_ABSORB / ENT_AXIS); unused dimensions: ENT_PERIODIC, n = 1
+};
+__device__ __forceinline__ bool filter_on_axis(const GridDev &g, const FilterGeom &L, int comp, int q1) {
+    return g.kind != ENT_CART && comp != 1 && (q1 == 0 || q1 == L.n[comp][1] - 1);      // theta lattice of J^1, J^3: nodes 0 .. N_2
+}
+__device__ __forceinline__ float filter_fetch(const GridDev &g, const FilterGeom &L, const float *A, int comp, int q0, int q1, int q2) {
+    int q[3] = { q0, q1, q2 };
+    float sign = 1.f;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const int n = L.n[comp][d];
+        if ((unsigned)q[d] < (unsigned)n) continue;
+        if (L.rule[d] == ENT_PERIODIC) q[d] += q[d] < 0 ? n : -n;
+        else if (L.rule[d] == ENT_AXIS) {
+            if (comp == d) { q[d] = q[d] < 0 ? -1 - q[d] : 2 * n - 1 - q[d]; sign = -sign; }      // (j + 1/2) -> -(j + 1/2): odd
+            else q[d] = q[d] < 0 ? -q[d] : 2 * (n - 1) - q[d];                                    // node j -> -j: even
+        } else return 0.f;
+    }
+    if (comp == 2 && filter_on_axis(g, L, comp, q[1])) return 0.f;              // J^3(i, 0) = 0: a condition on the INPUT of the stencil
+    const long long idx = (long long)(q[0] + NG) + (long long)g.P[0] * ((long long)(q[1] + NG) + (g.D == 3 ? (long long)g.P[1] * (q[2] + NG) : 0));
+    return sign * A[idx];
+}
+__device__ __forceinline__ float sqrt_h_at(const GridDev &g, double x1, double x2) {          // sqrt(h11 h22 h33)
+    if (g.kind == ENT_CART) return g.dx[0] * g.dx[1] * g.dx[2];
+    if (g.kind == ENT_SPH) { const double r = g.rmin + x1 * g.dr, th = x2 * g.dth; return (float)(g.dr * (r * g.dth) * (r * sin(th))); }
+    const double eR = exp(g.Rmin + x1 * g.dR), T = x2 * g.dT, r = g.r0 + eR;
+    return (float)((g.dR * eR) * (g.dT * dtheta_dT(g.vt, T) * r) * (r * sin(theta_of_T(g.vt, T))));
+}
+__global__ void __launch_bounds__(TPB) filter_pass_kernel(GridDev g, FilterGeom L, CurrentPtrs src, CurrentPtrs dst, int identity, int divide) {
+    const int comp = blockIdx.y;
+    const int n0 = L.n[comp][0], n1 = L.n[comp][1], n2 = L.n[comp][2];
+    const long long t = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (t >= (long long)n0 * n1 * n2) return;
+    const int i = (int)(t % n0), j = (int)((t / n0) % n1), k = (int)(t / ((long long)n0 * n1));
+    const float *A = src.c[comp];
+    const bool axis_node = filter_on_axis(g, L, comp, j);
+    float acc;
+    if (identity) acc = A[(long long)(i + NG) + (long long)g.P[0] * ((long long)(j + NG) + (g.D == 3 ? (long long)g.P[1] * (k + NG) : 0))];
+    else if (comp == 2 && axis_node) acc = 0.f;                                  // J^3(i, 0) = 0
+    else {
+        acc = 0.f;
+        const int kz = g.D == 3 ? 1 : 0;
+        for (int dk = -kz; dk <= kz; ++dk)
+#pragma unroll
+            for (int dj = -1; dj <= 1; ++dj) {
+                const float wjk = (dj ? 0.25f : 0.5f) * (g.D == 3 ? (dk ? 0.25f : 0.5f) : 1.0f);
+                const float a = filter_fetch(g, L, A, comp, i - 1, j + dj, k + dk), b = filter_fetch(g, L, A, comp, i, j + dj, k + dk),
+                            c = filter_fetch(g, L, A, comp, i + 1, j + dj, k + dk);
+                acc += wjk * (0.25f * a + 0.5f * b + 0.25f * c);                 // f = (1/2)^(D + |di| + |dj| + |dk|), Eqs. 9-11
+            }
+    }
+    if (divide && !axis_node)
+        acc /= sqrt_h_at(g, i + (comp == 0 ? 0.5 : 0.0), j + (comp == 1 ? 0.5 : 0.0));
+    dst.c[comp][(long long)(i + NG) + (long long)g.P[0] * ((long long)(j + NG) + (g.D == 3 ? (long long)g.P[1] * (k + NG) : 0))] = acc;
+}
+
 // ---- S10: counting sort by tile-major key ----
 template <int D>
 __global__ void __launch_bounds__(TPB) sort_hist_kernel(GridDev g, const int32_t *cell, long long n, int32_t *keys, int32_t *count) {
