@@ -251,6 +251,40 @@ void orc_boris(double u[3], const double E[3], const double B[3], double qm, dou
 }
 
 /* ------------------------------------------------------------------------------------------
+ * N3  the other "conventional particle pusher" P:95 names: J.-L. Vay, Phys. Plasmas 15, 056701 (2008).  Same interface and time
+ * levels as orc_boris (u^(n-1/2) -> u^(n+1/2), fields at n).  Written out from the published scheme:
+ *   u'   = u + eps (E + v x B) + eps E,  v = u / gamma(u),  eps = (q/m) dt / 2         (half step with the old velocity, then half E kick)
+ *   tau  = eps B,  u* = u'.tau,  sigma = gamma'^2 - tau^2,  gamma'^2 = 1 + u'^2
+ *   gamma_new^2 = [ sigma + sqrt(sigma^2 + 4 (tau^2 + u*^2)) ] / 2
+ *   t = tau / gamma_new,  u_new = [ u' + (u'.t) t + u' x t ] / (1 + t^2)
+ * ------------------------------------------------------------------------------------------ */
+void orc_vay(double u[3], const double E[3], const double B[3], double qm, double dt) {
+    double eps = qm * dt / 2.0;
+    double g0 = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+    double v[3] = { u[0] / g0, u[1] / g0, u[2] / g0 };
+    double up[3], tau[3], t[3];
+    up[0] = u[0] + eps * (2.0 * E[0] + (v[1] * B[2] - v[2] * B[1]));
+    up[1] = u[1] + eps * (2.0 * E[1] + (v[2] * B[0] - v[0] * B[2]));
+    up[2] = u[2] + eps * (2.0 * E[2] + (v[0] * B[1] - v[1] * B[0]));
+    for (int a = 0; a < 3; ++a) tau[a] = eps * B[a];
+    double tau2 = tau[0] * tau[0] + tau[1] * tau[1] + tau[2] * tau[2];
+    double ustar = up[0] * tau[0] + up[1] * tau[1] + up[2] * tau[2];
+    double gp2 = 1.0 + up[0] * up[0] + up[1] * up[1] + up[2] * up[2];
+    double sigma = gp2 - tau2;
+    double gnew = sqrt(0.5 * (sigma + sqrt(sigma * sigma + 4.0 * (tau2 + ustar * ustar))));
+    for (int a = 0; a < 3; ++a) t[a] = tau[a] / gnew;
+    double t2 = t[0] * t[0] + t[1] * t[1] + t[2] * t[2];
+    double udt = up[0] * t[0] + up[1] * t[1] + up[2] * t[2];
+    double sfac = 1.0 / (1.0 + t2);
+    u[0] = sfac * (up[0] + udt * t[0] + (up[1] * t[2] - up[2] * t[1]));
+    u[1] = sfac * (up[1] + udt * t[1] + (up[2] * t[0] - up[0] * t[2]));
+    u[2] = sfac * (up[2] + udt * t[2] + (up[0] * t[1] - up[1] * t[0]));
+}
+
+static int orc_pusher_kind = 0;           /* 0 = Boris (default), 1 = Vay; read by orc_gather_push */
+int orc_set_pusher(int kind) { int prev = orc_pusher_kind; if (kind == 0 || kind == 1) orc_pusher_kind = kind; return prev; }
+
+/* ------------------------------------------------------------------------------------------
  * steps 3-7 + O7 crossing bookkeeping (readings G9, G11)
  * ------------------------------------------------------------------------------------------ */
 static inline int floor_mod(int a, int n) { int r = a % n; return r < 0 ? r + n : r; }
@@ -279,7 +313,7 @@ int orc_gather_push(const orc_grid *g, const float *const F[6], const orc_partic
             orc_to_cartesian_basis(g, x, EB, E);
             orc_to_cartesian_basis(g, x, EB + 3, B);
             /* step 5: u^(n-1/2) -> u^(n+1/2) */
-            orc_boris(u, E, B, qm, dt);
+            if (orc_pusher_kind == 1) orc_vay(u, E, B, qm, dt); else orc_boris(u, E, B, qm, dt);
             /* step 6: x^(n) -> x^(n+1) with u^(n+1/2) / gamma^(n+1/2), in the global Cartesian frame */
             double gam = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
             double X[3], xn[3];

@@ -80,6 +80,10 @@ void orc_to_cartesian_basis(const orc_grid *g, const double x[3], const double A
 /* ---- O4 Boris ---- */
 void orc_boris(double u[3], const double E[3], const double B[3], double q_over_m, double dt);
 
+/* ---- N3: Vay (2008) pusher, same interface; orc_set_pusher selects the one orc_gather_push / orc_step use (0 Boris, 1 Vay) ---- */
+void orc_vay(double u[3], const double E[3], const double B[3], double q_over_m, double dt);
+int  orc_set_pusher(int kind);                                            /* returns the previous kind */
+
 /* ---- steps 3-7 for a particle block; out may alias in (arrays are overwritten element-wise) ---- */
 int orc_gather_push(const orc_grid *g, const float *const F[6], const orc_particles *in, orc_particles *out,
                     double q_over_m, double dt);

@@ -68,6 +68,8 @@ def lib():
         L.orc_gather.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p), C.POINTER(C.c_int32), dp, dp]
         L.orc_to_cartesian_basis.argtypes = [C.POINTER(_Grid), dp, dp, dp]
         L.orc_boris.argtypes = [dp, dp, dp, C.c_double, C.c_double]
+        L.orc_vay.argtypes = [dp, dp, dp, C.c_double, C.c_double]
+        L.orc_set_pusher.restype = C.c_int; L.orc_set_pusher.argtypes = [C.c_int]
         L.orc_gather_push.restype = C.c_int
         L.orc_gather_push.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p), C.POINTER(_Particles), C.POINTER(_Particles),
                                       C.c_double, C.c_double]
@@ -247,6 +249,17 @@ def boris(u, E, B, q_over_m, dt) -> np.ndarray:
     ua = np.array(u, dtype=np.float64); Ea, Ep = _vec(E); Ba, Bp = _vec(B)
     lib().orc_boris(ua.ctypes.data_as(C.POINTER(C.c_double)), Ep, Bp, q_over_m, dt)
     return ua
+
+
+def vay(u, E, B, q_over_m, dt) -> np.ndarray:
+    ua = np.array(u, dtype=np.float64); Ea, Ep = _vec(E); Ba, Bp = _vec(B)
+    lib().orc_vay(ua.ctypes.data_as(C.POINTER(C.c_double)), Ep, Bp, q_over_m, dt)
+    return ua
+
+
+def set_pusher(kind: int) -> int:
+    """0 = Boris (default), 1 = Vay: the pusher orc.gather_push / orc.step use; returns the previous kind"""
+    return lib().orc_set_pusher(int(kind))
 
 
 def gather_push(g: Grid, F, p: Particles, q_over_m: float, dt: float) -> Particles:

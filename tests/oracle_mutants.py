@@ -21,9 +21,9 @@ MUTANTS = [
      "double gm = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);",
      T + "test_boris_is_time_reversible_with_E_and_B"),
     ("move: gamma of the OLD momentum (reading G4)",
-     ["            orc_boris(u, E, B, qm, dt);\n",
+     ["            if (orc_pusher_kind == 1) orc_vay(u, E, B, qm, dt); else orc_boris(u, E, B, qm, dt);\n",
       "            double gam = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);\n            double X[3], xn[3];\n"],
-     ["            double gam = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);\n            orc_boris(u, E, B, qm, dt);\n",
+     ["            double gam = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);\n            if (orc_pusher_kind == 1) orc_vay(u, E, B, qm, dt); else orc_boris(u, E, B, qm, dt);\n",
       "            double X[3], xn[3];\n"],
      T + "test_hyperbolic_motion_converges_at_second_order"),
     ("deposit: J^3 from the old momentum (reading G8)",
@@ -46,6 +46,22 @@ MUTANTS = [
      "if (inew >= g->N[a]) { inew = g->N[a] - 1; dnew = nextafter(1.0, 0.0); }",
      "",
      T + "test_landing_on_theta_equals_pi_is_clamped_into_the_last_cell"),
+    ("vay: final rotation without the (u'.t) t term",
+     "u[0] = sfac * (up[0] + udt * t[0] + (up[1] * t[2] - up[2] * t[1]));",
+     "u[0] = sfac * (up[0] + (up[1] * t[2] - up[2] * t[1]));",
+     "tests/test_oracle_pins_vay.py::test_vay_keeps_a_drifting_particle_force_free"),
+    ("vay: half step with gamma of u' instead of the old velocity",
+     "double g0 = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);\n    double v[3]",
+     "double g0 = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * 1.05;\n    double v[3]",
+     "tests/test_oracle_pins_vay.py::test_vay_keeps_a_drifting_particle_force_free"),
+    ("filter: weight 1/4 for the centre tap (Eq. 9 garbled)",
+     "double f = pow(0.5, g->D + abs(di) + abs(dj) + abs(dk));",
+     "double f = pow(0.5, g->D + 1 + abs(di) + abs(dj) + abs(dk)) * (1 + (di == 0));",
+     "tests/test_oracle_pins_filter.py::test_fourier_mode_is_damped_by_cos2_of_half_k_per_pass"),
+    ("filter: J^2 even instead of odd about the axis (P:386)",
+     "{ q[d] = q[d] < 0 ? -1 - q[d] : 2 * n - 1 - q[d]; sign = -sign; }",
+     "{ q[d] = q[d] < 0 ? -1 - q[d] : 2 * n - 1 - q[d]; }",
+     "tests/test_oracle_pins_filter.py::test_axis_rules_hand_example"),
     # mutants the round-1 pins already killed, kept so that the list documents them
     ("deposit: 3D weights without the D_a D_b / 12 term (reading G7)",
      "+ sigma * Dv[a] * Dv[b] / 12.0",
