@@ -202,6 +202,7 @@ enum {
     ENT_OPT_STEP_IMPL = 1,     /* 0 = auto (tiled when the block is the sorted one), 1 = force untiled, 2 = two-kernel
                                   (gather_push to scratch copy + deposit; the paper's structure) */
     ENT_OPT_TILE_1 = 2, ENT_OPT_TILE_2 = 3, ENT_OPT_TILE_3 = 4,   /* tile extents in cells; takes effect at the next ent_set_grid */
+    ENT_OPT_PUSHER = 7,        /* momentum update of sub-step 5: 0 = relativistic Boris (default), 1 = Vay (2008).  Takes effect at once. */
     ENT_OPT_CURV_FP64 = 6,     /* SPH / QSPH grids: 0 (default) = the move is evaluated in fp32 as a DISPLACEMENT in the local frame at the
                                   particle (increments of the code coordinates added to the in-cell offsets; same mathematics as
                                   P:147-153 + P:285-327); 1 = fp64 coordinate maps through the global Cartesian frame (the literal

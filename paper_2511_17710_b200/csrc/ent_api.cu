@@ -22,6 +22,7 @@ struct ent_ctx {
     int tile_opt[3] = {0, 0, 0};          // 0 = default
     int step_impl = 0;
     int curv_f64 = 0;                     // ENT_OPT_CURV_FP64
+    int pusher = 0;                       // ENT_OPT_PUSHER
     int sort_mode = 0;                    // 0 auto (re-bin when the input is a sorted block), 1 always the full cell-level sort
     int last_sort_rebin = 0;
     int rebin_ordered = 1;                // re-bin keeps the particles that stay in a tile ordered by cell (Cartesian grids)
@@ -219,7 +220,7 @@ extern "C" int ent_set_grid(ent_ctx *ctx, const ent_grid *gr) {
         g.dT = PI_D / gr->N[1];
     }
     g.rminf = (float)g.rmin; g.drf = (float)g.dr; g.dthf = (float)g.dth; g.Rminf = (float)g.Rmin; g.dRf = (float)g.dR; g.dTf = (float)g.dT;
-    g.r0f = (float)g.r0; g.vtf = (float)g.vt; g.curv_f64 = ctx->curv_f64;
+    g.r0f = (float)g.r0; g.vtf = (float)g.vt; g.curv_f64 = ctx->curv_f64; g.pusher = ctx->pusher;
     ctx->grid = *gr; ctx->g = g; ctx->have_grid = true;
     forget_all(ctx);
     if (ctx->pool) {                                            // the pool was carved for the previous grid
@@ -644,6 +645,9 @@ extern "C" int ent_set_option(ent_ctx *ctx, int key, int64_t value) {
         case ENT_OPT_SORT_MODE:
             if (value < 0 || value > 2) return fail(ctx, ENT_EINVAL, "ENT_OPT_SORT_MODE must be 0, 1 or 2");
             ctx->sort_mode = value == 1 ? 1 : 0; ctx->rebin_ordered = value != 2; return ENT_OK;
+        case ENT_OPT_PUSHER:
+            if (value < 0 || value > 1) return fail(ctx, ENT_EINVAL, "ENT_OPT_PUSHER must be 0 (Boris) or 1 (Vay)");
+            ctx->pusher = (int)value; ctx->g.pusher = (int)value; return ENT_OK;
         case ENT_OPT_CURV_FP64:
             if (value < 0 || value > 1) return fail(ctx, ENT_EINVAL, "ENT_OPT_CURV_FP64 must be 0 or 1");
             ctx->curv_f64 = (int)value; ctx->g.curv_f64 = (int)value; return ENT_OK;

@@ -29,6 +29,7 @@ struct GridDev {
     double Rmin, dR, dT, r0, vt;
     // fp32 copies for the displacement form of the curvilinear move (ent_particle.cuh) and its switch
     float rminf, drf, dthf, Rminf, dRf, dTf, r0f, vtf;
+    int pusher;        // ENT_OPT_PUSHER: 0 Boris, 1 Vay
     int curv_f64;      // 1: coordinate maps of the axisymmetric grids in fp64 through the global Cartesian frame (round-1 form)
 };
 
@@ -248,6 +249,33 @@ __device__ __forceinline__ void boris(float u[3], const float E[3], const float 
     u[0] = um0 + (p1 * s2 - p2 * s1) + eps * E[0];
     u[1] = um1 + (p2 * s0 - p0 * s2) + eps * E[1];
     u[2] = um2 + (p0 * s1 - p1 * s0) + eps * E[2];
+}
+// the other conventional pusher P:95 names: J.-L. Vay, Phys. Plasmas 15, 056701 (2008); same interface and time levels
+__device__ __forceinline__ void vay(float u[3], const float E[3], const float B[3], float eps) {
+    float g2 = 1.0f + u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    float ig = rsqrtf(g2);
+    ig = ig * (1.5f - 0.5f * g2 * ig * ig);
+    const float v0 = u[0] * ig, v1 = u[1] * ig, v2 = u[2] * ig;
+    const float p0 = u[0] + eps * (2.0f * E[0] + (v1 * B[2] - v2 * B[1]));        // half step with the old velocity + half E kick
+    const float p1 = u[1] + eps * (2.0f * E[1] + (v2 * B[0] - v0 * B[2]));
+    const float p2 = u[2] + eps * (2.0f * E[2] + (v0 * B[1] - v1 * B[0]));
+    const float a0 = eps * B[0], a1 = eps * B[1], a2 = eps * B[2];                // tau
+    const float tau2 = a0 * a0 + a1 * a1 + a2 * a2;
+    const float us = p0 * a0 + p1 * a1 + p2 * a2;
+    const float sigma = 1.0f + p0 * p0 + p1 * p1 + p2 * p2 - tau2;
+    const float gn2 = 0.5f * (sigma + sqrtf(sigma * sigma + 4.0f * (tau2 + us * us)));
+    float ign = rsqrtf(gn2);
+    ign = ign * (1.5f - 0.5f * gn2 * ign * ign);
+    const float t0 = a0 * ign, t1 = a1 * ign, t2 = a2 * ign;
+    const float sf = 1.0f / (1.0f + t0 * t0 + t1 * t1 + t2 * t2);
+    const float ut = p0 * t0 + p1 * t1 + p2 * t2;
+    u[0] = sf * (p0 + ut * t0 + (p1 * t2 - p2 * t1));
+    u[1] = sf * (p1 + ut * t1 + (p2 * t0 - p0 * t2));
+    u[2] = sf * (p2 + ut * t2 + (p0 * t1 - p1 * t0));
+}
+// step 5 with the pusher the grid struct selects (ENT_OPT_PUSHER): 0 Boris, 1 Vay
+__device__ __forceinline__ void push_momentum(int pusher, float u[3], const float E[3], const float B[3], float eps) {
+    if (pusher == 1) vay(u, E, B, eps); else boris(u, E, B, eps);
 }
 __device__ __forceinline__ float inv_gamma(const float u[3]) {
     float g2 = 1.0f + u[0] * u[0] + u[1] * u[1] + u[2] * u[2];

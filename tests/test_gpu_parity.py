@@ -393,3 +393,19 @@ def test_error_paths_on_device(env):
     with pytest.raises(bind.EntError):
         bind.ent_step(ctx, F, pe, J, -1.0)                                                              # dt <= 0
     assert bind.ent_get_stat(ctx, bind.STAT_LAUNCHES) == before
+
+
+@pytest.mark.parametrize("name,impl,sort_first", [("C1", 0, True), ("C3/8", 0, True), ("C3/8", 1, False), ("C5/32", 0, True), ("ABS3", 0, True)])
+def test_vay_pusher_matches_oracle(env, name, impl, sort_first):
+    """ENT_OPT_PUSHER = 1 (Vay 2008) against the oracle's orc_vay through the whole step, tiled and untiled kernels"""
+    bind, synth, ctx, orc = env
+    wl = _workloads(synth)[name]()
+    bind.ent_set_option(ctx, bind.OPT_PUSHER, 1)
+    orc.set_pusher(1)
+    try:
+        stats = _run_case(env, wl, impl=impl, sort_first=sort_first, steps=min(wl.steps, 6), resort_every=3 if sort_first else 0)
+    finally:
+        bind.ent_set_option(ctx, bind.OPT_PUSHER, 0)
+        orc.set_pusher(0)
+    print(name, "vay", stats)
+    assert all(st["max_u_rel"] <= P.MOM_TOL for st in stats.values())
