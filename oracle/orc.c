@@ -622,6 +622,27 @@ double orc_continuity_residual(const orc_grid *g, double *const J[3], const doub
     return worst;
 }
 
+/* N4  tag sort: "sorts all the particle quantities based on their tag, after which npart always indicates the number
+ * of alive particles, while the dead ones are shuffled to the end".  Stable: alive particles keep their order, so do the dead.
+ * Returns the number of alive particles; out must not alias in. */
+int64_t orc_compact(int D, int axisym, const orc_particles *in, orc_particles *out) {
+    int64_t n = in->n, k = 0;
+    for (int pass = 0; pass < 2; ++pass)                    /* pass 0: alive, pass 1: dead */
+        for (int64_t p = 0; p < n; ++p) {
+            int alive = in->tag ? in->tag[p] != 0 : 1;
+            if (alive == pass) continue;
+            for (int a = 0; a < D; ++a) { out->i[a][k] = in->i[a][p]; out->d[a][k] = in->d[a][p]; }
+            for (int a = 0; a < 3; ++a) out->u[a][k] = in->u[a][p];
+            out->w[k] = in->w[p];
+            if (axisym) out->phi[k] = in->phi[p];
+            if (out->tag) out->tag[k] = (int8_t)alive;
+            ++k;
+        }
+    int64_t na = 0;
+    for (int64_t p = 0; p < n; ++p) na += in->tag ? in->tag[p] != 0 : 1;
+    return na;
+}
+
 /* S10 checker: keys non-decreasing; offsets[c] = number of keys < c (exclusive scan of the histogram) */
 int orc_sort_check(const int64_t n, const int32_t *keys, int64_t ncell, const int32_t *offsets) {
     for (int64_t p = 1; p < n; ++p) if (keys[p] < keys[p - 1]) return 1;

@@ -111,6 +111,9 @@ void   orc_charge_density(const orc_grid *g, const orc_particles *p, const int8_
 double orc_continuity_residual(const orc_grid *g, double *const J[3], const double *rho_old, const double *rho_new,
                                double dt, double *R_out /* padded or NULL */);
 
+/* ---- N4 tag sort: alive particles first (stable), dead ones after; returns the number of alive particles ---- */
+int64_t orc_compact(int D, int axisym, const orc_particles *in, orc_particles *out);
+
 /* ---- sort checker: keys non-decreasing, offsets = exclusive scan of histogram; returns 0 if ok ---- */
 int orc_sort_check(const int64_t n, const int32_t *keys_sorted, int64_t ncell, const int32_t *offsets /* ncell+1 or NULL */);
 

@@ -85,6 +85,8 @@ def lib():
         L.orc_charge_density.argtypes = [C.POINTER(_Grid), C.POINTER(_Particles), C.c_void_p, C.c_double, C.c_void_p]
         L.orc_continuity_residual.restype = C.c_double
         L.orc_continuity_residual.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p), C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
+        L.orc_compact.restype = C.c_int64
+        L.orc_compact.argtypes = [C.c_int, C.c_int, C.POINTER(_Particles), C.POINTER(_Particles)]
         L.orc_sort_check.restype = C.c_int
         L.orc_sort_check.argtypes = [C.c_int64, C.c_void_p, C.c_int64, C.c_void_p]
         L.orc_padded_size.restype = C.c_int64; L.orc_padded_size.argtypes = [C.POINTER(_Grid)]
@@ -318,6 +320,15 @@ def continuity_residual(g: Grid, J, rho_old, rho_new, dt, want_field=False):
     worst = lib().orc_continuity_residual(C.byref(g.c()), _jptrs(J), rho_old.ctypes.data, rho_new.ctypes.data, dt,
                                           None if R is None else R.ctypes.data)
     return (worst, R) if want_field else worst
+
+
+def compact(p: Particles):
+    """tag sort: returns (new block with the alive particles first, number alive)"""
+    out = p.copy()
+    if out.tag is None:
+        out.tag = np.ones(p.n, dtype=np.int8)
+    na = lib().orc_compact(len(p.i), 0 if p.phi is None else 1, C.byref(p.c()), C.byref(out.c()))
+    return out, int(na)
 
 
 def sort_check(keys_sorted, ncell, offsets=None) -> int:

@@ -283,3 +283,24 @@ def test_sort_check(orc):
     bad = offs.copy(); bad[3] = 4
     assert orc.sort_check(keys, 6, bad) == 3
     assert orc.sort_check(np.array([0, 7], dtype=np.int32), 6) == 2
+
+
+def test_tag_sort_is_a_stable_partition(orc):
+    """N4: after the tag sort the alive particles come first and npart counts them; hand example + the properties that
+    define a stable partition (same multiset, both groups in their original order)."""
+    i = [[3, 1], [0, 2], [5, 5], [4, 4], [1, 1], [2, 0]]
+    p = make_particles(orc, i, np.arange(12).reshape(6, 2) / 20.0, np.arange(18).reshape(6, 3) * 0.1, w=[1, 2, 3, 4, 5, 6],
+                       tag=[1, 0, 0, 1, 1, 0])
+    out, na = orc.compact(p)
+    assert na == 3
+    assert list(out.w) == [1, 4, 5, 2, 3, 6] and list(out.tag) == [1, 1, 1, 0, 0, 0]
+    assert list(out.i[0]) == [3, 4, 1, 0, 5, 2] and list(out.i[1]) == [1, 4, 1, 2, 5, 0]
+    assert np.allclose(out.u[2], [0.2, 1.1, 1.4, 0.5, 0.8, 1.7]) and np.allclose(out.d[1], [0.05, 0.35, 0.45, 0.15, 0.25, 0.55])
+    rng = np.random.default_rng(60)
+    n = 500
+    tag = (rng.uniform(size=n) < 0.7).astype(np.int8)
+    p = make_particles(orc, rng.integers(0, 9, (n, 3)), rng.uniform(0, 1, (n, 3)), rng.standard_normal((n, 3)), w=np.arange(n) + 1.0, tag=tag)
+    out, na = orc.compact(p)
+    assert na == int(tag.sum())
+    assert np.array_equal(out.w[:na], p.w[tag == 1]) and np.array_equal(out.w[na:], p.w[tag == 0])
+    assert np.all(out.tag[:na] == 1) and np.all(out.tag[na:] == 0)
