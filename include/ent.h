@@ -177,6 +177,14 @@ int ent_zero_current(ent_ctx *ctx, ent_current *J);
  * onto the opposite active layers, then refilled with the periodic image. */
 int ent_fold_current(ent_ctx *ctx, ent_current *J);
 
+/* ---- tag sort ---------------------------------------------------------------------------------------------
+ * ent_compact: out-of-place stable partition of a species by tag: the alive particles (tag != 0) come first, in their original
+ * order, the dead ones after them, so that the first *n_alive records are the population and later calls may pass n = *n_alive.
+ * Both blocks need tag arrays; in and out must not overlap; n_alive (may be NULL) is a DEVICE int64 written by the call.  A block
+ * that was sorted stays tile-contiguous in its alive part, but the ctx forgets `out` (call ent_sort on the shortened block).
+ * Scratch (12 bytes per particle) is allocated in the ctx on first use (may synchronise). */
+int ent_compact(ent_ctx *ctx, const ent_particles *in, ent_particles *out, int64_t *n_alive);
+
 /* ---- step 9 of the loop: current post-processing ------------------------------------------------------------
  * ent_filter_current: `npasses` digital filter passes on the conformal currents (Eqs. 9-11: the (1/4, 1/2, 1/4)
  * kernel along every grid dimension, each component on its own staggered lattice) and then, if divide_by_sqrt_h != 0, the

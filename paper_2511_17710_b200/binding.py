@@ -22,7 +22,7 @@ OPT_STEP_IMPL, OPT_TILE_1, OPT_TILE_2, OPT_TILE_3, OPT_SORT_MODE, OPT_CURV_FP64,
  STAT_SCRATCH_BYTES, STAT_LAST_STEP_TILED, STAT_LAST_SORT_REBIN, STAT_SLOT_ERRORS, STAT_CARRIES, STAT_GLOBAL_ADDS) = range(1, 15)
 
 SYMBOLS = ["ent_create", "ent_destroy", "ent_last_error", "ent_set_grid", "ent_gather_push", "ent_deposit", "ent_sort",
-           "ent_step", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_filter_current", "ent_step_host", "ent_set_option", "ent_get_stat", "ent_version"]
+           "ent_step", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_filter_current", "ent_compact", "ent_step_host", "ent_set_option", "ent_get_stat", "ent_version"]
 
 
 class EntError(RuntimeError):
@@ -78,6 +78,7 @@ def lib():
         L.ent_zero_current.argtypes = [vp, C.POINTER(_Current)]
         L.ent_fold_current.argtypes = [vp, C.POINTER(_Current)]
         L.ent_filter_current.argtypes = [vp, C.POINTER(_Current), C.c_int, C.c_int]
+        L.ent_compact.argtypes = [vp, C.POINTER(_Particles), C.POINTER(_Particles), vp]
         L.ent_step_host.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Current), C.c_float, C.c_int,
                                     C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.ent_set_option.argtypes = [vp, C.c_int, C.c_int64]
@@ -296,6 +297,13 @@ def ent_zero_current(ctx: Ctx, J) -> None:
 
 def ent_fold_current(ctx: Ctx, J) -> None:
     ctx._ck(lib().ent_fold_current(ctx._h, C.byref(_current(J))))
+
+
+def ent_compact(ctx: Ctx, pin: Particles, pout: Particles) -> torch.Tensor:
+    """tag sort; returns a one-element int64 device tensor holding the number of alive particles"""
+    na = torch.zeros(1, dtype=torch.int64, device=pin.cell.device)
+    ctx._ck(lib().ent_compact(ctx._h, C.byref(pin.c()), C.byref(pout.c()), na.data_ptr()))
+    return na
 
 
 def ent_filter_current(ctx: Ctx, J, npasses: int, divide_by_sqrt_h: bool = False) -> None:

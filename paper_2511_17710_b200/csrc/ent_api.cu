@@ -37,6 +37,7 @@ struct ent_ctx {
     void *oldbuf = nullptr; size_t oldbuf_cap = 0;
     void *hbuf = nullptr; size_t hbuf_cap = 0;
     void *fbuf = nullptr; size_t fbuf_cap = 0;          // second set of current arrays for the filter passes
+    void *cbuf = nullptr; size_t cbuf_cap = 0;          // flags and positions of ent_compact
     size_t side_bytes = 0;
     // the blocks ent_sort / ent_step_sorted produced: each keeps its own layout so that several species stay sorted at a time
     struct SortedBlock { const int32_t *cell = nullptr; long long n = -1; int32_t *tile_off = nullptr; float *tile_wmax = nullptr;
@@ -158,7 +159,7 @@ extern "C" int ent_destroy(ent_ctx *ctx) {
     if (!ctx) return ENT_EINVAL;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    cudaFree(ctx->counters); cudaFree(ctx->pool); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf); cudaFree(ctx->fbuf);
+    cudaFree(ctx->counters); cudaFree(ctx->pool); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf); cudaFree(ctx->fbuf); cudaFree(ctx->cbuf);
     cudaGetLastError();
     delete ctx;
     return ENT_OK;
@@ -579,6 +580,37 @@ extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *ou
         slot->cell = out->cell; slot->n = n; slot->stamp = ++ctx->sort_stamp; slot->wmax_valid = true; slot->counts_valid = true;
     }
     return ENT_OK;
+}
+
+// ---- N4: tag sort ------------------------------------------------------------------------------------
+extern "C" int ent_compact(ent_ctx *ctx, const ent_particles *in, ent_particles *out, int64_t *n_alive) {
+    ENTER();
+    int rc;
+    if ((rc = check_particles(ctx, in, "in", false)) || (rc = check_particles(ctx, out, "out", false))) return rc;
+    if (in->n != out->n) return fail(ctx, ENT_EINVAL, "in->n != out->n");
+    if (in->n > 0 && (in->cell == out->cell || in->w == out->w)) return fail(ctx, ENT_EINVAL, "ent_compact is out-of-place: in and out overlap");
+    if (!in->tag || !out->tag) return fail(ctx, ENT_EINVAL, "ent_compact needs tag arrays in both blocks");
+    const GridDev &g = ctx->g;
+    const long long n = in->n;
+    out->q = in->q; out->m = in->m;
+    forget_block(ctx, out->cell);
+    if (n == 0) { if (n_alive) CK(cudaMemsetAsync(n_alive, 0, sizeof(int64_t), ctx->stream)); return ENT_OK; }
+    const size_t slot = ((size_t)(n + 1) * 4 + 255) & ~(size_t)255;
+    const size_t nch = ((size_t)((n + SCAN_CHUNK - 1) / SCAN_CHUNK) * 4 + 255) & ~(size_t)255;
+    if ((rc = ensure(ctx, &ctx->cbuf, &ctx->cbuf_cap, 3 * slot + nch))) return rc;
+    int32_t *flag = (int32_t *)ctx->cbuf, *pos = (int32_t *)((char *)ctx->cbuf + slot), *copy = (int32_t *)((char *)ctx->cbuf + 2 * slot);
+    int32_t *chunk = (int32_t *)((char *)ctx->cbuf + 3 * slot);
+    const int nchunks = (int)((n + SCAN_CHUNK - 1) / SCAN_CHUNK);
+    compact_flag_kernel<<<nblk(n), TPB, 0, ctx->stream>>>(in->tag, n, flag);
+    if ((rc = launch_check(ctx, "compact_flag_kernel"))) return rc;
+    scan_reduce_kernel<<<nchunks, TPB, 0, ctx->stream>>>(flag, n, chunk);
+    if ((rc = launch_check(ctx, "scan_reduce_kernel"))) return rc;
+    scan_chunks_kernel<<<1, TPB, 0, ctx->stream>>>(chunk, nchunks);
+    if ((rc = launch_check(ctx, "scan_chunks_kernel"))) return rc;
+    scan_apply_kernel<<<nchunks, TPB, 0, ctx->stream>>>(flag, n, chunk, pos, copy);
+    if ((rc = launch_check(ctx, "scan_apply_kernel"))) return rc;
+    compact_scatter_kernel<<<nblk(n), TPB, 0, ctx->stream>>>(pos, pp(in), pp(out), n, g.D, g.kind != ENT_CART, (long long *)n_alive);
+    return launch_check(ctx, "compact_scatter_kernel");
 }
 
 // ---- fused step + re-bin: the timed entry point on Cartesian grids ----------------------------------------------

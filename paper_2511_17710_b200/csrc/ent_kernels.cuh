@@ -222,6 +222,28 @@ __global__ void __launch_bounds__(TPB) filter_pass_kernel(GridDev g, FilterGeom 
     dst.c[comp][(long long)(i + NG) + (long long)g.P[0] * ((long long)(j + NG) + (g.D == 3 ? (long long)g.P[1] * (k + NG) : 0))] = acc;
 }
 
+// ---- N4: tag sort: stable partition, alive particles first ----
+__global__ void __launch_bounds__(TPB) compact_flag_kernel(const uint8_t *tag, long long n, int32_t *flag) {
+    long long p = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (p < n) flag[p] = tag[p] != 0;
+}
+// pos[p] = number of alive particles before p (exclusive scan of the flags); pos[n] = number alive
+__global__ void __launch_bounds__(TPB) compact_scatter_kernel(const int32_t *pos, PartPtrs in, PartPtrs out, long long n, int D, int axisym,
+                                                              long long *n_alive) {
+    long long p = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (p >= n) return;
+    const long long na = pos[n];
+    if (p == 0 && n_alive) *n_alive = na;
+    const bool alive = in.tag[p] != 0;
+    const long long dst = alive ? (long long)pos[p] : na + (p - pos[p]);
+    out.cell[dst] = in.cell[p];
+    for (int a = 0; a < D; ++a) out.d[a][dst] = in.d[a][p];
+    for (int a = 0; a < 3; ++a) out.u[a][dst] = in.u[a][p];
+    out.w[dst] = in.w[p];
+    if (axisym) out.phi[dst] = in.phi[p];
+    out.tag[dst] = alive ? 1 : 0;
+}
+
 // ---- S10: counting sort by tile-major key ----
 template <int D>
 __global__ void __launch_bounds__(TPB) sort_hist_kernel(GridDev g, const int32_t *cell, long long n, int32_t *keys, int32_t *count) {

@@ -409,3 +409,39 @@ def test_vay_pusher_matches_oracle(env, name, impl, sort_first):
         orc.set_pusher(0)
     print(name, "vay", stats)
     assert all(st["max_u_rel"] <= P.MOM_TOL for st in stats.values())
+
+
+@pytest.mark.parametrize("name", ["ABS3", "C5/32", "C1"])
+def test_compact_matches_oracle(env, name):
+    """ent_compact (tag sort) after a few steps on grids that lose particles (and one that does not): bit-exact against the
+    oracle's stable partition of the same block -- every array, the tags and the count"""
+    bind, synth, ctx, orc = env
+    wl = _workloads(synth)[name]()
+    g = wl.grid
+    eg = P.grid_to_ent(bind, g)
+    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, 0)
+    bind.ent_set_grid(ctx, eg)
+    F = [f.cuda() for f in wl.fields]
+    J = bind.zeros_current(eg, "cuda")
+    pe = P.species_to_ent(bind, synth, g, wl.species[0], "cuda")
+    for _ in range(5):
+        bind.ent_step(ctx, F, pe, J, wl.dt)
+    out = pe.empty_like()
+    na = bind.ent_compact(ctx, pe, out)
+    torch.cuda.synchronize()
+    want, na_o = orc.compact(P.ent_to_orc(orc, g, pe))
+    assert int(na.item()) == na_o
+    if name != "C1":
+        assert 0 < na_o < pe.n
+    got = P.ent_to_orc(orc, g, out)
+    for a, b in zip(got.i + got.d + got.u + [got.w, got.tag] + ([got.phi] if got.phi is not None else []),
+                    want.i + want.d + want.u + [want.w, want.tag] + ([want.phi] if want.phi is not None else [])):
+        assert np.array_equal(a, b)
+    # the alive head of the compacted block is a block of its own: sort it and step it (n = number alive)
+    head = bind.Particles(cell=out.cell[:na_o], d=[t[:na_o] for t in out.d], u=[t[:na_o] for t in out.u], w=out.w[:na_o],
+                          phi=None if out.phi is None else out.phi[:na_o], tag=out.tag[:na_o], q=out.q, m=out.m)
+    srt = head.clone()
+    bind.ent_sort(ctx, head, srt, None)
+    bind.ent_step(ctx, F, srt, J, wl.dt)
+    torch.cuda.synchronize()
+    assert bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED) == 1
