@@ -353,27 +353,28 @@ extern "C" int ent_filter_current(ent_ctx *ctx, ent_current *J, int npasses, int
     const size_t slot = ((size_t)padded_size(g) * 4 + 255) & ~(size_t)255;
     if ((rc = ensure(ctx, &ctx->fbuf, &ctx->fbuf_cap, 3 * slot))) return rc;
     FilterGeom L;
-    long long maxpts = 1;
+    int nmax[3] = { 1, 1, 1 };
     for (int d = 0; d < 3; ++d) L.rule[d] = d < g.D ? g.bc[d] : ENT_PERIODIC;
-    for (int c = 0; c < 3; ++c) {
-        long long pts = 1;
+    for (int c = 0; c < 3; ++c)
         for (int d = 0; d < 3; ++d) {
             int n = 1;
             if (d < g.D) n = g.bc[d] == ENT_PERIODIC ? g.N[d] : (c == d ? g.N[d] : g.N[d] + 1);       // half-integer / integer lattice
-            L.n[c][d] = n; pts *= n;
+            L.n[c][d] = n;
+            if (n > nmax[d]) nmax[d] = n;
         }
-        if (pts > maxpts) maxpts = pts;
-    }
     CurrentPtrs a = cp(J), b;
     for (int c = 0; c < 3; ++c) b.c[c] = (float *)((char *)ctx->fbuf + slot * c);
+    const int nkc = (nmax[2] + FT_K - 1) / FT_K;
+    const dim3 fgrid((nmax[0] + FT_I - 1) / FT_I, (nmax[1] + FT_J - 1) / FT_J, 3 * nkc);
+    if (fgrid.y > 65535u || fgrid.z > 65535u) return fail(ctx, ENT_EUNSUPPORTED, "grid too large for the filter kernel");
     const int total = npasses ? npasses : 1;
     for (int pass = 0; pass < total; ++pass) {
         const bool last = pass == total - 1;
-        filter_pass_kernel<<<dim3(nblk(maxpts), 3), TPB, 0, ctx->stream>>>(g, L, (pass & 1) ? b : a, (pass & 1) ? a : b, npasses == 0, last && divide_by_sqrt_h);
+        filter_pass_kernel<<<fgrid, FT_I * FT_J, 0, ctx->stream>>>(g, L, (pass & 1) ? b : a, (pass & 1) ? a : b, npasses == 0 ? 1 : 0, last && divide_by_sqrt_h, nkc);
         if ((rc = launch_check(ctx, "filter_pass_kernel"))) return rc;
     }
     if (total & 1) {                                         // the result sits in the scratch arrays: copy the lattice points back
-        filter_pass_kernel<<<dim3(nblk(maxpts), 3), TPB, 0, ctx->stream>>>(g, L, b, a, 2, 0);
+        filter_pass_kernel<<<fgrid, FT_I * FT_J, 0, ctx->stream>>>(g, L, b, a, 2, 0, nkc);
         if ((rc = launch_check(ctx, "filter_pass_kernel"))) return rc;
     }
     return ENT_OK;

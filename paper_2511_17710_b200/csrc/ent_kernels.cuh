@@ -194,32 +194,83 @@ __device__ __forceinline__ float sqrt_h_at(const GridDev &g, double x1, double x
     const double eR = exp(g.Rmin + x1 * g.dR), T = x2 * g.dT, r = g.r0 + eR;
     return (float)((g.dR * eR) * (g.dT * dtheta_dT(g.vt, T) * r) * (r * sin(theta_of_T(g.vt, T))));
 }
-__global__ void __launch_bounds__(TPB) filter_pass_kernel(GridDev g, FilterGeom L, CurrentPtrs src, CurrentPtrs dst, int identity, int divide) {
-    const int comp = blockIdx.y;
+// One pass over a tile of FT_I x FT_J lattice points, marching along x3 (3D): the in-plane part of the stencil,
+// P_k = sum_{di,dj} w(di) w(dj) J(i+di, j+dj, k), comes from a shared-memory copy of plane k (one global load per point and plane,
+// halo columns included), and the thread keeps P_{k-1}, P_k, P_{k+1} in registers: out_k = P_{k-1}/4 + P_k/2 + P_{k+1}/4
+// (f = (1/2)^(D + |di| + |dj| + |dk|) = w(di) w(dj) w(dk), Eqs. 9-11).  In 2D out = P.  A tile whose whole neighbourhood lies inside
+// the lattice of a Cartesian grid loads without any boundary logic; the others go through filter_fetch.
+// mode 0: filter; 1: no convolution (scaling pass only); 2: copy.  blockIdx.z = component * nkc + chunk of FT_K planes.
+constexpr int FT_I = 32, FT_J = 8, FT_K = 32;
+__global__ void __launch_bounds__(FT_I * FT_J) filter_pass_kernel(GridDev g, FilterGeom L, CurrentPtrs src, CurrentPtrs dst, int mode, int divide, int nkc) {
+    __shared__ float s[2][FT_J + 2][FT_I + 4];
+    const int comp = blockIdx.z / nkc, kc = blockIdx.z - comp * nkc;
     const int n0 = L.n[comp][0], n1 = L.n[comp][1], n2 = L.n[comp][2];
-    const long long t = (long long)blockIdx.x * TPB + threadIdx.x;
-    if (t >= (long long)n0 * n1 * n2) return;
-    const int i = (int)(t % n0), j = (int)((t / n0) % n1), k = (int)(t / ((long long)n0 * n1));
+    const int i0 = blockIdx.x * FT_I, j0 = blockIdx.y * FT_J, k0 = kc * FT_K;
+    if (i0 >= n0 || j0 >= n1 || k0 >= n2) return;                    // the grid is sized for the largest lattice
+    const int k1 = min(k0 + FT_K, n2);
+    const int tid = threadIdx.x, tx = tid % FT_I, ty = tid / FT_I;
+    const int i = i0 + tx, j = j0 + ty;
+    const bool mine = i < n0 && j < n1;
     const float *A = src.c[comp];
+    float *O = dst.c[comp];
+    const long long P0 = g.P[0], P01 = g.D == 3 ? (long long)g.P[0] * g.P[1] : 0;
+    const long long at = (long long)(i + NG) + P0 * (j + NG) + (g.D == 3 ? P01 * NG : 0);     // (i, j, k = 0)
     const bool axis_node = filter_on_axis(g, L, comp, j);
-    float acc;
-    if (identity) acc = A[(long long)(i + NG) + (long long)g.P[0] * ((long long)(j + NG) + (g.D == 3 ? (long long)g.P[1] * (k + NG) : 0))];
-    else if (comp == 2 && axis_node) acc = 0.f;                                  // J^3(i, 0) = 0
-    else {
-        acc = 0.f;
-        const int kz = g.D == 3 ? 1 : 0;
-        for (int dk = -kz; dk <= kz; ++dk)
-#pragma unroll
-            for (int dj = -1; dj <= 1; ++dj) {
-                const float wjk = (dj ? 0.25f : 0.5f) * (g.D == 3 ? (dk ? 0.25f : 0.5f) : 1.0f);
-                const float a = filter_fetch(g, L, A, comp, i - 1, j + dj, k + dk), b = filter_fetch(g, L, A, comp, i, j + dj, k + dk),
-                            c = filter_fetch(g, L, A, comp, i + 1, j + dj, k + dk);
-                acc += wjk * (0.25f * a + 0.5f * b + 0.25f * c);                 // f = (1/2)^(D + |di| + |dj| + |dk|), Eqs. 9-11
+    float sh_here = 1.f;
+    if (divide && mine && !axis_node) sh_here = sqrt_h_at(g, i + (comp == 0 ? 0.5 : 0.0), j + (comp == 1 ? 0.5 : 0.0));
+    if (mode != 0) {
+        if (mine)
+            for (int k = k0; k < k1; ++k) {
+                float v = A[at + P01 * k];
+                if (divide && !axis_node) v /= sh_here;
+                O[at + P01 * k] = v;
             }
+        return;
     }
-    if (divide && !axis_node)
-        acc /= sqrt_h_at(g, i + (comp == 0 ? 0.5 : 0.0), j + (comp == 1 ? 0.5 : 0.0));
-    dst.c[comp][(long long)(i + NG) + (long long)g.P[0] * ((long long)(j + NG) + (g.D == 3 ? (long long)g.P[1] * (k + NG) : 0))] = acc;
+    const bool d3 = g.D == 3;
+    const bool interior = g.kind == ENT_CART && i0 >= 1 && i0 + FT_I + 1 <= n0 && j0 >= 1 && j0 + FT_J + 1 <= n1 && (!d3 || (k0 >= 1 && k1 + 1 <= n2));
+    auto load_plane = [&](int k, int buf) {
+        for (int e = tid; e < (FT_J + 2) * (FT_I + 2); e += FT_I * FT_J) {
+            const int jj = e / (FT_I + 2), ii = e - jj * (FT_I + 2);
+            const int q0 = i0 - 1 + ii, q1 = j0 - 1 + jj;
+            float v = 0.f;
+            if (interior) v = A[(long long)(q0 + NG) + P0 * (q1 + NG) + P01 * (k + NG)];
+            else if (q0 <= n0 && q1 <= n1) v = filter_fetch(g, L, A, comp, q0, q1, k);
+            s[buf][jj][ii] = v;
+        }
+    };
+    auto in_plane = [&](int buf) {
+        const float r0 = 0.25f * s[buf][ty][tx] + 0.5f * s[buf][ty][tx + 1] + 0.25f * s[buf][ty][tx + 2];
+        const float r1 = 0.25f * s[buf][ty + 1][tx] + 0.5f * s[buf][ty + 1][tx + 1] + 0.25f * s[buf][ty + 1][tx + 2];
+        const float r2 = 0.25f * s[buf][ty + 2][tx] + 0.5f * s[buf][ty + 2][tx + 1] + 0.25f * s[buf][ty + 2][tx + 2];
+        return 0.25f * r0 + 0.5f * r1 + 0.25f * r2;
+    };
+    auto emit = [&](int k, float acc) {
+        if (!mine) return;
+        if (comp == 2 && axis_node) acc = 0.f;                        // J^3(i, 0) = 0
+        if (divide && !axis_node) acc /= sh_here;
+        O[at + P01 * k] = acc;
+    };
+    if (!d3) {
+        load_plane(0, 0);
+        __syncthreads();
+        emit(0, in_plane(0));
+        return;
+    }
+    float Pm, Pc;
+    load_plane(k0 - 1, 0);
+    load_plane(k0, 1);
+    __syncthreads();
+    Pm = in_plane(0); Pc = in_plane(1);
+    for (int k = k0; k < k1; ++k) {
+        const int buf = (k - k0) & 1;                                // plane k + 1 overwrites the buffer of plane k - 1
+        __syncthreads();                                             // everyone is done reading that buffer
+        load_plane(k + 1, buf);
+        __syncthreads();
+        const float Pn = in_plane(buf);
+        emit(k, 0.25f * Pm + 0.5f * Pc + 0.25f * Pn);
+        Pm = Pc; Pc = Pn;
+    }
 }
 
 // ---- N4: tag sort: stable partition, alive particles first ----
