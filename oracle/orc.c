@@ -583,6 +583,149 @@ void orc_filter_current(const orc_grid *g, double *const J[3], int npasses, int 
 }
 
 /* ------------------------------------------------------------------------------------------
+ * N2  field solver, sub-steps 2, 10, 11 of the loop: discretized Faraday (Eq. A1) and Ampere (Eq. A2) laws
+ * on the Yee lattice in a diagonal metric (App. A), with the polar-axis treatment of Sec. 2.6.
+ * Arrays: six (three) padded planar DOUBLE arrays, contravariant components E^i, B^i at the positions of ent.h / P:1044-1053:
+ *   E^1 (i+1/2,j,k)  E^2 (i,j+1/2,k)  E^3 (i,j,k+1/2)   B^1 (i,j+1/2,k+1/2)  B^2 (i+1/2,j,k+1/2)  B^3 (i+1/2,j+1/2,k).
+ * Code coordinates are counted in cells, so Delta x^i = 1 in the difference operators of P:1060-1064 and the cell sizes live in
+ * h_ii.  Covariant components F_i = h_ii F^i, with h_ii and sqrt(h) evaluated at the component's own position.
+ * With (c, a, b) a cyclic permutation of (1, 2, 3):
+ *   A1:  B^c -= dt / sqrt(h) * { [E_b]_(+a) - [E_b] - ( [E_a]_(+b) - [E_a] ) }      at B^c's position (forward differences)
+ *   A2:  E^c += dt / sqrt(h) * { [B_b] - [B_b]_(-a) - ( [B_a] - [B_a]_(-b) ) - jc * conformal J^c }   (backward differences)
+ * (jc = 4 pi in Eq. A2; a parameter here because code units absorb it.)  A difference along a dimension the grid does not have
+ * (x3 in 2D) is zero.  Lattice of a component along dimension d: N_d points if d is PERIODIC (index wraps); otherwise N_d points
+ * for a component staggered along d and N_d + 1 (nodes 0 .. N_d) for one that is not.
+ * Readings: the left side of A2 is garbled in the source ("Delta_{n+1}^{n+1}"): it is (E^(n+1) - E^(n)) / dt.
+ * Faraday never reaches beyond the E lattices.  Ampere does, on a non-periodic side: there the E components tangential to that
+ * face (the ones whose stencil needs a B value outside the lattice) are NOT advanced -- they are the caller's boundary condition
+ * (the paper's conductor / absorbing layers are problem-generator code).  Polar axis (AXIS in x2, j = 0 and j = N_2):
+ *   Eq. 12:  E^3(i, j) = 0 and B^2(i+1/2, j) = 0 are imposed and their update skipped;
+ *   Eq. 13:  E^1(i+1/2, 0) += dt * { B_3(i+1/2, 1/2) - (jc/2) conformal J^1(i+1/2, 0) } / A(i+1/2), and the mirror image at
+ *            j = N_2: E^1(i+1/2, N_2) += dt * { -B_3(i+1/2, N_2 - 1/2) - (jc/2) J^1(i+1/2, N_2) } / A(i+1/2)  (integral of A2 over
+ *            the half cell next to the axis, where B_3 = h_33 B^3 vanishes on the axis);
+ *   A(x1) = integral_0^(1/2) sqrt(h) dx2, in the closed forms the paper prints:
+ *            SPH r^2 dr (1 - cos(dtheta/2));  QSPH (r0 + e^R)^2 e^R dR (1 - cos(theta(dT/2))).  (The line that defines A carries a
+ *            factor 2 pi that its own closed forms do not have; the closed forms are the ones consistent with the B_3 term.)
+ * ------------------------------------------------------------------------------------------ */
+static int fld_stag(int comp6, int d) { int c = comp6 % 3; return comp6 < 3 ? (d == c) : (d != c); }
+static int fld_extent(const orc_grid *g, int comp6, int d) {
+    if (d >= g->D) return 1;
+    if (g->bc[d] == ORC_PERIODIC) return g->N[d];
+    return fld_stag(comp6, d) ? g->N[d] : g->N[d] + 1;
+}
+/* covariant component h_cc F^c of field component comp6 at lattice index q (periodic wrap); *ok = 0 if q lies outside the lattice */
+static double fld_cov(const orc_grid *g, const double *A, int comp6, const int qin[3], int *ok) {
+    int q[3] = { qin[0], qin[1], qin[2] };
+    for (int d = 0; d < g->D; ++d) {
+        int n = fld_extent(g, comp6, d);
+        if (q[d] >= 0 && q[d] < n) continue;
+        if (g->bc[d] == ORC_PERIODIC) { q[d] = ((q[d] % n) + n) % n; continue; }
+        *ok = 0;
+        return 0.0;
+    }
+    double x[3], h[3];
+    for (int d = 0; d < 3; ++d) x[d] = d < g->D ? q[d] + (fld_stag(comp6, d) ? 0.5 : 0.0) : 0.0;
+    orc_metric_h(g, x, h);
+    return h[comp6 % 3] * A[pidx(g, q[0], q[1], g->D == 3 ? q[2] : 0)];
+}
+static double sqrt_h_at(const orc_grid *g, int comp6, const int q[3]) {
+    double x[3], h[3];
+    for (int d = 0; d < 3; ++d) x[d] = d < g->D ? q[d] + (fld_stag(comp6, d) ? 0.5 : 0.0) : 0.0;
+    orc_metric_h(g, x, h);
+    return sqrt(h[0] * h[1] * h[2]);
+}
+static int axis_dim(const orc_grid *g) { for (int d = 0; d < g->D; ++d) if (g->bc[d] == ORC_AXIS) return d; return -1; }
+
+/* A(x1) of Eq. 13, closed forms of P:372-382 */
+double orc_axis_area(const orc_grid *g, double x1) {
+    if (g->kind == ORC_SPH) {
+        double dr = cell_size(g, 0), dth = PI / (double)g->N[1], r = g->xmin[0] + x1 * dr;
+        return r * r * dr * (1.0 - cos(0.5 * dth));
+    }
+    double dR = qs_dR(g), dT = qs_dT(g), eR = exp(qs_Rmin(g) + x1 * dR), vt = g->vartheta;
+    double dtt = 0.5 * dT + vt * dT * (1.0 - dT / PI) * (1.0 - dT / (2.0 * PI));              /* = theta(dT / 2) */
+    return (g->r0 + eR) * (g->r0 + eR) * eR * dR * (1.0 - cos(dtt));
+}
+
+void orc_faraday(const orc_grid *g, const double *const E[3], double *const B[3], double dt) {
+    const int ax = axis_dim(g);
+    for (int c = 0; c < 3; ++c) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3, cB = 3 + c;
+        const int n[3] = { fld_extent(g, cB, 0), fld_extent(g, cB, 1), fld_extent(g, cB, 2) };
+        for (int k = 0; k < n[2]; ++k)
+            for (int j = 0; j < n[1]; ++j)
+                for (int i = 0; i < n[0]; ++i) {
+                    const int q[3] = { i, j, k };
+                    const int64_t at = pidx(g, i, j, g->D == 3 ? k : 0);
+                    if (ax >= 0 && c == 1 && (q[ax] == 0 || q[ax] == g->N[ax])) { B[c][at] = 0.0; continue; }     /* Eq. 12 */
+                    int ok = 1;
+                    double curl = 0.0;
+                    if (a < g->D) { int qp[3] = { i, j, k }; qp[a] += 1; curl += fld_cov(g, E[b], b, qp, &ok) - fld_cov(g, E[b], b, q, &ok); }
+                    if (b < g->D) { int qp[3] = { i, j, k }; qp[b] += 1; curl -= fld_cov(g, E[a], a, qp, &ok) - fld_cov(g, E[a], a, q, &ok); }
+                    if (!ok) continue;                                    /* cannot happen: A1 stays inside the E lattices */
+                    B[c][at] -= dt * curl / sqrt_h_at(g, cB, q);          /* Eq. A1 */
+                }
+    }
+}
+
+void orc_ampere(const orc_grid *g, double *const E[3], const double *const B[3], const double *const J[3], double dt, double jc) {
+    const int ax = axis_dim(g);
+    for (int c = 0; c < 3; ++c) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
+        const int n[3] = { fld_extent(g, c, 0), fld_extent(g, c, 1), fld_extent(g, c, 2) };
+        for (int k = 0; k < n[2]; ++k)
+            for (int j = 0; j < n[1]; ++j)
+                for (int i = 0; i < n[0]; ++i) {
+                    const int q[3] = { i, j, k };
+                    const int64_t at = pidx(g, i, j, g->D == 3 ? k : 0);
+                    const double Jc = J ? J[c][at] : 0.0;
+                    if (ax >= 0 && c != ax && (q[ax] == 0 || q[ax] == g->N[ax])) {          /* a point on the polar axis */
+                        if (c == 2) { E[c][at] = 0.0; continue; }                           /* Eq. 12 */
+                        /* c == 0: Eq. 13 */
+                        int ok = 1, qb[3] = { i, j, k };
+                        double sgn = 1.0;
+                        if (q[ax] != 0) { qb[ax] = g->N[ax] - 1; sgn = -1.0; }              /* B^3 at (i+1/2, N_2 - 1/2) */
+                        double B3 = fld_cov(g, B[2], 5, qb, &ok);
+                        E[c][at] += dt * (sgn * B3 - 0.5 * jc * Jc) / orc_axis_area(g, i + 0.5);
+                        continue;
+                    }
+                    int ok = 1;
+                    double curl = 0.0;
+                    if (a < g->D) { int qm[3] = { i, j, k }; qm[a] -= 1; curl += fld_cov(g, B[b], 3 + b, q, &ok) - fld_cov(g, B[b], 3 + b, qm, &ok); }
+                    if (b < g->D) { int qm[3] = { i, j, k }; qm[b] -= 1; curl -= fld_cov(g, B[a], 3 + a, q, &ok) - fld_cov(g, B[a], 3 + a, qm, &ok); }
+                    if (!ok) continue;                                    /* tangential E on a non-periodic face: the caller's boundary condition */
+                    E[c][at] += dt * (curl - jc * Jc) / sqrt_h_at(g, c, q);                 /* Eq. A2 */
+                }
+    }
+}
+
+/* Ghost layers of the six field arrays, as the gather expects them (harness convention, reading G10): PERIODIC dimension: the
+ * periodic image; AXIS: mirror image about the axis, E^1 / B^1 even, the theta- and phi-components odd; ABSORB: left alone. */
+void orc_fill_field_ghosts(const orc_grid *g, double *const F[6]) {
+    for (int c6 = 0; c6 < 6; ++c6)
+        for (int d = 0; d < g->D; ++d) {
+            if (g->bc[d] == ORC_ABSORB) continue;
+            const int n = fld_extent(g, c6, d), a = (d + 1) % 3, b = (d + 2) % 3;
+            const int lo_a = a < g->D ? -NG : 0, hi_a = a < g->D ? g->N[a] + NG : 1, lo_b = b < g->D ? -NG : 0, hi_b = b < g->D ? g->N[b] + NG : 1;
+            for (int ib = lo_b; ib < hi_b; ++ib)
+                for (int ia = lo_a; ia < hi_a; ++ia)
+                    for (int gi = -NG; gi < g->N[d] + NG; ++gi) {
+                        if (gi >= 0 && gi < n) continue;
+                        int src; double sign = 1.0;
+                        if (g->bc[d] == ORC_PERIODIC) src = ((gi % n) + n) % n;
+                        else {                                          /* AXIS */
+                            if (fld_stag(c6, d)) src = gi < 0 ? -1 - gi : 2 * n - 1 - gi;
+                            else src = gi < 0 ? -gi : 2 * (n - 1) - gi;
+                            if (c6 % 3 != 0) sign = -1.0;
+                        }
+                        int q[3], s[3];
+                        q[d] = gi; q[a] = ia; q[b] = ib; s[d] = src; s[a] = ia; s[b] = ib;
+                        F[c6][pidx(g, q[0], q[1], g->D == 3 ? q[2] : 0)] = sign * F[c6][pidx(g, s[0], s[1], g->D == 3 ? s[2] : 0)];
+                    }
+        }
+}
+
+/* ------------------------------------------------------------------------------------------
  * Eq. 6 checker.  Conformal nodal charge (no 1/sqrt(h)):  rho[n] = sum_p q w prod_d omega(delta_d, s_d)
  * ------------------------------------------------------------------------------------------ */
 void orc_charge_density(const orc_grid *g, const orc_particles *p, const int8_t *mask, double q, double *rho) {

@@ -13,6 +13,7 @@
  *   step 6  move          P:147-149          -> orc_gather_push (absolute coordinates, textbook way)
  *   step 7  back-map      P:151-153, App. B -> orc_cart_to_code
  *   step 8  deposit       P:105-109, P:155-157, P:575 -> orc_deposit (+ orc_fold_current)
+ *   steps 2, 10, 11  field solver  P:127-129, App. A, Sec. 2.6 -> orc_faraday, orc_ampere
  * plus the discrete continuity checker of Eq. 6 and a sort checker.
  * Readings of silent / garbled passages are those of SURVEY.md section 8(c) (G1..G19), listed in DESIGN.md.
  *
@@ -100,6 +101,15 @@ void orc_fold_scalar(const orc_grid *g, double *rho);
  *      then (divide != 0) J^i = conformal J^i / sqrt(h) at each component's own position.  In place; J must already be
  *      folded (orc_fold_current).  Ghost layers of the arrays are not touched. ---- */
 void orc_filter_current(const orc_grid *g, double *const J[3], int npasses, int divide);
+
+/* ---- N2 field solver (sub-steps 2, 10, 11; Eqs. A1, A2, 12, 13) on padded planar DOUBLE
+ *      arrays of contravariant components.  orc_faraday: B -= dt curl(h E) / sqrt(h) (the loop calls it twice with dt/2);
+ *      orc_ampere: E += dt (curl(h B) - jc conformal J) / sqrt(h), jc = 4 pi in Eq. A2, J may be NULL; axis rules inside.
+ *      orc_fill_field_ghosts: periodic / axis-mirror ghost layers as the gather wants them (reading G10). ---- */
+void   orc_faraday(const orc_grid *g, const double *const E[3], double *const B[3], double dt);
+void   orc_ampere(const orc_grid *g, double *const E[3], const double *const B[3], const double *const J[3], double dt, double jc);
+double orc_axis_area(const orc_grid *g, double x1);                        /* A(x1) of Eq. 13 */
+void   orc_fill_field_ghosts(const orc_grid *g, double *const F[6]);
 
 /* fused: gather_push then deposit (no fold) */
 int orc_step(const orc_grid *g, const float *const F[6], orc_particles *p, double *const J[3],

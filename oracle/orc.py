@@ -79,6 +79,10 @@ def lib():
         L.orc_fold_current.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p)]
         L.orc_fold_scalar.argtypes = [C.POINTER(_Grid), C.c_void_p]
         L.orc_filter_current.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p), C.c_int, C.c_int]
+        L.orc_faraday.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_double]
+        L.orc_ampere.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_void_p, C.c_double, C.c_double]
+        L.orc_axis_area.restype = C.c_double; L.orc_axis_area.argtypes = [C.POINTER(_Grid), C.c_double]
+        L.orc_fill_field_ghosts.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p)]
         L.orc_step.restype = C.c_int
         L.orc_step.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p), C.POINTER(_Particles), C.POINTER(C.c_void_p),
                                C.c_double, C.c_double, C.c_double]
@@ -296,6 +300,32 @@ def fold_scalar(g: Grid, rho) -> None:
 def filter_current(g: Grid, J, npasses: int, divide: bool = False) -> None:
     """step 9: digital filter passes (Eqs. 9-11) in place, then optionally J = conformal J / sqrt(h)"""
     lib().orc_filter_current(C.byref(g.c()), _jptrs(J), int(npasses), 1 if divide else 0)
+
+
+def _dptrs(A, n):
+    arr = (C.c_void_p * n)()
+    for c in range(n):
+        assert A[c].dtype == np.float64 and A[c].flags.c_contiguous
+        arr[c] = A[c].ctypes.data
+    return arr
+
+
+def faraday(g: Grid, E, B, dt: float) -> None:
+    """Eq. A1: B -= dt curl(h E) / sqrt(h), in place on the three float64 arrays of B; Eq. 12 on the axis"""
+    lib().orc_faraday(C.byref(g.c()), _dptrs(E, 3), _dptrs(B, 3), float(dt))
+
+
+def ampere(g: Grid, E, B, J, dt: float, jc: float) -> None:
+    """Eq. A2: E += dt (curl(h B) - jc conformal J) / sqrt(h), in place on E; Eqs. 12-13 on the axis; J may be None"""
+    lib().orc_ampere(C.byref(g.c()), _dptrs(E, 3), _dptrs(B, 3), None if J is None else _dptrs(J, 3), float(dt), float(jc))
+
+
+def axis_area(g: Grid, x1: float) -> float:
+    return lib().orc_axis_area(C.byref(g.c()), float(x1))
+
+
+def fill_field_ghosts(g: Grid, F) -> None:
+    lib().orc_fill_field_ghosts(C.byref(g.c()), _dptrs(F, 6))
 
 
 def step(g: Grid, F, p: Particles, J, q: float, m: float, dt: float) -> None:

@@ -62,6 +62,30 @@ MUTANTS = [
      "{ q[d] = q[d] < 0 ? -1 - q[d] : 2 * n - 1 - q[d]; sign = -sign; }",
      "{ q[d] = q[d] < 0 ? -1 - q[d] : 2 * n - 1 - q[d]; }",
      "tests/test_oracle_pins_filter.py::test_axis_rules_hand_example"),
+    ("ampere: current term with the wrong sign (Eq. A2)",
+     "E[c][at] += dt * (curl - jc * Jc) / sqrt_h_at(g, c, q);",
+     "E[c][at] += dt * (curl + jc * Jc) / sqrt_h_at(g, c, q);",
+     "tests/test_oracle_pins_fields.py::test_gauss_law_is_carried_by_the_deposited_current"),
+    ("faraday: sign of Eq. A1",
+     "B[c][at] -= dt * curl / sqrt_h_at(g, cB, q);",
+     "B[c][at] += dt * curl / sqrt_h_at(g, cB, q);",
+     "tests/test_oracle_pins_fields.py::test_vacuum_plane_wave_follows_the_yee_dispersion_relation_exactly"),
+    ("field solver: contravariant instead of covariant components under the curl (h_ii dropped, P:1066)",
+     "return h[comp6 % 3] * A[pidx(g, q[0], q[1], g->D == 3 ? q[2] : 0)];",
+     "return A[pidx(g, q[0], q[1], g->D == 3 ? q[2] : 0)];",
+     "tests/test_oracle_pins_fields.py::test_vacuum_plane_wave_follows_the_yee_dispersion_relation_exactly"),
+    ("ampere, Eq. 13: full 4 pi instead of 2 pi on the axis current",
+     "E[c][at] += dt * (sgn * B3 - 0.5 * jc * Jc) / orc_axis_area(g, i + 0.5);",
+     "E[c][at] += dt * (sgn * B3 - jc * Jc) / orc_axis_area(g, i + 0.5);",
+     "tests/test_oracle_pins_fields.py::test_axis_rules_eq12_and_eq13_hand_values"),
+    ("ampere, Eq. 13: south pole without the mirror sign",
+     "if (q[ax] != 0) { qb[ax] = g->N[ax] - 1; sgn = -1.0; }",
+     "if (q[ax] != 0) { qb[ax] = g->N[ax] - 1; sgn = 1.0; }",
+     "tests/test_oracle_pins_fields.py::test_axis_rules_eq12_and_eq13_hand_values"),
+    ("Eq. 13: A with the stray factor 2 pi of its defining line (P:370)",
+     "return r * r * dr * (1.0 - cos(0.5 * dth));",
+     "return 2.0 * PI * r * r * dr * (1.0 - cos(0.5 * dth));",
+     "tests/test_oracle_pins_fields.py::test_curvilinear_curl_converges_to_the_textbook_curl_at_second_order"),
     # mutants the round-1 pins already killed, kept so that the list documents them
     ("deposit: 3D weights without the D_a D_b / 12 term (reading G7)",
      "+ sigma * Dv[a] * Dv[b] / 12.0",
