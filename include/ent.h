@@ -196,6 +196,29 @@ int ent_compact(ent_ctx *ctx, const ent_particles *in, ent_particles *out, int64
  * current arrays is allocated in the ctx on first use (may synchronise). */
 int ent_filter_current(ent_ctx *ctx, ent_current *J, int npasses, int divide_by_sqrt_h);
 
+/* ---- field solver: sub-steps 2, 10, 11 of the loop --------------------------------------------------
+ * Six padded planar fp32 arrays as in ent_fields, but WRITTEN by the library (device pointers, 16-byte aligned). */
+typedef struct { float *comp[6]; } ent_fields_rw;
+
+/* ent_faraday: Eq. A1: B^c -= dt / sqrt(h) * { E_b(+a) - E_b - (E_a(+b) - E_a) } at every lattice point of B^c, (c, a, b)
+ * cyclic, E_i = h_ii E^i covariant, h_ii and sqrt(h) at the component's own Yee position, code coordinates in cells
+ * (Delta x^i = 1).  The loop calls it twice per step with dt/2 (sub-steps 2 and 10).  Polar axis (Eq. 12): B^2 = 0 at
+ * j = 0 and j = N_2, not advanced.  Only B is written, only on its lattice (periodic dimension: indices 0 .. N-1 with wrap-around
+ * reads; otherwise N points for a component staggered along that dimension, N + 1 for the others); ghost layers are not touched. */
+int ent_faraday(ent_ctx *ctx, ent_fields_rw *EB, float dt);
+
+/* ent_ampere: Eq. A2: E^c += dt / sqrt(h) * { B_b - B_b(-a) - (B_a - B_a(-b)) - j_coeff * conformal J^c }.  j_coeff is the
+ * 4 pi of Eq. A2 (a parameter: code units absorb it); J = the conformal currents of ent_deposit / ent_step after ent_fold_current
+ * and ent_filter_current(.., divide_by_sqrt_h = 0), or NULL (vacuum).  On a non-periodic (ABSORB) face the E components tangential
+ * to it are not advanced: they are the caller's boundary condition.  Polar axis: E^3 = 0 (Eq. 12); E^1 at j = 0 is advanced with the
+ * integrated form, Eq. 13: E^1 += dt * { B_3(i+1/2, 1/2) - (j_coeff/2) J^1(i+1/2, 0) } / A(i+1/2), A the closed forms of
+ * P:372-382, and its mirror image at j = N_2.  Only E is written, on its lattice. */
+int ent_ampere(ent_ctx *ctx, ent_fields_rw *EB, const ent_current *J, float dt, float j_coeff);
+
+/* Ghost layers of the six arrays as the gather of ent_step / ent_gather_push expects them: PERIODIC dimension: the periodic image;
+ * AXIS: the mirror image about the axis, E^1 and B^1 even, the theta- and phi-components odd; ABSORB: left to the caller. */
+int ent_fill_field_ghosts(ent_ctx *ctx, ent_fields_rw *EB);
+
 /* ---- host-buffer variant (end-to-end measurement) --------------------------------------------------------------
  * Every pointer in EB, p and J is a HOST pointer (pinned memory recommended).  Copies E,B and the particle block to ctx-owned
  * device staging, zeroes the device J, sorts the block by tile (ent_sort, full form), runs `nsteps` x ent_step on the sorted

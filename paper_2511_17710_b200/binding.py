@@ -22,7 +22,7 @@ OPT_STEP_IMPL, OPT_TILE_1, OPT_TILE_2, OPT_TILE_3, OPT_SORT_MODE, OPT_CURV_FP64,
  STAT_SCRATCH_BYTES, STAT_LAST_STEP_TILED, STAT_LAST_SORT_REBIN, STAT_SLOT_ERRORS, STAT_CARRIES, STAT_GLOBAL_ADDS) = range(1, 15)
 
 SYMBOLS = ["ent_create", "ent_destroy", "ent_last_error", "ent_set_grid", "ent_gather_push", "ent_deposit", "ent_sort",
-           "ent_step", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_filter_current", "ent_compact", "ent_step_host", "ent_set_option", "ent_get_stat", "ent_version"]
+           "ent_step", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_filter_current", "ent_faraday", "ent_ampere", "ent_fill_field_ghosts", "ent_compact", "ent_step_host", "ent_set_option", "ent_get_stat", "ent_version"]
 
 
 class EntError(RuntimeError):
@@ -78,6 +78,9 @@ def lib():
         L.ent_zero_current.argtypes = [vp, C.POINTER(_Current)]
         L.ent_fold_current.argtypes = [vp, C.POINTER(_Current)]
         L.ent_filter_current.argtypes = [vp, C.POINTER(_Current), C.c_int, C.c_int]
+        L.ent_faraday.argtypes = [vp, C.POINTER(_Fields), C.c_float]
+        L.ent_ampere.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Current), C.c_float, C.c_float]
+        L.ent_fill_field_ghosts.argtypes = [vp, C.POINTER(_Fields)]
         L.ent_compact.argtypes = [vp, C.POINTER(_Particles), C.POINTER(_Particles), vp]
         L.ent_step_host.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Current), C.c_float, C.c_int,
                                     C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
@@ -308,6 +311,18 @@ def ent_compact(ctx: Ctx, pin: Particles, pout: Particles) -> torch.Tensor:
 
 def ent_filter_current(ctx: Ctx, J, npasses: int, divide_by_sqrt_h: bool = False) -> None:
     ctx._ck(lib().ent_filter_current(ctx._h, C.byref(_current(J)), int(npasses), 1 if divide_by_sqrt_h else 0))
+
+
+def ent_faraday(ctx: Ctx, EB, dt: float) -> None:
+    ctx._ck(lib().ent_faraday(ctx._h, C.byref(_fields(EB)), dt))
+
+
+def ent_ampere(ctx: Ctx, EB, J, dt: float, j_coeff: float) -> None:
+    ctx._ck(lib().ent_ampere(ctx._h, C.byref(_fields(EB)), None if J is None else C.byref(_current(J)), dt, j_coeff))
+
+
+def ent_fill_field_ghosts(ctx: Ctx, EB) -> None:
+    ctx._ck(lib().ent_fill_field_ghosts(ctx._h, C.byref(_fields(EB))))
 
 
 def ent_step_host(ctx: Ctx, EB, p: Particles, J, dt: float, nsteps: int = 1):

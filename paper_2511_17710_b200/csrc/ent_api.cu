@@ -9,6 +9,7 @@
 #include "ent_kernels.cuh"
 #include "ent_tiled_axisym.cuh"
 #include "ent_sorted.cuh"
+#include "ent_fields.cuh"
 
 using namespace ent;
 
@@ -376,6 +377,78 @@ extern "C" int ent_filter_current(ent_ctx *ctx, ent_current *J, int npasses, int
     if (total & 1) {                                         // the result sits in the scratch arrays: copy the lattice points back
         filter_pass_kernel<<<fgrid, FT_I * FT_J, 0, ctx->stream>>>(g, L, b, a, 2, 0, nkc);
         if ((rc = launch_check(ctx, "filter_pass_kernel"))) return rc;
+    }
+    return ENT_OK;
+}
+
+// ---- N2: field solver (sub-steps 2, 10, 11; Eqs. A1, A2, 12, 13) and the ghost fill of the field arrays ----
+static int check_fields_rw(ent_ctx *ctx, const ent_fields_rw *F) {
+    if (!F) return fail(ctx, ENT_EINVAL, "fields struct is NULL");
+    for (int c = 0; c < 6; ++c) if (!F->comp[c] || !al16(F->comp[c])) return fail(ctx, ENT_EINVAL, "field component %d NULL or misaligned", c);
+    return ENT_OK;
+}
+static SolverGeom solver_geom(const GridDev &g) {
+    SolverGeom L;
+    L.axis = -1;
+    for (int d = 0; d < 3; ++d) { L.nmax[d] = 1; if (d < g.D && g.bc[d] == ENT_AXIS) L.axis = d; }
+    for (int c6 = 0; c6 < 6; ++c6)
+        for (int d = 0; d < 3; ++d) {
+            int n = 1;
+            if (d < g.D) n = g.bc[d] == ENT_PERIODIC ? g.N[d] : (fld_stag(c6, d) ? g.N[d] : g.N[d] + 1);
+            L.n[c6][d] = n;
+            if (n > L.nmax[d]) L.nmax[d] = n;
+        }
+    const double sh = (double)g.dx[0] * g.dx[1] * g.dx[2];
+    for (int c = 0; c < 3; ++c) L.cov[c] = g.dx[c] * g.dx[c];
+    L.inv_sqrt_h = (float)(1.0 / sh);
+    return L;
+}
+static FieldRW frw(const ent_fields_rw *F) { FieldRW r; for (int c = 0; c < 6; ++c) r.c[c] = F->comp[c]; return r; }
+static int solver_grid(ent_ctx *ctx, const SolverGeom &L, dim3 *grid) {
+    *grid = dim3((unsigned)((L.nmax[0] + TPB - 1) / TPB), (unsigned)L.nmax[1], (unsigned)(3 * L.nmax[2]));
+    if (grid->y > 65535u || grid->z > 65535u) return fail(ctx, ENT_EUNSUPPORTED, "grid too large for the field-solver kernels");
+    return ENT_OK;
+}
+
+extern "C" int ent_faraday(ent_ctx *ctx, ent_fields_rw *EB, float dt) {
+    ENTER();
+    int rc;
+    if ((rc = check_fields_rw(ctx, EB))) return rc;
+    const GridDev &g = ctx->g;
+    const SolverGeom L = solver_geom(g);
+    dim3 grid;
+    if ((rc = solver_grid(ctx, L, &grid))) return rc;
+    if (g.kind == ENT_CART) faraday_kernel<true><<<grid, TPB, 0, ctx->stream>>>(g, L, frw(EB), dt);
+    else faraday_kernel<false><<<grid, TPB, 0, ctx->stream>>>(g, L, frw(EB), dt);
+    return launch_check(ctx, "faraday_kernel");
+}
+
+extern "C" int ent_ampere(ent_ctx *ctx, ent_fields_rw *EB, const ent_current *J, float dt, float j_coeff) {
+    ENTER();
+    int rc;
+    if ((rc = check_fields_rw(ctx, EB))) return rc;
+    if (J && (rc = check_current(ctx, J))) return rc;
+    const GridDev &g = ctx->g;
+    const SolverGeom L = solver_geom(g);
+    dim3 grid;
+    if ((rc = solver_grid(ctx, L, &grid))) return rc;
+    CurrentPtrs j; for (int c = 0; c < 3; ++c) j.c[c] = J ? J->comp[c] : nullptr;
+    if (g.kind == ENT_CART) ampere_kernel<true><<<grid, TPB, 0, ctx->stream>>>(g, L, frw(EB), j, J != nullptr, dt, j_coeff);
+    else ampere_kernel<false><<<grid, TPB, 0, ctx->stream>>>(g, L, frw(EB), j, J != nullptr, dt, j_coeff);
+    return launch_check(ctx, "ampere_kernel");
+}
+
+extern "C" int ent_fill_field_ghosts(ent_ctx *ctx, ent_fields_rw *EB) {
+    ENTER();
+    int rc;
+    if ((rc = check_fields_rw(ctx, EB))) return rc;
+    const GridDev &g = ctx->g;
+    const SolverGeom L = solver_geom(g);
+    for (int d = 0; d < g.D; ++d) {
+        if (g.bc[d] == ENT_ABSORB) continue;
+        const long long nthreads = (long long)g.P[(d + 1) % 3] * g.P[(d + 2) % 3] * 2 * NG;
+        field_ghost_kernel<<<dim3(nblk(nthreads), 6), TPB, 0, ctx->stream>>>(g, L, frw(EB), d);
+        if ((rc = launch_check(ctx, "field_ghost_kernel"))) return rc;
     }
     return ENT_OK;
 }
