@@ -303,6 +303,20 @@ def measure(args, name, env, want_e2e):
     out["current_filter"] = {"passes": npass, "ms": f_ms, "algorithmic_bytes": f_bytes, "achieved_gbs": f_bytes / (f_ms * 1e-3) / 1e9,
                              "frac_of_hbm_peak": f_bytes / (f_ms * 1e-3) / 1e9 / peak, "note": "not part of `value` (sub-steps 3-8 only)"}
 
+    # ---- sub-steps 2/10 and 11: the Yee field solver on a copy of the fields (36 / 48 B per cell)
+    Fc = [f.clone() for f in F]
+    bind.ent_faraday(ctx, Fc, 0.5 * wl.dt); bind.ent_ampere(ctx, Fc, J, wl.dt, 1e-6)
+    fa_ev, am_ev = [], []
+    for _ in range(5):
+        timed(lambda: bind.ent_faraday(ctx, Fc, 0.5 * wl.dt), fa_ev)
+        timed(lambda: bind.ent_ampere(ctx, Fc, J, wl.dt, 1e-6), am_ev)
+    torch.cuda.synchronize()
+    fa_ms, am_ms = mean(fa_ev), mean(am_ev)
+    out["field_solver"] = {"faraday_ms": fa_ms, "ampere_ms": am_ms, "faraday_gbs": 36.0 * ncell / (fa_ms * 1e-3) / 1e9,
+                           "ampere_gbs": 48.0 * ncell / (am_ms * 1e-3) / 1e9, "frac_of_hbm_peak": [36.0 * ncell / (fa_ms * 1e-3) / 1e9 / peak,
+                           48.0 * ncell / (am_ms * 1e-3) / 1e9 / peak], "note": "not part of `value`; algorithmic bytes 36 / 48 B per cell"}
+    del Fc
+
     # ---- end to end through the host-buffer C-ABI call: H2D of the step's inputs and D2H of its results inside ----
     if want_e2e:
         hp = [p.to("cpu", pin=True) for p in parts]
@@ -368,6 +382,7 @@ def run_ours(args):
     if "e2e" in m:
         line["e2e"] = m["e2e"]
     line["current_filter"] = m["current_filter"]
+    line["field_solver"] = m["field_solver"]
     if args.workload is None and not args.no_per_config and world == 1:
         per = []
         for name in ("C4", "C4s", "C5", "C2", "C1"):

@@ -286,52 +286,9 @@ step_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
                 if (edge) edge_deposit<D, SortedArgs>(A, iold[0], iold[1], iold[2], a0[0], a0[1], a0[2], di[0], di[1], di[2], d[0], d[1], d[2], u[0], u[1], u[2], qw);
                 else {
                     // ---- S7 deposit into the shared-memory J tile (Eq. 6); node (b) of the box = element b of the J tile
-                    const float Q = qw * A.inv_dt * T.Sc;                                // in fixed-point units
-                    // 3D: one straight segment unless a face is crossed.  2D: always the two segments of P:575 (the out-of-plane
-                    // weights of two half segments do not sum to those of the whole one)
-                    const bool cross = (D == 2) || (di[0] | di[1] | di[2]) != 0;
-                    float s[3], e[3], r[3];
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) {
-                        if (a < D) {
-                            const float bnew = (float)di[a] + d[a];                      // new position in the old cell's frame
-                            r[a] = di[a] == 0 ? (cross ? 0.5f * (a0[a] + bnew) : bnew) : (di[a] > 0 ? 1.0f : 0.0f);
-                            s[a] = a0[a]; e[a] = r[a];
-                        } else { r[a] = s[a] = e[a] = 0.f; }
-                    }
-                    int base = b[0] + G::JX * (b[1] + G::JY * b[2]);
-                    const int dbase = di[0] + G::JX * (di[1] + G::JY * di[2]);
-                    float hv = 0.f;
-                    if (D == 2) hv = 0.5f * qw * T.Sc * (u[2] * ig);                     // out-of-plane rate per segment (G8), h33 = 1
-                    const int nseg = cross ? 2 : 1;
-#pragma unroll 1
-                    for (int seg = 0; seg < nseg; ++seg) {
-                        float Dv[3], W[3];
-#pragma unroll
-                        for (int a = 0; a < 3; ++a) { Dv[a] = e[a] - s[a]; W[a] = 0.5f * (e[a] + s[a]); }
-                        if (D == 3) {
-                            const int st[3] = { 1, G::JX, G::JX * G::JY };
-#pragma unroll
-                            for (int comp = 0; comp < 3; ++comp) {
-                                const int a = (comp + 1) % 3, bb = (comp + 2) % 3;
-                                const float QD = Q * Dv[comp];
-                                const float ta = QD * W[a], tb = QD * W[bb];
-                                const float v11 = fmaf(ta, W[bb], QD * (Dv[a] * Dv[bb] * (1.0f / 12.0f)));
-                                const float v10 = ta - v11, v01 = tb - v11, v00 = (QD - ta) - v01;
-                                acc_fixed4(T.sJ, T.cc, comp, base, base + st[a], base + st[bb], base + st[a] + st[bb], v00, v10, v01, v11);
-                            }
-                        } else {
-                            const float q0 = Q * Dv[0], q1 = Q * Dv[1];
-                            const float h1 = hv * W[1], h0 = hv - h1;
-                            acc_fixed4(T.sJ, T.cc, 0, base, base + G::JX, base, base + G::JX, q0 * (1.0f - W[1]), q0 * W[1], 0.f, 0.f);
-                            acc_fixed4(T.sJ, T.cc, 1, base, base + 1, base, base + 1, q1 * (1.0f - W[0]), q1 * W[0], 0.f, 0.f);
-                            acc_fixed4(T.sJ, T.cc, 2, base, base + 1, base + G::JX, base + G::JX + 1,
-                                       h0 * (1.0f - W[0]), h0 * W[0], h1 * (1.0f - W[0]), h1 * W[0]);
-                        }
-#pragma unroll
-                        for (int a = 0; a < 3; ++a) { s[a] = r[a] - (float)di[a]; e[a] = d[a]; }
-                        base += dbase;
-                    }
+                    const float a3[3] = { a0[0], a0[1], (D == 3) ? a0[2] : 0.f };
+                    const float hv = (D == 2) ? 0.5f * qw * T.Sc * (u[2] * ig) : 0.f;   // out-of-plane rate per segment (G8), h33 = 1
+                    tile_deposit<D, G>(T.sJ, T.cc, b, a3, d, di, qw * A.inv_dt * T.Sc, hv);
                 }
             }
         }

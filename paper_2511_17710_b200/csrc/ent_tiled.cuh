@@ -204,6 +204,58 @@ __device__ __forceinline__ void acc_fixed4(int *sJ, const CarryCtx &cc, int comp
         if (((a3 ^ n3) & (v3 ^ n3)) < 0) carry_fix(cc, comp, o3, v3 > 0);
     }
 }
+// One straight segment s -> e (cell-local coordinates) of the zig-zag deposit into the fixed-point J tile, element `base` = the
+// segment's cell (Eq. 6).  3D: per component the four products Q D_c [w(W_a) w(W_b) +- D_a D_b / 12] (reading G7), written
+// as v11 = QD (W_a W_b + D_a D_b / 12), v10 = QD W_a - v11, v01 = QD W_b - v11, v00 = QD - QD W_a - v01.  2D: in-plane components
+// with linear weights and the out-of-plane rate hv (G8) with bilinear weights.
+template <int D, class G>
+__device__ __forceinline__ void tile_segment(int *sJ, const CarryCtx &cc, int base, const float s[3], const float e[3], float Q, float hv) {
+    float Dv[3], W[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { Dv[a] = e[a] - s[a]; W[a] = 0.5f * (e[a] + s[a]); }
+    if (D == 3) {
+        const int st[3] = { 1, G::JX, G::JX * G::JY };
+#pragma unroll
+        for (int comp = 0; comp < 3; ++comp) {
+            const int a = (comp + 1) % 3, bb = (comp + 2) % 3;
+            const float QD = Q * Dv[comp];
+            const float ta = QD * W[a], tb = QD * W[bb];
+            const float v11 = fmaf(ta, W[bb], QD * (Dv[a] * Dv[bb] * (1.0f / 12.0f)));
+            const float v10 = ta - v11, v01 = tb - v11, v00 = (QD - ta) - v01;
+            acc_fixed4(sJ, cc, comp, base, base + st[a], base + st[bb], base + st[a] + st[bb], v00, v10, v01, v11);
+        }
+    } else {
+        const float q0 = Q * Dv[0], q1 = Q * Dv[1];
+        const float h1 = hv * W[1], h0 = hv - h1;
+        acc_fixed4(sJ, cc, 0, base, base + G::JX, base, base + G::JX, q0 * (1.0f - W[1]), q0 * W[1], 0.f, 0.f);
+        acc_fixed4(sJ, cc, 1, base, base + 1, base, base + 1, q1 * (1.0f - W[0]), q1 * W[0], 0.f, 0.f);
+        acc_fixed4(sJ, cc, 2, base, base + 1, base + G::JX, base + G::JX + 1, h0 * (1.0f - W[0]), h0 * W[0], h1 * (1.0f - W[0]), h1 * W[0]);
+    }
+}
+// S7 for one particle: old offsets a0 in cell b (box coordinates), new offsets d in cell b + di.  The relay point of P:575 per
+// dimension, r = min(min(0, di) + 1, max(max(0, di), (a0 + di + d) / 2)) in the old cell's frame (Umeda's form: the midpoint if no
+// face is crossed, else the face), without branches.  3D: a particle that crosses no face deposits its move as ONE segment (the two
+// half segments are collinear and the weights above are the exact line integral).  2D: always two segments (the bilinear
+// out-of-plane weights of two half segments do not sum to those of the whole one).
+template <int D, class G>
+__device__ __forceinline__ void tile_deposit(int *sJ, const CarryCtx &cc, const int b[3], const float a0[3], const float d[3], const int di[3],
+                                             float Q, float hv) {
+    const bool cross = (D == 2) || (di[0] | di[1] | di[2]) != 0;
+    float r[3], s2[3], e2[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (a < D) {
+            const float fdi = (float)di[a], bn = fdi + d[a];
+            const float rr = fminf(fminf(fdi, 0.f) + 1.0f, fmaxf(fmaxf(fdi, 0.f), 0.5f * (a0[a] + bn)));
+            r[a] = cross ? rr : bn;
+            s2[a] = rr - fdi; e2[a] = d[a];
+        } else { r[a] = 0.f; s2[a] = 0.f; e2[a] = 0.f; }
+    }
+    const int base = b[0] + G::JX * (b[1] + G::JY * b[2]);
+    tile_segment<D, G>(sJ, cc, base, a0, r, Q, hv);
+    if (cross) tile_segment<D, G>(sJ, cc, base + di[0] + G::JX * (di[1] + G::JY * di[2]), s2, e2, Q, hv);
+}
+
 #ifndef ENT_TILED_MINB
 #define ENT_TILED_MINB 3
 #endif
@@ -312,53 +364,9 @@ __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D
     if (edge) { edge_deposit<D, TiledArgs>(A, iold[0], iold[1], iold[2], a0[0], a0[1], a0[2], di[0], di[1], di[2], d[0], d[1], d[2], u[0], u[1], u[2], qw); return 0; }     // rare: global atomics, un-wrapped from the true cell
     // ---- S7 deposit into the shared-memory J tile (Eq. 6); node (b) of the box = element b of the J tile
     {
-        const float Q = qw * A.inv_dt * T.Sc;                                // Q in fixed-point units
-        // 3D: one straight segment unless a face is crossed.  2D: always the two segments of P:575, because the
-        // out-of-plane weights (bilinear, G8) of two half segments do not sum to those of the whole one
-        const bool cross = (D == 2) || (di[0] | di[1] | di[2]) != 0;
-        float s[3], e[3], r[3];
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            if (a < D) {
-                float bn = (float)di[a] + d[a];                              // new position in the old cell's frame
-                r[a] = di[a] == 0 ? (cross ? 0.5f * (a0[a] + bn) : bn) : (di[a] > 0 ? 1.0f : 0.0f);
-                s[a] = a0[a]; e[a] = r[a];
-            } else { r[a] = s[a] = e[a] = 0.f; }
-        }
-        int base = b[0] + G::JX * (b[1] + G::JY * b[2]);
-        const int dbase = di[0] + G::JX * (di[1] + G::JY * di[2]);
-        float hv = 0.f;
-        if (D == 2) hv = 0.5f * qw * T.Sc * (u[2] * ig);                     // out-of-plane rate per segment (G8), h33 = 1
-        const int nseg = cross ? 2 : 1;
-#pragma unroll 1
-        for (int seg = 0; seg < nseg; ++seg) {
-            float Dv[3], W[3];
-#pragma unroll
-            for (int a = 0; a < 3; ++a) { Dv[a] = e[a] - s[a]; W[a] = 0.5f * (e[a] + s[a]); }
-            if (D == 3) {
-                const int st[3] = { 1, G::JX, G::JX * G::JY };
-#pragma unroll
-                for (int comp = 0; comp < 3; ++comp) {
-                    const int a = (comp + 1) % 3, bb = (comp + 2) % 3;
-                    // the four products Q D_comp [w(W_a) w(W_b) +- D_a D_b / 12] directly: v11 = QD (W_a W_b + c), v10 = QD W_a - v11, ...
-                    const float QD = Q * Dv[comp];
-                    const float ta = QD * W[a], tb = QD * W[bb];
-                    const float v11 = fmaf(ta, W[bb], QD * (Dv[a] * Dv[bb] * (1.0f / 12.0f)));
-                    const float v10 = ta - v11, v01 = tb - v11, v00 = (QD - ta) - v01;
-                    acc_fixed4(T.sJ, T.cc, comp, base, base + st[a], base + st[bb], base + st[a] + st[bb], v00, v10, v01, v11);
-                }
-            } else {
-                float q0 = Q * Dv[0], q1 = Q * Dv[1];
-                float h1 = hv * W[1], h0 = hv - h1;
-                acc_fixed4(T.sJ, T.cc, 0, base, base + G::JX, base, base + G::JX, q0 * (1.0f - W[1]), q0 * W[1], 0.f, 0.f);
-                acc_fixed4(T.sJ, T.cc, 1, base, base + 1, base, base + 1, q1 * (1.0f - W[0]), q1 * W[0], 0.f, 0.f);
-                acc_fixed4(T.sJ, T.cc, 2, base, base + 1, base + G::JX, base + G::JX + 1,
-                           h0 * (1.0f - W[0]), h0 * W[0], h1 * (1.0f - W[0]), h1 * W[0]);
-            }
-#pragma unroll
-            for (int a = 0; a < 3; ++a) { s[a] = r[a] - (float)di[a]; e[a] = d[a]; }
-            base += dbase;
-        }
+        const float a3[3] = { a0[0], a0[1], (D == 3) ? a0[2] : 0.f };
+        const float hv = (D == 2) ? 0.5f * qw * T.Sc * (u[2] * ig) : 0.f;       // out-of-plane rate per segment (G8), h33 = 1
+        tile_deposit<D, G>(T.sJ, T.cc, b, a3, d, di, qw * A.inv_dt * T.Sc, hv);   // Q in fixed-point units
     }
     return 0;
 }
