@@ -213,6 +213,8 @@ def measure(args, name, env, want_e2e):
     ncell = g.ncells
     pbytes = PARTICLE_BYTES[("cart" if g.kind == synth.CART else "axisym", g.D)]
     fused = args.mode == "sorted"
+    paired = args.mode == "pair" and len(parts) == 2 and g.kind == synth.CART
+    per_launch = len(parts) if paired else 1             # species advanced by one launch of the dominant kernel
     step_ev, sort_ev = [], []          # (start, end) CUDA events around each ent_step / ent_sort call in the timed region
 
     def timed(fn, store):
@@ -229,7 +231,10 @@ def measure(args, name, env, want_e2e):
         if not fused and args.sort_every > 0 and it > 0 and it % args.sort_every == 0:
             do_sort(record)
         bind.ent_zero_current(ctx, J)
-        for k in range(len(parts)):
+        if paired:                                           # both species of the pair plasma through one launch of the tiled kernel
+            f = lambda: bind.ent_step_pair(ctx, F, parts[0], parts[1], J, wl.dt)
+            timed(f, step_ev) if record else f()
+        for k in range(0 if paired else len(parts)):
             if fused:                                    # fused step + re-bin, ping-pong between the two blocks: no ent_sort at all
                 def f():
                     bind.ent_step_sorted(ctx, F, parts[k], spare[k], J, wl.dt)
@@ -278,18 +283,19 @@ def measure(args, name, env, want_e2e):
 
     # ---- roofline of the dominant kernel (the fused gather+push+move+deposit kernel), per launch ----
     k_ms = sum(a.elapsed_time(b) for a, b in step_ev) / max(1, len(step_ev))
-    alg_bytes = pbytes * npart / len(parts) + GRID_BYTES_PER_CELL * ncell
+    alg_bytes = pbytes * npart / len(parts) * per_launch + GRID_BYTES_PER_CELL * ncell
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
     mean = lambda ev: (sum(a.elapsed_time(b) for a, b in ev) / len(ev)) if ev else None
     out = {"name": name, "value": value, "ms_per_step": ms_per_step, "ms_timed": ms, "reps": reps, "npart": npart, "launches": launches,
            "clocks": clk, "tiled": bool(tiled), "strays": strays, "bad_moves": bad, "kernel_ms": k_ms,
-           "sort_ms_per_species": mean(sort_ev), "first_sort_ms_per_species": mean(first_sort), "fused": fused,
+           "sort_ms_per_species": mean(sort_ev), "first_sort_ms_per_species": mean(first_sort), "fused": fused, "paired": paired,
            "workload": f"{wl.name} ({wl.note})", "grid": list(g.N), "species": len(parts), "dt": wl.dt, "pbytes": pbytes,
            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                         "traffic": args.traffic, "traffic_source": args.traffic_source if args.traffic is not None else None,
-                        "kernel": ("ent_step_sorted" if fused else "ent_step") + " (fused gather+push+move+deposit), one species per launch",
+                        "kernel": ("ent_step_sorted" if fused else "ent_step_pair" if paired else "ent_step") + " (fused gather+push+move+deposit), "
+                                  + ("both species of the pair plasma per launch" if paired else "one species per launch"),
                         "kernel_ms": k_ms, "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
-                        "step_share": k_ms * len(parts) / ms_per_step}}
+                        "step_share": k_ms * len(parts) / per_launch / ms_per_step}}
 
     # ---- step 9: 4 digital filter passes (the count of the paper's magnetosphere runs) + J = conformal J / sqrt(h)
     npass = 4
@@ -370,7 +376,7 @@ def run_ours(args):
             "data": "synthetic",
             "config": {"workload": m["workload"], "grid": m["grid"], "particles_per_gpu": npart, "species": m["species"],
                        "dt": m["dt"], "shrink": args.shrink, "sorted_at_start": True, "sort_every": 0 if m["fused"] else args.sort_every,
-                       "step_call": "ent_step_sorted" if m["fused"] else "ent_step", "tiled_kernel": m["tiled"],
+                       "step_call": "ent_step_sorted" if m["fused"] else "ent_step_pair" if m["paired"] else "ent_step", "tiled_kernel": m["tiled"],
                        "timed_region_repeats": m["reps"],
                        "l2": "inputs larger than L2 (no flush needed)" if npart * m["pbytes"] > 4e8 else
                        "inputs smaller than L2: the workload itself is L2-resident (BASELINE.json's size), no flush",
@@ -420,8 +426,9 @@ def main():
     ap.add_argument("--step-impl", type=int, default=0, help="ENT_OPT_STEP_IMPL: 0 auto, 1 untiled, 2 two-kernel")
     ap.add_argument("--sort-mode", type=int, default=0, help="ENT_OPT_SORT_MODE: 0 auto (incremental re-bin), 1 always the full sort")
     ap.add_argument("--tile", default="", help="tile extents in cells, e.g. 8,8,4 (ENT_OPT_TILE_*; default: the library's)")
-    ap.add_argument("--mode", default="inplace", choices=["sorted", "inplace"],
-                    help="inplace (default): ent_step + ent_sort every --sort-every steps; sorted: ent_step_sorted (fused step + re-bin, out of place)")
+    ap.add_argument("--mode", default="pair", choices=["pair", "sorted", "inplace"],
+                    help="pair (default): ent_step_pair (both species per launch where the grid is Cartesian, else as inplace) + ent_sort every "
+                         "--sort-every steps; inplace: ent_step per species; sorted: ent_step_sorted (fused step + re-bin, out of place)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

@@ -145,6 +145,14 @@ int ent_tile_offsets(ent_ctx *ctx, const ent_particles *block, int32_t *tile_off
  * Otherwise the untiled kernel (global gathers, global atomics) runs.  Results agree up to fp32 summation order. */
 int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_current *J, float dt);
 
+/* ent_step_pair = ent_step(p1) + ent_step(p2) for two species on the same grid (the pair plasma of the paper's runs) in ONE
+ * launch of the tiled kernel: a CTA stages the E,B box of its tile once, advances the tile's particles of both blocks and flushes
+ * one J tile (half the per-tile work and half the field / current traffic of two launches).  Both blocks must be sorted blocks of
+ * this ctx on a Cartesian grid the tiled kernel supports and either both or neither carry tags; otherwise the call is exactly the
+ * two ent_step calls.  A tile is not split across CTAs here: meant for plasmas whose tile populations are of one order.
+ * Results agree with two ent_step calls up to fp32 summation order of J. */
+int ent_step_pair(ent_ctx *ctx, const ent_fields *EB, ent_particles *p1, ent_particles *p2, ent_current *J, float dt);
+
 /* ent_step_sorted = ent_step + the tile sort in ONE pass, out of place: every particle of `in` is advanced exactly as by
  * ent_step (accumulating into J un-wrapped) and written to `out`, in the range of the tile its cell lay in BEFORE the step.
  * `in` must be a sorted block of this ctx (the `out` of ent_sort or of a previous ent_step_sorted); `out` becomes one, ordered

@@ -22,7 +22,7 @@ OPT_STEP_IMPL, OPT_TILE_1, OPT_TILE_2, OPT_TILE_3, OPT_SORT_MODE, OPT_CURV_FP64,
  STAT_SCRATCH_BYTES, STAT_LAST_STEP_TILED, STAT_LAST_SORT_REBIN, STAT_SLOT_ERRORS, STAT_CARRIES, STAT_GLOBAL_ADDS) = range(1, 15)
 
 SYMBOLS = ["ent_create", "ent_destroy", "ent_last_error", "ent_set_grid", "ent_gather_push", "ent_deposit", "ent_sort",
-           "ent_step", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_filter_current", "ent_faraday", "ent_ampere", "ent_fill_field_ghosts", "ent_compact", "ent_step_host", "ent_set_option", "ent_get_stat", "ent_version"]
+           "ent_step", "ent_step_pair", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_filter_current", "ent_faraday", "ent_ampere", "ent_fill_field_ghosts", "ent_compact", "ent_step_host", "ent_set_option", "ent_get_stat", "ent_version"]
 
 
 class EntError(RuntimeError):
@@ -75,6 +75,7 @@ def lib():
         L.ent_reserve.argtypes = [vp, C.c_int64]
         L.ent_forget.argtypes = [vp, C.POINTER(_Particles)]
         L.ent_step.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Current), C.c_float]
+        L.ent_step_pair.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Particles), C.POINTER(_Current), C.c_float]
         L.ent_zero_current.argtypes = [vp, C.POINTER(_Current)]
         L.ent_fold_current.argtypes = [vp, C.POINTER(_Current)]
         L.ent_filter_current.argtypes = [vp, C.POINTER(_Current), C.c_int, C.c_int]
@@ -274,6 +275,10 @@ def ent_tile_offsets(ctx: Ctx, block: Particles) -> torch.Tensor:
 
 def ent_step(ctx: Ctx, EB, p: Particles, J, dt: float) -> None:
     ctx._ck(lib().ent_step(ctx._h, C.byref(_fields(EB)), C.byref(p.c()), C.byref(_current(J)), dt))
+
+
+def ent_step_pair(ctx: Ctx, EB, p1: Particles, p2: Particles, J, dt: float) -> None:
+    ctx._ck(lib().ent_step_pair(ctx._h, C.byref(_fields(EB)), C.byref(p1.c()), C.byref(p2.c()), C.byref(_current(J)), dt))
 
 
 def ent_step_sorted(ctx: Ctx, EB, pin: Particles, pout: Particles, J, dt: float) -> None:

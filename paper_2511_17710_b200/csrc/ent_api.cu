@@ -528,6 +528,38 @@ extern "C" int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, en
     return launch_check(ctx, "step_untiled_kernel");
 }
 
+// two species through ONE launch of the tiled kernel (one E,B box, one J tile and one flush per tile for both)
+extern "C" int ent_step_pair(ent_ctx *ctx, const ent_fields *EB, ent_particles *p1, ent_particles *p2, ent_current *J, float dt) {
+    ENTER();
+    int rc;
+    if ((rc = check_fields(ctx, EB)) || (rc = check_current(ctx, J)) || (rc = check_particles(ctx, p1, "p1", true)) || (rc = check_particles(ctx, p2, "p2", true))) return rc;
+    if (!(dt > 0.f)) return fail(ctx, ENT_EINVAL, "dt must be positive");
+    if (!(p1->m != 0.f) || !(p2->m != 0.f)) return fail(ctx, ENT_EINVAL, "mass is zero");
+    if (p1->n > 0 && p1->cell == p2->cell) return fail(ctx, ENT_EINVAL, "ent_step_pair: the two blocks are the same");
+    ent_ctx::SortedBlock *s1 = find_block(ctx, p1), *s2 = find_block(ctx, p2);
+    const bool pairable = ctx->step_impl == 0 && s1 && s2 && p1->n > 0 && p2->n > 0 && ctx->g.kind == ENT_CART && tiled_supported(ctx->tiled, ctx->g) &&
+                          (p1->tag != nullptr) == (p2->tag != nullptr);
+    if (!pairable) {                                             // the same result through two launches
+        if ((rc = ent_step(ctx, EB, p1, J, dt))) return rc;
+        return ent_step(ctx, EB, p2, J, dt);
+    }
+    ent_ctx::SortedBlock *sb[2] = { s1, s2 };
+    const ent_particles *pp2[2] = { p1, p2 };
+    for (int k = 0; k < 2; ++k)
+        if (!sb[k]->wmax_valid) {
+            tile_wmax_kernel<<<(unsigned)((long long)ctx->g.nt[0] * ctx->g.nt[1] * ctx->g.nt[2]), 128, 0, ctx->stream>>>(sb[k]->tile_off, pp2[k]->w, sb[k]->tile_wmax);
+            if ((rc = launch_check(ctx, "tile_wmax_kernel"))) return rc;
+            sb[k]->wmax_valid = true;
+        }
+    CK(cudaMemsetAsync(ctx->counters + 1, 0, 2 * sizeof(unsigned long long), ctx->stream));
+    PairSpecies second{ pp(p2), s2->tile_off, s2->tile_wmax, 0.5f * (p2->q / p2->m) * dt, p2->q };
+    rc = tiled_step(ctx->tiled, ctx->g, ctx->stream, fp(EB), pp(p1), cp(J), (long long)p1->n, s1->tile_off, s1->tile_wmax, s1->chunk_off,
+                    0.5f * (p1->q / p1->m) * dt, dt, p1->q, 1.0f / dt, ctx->counters, &ctx->launches, ctx->err, sizeof(ctx->err), &second);
+    if (rc == ENT_OK) ctx->last_step_tiled = 1;
+    s1->counts_valid = false; s2->counts_valid = false;
+    return rc;
+}
+
 // claims a SortedBlock slot for `out` (never the one in `keep`)
 static ent_ctx::SortedBlock *claim_slot(ent_ctx *ctx, const ent_ctx::SortedBlock *keep, const int32_t *out_cell) {
     forget_block(ctx, out_cell);

@@ -166,10 +166,10 @@ step_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
         float rate = fminf(A.inv_dt, 1.02f * fmaxf(g.inv_dx[0], fmaxf(g.inv_dx[1], (D == 3) ? g.inv_dx[2] : 0.f)));
         if (D == 2) rate = fmaxf(rate, 0.5f);
         const float qmax = fabsf(A.q) * wm * rate * 1.0834f;
-        float Sc = (qmax > 0.f && qmax < 1e37f) ? 16777000.0f / qmax : 0.f;
+        float Sc = (qmax > 0.f && qmax < 1e37f) ? FIXED_ONE / qmax : 0.f;
         if (!(Sc > 1e-30f && Sc < 1e30f)) Sc = 0.f;
         invSc = Sc > 0.f ? 1.0f / Sc : 0.f;
-        T.Sc = Sc; T.wguard = Sc > 0.f ? 60.0f * wm : -1.0f;
+        T.Sc = Sc; T.wguard = Sc > 0.f ? (ENT_FIXED_MAGIC ? wm : 60.0f * wm) : -1.0f;   // magic conversion: |value| must stay below 2^22
     }
     T.cc.J = A.J.c; T.cc.P0 = g.P[0]; T.cc.P01 = g.P[0] * g.P[1]; T.cc.unit = 4294967296.0f * invSc;
     T.cc.JX = G::JX; T.cc.JY = G::JY; T.cc.JNP = G::JNP; T.cc.carries = A.counters + 4;

@@ -129,6 +129,9 @@ struct TiledArgs {
     long long n;
     float eps, dt, q, inv_dt;
     float cdt[3];                 // dt / dx_d
+    // second species of a pair launch (ent_step_pair): same tile geometry, its own block, layout, charge and q/m
+    int nsp;                      // 1, or 2: one CTA per tile advances both blocks through one E,B box and one J tile
+    PartPtrs P2; const int32_t *key_off2; const float *tile_wmax2; float eps2, q2;
     unsigned long long *counters; // [0] bad moves, [1] strays, [2] length of stray_list, [4] carries of the fixed-point J tile
     int32_t *stray_list; long long stray_cap;   // particles left to stray_kernel (all lanes busy there instead of one per warp here)
     MagicDiv divN0, divN01;
@@ -136,30 +139,32 @@ struct TiledArgs {
 
 // the global path for one particle (same code as step_untiled_kernel); kept out of line so that the tile loop stays lean
 template <int D>
-__device__ __noinline__ void stray_step(const TiledArgs &A, long long p) {
+__device__ __noinline__ void stray_step(const TiledArgs &A, long long p, int sp = 0) {
     const GridDev &g = A.g;
+    const PartPtrs &P = sp ? A.P2 : A.P;
+    const float q = sp ? A.q2 : A.q, eps = sp ? A.eps2 : A.eps;
     int i[3], i0[3], di[3]; float d[3] = {0.f, 0.f, 0.f}, a[3], u[3], phi = 0.f;
-    unpack_cell<D>(g, A.P.cell[p], i);
+    unpack_cell<D>(g, P.cell[p], i);
 #pragma unroll
-    for (int k = 0; k < D; ++k) d[k] = A.P.d[k][p];
+    for (int k = 0; k < D; ++k) d[k] = P.d[k][p];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) { u[k] = A.P.u[k][p]; a[k] = d[k]; i0[k] = i[k]; }
+    for (int k = 0; k < 3; ++k) { u[k] = P.u[k][p]; a[k] = d[k]; i0[k] = i[k]; }
     GlobalFieldLoader ld{A.F.c};
     bool alive = true;
-    push_particle<D, ENT_CART>(g, ld, i, d, phi, u, A.eps, A.dt, di, alive);
-    A.P.cell[p] = pack_cell<D>(g, i);
+    push_particle<D, ENT_CART>(g, ld, i, d, phi, u, eps, A.dt, di, alive);
+    P.cell[p] = pack_cell<D>(g, i);
 #pragma unroll
-    for (int k = 0; k < D; ++k) A.P.d[k][p] = d[k];
+    for (int k = 0; k < D; ++k) P.d[k][p] = d[k];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) A.P.u[k][p] = u[k];
+    for (int k = 0; k < 3; ++k) P.u[k][p] = u[k];
     atomicAdd(A.counters + 1, 1ULL);
-    if (!alive) { A.P.tag[p] = 0; return; }
+    if (!alive) { P.tag[p] = 0; return; }
     bool bad = false;
 #pragma unroll
     for (int k = 0; k < D; ++k) bad |= (di[k] < -1 || di[k] > 1);
     if (bad) { atomicAdd(A.counters + 0, 1ULL); return; }
     GlobalAcc acc{A.J.c};
-    deposit_particle<D, ENT_CART>(g, acc, i0, a, di, d, 0.f, 0.f, u, A.q * A.P.w[p], A.inv_dt);
+    deposit_particle<D, ENT_CART>(g, acc, i0, a, di, d, 0.f, 0.f, u, q * P.w[p], A.inv_dt);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -171,6 +176,19 @@ __device__ __noinline__ void stray_step(const TiledArgs &A, long long p) {
 // particles' worth of current on one node) is detected from the value the atomic returns and carried straight into
 // the global array as +-2^32 / 2^k, so the sum stays exact for any input.
 // ---------------------------------------------------------------------------------------------------------
+// fixed-point conversion: round(value) as an integer.  ENT_FIXED_MAGIC: value + 1.5 * 2^23 in fp32 leaves round-to-nearest-even(value)
+// in the low mantissa bits (|value| < 2^22): one FADD + one IADD on the full-rate pipes instead of F2I on the quarter-rate XU pipe
+// behind the MIO queue.  The largest contribution then gets 22 bits instead of 24.
+#ifndef ENT_FIXED_MAGIC
+#define ENT_FIXED_MAGIC 0
+#endif
+#if ENT_FIXED_MAGIC
+constexpr float FIXED_ONE = 4194000.0f;
+__device__ __forceinline__ int fixed_rn(float v) { return __float_as_int(v + 12582912.0f) - 0x4B400000; }
+#else
+constexpr float FIXED_ONE = 16777000.0f;
+__device__ __forceinline__ int fixed_rn(float v) { return __float2int_rn(v); }
+#endif
 struct CarryCtx { float *const *J; long long gbase; int P0, P01; float unit; int JX, JY, JNP; unsigned long long *carries; };
 
 __device__ __noinline__ void carry_fix(const CarryCtx &c, int comp, int off, int positive) {
@@ -180,7 +198,7 @@ __device__ __noinline__ void carry_fix(const CarryCtx &c, int comp, int off, int
     atomicAdd(c.carries, 1ULL);
 }
 __device__ __forceinline__ void acc_fixed(int *sJ, const CarryCtx &cc, int comp, int off, float scaled) {
-    int v = __float2int_rn(scaled);
+    int v = fixed_rn(scaled);
     int old = atomicAdd(sJ + comp * cc.JNP + off, v);
     if ((int)((unsigned)old + 0x40000000u) < 0) {     // |old| >= 2^30: only then can |v| < 2^30 wrap the accumulator (conservative, cheap;
                                                       // unsigned: a signed overflow here would be undefined and was optimised away)
@@ -194,7 +212,7 @@ __device__ __forceinline__ void acc_fixed(int *sJ, const CarryCtx &cc, int comp,
 __device__ __forceinline__ void acc_fixed4(int *sJ, const CarryCtx &cc, int comp, int o0, int o1, int o2, int o3,
                                            float s0, float s1, float s2, float s3) {
     int *Jc = sJ + comp * cc.JNP;
-    int v0 = __float2int_rn(s0), v1 = __float2int_rn(s1), v2 = __float2int_rn(s2), v3 = __float2int_rn(s3);
+    int v0 = fixed_rn(s0), v1 = fixed_rn(s1), v2 = fixed_rn(s2), v3 = fixed_rn(s3);
     int a0 = atomicAdd(Jc + o0, v0), a1 = atomicAdd(Jc + o1, v1), a2 = atomicAdd(Jc + o2, v2), a3 = atomicAdd(Jc + o3, v3);
     if ((int)((((unsigned)a0 + 0x40000000u) | ((unsigned)a1 + 0x40000000u)) | (((unsigned)a2 + 0x40000000u) | ((unsigned)a3 + 0x40000000u))) < 0) {
         int n0 = a0 + v0, n1 = a1 + v1, n2 = a2 + v2, n3 = a3 + v3;
@@ -260,7 +278,10 @@ __device__ __forceinline__ void tile_deposit(int *sJ, const CarryCtx &cc, const 
 #define ENT_TILED_MINB 3
 #endif
 
-constexpr int TILED_TPB = 256;
+#ifndef ENT_TILED_TPB
+#define ENT_TILED_TPB 256
+#endif
+constexpr int TILED_TPB = ENT_TILED_TPB;
 constexpr int TILE_CHUNK = 4096;              // particles per CTA: a heavy tile is shared by several CTAs, each with its own J tile
 
 // work-list lookup: the tile whose chunk range contains CTA `vb` (binary search in the exclusive scan), or -1
@@ -299,6 +320,7 @@ struct TileCtx {
     const float *sF;      // [6][FNP] E,B box
     int *sJ;              // [3][JNP] fixed-point J tile
     int o[3];             // tile origin (active cell coordinates)
+    int corner;           // linear index of the box corner o - 2 (inner tiles)
     float sx[3];          // sqrt(h_ii) = cell sizes
     float Sc;             // fixed-point scale of this tile
     float wguard;         // weights above this deposit through the global path (contribution would not fit 2^30)
@@ -308,36 +330,54 @@ struct TileCtx {
 // One particle through sub-steps 3-8 inside a tile.  cell, d[], u[] are updated in place.
 // Returns 0: advanced (write the record back), 1: taken by the global path (already written), 2: advanced and left
 // through an ABSORB side (write back, tag = 0), 3: dead or not ours (untouched).
-template <int D, int TX, int TY, int TZ, bool ALLPER>
+// INNER: the tile's box [o - 2, o + T + 2) lies inside the grid in every dimension (CTA-uniform; 82 % of the tiles of a 256^3 grid):
+// no particle of the range can wrap or touch the edge of the padded arrays, so box coordinates come straight from the linear
+// index relative to the box corner and the new cell is the old one plus the crossing increments.
+template <int D, int TX, int TY, int TZ, bool ALLPER, bool INNER, bool PAIR>
 __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D> &T, long long p, int &cell, float d[3], float u[3],
-                                             float wgt) {
+                                             float wgt, float q, float eps, int sp) {
     using G = TileGeom<D, TX, TY, TZ>;
     const GridDev &g = A.g;
     // ---- where is the cell relative to the tile box?  b = cell index in box coordinates (box origin = o-2)
-    int i[3];
-    if (D == 2) { i[1] = A.divN0.div(cell); i[0] = cell - i[1] * g.N[0]; i[2] = 0; }
-    else { i[2] = A.divN01.div(cell); int r = cell - i[2] * (g.N[0] * g.N[1]); i[1] = A.divN0.div(r); i[0] = r - i[1] * g.N[0]; }
-    const int iold[3] = { i[0], i[1], i[2] };
-    int b[3] = { i[0] - T.o[0] + 2, i[1] - T.o[1] + 2, (D == 3) ? i[2] - T.o[2] + 2 : 0 };
+    int i[3] = { 0, 0, 0 }, b[3];
     const int TT[3] = { TX, TY, TZ };
     bool local = true, edge = false;
+    if (INNER) {
+        const int rel = cell - T.corner;                                  // b0 + N0 (b1 + N1 b2) for a cell inside the box
+        local = rel >= 0;
+        const int rr = local ? rel : 0;
+        if (D == 2) { b[1] = A.divN0.div(rr); b[0] = rr - b[1] * g.N[0]; b[2] = 0; }
+        else { b[2] = A.divN01.div(rr); int r = rr - b[2] * (g.N[0] * g.N[1]); b[1] = A.divN0.div(r); b[0] = r - b[1] * g.N[0]; }
 #pragma unroll
-    for (int a = 0; a < D; ++a) {
-        const int wrapN = (ALLPER || g.bc[a] == ENT_PERIODIC) ? g.N[a] : 0;
-        b[a] += (b[a] < 1) ? wrapN : 0;
-        b[a] -= (b[a] > g.N[a]) ? wrapN : 0;
-        local &= (unsigned)(b[a] - 1) < (unsigned)(TT[a] + 2);           // inside the box with one cell of margin
-        // un-wrapped cell N (a particle that crossed the upper periodic face since the sort): its +1 crossing would deposit
-        // at node N+2, outside the padded array -> it gathers from the box but deposits through the global path
-        edge |= (T.o[a] - 2 + b[a] > g.N[a] - 1);
+        for (int a = 0; a < D; ++a) local &= (unsigned)(b[a] - 1) < (unsigned)(TT[a] + 2);
+    } else {
+        if (D == 2) { i[1] = A.divN0.div(cell); i[0] = cell - i[1] * g.N[0]; i[2] = 0; }
+        else { i[2] = A.divN01.div(cell); int r = cell - i[2] * (g.N[0] * g.N[1]); i[1] = A.divN0.div(r); i[0] = r - i[1] * g.N[0]; }
+        b[0] = i[0] - T.o[0] + 2; b[1] = i[1] - T.o[1] + 2; b[2] = (D == 3) ? i[2] - T.o[2] + 2 : 0;
+#pragma unroll
+        for (int a = 0; a < D; ++a) {
+            const int wrapN = (ALLPER || g.bc[a] == ENT_PERIODIC) ? g.N[a] : 0;
+            b[a] += (b[a] < 1) ? wrapN : 0;
+            b[a] -= (b[a] > g.N[a]) ? wrapN : 0;
+            local &= (unsigned)(b[a] - 1) < (unsigned)(TT[a] + 2);           // inside the box with one cell of margin
+            // un-wrapped cell N (a particle that crossed the upper periodic face since the sort): its +1 crossing would deposit
+            // at node N+2, outside the padded array -> it gathers from the box but deposits through the global path
+            edge |= (T.o[a] - 2 + b[a] > g.N[a] - 1);
+        }
     }
-    if (!local) { defer_stray(A, p, [&] { stray_step<D>(A, p); }); return 1; }
+    // the true old cell (needed by the global-path deposit only)
+    const int iold[3] = { INNER ? T.o[0] - 2 + b[0] : i[0], INNER ? T.o[1] - 2 + b[1] : i[1], INNER ? ((D == 3) ? T.o[2] - 2 + b[2] : 0) : i[2] };
+    if (!local) {
+        if (PAIR) stray_step<D>(A, p, sp);         // pair launch: the stray list does not record the species
+        else defer_stray(A, p, [&] { stray_step<D>(A, p); });
+        return 1;
+    }
     // ---- S1 gather from the shared-memory box (same stencil as ent_dev.cuh gather)
     float EBv[6];
     gather_box<D, G::FX, G::FY, G::FNP>(T.sF, b, d, EBv);
     // ---- S2 tetrad (A^hat = sqrt(h_ii) A^i), S3 Boris (Eq. 3), S4-S5 move + crossing
     float E[3] = { T.sx[0] * EBv[0], T.sx[1] * EBv[1], T.sx[2] * EBv[2] }, B[3] = { T.sx[0] * EBv[3], T.sx[1] * EBv[4], T.sx[2] * EBv[5] };
-    push_momentum(g.pusher, u, E, B, A.eps);
+    push_momentum(g.pusher, u, E, B, eps);
     const float ig = inv_gamma(u);
     const float a0[3] = { d[0], d[1], d[2] };
     int di[3] = {0, 0, 0};
@@ -346,6 +386,7 @@ __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D
     for (int a = 0; a < D; ++a) {
         float x = d[a] + (u[a] * ig) * A.cdt[a];
         split_offset(x, di[a], d[a]);
+        if (INNER) continue;
         int in = i[a] + di[a];
         const int wrapN = (ALLPER || g.bc[a] == ENT_PERIODIC) ? g.N[a] : 0;
         in += (in < 0) ? wrapN : 0;
@@ -353,13 +394,14 @@ __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D
         if (!ALLPER) { if (in < 0) { alive = false; in = 0; } if (in >= g.N[a]) { alive = false; in = g.N[a] - 1; } }
         i[a] = in;
     }
-    cell = (D == 2) ? i[0] + g.N[0] * i[1] : i[0] + g.N[0] * (i[1] + g.N[1] * i[2]);
+    if (INNER) cell += di[0] + g.N[0] * (di[1] + ((D == 3) ? g.N[1] * di[2] : 0));
+    else cell = (D == 2) ? i[0] + g.N[0] * i[1] : i[0] + g.N[0] * (i[1] + g.N[1] * i[2]);
     if (!alive) return 2;
     bool bad = false;
 #pragma unroll
     for (int a = 0; a < D; ++a) bad |= (di[a] < -1) | (di[a] > 1);
     if (bad) { atomicAdd(A.counters + 0, 1ULL); return 0; }
-    const float qw = A.q * wgt;
+    const float qw = q * wgt;
     edge |= !(fabsf(wgt) <= T.wguard);        // a weight far above the tile's recorded maximum (changed since the sort) cannot use the tile's scale
     if (edge) { edge_deposit<D, TiledArgs>(A, iold[0], iold[1], iold[2], a0[0], a0[1], a0[2], di[0], di[1], di[2], d[0], d[1], d[2], u[0], u[1], u[2], qw); return 0; }     // rare: global atomics, un-wrapped from the true cell
     // ---- S7 deposit into the shared-memory J tile (Eq. 6); node (b) of the box = element b of the J tile
@@ -371,7 +413,7 @@ __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D
     return 0;
 }
 
-template <int D, int TX, int TY, int TZ, bool ALLPER>     // ALLPER: every dimension periodic (no ABSORB bookkeeping)
+template <int D, int TX, int TY, int TZ, bool ALLPER, bool PAIR>     // ALLPER: every dimension periodic (no ABSORB bookkeeping); PAIR: two blocks
 __global__ void __launch_bounds__(TILED_TPB, ENT_TILED_MINB)
 step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ TiledArgs A) {
     using G = TileGeom<D, TX, TY, TZ>;
@@ -382,13 +424,21 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     const GridDev &g = A.g;
     const int tid = threadIdx.x;
 
-    const int tile = find_tile(A.chunk_off, A.ntiles, blockIdx.x);
+    // pair launch: one CTA per tile, whole ranges of both blocks; otherwise the work list (chunks of TILE_CHUNK particles)
+    const int tile = PAIR ? (int)blockIdx.x : find_tile(A.chunk_off, A.ntiles, blockIdx.x);
     if (tile < 0) return;                                        // the grid is an upper bound of the work list
     const int t0 = tile % g.nt[0], t12 = tile / g.nt[0];
     const int t1 = (D == 3) ? t12 % g.nt[1] : t12, t2 = (D == 3) ? t12 / g.nt[1] : 0;
     TileCtx<D> T;
     T.sF = sF; T.sJ = sJ;
     T.o[0] = t0 * TX; T.o[1] = t1 * TY; T.o[2] = t2 * TZ;
+    bool inner = ALLPER;
+    {
+        const int TT[3] = { TX, TY, TZ };
+#pragma unroll
+        for (int a = 0; a < D; ++a) inner &= T.o[a] >= 2 && T.o[a] + TT[a] + 2 <= g.N[a];
+    }
+    T.corner = (T.o[0] - 2) + g.N[0] * ((T.o[1] - 2) + ((D == 3) ? g.N[1] * (T.o[2] - 2) : 0));
     T.sx[0] = g.dx[0]; T.sx[1] = g.dx[1]; T.sx[2] = g.dx[2];
 
     if (tid == 0) {
@@ -400,23 +450,29 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     }
     for (int k = tid; k < 3 * G::JNP / 4; k += TILED_TPB) reinterpret_cast<int4 *>(sJ)[k] = make_int4(0, 0, 0, 0);
 
-    long long p0 = A.key_off[tile], p1 = A.key_off[tile + 1];
-    p0 += (long long)(blockIdx.x - A.chunk_off[tile]) * TILE_CHUNK;
-    if (p1 > p0 + TILE_CHUNK) p1 = p0 + TILE_CHUNK;
-    float invSc;
+    float invSc, wguard2 = -1.0f;
     {
         // fixed-point scale of this tile.  Largest contribution: |q| wmax / dt * |D| * weight with |D| <= 1, weight <= 13/12
         // (2D: J^3 = q w v^3 has no 1/dt); wmax = max |w| over the tile's particles (ent_sort).  It gets 24 bits; a nodal sum
         // beyond 2^31 (128 such contributions adding coherently) wraps and is carried exactly (carry_fix).
-        const float wm = A.tile_wmax[tile];
+        float wm = A.tile_wmax[tile];
         // |D_a| <= min(1, dt / dx_a): the rate q w D / dt is at most q w / min dx (2D: J^3 = q w v^3, |v^3| < 1, h33 = 1)
         float rate = fminf(A.inv_dt, 1.02f * fmaxf(g.inv_dx[0], fmaxf(g.inv_dx[1], (D == 3) ? g.inv_dx[2] : 0.f)));
         if (D == 2) rate = fmaxf(rate, 0.5f);
-        float qmax = fabsf(A.q) * wm * rate * 1.0834f;
-        float Sc = (qmax > 0.f && qmax < 1e37f) ? 16777000.0f / qmax : 0.f;
+        float qw1 = fabsf(A.q) * wm;
+        if (PAIR) {                                              // one scale for both species: the larger |q| wmax
+            const float wm2 = A.tile_wmax2[tile], qw2 = fabsf(A.q2) * wm2;
+            const float qwm = fmaxf(qw1, qw2);
+            wguard2 = (ENT_FIXED_MAGIC ? 1.0f : 60.0f) * (fabsf(A.q2) > 0.f ? qwm / fabsf(A.q2) : 0.f);
+            wm = fabsf(A.q) > 0.f ? qwm / fabsf(A.q) : 0.f;
+            qw1 = qwm;
+        }
+        float qmax = qw1 * rate * 1.0834f;
+        float Sc = (qmax > 0.f && qmax < 1e37f) ? FIXED_ONE / qmax : 0.f;
         if (!(Sc > 1e-30f && Sc < 1e30f)) Sc = 0.f;
         invSc = Sc > 0.f ? 1.0f / Sc : 0.f;
-        T.Sc = Sc; T.wguard = Sc > 0.f ? 60.0f * wm : -1.0f;
+        T.Sc = Sc; T.wguard = Sc > 0.f ? (ENT_FIXED_MAGIC ? wm : 60.0f * wm) : -1.0f;   // magic conversion: |value| must stay below 2^22
+        if (!(Sc > 0.f)) wguard2 = -1.0f;
     }
     T.cc.J = A.J.c; T.cc.P0 = g.P[0]; T.cc.P01 = g.P[0] * g.P[1]; T.cc.unit = 4294967296.0f * invSc;
     T.cc.JX = G::JX; T.cc.JY = G::JY; T.cc.JNP = G::JNP; T.cc.carries = A.counters + 4;
@@ -428,12 +484,23 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     // coalesced 128-byte line per warp, the work of a tile is balanced to within one particle per thread, and the order of the
     // particles inside the tile's range does not matter (the incremental ent_sort does not keep one)
     // software pipeline: the record of the thread's next particle is requested before the current one is advanced
+#pragma unroll 1
+  for (int sp = 0; sp < (PAIR ? 2 : 1); ++sp) {
+    const PartPtrs &P = (PAIR && sp) ? A.P2 : A.P;
+    const float q = (PAIR && sp) ? A.q2 : A.q, eps = (PAIR && sp) ? A.eps2 : A.eps;
+    if (PAIR && sp) T.wguard = wguard2;
+    const int32_t *koff = (PAIR && sp) ? A.key_off2 : A.key_off;
+    long long p0 = koff[tile], p1 = koff[tile + 1];
+    if (!PAIR) {
+        p0 += (long long)(blockIdx.x - A.chunk_off[tile]) * TILE_CHUNK;
+        if (p1 > p0 + TILE_CHUNK) p1 = p0 + TILE_CHUNK;
+    }
     long long p = p0 + tid;
     int ncell = 0; float nd0 = 0.f, nd1 = 0.f, nd2 = 0.f, nu0 = 0.f, nu1 = 0.f, nu2 = 0.f, nw = 0.f; bool nlive = true;
     if (p < p1) {
-        ncell = A.P.cell[p]; nd0 = A.P.d[0][p]; nd1 = A.P.d[1][p]; if (D == 3) nd2 = A.P.d[2][p];
-        nu0 = A.P.u[0][p]; nu1 = A.P.u[1][p]; nu2 = A.P.u[2][p]; nw = A.P.w[p];
-        if (A.P.tag) nlive = A.P.tag[p] != 0;
+        ncell = P.cell[p]; nd0 = P.d[0][p]; nd1 = P.d[1][p]; if (D == 3) nd2 = P.d[2][p];
+        nu0 = P.u[0][p]; nu1 = P.u[1][p]; nu2 = P.u[2][p]; nw = P.w[p];
+        if (P.tag) nlive = P.tag[p] != 0;
     }
     for (; p < p1; p += TILED_TPB) {
         int cell = ncell;
@@ -441,19 +508,21 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
         const float wgt = nw; const bool live = nlive;
         const long long pn = p + TILED_TPB;
         if (pn < p1) {
-            ncell = A.P.cell[pn]; nd0 = A.P.d[0][pn]; nd1 = A.P.d[1][pn]; if (D == 3) nd2 = A.P.d[2][pn];
-            nu0 = A.P.u[0][pn]; nu1 = A.P.u[1][pn]; nu2 = A.P.u[2][pn]; nw = A.P.w[pn];
-            if (A.P.tag) nlive = A.P.tag[pn] != 0;
+            ncell = P.cell[pn]; nd0 = P.d[0][pn]; nd1 = P.d[1][pn]; if (D == 3) nd2 = P.d[2][pn];
+            nu0 = P.u[0][pn]; nu1 = P.u[1][pn]; nu2 = P.u[2][pn]; nw = P.w[pn];
+            if (P.tag) nlive = P.tag[pn] != 0;
         }
         if (!waited) { mbar_wait(&bar, 0); waited = true; }
         if (!live) continue;
-        const int code = tile_particle<D, TX, TY, TZ, ALLPER>(A, T, p, cell, d, u, wgt);
+        const int code = inner ? tile_particle<D, TX, TY, TZ, ALLPER, true, PAIR>(A, T, p, cell, d, u, wgt, q, eps, sp)
+                               : tile_particle<D, TX, TY, TZ, ALLPER, false, PAIR>(A, T, p, cell, d, u, wgt, q, eps, sp);
         if (code & 1) continue;
-        A.P.cell[p] = cell;
-        A.P.d[0][p] = d[0]; A.P.d[1][p] = d[1]; if (D == 3) A.P.d[2][p] = d[2];
-        A.P.u[0][p] = u[0]; A.P.u[1][p] = u[1]; A.P.u[2][p] = u[2];
-        if (!ALLPER && code == 2) A.P.tag[p] = 0;
+        P.cell[p] = cell;
+        P.d[0][p] = d[0]; P.d[1][p] = d[1]; if (D == 3) P.d[2][p] = d[2];
+        P.u[0][p] = u[0]; P.u[1][p] = u[1]; P.u[2][p] = u[2];
+        if (!ALLPER && code == 2) P.tag[p] = 0;
     }
+  }
     if (!waited) mbar_wait(&bar, 0);          // never leave with a TMA load still in flight into this CTA's shared memory
     // ---- S8 flush: one TMA reduce-add per component into the un-wrapped padded J (ghost fold = ent_fold_current)
     __syncthreads();
@@ -496,7 +565,7 @@ struct TiledState {
     const void *ptrF[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     const void *ptrJ[3] = {nullptr, nullptr, nullptr};
     TileMaps maps;
-    bool attr_set[16] = {};
+    bool attr_set[32] = {};
 };
 
 
@@ -569,8 +638,11 @@ inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, 
     if (rc) return rc;
     bool allper = true;
     for (int a = 0; a < D; ++a) allper &= A.g.bc[a] == ENT_PERIODIC;
-    void (*kern)(const TileMaps, const TiledArgs) = allper ? step_tiled_kernel<D, TX, TY, TZ, true> : step_tiled_kernel<D, TX, TY, TZ, false>;
-    int slot = 2 * IDX + (allper ? 1 : 0);
+    const bool pair = A.nsp == 2;
+    void (*kern)(const TileMaps, const TiledArgs) =
+        pair ? (allper ? step_tiled_kernel<D, TX, TY, TZ, true, true> : step_tiled_kernel<D, TX, TY, TZ, false, true>)
+             : (allper ? step_tiled_kernel<D, TX, TY, TZ, true, false> : step_tiled_kernel<D, TX, TY, TZ, false, false>);
+    int slot = 2 * IDX + (allper ? 1 : 0) + (pair ? 16 : 0);
     int smem_bytes = G::SMEM_BYTES;
     if constexpr (D == 2) {
         if (A.g.kind == ENT_SPH) { kern = step_tiled_axisym_kernel<ENT_SPH, TX, TY>; slot = 6; }
@@ -583,7 +655,7 @@ inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, 
         t.attr_set[slot] = true;
     }
     const int ntiles = A.g.nt[0] * A.g.nt[1] * A.g.nt[2];
-    const long long grid = (long long)ntiles + A.n / TILE_CHUNK + 1;        // upper bound of the number of chunks
+    const long long grid = A.nsp == 2 ? (long long)ntiles : (long long)ntiles + A.n / TILE_CHUNK + 1;        // upper bound of the number of chunks
     kern<<<(unsigned)grid, TILED_TPB, smem_bytes, stream>>>(t.maps, A);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { snprintf(err, errn, "launch of step_tiled_kernel failed: %s", cudaGetErrorString(e)); return ENT_ECUDA; }
@@ -593,12 +665,16 @@ inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, 
     return ENT_OK;
 }
 
+struct PairSpecies { PartPtrs P; const int32_t *key_off; const float *tile_wmax; float eps, q; };   // second block of ent_step_pair
+
 inline int tiled_step(TiledState &t, const GridDev &g, cudaStream_t stream, FieldPtrs F, PartPtrs P, CurrentPtrs J, long long n,
                       const int32_t *key_off, const float *tile_wmax, const int32_t *chunk_off, float eps, float dt, float q, float inv_dt, unsigned long long *counters,
-                      long long *launches, char *err, size_t errn) {
+                      long long *launches, char *err, size_t errn, const PairSpecies *pair = nullptr) {
     TiledArgs A;
     A.g = g; A.F = F; A.J = J; A.P = P; A.key_off = key_off; A.tile_wmax = tile_wmax; A.chunk_off = chunk_off; A.ntiles = g.nt[0] * g.nt[1] * g.nt[2]; A.n = n;
     A.eps = eps; A.dt = dt; A.q = q; A.inv_dt = inv_dt; A.counters = counters;
+    A.nsp = 1; A.P2 = P; A.key_off2 = key_off; A.tile_wmax2 = tile_wmax; A.eps2 = eps; A.q2 = q;
+    if (pair) { A.nsp = 2; A.P2 = pair->P; A.key_off2 = pair->key_off; A.tile_wmax2 = pair->tile_wmax; A.eps2 = pair->eps; A.q2 = pair->q; }
     A.stray_list = t.stray_list; A.stray_cap = t.stray_cap;
     for (int a = 0; a < 3; ++a) A.cdt[a] = dt * g.inv_dx[a];
     A.divN0 = make_magicdiv((uint32_t)g.N[0]);

@@ -445,3 +445,63 @@ def test_compact_matches_oracle(env, name):
     bind.ent_step(ctx, F, srt, J, wl.dt)
     torch.cuda.synchronize()
     assert bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED) == 1
+
+
+@pytest.mark.parametrize("name", ["C1", "C3/8", "C4/16-shuffled", "ABS3", "ABS2"])
+def test_step_pair_matches_oracle(env, name):
+    """ent_step_pair: both species of the pair plasma through one launch of the tiled kernel (one E,B box, one J tile per tile).
+    Same bars as the single-species tests: the summed current of the two species against the oracle's, particles per species,
+    continuity of the GPU's own output; blocks re-binned every 3 steps."""
+    bind, synth, ctx, orc = env
+    wl = _workloads(synth)[name]()
+    g = wl.grid
+    eg, og = P.grid_to_ent(bind, g), P.grid_to_orc(orc, g)
+    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, 0)
+    bind.ent_set_grid(ctx, eg)
+    F_dev, F_orc = [f.cuda() for f in wl.fields], P.fields_to_orc(wl.fields)
+    assert len(wl.species) == 2
+    pes, pos, orders = [], [], []
+    bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 1)
+    for sp in wl.species:
+        pe = P.species_to_ent(bind, synth, g, sp, "cuda")
+        ps = pe.empty_like()
+        bind.ent_sort(ctx, pe, ps, None)
+        orders.append(_match_perm(g, pe, ps)); pes.append(ps); pos.append(P.species_to_orc(orc, sp))
+    bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 0)
+    Jg = bind.zeros_current(eg, "cuda")
+    steps = min(wl.steps, 8)
+    worstJ = worstC = 0.0
+    for s in range(steps):
+        if s > 0 and s % 3 == 0:
+            for k in range(2):
+                ps = pes[k].empty_like()
+                bind.ent_sort(ctx, pes[k], ps, None)
+                assert bind.ent_get_stat(ctx, bind.STAT_LAST_SORT_REBIN) == 1
+                orders[k] = orders[k][_match_perm(g, pes[k], ps)]
+                pes[k] = ps
+        before = [P.ent_to_orc(orc, g, pe) for pe in pes]
+        bind.ent_zero_current(ctx, Jg)
+        bind.ent_step_pair(ctx, F_dev, pes[0], pes[1], Jg, wl.dt)
+        bind.ent_fold_current(ctx, Jg)
+        torch.cuda.synchronize()
+        assert bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED) == 1
+        after = [P.ent_to_orc(orc, g, pe) for pe in pes]
+        Jo = orc.zeros_current(og)
+        Jown = orc.zeros_current(og)                       # the oracle's deposit of the GPU's own stored moves (strict, no allowance)
+        for k, sp in enumerate(wl.species):
+            po_before = pos[k].copy()
+            orc.step(og, F_orc, pos[k], Jo, sp.q, sp.m, wl.dt)
+            _, corr = P.straddler_correction(orc, g, og, po_before, pos[k], before[k], after[k], sp.q, wl.dt, orders[k])
+            if corr is not None:
+                Jo = [a + b for a, b in zip(Jo, corr)]
+            own = P.deposit_of_gpu_positions(orc, og, before[k], after[k], sp.q, wl.dt, fold=False)
+            Jown = [a + b for a, b in zip(Jown, own)]
+        orc.fold_current(og, Jo)
+        orc.fold_current(og, Jown)
+        worstJ = max(worstJ, P.compare_current(Jg, Jo), P.compare_current(Jg, Jown))
+    for k in range(2):
+        st = P.compare_particles(g, pes[k], pos[k], orders[k], steps=steps)
+        assert st["tag_mismatch"] == 0
+    assert bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES) == 0
+    print(name, "pair: max|dJ|/max|J| =", worstJ)
+    assert worstJ <= P.J_TOL
