@@ -44,22 +44,39 @@ __device__ __forceinline__ double axis_area(const GridDev &g, double x1) {
     return r * r * eR * g.dR * (1.0 - cos(theta_of_T(g.vt, 0.5 * g.dT)));
 }
 
-// covariant component h_cc F^c of component c6 at lattice index q (periodic wrap); ok = false if q is outside the lattice
-template <bool CARTESIAN>
-__device__ __forceinline__ float fld_cov(const GridDev &g, const SolverGeom &L, const float *A, int c6, int q0, int q1, int q2, bool &ok) {
-    int q[3] = { q0, q1, q2 };
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        const int n = L.n[c6][d];
-        if ((unsigned)q[d] < (unsigned)n) continue;
-        if (d < g.D && g.bc[d] == ENT_PERIODIC) q[d] += q[d] < 0 ? n : -n;
-        else { ok = false; return 0.f; }
-    }
-    const float v = A[(long long)(q[0] + NG) + (long long)g.P[0] * ((long long)(q[1] + NG) + (g.D == 3 ? (long long)g.P[1] * (q[2] + NG) : 0))];
-    if (CARTESIAN) return L.cov[c6 % 3] * v;
+// padded linear index of lattice index (i, j, k)
+__device__ __forceinline__ long long fld_at(const GridDev &g, int i, int j, int k) {
+    return (long long)(i + NG) + (long long)g.P[0] * ((long long)(j + NG) + (g.D == 3 ? (long long)g.P[1] * (k + NG) : 0));
+}
+// index of the neighbour of q along dimension A (compile time) at distance S = +1 / -1 on the lattice of component C6, periodic
+// wrap; ok = false if it lies outside a non-periodic lattice
+template <int C6, int A, int S>
+__device__ __forceinline__ void fld_shift(const GridDev &g, const SolverGeom &L, int &i, int &j, int &k, bool &ok) {
+    int &q = A == 0 ? i : (A == 1 ? j : k);
+    const int n = L.n[C6][A];
+    q += S;
+    if (q < 0 || q >= n) { if (g.bc[A] == ENT_PERIODIC) q += q < 0 ? n : -n; else ok = false; }
+}
+// covariant component h_cc F^c of component C6 at lattice index (i, j, k) of its own lattice
+template <bool CARTESIAN, int C6>
+__device__ __forceinline__ float fld_cov(const GridDev &g, const SolverGeom &L, const float *A, int i, int j, int k) {
+    const float v = A[fld_at(g, i, j, k)];
+    if (CARTESIAN) return L.cov[C6 % 3] * v;
     double h[3];
-    metric_h_axisym(g, q[0] + (fld_stag(c6, 0) ? 0.5 : 0.0), q[1] + (fld_stag(c6, 1) ? 0.5 : 0.0), h);
-    return (float)(h[c6 % 3] * (double)v);
+    metric_h_axisym(g, i + (fld_stag(C6, 0) ? 0.5 : 0.0), j + (fld_stag(C6, 1) ? 0.5 : 0.0), h);
+    return (float)(h[C6 % 3] * (double)v);
+}
+// F_C6(q + S e_A) - F_C6(q) (S = +1) or F_C6(q) - F_C6(q - e_A) (S = -1), covariant
+template <bool CARTESIAN, int C6, int A, int S>
+__device__ __forceinline__ float fld_diff(const GridDev &g, const SolverGeom &L, const float *F, int i, int j, int k, bool &ok) {
+    int i2 = i, j2 = j, k2 = k;
+    // the lattices of the updated component and of C6 differ along A only (node against half-integer points): on a non-periodic
+    // dimension the last node has no C6 value "here" either
+    if ((A == 0 ? i : (A == 1 ? j : k)) >= L.n[C6][A]) ok = false;
+    fld_shift<C6, A, S>(g, L, i2, j2, k2, ok);
+    if (!ok) return 0.f;
+    const float here = fld_cov<CARTESIAN, C6>(g, L, F, i, j, k), there = fld_cov<CARTESIAN, C6>(g, L, F, i2, j2, k2);
+    return S > 0 ? there - here : here - there;
 }
 template <bool CARTESIAN>
 __device__ __forceinline__ float inv_sqrt_h_of(const GridDev &g, const SolverGeom &L, int c6, int i, int j) {
@@ -69,45 +86,58 @@ __device__ __forceinline__ float inv_sqrt_h_of(const GridDev &g, const SolverGeo
     return (float)(1.0 / sqrt(h[0] * h[1] * h[2]));
 }
 
+// one lattice point of B^C (Eq. A1); C, and with it the stencil, is a compile-time constant
+template <bool CARTESIAN, int C>
+__device__ __forceinline__ void faraday_point(const GridDev &g, const SolverGeom &L, const FieldRW &F, float dt, int i, int j, int k) {
+    constexpr int CB = 3 + C, A = (C + 1) % 3, B = (C + 2) % 3;
+    if (i >= L.n[CB][0] || j >= L.n[CB][1] || k >= L.n[CB][2]) return;
+    float *Bc = F.c[CB] + fld_at(g, i, j, k);
+    if (!CARTESIAN && C == 1 && (j == 0 || j == g.N[1])) { *Bc = 0.f; return; }                 // Eq. 12: B^2 = 0 on the axis
+    bool ok = true;
+    float curl = 0.f;
+    if (A < 2 || g.D == 3) curl += fld_diff<CARTESIAN, B, A, +1>(g, L, F.c[B], i, j, k, ok);     // E_b(+a) - E_b
+    if (B < 2 || g.D == 3) curl -= fld_diff<CARTESIAN, A, B, +1>(g, L, F.c[A], i, j, k, ok);     // E_a(+b) - E_a
+    if (!ok) return;                                                                           // cannot happen: A1 stays inside the E lattices
+    *Bc -= dt * curl * inv_sqrt_h_of<CARTESIAN>(g, L, CB, i, j);                                // Eq. A1
+}
+// one lattice point of E^C (Eq. A2, Eqs. 12-13 on the axis)
+template <bool CARTESIAN, int C>
+__device__ __forceinline__ void ampere_point(const GridDev &g, const SolverGeom &L, const FieldRW &F, const CurrentPtrs &J, int haveJ, float dt,
+                                             float jc, int i, int j, int k) {
+    constexpr int A = (C + 1) % 3, B = (C + 2) % 3;
+    if (i >= L.n[C][0] || j >= L.n[C][1] || k >= L.n[C][2]) return;
+    const long long at = fld_at(g, i, j, k);
+    float *Ec = F.c[C] + at;
+    const float Jc = haveJ ? J.c[C][at] : 0.f;
+    if (!CARTESIAN && C != 1 && (j == 0 || j == g.N[1])) {                                       // a point on the polar axis
+        if (C == 2) { *Ec = 0.f; return; }                                                      // Eq. 12: E^3 = 0
+        const bool north = j == 0;                                                              // Eq. 13 and its mirror image at theta = pi
+        const float B3 = fld_cov<CARTESIAN, 5>(g, L, F.c[5], i, north ? 0 : g.N[1] - 1, 0);
+        *Ec += (float)((double)dt * ((north ? B3 : -B3) - 0.5f * jc * Jc) / axis_area(g, i + 0.5));
+        return;
+    }
+    bool ok = true;
+    float curl = 0.f;
+    if (A < 2 || g.D == 3) curl += fld_diff<CARTESIAN, 3 + B, A, -1>(g, L, F.c[3 + B], i, j, k, ok);   // B_b - B_b(-a)
+    if (B < 2 || g.D == 3) curl -= fld_diff<CARTESIAN, 3 + A, B, -1>(g, L, F.c[3 + A], i, j, k, ok);   // B_a - B_a(-b)
+    if (!ok) return;                                   // tangential E on a non-periodic face: the caller's boundary condition
+    *Ec += dt * (curl - jc * Jc) * inv_sqrt_h_of<CARTESIAN>(g, L, C, i, j);                      // Eq. A2
+}
+
 // blockIdx.x: chunk of x1, blockIdx.y: x2 index, blockIdx.z = component * nmax[2] + x3 index
 template <bool CARTESIAN>
 __global__ void __launch_bounds__(TPB) faraday_kernel(GridDev g, SolverGeom L, FieldRW F, float dt) {
     const int c = blockIdx.z / L.nmax[2], k = blockIdx.z - c * L.nmax[2], j = blockIdx.y, i = blockIdx.x * TPB + threadIdx.x;
-    const int cB = 3 + c, a = (c + 1) % 3, b = (c + 2) % 3;
-    if (i >= L.n[cB][0] || j >= L.n[cB][1] || k >= L.n[cB][2]) return;
-    float *Bc = F.c[cB] + ((long long)(i + NG) + (long long)g.P[0] * ((long long)(j + NG) + (g.D == 3 ? (long long)g.P[1] * (k + NG) : 0)));
-    if (!CARTESIAN && c == 1 && (j == 0 || j == g.N[1])) { *Bc = 0.f; return; }                 // Eq. 12: B^2 = 0 on the axis
-    bool ok = true;
-    float curl = 0.f;
-    const int e[3][3] = { {1, 0, 0}, {0, 1, 0}, {0, 0, 1} };
-    if (a < g.D) curl += fld_cov<CARTESIAN>(g, L, F.c[b], b, i + e[a][0], j + e[a][1], k + e[a][2], ok) - fld_cov<CARTESIAN>(g, L, F.c[b], b, i, j, k, ok);
-    if (b < g.D) curl -= fld_cov<CARTESIAN>(g, L, F.c[a], a, i + e[b][0], j + e[b][1], k + e[b][2], ok) - fld_cov<CARTESIAN>(g, L, F.c[a], a, i, j, k, ok);
-    if (!ok) return;                                                                           // cannot happen: A1 stays inside the E lattices
-    *Bc -= dt * curl * inv_sqrt_h_of<CARTESIAN>(g, L, cB, i, j);                                // Eq. A1
+    if (c == 0) faraday_point<CARTESIAN, 0>(g, L, F, dt, i, j, k);
+    else if (c == 1) faraday_point<CARTESIAN, 1>(g, L, F, dt, i, j, k);
+    else faraday_point<CARTESIAN, 2>(g, L, F, dt, i, j, k);
 }
-
 template <bool CARTESIAN>
 __global__ void __launch_bounds__(TPB) ampere_kernel(GridDev g, SolverGeom L, FieldRW F, CurrentPtrs J, int haveJ, float dt, float jc) {
     const int c = blockIdx.z / L.nmax[2], k = blockIdx.z - c * L.nmax[2], j = blockIdx.y, i = blockIdx.x * TPB + threadIdx.x;
-    const int a = (c + 1) % 3, b = (c + 2) % 3;
-    if (i >= L.n[c][0] || j >= L.n[c][1] || k >= L.n[c][2]) return;
-    const long long at = (long long)(i + NG) + (long long)g.P[0] * ((long long)(j + NG) + (g.D == 3 ? (long long)g.P[1] * (k + NG) : 0));
-    float *Ec = F.c[c] + at;
-    const float Jc = haveJ ? J.c[c][at] : 0.f;
-    bool ok = true;
-    if (!CARTESIAN && c != 1 && (j == 0 || j == g.N[1])) {                                       // a point on the polar axis
-        if (c == 2) { *Ec = 0.f; return; }                                                      // Eq. 12: E^3 = 0
-        const bool north = j == 0;                                                              // Eq. 13 and its mirror image at theta = pi
-        const float B3 = fld_cov<CARTESIAN>(g, L, F.c[5], 5, i, north ? 0 : g.N[1] - 1, 0, ok);
-        *Ec += (float)((double)dt * ((north ? B3 : -B3) - 0.5f * jc * Jc) / axis_area(g, i + 0.5));
-        return;
-    }
-    float curl = 0.f;
-    const int e[3][3] = { {1, 0, 0}, {0, 1, 0}, {0, 0, 1} };
-    if (a < g.D) curl += fld_cov<CARTESIAN>(g, L, F.c[3 + b], 3 + b, i, j, k, ok) - fld_cov<CARTESIAN>(g, L, F.c[3 + b], 3 + b, i - e[a][0], j - e[a][1], k - e[a][2], ok);
-    if (b < g.D) curl -= fld_cov<CARTESIAN>(g, L, F.c[3 + a], 3 + a, i, j, k, ok) - fld_cov<CARTESIAN>(g, L, F.c[3 + a], 3 + a, i - e[b][0], j - e[b][1], k - e[b][2], ok);
-    if (!ok) return;                                   // tangential E on a non-periodic face: the caller's boundary condition
-    *Ec += dt * (curl - jc * Jc) * inv_sqrt_h_of<CARTESIAN>(g, L, c, i, j);                      // Eq. A2
+    if (c == 0) ampere_point<CARTESIAN, 0>(g, L, F, J, haveJ, dt, jc, i, j, k);
+    else if (c == 1) ampere_point<CARTESIAN, 1>(g, L, F, J, haveJ, dt, jc, i, j, k);
+    else ampere_point<CARTESIAN, 2>(g, L, F, J, haveJ, dt, jc, i, j, k);
 }
 
 // ghost layers of the six arrays along dimension `dim` (the transverse range is the whole padded extent, so edges and corners
