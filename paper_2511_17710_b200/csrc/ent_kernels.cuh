@@ -435,13 +435,21 @@ struct RebinGeom {
         else { int n01 = N[0] * N[1]; i2 = dN01.div(cell); int r = cell - i2 * n01; i1 = dN0.div(r); i0 = r - i1 * N[0]; }
         t[0] = dT[0].div(i0); t[1] = dT[1].div(i1); t[2] = (D == 3) ? dT[2].div(i2) : 0;
     }
-    // index of the cell inside its own tile: l0 + T0*(l1 + T1*l2)
-    __device__ __forceinline__ int local_cell(int cell) const {
+    // Destination class of a particle of source tile s (origin o, extent te: the last tile of a dimension may be partial), its
+    // destination tile td and, for a particle that stays (class 13), the index lc of its cell inside the tile.  The ~87 % that
+    // stay need the two divisions of the cell decode only; the others take the tile divisions and the wrap logic of classify.
+    __device__ __forceinline__ int classify_cell(int cell, int src, const int s[3], const int o[3], const int te[3], int &td, int &lc) const {
         int i0, i1, i2 = 0;
         if (D == 2) { i1 = dN0.div(cell); i0 = cell - i1 * N[0]; }
         else { int n01 = N[0] * N[1]; i2 = dN01.div(cell); int r = cell - i2 * n01; i1 = dN0.div(r); i0 = r - i1 * N[0]; }
-        int l0 = i0 - dT[0].div(i0) * T[0], l1 = i1 - dT[1].div(i1) * T[1], l2 = (D == 3) ? i2 - dT[2].div(i2) * T[2] : 0;
-        return l0 + T[0] * (l1 + T[1] * l2);
+        const int u0 = i0 - o[0], u1 = i1 - o[1], u2 = i2 - o[2];
+        if ((unsigned)u0 < (unsigned)te[0] && (unsigned)u1 < (unsigned)te[1] && (unsigned)u2 < (unsigned)te[2]) {
+            td = src; lc = u0 + T[0] * (u1 + T[1] * u2);
+            return 13;
+        }
+        int t[3] = { dT[0].div(i0), dT[1].div(i1), (D == 3) ? dT[2].div(i2) : 0 };
+        td = t[0] + nt[0] * (t[1] + nt[1] * t[2]); lc = 0;
+        return classify(s, t);
     }
     // class of destination tile t seen from source tile s: 0..26 = neighbour (dz+1)*9 + (dy+1)*3 + (dx+1), 27 = far
     __device__ __forceinline__ int classify(const int s[3], const int t[3]) const {
@@ -474,13 +482,15 @@ __global__ void __launch_bounds__(REBIN_TPB) rebin_count_kernel(RebinGeom G, con
     __shared__ int cnt[REBIN_CLASSES];
     const int src = blockIdx.x;
     int s[3] = { src % G.nt[0], (src / G.nt[0]) % G.nt[1], src / (G.nt[0] * G.nt[1]) };
+    const int o[3] = { s[0] * G.T[0], s[1] * G.T[1], s[2] * G.T[2] };
+    const int te[3] = { min(G.T[0], G.N[0] - o[0]), min(G.T[1], G.N[1] - o[1]), G.D == 3 ? min(G.T[2], G.N[2] - o[2]) : 1 };
     if (threadIdx.x < REBIN_CLASSES) cnt[threadIdx.x] = 0;
     __syncthreads();
     const long long p0 = tile_off[src], p1 = tile_off[src + 1];
     for (long long base = p0; base < p1; base += REBIN_TPB) {
         long long p = base + threadIdx.x;
         int rel = -1, td = 0;
-        if (p < p1) { int t[3]; G.tile_of_cell(cell[p], t); rel = G.classify(s, t); td = t[0] + G.nt[0] * (t[1] + G.nt[1] * t[2]); }
+        if (p < p1) { int lc; rel = G.classify_cell(cell[p], src, s, o, te, td, lc); }
         // the ~90 % that stay (class 13 = the source tile itself) are counted with one ballot; the few others one by one
         const unsigned stay = __ballot_sync(0xffffffffu, rel == 13);
         if (rel == 13) { if ((int)(__ffs(stay) - 1) == (int)(threadIdx.x & 31)) atomicAdd(&cnt[13], __popc(stay)); }
@@ -502,6 +512,8 @@ __global__ void __launch_bounds__(REBIN_TPB) rebin_scatter_kernel(RebinGeom G, c
     __shared__ unsigned wmx[REBIN_CLASSES];
     const int src = blockIdx.x;
     int s[3] = { src % G.nt[0], (src / G.nt[0]) % G.nt[1], src / (G.nt[0] * G.nt[1]) };
+    const int o[3] = { s[0] * G.T[0], s[1] * G.T[1], s[2] * G.T[2] };
+    const int te[3] = { min(G.T[0], G.N[0] - o[0]), min(G.T[1], G.N[1] - o[1]), G.D == 3 ? min(G.T[2], G.N[2] - o[2]) : 1 };
     if (threadIdx.x < REBIN_CLASSES) {
         int c = class_count[(long long)src * REBIN_CLASSES + threadIdx.x];
         int d = threadIdx.x < 27 ? G.dest_tile(s, threadIdx.x) : -1;
@@ -523,7 +535,7 @@ __global__ void __launch_bounds__(REBIN_TPB) rebin_scatter_kernel(RebinGeom G, c
             w = in.w[p];
             if (axisym) rphi = in.phi[p];
             if (in.tag) rtag = in.tag[p];
-            int t[3]; G.tile_of_cell(c, t); rel = G.classify(s, t); td = t[0] + G.nt[0] * (t[1] + G.nt[1] * t[2]);
+            int lc; rel = G.classify_cell(c, src, s, o, te, td, lc);
         }
         // stayers (class 13): one ballot, one reservation per warp, slots in lane order; the few others one by one
         const unsigned stay = __ballot_sync(0xffffffffu, rel == 13);
@@ -581,6 +593,8 @@ __global__ void __launch_bounds__(ORD_TPB) rebin_scatter_ordered_kernel(RebinGeo
     __shared__ unsigned wmx[REBIN_CLASSES];
     const int src = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
     int s[3] = { src % G.nt[0], (src / G.nt[0]) % G.nt[1], src / (G.nt[0] * G.nt[1]) };
+    const int o[3] = { s[0] * G.T[0], s[1] * G.T[1], s[2] * G.T[2] };
+    const int te[3] = { min(G.T[0], G.N[0] - o[0]), min(G.T[1], G.N[1] - o[1]), G.D == 3 ? min(G.T[2], G.N[2] - o[2]) : 1 };
     if (tid < REBIN_CLASSES) {
         int c = class_count[(long long)src * REBIN_CLASSES + tid];
         int d = tid < 27 ? G.dest_tile(s, tid) : -1;
@@ -596,14 +610,14 @@ __global__ void __launch_bounds__(ORD_TPB) rebin_scatter_ordered_kernel(RebinGeo
     // every record is read once; a stayer is staged in arrival order (ordered tile) or placed at once (too full a tile)
     for (long long base = p0; base < p1; base += ORD_TPB) {
         const long long p = base + tid;
-        int rel = -1, td = 0, c = 0;
+        int rel = -1, td = 0, c = 0, lc = 0;
         float rd[3] = {0.f, 0.f, 0.f}, ru[3] = {0.f, 0.f, 0.f}, w = 0.f; uint8_t rtag = 1;
         if (p < p1) {
             c = in.cell[p];
             for (int a = 0; a < 3; ++a) { if (a < G.D) rd[a] = in.d[a][p]; ru[a] = in.u[a][p]; }
             w = in.w[p];
             if (in.tag) rtag = in.tag[p];
-            int t[3]; G.tile_of_cell(c, t); rel = G.classify(s, t); td = t[0] + G.nt[0] * (t[1] + G.nt[1] * t[2]);
+            rel = G.classify_cell(c, src, s, o, te, td, lc);
         }
         const unsigned wbits = __float_as_uint(fabsf(w));
         const unsigned stay = __ballot_sync(0xffffffffu, rel == 13);
@@ -615,7 +629,6 @@ __global__ void __launch_bounds__(ORD_TPB) rebin_scatter_ordered_kernel(RebinGeo
         if (rel < 0) continue;
         const int mine = r0 + __popc(stay & ((1u << lane) - 1u));              // stayers: slot in arrival order
         if (rel == 13 && ordered) {
-            const int lc = G.local_cell(c);
             st_cell[mine] = c;
             for (int a = 0; a < 3; ++a) { st_f[a * cap + mine] = rd[a]; st_f[(3 + a) * cap + mine] = ru[a]; }
             st_f[6 * cap + mine] = w;
