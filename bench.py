@@ -44,6 +44,19 @@ def _peaks():
 
 
 
+def _committed_traffic(workload, mode):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture table (profiles/r2_traffic.csv), or (None, None)"""
+    import csv
+    p = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+    try:
+        for row in csv.DictReader(open(p)):
+            if row["workload"] == workload and row["mode"] == mode:
+                return float(row["dram_bytes_per_launch"]), row["source"]
+    except OSError:
+        pass
+    return None, None
+
+
 def max_over_ranks(value: float, device) -> float:
     """time-like quantities are reduced with MAX over the ranks of the job (no-op for a single process)"""
     import torch
@@ -286,12 +299,15 @@ def measure(args, name, env, want_e2e):
     alg_bytes = pbytes * npart / len(parts) * per_launch + GRID_BYTES_PER_CELL * ncell
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
     mean = lambda ev: (sum(a.elapsed_time(b) for a, b in ev) / len(ev)) if ev else None
+    traffic, traffic_src = args.traffic, args.traffic_source
+    if traffic is None and args.shrink == 1 and not args.tile:
+        traffic, traffic_src = _committed_traffic(name, "pair" if paired else ("sorted" if fused else "inplace"))
     out = {"name": name, "value": value, "ms_per_step": ms_per_step, "ms_timed": ms, "reps": reps, "npart": npart, "launches": launches,
            "clocks": clk, "tiled": bool(tiled), "strays": strays, "bad_moves": bad, "kernel_ms": k_ms,
            "sort_ms_per_species": mean(sort_ev), "first_sort_ms_per_species": mean(first_sort), "fused": fused, "paired": paired,
            "workload": f"{wl.name} ({wl.note})", "grid": list(g.N), "species": len(parts), "dt": wl.dt, "pbytes": pbytes,
            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                        "traffic": args.traffic, "traffic_source": args.traffic_source if args.traffic is not None else None,
+                        "traffic": traffic, "traffic_source": traffic_src,
                         "kernel": ("ent_step_sorted" if fused else "ent_step_pair" if paired else "ent_step") + " (fused gather+push+move+deposit), "
                                   + ("both species of the pair plasma per launch" if paired else "one species per launch"),
                         "kernel_ms": k_ms, "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,

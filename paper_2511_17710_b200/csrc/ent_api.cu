@@ -371,11 +371,11 @@ extern "C" int ent_filter_current(ent_ctx *ctx, ent_current *J, int npasses, int
     const int total = npasses ? npasses : 1;
     for (int pass = 0; pass < total; ++pass) {
         const bool last = pass == total - 1;
-        filter_pass_kernel<<<fgrid, FT_I * FT_J, 0, ctx->stream>>>(g, L, (pass & 1) ? b : a, (pass & 1) ? a : b, npasses == 0 ? 1 : 0, last && divide_by_sqrt_h, nkc);
+        filter_pass_kernel<<<fgrid, FT_TX * FT_J, 0, ctx->stream>>>(g, L, (pass & 1) ? b : a, (pass & 1) ? a : b, npasses == 0 ? 1 : 0, last && divide_by_sqrt_h, nkc);
         if ((rc = launch_check(ctx, "filter_pass_kernel"))) return rc;
     }
     if (total & 1) {                                         // the result sits in the scratch arrays: copy the lattice points back
-        filter_pass_kernel<<<fgrid, FT_I * FT_J, 0, ctx->stream>>>(g, L, b, a, 2, 0, nkc);
+        filter_pass_kernel<<<fgrid, FT_TX * FT_J, 0, ctx->stream>>>(g, L, b, a, 2, 0, nkc);
         if ((rc = launch_check(ctx, "filter_pass_kernel"))) return rc;
     }
     return ENT_OK;

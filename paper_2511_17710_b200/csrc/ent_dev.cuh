@@ -11,6 +11,7 @@ namespace ent {
 constexpr int NG = ENT_NGHOST;
 constexpr double PI_D = 3.14159265358979323846264338327950288;
 constexpr float TWO_PI_F = 6.28318548202514648f;   // float nearest to 2*pi (slightly above it)
+constexpr float TWO_PI_LO = 1.74845553e-7f;         // TWO_PI_F - 2*pi
 
 // Grid + metric constants, passed to kernels by value (the paper passes its metric object by value too).
 struct GridDev {

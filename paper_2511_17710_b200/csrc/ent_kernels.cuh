@@ -197,40 +197,55 @@ __device__ __forceinline__ float sqrt_h_at(const GridDev &g, double x1, double x
 // One pass over a tile of FT_I x FT_J lattice points, marching along x3 (3D): the in-plane part of the stencil,
 // P_k = sum_{di,dj} w(di) w(dj) J(i+di, j+dj, k), comes from a shared-memory copy of plane k (one global load per point and plane,
 // halo columns included), and the thread keeps P_{k-1}, P_k, P_{k+1} in registers: out_k = P_{k-1}/4 + P_k/2 + P_{k+1}/4
-// (f = (1/2)^(D + |di| + |dj| + |dk|) = w(di) w(dj) w(dk), Eqs. 9-11).  In 2D out = P.  A tile whose whole neighbourhood lies inside
-// the lattice of a Cartesian grid loads without any boundary logic; the others go through filter_fetch.
+// (f = (1/2)^(D + |di| + |dj| + |dk|) = w(di) w(dj) w(dk), Eqs. 9-11).  In 2D out = P.  A thread owns FT_V = 4 consecutive points
+// of a row (six shared values per stencil row: one 128-bit and one 64-bit load), the plane copies are double-buffered (one
+// barrier per plane).  A tile whose whole neighbourhood lies inside the lattice of a Cartesian grid loads without any boundary
+// logic; the others go through filter_fetch.
 // mode 0: filter; 1: no convolution (scaling pass only); 2: copy.  blockIdx.z = component * nkc + chunk of FT_K planes.
-constexpr int FT_I = 32, FT_J = 8, FT_K = 32;
-__global__ void __launch_bounds__(FT_I * FT_J) filter_pass_kernel(GridDev g, FilterGeom L, CurrentPtrs src, CurrentPtrs dst, int mode, int divide, int nkc) {
-    __shared__ float s[2][FT_J + 2][FT_I + 4];
+constexpr int FT_V = 4, FT_TX = 32, FT_I = FT_TX * FT_V, FT_J = 8, FT_K = 32, FT_ROW = FT_I + 4;   // row: halo, FT_I points, halo, pad
+__global__ void __launch_bounds__(FT_TX * FT_J) filter_pass_kernel(GridDev g, FilterGeom L, CurrentPtrs src, CurrentPtrs dst, int mode, int divide, int nkc) {
+    __shared__ __align__(16) float s[2][FT_J + 2][FT_ROW];
     const int comp = blockIdx.z / nkc, kc = blockIdx.z - comp * nkc;
     const int n0 = L.n[comp][0], n1 = L.n[comp][1], n2 = L.n[comp][2];
     const int i0 = blockIdx.x * FT_I, j0 = blockIdx.y * FT_J, k0 = kc * FT_K;
     if (i0 >= n0 || j0 >= n1 || k0 >= n2) return;                    // the grid is sized for the largest lattice
     const int k1 = min(k0 + FT_K, n2);
-    const int tid = threadIdx.x, tx = tid % FT_I, ty = tid / FT_I;
-    const int i = i0 + tx, j = j0 + ty;
-    const bool mine = i < n0 && j < n1;
+    const int tid = threadIdx.x, tx = tid % FT_TX, ty = tid / FT_TX;
+    const int i = i0 + FT_V * tx, j = j0 + ty;
+    const bool row = j < n1;
     const float *A = src.c[comp];
     float *O = dst.c[comp];
     const long long P0 = g.P[0], P01 = g.D == 3 ? (long long)g.P[0] * g.P[1] : 0;
     const long long at = (long long)(i + NG) + P0 * (j + NG) + (g.D == 3 ? P01 * NG : 0);     // (i, j, k = 0)
     const bool axis_node = filter_on_axis(g, L, comp, j);
-    float sh_here = 1.f;
-    if (divide && mine && !axis_node) sh_here = sqrt_h_at(g, i + (comp == 0 ? 0.5 : 0.0), j + (comp == 1 ? 0.5 : 0.0));
+    float sh[FT_V];
+#pragma unroll
+    for (int v = 0; v < FT_V; ++v) sh[v] = (divide && row && i + v < n0 && !axis_node) ? sqrt_h_at(g, i + v + (comp == 0 ? 0.5 : 0.0), j + (comp == 1 ? 0.5 : 0.0)) : 1.f;
+    auto emit = [&](int k, const float acc[FT_V]) {
+        if (!row) return;
+#pragma unroll
+        for (int v = 0; v < FT_V; ++v) {
+            if (i + v >= n0) continue;
+            float a = acc[v];
+            if (mode == 0 && comp == 2 && axis_node) a = 0.f;          // J^3(i, 0) = 0
+            if (divide && !axis_node) a /= sh[v];
+            O[at + v + P01 * k] = a;
+        }
+    };
     if (mode != 0) {
-        if (mine)
+        if (row)
             for (int k = k0; k < k1; ++k) {
-                float v = A[at + P01 * k];
-                if (divide && !axis_node) v /= sh_here;
-                O[at + P01 * k] = v;
+                float a[FT_V];
+#pragma unroll
+                for (int v = 0; v < FT_V; ++v) a[v] = i + v < n0 ? A[at + v + P01 * k] : 0.f;
+                emit(k, a);
             }
         return;
     }
     const bool d3 = g.D == 3;
     const bool interior = g.kind == ENT_CART && i0 >= 1 && i0 + FT_I + 1 <= n0 && j0 >= 1 && j0 + FT_J + 1 <= n1 && (!d3 || (k0 >= 1 && k1 + 1 <= n2));
-    auto load_plane = [&](int k, int buf) {
-        for (int e = tid; e < (FT_J + 2) * (FT_I + 2); e += FT_I * FT_J) {
+    auto load_plane = [&](int k, int buf) {                             // s[buf][jj][ii] = J(i0 - 1 + ii, j0 - 1 + jj, k)
+        for (int e = tid; e < (FT_J + 2) * (FT_I + 2); e += FT_TX * FT_J) {
             const int jj = e / (FT_I + 2), ii = e - jj * (FT_I + 2);
             const int q0 = i0 - 1 + ii, q1 = j0 - 1 + jj;
             float v = 0.f;
@@ -239,37 +254,42 @@ __global__ void __launch_bounds__(FT_I * FT_J) filter_pass_kernel(GridDev g, Fil
             s[buf][jj][ii] = v;
         }
     };
-    auto in_plane = [&](int buf) {
-        const float r0 = 0.25f * s[buf][ty][tx] + 0.5f * s[buf][ty][tx + 1] + 0.25f * s[buf][ty][tx + 2];
-        const float r1 = 0.25f * s[buf][ty + 1][tx] + 0.5f * s[buf][ty + 1][tx + 1] + 0.25f * s[buf][ty + 1][tx + 2];
-        const float r2 = 0.25f * s[buf][ty + 2][tx] + 0.5f * s[buf][ty + 2][tx + 1] + 0.25f * s[buf][ty + 2][tx + 2];
-        return 0.25f * r0 + 0.5f * r1 + 0.25f * r2;
-    };
-    auto emit = [&](int k, float acc) {
-        if (!mine) return;
-        if (comp == 2 && axis_node) acc = 0.f;                        // J^3(i, 0) = 0
-        if (divide && !axis_node) acc /= sh_here;
-        O[at + P01 * k] = acc;
+    auto in_plane = [&](int buf, float P[FT_V]) {
+        float r[3][FT_V];
+#pragma unroll
+        for (int rr = 0; rr < 3; ++rr) {
+            const float4 a = *reinterpret_cast<const float4 *>(&s[buf][ty + rr][FT_V * tx]);
+            const float2 b = *reinterpret_cast<const float2 *>(&s[buf][ty + rr][FT_V * tx + 4]);
+            const float v[6] = { a.x, a.y, a.z, a.w, b.x, b.y };
+#pragma unroll
+            for (int q = 0; q < FT_V; ++q) r[rr][q] = 0.25f * v[q] + 0.5f * v[q + 1] + 0.25f * v[q + 2];
+        }
+#pragma unroll
+        for (int q = 0; q < FT_V; ++q) P[q] = 0.25f * r[0][q] + 0.5f * r[1][q] + 0.25f * r[2][q];
     };
     if (!d3) {
         load_plane(0, 0);
         __syncthreads();
-        emit(0, in_plane(0));
+        float P[FT_V];
+        in_plane(0, P);
+        emit(0, P);
         return;
     }
-    float Pm, Pc;
+    float Pm[FT_V], Pc[FT_V], Pn[FT_V];
     load_plane(k0 - 1, 0);
     load_plane(k0, 1);
     __syncthreads();
-    Pm = in_plane(0); Pc = in_plane(1);
+    in_plane(0, Pm); in_plane(1, Pc);
+    __syncthreads();                                                 // both initial copies have been read
     for (int k = k0; k < k1; ++k) {
-        const int buf = (k - k0) & 1;                                // plane k + 1 overwrites the buffer of plane k - 1
-        __syncthreads();                                             // everyone is done reading that buffer
-        load_plane(k + 1, buf);
+        const int buf = (k - k0) & 1;                                // plane k + 1 goes where plane k - 1 was: everyone has passed the barrier
+        load_plane(k + 1, buf);                                      // that followed its last read (double buffering, one barrier per plane)
         __syncthreads();
-        const float Pn = in_plane(buf);
-        emit(k, 0.25f * Pm + 0.5f * Pc + 0.25f * Pn);
-        Pm = Pc; Pc = Pn;
+        in_plane(buf, Pn);
+        float out[FT_V];
+#pragma unroll
+        for (int q = 0; q < FT_V; ++q) { out[q] = 0.25f * Pm[q] + 0.5f * Pc[q] + 0.25f * Pn[q]; Pm[q] = Pc[q]; Pc[q] = Pn[q]; }
+        emit(k, out);
     }
 }
 

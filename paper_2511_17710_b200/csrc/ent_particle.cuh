@@ -97,8 +97,10 @@ __device__ __forceinline__ void push_from_fields_geo(const GridDev &g, const GEO
         split_offset(d[1] + x2n, di[1], d[1]);
         di[2] = 0;
         float phn = phi + Dph;
-        if (phn >= TWO_PI_F) phn -= TWO_PI_F;
-        if (phn < 0.f) phn += TWO_PI_F;
+        // wrap into [0, 2 pi) with the two-constant form 2 pi = TWO_PI_F - TWO_PI_LO (TWO_PI_F alone is 1.75e-7 above 2 pi, which is
+        // most of an fp32 ulp of an azimuth near 2 pi and showed up in the full-size parity of C5)
+        if (phn >= TWO_PI_F) phn = (phn - TWO_PI_F) + TWO_PI_LO;
+        if (phn < 0.f) phn = (phn - TWO_PI_LO) + TWO_PI_F;
         if (phn >= TWO_PI_F) phn = 0.f;
         phi = phn;
     } else {

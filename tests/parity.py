@@ -236,6 +236,25 @@ def continuity_of_gpu_step(orc, og, p_before, p_after, Jg_folded, q, dt):
     return res / scale if scale > 0 else res
 
 
+def continuity_of_gpu_steps(orc, og, befores, afters, Jg_folded, qs, dt):
+    """continuity_of_gpu_step for several species that deposited into the same J (ent_step_pair): the charge arrays are summed"""
+    rho0 = rho1 = norm = None
+    for pb, pa, q in zip(befores, afters, qs):
+        alive = np.ones(pb.n, dtype=np.int8)
+        if pb.tag is not None:
+            alive &= (pb.tag != 0).astype(np.int8)
+        if pa.tag is not None:
+            alive &= (pa.tag != 0).astype(np.int8)
+        rho0 = orc.charge_density(og, pb, q, mask=alive, rho=rho0)
+        rho1 = orc.charge_density(og, pa, q, mask=alive, rho=rho1)
+        norm = orc.charge_density(og, pb, abs(q), mask=alive, rho=norm)
+    J = [np.ascontiguousarray(j.detach().cpu().numpy().astype(np.float64)) for j in Jg_folded]
+    orc.fold_scalar(og, rho0); orc.fold_scalar(og, rho1); orc.fold_scalar(og, norm)
+    res = orc.continuity_residual(og, J, rho0, rho1, dt)
+    scale = float(np.abs(norm).max()) / dt
+    return res / scale if scale > 0 else res
+
+
 def ent_to_orc(orc, grid, pe):
     """binding.Particles (GPU result) -> orc.Particles holding the same values (for the continuity checker)"""
     cell = pe.cell.detach().cpu().numpy()

@@ -111,6 +111,83 @@ def test_full_size_last_step(orc, name):
         bind.ent_destroy(ctx)
 
 
+@pytest.mark.parametrize("name", ["C3", "C4"])
+def test_full_size_pair_launch_last_step(orc, name):
+    """The launch configuration bench.py times by default: BOTH species through ent_step_pair (one launch of the tiled kernel),
+    blocks sorted, re-binned every 3 steps.  Sampled particles of each species, the summed current of the two species in two
+    sub-boxes against the oracle, whole-grid continuity of the summed charge."""
+    from paper_2511_17710_b200 import binding as bind, synth
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    if torch.cuda.mem_get_info()[1] < 100e9:
+        pytest.skip("needs a GPU with > 100 GB for the full-size workloads")
+    wl = synth.CONFIGS[name](1, device="cuda")
+    g = wl.grid
+    eg, og = P.grid_to_ent(bind, g), P.grid_to_orc(orc, g)
+    ctx = bind.ent_create(0, None)
+    try:
+        bind.ent_set_grid(ctx, eg)
+        F = wl.fields
+        pes = [bind.Particles(cell=synth.pack_cell(g, sp.i), d=sp.d, u=sp.u, w=sp.w, q=sp.q, m=sp.m) for sp in wl.species]
+        wl.species = None
+        spares = [pe.empty_like() for pe in pes]
+        bind.ent_reserve(ctx, max(pe.n for pe in pes))
+        bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 1)
+        for k in range(2):
+            bind.ent_sort(ctx, pes[k], spares[k], None)
+            pes[k], spares[k] = spares[k], pes[k]
+        bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 0)
+        J = bind.zeros_current(eg, "cuda")
+        befores = None
+        for s in range(5):                                  # steps 0-2, re-bin, steps 3-4; step 4 is checked
+            if s == 3:
+                for k in range(2):
+                    bind.ent_sort(ctx, pes[k], spares[k], None)
+                    assert bind.ent_get_stat(ctx, bind.STAT_LAST_SORT_REBIN) == 1
+                    pes[k], spares[k] = spares[k], pes[k]
+            if s == 4:
+                del spares
+                befores = [pe.clone() for pe in pes]
+            bind.ent_zero_current(ctx, J)
+            bind.ent_step_pair(ctx, F, pes[0], pes[1], J, wl.dt)
+            assert bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED) == 1
+        bind.ent_fold_current(ctx, J)
+        torch.cuda.synchronize()
+        assert bind.ent_get_stat(ctx, bind.STAT_STRAYS) == 0 and bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES) == 0
+        F_orc = P.fields_to_orc(F)
+        gen = torch.Generator(device="cuda"); gen.manual_seed(4321)
+        for k in range(2):
+            idx = torch.randint(0, pes[k].n, (NSAMPLE // 2,), device="cuda", generator=gen)
+            pb = P.ent_to_orc(orc, g, _subset(bind, befores[k], idx))
+            po = orc.gather_push(og, F_orc, pb, befores[k].q / befores[k].m, wl.dt)
+            print(f"species {k} sample:", P.compare_particles(g, _subset(bind, pes[k], idx), po, steps=1, orc_metric=(orc, og)))
+        Jscale = max(float(j.abs().max()) for j in J)
+        N = [int(n) for n in g.N]
+        for lo in ((40, 100, 200), (N[0] - 8, N[1] - 8, N[2] - 8)):
+            Jo = orc.zeros_current(og)
+            npart = 0
+            for k in range(2):
+                ib = synth.unpack_cell(g, befores[k].cell)
+                sel = torch.nonzero(_in_box_periodic(ib, [l - 2 for l in lo], BOX + 4, N)).squeeze(1)
+                del ib
+                npart += sel.numel()
+                orc.step(og, F_orc, P.ent_to_orc(orc, g, _subset(bind, befores[k], sel)), Jo, befores[k].q, befores[k].m, wl.dt)
+            orc.fold_current(og, Jo)
+            ax = [np.array([(lo[a] + k) % N[a] for k in range(BOX)]) + 2 for a in range(3)]
+            worst = max(float(np.abs(J[c].cpu().numpy().astype(np.float64)[np.ix_(ax[2], ax[1], ax[0])] - Jo[c][np.ix_(ax[2], ax[1], ax[0])]).max())
+                        for c in range(3))
+            print(f"box at {lo}: {npart} particles of both species, max|dJ|/max|J| = {worst / Jscale:.3e}")
+            assert worst <= P.J_TOL * Jscale
+        del Jo
+        if name == "C3":                                      # host memory: the checker holds every particle of both species in fp64
+            c = P.continuity_of_gpu_steps(orc, og, [P.ent_to_orc(orc, g, b) for b in befores], [P.ent_to_orc(orc, g, pe) for pe in pes], J,
+                                          [b.q for b in befores], wl.dt)
+            print(f"continuity residual (whole grid, both species): {c:.3e}")
+            assert c <= P.CONT_TOL
+    finally:
+        bind.ent_destroy(ctx)
+
+
 def test_c5_full_size_last_step(orc):
     """C5 at full size (quasi-spherical 2048^2, ~134 M particles per species, tiled axisymmetric kernel, heavy tiles split over
     several CTAs): sampled particles against the oracle, the current of an inner (dense) box, whole-grid continuity."""

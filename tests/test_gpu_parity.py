@@ -499,9 +499,12 @@ def test_step_pair_matches_oracle(env, name):
         orc.fold_current(og, Jo)
         orc.fold_current(og, Jown)
         worstJ = max(worstJ, P.compare_current(Jg, Jo), P.compare_current(Jg, Jown))
+        c = P.continuity_of_gpu_steps(orc, og, before, after, Jg, [sp.q for sp in wl.species], wl.dt)
+        assert c <= P.CONT_TOL, f"continuity residual {c:.3e} at step {s}"
+        worstC = max(worstC, c)
     for k in range(2):
         st = P.compare_particles(g, pes[k], pos[k], orders[k], steps=steps)
         assert st["tag_mismatch"] == 0
     assert bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES) == 0
-    print(name, "pair: max|dJ|/max|J| =", worstJ)
+    print(name, "pair: max|dJ|/max|J| =", worstJ, " continuity", worstC)
     assert worstJ <= P.J_TOL
