@@ -366,16 +366,16 @@ extern "C" int ent_filter_current(ent_ctx *ctx, ent_current *J, int npasses, int
     CurrentPtrs a = cp(J), b;
     for (int c = 0; c < 3; ++c) b.c[c] = (float *)((char *)ctx->fbuf + slot * c);
     const int nkc = (nmax[2] + FT_K - 1) / FT_K;
-    const dim3 fgrid((nmax[0] + FT_I - 1) / FT_I, (nmax[1] + FT_J - 1) / FT_J, 3 * nkc);
+    const dim3 fgrid((nmax[0] + FT_W - 1) / FT_W, (nmax[1] + FT_J - 1) / FT_J, 3 * nkc);
     if (fgrid.y > 65535u || fgrid.z > 65535u) return fail(ctx, ENT_EUNSUPPORTED, "grid too large for the filter kernel");
     const int total = npasses ? npasses : 1;
     for (int pass = 0; pass < total; ++pass) {
         const bool last = pass == total - 1;
-        filter_pass_kernel<<<fgrid, FT_TX * FT_J, 0, ctx->stream>>>(g, L, (pass & 1) ? b : a, (pass & 1) ? a : b, npasses == 0 ? 1 : 0, last && divide_by_sqrt_h, nkc);
+        filter_pass_kernel<<<fgrid, FT_TPB, 0, ctx->stream>>>(g, L, (pass & 1) ? b : a, (pass & 1) ? a : b, npasses == 0 ? 1 : 0, last && divide_by_sqrt_h, nkc);
         if ((rc = launch_check(ctx, "filter_pass_kernel"))) return rc;
     }
     if (total & 1) {                                         // the result sits in the scratch arrays: copy the lattice points back
-        filter_pass_kernel<<<fgrid, FT_TX * FT_J, 0, ctx->stream>>>(g, L, b, a, 2, 0, nkc);
+        filter_pass_kernel<<<fgrid, FT_TPB, 0, ctx->stream>>>(g, L, b, a, 2, 0, nkc);
         if ((rc = launch_check(ctx, "filter_pass_kernel"))) return rc;
     }
     return ENT_OK;

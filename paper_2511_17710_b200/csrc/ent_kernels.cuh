@@ -194,103 +194,88 @@ __device__ __forceinline__ float sqrt_h_at(const GridDev &g, double x1, double x
     const double eR = exp(g.Rmin + x1 * g.dR), T = x2 * g.dT, r = g.r0 + eR;
     return (float)((g.dR * eR) * (g.dT * dtheta_dT(g.vt, T) * r) * (r * sin(theta_of_T(g.vt, T))));
 }
-// One pass over a tile of FT_I x FT_J lattice points, marching along x3 (3D): the in-plane part of the stencil,
-// P_k = sum_{di,dj} w(di) w(dj) J(i+di, j+dj, k), comes from a shared-memory copy of plane k (one global load per point and plane,
-// halo columns included), and the thread keeps P_{k-1}, P_k, P_{k+1} in registers: out_k = P_{k-1}/4 + P_k/2 + P_{k+1}/4
-// (f = (1/2)^(D + |di| + |dj| + |dk|) = w(di) w(dj) w(dk), Eqs. 9-11).  In 2D out = P.  A thread owns FT_V = 4 consecutive points
-// of a row (six shared values per stencil row: one 128-bit and one 64-bit load), the plane copies are double-buffered (one
-// barrier per plane).  A tile whose whole neighbourhood lies inside the lattice of a Cartesian grid loads without any boundary
-// logic; the others go through filter_fetch.
+// One pass, no shared memory and no barriers: a warp owns FT_W = 30 consecutive points of one lattice row (its 32 lanes sit on
+// x = i0 - 1 .. i0 + 30, the two outer lanes are halo) and marches along x3.  Per plane a lane loads the three values
+// J(x, j - 1 .. j + 1, k) (coalesced rows; the rows shared with the neighbouring warps of the CTA come from L1), filters them along
+// x2 in registers, gets its x1 neighbours by two shuffles, and keeps the in-plane sums P_{k-1}, P_k, P_{k+1} in registers:
+// out_k = P_{k-1}/4 + P_k/2 + P_{k+1}/4 (f = (1/2)^(D + |di| + |dj| + |dk|) = w(di) w(dj) w(dk), Eqs. 9-11); in 2D out = P.  The
+// loads of FT_U planes are issued together before the first of them is used.  A CTA whose whole neighbourhood lies inside the lattice of a
+// Cartesian grid loads without boundary logic (INTERIOR, compile time); the others go through filter_fetch.
 // mode 0: filter; 1: no convolution (scaling pass only); 2: copy.  blockIdx.z = component * nkc + chunk of FT_K planes.
-constexpr int FT_V = 4, FT_TX = 32, FT_I = FT_TX * FT_V, FT_J = 8, FT_K = 32, FT_ROW = FT_I + 4;   // row: halo, FT_I points, halo, pad
-__global__ void __launch_bounds__(FT_TX * FT_J) filter_pass_kernel(GridDev g, FilterGeom L, CurrentPtrs src, CurrentPtrs dst, int mode, int divide, int nkc) {
-    __shared__ __align__(16) float s[2][FT_J + 2][FT_ROW];
-    const int comp = blockIdx.z / nkc, kc = blockIdx.z - comp * nkc;
-    const int n0 = L.n[comp][0], n1 = L.n[comp][1], n2 = L.n[comp][2];
-    const int i0 = blockIdx.x * FT_I, j0 = blockIdx.y * FT_J, k0 = kc * FT_K;
-    if (i0 >= n0 || j0 >= n1 || k0 >= n2) return;                    // the grid is sized for the largest lattice
-    const int k1 = min(k0 + FT_K, n2);
-    const int tid = threadIdx.x, tx = tid % FT_TX, ty = tid / FT_TX;
-    const int i = i0 + FT_V * tx, j = j0 + ty;
-    const bool row = j < n1;
-    const float *A = src.c[comp];
-    float *O = dst.c[comp];
-    const long long P0 = g.P[0], P01 = g.D == 3 ? (long long)g.P[0] * g.P[1] : 0;
-    const long long at = (long long)(i + NG) + P0 * (j + NG) + (g.D == 3 ? P01 * NG : 0);     // (i, j, k = 0)
-    const bool axis_node = filter_on_axis(g, L, comp, j);
-    float sh[FT_V];
+constexpr int FT_W = 30, FT_J = 8, FT_K = 32, FT_TPB = 32 * FT_J, FT_U = 1;
+struct FilterRow { const float *A; int comp, x, j, k0, k1, n0, n1; long long P0, P01; };
+template <bool INTERIOR>
+__device__ __forceinline__ void filter_load3(const GridDev &g, const FilterGeom &L, const FilterRow &t, int k, float v[3]) {
+    if (INTERIOR) {
+        const float *p = t.A + ((long long)(t.x + NG) + t.P0 * (t.j - 1 + NG) + t.P01 * (k + NG));
+        v[0] = __ldg(p); v[1] = __ldg(p + t.P0); v[2] = __ldg(p + 2 * t.P0);
+    } else {
 #pragma unroll
-    for (int v = 0; v < FT_V; ++v) sh[v] = (divide && row && i + v < n0 && !axis_node) ? sqrt_h_at(g, i + v + (comp == 0 ? 0.5 : 0.0), j + (comp == 1 ? 0.5 : 0.0)) : 1.f;
-    auto emit = [&](int k, const float acc[FT_V]) {
-        if (!row) return;
+        for (int r = 0; r < 3; ++r) v[r] = (t.x <= t.n0 && t.j - 1 + r <= t.n1) ? filter_fetch(g, L, t.A, t.comp, t.x, t.j - 1 + r, k) : 0.f;
+    }
+}
+__device__ __forceinline__ float filter_in_plane(const float v[3]) {
+    const float c = 0.25f * v[0] + 0.5f * v[1] + 0.25f * v[2];                  // along x2, in the lane
+    const float l = __shfl_up_sync(0xffffffffu, c, 1), r = __shfl_down_sync(0xffffffffu, c, 1);
+    return 0.25f * l + 0.5f * c + 0.25f * r;                                    // along x1, across lanes (valid on lanes 1 .. 30)
+}
+template <bool INTERIOR, class EMIT>
+__device__ __forceinline__ void filter_march(const GridDev &g, const FilterGeom &L, const FilterRow &t, bool d3, EMIT &&emit) {
+    float v[3];
+    if (!d3) { filter_load3<INTERIOR>(g, L, t, 0, v); emit(0, filter_in_plane(v)); return; }
+    filter_load3<INTERIOR>(g, L, t, t.k0 - 1, v);
+    float Pm = filter_in_plane(v);
+    filter_load3<INTERIOR>(g, L, t, t.k0, v);
+    float Pc = filter_in_plane(v);
+    for (int kb = t.k0; kb < t.k1; kb += FT_U) {                     // FT_U planes per trip (1 measured best: 2 and 4 were 4 % and 12 % slower)
+        float w[FT_U][3];
 #pragma unroll
-        for (int v = 0; v < FT_V; ++v) {
-            if (i + v >= n0) continue;
-            float a = acc[v];
-            if (mode == 0 && comp == 2 && axis_node) a = 0.f;          // J^3(i, 0) = 0
-            if (divide && !axis_node) a /= sh[v];
-            O[at + v + P01 * k] = a;
+        for (int u = 0; u < FT_U; ++u) {
+            w[u][0] = w[u][1] = w[u][2] = 0.f;
+            if (kb + u < t.k1) filter_load3<INTERIOR>(g, L, t, kb + u + 1, w[u]);
         }
+#pragma unroll
+        for (int u = 0; u < FT_U; ++u) {
+            if (kb + u >= t.k1) break;
+            const float Pn = filter_in_plane(w[u]);
+            emit(kb + u, 0.25f * Pm + 0.5f * Pc + 0.25f * Pn);
+            Pm = Pc; Pc = Pn;
+        }
+    }
+}
+__global__ void __launch_bounds__(FT_TPB) filter_pass_kernel(GridDev g, FilterGeom L, CurrentPtrs src, CurrentPtrs dst, int mode, int divide, int nkc) {
+    FilterRow t;
+    t.comp = blockIdx.z / nkc;
+    const int kc = blockIdx.z - t.comp * nkc;
+    const int n2 = L.n[t.comp][2];
+    t.n0 = L.n[t.comp][0]; t.n1 = L.n[t.comp][1];
+    const int lane = threadIdx.x & 31, i0 = blockIdx.x * FT_W, j0 = blockIdx.y * FT_J;
+    t.k0 = kc * FT_K;
+    if (i0 >= t.n0 || j0 >= t.n1 || t.k0 >= n2) return;              // the grid is sized for the largest lattice
+    t.k1 = min(t.k0 + FT_K, n2);
+    t.x = i0 - 1 + lane; t.j = j0 + (threadIdx.x >> 5);
+    t.A = src.c[t.comp];
+    float *O = dst.c[t.comp];
+    t.P0 = g.P[0]; t.P01 = g.D == 3 ? (long long)g.P[0] * g.P[1] : 0;
+    const bool mine = lane >= 1 && lane <= FT_W && t.x < t.n0 && t.j < t.n1;    // this lane owns the lattice point (x, j)
+    const long long at = (long long)(t.x + NG) + t.P0 * (t.j + NG) + (g.D == 3 ? t.P01 * NG : 0);     // (x, j, k = 0)
+    const bool axis_node = filter_on_axis(g, L, t.comp, t.j);
+    const float sh = (divide && mine && !axis_node) ? sqrt_h_at(g, t.x + (t.comp == 0 ? 0.5 : 0.0), t.j + (t.comp == 1 ? 0.5 : 0.0)) : 1.f;
+    const bool zero = mode == 0 && t.comp == 2 && axis_node;                    // J^3(i, 0) = 0
+    auto emit = [&](int k, float a) {
+        if (!mine) return;
+        if (zero) a = 0.f;
+        if (divide && !axis_node) a /= sh;
+        O[at + t.P01 * k] = a;
     };
     if (mode != 0) {
-        if (row)
-            for (int k = k0; k < k1; ++k) {
-                float a[FT_V];
-#pragma unroll
-                for (int v = 0; v < FT_V; ++v) a[v] = i + v < n0 ? A[at + v + P01 * k] : 0.f;
-                emit(k, a);
-            }
+        if (mine) for (int k = t.k0; k < t.k1; ++k) emit(k, t.A[at + t.P01 * k]);
         return;
     }
     const bool d3 = g.D == 3;
-    const bool interior = g.kind == ENT_CART && i0 >= 1 && i0 + FT_I + 1 <= n0 && j0 >= 1 && j0 + FT_J + 1 <= n1 && (!d3 || (k0 >= 1 && k1 + 1 <= n2));
-    auto load_plane = [&](int k, int buf) {                             // s[buf][jj][ii] = J(i0 - 1 + ii, j0 - 1 + jj, k)
-        for (int e = tid; e < (FT_J + 2) * (FT_I + 2); e += FT_TX * FT_J) {
-            const int jj = e / (FT_I + 2), ii = e - jj * (FT_I + 2);
-            const int q0 = i0 - 1 + ii, q1 = j0 - 1 + jj;
-            float v = 0.f;
-            if (interior) v = A[(long long)(q0 + NG) + P0 * (q1 + NG) + P01 * (k + NG)];
-            else if (q0 <= n0 && q1 <= n1) v = filter_fetch(g, L, A, comp, q0, q1, k);
-            s[buf][jj][ii] = v;
-        }
-    };
-    auto in_plane = [&](int buf, float P[FT_V]) {
-        float r[3][FT_V];
-#pragma unroll
-        for (int rr = 0; rr < 3; ++rr) {
-            const float4 a = *reinterpret_cast<const float4 *>(&s[buf][ty + rr][FT_V * tx]);
-            const float2 b = *reinterpret_cast<const float2 *>(&s[buf][ty + rr][FT_V * tx + 4]);
-            const float v[6] = { a.x, a.y, a.z, a.w, b.x, b.y };
-#pragma unroll
-            for (int q = 0; q < FT_V; ++q) r[rr][q] = 0.25f * v[q] + 0.5f * v[q + 1] + 0.25f * v[q + 2];
-        }
-#pragma unroll
-        for (int q = 0; q < FT_V; ++q) P[q] = 0.25f * r[0][q] + 0.5f * r[1][q] + 0.25f * r[2][q];
-    };
-    if (!d3) {
-        load_plane(0, 0);
-        __syncthreads();
-        float P[FT_V];
-        in_plane(0, P);
-        emit(0, P);
-        return;
-    }
-    float Pm[FT_V], Pc[FT_V], Pn[FT_V];
-    load_plane(k0 - 1, 0);
-    load_plane(k0, 1);
-    __syncthreads();
-    in_plane(0, Pm); in_plane(1, Pc);
-    __syncthreads();                                                 // both initial copies have been read
-    for (int k = k0; k < k1; ++k) {
-        const int buf = (k - k0) & 1;                                // plane k + 1 goes where plane k - 1 was: everyone has passed the barrier
-        load_plane(k + 1, buf);                                      // that followed its last read (double buffering, one barrier per plane)
-        __syncthreads();
-        in_plane(buf, Pn);
-        float out[FT_V];
-#pragma unroll
-        for (int q = 0; q < FT_V; ++q) { out[q] = 0.25f * Pm[q] + 0.5f * Pc[q] + 0.25f * Pn[q]; Pm[q] = Pc[q]; Pc[q] = Pn[q]; }
-        emit(k, out);
-    }
+    const bool interior = g.kind == ENT_CART && i0 >= 1 && i0 + FT_W + 1 <= t.n0 && j0 >= 1 && j0 + FT_J + 1 <= t.n1 &&
+                          (!d3 || (t.k0 >= 1 && t.k1 + 1 <= n2));
+    if (interior) filter_march<true>(g, L, t, d3, emit); else filter_march<false>(g, L, t, d3, emit);
 }
 
 // ---- N4: tag sort: stable partition, alive particles first ----
