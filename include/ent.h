@@ -246,6 +246,11 @@ enum {
                                   particle (increments of the code coordinates added to the in-cell offsets; same mathematics as
                                   P:147-153 + P:285-327); 1 = fp64 coordinate maps through the global Cartesian frame (the literal
                                   round trip; slower, kept for comparison).  Takes effect at once. */
+    ENT_OPT_SORT_STAGING = 8,  /* 1 = the full form of ent_sort stages the records through a 32-byte-per-particle array-of-structures side buffer in
+                                  the ctx (allocated on first use: may synchronise): every record is written as one full DRAM sector and unpacked
+                                  by a second, coalesced pass.  For blocks that arrive in an unrelated (shuffled) order, where scattering eight
+                                  4-byte arrays costs a sector read-modify-write per word; slower than the default (0) for blocks that are nearly
+                                  ordered already.  Takes effect at once. */
     ENT_OPT_SORT_MODE = 5      /* 0 = auto (incremental re-bin when `in` is itself a block ent_sort produced and key_offsets is NULL),
                                   1 = always the full cell-level counting sort,
                                   2 = like 0, but the re-bin does not order the particles that stay in a tile by cell */

@@ -17,7 +17,7 @@ CART, SPH, QSPH = 0, 1, 2
 PERIODIC, ABSORB, AXIS = 0, 1, 2
 NGHOST = 2
 OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM = 0, -1, -2, -3, -4
-OPT_STEP_IMPL, OPT_TILE_1, OPT_TILE_2, OPT_TILE_3, OPT_SORT_MODE, OPT_CURV_FP64, OPT_PUSHER = 1, 2, 3, 4, 5, 6, 7
+OPT_STEP_IMPL, OPT_TILE_1, OPT_TILE_2, OPT_TILE_3, OPT_SORT_MODE, OPT_CURV_FP64, OPT_PUSHER, OPT_SORT_STAGING = 1, 2, 3, 4, 5, 6, 7, 8
 (STAT_TILE_1, STAT_TILE_2, STAT_TILE_3, STAT_NKEYS, STAT_NTILES, STAT_LAUNCHES, STAT_BAD_MOVES, STAT_STRAYS,
  STAT_SCRATCH_BYTES, STAT_LAST_STEP_TILED, STAT_LAST_SORT_REBIN, STAT_SLOT_ERRORS, STAT_CARRIES, STAT_GLOBAL_ADDS) = range(1, 15)
 

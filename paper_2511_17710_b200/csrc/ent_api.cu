@@ -39,6 +39,8 @@ struct ent_ctx {
     void *hbuf = nullptr; size_t hbuf_cap = 0;
     void *fbuf = nullptr; size_t fbuf_cap = 0;          // second set of current arrays for the filter passes
     void *cbuf = nullptr; size_t cbuf_cap = 0;          // flags and positions of ent_compact
+    void *sbuf = nullptr; size_t sbuf_cap = 0;          // array-of-structures staging of the full sort (ENT_OPT_SORT_STAGING)
+    int sort_staging = 0;
     size_t side_bytes = 0;
     // the blocks ent_sort / ent_step_sorted produced: each keeps its own layout so that several species stay sorted at a time
     struct SortedBlock { const int32_t *cell = nullptr; long long n = -1; int32_t *tile_off = nullptr; float *tile_wmax = nullptr;
@@ -160,7 +162,7 @@ extern "C" int ent_destroy(ent_ctx *ctx) {
     if (!ctx) return ENT_EINVAL;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    cudaFree(ctx->counters); cudaFree(ctx->pool); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf); cudaFree(ctx->fbuf); cudaFree(ctx->cbuf);
+    cudaFree(ctx->counters); cudaFree(ctx->pool); cudaFree(ctx->oldbuf); cudaFree(ctx->hbuf); cudaFree(ctx->fbuf); cudaFree(ctx->cbuf); cudaFree(ctx->sbuf);
     cudaGetLastError();
     delete ctx;
     return ENT_OK;
@@ -669,8 +671,16 @@ extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *ou
     }
     if ((rc = exclusive_scan(ctx, ctx->count, nkeys, ctx->offsets, ctx->cursor))) return rc;
     if (n > 0) {
-        sort_scatter_kernel<<<nblk(n), TPB, 0, ctx->stream>>>(ctx->keys, ctx->cursor, pp(in), pp(out), n, g.D, g.kind != ENT_CART);
-        if ((rc = launch_check(ctx, "sort_scatter_kernel"))) return rc;
+        if (ctx->sort_staging) {                       // unordered input: full-sector writes to a side buffer, then a coalesced unpack
+            if ((rc = ensure(ctx, &ctx->sbuf, &ctx->sbuf_cap, (size_t)n * 32))) return rc;
+            sort_scatter_aos_kernel<<<nblk(n), TPB, 0, ctx->stream>>>(ctx->keys, ctx->cursor, pp(in), (float4 *)ctx->sbuf, out->tag, n, g.D, g.kind != ENT_CART);
+            if ((rc = launch_check(ctx, "sort_scatter_aos_kernel"))) return rc;
+            sort_unpack_aos_kernel<<<nblk(n), TPB, 0, ctx->stream>>>((const float4 *)ctx->sbuf, pp(out), n, g.D, g.kind != ENT_CART);
+            if ((rc = launch_check(ctx, "sort_unpack_aos_kernel"))) return rc;
+        } else {
+            sort_scatter_kernel<<<nblk(n), TPB, 0, ctx->stream>>>(ctx->keys, ctx->cursor, pp(in), pp(out), n, g.D, g.kind != ENT_CART);
+            if ((rc = launch_check(ctx, "sort_scatter_kernel"))) return rc;
+        }
         // in has no tags but out has: every particle is alive (ent.h)
         if (!in->tag && out->tag) CK(cudaMemsetAsync(out->tag, 1, (size_t)n, ctx->stream));
     }
@@ -786,6 +796,9 @@ extern "C" int ent_set_option(ent_ctx *ctx, int key, int64_t value) {
         case ENT_OPT_PUSHER:
             if (value < 0 || value > 1) return fail(ctx, ENT_EINVAL, "ENT_OPT_PUSHER must be 0 (Boris) or 1 (Vay)");
             ctx->pusher = (int)value; ctx->g.pusher = (int)value; return ENT_OK;
+        case ENT_OPT_SORT_STAGING:
+            if (value < 0 || value > 1) return fail(ctx, ENT_EINVAL, "ENT_OPT_SORT_STAGING must be 0 or 1");
+            ctx->sort_staging = (int)value; return ENT_OK;
         case ENT_OPT_CURV_FP64:
             if (value < 0 || value > 1) return fail(ctx, ENT_EINVAL, "ENT_OPT_CURV_FP64 must be 0 or 1");
             ctx->curv_f64 = (int)value; ctx->g.curv_f64 = (int)value; return ENT_OK;

@@ -421,6 +421,31 @@ __global__ void __launch_bounds__(TPB) sort_scatter_kernel(const int32_t *keys, 
 }
 
 
+// Staged form of the scatter for blocks that arrive in an unrelated order (ENT_OPT_SORT_STAGING): scattering eight 4-byte arrays
+// to random slots writes one word of every 32-byte DRAM sector it touches (a read-modify-write of the sector per word: measured
+// 131 ms per species on the shuffled C4 block).  Here the record is packed to 32 bytes and written to its slot of an
+// array-of-structures side buffer as ONE full sector (two 16-byte stores), and a second, fully coalesced pass unpacks the side
+// buffer into the caller's arrays.  Record: cell, d0, d1, (d2 | phi | 0), u0, u1, u2, w.
+__global__ void __launch_bounds__(TPB) sort_scatter_aos_kernel(const int32_t *keys, int32_t *cursor, PartPtrs in, float4 *aos, uint8_t *tag_out,
+                                                               long long n, int D, int axisym) {
+    long long p = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (p >= n) return;
+    const long long dst = atomicAdd(cursor + keys[p], 1);
+    const float third = D == 3 ? in.d[2][p] : (axisym ? in.phi[p] : 0.f);
+    aos[2 * dst] = make_float4(__int_as_float(in.cell[p]), in.d[0][p], in.d[1][p], third);
+    aos[2 * dst + 1] = make_float4(in.u[0][p], in.u[1][p], in.u[2][p], in.w[p]);
+    if (in.tag) tag_out[dst] = in.tag[p];
+}
+__global__ void __launch_bounds__(TPB) sort_unpack_aos_kernel(const float4 *aos, PartPtrs out, long long n, int D, int axisym) {
+    long long p = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (p >= n) return;
+    const float4 a = aos[2 * p], b = aos[2 * p + 1];
+    out.cell[p] = __float_as_int(a.x);
+    out.d[0][p] = a.y; out.d[1][p] = a.z;
+    if (D == 3) out.d[2][p] = a.w; else if (axisym) out.phi[p] = a.w;
+    out.u[0][p] = b.x; out.u[1][p] = b.y; out.u[2][p] = b.z; out.w[p] = b.w;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // S10, incremental form ("re-bin"): the input block is tile-contiguous already (a previous ent_sort produced it) and its
 // particles have drifted a few cells, so almost all of them stay in their tile and the rest go to one of the 3^D - 1

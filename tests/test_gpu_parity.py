@@ -292,8 +292,9 @@ def _host_keys(synth, bind, ctx, g, cell):
     return synth.sort_key(g, synth.unpack_cell(g, cell.cpu()), T).numpy().astype(np.int32), T
 
 
+@pytest.mark.parametrize("staging", [0, 1])
 @pytest.mark.parametrize("name", ["C1", "C3/8", "C4/16-shuffled", "C5/32", "ABS3", "ABS2"])
-def test_full_sort_passes_the_oracle_checker(env, name):
+def test_full_sort_passes_the_oracle_checker(env, name, staging):
     """S10: ent_sort (full form) with a key_offsets output.  Keys are recomputed on the host from out.cell; the ORACLE's checker
     (orc_sort_check: non-decreasing keys, offsets = exclusive scan of the key histogram) must accept them, and the records must
     be a permutation of the input (every array permuted alike)."""
@@ -307,7 +308,11 @@ def test_full_sort_passes_the_oracle_checker(env, name):
         pe = P.species_to_ent(bind, synth, g, sp, "cuda")
         ps = pe.empty_like()
         ko = torch.full((nkeys + 1,), -7, dtype=torch.int32, device="cuda")
-        bind.ent_sort(ctx, pe, ps, ko)
+        bind.ent_set_option(ctx, bind.OPT_SORT_STAGING, staging)      # 1: records staged through the 32-byte side buffer
+        try:
+            bind.ent_sort(ctx, pe, ps, ko)
+        finally:
+            bind.ent_set_option(ctx, bind.OPT_SORT_STAGING, 0)
         torch.cuda.synchronize()
         assert bind.ent_get_stat(ctx, bind.STAT_LAST_SORT_REBIN) == 0
         _match_perm(g, pe, ps)
