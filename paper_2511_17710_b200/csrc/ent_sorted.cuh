@@ -169,7 +169,7 @@ step_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
         float Sc = (qmax > 0.f && qmax < 1e37f) ? FIXED_ONE / qmax : 0.f;
         if (!(Sc > 1e-30f && Sc < 1e30f)) Sc = 0.f;
         invSc = Sc > 0.f ? 1.0f / Sc : 0.f;
-        T.Sc = Sc; T.wguard = Sc > 0.f ? (ENT_FIXED_MAGIC ? wm : 60.0f * wm) : -1.0f;   // magic conversion: |value| must stay below 2^22
+        T.Sc = Sc; T.wguard = Sc > 0.f ? 60.0f * wm : -1.0f;
     }
     T.cc.J = A.J.c; T.cc.P0 = g.P[0]; T.cc.P01 = g.P[0] * g.P[1]; T.cc.unit = 4294967296.0f * invSc;
     T.cc.JX = G::JX; T.cc.JY = G::JY; T.cc.JNP = G::JNP; T.cc.carries = A.counters + 4;

@@ -176,19 +176,8 @@ __device__ __noinline__ void stray_step(const TiledArgs &A, long long p, int sp 
 // particles' worth of current on one node) is detected from the value the atomic returns and carried straight into
 // the global array as +-2^32 / 2^k, so the sum stays exact for any input.
 // ---------------------------------------------------------------------------------------------------------
-// fixed-point conversion: round(value) as an integer.  ENT_FIXED_MAGIC: value + 1.5 * 2^23 in fp32 leaves round-to-nearest-even(value)
-// in the low mantissa bits (|value| < 2^22): one FADD + one IADD on the full-rate pipes instead of F2I on the quarter-rate XU pipe
-// behind the MIO queue.  The largest contribution then gets 22 bits instead of 24.
-#ifndef ENT_FIXED_MAGIC
-#define ENT_FIXED_MAGIC 0
-#endif
-#if ENT_FIXED_MAGIC
-constexpr float FIXED_ONE = 4194000.0f;
-__device__ __forceinline__ int fixed_rn(float v) { return __float_as_int(v + 12582912.0f) - 0x4B400000; }
-#else
-constexpr float FIXED_ONE = 16777000.0f;
+constexpr float FIXED_ONE = 16777000.0f;     // the largest contribution of a tile in fixed-point units (just below 2^24)
 __device__ __forceinline__ int fixed_rn(float v) { return __float2int_rn(v); }
-#endif
 struct CarryCtx { float *const *J; long long gbase; int P0, P01; float unit; int JX, JY, JNP; unsigned long long *carries; };
 
 __device__ __noinline__ void carry_fix(const CarryCtx &c, int comp, int off, int positive) {
@@ -232,7 +221,10 @@ __device__ __forceinline__ void tile_segment(int *sJ, const CarryCtx &cc, int ba
 #pragma unroll
     for (int a = 0; a < 3; ++a) { Dv[a] = e[a] - s[a]; W[a] = 0.5f * (e[a] + s[a]); }
     if (D == 3) {
-        const int st[3] = { 1, G::JX, G::JX * G::JY };
+        // the twelve adds of the segment are all issued before the first returned value is looked at; one conservative test
+        // (|old| >= 2^30 somewhere) covers the twelve carries, the exact per-add test runs only then
+        constexpr int st[3] = { 1, G::JX, G::JX * G::JY };
+        int v[12], old[12];
 #pragma unroll
         for (int comp = 0; comp < 3; ++comp) {
             const int a = (comp + 1) % 3, bb = (comp + 2) % 3;
@@ -240,7 +232,22 @@ __device__ __forceinline__ void tile_segment(int *sJ, const CarryCtx &cc, int ba
             const float ta = QD * W[a], tb = QD * W[bb];
             const float v11 = fmaf(ta, W[bb], QD * (Dv[a] * Dv[bb] * (1.0f / 12.0f)));
             const float v10 = ta - v11, v01 = tb - v11, v00 = (QD - ta) - v01;
-            acc_fixed4(sJ, cc, comp, base, base + st[a], base + st[bb], base + st[a] + st[bb], v00, v10, v01, v11);
+            v[4 * comp] = fixed_rn(v00); v[4 * comp + 1] = fixed_rn(v10); v[4 * comp + 2] = fixed_rn(v01); v[4 * comp + 3] = fixed_rn(v11);
+            int *Jc = sJ + comp * cc.JNP + base;
+            old[4 * comp] = atomicAdd(Jc, v[4 * comp]); old[4 * comp + 1] = atomicAdd(Jc + st[a], v[4 * comp + 1]);
+            old[4 * comp + 2] = atomicAdd(Jc + st[bb], v[4 * comp + 2]); old[4 * comp + 3] = atomicAdd(Jc + st[a] + st[bb], v[4 * comp + 3]);
+        }
+        unsigned flag = 0u;
+#pragma unroll
+        for (int k = 0; k < 12; ++k) flag |= (unsigned)old[k] + 0x40000000u;
+        if ((int)flag < 0) {
+#pragma unroll
+            for (int k = 0; k < 12; ++k) {
+                const int comp = k / 4, a = (comp + 1) % 3, bb = (comp + 2) % 3;
+                const int off = base + ((k & 1) ? st[a] : 0) + ((k & 2) ? st[bb] : 0);
+                const int nw = old[k] + v[k];
+                if (((old[k] ^ nw) & (v[k] ^ nw)) < 0) carry_fix(cc, comp, off, v[k] > 0);
+            }
         }
     } else {
         const float q0 = Q * Dv[0], q1 = Q * Dv[1];
@@ -463,7 +470,7 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
         if (PAIR) {                                              // one scale for both species: the larger |q| wmax
             const float wm2 = A.tile_wmax2[tile], qw2 = fabsf(A.q2) * wm2;
             const float qwm = fmaxf(qw1, qw2);
-            wguard2 = (ENT_FIXED_MAGIC ? 1.0f : 60.0f) * (fabsf(A.q2) > 0.f ? qwm / fabsf(A.q2) : 0.f);
+            wguard2 = 60.0f * (fabsf(A.q2) > 0.f ? qwm / fabsf(A.q2) : 0.f);
             wm = fabsf(A.q) > 0.f ? qwm / fabsf(A.q) : 0.f;
             qw1 = qwm;
         }
@@ -471,7 +478,7 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
         float Sc = (qmax > 0.f && qmax < 1e37f) ? FIXED_ONE / qmax : 0.f;
         if (!(Sc > 1e-30f && Sc < 1e30f)) Sc = 0.f;
         invSc = Sc > 0.f ? 1.0f / Sc : 0.f;
-        T.Sc = Sc; T.wguard = Sc > 0.f ? (ENT_FIXED_MAGIC ? wm : 60.0f * wm) : -1.0f;   // magic conversion: |value| must stay below 2^22
+        T.Sc = Sc; T.wguard = Sc > 0.f ? 60.0f * wm : -1.0f;
         if (!(Sc > 0.f)) wguard2 = -1.0f;
     }
     T.cc.J = A.J.c; T.cc.P0 = g.P[0]; T.cc.P01 = g.P[0] * g.P[1]; T.cc.unit = 4294967296.0f * invSc;
