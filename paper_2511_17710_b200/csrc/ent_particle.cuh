@@ -47,7 +47,7 @@ __device__ __forceinline__ void push_from_fields_geo(const GridDev &g, const GEO
         // (r, theta, phi)-hat at the old point and turned into increments of the code coordinates, which are added to the in-cell
         // offsets exactly as on the Cartesian grids; no absolute position is ever formed in fp32.  Same mathematics as the
         // global-Cartesian round trip of P:147-153, P:285-327 (the oracle's), which in fp32 would lose the displacement.
-        SphF s;
+        SphF s{};
         if constexpr (KIND != ENT_CART) s = sphf_of_code<KIND>(g, geo, i[0], d[0], i[1], d[1]);
         float sp, cp;
         sincosf(phi, &sp, &cp);
@@ -243,7 +243,7 @@ __device__ __forceinline__ float half_qw_v3(const GridDev &g, const GEO &geo, co
         float dphi = phi1 - phi0;                                             // shorter arc
         if (dphi > 3.14159265358979f) dphi -= TWO_PI_F;
         if (dphi <= -3.14159265358979f) dphi += TWO_PI_F;
-        SphF s;
+        SphF s{};
         if constexpr (KIND != ENT_CART) s = sphf_of_code<KIND>(g, geo, i0[0], 0.5f * (a[0] + b[0]), i0[1], 0.5f * (a[1] + b[1]));
         if (s.sh3 < 1e-12f) return 0.f;
         float sp, cp;
