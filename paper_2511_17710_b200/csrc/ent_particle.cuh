@@ -197,6 +197,11 @@ __device__ __forceinline__ void red_global_f32(float *p, float v) {
 struct GlobalAcc {
     float *const *J;
     __device__ __forceinline__ void add(int comp, long long idx, float v) const { red_global_f32(J[comp] + idx, v); }
+    // four contributions at once (an accumulator may treat them together: the shared-memory tile tests their carries with one branch)
+    __device__ __forceinline__ void add4(int c0, long long i0, float v0, int c1, long long i1, float v1,
+                                         int c2, long long i2, float v2, int c3, long long i3, float v3) const {
+        add(c0, i0, v0); add(c1, i1, v1); add(c2, i2, v2); add(c3, i3, v3);
+    }
 };
 
 template <int D, class Acc>
@@ -221,15 +226,9 @@ __device__ __forceinline__ void deposit_segment(const Acc &acc, long long base, 
         }
     } else {
         float q0 = Q * Dv[0], q1 = Q * Dv[1];
-        acc.add(0, base, q0 * (1.0f - W[1]));
-        acc.add(0, base + s1, q0 * W[1]);
-        acc.add(1, base, q1 * (1.0f - W[0]));
-        acc.add(1, base + 1, q1 * W[0]);
+        acc.add4(0, base, q0 * (1.0f - W[1]), 0, base + s1, q0 * W[1], 1, base, q1 * (1.0f - W[0]), 1, base + 1, q1 * W[0]);
         float h1 = hv * W[1], h0 = hv - h1;                                   // out-of-plane, velocity form (G8)
-        acc.add(2, base, h0 * (1.0f - W[0]));
-        acc.add(2, base + 1, h0 * W[0]);
-        acc.add(2, base + s1, h1 * (1.0f - W[0]));
-        acc.add(2, base + s1 + 1, h1 * W[0]);
+        acc.add4(2, base, h0 * (1.0f - W[0]), 2, base + 1, h0 * W[0], 2, base + s1, h1 * (1.0f - W[0]), 2, base + s1 + 1, h1 * W[0]);
     }
 }
 

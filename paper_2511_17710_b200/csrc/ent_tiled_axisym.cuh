@@ -35,6 +35,25 @@ struct TileAcc {                         // Acc of deposit_particle_at: fixed-po
         if (fabsf(sv) < 1.0e9f) acc_fixed(sJ, *cc, comp, (int)idx, sv);
         else if (sv == sv) global_add(*cc, comp, (int)idx, v);
     }
+    // four contributions: if all fit the fixed-point range (the rule), the four atomics are issued together and one conservative
+    // test covers their carries (|old| >= 2^30 somewhere; a contribution is below 2^30 in magnitude); else one by one
+    __device__ __forceinline__ void add4(int c0, long long i0, float v0, int c1, long long i1, float v1,
+                                         int c2, long long i2, float v2, int c3, long long i3, float v3) const {
+        const float s0 = v0 * Sc, s1 = v1 * Sc, s2 = v2 * Sc, s3 = v3 * Sc;
+        if (fmaxf(fmaxf(fabsf(s0), fabsf(s1)), fmaxf(fabsf(s2), fabsf(s3))) < 1.0e9f) {       // false for NaN as well
+            const int JNP = cc->JNP;
+            const int w0 = fixed_rn(s0), w1 = fixed_rn(s1), w2 = fixed_rn(s2), w3 = fixed_rn(s3);
+            const int a0 = atomicAdd(sJ + c0 * JNP + (int)i0, w0), a1 = atomicAdd(sJ + c1 * JNP + (int)i1, w1),
+                      a2 = atomicAdd(sJ + c2 * JNP + (int)i2, w2), a3 = atomicAdd(sJ + c3 * JNP + (int)i3, w3);
+            if ((int)((((unsigned)a0 + 0x40000000u) | ((unsigned)a1 + 0x40000000u)) | (((unsigned)a2 + 0x40000000u) | ((unsigned)a3 + 0x40000000u))) < 0) {
+                const int n0 = a0 + w0, n1 = a1 + w1, n2 = a2 + w2, n3 = a3 + w3;
+                if (((a0 ^ n0) & (w0 ^ n0)) < 0) carry_fix(*cc, c0, (int)i0, w0 > 0);
+                if (((a1 ^ n1) & (w1 ^ n1)) < 0) carry_fix(*cc, c1, (int)i1, w1 > 0);
+                if (((a2 ^ n2) & (w2 ^ n2)) < 0) carry_fix(*cc, c2, (int)i2, w2 > 0);
+                if (((a3 ^ n3) & (w3 ^ n3)) < 0) carry_fix(*cc, c3, (int)i3, w3 > 0);
+            }
+        } else { add(c0, i0, v0); add(c1, i1, v1); add(c2, i2, v2); add(c3, i3, v3); }
+    }
 };
 
 template <int KIND>
