@@ -12,6 +12,15 @@ constexpr int NG = ENT_NGHOST;
 constexpr double PI_D = 3.14159265358979323846264338327950288;
 constexpr float TWO_PI_F = 6.28318548202514648f;   // float nearest to 2*pi (slightly above it)
 constexpr float TWO_PI_LO = 1.74845553e-7f;         // TWO_PI_F - 2*pi
+// sin and cos of an azimuth in [-pi, 3 pi] (phi or a midpoint of two phis): the argument is shifted by pi into the range where
+// MUFU.SIN / MUFU.COS (__sincosf) are good to 2^-21.4 absolute, sin(x) = -sin(x - pi).  5e-7 on a rotation of the field basis and of
+// the displacement is 2.5e-7 cells and 5e-7 of |E|, |B| at most: inside the 1e-5 bars with the margin the parity tests print.
+__device__ __forceinline__ void sincos_azimuth(float phi, float &s, float &c) {
+    float x = phi - 3.14159274101257324f;
+    if (x > 3.14159274101257324f) x -= TWO_PI_F;
+    __sincosf(x, &s, &c);
+    s = -s; c = -c;
+}
 
 // Grid + metric constants, passed to kernels by value (the paper passes its metric object by value too).
 struct GridDev {

@@ -50,7 +50,7 @@ __device__ __forceinline__ void push_from_fields_geo(const GridDev &g, const GEO
         SphF s{};
         if constexpr (KIND != ENT_CART) s = sphf_of_code<KIND>(g, geo, i[0], d[0], i[1], d[1]);
         float sp, cp;
-        sincosf(phi, &sp, &cp);
+        sincos_azimuth(phi, sp, cp);
         {   // step 4: tetrad (at the particle, G2) then rotation (r,th,phi)-hat -> (x,y,z)-hat
             float Ar = s.sh1 * EB[0], At = s.sh2 * EB[1], Ap = s.sh3 * EB[2];
             E[0] = Ar * s.st * cp + At * s.ct * cp - Ap * sp;
@@ -246,7 +246,7 @@ __device__ __forceinline__ float half_qw_v3(const GridDev &g, const GEO &geo, co
         if constexpr (KIND != ENT_CART) s = sphf_of_code<KIND>(g, geo, i0[0], 0.5f * (a[0] + b[0]), i0[1], 0.5f * (a[1] + b[1]));
         if (s.sh3 < 1e-12f) return 0.f;
         float sp, cp;
-        sincosf(phi0 + 0.5f * dphi, &sp, &cp);
+        sincos_azimuth(phi0 + 0.5f * dphi, sp, cp);
         return 0.5f * qw * (((u[1] * cp - u[0] * sp) * ig) / s.sh3);
     }
     double dphi = (double)phi1 - (double)phi0;
