@@ -114,6 +114,7 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
     __shared__ CarryCtx s_cc;
     __shared__ float s_gx[TX + 4];
     __shared__ NodeY s_gy[TY + 4];
+    __shared__ float s_h[6];
     const GridDev &g = A.g;
     const int tid = threadIdx.x;
     const int tile = find_tile(A.chunk_off, A.ntiles, blockIdx.x);
@@ -140,14 +141,16 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
         // log-r grids, where a particle moves ~1e-3 cells per step.  J^3 = q w v^phi / sqrt(h33) is of the same size except next
         // to the axis, where the contributions that do not fit go to the global array (TileAcc).
         const float wm = A.tile_wmax[tile];
-        double x1a = fmax(0.0, (double)o0 - 1.0), x1b = fmin((double)g.N[0], (double)(o0 + TX) + 1.0);
-        double x2a = fmax(0.0, (double)o1 - 1.0), x2b = fmin((double)g.N[1], (double)(o1 + TY) + 1.0);
-        double hmin = 1e300;
-        for (int c = 0; c < 6; ++c) {
+        if (tid >= 64 && tid < 70) {                                     // six sample points of the tile, one thread each (fp64 maps)
+            const int c = tid - 64;
+            const double x1a = fmax(0.0, (double)o0 - 1.0), x1b = fmin((double)g.N[0], (double)(o0 + TX) + 1.0);
+            const double x2a = fmax(0.0, (double)o1 - 1.0), x2b = fmin((double)g.N[1], (double)(o1 + TY) + 1.0);
             Sph sp = sph_of_code<KIND>(g, (c & 1) ? x1b : x1a, c < 2 ? x2a : (c < 4 ? x2b : 0.5 * (x2a + x2b)));
-            hmin = fmin(hmin, fmin(sp.sh1, sp.sh2));
+            s_h[c] = (float)fmin(sp.sh1, sp.sh2);
         }
-        float rate = fminf(A.inv_dt, (float)(1.25 / hmin));              // 1/dt: |D| <= 1 always
+        __syncthreads();
+        const float hmin = fminf(fminf(fminf(s_h[0], s_h[1]), fminf(s_h[2], s_h[3])), fminf(s_h[4], s_h[5]));
+        float rate = fminf(A.inv_dt, 1.25f / hmin);                      // 1/dt: |D| <= 1 always
         float qmax = fabsf(A.q) * wm * fmaxf(rate, 1e-30f) * 1.0834f;
         Sc = (qmax > 0.f && qmax < 1e37f) ? 67100000.0f / qmax : 0.f;       // 26 bits: weights vary strongly inside a tile of a coarse grid
         if (!(Sc > 1e-30f && Sc < 1e30f)) Sc = 0.f;
