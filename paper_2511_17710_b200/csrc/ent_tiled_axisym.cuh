@@ -8,11 +8,6 @@
 
 namespace ent {
 
-struct BoxLoader {                       // gather() hands over the index inside a (FX x FY) box addressed like a padded array
-    const float *sF; int fnp;
-    __device__ __forceinline__ float operator()(int c, long long idx) const { return sF[c * fnp + (int)idx]; }
-};
-
 // a contribution that does not fit the tile's fixed-point range goes straight to the global array (J^3 = q w v^phi / (r sin theta)
 // is unbounded towards the axis, reading G8)
 __device__ __noinline__ void global_add(const CarryCtx &c, int comp, int off, float v) {
@@ -163,7 +158,6 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
     }
     __syncthreads();
     const TileAcc acc{sJ + (tid & (AXI_NCOPY - 1)) * X::CSTRIDE, &s_cc, Sc};
-    const BoxLoader ld{sF, G::FNP};
     const TileGeo geo{s_gx, s_gy, o0, o1};
     const float wguard = Sc > 0.f ? 60.0f * A.tile_wmax[tile] : -1.0f;
     bool waited = false;
@@ -184,10 +178,9 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
         if (!local) { defer_stray(A, p, [&] { stray_step_axisym<KIND>(A, p); }); continue; }
         // gather from the box: the box is addressed like a padded array of extents FX x FY whose "active" origin is the tile
         // origin, so the cell's coordinates in it are (b - 2)
-        GridDev gb = g; gb.P[0] = G::FX; gb.P[1] = G::FY; gb.P[2] = 1;
-        const int ib[3] = { b0 - NG, b1 - NG, 0 };
+        const int ib[3] = { b0 - NG, b1 - NG, 0 }, bb[3] = { b0, b1, 0 };
         float EB[6];
-        gather<2>(gb, ld, ib, d, EB);
+        gather_box<2, G::FX, G::FY, G::FNP>(sF, bb, d, EB);        // the gather of ent_tiled.cuh (packed pairs), same arithmetic as ent_dev.cuh
         const int i0[3] = { i[0], i[1], 0 };
         const float a[3] = { d[0], d[1], 0.f };
         const float phi0 = phi;
