@@ -12,6 +12,8 @@ namespace ent {
 // push_from_fields: everything after the gather (EB = the six interpolated contravariant components).
 struct NoGeo {};                          // Cartesian grids need no node factors
 
+// The divisions of the fp32 displacement form are MUFU.RCP quotients (__fdividef, 2 ulp): increments of at most one cell, so 2.4e-7
+// cells at worst against the 1e-5 bar.
 // atan2(y, x) and log1p(x) with a short series where the argument is small (the displacement of one step is a small fraction
 // of r), the library routine otherwise; truncation error below 2e-12
 __device__ __forceinline__ float atan2_step(float y, float x) {
@@ -69,29 +71,29 @@ __device__ __forceinline__ void push_from_fields_geo(const GridDev &g, const GEO
         const float rp = s.r + dr_;
         const float d2 = dr_ * dr_ + dth_ * dth_ + dph_ * dph_;
         const float rn = sqrtf(rp * rp + dth_ * dth_ + dph_ * dph_);
-        const float Dr = (2.0f * s.r * dr_ + d2) / (rn + s.r);                 // r' - r without cancellation
+        const float Dr = __fdividef(2.0f * s.r * dr_ + d2, rn + s.r);                 // r' - r without cancellation
         const float a = rp * s.st + dth_ * s.ct;                               // new cylindrical radius vector in the old meridional plane
         const float rho = sqrtf(a * a + dph_ * dph_);
         const float zn = rp * s.ct - dth_ * s.st;
-        const float rma = a > 0.f ? (dph_ * dph_) / (rho + a) : rho - a;       // rho' - a
+        const float rma = a > 0.f ? __fdividef(dph_ * dph_, rho + a) : rho - a;       // rho' - a
         const float Dth = atan2_step(dth_ + rma * s.ct, zn * s.ct + rho * s.st);   // theta' - theta
         const float Dph = atan2_step(dph_, a);
         float x1n, x2n;
-        if (KIND == ENT_SPH) { x1n = Dr / g.drf; x2n = Dth / g.dthf; }
+        if (KIND == ENT_SPH) { x1n = __fdividef(Dr, g.drf); x2n = __fdividef(Dth, g.dthf); }
         else {
-            x1n = log1p_step(Dr / s.rr0) / g.dRf;
+            x1n = __fdividef(log1p_step(__fdividef(Dr, s.rr0)), g.dRf);
             float DT = Dth;
             if (g.vtf != 0.f) {                                               // theta(T + DT) - theta(T) = Dth: theta is a cubic, so its
                 const float c3 = 4.0f * g.vtf * 0.101321183642337771f;        // Taylor series ends: th1 DT + c2 DT^2 + c3 DT^3, c3 = 4 vt / pi^2
-                DT = Dth / s.th1;
+                DT = __fdividef(Dth, s.th1);
 #pragma unroll
                 for (int it = 0; it < 2; ++it) {                              // two Newton steps from the linear guess (no cube root, cf. App. B)
                     const float f = ((c3 * DT + s.c2) * DT + s.th1) * DT - Dth;
                     const float fp = (3.0f * c3 * DT + 2.0f * s.c2) * DT + s.th1;
-                    DT -= f / fp;
+                    DT -= __fdividef(f, fp);
                 }
             }
-            x2n = DT / g.dTf;
+            x2n = __fdividef(DT, g.dTf);
         }
         split_offset(d[0] + x1n, di[0], d[0]);
         split_offset(d[1] + x2n, di[1], d[1]);
@@ -247,7 +249,7 @@ __device__ __forceinline__ float half_qw_v3(const GridDev &g, const GEO &geo, co
         if (s.sh3 < 1e-12f) return 0.f;
         float sp, cp;
         sincos_azimuth(phi0 + 0.5f * dphi, sp, cp);
-        return 0.5f * qw * (((u[1] * cp - u[0] * sp) * ig) / s.sh3);
+        return 0.5f * qw * __fdividef((u[1] * cp - u[0] * sp) * ig, s.sh3);
     }
     double dphi = (double)phi1 - (double)phi0;
     dphi -= 2.0 * PI_D * floor((dphi + PI_D) / (2.0 * PI_D));                 // shorter arc
