@@ -274,10 +274,11 @@ __device__ __forceinline__ void deposit_particle_at(const GridDev &g, const GEO 
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
         if (k < D) {
-            b[k] = (float)di[k] + dn[k];                                      // new position in the old cell's frame
-            float r = di[k] == 0 ? 0.5f * (a[k] + b[k]) : (di[k] > 0 ? 1.0f : 0.0f);   // relay point
+            const float fdi = (float)di[k];
+            b[k] = fdi + dn[k];                                               // new position in the old cell's frame
+            float r = fminf(fminf(fdi, 0.f) + 1.0f, fmaxf(fmaxf(fdi, 0.f), 0.5f * (a[k] + b[k])));   // relay point, branch-free
             D1[k] = r - a[k];  W1[k] = 0.5f * (a[k] + r);
-            D2[k] = b[k] - r;  W2[k] = 0.5f * (r + b[k]) - (float)di[k];
+            D2[k] = b[k] - r;  W2[k] = 0.5f * (r + b[k]) - fdi;
         } else { b[k] = 0.f; D1[k] = W1[k] = D2[k] = W2[k] = 0.f; }
     }
     const long long s1 = gi.P[0], s2 = (long long)gi.P[0] * gi.P[1];
