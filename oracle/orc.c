@@ -281,8 +281,30 @@ void orc_vay(double u[3], const double E[3], const double B[3], double qm, doubl
     u[2] = sfac * (up[2] + udt * t[2] + (up[0] * t[1] - up[1] * t[0]));
 }
 
-static int orc_pusher_kind = 0;           /* 0 = Boris (default), 1 = Vay; read by orc_gather_push */
-int orc_set_pusher(int kind) { int prev = orc_pusher_kind; if (kind == 0 || kind == 1) orc_pusher_kind = kind; return prev; }
+static int orc_pusher_kind = 0;           /* 0 = Boris (default), 1 = Vay, 2 = Boris,GCA, 3 = Vay,GCA; read by orc_gather_push */
+int orc_set_pusher(int kind) { int prev = orc_pusher_kind; if (kind >= 0 && kind <= 3) orc_pusher_kind = kind; return prev; }
+
+/* N3, the hybrid pusher of P:976-980 ("Boris,GCA" / "Vay,GCA", fn. 21).  The paper gives two sentences: the pusher "switches between
+ * the conventional algorithm ... and the guiding center approximation ... depending on the ratio of |E|/|B| and the particle's
+ * nominal gyroradius at a given timestep, rho_L ~ gamma beta m c^2 / q|B|", with "the critical Larmor radius for the transition" an
+ * input, and "in the guiding center regime, the particle's momentum perpendicular to the local magnetic field is set to zero,
+ * effectively reducing its motion to that of its guiding center".  Reading (G26; parity unpinned beyond those sentences,
+ * the cited scheme of Bacchini et al. 2020 is not in the paper): with E, B the fields at the particle in the orthonormal basis and
+ * u the momentum BEFORE the push (the "given timestep"), the guiding-centre regime holds when
+ *     |B| > 0,   |E| < eovb |B|,   rho_L = |u| m / (|q| |B|) < rho_crit            (c = 1; eovb, rho_crit: inputs)
+ * and then the conventional push is followed by u <- (u . b) b, b = B/|B|: the rotation about B leaves u.b alone, so this is
+ * u_par + (q/m) E_par dt along b with u_perp = 0; the move of sub-step 6 is unchanged (the particle slides along the field line). */
+static double orc_gca_rho = 0.0, orc_gca_eovb = 0.0;
+void orc_set_gca(double rho_crit, double eovb) { orc_gca_rho = rho_crit; orc_gca_eovb = eovb; }
+int orc_gca_project(double u[3], const double u_before[3], const double E[3], const double B[3], double qm) {
+    double B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2], E2 = E[0] * E[0] + E[1] * E[1] + E[2] * E[2];
+    double U2 = u_before[0] * u_before[0] + u_before[1] * u_before[1] + u_before[2] * u_before[2];
+    double k = orc_gca_rho * fabs(qm);                                   /* rho_L < rho_crit  <=>  |u|^2 < (rho_crit |q|/m)^2 |B|^2 */
+    if (!(B2 > 0.0) || !(E2 < orc_gca_eovb * orc_gca_eovb * B2) || !(U2 < k * k * B2)) return 0;
+    double up = (u[0] * B[0] + u[1] * B[1] + u[2] * B[2]) / B2;
+    for (int a = 0; a < 3; ++a) u[a] = up * B[a];
+    return 1;
+}
 
 /* ------------------------------------------------------------------------------------------
  * steps 3-7 + O7 crossing bookkeeping (readings G9, G11)
@@ -313,7 +335,9 @@ int orc_gather_push(const orc_grid *g, const float *const F[6], const orc_partic
             orc_to_cartesian_basis(g, x, EB, E);
             orc_to_cartesian_basis(g, x, EB + 3, B);
             /* step 5: u^(n-1/2) -> u^(n+1/2) */
-            if (orc_pusher_kind == 1) orc_vay(u, E, B, qm, dt); else orc_boris(u, E, B, qm, dt);
+            double u_before[3] = { u[0], u[1], u[2] };
+            if (orc_pusher_kind & 1) orc_vay(u, E, B, qm, dt); else orc_boris(u, E, B, qm, dt);
+            if (orc_pusher_kind & 2) orc_gca_project(u, u_before, E, B, qm);
             /* step 6: x^(n) -> x^(n+1) with u^(n+1/2) / gamma^(n+1/2), in the global Cartesian frame */
             double gam = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
             double X[3], xn[3];

@@ -83,7 +83,11 @@ void orc_boris(double u[3], const double E[3], const double B[3], double q_over_
 
 /* ---- N3: Vay (2008) pusher, same interface; orc_set_pusher selects the one orc_gather_push / orc_step use (0 Boris, 1 Vay) ---- */
 void orc_vay(double u[3], const double E[3], const double B[3], double q_over_m, double dt);
-int  orc_set_pusher(int kind);                                            /* returns the previous kind */
+int  orc_set_pusher(int kind);                                            /* 0 Boris, 1 Vay, 2 Boris,GCA, 3 Vay,GCA; returns the previous kind */
+/* hybrid pusher of P:976-980 (reading G26): thresholds, and the guiding-centre step u <- (u.b) b when |E| < eovb |B| and
+ * |u_before| m / (|q||B|) < rho_crit (returns 1 if applied) */
+void orc_set_gca(double rho_crit, double eovb);
+int  orc_gca_project(double u[3], const double u_before[3], const double E[3], const double B[3], double q_over_m);
 
 /* ---- steps 3-7 for a particle block; out may alias in (arrays are overwritten element-wise) ---- */
 int orc_gather_push(const orc_grid *g, const float *const F[6], const orc_particles *in, orc_particles *out,

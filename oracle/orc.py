@@ -70,6 +70,8 @@ def lib():
         L.orc_boris.argtypes = [dp, dp, dp, C.c_double, C.c_double]
         L.orc_vay.argtypes = [dp, dp, dp, C.c_double, C.c_double]
         L.orc_set_pusher.restype = C.c_int; L.orc_set_pusher.argtypes = [C.c_int]
+        L.orc_set_gca.argtypes = [C.c_double, C.c_double]
+        L.orc_gca_project.restype = C.c_int; L.orc_gca_project.argtypes = [dp, dp, dp, dp, C.c_double]
         L.orc_gather_push.restype = C.c_int
         L.orc_gather_push.argtypes = [C.POINTER(_Grid), C.POINTER(C.c_void_p), C.POINTER(_Particles), C.POINTER(_Particles),
                                       C.c_double, C.c_double]
@@ -261,6 +263,19 @@ def vay(u, E, B, q_over_m, dt) -> np.ndarray:
     ua = np.array(u, dtype=np.float64); Ea, Ep = _vec(E); Ba, Bp = _vec(B)
     lib().orc_vay(ua.ctypes.data_as(C.POINTER(C.c_double)), Ep, Bp, q_over_m, dt)
     return ua
+
+
+def set_gca(rho_crit: float, eovb: float) -> None:
+    """thresholds of the hybrid pusher: critical Larmor radius and the largest |E|/|B| of the guiding-centre regime"""
+    lib().orc_set_gca(float(rho_crit), float(eovb))
+
+
+def gca_project(u, u_before, E, B, q_over_m):
+    """returns (u after the guiding-centre step, applied?)"""
+    a, pa = _vec(u); _, pb = _vec(u_before); _, pe = _vec(E); _, pB = _vec(B)
+    a = a.copy(); pa = a.ctypes.data_as(C.POINTER(C.c_double))
+    r = lib().orc_gca_project(pa, pb, pe, pB, float(q_over_m))
+    return a, bool(r)
 
 
 def set_pusher(kind: int) -> int:

@@ -86,6 +86,14 @@ MUTANTS = [
      "return r * r * dr * (1.0 - cos(0.5 * dth));",
      "return 2.0 * PI * r * r * dr * (1.0 - cos(0.5 * dth));",
      "tests/test_oracle_pins_fields.py::test_curvilinear_curl_converges_to_the_textbook_curl_at_second_order"),
+    ("gca: gyroradius of the momentum AFTER the push (P:976 'at a given timestep', reading G26)",
+     "if (orc_pusher_kind & 2) orc_gca_project(u, u_before, E, B, qm);",
+     "if (orc_pusher_kind & 2) orc_gca_project(u, u, E, B, qm);",
+     "tests/test_oracle_pins_gca.py::test_switch_on_the_gyroradius_of_the_momentum_before_the_push"),
+    ("gca: projection on B without the 1/|B|^2",
+     "double up = (u[0] * B[0] + u[1] * B[1] + u[2] * B[2]) / B2;",
+     "double up = (u[0] * B[0] + u[1] * B[1] + u[2] * B[2]);",
+     "tests/test_oracle_pins_gca.py::test_guiding_centre_regime_kills_u_perp_and_follows_E_par"),
     # mutants the round-1 pins already killed, kept so that the list documents them
     ("deposit: 3D weights without the D_a D_b / 12 term (reading G7)",
      "+ sigma * Dv[a] * Dv[b] / 12.0",
