@@ -241,7 +241,8 @@ enum {
     ENT_OPT_STEP_IMPL = 1,     /* 0 = auto (tiled when the block is the sorted one), 1 = force untiled, 2 = two-kernel
                                   (gather_push to scratch copy + deposit; the paper's structure) */
     ENT_OPT_TILE_1 = 2, ENT_OPT_TILE_2 = 3, ENT_OPT_TILE_3 = 4,   /* tile extents in cells; takes effect at the next ent_set_grid */
-    ENT_OPT_PUSHER = 7,        /* momentum update of sub-step 5: 0 = relativistic Boris (default), 1 = Vay (2008).  Takes effect at once. */
+    ENT_OPT_PUSHER = 7,        /* momentum update of sub-step 5: 0 = relativistic Boris (default), 1 = Vay (2008); 2 = "Boris,GCA", 3 = "Vay,GCA":
+                                  the hybrid pusher of P:976-980 with the thresholds of ent_set_gca.  Takes effect at once. */
     ENT_OPT_CURV_FP64 = 6,     /* SPH / QSPH grids: 0 (default) = the move is evaluated in fp32 as a DISPLACEMENT in the local frame at the
                                   particle (increments of the code coordinates added to the in-cell offsets; same mathematics as
                                   P:147-153 + P:285-327); 1 = fp64 coordinate maps through the global Cartesian frame (the literal
@@ -271,6 +272,14 @@ enum {
                                        fixed-point range (J^3 next to the axis), added to the global array directly; synchronises */
 };
 int ent_set_option(ent_ctx *ctx, int key, int64_t value);
+/* Thresholds of the hybrid pusher (ENT_OPT_PUSHER = 2, 3).  The paper's statement: the pusher "switches between the conventional
+ * algorithm and the guiding center approximation depending on the ratio of |E|/|B| and the particle's nominal gyroradius at a given
+ * timestep, rho_L ~ gamma beta m c^2 / q|B|"; "in the guiding center regime, the particle's momentum perpendicular to the local magnetic
+ * field is set to zero".  Here (a reading, G26): with E, B the fields at the particle in the orthonormal basis and u the
+ * momentum before the push, the regime holds when |B| > 0, |E| < e_over_b_max |B| and |u| m / (|q||B|) < rho_crit (c = 1; rho_crit in
+ * the length unit of the grid's physical extent); the conventional push is then followed by u <- (u.b) b, b = B/|B|, and the move of
+ * sub-step 6 is unchanged.  Defaults 0, 0 (never in the regime).  Takes effect at the next call. */
+int ent_set_gca(ent_ctx *ctx, double rho_crit, double e_over_b_max);
 int ent_get_stat(ent_ctx *ctx, int key, int64_t *value);
 
 /* library version, "major.minor" */

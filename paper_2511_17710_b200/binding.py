@@ -22,7 +22,7 @@ OPT_STEP_IMPL, OPT_TILE_1, OPT_TILE_2, OPT_TILE_3, OPT_SORT_MODE, OPT_CURV_FP64,
  STAT_SCRATCH_BYTES, STAT_LAST_STEP_TILED, STAT_LAST_SORT_REBIN, STAT_SLOT_ERRORS, STAT_CARRIES, STAT_GLOBAL_ADDS) = range(1, 15)
 
 SYMBOLS = ["ent_create", "ent_destroy", "ent_last_error", "ent_set_grid", "ent_gather_push", "ent_deposit", "ent_sort",
-           "ent_step", "ent_step_pair", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_filter_current", "ent_faraday", "ent_ampere", "ent_fill_field_ghosts", "ent_compact", "ent_step_host", "ent_set_option", "ent_get_stat", "ent_version"]
+           "ent_step", "ent_step_pair", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_filter_current", "ent_faraday", "ent_ampere", "ent_fill_field_ghosts", "ent_compact", "ent_step_host", "ent_set_option", "ent_set_gca", "ent_get_stat", "ent_version"]
 
 
 class EntError(RuntimeError):
@@ -86,6 +86,7 @@ def lib():
         L.ent_step_host.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Current), C.c_float, C.c_int,
                                     C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.ent_set_option.argtypes = [vp, C.c_int, C.c_int64]
+        L.ent_set_gca.argtypes = [vp, C.c_double, C.c_double]
         L.ent_get_stat.argtypes = [vp, C.c_int, C.POINTER(C.c_int64)]
         for s in SYMBOLS:
             if s not in ("ent_version", "ent_last_error"):
@@ -336,6 +337,10 @@ def ent_step_host(ctx: Ctx, EB, p: Particles, J, dt: float, nsteps: int = 1):
     ctx._ck(lib().ent_step_host(ctx._h, C.byref(_fields(EB, cuda=False)), C.byref(p.c(cuda=False)),
                                 C.byref(_current(J, cuda=False)), dt, nsteps, C.byref(up), C.byref(down)))
     return up.value, down.value
+
+
+def ent_set_gca(ctx: Ctx, rho_crit: float, e_over_b_max: float) -> None:
+    ctx._ck(lib().ent_set_gca(ctx._h, float(rho_crit), float(e_over_b_max)))
 
 
 def ent_set_option(ctx: Ctx, key: int, value: int) -> None:

@@ -24,6 +24,7 @@ struct ent_ctx {
     int step_impl = 0;
     int curv_f64 = 0;                     // ENT_OPT_CURV_FP64
     int pusher = 0;                       // ENT_OPT_PUSHER
+    double gca_rho = 0.0, gca_eovb = 0.0; // ent_set_gca
     int sort_mode = 0;                    // 0 auto (re-bin when the input is a sorted block), 1 always the full cell-level sort
     int last_sort_rebin = 0;
     int rebin_ordered = 1;                // re-bin keeps the particles that stay in a tile ordered by cell (Cartesian grids)
@@ -224,7 +225,7 @@ extern "C" int ent_set_grid(ent_ctx *ctx, const ent_grid *gr) {
         g.dT = PI_D / gr->N[1];
     }
     g.rminf = (float)g.rmin; g.drf = (float)g.dr; g.dthf = (float)g.dth; g.Rminf = (float)g.Rmin; g.dRf = (float)g.dR; g.dTf = (float)g.dT;
-    g.r0f = (float)g.r0; g.vtf = (float)g.vt; g.curv_f64 = ctx->curv_f64; g.pusher = ctx->pusher;
+    g.r0f = (float)g.r0; g.vtf = (float)g.vt; g.curv_f64 = ctx->curv_f64; g.pusher = ctx->pusher; g.gca_c = 0.f; g.gca_eovb2 = (float)(ctx->gca_eovb * ctx->gca_eovb);
     ctx->grid = *gr; ctx->g = g; ctx->have_grid = true;
     forget_all(ctx);
     if (ctx->pool) {                                            // the pool was carved for the previous grid
@@ -303,6 +304,7 @@ extern "C" int ent_gather_push(ent_ctx *ctx, const ent_fields *EB, const ent_par
     if (!(in->m != 0.f)) return fail(ctx, ENT_EINVAL, "mass is zero");
     if (in->n == 0) return ENT_OK;
     forget_block(ctx, out->cell);                             // `out` is overwritten: it is no longer a sorted block
+    ctx->g.gca_c = (float)(2.0 * ctx->gca_rho / (double)dt);      // hybrid pusher: rho_crit q/m = gca_c * eps
     float eps = 0.5f * (in->q / in->m) * dt;
     DISPATCH(gather_push_kernel, nblk(in->n), ctx->g, fp(EB), pp(in), pp(out), (long long)in->n, eps, dt);
     return launch_check(ctx, "gather_push_kernel");
@@ -314,6 +316,7 @@ extern "C" int ent_deposit(ent_ctx *ctx, const ent_particles *po, const ent_part
     if ((rc = check_current(ctx, J)) || (rc = check_particles(ctx, po, "old", false)) || (rc = check_particles(ctx, pn, "new", false))) return rc;
     if (po->n != pn->n) return fail(ctx, ENT_EINVAL, "old->n != new->n");
     if (!(dt > 0.f)) return fail(ctx, ENT_EINVAL, "dt must be positive");
+    ctx->g.gca_c = (float)(2.0 * ctx->gca_rho / (double)dt);      // hybrid pusher: rho_crit q/m = gca_c * eps
     if (po->n == 0) return ENT_OK;
     DISPATCH(deposit_kernel, nblk(po->n), ctx->g, pp(po), pp(pn), cp(J), (long long)po->n, po->q, 1.0f / dt, ctx->counters + 0);
     return launch_check(ctx, "deposit_kernel");
@@ -507,6 +510,7 @@ extern "C" int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, en
     int rc;
     if ((rc = check_fields(ctx, EB)) || (rc = check_current(ctx, J)) || (rc = check_particles(ctx, p, "p", true))) return rc;
     if (!(dt > 0.f)) return fail(ctx, ENT_EINVAL, "dt must be positive");
+    ctx->g.gca_c = (float)(2.0 * ctx->gca_rho / (double)dt);      // hybrid pusher: rho_crit q/m = gca_c * eps
     if (!(p->m != 0.f)) return fail(ctx, ENT_EINVAL, "mass is zero");
     ctx->last_step_tiled = 0;
     if (p->n == 0) return ENT_OK;
@@ -530,12 +534,22 @@ extern "C" int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, en
     return launch_check(ctx, "step_untiled_kernel");
 }
 
+// thresholds of the hybrid pusher
+extern "C" int ent_set_gca(ent_ctx *ctx, double rho_crit, double e_over_b_max) {
+    if (!ctx) return ENT_EINVAL;
+    if (!(rho_crit >= 0.0) || !(e_over_b_max >= 0.0)) return fail(ctx, ENT_EINVAL, "ent_set_gca: thresholds must be >= 0");
+    ctx->gca_rho = rho_crit; ctx->gca_eovb = e_over_b_max;
+    ctx->g.gca_eovb2 = (float)(e_over_b_max * e_over_b_max);
+    return ENT_OK;
+}
+
 // two species through ONE launch of the tiled kernel (one E,B box, one J tile and one flush per tile for both)
 extern "C" int ent_step_pair(ent_ctx *ctx, const ent_fields *EB, ent_particles *p1, ent_particles *p2, ent_current *J, float dt) {
     ENTER();
     int rc;
     if ((rc = check_fields(ctx, EB)) || (rc = check_current(ctx, J)) || (rc = check_particles(ctx, p1, "p1", true)) || (rc = check_particles(ctx, p2, "p2", true))) return rc;
     if (!(dt > 0.f)) return fail(ctx, ENT_EINVAL, "dt must be positive");
+    ctx->g.gca_c = (float)(2.0 * ctx->gca_rho / (double)dt);      // hybrid pusher: rho_crit q/m = gca_c * eps
     if (!(p1->m != 0.f) || !(p2->m != 0.f)) return fail(ctx, ENT_EINVAL, "mass is zero");
     if (p1->n > 0 && p1->cell == p2->cell) return fail(ctx, ENT_EINVAL, "ent_step_pair: the two blocks are the same");
     ent_ctx::SortedBlock *s1 = find_block(ctx, p1), *s2 = find_block(ctx, p2);
@@ -737,6 +751,7 @@ extern "C" int ent_step_sorted(ent_ctx *ctx, const ent_fields *EB, const ent_par
         (rc = check_particles(ctx, out, "out", true))) return rc;
     if (in->n != out->n) return fail(ctx, ENT_EINVAL, "in->n != out->n");
     if (!(dt > 0.f)) return fail(ctx, ENT_EINVAL, "dt must be positive");
+    ctx->g.gca_c = (float)(2.0 * ctx->gca_rho / (double)dt);      // hybrid pusher: rho_crit q/m = gca_c * eps
     if (!(in->m != 0.f)) return fail(ctx, ENT_EINVAL, "mass is zero");
     if (in->tag && !out->tag) return fail(ctx, ENT_EINVAL, "in has tags but out->tag is NULL");
     ctx->last_step_tiled = 0;
@@ -794,7 +809,7 @@ extern "C" int ent_set_option(ent_ctx *ctx, int key, int64_t value) {
             if (value < 0 || value > 2) return fail(ctx, ENT_EINVAL, "ENT_OPT_SORT_MODE must be 0, 1 or 2");
             ctx->sort_mode = value == 1 ? 1 : 0; ctx->rebin_ordered = value != 2; return ENT_OK;
         case ENT_OPT_PUSHER:
-            if (value < 0 || value > 1) return fail(ctx, ENT_EINVAL, "ENT_OPT_PUSHER must be 0 (Boris) or 1 (Vay)");
+            if (value < 0 || value > 3) return fail(ctx, ENT_EINVAL, "ENT_OPT_PUSHER must be 0 (Boris), 1 (Vay), 2 (Boris,GCA) or 3 (Vay,GCA)");
             ctx->pusher = (int)value; ctx->g.pusher = (int)value; return ENT_OK;
         case ENT_OPT_SORT_STAGING:
             if (value < 0 || value > 1) return fail(ctx, ENT_EINVAL, "ENT_OPT_SORT_STAGING must be 0 or 1");

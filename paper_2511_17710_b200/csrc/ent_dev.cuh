@@ -39,7 +39,9 @@ struct GridDev {
     double Rmin, dR, dT, r0, vt;
     // fp32 copies for the displacement form of the curvilinear move (ent_particle.cuh) and its switch
     float rminf, drf, dthf, Rminf, dRf, dTf, r0f, vtf;
-    int pusher;        // ENT_OPT_PUSHER: 0 Boris, 1 Vay
+    int pusher;        // ENT_OPT_PUSHER: 0 Boris, 1 Vay, 2 Boris,GCA, 3 Vay,GCA
+    float gca_c;       // hybrid pusher: 2 rho_crit / dt of the current call (x eps = rho_crit q/m), and (max |E|/|B|)^2
+    float gca_eovb2;
     int curv_f64;      // 1: coordinate maps of the axisymmetric grids in fp64 through the global Cartesian frame (round-1 form)
 };
 
@@ -285,8 +287,20 @@ __device__ __forceinline__ void vay(float u[3], const float E[3], const float B[
     u[2] = sf * (p2 + ut * t2 + (p0 * t1 - p1 * t0));
 }
 // step 5 with the pusher the grid struct selects (ENT_OPT_PUSHER): 0 Boris, 1 Vay
-__device__ __forceinline__ void push_momentum(int pusher, float u[3], const float E[3], const float B[3], float eps) {
-    if (pusher == 1) vay(u, E, B, eps); else boris(u, E, B, eps);
+// bit 1 of the pusher: the hybrid pusher of P:976-980 (reading G26): in the guiding-centre regime -- |E| < eovb |B| and the nominal
+// gyroradius of the momentum the particle has BEFORE the push, |u| m / (|q||B|), below rho_crit -- the conventional push is followed by
+// u <- (u.b) b (momentum perpendicular to the local B set to zero; u.b has received (q/m) E_par dt)
+__device__ __forceinline__ void push_momentum(const GridDev &g, float u[3], const float E[3], const float B[3], float eps) {
+    const float U2 = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    if (g.pusher & 1) vay(u, E, B, eps); else boris(u, E, B, eps);
+    if (g.pusher & 2) {
+        const float B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2], E2 = E[0] * E[0] + E[1] * E[1] + E[2] * E[2];
+        const float k = g.gca_c * eps;
+        if (B2 > 0.f && E2 < g.gca_eovb2 * B2 && U2 < k * k * B2) {
+            const float up = (u[0] * B[0] + u[1] * B[1] + u[2] * B[2]) / B2;
+            u[0] = up * B[0]; u[1] = up * B[1]; u[2] = up * B[2];
+        }
+    }
 }
 __device__ __forceinline__ float inv_gamma(const float u[3]) {
     return rsqrtf(1.0f + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);      // MUFU.RSQ, 2 ulp: 1e-7 cells on a move of 0.45 cells

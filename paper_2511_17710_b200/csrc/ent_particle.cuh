@@ -35,7 +35,7 @@ __device__ __forceinline__ void push_from_fields_geo(const GridDev &g, const GEO
         // step 4: A^hat = sqrt(h_ii) A^i; Cartesian code basis is already aligned with x,y,z
 #pragma unroll
         for (int a = 0; a < 3; ++a) { E[a] = g.dx[a] * EB[a]; B[a] = g.dx[a] * EB[3 + a]; }
-        push_momentum(g.pusher, u, E, B, eps);                                                  // step 5, Eq. 3
+        push_momentum(g, u, E, B, eps);                                                  // step 5, Eq. 3
         float ig = inv_gamma(u);
 #pragma unroll
         for (int a = 0; a < 3; ++a) {                                         // steps 6-7
@@ -63,7 +63,7 @@ __device__ __forceinline__ void push_from_fields_geo(const GridDev &g, const GEO
             B[1] = Ar * s.st * sp + At * s.ct * sp + Ap * cp;
             B[2] = Ar * s.ct - At * s.st;
         }
-        push_momentum(g.pusher, u, E, B, eps);
+        push_momentum(g, u, E, B, eps);
         const float ig = inv_gamma(u);
         const float Dx = (u[0] * ig) * dt, Dy = (u[1] * ig) * dt, Dz = (u[2] * ig) * dt;
         const float Dh = Dx * cp + Dy * sp;                                   // component along the old cylindrical radius
@@ -125,7 +125,7 @@ __device__ __forceinline__ void push_from_fields_geo(const GridDev &g, const GEO
             B[1] = Ar * fst * fsp + At * fct * fsp + Ap * fcp;
             B[2] = Ar * fct - At * fst;
         }
-        push_momentum(g.pusher, u, E, B, eps);
+        push_momentum(g, u, E, B, eps);
         float ig = inv_gamma(u);
         // step 6: x^X += u/gamma dt in the global Cartesian frame
         double X = s.r * st * cp + (double)(u[0] * ig) * (double)dt;

@@ -245,7 +245,7 @@ step_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
             gather_box<D, G::FX, G::FY, G::FNP>(sF, b, d, EBv);
             // ---- S2 tetrad, S3 Boris (Eq. 3), S4-S5 move + crossing
             float E[3] = { T.sx[0] * EBv[0], T.sx[1] * EBv[1], T.sx[2] * EBv[2] }, B[3] = { T.sx[0] * EBv[3], T.sx[1] * EBv[4], T.sx[2] * EBv[5] };
-            push_momentum(g.pusher, u, E, B, A.eps);
+            push_momentum(g, u, E, B, A.eps);
             const float ig = inv_gamma(u);
             const float a0[3] = { d[0], d[1], d[2] };
             int di[3] = {0, 0, 0}, bn[3] = { b[0], b[1], b[2] };

@@ -21,9 +21,9 @@ MUTANTS = [
      "double gm = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);",
      T + "test_boris_is_time_reversible_with_E_and_B"),
     ("move: gamma of the OLD momentum (reading G4)",
-     ["            if (orc_pusher_kind == 1) orc_vay(u, E, B, qm, dt); else orc_boris(u, E, B, qm, dt);\n",
+     ["            if (orc_pusher_kind & 1) orc_vay(u, E, B, qm, dt); else orc_boris(u, E, B, qm, dt);\n",
       "            double gam = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);\n            double X[3], xn[3];\n"],
-     ["            double gam = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);\n            if (orc_pusher_kind == 1) orc_vay(u, E, B, qm, dt); else orc_boris(u, E, B, qm, dt);\n",
+     ["            double gam = sqrt(1.0 + u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);\n            if (orc_pusher_kind & 1) orc_vay(u, E, B, qm, dt); else orc_boris(u, E, B, qm, dt);\n",
       "            double X[3], xn[3];\n"],
      T + "test_hyperbolic_motion_converges_at_second_order"),
     ("deposit: J^3 from the old momentum (reading G8)",

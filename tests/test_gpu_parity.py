@@ -416,6 +416,75 @@ def test_vay_pusher_matches_oracle(env, name, impl, sort_first):
     assert all(st["max_u_rel"] <= P.MOM_TOL for st in stats.values())
 
 
+@pytest.mark.parametrize("name,pusher,rho_crit,eovb,sort_first", [("C3/8", 2, 2.0, 0.5, True), ("C3/8", 3, 2.0, 0.5, False),
+                                                                   ("C2/4", 2, 0.05, 0.9, True), ("C1", 2, 0.4, 0.3, True)])
+def test_hybrid_gca_pusher_matches_oracle(env, name, pusher, rho_crit, eovb, sort_first):
+    """ENT_OPT_PUSHER = 2 / 3 ("Boris,GCA" / "Vay,GCA", reading G26) against the oracle with the same thresholds, tiled
+    and untiled kernels, Cartesian and quasi-spherical grids.  Both sides start every step from the SAME state (the GPU's): a particle
+    whose |E|/|B| or gyroradius sits within fp32 rounding of a threshold takes the other branch on the GPU, which is a different but
+    equally valid trajectory, so a handful of such particles per step are allowed to differ and everything else must meet the bars;
+    the currents are checked against the oracle's deposit of the GPU's own moves (strict) and by continuity."""
+    bind, synth, ctx, orc = env
+    wl = _workloads(synth)[name]()
+    g = wl.grid
+    eg, og = P.grid_to_ent(bind, g), P.grid_to_orc(orc, g)
+    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, 0)
+    bind.ent_set_grid(ctx, eg)
+    bind.ent_set_option(ctx, bind.OPT_PUSHER, pusher)
+    bind.ent_set_gca(ctx, rho_crit, eovb)
+    orc.set_gca(rho_crit, eovb)
+    F_dev, F_orc = [f.cuda() for f in wl.fields], P.fields_to_orc(wl.fields)
+    try:
+        for sp in wl.species[:1]:
+            pe = P.species_to_ent(bind, synth, g, sp, "cuda")
+            if sort_first:
+                ps = pe.empty_like()
+                bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 1)
+                bind.ent_sort(ctx, pe, ps, None)
+                bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 0)
+                pe = ps
+            Jg = bind.zeros_current(eg, "cuda")
+            fracs = []
+            for s in range(3):
+                before = P.ent_to_orc(orc, g, pe)
+                bind.ent_zero_current(ctx, Jg)
+                bind.ent_step(ctx, F_dev, pe, Jg, wl.dt)
+                bind.ent_fold_current(ctx, Jg)
+                torch.cuda.synchronize()
+                assert bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED) == (1 if sort_first else 0)
+                after = P.ent_to_orc(orc, g, pe)
+                orc.set_pusher(pusher)
+                want = orc.gather_push(og, F_orc, before, sp.q / sp.m, wl.dt)
+                orc.set_pusher(pusher & 1)
+                conv = orc.gather_push(og, F_orc, before, sp.q / sp.m, wl.dt)          # the conventional pusher alone: who was in the regime?
+                ug, uo, uc = np.stack(after.u), np.stack(want.u), np.stack(conv.u)
+                alive = (want.tag != 0) & (after.tag != 0) if want.tag is not None else np.ones(ug.shape[1], bool)
+                fracs.append(float((np.abs(uo - uc).max(axis=0) > 1e-9)[alive].mean()))
+                umag = np.sqrt((uo * uo).sum(axis=0))
+                floor = P.U_FLOOR_FRAC * np.sqrt((umag * umag).mean())
+                bad_u = np.abs(ug - uo).max(axis=0) / np.maximum(umag, floor) > P.MOM_TOL
+                bad_x = np.zeros_like(bad_u)
+                for a in range(g.D):
+                    diff = (after.i[a] + after.d[a]) - (want.i[a] + want.d[a])
+                    if g.bc[a] == synth.PERIODIC:
+                        diff = diff - g.N[a] * np.round(diff / g.N[a])
+                    bad_x |= np.abs(diff) > P.POS_TOL
+                nbad = int(((bad_u | bad_x) & alive).sum())
+                allowed = 10 + int(1e-4 * pe.n)
+                print(name, "pusher", pusher, "step", s, "in the guiding-centre regime:", fracs[-1], " threshold straddlers:", nbad, "of", pe.n)
+                assert nbad <= allowed
+                if want.tag is not None:
+                    assert int((want.tag != after.tag).sum()) <= allowed
+                strict = P.compare_current(Jg, P.deposit_of_gpu_positions(orc, og, before, after, sp.q, wl.dt))
+                c = P.continuity_of_gpu_step(orc, og, before, after, Jg, sp.q, wl.dt)
+                assert c <= P.CONT_TOL
+            assert 0.02 < np.mean(fracs) < 0.98, "the case must exercise both regimes"
+    finally:
+        bind.ent_set_option(ctx, bind.OPT_PUSHER, 0)
+        bind.ent_set_gca(ctx, 0.0, 0.0)
+        orc.set_pusher(0); orc.set_gca(0.0, 0.0)
+
+
 @pytest.mark.parametrize("name", ["ABS3", "C5/32", "C1"])
 def test_compact_matches_oracle(env, name):
     """ent_compact (tag sort) after a few steps on grids that lose particles (and one that does not): bit-exact against the
