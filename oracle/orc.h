@@ -22,7 +22,9 @@
  * out-of-plane current, the theta = pi clamp, the D_a D_b / 12 term, ...).  One choice stays a READING the paper does
  * not fix: the FORM of the 2D out-of-plane current J^3 (velocity form, half per segment, bilinear weights at the
  * segment midpoints, reading G8) -- "parity unpinned" by the paper beyond its nodal sum, time level and evaluation
- * point, which are pinned; see DESIGN.md.
+ * point, which are pinned; see DESIGN.md.  A second one: the hybrid pusher (orc_gca_project, reading G26) -- the paper gives two
+ * sentences and cites a scheme that is not in it; the switch and the zeroing of u_perp are pinned as stated, the rest
+ * (no drift terms, the move unchanged) is "parity unpinned".
  *
  * All arithmetic is double.  Field arrays are the fp32 arrays handed to the GPU (up-cast on load).
  */
