@@ -291,7 +291,8 @@ __device__ __forceinline__ void vay(float u[3], const float E[3], const float B[
 // gyroradius of the momentum the particle has BEFORE the push, |u| m / (|q||B|), below rho_crit -- the conventional push is followed by
 // u <- (u.b) b (momentum perpendicular to the local B set to zero; u.b has received (q/m) E_par dt)
 __device__ __forceinline__ void push_momentum(const GridDev &g, float u[3], const float E[3], const float B[3], float eps) {
-    const float U2 = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    float U2 = 0.f;
+    if (g.pusher & 2) U2 = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];     // uniform branch: nothing extra for the conventional pushers
     if (g.pusher & 1) vay(u, E, B, eps); else boris(u, E, B, eps);
     if (g.pusher & 2) {
         const float B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2], E2 = E[0] * E[0] + E[1] * E[1] + E[2] * E[2];
