@@ -22,7 +22,7 @@ OPT_STEP_IMPL, OPT_TILE_1, OPT_TILE_2, OPT_TILE_3, OPT_SORT_MODE, OPT_CURV_FP64,
  STAT_SCRATCH_BYTES, STAT_LAST_STEP_TILED, STAT_LAST_SORT_REBIN, STAT_SLOT_ERRORS, STAT_CARRIES, STAT_GLOBAL_ADDS) = range(1, 15)
 
 SYMBOLS = ["ent_create", "ent_destroy", "ent_last_error", "ent_set_grid", "ent_gather_push", "ent_deposit", "ent_sort",
-           "ent_step", "ent_step_pair", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_filter_current", "ent_faraday", "ent_ampere", "ent_fill_field_ghosts", "ent_compact", "ent_step_host", "ent_set_option", "ent_set_gca", "ent_get_stat", "ent_version"]
+           "ent_step", "ent_step_pair", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_filter_current", "ent_faraday", "ent_ampere", "ent_fill_field_ghosts", "ent_compact", "ent_step_host", "ent_step_host_pair", "ent_set_option", "ent_set_gca", "ent_get_stat", "ent_version"]
 
 
 class EntError(RuntimeError):
@@ -85,6 +85,8 @@ def lib():
         L.ent_compact.argtypes = [vp, C.POINTER(_Particles), C.POINTER(_Particles), vp]
         L.ent_step_host.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Current), C.c_float, C.c_int,
                                     C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+        L.ent_step_host_pair.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Particles), C.POINTER(_Current), C.c_float, C.c_int,
+                                         C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.ent_set_option.argtypes = [vp, C.c_int, C.c_int64]
         L.ent_set_gca.argtypes = [vp, C.c_double, C.c_double]
         L.ent_get_stat.argtypes = [vp, C.c_int, C.POINTER(C.c_int64)]
@@ -336,6 +338,14 @@ def ent_step_host(ctx: Ctx, EB, p: Particles, J, dt: float, nsteps: int = 1):
     up, down = C.c_int64(0), C.c_int64(0)
     ctx._ck(lib().ent_step_host(ctx._h, C.byref(_fields(EB, cuda=False)), C.byref(p.c(cuda=False)),
                                 C.byref(_current(J, cuda=False)), dt, nsteps, C.byref(up), C.byref(down)))
+    return up.value, down.value
+
+
+def ent_step_host_pair(ctx: Ctx, EB, p1: Particles, p2: Particles, J, dt: float, nsteps: int = 1):
+    """Host tensors in, host tensors out, both species pipelined; returns (h2d_bytes, d2h_bytes)."""
+    up, down = C.c_int64(0), C.c_int64(0)
+    ctx._ck(lib().ent_step_host_pair(ctx._h, C.byref(_fields(EB, cuda=False)), C.byref(p1.c(cuda=False)), C.byref(p2.c(cuda=False)),
+                                     C.byref(_current(J, cuda=False)), dt, nsteps, C.byref(up), C.byref(down)))
     return up.value, down.value
 
 

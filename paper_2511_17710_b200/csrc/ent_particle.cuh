@@ -16,6 +16,8 @@ struct NoGeo {};                          // Cartesian grids need no node factor
 // cells at worst against the 1e-5 bar.
 // atan2(y, x) and log1p(x) with a short series where the argument is small (the displacement of one step is a small fraction
 // of r), the library routine otherwise; truncation error below 2e-12
+// sqrt.approx.f32 (MUFU.SQRT, relative error 2^-23, exact zero for zero) instead of the IEEE sequence
+__device__ __forceinline__ float sqrt_approx(float x) { float r; asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float atan2_step(float y, float x) {
     if (x > 0.f && fabsf(y) < 0.0625f * x) {
         const float t = __fdividef(y, x), t2 = t * t;
@@ -70,10 +72,10 @@ __device__ __forceinline__ void push_from_fields_geo(const GridDev &g, const GEO
         const float dr_ = Dh * s.st + Dz * s.ct, dth_ = Dh * s.ct - Dz * s.st, dph_ = Dy * cp - Dx * sp;
         const float rp = s.r + dr_;
         const float d2 = dr_ * dr_ + dth_ * dth_ + dph_ * dph_;
-        const float rn = sqrtf(rp * rp + dth_ * dth_ + dph_ * dph_);
+        const float rn = sqrt_approx(rp * rp + dth_ * dth_ + dph_ * dph_);
         const float Dr = __fdividef(2.0f * s.r * dr_ + d2, rn + s.r);                 // r' - r without cancellation
         const float a = rp * s.st + dth_ * s.ct;                               // new cylindrical radius vector in the old meridional plane
-        const float rho = sqrtf(a * a + dph_ * dph_);
+        const float rho = sqrt_approx(a * a + dph_ * dph_);
         const float zn = rp * s.ct - dth_ * s.st;
         const float rma = a > 0.f ? __fdividef(dph_ * dph_, rho + a) : rho - a;       // rho' - a
         const float Dth = atan2_step(dth_ + rma * s.ct, zn * s.ct + rho * s.st);   // theta' - theta
