@@ -41,7 +41,7 @@ struct ent_ctx {
     void *fbuf = nullptr; size_t fbuf_cap = 0;          // second set of current arrays for the filter passes
     void *cbuf = nullptr; size_t cbuf_cap = 0;          // flags and positions of ent_compact
     cudaStream_t up_stream = nullptr, down_stream = nullptr;   // copy streams of ent_step_host_pair
-    cudaEvent_t ev[6] = {};
+    cudaEvent_t ev[33] = {};                                    // 2 per sub-block of ent_step_host_pair + 1
     void *sbuf = nullptr; size_t sbuf_cap = 0;          // array-of-structures staging of the full sort (ENT_OPT_SORT_STAGING)
     int sort_staging = 0;
     size_t side_bytes = 0;
@@ -921,9 +921,11 @@ extern "C" int ent_step_host(ent_ctx *ctx, const ent_fields *EB, ent_particles *
     return ENT_OK;
 }
 
-// Both species of a pair plasma from host buffers, pipelined over three streams: while species 1 is sorted and advanced, species 2
-// is still arriving over PCIe, and while species 2 is advanced, species 1 is already on its way back (PCIe is full duplex).
-// Fields go up once, J comes back once.
+// Both species of a pair plasma from host buffers, pipelined over three streams.  Each species is cut into HOST_CHUNKS independent
+// sub-blocks (particles are independent; J accumulates): while one sub-block is sorted and advanced, the next ones are still arriving
+// over PCIe and the previous ones are already on their way back (the link is full duplex), so the call takes about the time of
+// the larger of the two transfers plus one sub-block's work.  Fields go up once, J comes back once.
+constexpr int HOST_CHUNKS = 4;
 extern "C" int ent_step_host_pair(ent_ctx *ctx, const ent_fields *EB, ent_particles *p1, ent_particles *p2, ent_current *J, float dt, int nsteps,
                                   int64_t *h2d_bytes, int64_t *d2h_bytes) {
     ENTER();
@@ -932,18 +934,20 @@ extern "C" int ent_step_host_pair(ent_ctx *ctx, const ent_fields *EB, ent_partic
     const GridDev &g = ctx->g;
     ent_particles *hp[2] = { p1, p2 };
     const size_t pad = (size_t)padded_size(g), fslot = (pad * 4 + 255) & ~(size_t)255;
-    const size_t nmax = (size_t)(p1->n > p2->n ? p1->n : p2->n), pslot = (nmax * 4 + 255) & ~(size_t)255;
+    const size_t nmax = (size_t)(p1->n > p2->n ? p1->n : p2->n);
+    const size_t cmax = (nmax + HOST_CHUNKS - 1) / HOST_CHUNKS + 4, pslot = (cmax * 4 + 255) & ~(size_t)255;   // per sub-block and array
     const bool axisym = g.kind != ENT_CART;
+    constexpr int NJOB = 2 * HOST_CHUNKS;
     int rc;
-    if ((rc = ensure(ctx, &ctx->hbuf, &ctx->hbuf_cap, fslot * 9 + pslot * 40))) return rc;      // fields, J, 2 x (staged block + sorted copy)
-    if ((rc = reserve_pool(ctx, (long long)nmax))) return rc;
+    if ((rc = ensure(ctx, &ctx->hbuf, &ctx->hbuf_cap, fslot * 9 + pslot * 20 * NJOB))) return rc;   // fields, J, per sub-block: staged + sorted copy
+    if ((rc = reserve_pool(ctx, (long long)cmax))) return rc;
     if (!ctx->up_stream) {
         CK(cudaStreamCreateWithFlags(&ctx->up_stream, cudaStreamNonBlocking));
         CK(cudaStreamCreateWithFlags(&ctx->down_stream, cudaStreamNonBlocking));
         for (auto &e : ctx->ev) CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
-    CK(cudaEventRecord(ctx->ev[4], ctx->stream));                // whatever the caller enqueued before must finish first
-    CK(cudaStreamWaitEvent(ctx->up_stream, ctx->ev[4], 0));
+    CK(cudaEventRecord(ctx->ev[2 * NJOB], ctx->stream));         // whatever the caller enqueued before must finish first
+    CK(cudaStreamWaitEvent(ctx->up_stream, ctx->ev[2 * NJOB], 0));
     char *b = (char *)ctx->hbuf;
     int64_t up = 0, down = 0;
     ent_fields dEB; ent_current dJ;
@@ -957,46 +961,50 @@ extern "C" int ent_step_host_pair(ent_ctx *ctx, const ent_fields *EB, ent_partic
         if (!J->comp[c]) return fail(ctx, ENT_EINVAL, "host current component %d is NULL", c);
         dJ.comp[c] = (float *)(b + fslot * (6 + c));
     }
-    struct Arr { void *dev; void *srt; void *host; size_t bytes; };
-    Arr arrs[2][10]; int na[2] = { 0, 0 };
-    ent_particles dp[2], ds[2];
-    for (int k = 0; k < 2; ++k) {
-        const ent_particles *p = hp[k];
-        const size_t n = (size_t)p->n;
+    struct Arr { void *dev; void *srt; char *host; size_t bytes; };
+    Arr arrs[NJOB][10]; int na[NJOB] = {};
+    ent_particles dp[NJOB], ds[NJOB];
+    for (int k = 0; k < NJOB; ++k) {                              // uploads, in the order the sub-blocks will be advanced
+        const ent_particles *p = hp[k / HOST_CHUNKS];
+        const int ch = k % HOST_CHUNKS;
+        const size_t i0 = (size_t)p->n * ch / HOST_CHUNKS, i1 = (size_t)p->n * (ch + 1) / HOST_CHUNKS, n = i1 - i0;
         char *pb = b + fslot * 9 + pslot * 20 * k, *sb = pb + pslot * 10;
-        dp[k] = *p; ds[k] = *p;
-        auto add = [&](void **d, void **s_, void *host, int slot, size_t bytes) {
-            *d = pb + pslot * slot; *s_ = sb + pslot * slot; arrs[k][na[k]++] = { *d, *s_, host, bytes };
+        dp[k] = *p; ds[k] = *p; dp[k].n = ds[k].n = (int64_t)n;
+        auto add = [&](void **d, void **s_, void *host, int slot, size_t elem) {
+            *d = pb + pslot * slot; *s_ = sb + pslot * slot;
+            arrs[k][na[k]++] = { *d, *s_, host ? (char *)host + i0 * elem : nullptr, n * elem };
         };
-        add((void **)&dp[k].cell, (void **)&ds[k].cell, p->cell, 0, n * 4);
+        add((void **)&dp[k].cell, (void **)&ds[k].cell, p->cell, 0, 4);
         for (int a = 0; a < 3; ++a) {
-            if (a < g.D) add((void **)&dp[k].d[a], (void **)&ds[k].d[a], p->d[a], 1 + a, n * 4); else dp[k].d[a] = ds[k].d[a] = nullptr;
-            add((void **)&dp[k].u[a], (void **)&ds[k].u[a], p->u[a], 4 + a, n * 4);
+            if (a < g.D) add((void **)&dp[k].d[a], (void **)&ds[k].d[a], p->d[a], 1 + a, 4); else dp[k].d[a] = ds[k].d[a] = nullptr;
+            add((void **)&dp[k].u[a], (void **)&ds[k].u[a], p->u[a], 4 + a, 4);
         }
-        add((void **)&dp[k].w, (void **)&ds[k].w, p->w, 7, n * 4);
-        if (axisym) add((void **)&dp[k].phi, (void **)&ds[k].phi, p->phi, 8, n * 4); else dp[k].phi = ds[k].phi = nullptr;
-        if (p->tag) add((void **)&dp[k].tag, (void **)&ds[k].tag, p->tag, 9, n); else dp[k].tag = ds[k].tag = nullptr;
+        add((void **)&dp[k].w, (void **)&ds[k].w, p->w, 7, 4);
+        if (axisym) add((void **)&dp[k].phi, (void **)&ds[k].phi, p->phi, 8, 4); else dp[k].phi = ds[k].phi = nullptr;
+        if (p->tag) add((void **)&dp[k].tag, (void **)&ds[k].tag, p->tag, 9, 1); else dp[k].tag = ds[k].tag = nullptr;
         for (int j = 0; j < na[k]; ++j) {
             if (!arrs[k][j].host) return fail(ctx, ENT_EINVAL, "a required host particle array is NULL");
             if (arrs[k][j].bytes) CK(cudaMemcpyAsync(arrs[k][j].dev, arrs[k][j].host, arrs[k][j].bytes, cudaMemcpyHostToDevice, ctx->up_stream));
             up += (int64_t)arrs[k][j].bytes;
         }
-        CK(cudaEventRecord(ctx->ev[k], ctx->up_stream));         // species k (and, for k = 0, the fields) has arrived
+        CK(cudaEventRecord(ctx->ev[k], ctx->up_stream));         // sub-block k (and, for k = 0, the fields) has arrived
     }
     if ((rc = ent_zero_current(ctx, &dJ))) return rc;
     const int saved_mode = ctx->sort_mode;
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < NJOB; ++k) {
         CK(cudaStreamWaitEvent(ctx->stream, ctx->ev[k], 0));
-        forget_block(ctx, dp[k].cell);
-        ctx->sort_mode = 1;
-        rc = hp[k]->n ? ent_sort(ctx, &dp[k], &ds[k], nullptr) : ENT_OK;
-        ctx->sort_mode = saved_mode;
-        if (rc) return rc;
-        for (int s_ = 0; s_ < nsteps; ++s_)
-            if ((rc = ent_step(ctx, &dEB, &ds[k], &dJ, dt))) return rc;
-        forget_block(ctx, ds[k].cell);                           // the staging memory is reused by the next call
-        CK(cudaEventRecord(ctx->ev[2 + k], ctx->stream));
-        CK(cudaStreamWaitEvent(ctx->down_stream, ctx->ev[2 + k], 0));
+        if (dp[k].n > 0) {
+            forget_block(ctx, dp[k].cell);
+            ctx->sort_mode = 1;
+            rc = ent_sort(ctx, &dp[k], &ds[k], nullptr);
+            ctx->sort_mode = saved_mode;
+            if (rc) return rc;
+            for (int s_ = 0; s_ < nsteps; ++s_)
+                if ((rc = ent_step(ctx, &dEB, &ds[k], &dJ, dt))) return rc;
+            forget_block(ctx, ds[k].cell);                       // the staging memory is reused by the next call
+        }
+        CK(cudaEventRecord(ctx->ev[NJOB + k], ctx->stream));
+        CK(cudaStreamWaitEvent(ctx->down_stream, ctx->ev[NJOB + k], 0));
         for (int j = 0; j < na[k]; ++j) {
             if (arrs[k][j].bytes) CK(cudaMemcpyAsync(arrs[k][j].host, arrs[k][j].srt, arrs[k][j].bytes, cudaMemcpyDeviceToHost, ctx->down_stream));
             down += (int64_t)arrs[k][j].bytes;
