@@ -411,6 +411,11 @@ static SolverGeom solver_geom(const GridDev &g) {
     L.inv_sqrt_h = (float)(1.0 / sh);
     return L;
 }
+static bool all_periodic_cart(const GridDev &g) {
+    if (g.kind != ENT_CART) return false;
+    for (int d = 0; d < g.D; ++d) if (g.bc[d] != ENT_PERIODIC) return false;
+    return true;
+}
 static FieldRW frw(const ent_fields_rw *F) { FieldRW r; for (int c = 0; c < 6; ++c) r.c[c] = F->comp[c]; return r; }
 static int solver_grid(ent_ctx *ctx, const SolverGeom &L, dim3 *grid) {
     *grid = dim3((unsigned)((L.nmax[0] + TPB - 1) / TPB), (unsigned)L.nmax[1], (unsigned)(3 * L.nmax[2]));
@@ -426,7 +431,8 @@ extern "C" int ent_faraday(ent_ctx *ctx, ent_fields_rw *EB, float dt) {
     const SolverGeom L = solver_geom(g);
     dim3 grid;
     if ((rc = solver_grid(ctx, L, &grid))) return rc;
-    if (g.kind == ENT_CART) faraday_kernel<true><<<grid, TPB, 0, ctx->stream>>>(g, L, frw(EB), dt);
+    if (all_periodic_cart(g)) faraday_cart_kernel<<<dim3(grid.x, (unsigned)g.N[1], (unsigned)g.N[2]), TPB, 0, ctx->stream>>>(g, L, frw(EB), dt);
+    else if (g.kind == ENT_CART) faraday_kernel<true><<<grid, TPB, 0, ctx->stream>>>(g, L, frw(EB), dt);
     else faraday_kernel<false><<<grid, TPB, 0, ctx->stream>>>(g, L, frw(EB), dt);
     return launch_check(ctx, "faraday_kernel");
 }
@@ -441,7 +447,8 @@ extern "C" int ent_ampere(ent_ctx *ctx, ent_fields_rw *EB, const ent_current *J,
     dim3 grid;
     if ((rc = solver_grid(ctx, L, &grid))) return rc;
     CurrentPtrs j; for (int c = 0; c < 3; ++c) j.c[c] = J ? J->comp[c] : nullptr;
-    if (g.kind == ENT_CART) ampere_kernel<true><<<grid, TPB, 0, ctx->stream>>>(g, L, frw(EB), j, J != nullptr, dt, j_coeff);
+    if (all_periodic_cart(g)) ampere_cart_kernel<<<dim3(grid.x, (unsigned)g.N[1], (unsigned)g.N[2]), TPB, 0, ctx->stream>>>(g, L, frw(EB), j, J != nullptr, dt, j_coeff);
+    else if (g.kind == ENT_CART) ampere_kernel<true><<<grid, TPB, 0, ctx->stream>>>(g, L, frw(EB), j, J != nullptr, dt, j_coeff);
     else ampere_kernel<false><<<grid, TPB, 0, ctx->stream>>>(g, L, frw(EB), j, J != nullptr, dt, j_coeff);
     return launch_check(ctx, "ampere_kernel");
 }

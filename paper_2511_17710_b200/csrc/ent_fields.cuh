@@ -140,6 +140,48 @@ __global__ void __launch_bounds__(TPB) ampere_kernel(GridDev g, SolverGeom L, Fi
     else ampere_point<CARTESIAN, 2>(g, L, F, J, haveJ, dt, jc, i, j, k);
 }
 
+// All-periodic Cartesian grids (every lattice is N1 x N2 x N3): one thread per CELL advances the three components at once, so that
+// every array is read from DRAM once per call (the per-component kernels read each source array twice) and the neighbours come from
+// L1/L2; cells whose stencil wraps around the box (the last / first layer of a dimension) take the per-component code.
+// Same arithmetic as faraday_point / ampere_point.  blockIdx.y = x2 index, blockIdx.z = x3 index.
+__global__ void __launch_bounds__(TPB) faraday_cart_kernel(GridDev g, SolverGeom L, FieldRW F, float dt) {
+    const int i = blockIdx.x * TPB + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+    if (i >= g.N[0]) return;
+    const bool d3 = g.D == 3;
+    if (i + 1 < g.N[0] && j + 1 < g.N[1] && (!d3 || k + 1 < g.N[2])) {
+        const long long at = fld_at(g, i, j, k), sy = g.P[0], sz = d3 ? (long long)g.P[0] * g.P[1] : 0;
+        const float *E1 = F.c[0] + at, *E2 = F.c[1] + at, *E3 = F.c[2] + at;
+        const float e1 = E1[0], e2 = E2[0], e3 = E3[0];
+        const float c1 = L.cov[0], c2 = L.cov[1], c3 = L.cov[2], f = dt * L.inv_sqrt_h;
+        float curl1 = c3 * E3[sy] - c3 * e3, curl2 = -(c3 * E3[1] - c3 * e3), curl3 = (c2 * E2[1] - c2 * e2) - (c1 * E1[sy] - c1 * e1);
+        if (d3) { curl1 -= c2 * E2[sz] - c2 * e2; curl2 += c1 * E1[sz] - c1 * e1; }
+        F.c[3][at] -= curl1 * f; F.c[4][at] -= curl2 * f; F.c[5][at] -= curl3 * f;
+        return;
+    }
+    faraday_point<true, 0>(g, L, F, dt, i, j, k);
+    faraday_point<true, 1>(g, L, F, dt, i, j, k);
+    faraday_point<true, 2>(g, L, F, dt, i, j, k);
+}
+__global__ void __launch_bounds__(TPB) ampere_cart_kernel(GridDev g, SolverGeom L, FieldRW F, CurrentPtrs J, int haveJ, float dt, float jc) {
+    const int i = blockIdx.x * TPB + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+    if (i >= g.N[0]) return;
+    const bool d3 = g.D == 3;
+    if (i >= 1 && j >= 1 && (!d3 || k >= 1)) {
+        const long long at = fld_at(g, i, j, k), sy = g.P[0], sz = d3 ? (long long)g.P[0] * g.P[1] : 0;
+        const float *B1 = F.c[3] + at, *B2 = F.c[4] + at, *B3 = F.c[5] + at;
+        const float b1 = B1[0], b2 = B2[0], b3 = B3[0];
+        const float c1 = L.cov[0], c2 = L.cov[1], c3 = L.cov[2], f = dt * L.inv_sqrt_h;
+        float curl1 = c3 * b3 - c3 * B3[-sy], curl2 = -(c3 * b3 - c3 * B3[-1]), curl3 = (c2 * b2 - c2 * B2[-1]) - (c1 * b1 - c1 * B1[-sy]);
+        if (d3) { curl1 -= c2 * b2 - c2 * B2[-sz]; curl2 += c1 * b1 - c1 * B1[-sz]; }
+        const float j1 = haveJ ? J.c[0][at] : 0.f, j2 = haveJ ? J.c[1][at] : 0.f, j3 = haveJ ? J.c[2][at] : 0.f;
+        F.c[0][at] += (curl1 - jc * j1) * f; F.c[1][at] += (curl2 - jc * j2) * f; F.c[2][at] += (curl3 - jc * j3) * f;
+        return;
+    }
+    ampere_point<true, 0>(g, L, F, J, haveJ, dt, jc, i, j, k);
+    ampere_point<true, 1>(g, L, F, J, haveJ, dt, jc, i, j, k);
+    ampere_point<true, 2>(g, L, F, J, haveJ, dt, jc, i, j, k);
+}
+
 // ghost layers of the six arrays along dimension `dim` (the transverse range is the whole padded extent, so edges and corners
 // are completed dimension after dimension): PERIODIC: periodic image; AXIS: mirror image, E^1 / B^1 even, the others odd
 // (reading G10); ABSORB: not touched.  blockIdx.y = component.
