@@ -517,15 +517,27 @@ __global__ void __launch_bounds__(REBIN_TPB) rebin_count_kernel(RebinGeom G, con
     if (threadIdx.x < REBIN_CLASSES) cnt[threadIdx.x] = 0;
     __syncthreads();
     const long long p0 = tile_off[src], p1 = tile_off[src + 1];
-    for (long long base = p0; base < p1; base += REBIN_TPB) {
-        long long p = base + threadIdx.x;
-        int rel = -1, td = 0;
-        if (p < p1) { int lc; rel = G.classify_cell(cell[p], src, s, o, te, td, lc); }
-        // the ~90 % that stay (class 13 = the source tile itself) are counted with one ballot; the few others one by one
-        const unsigned stay = __ballot_sync(0xffffffffu, rel == 13);
-        if (rel == 13) { if ((int)(__ffs(stay) - 1) == (int)(threadIdx.x & 31)) atomicAdd(&cnt[13], __popc(stay)); }
-        else if (rel == 27) atomicAdd(tile_count + td, 1);
-        else if (rel >= 0) atomicAdd(&cnt[rel], 1);
+    // only the particles that LEAVE are counted (one shared atomic each, ~13 %); those that stay are the rest of the range.  Four
+    // independent loads per thread and trip.
+    for (long long base = p0; base < p1; base += 4 * REBIN_TPB) {
+        int c4[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) { const long long p = base + r * REBIN_TPB + threadIdx.x; c4[r] = p < p1 ? cell[p] : -1; }
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            if (c4[r] < 0) continue;
+            int td, lc;
+            const int rel = G.classify_cell(c4[r], src, s, o, te, td, lc);
+            if (rel == 13) continue;
+            atomicAdd(&cnt[rel], 1);
+            if (rel == 27) atomicAdd(tile_count + td, 1);
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int others = 0;
+        for (int r = 0; r < REBIN_CLASSES; ++r) if (r != 13) others += cnt[r];
+        cnt[13] = (int)(p1 - p0) - others;
     }
     __syncthreads();
     if (threadIdx.x < REBIN_CLASSES) {
