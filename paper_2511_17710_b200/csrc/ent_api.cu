@@ -620,6 +620,8 @@ static RebinGeom rebin_geom(const GridDev &g) {
     G.D = g.D;
     for (int a = 0; a < 3; ++a) { G.N[a] = g.N[a]; G.T[a] = g.T[a]; G.nt[a] = g.nt[a]; G.per[a] = g.bc[a] == ENT_PERIODIC; G.dT[a] = make_magicdiv((uint32_t)g.T[a]); }
     G.dN0 = make_magicdiv((uint32_t)g.N[0]); G.dN01 = make_magicdiv((uint32_t)(g.N[0] * g.N[1]));
+    G.dnt0 = make_magicdiv((uint32_t)g.nt[0]); G.dnt01 = make_magicdiv((uint32_t)(g.nt[0] * g.nt[1]));
+    for (int a = 0; a < 3; ++a) { int last = g.N[a] - (g.nt[a] - 1) * g.T[a]; G.mext[a] = last < g.T[a] ? last : g.T[a]; }
     return G;
 }
 

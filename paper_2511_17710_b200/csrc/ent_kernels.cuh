@@ -458,7 +458,11 @@ constexpr int REBIN_CLASSES = 28;            // 27 neighbours (3^D used) + "far"
 
 struct RebinGeom {
     int D, N[3], T[3], nt[3], per[3];
-    MagicDiv dN0, dN01, dT[3];
+    int mext[3];                 // smallest tile extent of a dimension (the last tile may be partial)
+    MagicDiv dN0, dN01, dT[3], dnt0, dnt01;
+    __device__ __forceinline__ void tile_coords(int tile, int s[3]) const {
+        s[2] = dnt01.div(tile); const int r = tile - s[2] * nt[0] * nt[1]; s[1] = dnt0.div(r); s[0] = r - s[1] * nt[0];
+    }
     __device__ __forceinline__ void tile_of_cell(int cell, int t[3]) const {
         int i0, i1, i2 = 0;
         if (D == 2) { i1 = dN0.div(cell); i0 = cell - i1 * N[0]; }
@@ -467,7 +471,9 @@ struct RebinGeom {
     }
     // Destination class of a particle of source tile s (origin o, extent te: the last tile of a dimension may be partial), its
     // destination tile td and, for a particle that stays (class 13), the index lc of its cell inside the tile.  The ~87 % that
-    // stay need the two divisions of the cell decode only; the others take the tile divisions and the wrap logic of classify.
+    // stay need the two divisions of the cell decode only; one that lands within one (smallest) tile extent of the source tile's
+    // box, the shorter way round on a periodic axis, is in the neighbour tile that three comparisons name (td is not set: only
+    // class 27 uses it); the rest take the tile divisions and the wrap logic of classify.
     __device__ __forceinline__ int classify_cell(int cell, int src, const int s[3], const int o[3], const int te[3], int &td, int &lc) const {
         int i0, i1, i2 = 0;
         if (D == 2) { i1 = dN0.div(cell); i0 = cell - i1 * N[0]; }
@@ -476,6 +482,17 @@ struct RebinGeom {
         if ((unsigned)u0 < (unsigned)te[0] && (unsigned)u1 < (unsigned)te[1] && (unsigned)u2 < (unsigned)te[2]) {
             td = src; lc = u0 + T[0] * (u1 + T[1] * u2);
             return 13;
+        }
+        {
+            int v[3] = { u0, u1, u2 }, rel = 0, mul = 1;
+            bool near = true;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                if (per[a]) { if (2 * v[a] > N[a]) v[a] -= N[a]; else if (2 * v[a] < -N[a]) v[a] += N[a]; }
+                near = near && v[a] >= -mext[a] && v[a] < te[a] + mext[a];
+                rel += (v[a] < 0 ? 0 : v[a] >= te[a] ? 2 : 1) * mul; mul *= 3;
+            }
+            if (near) { td = -1; lc = 0; return rel; }
         }
         int t[3] = { dT[0].div(i0), dT[1].div(i1), (D == 3) ? dT[2].div(i2) : 0 };
         td = t[0] + nt[0] * (t[1] + nt[1] * t[2]); lc = 0;
@@ -511,7 +528,7 @@ __global__ void __launch_bounds__(REBIN_TPB) rebin_count_kernel(RebinGeom G, con
                                                                 int32_t *class_count /* [ntiles][28] */, int32_t *tile_count) {
     __shared__ int cnt[REBIN_CLASSES];
     const int src = blockIdx.x;
-    int s[3] = { src % G.nt[0], (src / G.nt[0]) % G.nt[1], src / (G.nt[0] * G.nt[1]) };
+    int s[3]; G.tile_coords(src, s);
     const int o[3] = { s[0] * G.T[0], s[1] * G.T[1], s[2] * G.T[2] };
     const int te[3] = { min(G.T[0], G.N[0] - o[0]), min(G.T[1], G.N[1] - o[1]), G.D == 3 ? min(G.T[2], G.N[2] - o[2]) : 1 };
     if (threadIdx.x < REBIN_CLASSES) cnt[threadIdx.x] = 0;
@@ -553,7 +570,7 @@ __global__ void __launch_bounds__(REBIN_TPB) rebin_scatter_kernel(RebinGeom G, c
     __shared__ int base_s[REBIN_CLASSES], fill[REBIN_CLASSES], dest_s[REBIN_CLASSES];
     __shared__ unsigned wmx[REBIN_CLASSES];
     const int src = blockIdx.x;
-    int s[3] = { src % G.nt[0], (src / G.nt[0]) % G.nt[1], src / (G.nt[0] * G.nt[1]) };
+    int s[3]; G.tile_coords(src, s);
     const int o[3] = { s[0] * G.T[0], s[1] * G.T[1], s[2] * G.T[2] };
     const int te[3] = { min(G.T[0], G.N[0] - o[0]), min(G.T[1], G.N[1] - o[1]), G.D == 3 ? min(G.T[2], G.N[2] - o[2]) : 1 };
     if (threadIdx.x < REBIN_CLASSES) {
@@ -634,7 +651,7 @@ __global__ void __launch_bounds__(ORD_TPB) rebin_scatter_ordered_kernel(RebinGeo
     __shared__ int base_s[REBIN_CLASSES], fill[REBIN_CLASSES], dest_s[REBIN_CLASSES];
     __shared__ unsigned wmx[REBIN_CLASSES];
     const int src = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
-    int s[3] = { src % G.nt[0], (src / G.nt[0]) % G.nt[1], src / (G.nt[0] * G.nt[1]) };
+    int s[3]; G.tile_coords(src, s);
     const int o[3] = { s[0] * G.T[0], s[1] * G.T[1], s[2] * G.T[2] };
     const int te[3] = { min(G.T[0], G.N[0] - o[0]), min(G.T[1], G.N[1] - o[1]), G.D == 3 ? min(G.T[2], G.N[2] - o[2]) : 1 };
     if (tid < REBIN_CLASSES) {

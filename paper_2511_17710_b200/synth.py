@@ -465,4 +465,19 @@ def cart_absorb_small(D: int = 3, device="cpu") -> Workload:
     return Workload(f"CART-absorb-{D}D", grid, 0.45 * 0.5, 12, fields, sp, seed, "absorbing Cartesian box, partial tiles, ragged n")
 
 
+def cart_periodic_odd(device="cpu") -> Workload:
+    """parity-only edge case: fully periodic 3D box whose extents are not multiples of the tile (20 x 12 x 9 with 8^3 tiles: the last
+    tiles are 4, 4 and 1 cells thick and wrap onto the first), two tiles per periodic axis, hot plasma"""
+    seed = 9
+    N = (20, 12, 9)
+    grid = GridSpec(D=3, N=N, bc=(PERIODIC,) * 3, kind=CART, xmin=(0.0,) * 3, xmax=tuple(0.5 * n for n in N))
+    Um = uniform(seed, 8, 6 * 4 * 4, "cpu", dtype=torch.float64).view(6, 4, 4)
+    modes = [[(0.2, (int(Um[c, k, 0] * 3) + 1, int(Um[c, k, 1] * 3), int(Um[c, k, 2] * 3)), 2.0 * math.pi * float(Um[c, k, 3]))
+              for k in range(4)] for c in range(6)]
+    fields = _cart_fields_from_modes(grid, modes, (0, 0, 0, 0, 0, 1.0), device)
+    counts = torch.full((grid.ncells,), 5, dtype=torch.int64)
+    sp = load_pairs(grid, seed, counts, 0.5, 1.0, 1.0, device)
+    return Workload("CART-periodic-odd", grid, 0.45 * 0.5, 12, fields, sp, seed, "periodic Cartesian box, partial tiles that wrap")
+
+
 CONFIGS = {"C1": config1, "C2": config2, "C3": config3, "C4": config4, "C5": config5}

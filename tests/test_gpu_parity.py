@@ -32,6 +32,7 @@ def _workloads(synth):
         "SPH": lambda: synth.sph_small(48),             # linear-r spherical metric
         "ABS3": lambda: synth.cart_absorb_small(3),     # absorbing Cartesian box, partial tiles, n % 4 != 0
         "ABS2": lambda: synth.cart_absorb_small(2),
+        "PER3": lambda: synth.cart_periodic_odd(),      # periodic box 20 x 12 x 9: partial tiles (one of them 1 cell thick) that wrap
     }
 
 
@@ -147,7 +148,7 @@ def test_sorted_step_auto_path_matches_oracle(env, name):
     assert all(st["tiled"] == 1 for st in stats.values()), "the tiled kernel did not run on a sorted block"
 
 
-@pytest.mark.parametrize("name", ["C1", "C2/4", "C3/8", "C4/16-shuffled", "C5/32", "SPH", "ABS3", "ABS2"])
+@pytest.mark.parametrize("name", ["C1", "C2/4", "C3/8", "C4/16-shuffled", "C5/32", "SPH", "ABS3", "ABS2", "PER3"])
 def test_rebinned_block_matches_oracle(env, name):
     """ent_sort, steps, incremental ent_sort (re-bin) every 3 steps, steps: the tiled kernel on re-binned blocks"""
     wl = _workloads(env[1])[name]()
@@ -323,7 +324,7 @@ def test_full_sort_passes_the_oracle_checker(env, name, staging):
         assert np.array_equal(toff, ko.cpu().numpy()[::tcells]), "tile offsets != key offsets at the tile boundaries"
 
 
-@pytest.mark.parametrize("name", ["C1", "C3/8", "C4/16-shuffled", "C5/32", "ABS3"])
+@pytest.mark.parametrize("name", ["C1", "C3/8", "C4/16-shuffled", "C5/32", "ABS3", "PER3"])
 def test_rebin_tile_offsets_are_the_scan_of_the_tile_histogram(env, name):
     """S10, incremental form: after steps + re-bin, the block is tile-contiguous and the ctx's tile offsets equal the exclusive scan
     of the histogram of tile(key) recomputed on the host (checked with the oracle's checker on the TILE keys)."""
@@ -521,7 +522,7 @@ def test_compact_matches_oracle(env, name):
     assert bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED) == 1
 
 
-@pytest.mark.parametrize("name", ["C1", "C3/8", "C3/8-uneven", "C4/16-shuffled", "ABS3", "ABS2"])
+@pytest.mark.parametrize("name", ["C1", "C3/8", "C3/8-uneven", "C4/16-shuffled", "ABS3", "ABS2", "PER3"])
 def test_step_pair_matches_oracle(env, name):
     """ent_step_pair: both species of the pair plasma through one launch of the tiled kernel (one E,B box, one J tile per tile).
     Same bars as the single-species tests: the summed current of the two species against the oracle's, particles per species,
