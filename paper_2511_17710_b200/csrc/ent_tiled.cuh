@@ -237,10 +237,11 @@ __device__ __forceinline__ void tile_segment(int *sJ, const CarryCtx &cc, int ba
             old[4 * comp] = atomicAdd(Jc, v[4 * comp]); old[4 * comp + 1] = atomicAdd(Jc + st[a], v[4 * comp + 1]);
             old[4 * comp + 2] = atomicAdd(Jc + st[bb], v[4 * comp + 2]); old[4 * comp + 3] = atomicAdd(Jc + st[a] + st[bb], v[4 * comp + 3]);
         }
-        unsigned flag = 0u;
+        int mx = __vimax3_s32(old[0], old[1], old[2]), mn = __vimin3_s32(old[0], old[1], old[2]);     // VIMNMX3
 #pragma unroll
-        for (int k = 0; k < 12; ++k) flag |= (unsigned)old[k] + 0x40000000u;
-        if ((int)flag < 0) {
+        for (int k = 3; k < 11; k += 2) { mx = __vimax3_s32(mx, old[k], old[k + 1]); mn = __vimin3_s32(mn, old[k], old[k + 1]); }
+        mx = max(mx, old[11]); mn = min(mn, old[11]);
+        if (mx >= 0x40000000 || mn < -0x40000000) {
 #pragma unroll
             for (int k = 0; k < 12; ++k) {
                 const int comp = k / 4, a = (comp + 1) % 3, bb = (comp + 2) % 3;
