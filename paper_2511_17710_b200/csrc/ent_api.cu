@@ -374,7 +374,7 @@ extern "C" int ent_filter_current(ent_ctx *ctx, ent_current *J, int npasses, int
     CurrentPtrs a = cp(J), b;
     for (int c = 0; c < 3; ++c) b.c[c] = (float *)((char *)ctx->fbuf + slot * c);
     const int nkc = (nmax[2] + FT_K - 1) / FT_K;
-    const dim3 fgrid((nmax[0] + FT_W - 1) / FT_W, (nmax[1] + FT_J - 1) / FT_J, 3 * nkc);
+    const dim3 fgrid((nmax[0] + FT_W - 1) / FT_W, (nmax[1] + FT_ROWS - 1) / FT_ROWS, 3 * nkc);
     if (fgrid.y > 65535u || fgrid.z > 65535u) return fail(ctx, ENT_EUNSUPPORTED, "grid too large for the filter kernel");
     const int total = npasses ? npasses : 1;
     for (int pass = 0; pass < total; ++pass) {

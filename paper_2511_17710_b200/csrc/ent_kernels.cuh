@@ -194,53 +194,71 @@ __device__ __forceinline__ float sqrt_h_at(const GridDev &g, double x1, double x
     const double eR = exp(g.Rmin + x1 * g.dR), T = x2 * g.dT, r = g.r0 + eR;
     return (float)((g.dR * eR) * (g.dT * dtheta_dT(g.vt, T) * r) * (r * sin(theta_of_T(g.vt, T))));
 }
-// One pass, no shared memory and no barriers: a warp owns FT_W = 30 consecutive points of one lattice row (its 32 lanes sit on
-// x = i0 - 1 .. i0 + 30, the two outer lanes are halo) and marches along x3.  Per plane a lane loads the three values
-// J(x, j - 1 .. j + 1, k) (coalesced rows; the rows shared with the neighbouring warps of the CTA come from L1), filters them along
-// x2 in registers, gets its x1 neighbours by two shuffles, and keeps the in-plane sums P_{k-1}, P_k, P_{k+1} in registers:
-// out_k = P_{k-1}/4 + P_k/2 + P_{k+1}/4 (f = (1/2)^(D + |di| + |dj| + |dk|) = w(di) w(dj) w(dk), Eqs. 9-11); in 2D out = P.  The
-// loads of FT_U planes are issued together before the first of them is used.  A CTA whose whole neighbourhood lies inside the lattice of a
-// Cartesian grid loads without boundary logic (INTERIOR, compile time); the others go through filter_fetch.
+// One pass, no shared memory and no barriers: a warp owns FT_W = 30 consecutive points of FT_R consecutive lattice rows (its 32
+// lanes sit on x = i0 - 1 .. i0 + 30, the two outer lanes are halo) and marches along x3.  Per plane a lane loads the FT_R + 2
+// values J(x, j - 1 .. j + FT_R, k) (coalesced rows, all in flight together; the two rows shared with the neighbouring warps of the
+// CTA come from L1), filters them along x2 in registers, gets its x1 neighbours by two shuffles per row, and keeps the in-plane sums
+// P_{k-1}, P_k, P_{k+1} of its rows in registers: out_k = P_{k-1}/4 + P_k/2 + P_{k+1}/4 (f = (1/2)^(D + |di| + |dj| + |dk|) =
+// w(di) w(dj) w(dk), Eqs. 9-11); in 2D out = P.  The boundary rules are applied once per lane column, warp row and plane (MAPPED,
+// see filter_load_rows), not per load.
 // mode 0: filter; 1: no convolution (scaling pass only); 2: copy.  blockIdx.z = component * nkc + chunk of FT_K planes.
-constexpr int FT_W = 30, FT_J = 8, FT_K = 32, FT_TPB = 32 * FT_J, FT_U = 1;
-struct FilterRow { const float *A; int comp, x, j, k0, k1, n0, n1; long long P0, P01; };
-template <bool INTERIOR>
-__device__ __forceinline__ void filter_load3(const GridDev &g, const FilterGeom &L, const FilterRow &t, int k, float v[3]) {
-    if (INTERIOR) {
-        const float *p = t.A + ((long long)(t.x + NG) + t.P0 * (t.j - 1 + NG) + t.P01 * (k + NG));
-        v[0] = __ldg(p); v[1] = __ldg(p + t.P0); v[2] = __ldg(p + 2 * t.P0);
+constexpr int FT_W = 30, FT_R = 3, FT_J = 4, FT_ROWS = FT_R * FT_J, FT_K = 16, FT_TPB = 32 * FT_J;   // measured: (R, warps, planes) = (3, 4, 16) .. (4, 4, 64) within 5 %
+struct FilterRow { const float *A; int comp, x, j, k0, k1, n0, n1, n2; long long P0, P01;
+                   int xo, ro[FT_R + 2], P01i; float xf, rf[FT_R + 2]; };     // MAPPED path: element offsets (a padded array has < 2^31 elements) and factors of the lane's column and the warp's rows
+// the boundary rule of one dimension as (mapped index, factor): periodic image, mirror image about the polar axis (odd for the
+// component along the dimension, even otherwise), zero beyond an ABSORB side.  An index more than one image away is not needed by
+// any lattice point and maps to (0, 0).
+__device__ __forceinline__ void filter_map1(const FilterGeom &L, int comp, int d, int q, int &qq, float &f) {
+    const int n = L.n[comp][d];
+    qq = q; f = 1.f;
+    if ((unsigned)q < (unsigned)n) return;
+    if (L.rule[d] == ENT_PERIODIC) qq = q + (q < 0 ? n : -n);
+    else if (L.rule[d] == ENT_AXIS) {
+        if (comp == d) { qq = q < 0 ? -1 - q : 2 * n - 1 - q; f = -1.f; }
+        else qq = q < 0 ? -q : 2 * (n - 1) - q;
+    } else { qq = 0; f = 0.f; }
+    if ((unsigned)qq >= (unsigned)n) { qq = 0; f = 0.f; }
+}
+// MAPPED: the rules of filter_fetch are separable, so the lane's column, the warp's rows and the plane are mapped once each and a
+// load is one address and (SIGNED: grids with a side that is not periodic) one multiplication.  !MAPPED: filter_fetch per load
+// (lattices too small for the one-image mapping).
+template <bool MAPPED, bool SIGNED>
+__device__ __forceinline__ void filter_load_rows(const GridDev &g, const FilterGeom &L, const FilterRow &t, int k, float v[FT_R + 2]) {
+    if (MAPPED) {
+        int kk = k; float kf = 1.f;                                                          // warp-uniform
+        if (SIGNED) filter_map1(L, t.comp, 2, k, kk, kf);
+        else { kk += kk < 0 ? t.n2 : 0; kk -= kk >= t.n2 ? t.n2 : 0; }                       // every side periodic
+        const float *p = t.A + (t.xo + t.P01i * (kk + NG));
+#pragma unroll
+        for (int r = 0; r < FT_R + 2; ++r) { v[r] = __ldg(p + t.ro[r]); if (SIGNED) v[r] *= t.xf * t.rf[r] * kf; }
     } else {
 #pragma unroll
-        for (int r = 0; r < 3; ++r) v[r] = (t.x <= t.n0 && t.j - 1 + r <= t.n1) ? filter_fetch(g, L, t.A, t.comp, t.x, t.j - 1 + r, k) : 0.f;
+        for (int r = 0; r < FT_R + 2; ++r) v[r] = (t.x <= t.n0 && t.j - 1 + r <= t.n1) ? filter_fetch(g, L, t.A, t.comp, t.x, t.j - 1 + r, k) : 0.f;
     }
 }
-__device__ __forceinline__ float filter_in_plane(const float v[3]) {
-    const float c = 0.25f * v[0] + 0.5f * v[1] + 0.25f * v[2];                  // along x2, in the lane
-    const float l = __shfl_up_sync(0xffffffffu, c, 1), r = __shfl_down_sync(0xffffffffu, c, 1);
-    return 0.25f * l + 0.5f * c + 0.25f * r;                                    // along x1, across lanes (valid on lanes 1 .. 30)
+__device__ __forceinline__ void filter_in_plane(const float v[FT_R + 2], float P[FT_R]) {
+#pragma unroll
+    for (int r = 0; r < FT_R; ++r) {
+        const float c = 0.25f * v[r] + 0.5f * v[r + 1] + 0.25f * v[r + 2];      // along x2, in the lane
+        const float l = __shfl_up_sync(0xffffffffu, c, 1), rr = __shfl_down_sync(0xffffffffu, c, 1);
+        P[r] = 0.25f * l + 0.5f * c + 0.25f * rr;                               // along x1, across lanes (valid on lanes 1 .. 30)
+    }
 }
-template <bool INTERIOR, class EMIT>
+template <bool MAPPED, bool SIGNED, class EMIT>
 __device__ __forceinline__ void filter_march(const GridDev &g, const FilterGeom &L, const FilterRow &t, bool d3, EMIT &&emit) {
-    float v[3];
-    if (!d3) { filter_load3<INTERIOR>(g, L, t, 0, v); emit(0, filter_in_plane(v)); return; }
-    filter_load3<INTERIOR>(g, L, t, t.k0 - 1, v);
-    float Pm = filter_in_plane(v);
-    filter_load3<INTERIOR>(g, L, t, t.k0, v);
-    float Pc = filter_in_plane(v);
-    for (int kb = t.k0; kb < t.k1; kb += FT_U) {                     // FT_U planes per trip (1 measured best: 2 and 4 were 4 % and 12 % slower)
-        float w[FT_U][3];
+    float v[FT_R + 2], Pm[FT_R], Pc[FT_R], Pn[FT_R];
+    if (!d3) {
+        filter_load_rows<MAPPED, SIGNED>(g, L, t, 0, v); filter_in_plane(v, Pc);
 #pragma unroll
-        for (int u = 0; u < FT_U; ++u) {
-            w[u][0] = w[u][1] = w[u][2] = 0.f;
-            if (kb + u < t.k1) filter_load3<INTERIOR>(g, L, t, kb + u + 1, w[u]);
-        }
+        for (int r = 0; r < FT_R; ++r) emit(0, r, Pc[r]);
+        return;
+    }
+    filter_load_rows<MAPPED, SIGNED>(g, L, t, t.k0 - 1, v); filter_in_plane(v, Pm);
+    filter_load_rows<MAPPED, SIGNED>(g, L, t, t.k0, v); filter_in_plane(v, Pc);
+    for (int k = t.k0; k < t.k1; ++k) {
+        filter_load_rows<MAPPED, SIGNED>(g, L, t, k + 1, v); filter_in_plane(v, Pn);
 #pragma unroll
-        for (int u = 0; u < FT_U; ++u) {
-            if (kb + u >= t.k1) break;
-            const float Pn = filter_in_plane(w[u]);
-            emit(kb + u, 0.25f * Pm + 0.5f * Pc + 0.25f * Pn);
-            Pm = Pc; Pc = Pn;
-        }
+        for (int r = 0; r < FT_R; ++r) { emit(k, r, 0.25f * Pm[r] + 0.5f * Pc[r] + 0.25f * Pn[r]); Pm[r] = Pc[r]; Pc[r] = Pn[r]; }
     }
 }
 __global__ void __launch_bounds__(FT_TPB) filter_pass_kernel(GridDev g, FilterGeom L, CurrentPtrs src, CurrentPtrs dst, int mode, int divide, int nkc) {
@@ -249,33 +267,53 @@ __global__ void __launch_bounds__(FT_TPB) filter_pass_kernel(GridDev g, FilterGe
     const int kc = blockIdx.z - t.comp * nkc;
     const int n2 = L.n[t.comp][2];
     t.n0 = L.n[t.comp][0]; t.n1 = L.n[t.comp][1];
-    const int lane = threadIdx.x & 31, i0 = blockIdx.x * FT_W, j0 = blockIdx.y * FT_J;
+    const int lane = threadIdx.x & 31, i0 = blockIdx.x * FT_W, j0 = blockIdx.y * FT_ROWS;
     t.k0 = kc * FT_K;
     if (i0 >= t.n0 || j0 >= t.n1 || t.k0 >= n2) return;              // the grid is sized for the largest lattice
     t.k1 = min(t.k0 + FT_K, n2);
-    t.x = i0 - 1 + lane; t.j = j0 + (threadIdx.x >> 5);
+    t.x = i0 - 1 + lane; t.j = j0 + (threadIdx.x >> 5) * FT_R;       // first of the warp's rows
+    if (t.j >= t.n1) return;                                         // whole warp: none of its rows exists (no barriers in this kernel)
     t.A = src.c[t.comp];
     float *O = dst.c[t.comp];
     t.P0 = g.P[0]; t.P01 = g.D == 3 ? (long long)g.P[0] * g.P[1] : 0;
-    const bool mine = lane >= 1 && lane <= FT_W && t.x < t.n0 && t.j < t.n1;    // this lane owns the lattice point (x, j)
+    const bool mine_x = lane >= 1 && lane <= FT_W && t.x < t.n0;     // this lane owns the lattice points (x, j .. j + FT_R - 1)
     const long long at = (long long)(t.x + NG) + t.P0 * (t.j + NG) + (g.D == 3 ? t.P01 * NG : 0);     // (x, j, k = 0)
-    const bool axis_node = filter_on_axis(g, L, t.comp, t.j);
-    const float sh = (divide && mine && !axis_node) ? sqrt_h_at(g, t.x + (t.comp == 0 ? 0.5 : 0.0), t.j + (t.comp == 1 ? 0.5 : 0.0)) : 1.f;
-    const bool zero = mode == 0 && t.comp == 2 && axis_node;                    // J^3(i, 0) = 0
-    auto emit = [&](int k, float a) {
-        if (!mine) return;
-        if (zero) a = 0.f;
-        if (divide && !axis_node) a /= sh;
-        O[at + t.P01 * k] = a;
+    float sh[FT_R]; bool axis_node[FT_R];
+#pragma unroll
+    for (int r = 0; r < FT_R; ++r) {
+        axis_node[r] = filter_on_axis(g, L, t.comp, t.j + r);
+        sh[r] = (divide && mine_x && t.j + r < t.n1 && !axis_node[r]) ? sqrt_h_at(g, t.x + (t.comp == 0 ? 0.5 : 0.0), t.j + r + (t.comp == 1 ? 0.5 : 0.0)) : 1.f;
+    }
+    auto emit = [&](int k, int r, float a) {
+        if (!mine_x || t.j + r >= t.n1) return;
+        if (mode == 0 && t.comp == 2 && axis_node[r]) a = 0.f;                  // J^3(i, 0) = 0
+        if (divide && !axis_node[r]) a /= sh[r];
+        O[at + t.P0 * r + t.P01 * k] = a;
     };
     if (mode != 0) {
-        if (mine) for (int k = t.k0; k < t.k1; ++k) emit(k, t.A[at + t.P01 * k]);
+        if (mine_x)
+            for (int k = t.k0; k < t.k1; ++k)
+#pragma unroll
+                for (int r = 0; r < FT_R; ++r) if (t.j + r < t.n1) emit(k, r, t.A[at + t.P0 * r + t.P01 * k]);
         return;
     }
     const bool d3 = g.D == 3;
-    const bool interior = g.kind == ENT_CART && i0 >= 1 && i0 + FT_W + 1 <= t.n0 && j0 >= 1 && j0 + FT_J + 1 <= t.n1 &&
-                          (!d3 || (t.k0 >= 1 && t.k1 + 1 <= n2));
-    if (interior) filter_march<true>(g, L, t, d3, emit); else filter_march<false>(g, L, t, d3, emit);
+    const bool mapped = t.n0 >= 2 && t.n1 >= FT_R + 2 && (!d3 || n2 >= 3);
+    if (mapped) {
+        bool sgn = false;
+        for (int d = 0; d < g.D; ++d) sgn = sgn || L.rule[d] != ENT_PERIODIC;
+        int xx; float f; filter_map1(L, t.comp, 0, t.x, xx, f);
+        if (sgn) t.xf = f;                                            // every side periodic: the factors are 1 and are not kept
+        t.xo = xx + NG; t.P01i = (int)t.P01; t.n2 = n2;
+#pragma unroll
+        for (int r = 0; r < FT_R + 2; ++r) {
+            int jj; filter_map1(L, t.comp, 1, t.j - 1 + r, jj, f);
+            if (t.comp == 2 && filter_on_axis(g, L, t.comp, jj)) f = 0.f;                       // J^3(i, 0) = 0: a condition on the INPUT of the stencil
+            if (sgn) t.rf[r] = f;
+            t.ro[r] = (int)t.P0 * (jj + NG);
+        }
+        if (sgn) filter_march<true, true>(g, L, t, d3, emit); else filter_march<true, false>(g, L, t, d3, emit);
+    } else filter_march<false, false>(g, L, t, d3, emit);
 }
 
 // ---- N4: tag sort: stable partition, alive particles first ----
