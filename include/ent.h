@@ -193,6 +193,19 @@ int ent_fold_current(ent_ctx *ctx, ent_current *J);
  * Scratch (12 bytes per particle) is allocated in the ctx on first use (may synchronise). */
 int ent_compact(ent_ctx *ctx, const ent_particles *in, ent_particles *out, int64_t *n_alive);
 
+/* ent_compact_static: the same operation and arguments as ent_compact for callers that cannot allocate device memory
+ * (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the call makes NO cudaMalloc / cudaFree and calls
+ * no allocating routine, and does not synchronise.  Its scratch (flags, positions and chunk sums of the scan, 12 bytes per particle)
+ * is a static __device__ array inside the library, 12.6 MB, which every GPU that loads the library holds until the process exits;
+ * its device address is looked up once per device (cudaGetSymbolAddress) when a ctx is created on that device.
+ * Limit: n <= ENT_COMPACT_STATIC_MAX_N particles; a larger block is refused with ENT_EINVAL (message in ent_last_error), nothing is
+ * launched.  in, out and n_alive are the caller's device memory as for ent_compact; the result is identical (bit for bit) to
+ * ent_compact's.  The array is shared by EVERY call in the process on that GPU, whatever the ctx or stream, and keeps the last
+ * call's contents (nothing in it has to start at zero: each call writes what it reads): two calls that overlap on the GPU race;
+ * order them on one stream or with events. */
+#define ENT_COMPACT_STATIC_MAX_N (1 << 20)
+int ent_compact_static(ent_ctx *ctx, const ent_particles *in, ent_particles *out, int64_t *n_alive);
+
 /* ---- step 9 of the loop: current post-processing ------------------------------------------------------------
  * ent_filter_current: `npasses` digital filter passes on the conformal currents (Eqs. 9-11: the (1/4, 1/2, 1/4)
  * kernel along every grid dimension, each component on its own staggered lattice) and then, if divide_by_sqrt_h != 0, the

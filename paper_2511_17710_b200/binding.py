@@ -22,7 +22,7 @@ OPT_STEP_IMPL, OPT_TILE_1, OPT_TILE_2, OPT_TILE_3, OPT_SORT_MODE, OPT_CURV_FP64,
  STAT_SCRATCH_BYTES, STAT_LAST_STEP_TILED, STAT_LAST_SORT_REBIN, STAT_SLOT_ERRORS, STAT_CARRIES, STAT_GLOBAL_ADDS) = range(1, 15)
 
 SYMBOLS = ["ent_create", "ent_destroy", "ent_last_error", "ent_set_grid", "ent_gather_push", "ent_deposit", "ent_sort",
-           "ent_step", "ent_step_pair", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_filter_current", "ent_faraday", "ent_ampere", "ent_fill_field_ghosts", "ent_compact", "ent_step_host", "ent_step_host_pair", "ent_set_option", "ent_set_gca", "ent_get_stat", "ent_version"]
+           "ent_step", "ent_step_pair", "ent_step_sorted", "ent_workspace_bytes", "ent_reserve", "ent_forget", "ent_tile_offsets", "ent_zero_current", "ent_fold_current", "ent_filter_current", "ent_faraday", "ent_ampere", "ent_fill_field_ghosts", "ent_compact", "ent_compact_static", "ent_step_host", "ent_step_host_pair", "ent_set_option", "ent_set_gca", "ent_get_stat", "ent_version"]
 
 
 class EntError(RuntimeError):
@@ -83,6 +83,7 @@ def lib():
         L.ent_ampere.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Current), C.c_float, C.c_float]
         L.ent_fill_field_ghosts.argtypes = [vp, C.POINTER(_Fields)]
         L.ent_compact.argtypes = [vp, C.POINTER(_Particles), C.POINTER(_Particles), vp]
+        L.ent_compact_static.argtypes = [vp, C.POINTER(_Particles), C.POINTER(_Particles), vp]
         L.ent_step_host.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Current), C.c_float, C.c_int,
                                     C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.ent_step_host_pair.argtypes = [vp, C.POINTER(_Fields), C.POINTER(_Particles), C.POINTER(_Particles), C.POINTER(_Current), C.c_float, C.c_int,
@@ -315,6 +316,15 @@ def ent_compact(ctx: Ctx, pin: Particles, pout: Particles) -> torch.Tensor:
     na = torch.zeros(1, dtype=torch.int64, device=pin.cell.device)
     ctx._ck(lib().ent_compact(ctx._h, C.byref(pin.c()), C.byref(pout.c()), na.data_ptr()))
     return na
+
+
+COMPACT_STATIC_MAX_N = 1 << 20
+
+
+def ent_compact_static(ctx: Ctx, pin: Particles, pout: Particles, n_alive: torch.Tensor) -> None:
+    """ent_compact with the library's static scratch: no device allocation by the call (n <= COMPACT_STATIC_MAX_N); n_alive is the
+    caller's one-element int64 device tensor"""
+    ctx._ck(lib().ent_compact_static(ctx._h, C.byref(pin.c()), C.byref(pout.c()), n_alive.data_ptr()))
 
 
 def ent_filter_current(ctx: Ctx, J, npasses: int, divide_by_sqrt_h: bool = False) -> None:

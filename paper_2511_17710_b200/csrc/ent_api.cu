@@ -5,6 +5,7 @@
 #include <stdio.h>
 #include <string.h>
 #include <new>
+#include <mutex>
 
 #include "ent_kernels.cuh"
 #include "ent_tiled_axisym.cuh"
@@ -142,6 +143,34 @@ extern "C" const char *ent_version(void) { return "0.2"; }
 
 extern "C" const char *ent_last_error(const ent_ctx *ctx) { return ctx ? ctx->err : "null ctx"; }
 
+// ---- scratch of ent_compact_static: lives in the module image, no allocation call ever made for it ------------------------
+// Layout = the one ent_compact carves out of its heap buffer: flags, positions, cursor copy ((n + 1) int32 each, 256-byte slots)
+// and the chunk sums of the scan.  Every GPU that loads the library holds these bytes until the process exits.
+constexpr long long COMPACT_STATIC_MAX_N = ENT_COMPACT_STATIC_MAX_N;
+constexpr size_t COMPACT_STATIC_SLOT = ((size_t)(COMPACT_STATIC_MAX_N + 1) * 4 + 255) & ~(size_t)255;
+constexpr size_t COMPACT_STATIC_CHUNKS = ((size_t)((COMPACT_STATIC_MAX_N + SCAN_CHUNK - 1) / SCAN_CHUNK) * 4 + 255) & ~(size_t)255;
+constexpr size_t COMPACT_STATIC_BYTES = 3 * COMPACT_STATIC_SLOT + COMPACT_STATIC_CHUNKS;       // 12.6 MB for 2^20 particles
+static __device__ __align__(256) unsigned char compact_static_scratch[COMPACT_STATIC_BYTES];
+
+// In host code `compact_static_scratch` is a host-side stand-in, NOT a device address: the address the kernels get is looked up
+// once per device (that device current) with cudaGetSymbolAddress and kept here.
+constexpr int STATIC_MAX_DEVICES = 64;
+static std::mutex static_scratch_mutex;
+static void *static_scratch_addr[STATIC_MAX_DEVICES] = {};
+static cudaError_t static_scratch_lookup(int device, void **ptr) {           // the caller has made `device` current
+    *ptr = nullptr;
+    if (device < 0 || device >= STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(static_scratch_mutex);
+    if (!static_scratch_addr[device]) {
+        void *a = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&a, compact_static_scratch);
+        if (e != cudaSuccess) { cudaGetLastError(); return e; }
+        static_scratch_addr[device] = a;
+    }
+    *ptr = static_scratch_addr[device];
+    return cudaSuccess;
+}
+
 extern "C" int ent_create(ent_ctx **out, int device, void *cuda_stream) {
     if (!out) return ENT_EINVAL;
     *out = nullptr;
@@ -157,6 +186,7 @@ extern "C" int ent_create(ent_ctx **out, int device, void *cuda_stream) {
         cudaMemsetAsync(ctx->counters, 0, 8 * sizeof(unsigned long long), ctx->stream) != cudaSuccess) {
         cudaGetLastError(); delete ctx; return ENT_ECUDA;
     }
+    { void *unused; (void)static_scratch_lookup(device, &unused); }   // set-up of ent_compact_static; a failure is reported by that call
     *out = ctx;
     return ENT_OK;
 }
@@ -742,6 +772,42 @@ extern "C" int ent_compact(ent_ctx *ctx, const ent_particles *in, ent_particles 
     if ((rc = ensure(ctx, &ctx->cbuf, &ctx->cbuf_cap, 3 * slot + nch))) return rc;
     int32_t *flag = (int32_t *)ctx->cbuf, *pos = (int32_t *)((char *)ctx->cbuf + slot), *copy = (int32_t *)((char *)ctx->cbuf + 2 * slot);
     int32_t *chunk = (int32_t *)((char *)ctx->cbuf + 3 * slot);
+    const int nchunks = (int)((n + SCAN_CHUNK - 1) / SCAN_CHUNK);
+    compact_flag_kernel<<<nblk(n), TPB, 0, ctx->stream>>>(in->tag, n, flag);
+    if ((rc = launch_check(ctx, "compact_flag_kernel"))) return rc;
+    scan_reduce_kernel<<<nchunks, TPB, 0, ctx->stream>>>(flag, n, chunk);
+    if ((rc = launch_check(ctx, "scan_reduce_kernel"))) return rc;
+    scan_chunks_kernel<<<1, TPB, 0, ctx->stream>>>(chunk, nchunks);
+    if ((rc = launch_check(ctx, "scan_chunks_kernel"))) return rc;
+    scan_apply_kernel<<<nchunks, TPB, 0, ctx->stream>>>(flag, n, chunk, pos, copy);
+    if ((rc = launch_check(ctx, "scan_apply_kernel"))) return rc;
+    compact_scatter_kernel<<<nblk(n), TPB, 0, ctx->stream>>>(pos, pp(in), pp(out), n, g.D, g.kind != ENT_CART, (long long *)n_alive);
+    return launch_check(ctx, "compact_scatter_kernel");
+}
+
+// ent_compact without any allocation: the scan's scratch is the module's static array (see compact_static_scratch above)
+extern "C" int ent_compact_static(ent_ctx *ctx, const ent_particles *in, ent_particles *out, int64_t *n_alive) {
+    ENTER();
+    int rc;
+    if ((rc = check_particles(ctx, in, "in", false)) || (rc = check_particles(ctx, out, "out", false))) return rc;
+    if (in->n != out->n) return fail(ctx, ENT_EINVAL, "in->n != out->n");
+    if (in->n > COMPACT_STATIC_MAX_N)
+        return fail(ctx, ENT_EINVAL, "ent_compact_static: n = %lld exceeds the static scratch (ENT_COMPACT_STATIC_MAX_N = %lld particles); use ent_compact",
+                    (long long)in->n, (long long)COMPACT_STATIC_MAX_N);
+    if (in->n > 0 && (in->cell == out->cell || in->w == out->w)) return fail(ctx, ENT_EINVAL, "ent_compact_static is out-of-place: in and out overlap");
+    if (!in->tag || !out->tag) return fail(ctx, ENT_EINVAL, "ent_compact_static needs tag arrays in both blocks");
+    const GridDev &g = ctx->g;
+    const long long n = in->n;
+    out->q = in->q; out->m = in->m;
+    forget_block(ctx, out->cell);
+    if (n == 0) { if (n_alive) CK(cudaMemsetAsync(n_alive, 0, sizeof(int64_t), ctx->stream)); return ENT_OK; }
+    void *base = nullptr;
+    cudaError_t e = static_scratch_lookup(ctx->device, &base);
+    if (e != cudaSuccess || !base) return fail(ctx, ENT_ECUDA, "cudaGetSymbolAddress of the static scratch failed: %s", cudaGetErrorString(e));
+    // nothing has to start at zero: every element read below (flags 0 .. n-1, chunk sums, positions 0 .. n) is written by this call first
+    const size_t slot = ((size_t)(n + 1) * 4 + 255) & ~(size_t)255;
+    int32_t *flag = (int32_t *)base, *pos = (int32_t *)((char *)base + slot), *copy = (int32_t *)((char *)base + 2 * slot);
+    int32_t *chunk = (int32_t *)((char *)base + 3 * slot);
     const int nchunks = (int)((n + SCAN_CHUNK - 1) / SCAN_CHUNK);
     compact_flag_kernel<<<nblk(n), TPB, 0, ctx->stream>>>(in->tag, n, flag);
     if ((rc = launch_check(ctx, "compact_flag_kernel"))) return rc;
