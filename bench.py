@@ -45,16 +45,32 @@ def _peaks():
 
 
 def _committed_traffic(workload, mode):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture table (profiles/r2_traffic.csv), or (None, None)"""
+    """(DRAM bytes, warp instructions) per launch of the dominant kernel and their source from the committed ncu capture table
+    (profiles/r2_traffic.csv), or (None, None, None)"""
     import csv
     p = os.path.join(ROOT, "profiles", "r2_traffic.csv")
     try:
         for row in csv.DictReader(open(p)):
             if row["workload"] == workload and row["mode"] == mode:
-                return float(row["dram_bytes_per_launch"]), row["source"]
+                wi = row.get("warp_instructions_per_launch")
+                return float(row["dram_bytes_per_launch"]), (float(wi) if wi else None), row["source"]
     except OSError:
         pass
-    return None, None
+    return None, None, None
+
+
+def _issue_ceiling(warp_instr, k_ms, sm_max_mhz, alg_bytes, peak_gbs):
+    """Second ceiling of the step kernel (DESIGN.md sect. 5): a B200 issues at most 148 SMs x 4 schedulers x 1 warp instruction per
+    cycle.  With the warp instructions of one launch (committed ncu capture) this gives the issue rate the launch reached and the
+    fraction of the HBM roofline the same instruction stream could reach at 100 % issue."""
+    if not warp_instr or not sm_max_mhz:
+        return None
+    peak = 148 * 4 * sm_max_mhz * 1e6                       # warp instructions per second
+    rate = warp_instr / (k_ms * 1e-3)
+    t_min = warp_instr / peak                               # seconds per launch at 100 % issue
+    return {"warp_instructions_per_launch": warp_instr, "achieved_ginst_s": rate / 1e9, "peak_ginst_s": peak / 1e9, "frac": rate / peak,
+            "hbm_frac_at_full_issue": alg_bytes / t_min / 1e9 / peak_gbs,
+            "note": "148 SMs x 4 schedulers x SM clock; instruction count from the committed ncu capture named in traffic_source"}
 
 
 def max_over_ranks(value: float, device) -> float:
@@ -310,9 +326,9 @@ def measure(args, name, env, want_e2e):
     alg_bytes = pbytes * npart / len(parts) * per_launch + GRID_BYTES_PER_CELL * ncell
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
     mean = lambda ev: (sum(a.elapsed_time(b) for a, b in ev) / len(ev)) if ev else None
-    traffic, traffic_src = args.traffic, args.traffic_source
+    traffic, traffic_src, warp_instr = args.traffic, args.traffic_source, None
     if traffic is None and args.shrink == 1 and not args.tile:
-        traffic, traffic_src = _committed_traffic(name, "pair" if paired else ("sorted" if fused else "inplace"))
+        traffic, warp_instr, traffic_src = _committed_traffic(name, "pair" if paired else ("sorted" if fused else "inplace"))
     out = {"name": name, "value": value, "ms_per_step": ms_per_step, "ms_timed": ms, "reps": reps, "npart": npart, "launches": launches,
            "clocks": clk, "tiled": bool(tiled), "strays": strays, "bad_moves": bad, "kernel_ms": k_ms,
            "sort_ms_per_species": mean(sort_ev), "first_sort_ms_per_species": mean(first_sort), "first_sort_direct_ms": mean(first_direct), "fused": fused, "paired": paired,
@@ -322,7 +338,8 @@ def measure(args, name, env, want_e2e):
                         "kernel": ("ent_step_sorted" if fused else "ent_step_pair" if paired else "ent_step") + " (fused gather+push+move+deposit), "
                                   + ("both species of the pair plasma per launch" if paired else "one species per launch"),
                         "kernel_ms": k_ms, "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
-                        "step_share": k_ms * len(parts) / per_launch / ms_per_step}}
+                        "step_share": k_ms * len(parts) / per_launch / ms_per_step,
+                        "issue": _issue_ceiling(warp_instr, k_ms, (clk or {}).get("sm_max_mhz"), alg_bytes, peak)}}
 
     # ---- step 9: 4 digital filter passes (the count of the paper's magnetosphere runs) + J = conformal J / sqrt(h)
     npass = 4
