@@ -475,7 +475,7 @@ def main():
                     help="default: C3 as the headline plus the per_config list of the other configurations")
     ap.add_argument("--shrink", type=int, default=1)
     ap.add_argument("--sort-every", type=int, default=3, help="ent_sort every k steps inside the timed region (0 = never)")
-    ap.add_argument("--step-impl", type=int, default=0, help="ENT_OPT_STEP_IMPL: 0 auto, 1 untiled, 2 two-kernel")
+    ap.add_argument("--step-impl", type=int, default=0, help="ENT_OPT_STEP_IMPL: 0 auto, 1 untiled, 2 two-kernel, 3 auto with the one-launch pair step on any grid")
     ap.add_argument("--sort-mode", type=int, default=0, help="ENT_OPT_SORT_MODE: 0 auto (incremental re-bin), 1 always the full sort")
     ap.add_argument("--tile", default="", help="tile extents in cells, e.g. 8,8,4 (ENT_OPT_TILE_*; default: the library's)")
     ap.add_argument("--mode", default="pair", choices=["pair", "sorted", "inplace"],

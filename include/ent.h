@@ -148,8 +148,8 @@ int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_current *
 /* ent_step_pair = ent_step(p1) + ent_step(p2) for two species on the same grid (the pair plasma of the paper's runs) in ONE
  * launch of the tiled kernel: a CTA stages the E,B box of its tile once, advances the tile's particles of both blocks and flushes
  * one J tile (half the per-tile work and half the field / current traffic of two launches).  Both blocks must be sorted blocks of
- * this ctx on a Cartesian grid the tiled kernel supports and either both or neither carry tags; otherwise the call is exactly the
- * two ent_step calls.  A tile is not split across CTAs here: meant for plasmas whose tile populations are of one order.
+ * this ctx on a Cartesian grid the tiled kernel supports, of at least 444 tiles (3 CTAs on each of the 148 SMs; ENT_OPT_STEP_IMPL = 3
+ * lifts this), and either both or neither carry tags; otherwise the call is exactly the two ent_step calls.  A tile is not split across CTAs here: meant for plasmas whose tile populations are of one order.
  * Results agree with two ent_step calls up to fp32 summation order of J. */
 int ent_step_pair(ent_ctx *ctx, const ent_fields *EB, ent_particles *p1, ent_particles *p2, ent_current *J, float dt);
 
@@ -260,7 +260,9 @@ int ent_step_host_pair(ent_ctx *ctx, const ent_fields *EB, ent_particles *p1, en
 /* ---- options and counters ----------------------------------------------------------------------------------- */
 enum {
     ENT_OPT_STEP_IMPL = 1,     /* 0 = auto (tiled when the block is the sorted one), 1 = force untiled, 2 = two-kernel
-                                  (gather_push to scratch copy + deposit; the paper's structure) */
+                                  (gather_push to scratch copy + deposit; the paper's structure), 3 = as 0, and ent_step_pair
+                                  takes its one-launch form on any grid (by default only on grids of at least 444 tiles: on a smaller
+                                  one a CTA per tile cannot fill the GPU and two work-list launches are faster) */
     ENT_OPT_TILE_1 = 2, ENT_OPT_TILE_2 = 3, ENT_OPT_TILE_3 = 4,   /* tile extents in cells; takes effect at the next ent_set_grid */
     ENT_OPT_PUSHER = 7,        /* momentum update of sub-step 5: 0 = relativistic Boris (default), 1 = Vay (2008); 2 = "Boris,GCA", 3 = "Vay,GCA":
                                   the hybrid pusher of P:976-980 with the thresholds of ent_set_gca.  Takes effect at once. */

@@ -48,7 +48,7 @@ struct ent_ctx {
     size_t side_bytes = 0;
     // the blocks ent_sort / ent_step_sorted produced: each keeps its own layout so that several species stay sorted at a time
     struct SortedBlock { const int32_t *cell = nullptr; long long n = -1; int32_t *tile_off = nullptr; float *tile_wmax = nullptr;
-                         int32_t *chunk_off = nullptr;      // work list of the tiled kernels (TILE_CHUNK particles per CTA)
+                         int32_t *chunk_off = nullptr;      // work list of the tiled kernels (tile_chunk_for(n) particles per CTA)
                          int32_t *next_count = nullptr;     // particles per tile by their CURRENT cell (layout of the next ent_step_sorted output)
                          bool wmax_valid = false, counts_valid = false; unsigned long long stamp = 0; };
     SortedBlock sorted[8];
@@ -155,6 +155,7 @@ static __device__ __align__(256) unsigned char compact_static_scratch[COMPACT_ST
 // In host code `compact_static_scratch` is a host-side stand-in, NOT a device address: the address the kernels get is looked up
 // once per device (that device current) with cudaGetSymbolAddress and kept here.
 constexpr int STATIC_MAX_DEVICES = 64;
+constexpr long long PAIR_MIN_TILES = 148 * 3;      // ent_step_pair: one CTA per tile needs at least one full wave of tiles
 static std::mutex static_scratch_mutex;
 static void *static_scratch_addr[STATIC_MAX_DEVICES] = {};
 static cudaError_t static_scratch_lookup(int device, void **ptr) {           // the caller has made `device` current
@@ -557,7 +558,7 @@ extern "C" int ent_step(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, en
     if (ctx->step_impl == 2) return step_two_kernel(ctx, EB, p, J, dt);
     float eps = 0.5f * (p->q / p->m) * dt;
     ent_ctx::SortedBlock *sb = find_block(ctx, p);
-    if (ctx->step_impl == 0 && sb && tiled_supported(ctx->tiled, ctx->g)) {
+    if ((ctx->step_impl == 0 || ctx->step_impl == 3) && sb && tiled_supported(ctx->tiled, ctx->g)) {
         if (!sb->wmax_valid) {                                   // a block ent_step_sorted produced: its per-tile max |w| was never needed
             tile_wmax_kernel<<<(unsigned)((long long)ctx->g.nt[0] * ctx->g.nt[1] * ctx->g.nt[2]), 128, 0, ctx->stream>>>(sb->tile_off, p->w, sb->tile_wmax);
             if ((rc = launch_check(ctx, "tile_wmax_kernel"))) return rc;
@@ -593,8 +594,11 @@ extern "C" int ent_step_pair(ent_ctx *ctx, const ent_fields *EB, ent_particles *
     if (!(p1->m != 0.f) || !(p2->m != 0.f)) return fail(ctx, ENT_EINVAL, "mass is zero");
     if (p1->n > 0 && p1->cell == p2->cell) return fail(ctx, ENT_EINVAL, "ent_step_pair: the two blocks are the same");
     ent_ctx::SortedBlock *s1 = find_block(ctx, p1), *s2 = find_block(ctx, p2);
-    const bool pairable = ctx->step_impl == 0 && s1 && s2 && p1->n > 0 && p2->n > 0 && ctx->g.kind == ENT_CART && tiled_supported(ctx->tiled, ctx->g) &&
-                          (p1->tag != nullptr) == (p2->tag != nullptr);
+    // one CTA per tile: worth it only when the tiles fill the GPU (148 SMs x 3 CTAs); smaller grids go through the work lists of two
+    // launches (tile_chunk_for), unless ENT_OPT_STEP_IMPL = 3 asks for the pair launch
+    const long long ntiles_pair = (long long)ctx->g.nt[0] * ctx->g.nt[1] * ctx->g.nt[2];
+    const bool pairable = (ctx->step_impl == 3 || (ctx->step_impl == 0 && ntiles_pair >= PAIR_MIN_TILES)) && s1 && s2 && p1->n > 0 && p2->n > 0 &&
+                          ctx->g.kind == ENT_CART && tiled_supported(ctx->tiled, ctx->g) && (p1->tag != nullptr) == (p2->tag != nullptr);
     if (!pairable) {                                             // the same result through two launches
         if ((rc = ent_step(ctx, EB, p1, J, dt))) return rc;
         return ent_step(ctx, EB, p2, J, dt);
@@ -636,11 +640,11 @@ static int exclusive_scan(ent_ctx *ctx, const int32_t *in, long long m, int32_t 
     return launch_check(ctx, "scan_apply_kernel");
 }
 
-// work list of a sorted block: exclusive scan of ceil(tile population / TILE_CHUNK).  Scratch: ctx->count, ctx->offsets (second
+// work list of a sorted block: exclusive scan of ceil(tile population / tile_chunk_for(n)), n = particles of the block.  Scratch: ctx->count, ctx->offsets (second
 // copy of the scan, unused), both idle between the phases of ent_sort / ent_step_sorted.
-static int build_work_lists(ent_ctx *ctx, ent_ctx::SortedBlock *slot, long long ntiles) {
+static int build_work_lists(ent_ctx *ctx, ent_ctx::SortedBlock *slot, long long ntiles, long long n) {
     int rc;
-    tile_chunks_kernel<<<nblk(ntiles), TPB, 0, ctx->stream>>>(slot->tile_off, ntiles, TILE_CHUNK, ctx->count);
+    tile_chunks_kernel<<<nblk(ntiles), TPB, 0, ctx->stream>>>(slot->tile_off, ntiles, tile_chunk_for(n), ctx->count);
     if ((rc = launch_check(ctx, "tile_chunks_kernel"))) return rc;
     return exclusive_scan(ctx, ctx->count, ntiles, slot->chunk_off, ctx->offsets);
 }
@@ -694,7 +698,7 @@ static int sort_rebin(ent_ctx *ctx, ent_ctx::SortedBlock *src, const ent_particl
                                                                             g.kind != ENT_CART, (unsigned *)slot->tile_wmax);
         if ((rc = launch_check(ctx, "rebin_scatter_kernel"))) return rc;
     }
-    if ((rc = build_work_lists(ctx, slot, ntiles))) return rc;
+    if ((rc = build_work_lists(ctx, slot, ntiles, in->n))) return rc;
     out->q = in->q; out->m = in->m;
     slot->cell = out->cell; slot->n = in->n; slot->stamp = ++ctx->sort_stamp; slot->wmax_valid = true; slot->counts_valid = true;
     ctx->last_sort_rebin = 1;
@@ -748,7 +752,7 @@ extern "C" int ent_sort(ent_ctx *ctx, const ent_particles *in, ent_particles *ou
         if ((rc = launch_check(ctx, "tile_offsets_kernel"))) return rc;
         tile_wmax_kernel<<<(unsigned)ntiles, 128, 0, ctx->stream>>>(slot->tile_off, out->w, slot->tile_wmax);
         if ((rc = launch_check(ctx, "tile_wmax_kernel"))) return rc;
-        if ((rc = build_work_lists(ctx, slot, ntiles))) return rc;
+        if ((rc = build_work_lists(ctx, slot, ntiles, n))) return rc;
         slot->cell = out->cell; slot->n = n; slot->stamp = ++ctx->sort_stamp; slot->wmax_valid = true; slot->counts_valid = true;
     }
     return ENT_OK;
@@ -857,10 +861,10 @@ extern "C" int ent_step_sorted(ent_ctx *ctx, const ent_fields *EB, const ent_par
     A.g = g; A.F = fp(EB); A.J = cp(J); A.in = pp(in); A.out = pp(out);
     A.tile_off = src->tile_off; A.chunk_off = src->chunk_off; A.tile_wmax = src->tile_wmax; A.cursor = ctx->cursor;
     A.next_count = dst->next_count; A.wmax_out = (unsigned *)dst->tile_wmax;
-    A.n = in->n; A.eps = 0.5f * (in->q / in->m) * dt; A.dt = dt; A.q = in->q; A.inv_dt = 1.0f / dt; A.counters = ctx->counters;
+    A.n = in->n; A.chunk = tile_chunk_for(in->n); A.eps = 0.5f * (in->q / in->m) * dt; A.dt = dt; A.q = in->q; A.inv_dt = 1.0f / dt; A.counters = ctx->counters;
     if ((rc = sorted_step(ctx->tiled, A, dt, ctx->stream, ctx->err, sizeof(ctx->err)))) return rc;
     ctx->launches += 1;
-    if ((rc = build_work_lists(ctx, dst, ntiles))) return rc;
+    if ((rc = build_work_lists(ctx, dst, ntiles, in->n))) return rc;
     dst->cell = out->cell; dst->n = in->n; dst->stamp = ++ctx->sort_stamp; dst->wmax_valid = true; dst->counts_valid = true;
     ctx->last_step_tiled = 1;
     return ENT_OK;
@@ -881,7 +885,7 @@ extern "C" int ent_set_option(ent_ctx *ctx, int key, int64_t value) {
     if (!ctx) return ENT_EINVAL;
     switch (key) {
         case ENT_OPT_STEP_IMPL:
-            if (value < 0 || value > 2) return fail(ctx, ENT_EINVAL, "ENT_OPT_STEP_IMPL must be 0, 1 or 2");
+            if (value < 0 || value > 3) return fail(ctx, ENT_EINVAL, "ENT_OPT_STEP_IMPL must be 0, 1, 2 or 3");
             ctx->step_impl = (int)value; return ENT_OK;
         case ENT_OPT_SORT_MODE:
             if (value < 0 || value > 2) return fail(ctx, ENT_EINVAL, "ENT_OPT_SORT_MODE must be 0, 1 or 2");

@@ -7,7 +7,7 @@
 // populations per tile of the NEW positions are counted on the way (next_count), so the next call knows its output layout
 // before it starts, and the per-tile max |w| of the output ranges is maintained.  No sort pass ever runs between steps.
 //
-// A CTA works on one chunk (<= TILE_CHUNK particles) of one tile, streaming: one particle per thread and iteration straight
+// A CTA works on one chunk (<= tile_chunk_for(n) particles) of one tile, streaming: one particle per thread and iteration straight
 // from global memory (consecutive lanes on consecutive particles, next record requested before the current one is advanced).
 //   * slot in `out`: particles that stay in the tile (~87 %) take consecutive slots from ONE global reservation per warp and
 //     iteration (ballot), the others one reservation each; the atomics are issued right after the cell index is decoded and
@@ -34,7 +34,8 @@ struct SortedArgs {
     CurrentPtrs J;
     PartPtrs in, out;
     const int32_t *tile_off;      // layout of `in`: tile t owns particles [tile_off[t], tile_off[t+1])
-    const int32_t *chunk_off;     // work list of `in` (chunks of TILE_CHUNK particles)
+    const int32_t *chunk_off;     // work list of `in` (chunks of tile_chunk_for(n) particles)
+    int chunk;
     const float *tile_wmax;       // max |w| per range of `in`
     int32_t *cursor;              // per tile: next free slot of its range in `out` (starts at the out layout's offsets)
     int32_t *next_count;          // per tile: particles whose cell AFTER this step lies in it (layout of the next step's output)
@@ -154,8 +155,8 @@ step_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     }
 
     long long p0 = A.tile_off[tile], p1 = A.tile_off[tile + 1];
-    p0 += (long long)(blockIdx.x - A.chunk_off[tile]) * TILE_CHUNK;
-    if (p1 > p0 + TILE_CHUNK) p1 = p0 + TILE_CHUNK;
+    p0 += (long long)(blockIdx.x - A.chunk_off[tile]) * A.chunk;
+    if (p1 > p0 + A.chunk) p1 = p0 + A.chunk;
     TileCtx<D> T;
     T.sF = sF; T.sJ = sJ;
     T.o[0] = o[0]; T.o[1] = o[1]; T.o[2] = o[2];
@@ -351,7 +352,7 @@ inline int sorted_launch(TiledState &t, int attr_slot, const SortedArgs &A, cuda
         if (e != cudaSuccess) { snprintf(err, errn, "cudaFuncSetAttribute(smem %d) failed: %s", G::SMEM_BYTES, cudaGetErrorString(e)); return ENT_ECUDA; }
         t.attr_set[slot] = true;
     }
-    const long long grid = (long long)A.ntiles + A.n / TILE_CHUNK + 1;        // upper bound of the number of chunks
+    const long long grid = (long long)A.ntiles + A.n / A.chunk + 1;        // upper bound of the number of chunks
     kern<<<(unsigned)grid, FUSED_TPB, G::SMEM_BYTES, stream>>>(t.maps, A);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { snprintf(err, errn, "launch of step_fused_kernel failed: %s", cudaGetErrorString(e)); return ENT_ECUDA; }

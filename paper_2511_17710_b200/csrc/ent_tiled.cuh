@@ -1,6 +1,6 @@
 // ent_tiled.cuh -- tiled fused step for the Cartesian grids (sub-steps 3-8), sm_100a.
 //
-// A CTA works on one tile of TX x TY x TZ cells (a tile with more than TILE_CHUNK particles is shared by several CTAs: work
+// A CTA works on one tile of TX x TY x TZ cells (a tile with more than tile_chunk_for(n) particles is shared by several CTAs: work
 // list built by ent_sort).  The block handed to ent_step is the one ent_sort produced, so the particles of a tile are one
 // contiguous range of the SoA arrays (tile-major key, ent.h).
 //   * E,B: the tile's box of the six padded planar arrays, [o-2, o+T+2) per dimension, lands in shared memory by
@@ -124,12 +124,13 @@ struct TiledArgs {
     PartPtrs P;
     const int32_t *key_off;       // tile offsets: tile t owns particles [key_off[t], key_off[t+1]) (ent_sort)
     const float *tile_wmax;       // max |w| over the particles of each tile (ent_sort)
-    const int32_t *chunk_off;     // work list: tile t is processed by CTAs [chunk_off[t], chunk_off[t+1]), TILE_CHUNK particles each
+    const int32_t *chunk_off;     // work list: tile t is processed by CTAs [chunk_off[t], chunk_off[t+1]), tile_chunk_for(n) particles each
     int ntiles;
     long long n;
     float eps, dt, q, inv_dt;
     float cdt[3];                 // dt / dx_d
     // second species of a pair launch (ent_step_pair): same tile geometry, its own block, layout, charge and q/m
+    int chunk;                    // particles per CTA of the work list (tile_chunk_for(n))
     int nsp;                      // 1, or 2: one CTA per tile advances both blocks through one E,B box and one J tile
     PartPtrs P2; const int32_t *key_off2; const float *tile_wmax2; float eps2, q2;
     unsigned long long *counters; // [0] bad moves, [1] strays, [2] length of stray_list, [4] carries of the fixed-point J tile
@@ -290,7 +291,14 @@ __device__ __forceinline__ void tile_deposit(int *sJ, const CarryCtx &cc, const 
 #define ENT_TILED_TPB 256
 #endif
 constexpr int TILED_TPB = ENT_TILED_TPB;
-constexpr int TILE_CHUNK = 4096;              // particles per CTA: a heavy tile is shared by several CTAs, each with its own J tile
+constexpr int TILE_CHUNK_MAX = 4096;          // particles per CTA: a heavy tile is shared by several CTAs, each with its own J tile
+// The chunk of a block of n particles: 4096 for the large blocks (per-tile prologue and flush amortised over 16 particles per thread),
+// smaller for small blocks so that the launch still fills the 148 SMs a few times over (a 64^2 grid has 16 tiles).  A function of n
+// alone: the work list (ent_sort) and the launches that use it agree without carrying the value.
+inline int tile_chunk_for(long long n) {
+    long long c = (n / (148LL * 3 * 4) + 255) / 256 * 256;
+    return (int)(c < 512 ? 512 : c > TILE_CHUNK_MAX ? TILE_CHUNK_MAX : c);
+}
 
 // work-list lookup: the tile whose chunk range contains CTA `vb` (binary search in the exclusive scan), or -1
 __device__ __forceinline__ int find_tile(const int32_t *chunk_off, int ntiles, int vb) {
@@ -432,7 +440,7 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     const GridDev &g = A.g;
     const int tid = threadIdx.x;
 
-    // pair launch: one CTA per tile, whole ranges of both blocks; otherwise the work list (chunks of TILE_CHUNK particles)
+    // pair launch: one CTA per tile, whole ranges of both blocks; otherwise the work list (chunks of tile_chunk_for(n) particles)
     const int tile = PAIR ? (int)blockIdx.x : find_tile(A.chunk_off, A.ntiles, blockIdx.x);
     if (tile < 0) return;                                        // the grid is an upper bound of the work list
     const int t0 = tile % g.nt[0], t12 = tile / g.nt[0];
@@ -500,8 +508,8 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     const int32_t *koff = (PAIR && sp) ? A.key_off2 : A.key_off;
     long long p0 = koff[tile], p1 = koff[tile + 1];
     if (!PAIR) {
-        p0 += (long long)(blockIdx.x - A.chunk_off[tile]) * TILE_CHUNK;
-        if (p1 > p0 + TILE_CHUNK) p1 = p0 + TILE_CHUNK;
+        p0 += (long long)(blockIdx.x - A.chunk_off[tile]) * A.chunk;
+        if (p1 > p0 + A.chunk) p1 = p0 + A.chunk;
     }
     long long p = p0 + tid;
     int ncell = 0; float nd0 = 0.f, nd1 = 0.f, nd2 = 0.f, nu0 = 0.f, nu1 = 0.f, nu2 = 0.f, nw = 0.f; bool nlive = true;
@@ -663,7 +671,7 @@ inline int tiled_launch(TiledState &t, const TiledArgs &A, cudaStream_t stream, 
         t.attr_set[slot] = true;
     }
     const int ntiles = A.g.nt[0] * A.g.nt[1] * A.g.nt[2];
-    const long long grid = A.nsp == 2 ? (long long)ntiles : (long long)ntiles + A.n / TILE_CHUNK + 1;        // upper bound of the number of chunks
+    const long long grid = A.nsp == 2 ? (long long)ntiles : (long long)ntiles + A.n / A.chunk + 1;        // upper bound of the number of chunks
     kern<<<(unsigned)grid, TILED_TPB, smem_bytes, stream>>>(t.maps, A);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { snprintf(err, errn, "launch of step_tiled_kernel failed: %s", cudaGetErrorString(e)); return ENT_ECUDA; }
@@ -679,7 +687,7 @@ inline int tiled_step(TiledState &t, const GridDev &g, cudaStream_t stream, Fiel
                       const int32_t *key_off, const float *tile_wmax, const int32_t *chunk_off, float eps, float dt, float q, float inv_dt, unsigned long long *counters,
                       long long *launches, char *err, size_t errn, const PairSpecies *pair = nullptr) {
     TiledArgs A;
-    A.g = g; A.F = F; A.J = J; A.P = P; A.key_off = key_off; A.tile_wmax = tile_wmax; A.chunk_off = chunk_off; A.ntiles = g.nt[0] * g.nt[1] * g.nt[2]; A.n = n;
+    A.g = g; A.F = F; A.J = J; A.P = P; A.key_off = key_off; A.tile_wmax = tile_wmax; A.chunk_off = chunk_off; A.ntiles = g.nt[0] * g.nt[1] * g.nt[2]; A.n = n; A.chunk = tile_chunk_for(n);
     A.eps = eps; A.dt = dt; A.q = q; A.inv_dt = inv_dt; A.counters = counters;
     A.nsp = 1; A.P2 = P; A.key_off2 = key_off; A.tile_wmax2 = tile_wmax; A.eps2 = eps; A.q2 = q;
     if (pair) { A.nsp = 2; A.P2 = pair->P; A.key_off2 = pair->key_off; A.tile_wmax2 = pair->tile_wmax; A.eps2 = pair->eps; A.q2 = pair->q; }

@@ -128,8 +128,8 @@ step_tiled_axisym_kernel(const __grid_constant__ TileMaps maps, const __grid_con
     for (int k = tid; k < X::JWORDS / 4; k += TILED_TPB) reinterpret_cast<int4 *>(sJ)[k] = make_int4(0, 0, 0, 0);
 
     long long p0 = A.key_off[tile], p1 = A.key_off[tile + 1];
-    p0 += (long long)(blockIdx.x - A.chunk_off[tile]) * TILE_CHUNK;
-    if (p1 > p0 + TILE_CHUNK) p1 = p0 + TILE_CHUNK;
+    p0 += (long long)(blockIdx.x - A.chunk_off[tile]) * A.chunk;
+    if (p1 > p0 + A.chunk) p1 = p0 + A.chunk;
     float Sc, invSc;
     {   // fixed-point scale of this CTA's J tile.  A contribution is q w / dt * D * weight with |D_a| <= dt / sqrt(h_aa) (|v| < 1), i.e.
         // at most |q| wmax / min sqrt(h_aa) over the tile (x 13/12); bounding |D| by 1 instead would waste ~10 bits on the

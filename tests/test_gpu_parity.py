@@ -522,8 +522,9 @@ def test_compact_matches_oracle(env, name):
     assert bind.ent_get_stat(ctx, bind.STAT_LAST_STEP_TILED) == 1
 
 
+@pytest.mark.parametrize("forced", [True, False])
 @pytest.mark.parametrize("name", ["C1", "C3/8", "C3/8-uneven", "C4/16-shuffled", "ABS3", "ABS2", "PER3"])
-def test_step_pair_matches_oracle(env, name):
+def test_step_pair_matches_oracle(env, name, forced):
     """ent_step_pair: both species of the pair plasma through one launch of the tiled kernel (one E,B box, one J tile per tile).
     Same bars as the single-species tests: the summed current of the two species against the oracle's, particles per species,
     continuity of the GPU's own output; blocks re-binned every 3 steps."""
@@ -537,7 +538,8 @@ def test_step_pair_matches_oracle(env, name):
                                       u=[t[keep] for t in sp.u], w=7.3 * sp.w[keep])
     g = wl.grid
     eg, og = P.grid_to_ent(bind, g), P.grid_to_orc(orc, g)
-    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, 0)
+    # these grids have fewer than 444 tiles: ENT_OPT_STEP_IMPL = 3 asks for the one-launch form, 0 takes two work-list launches
+    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, 3 if forced else 0)
     bind.ent_set_grid(ctx, eg)
     F_dev, F_orc = [f.cuda() for f in wl.fields], P.fields_to_orc(wl.fields)
     assert len(wl.species) == 2
@@ -588,4 +590,5 @@ def test_step_pair_matches_oracle(env, name):
         assert st["tag_mismatch"] == 0
     assert bind.ent_get_stat(ctx, bind.STAT_BAD_MOVES) == 0
     print(name, "pair: max|dJ|/max|J| =", worstJ, " continuity", worstC)
+    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, 0)
     assert worstJ <= P.J_TOL
