@@ -249,7 +249,7 @@ int ent_fill_field_ghosts(ent_ctx *ctx, ent_fields_rw *EB);
 int ent_step_host(ent_ctx *ctx, const ent_fields *EB, ent_particles *p, ent_current *J, float dt, int nsteps,
                   int64_t *h2d_bytes, int64_t *d2h_bytes);
 
-/* The same for the two species of a pair plasma in one call, pipelined over three streams: each block is cut into four sub-blocks
+/* The same for the two species of a pair plasma in one call, pipelined over three streams: each block is cut into eight sub-blocks
  * (consecutive quarters of its arrays) that are uploaded, sorted and advanced, and downloaded independently, so that the transfers
  * of neighbouring sub-blocks overlap the work and each other (the link is full duplex); E,B go up once, J (the sum of both species)
  * comes back once.  Every pointer is a HOST pointer (pinned memory: pageable memory serialises the copies).  Both blocks come back

@@ -1004,7 +1004,7 @@ extern "C" int ent_step_host(ent_ctx *ctx, const ent_fields *EB, ent_particles *
 // sub-blocks (particles are independent; J accumulates): while one sub-block is sorted and advanced, the next ones are still arriving
 // over PCIe and the previous ones are already on their way back (the link is full duplex), so the call takes about the time of
 // the larger of the two transfers plus one sub-block's work.  Fields go up once, J comes back once.
-constexpr int HOST_CHUNKS = 4;
+constexpr int HOST_CHUNKS = 8;
 extern "C" int ent_step_host_pair(ent_ctx *ctx, const ent_fields *EB, ent_particles *p1, ent_particles *p2, ent_current *J, float dt, int nsteps,
                                   int64_t *h2d_bytes, int64_t *d2h_bytes) {
     ENTER();
