@@ -699,6 +699,7 @@ static int sort_rebin(ent_ctx *ctx, ent_ctx::SortedBlock *src, const ent_particl
         if ((rc = launch_check(ctx, "rebin_scatter_kernel"))) return rc;
     }
     if ((rc = build_work_lists(ctx, slot, ntiles, in->n))) return rc;
+    if (!in->tag && out->tag) CK(cudaMemsetAsync(out->tag, 1, (size_t)in->n, ctx->stream));       // as in the full sort: every particle is alive
     out->q = in->q; out->m = in->m;
     slot->cell = out->cell; slot->n = in->n; slot->stamp = ++ctx->sort_stamp; slot->wmax_valid = true; slot->counts_valid = true;
     ctx->last_sort_rebin = 1;

@@ -357,6 +357,35 @@ def test_rebin_tile_offsets_are_the_scan_of_the_tile_histogram(env, name):
     assert orc.sort_check(tile_keys, ntiles, toff) == 0, "re-binned block / tile offsets rejected by orc_sort_check"
 
 
+def test_sort_into_a_block_with_tags_from_one_without_marks_every_particle_alive(env):
+    """ent.h (ent_sort): `in` without a tag array and `out` with one -> every particle of `out` is alive.  Both forms of the sort: the
+    full counting sort and, from the sorted block after a few steps, the incremental re-bin."""
+    bind, synth, ctx, orc = env
+    wl = _workloads(synth)["C3/8"]()
+    g = wl.grid
+    eg = P.grid_to_ent(bind, g)
+    bind.ent_set_option(ctx, bind.OPT_STEP_IMPL, 0)
+    bind.ent_set_option(ctx, bind.OPT_SORT_MODE, 0)
+    bind.ent_set_grid(ctx, eg)
+    F = [f.cuda() for f in wl.fields]
+    J = bind.zeros_current(eg, "cuda")
+    src = P.species_to_ent(bind, synth, g, wl.species[0], "cuda", with_tag=False)
+    mk = lambda: bind.Particles(cell=torch.empty_like(src.cell), d=[torch.empty_like(t) for t in src.d], u=[torch.empty_like(t) for t in src.u],
+                                w=torch.empty_like(src.w), phi=None, tag=torch.full((src.n,), 7, dtype=torch.uint8, device="cuda"), q=src.q, m=src.m)
+    a = mk()
+    bind.ent_sort(ctx, src, a, None)                      # full sort
+    torch.cuda.synchronize()
+    assert bind.ent_get_stat(ctx, bind.STAT_LAST_SORT_REBIN) == 0 and bool((a.tag == 1).all())
+    notag = bind.Particles(cell=a.cell, d=a.d, u=a.u, w=a.w, phi=None, tag=None, q=a.q, m=a.m)      # the same sorted block, seen without tags
+    for _ in range(3):
+        bind.ent_step(ctx, F, notag, J, wl.dt)
+    b = mk()
+    bind.ent_sort(ctx, notag, b, None)                    # re-bin
+    torch.cuda.synchronize()
+    assert bind.ent_get_stat(ctx, bind.STAT_LAST_SORT_REBIN) == 1 and bool((b.tag == 1).all())
+    _match_perm(g, bind.Particles(cell=a.cell, d=a.d, u=a.u, w=a.w, phi=None, tag=b.tag, q=a.q, m=a.m), b)
+
+
 def test_empty_block_is_accepted(env):
     """n = 0: every call returns ENT_OK and touches nothing (ent.h: n may be any value >= 0)"""
     bind, synth, ctx, orc = env
