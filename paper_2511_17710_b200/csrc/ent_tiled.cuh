@@ -336,7 +336,6 @@ struct TileCtx {
     const float *sF;      // [6][FNP] E,B box
     int *sJ;              // [3][JNP] fixed-point J tile
     int o[3];             // tile origin (active cell coordinates)
-    int corner;           // linear index of the box corner o - 2 (inner tiles)
     float sx[3];          // sqrt(h_ii) = cell sizes
     float Sc;             // fixed-point scale of this tile
     float wguard;         // weights above this deposit through the global path (contribution would not fit 2^30)
@@ -346,10 +345,7 @@ struct TileCtx {
 // One particle through sub-steps 3-8 inside a tile.  cell, d[], u[] are updated in place.
 // Returns 0: advanced (write the record back), 1: taken by the global path (already written), 2: advanced and left
 // through an ABSORB side (write back, tag = 0), 3: dead or not ours (untouched).
-// INNER: the tile's box [o - 2, o + T + 2) lies inside the grid in every dimension (CTA-uniform; 82 % of the tiles of a 256^3 grid):
-// no particle of the range can wrap or touch the edge of the padded arrays, so box coordinates come straight from the linear
-// index relative to the box corner and the new cell is the old one plus the crossing increments.
-template <int D, int TX, int TY, int TZ, bool ALLPER, bool INNER, bool PAIR>
+template <int D, int TX, int TY, int TZ, bool ALLPER, bool PAIR>
 __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D> &T, long long p, int &cell, float d[3], float u[3],
                                              float wgt, float q, float eps, int sp) {
     using G = TileGeom<D, TX, TY, TZ>;
@@ -358,15 +354,7 @@ __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D
     int i[3] = { 0, 0, 0 }, b[3];
     const int TT[3] = { TX, TY, TZ };
     bool local = true, edge = false;
-    if (INNER) {
-        const int rel = cell - T.corner;                                  // b0 + N0 (b1 + N1 b2) for a cell inside the box
-        local = rel >= 0;
-        const int rr = local ? rel : 0;
-        if (D == 2) { b[1] = A.divN0.div(rr); b[0] = rr - b[1] * g.N[0]; b[2] = 0; }
-        else { b[2] = A.divN01.div(rr); int r = rr - b[2] * (g.N[0] * g.N[1]); b[1] = A.divN0.div(r); b[0] = r - b[1] * g.N[0]; }
-#pragma unroll
-        for (int a = 0; a < D; ++a) local &= (unsigned)(b[a] - 1) < (unsigned)(TT[a] + 2);
-    } else {
+    {
         if (D == 2) { i[1] = A.divN0.div(cell); i[0] = cell - i[1] * g.N[0]; i[2] = 0; }
         else { i[2] = A.divN01.div(cell); int r = cell - i[2] * (g.N[0] * g.N[1]); i[1] = A.divN0.div(r); i[0] = r - i[1] * g.N[0]; }
         b[0] = i[0] - T.o[0] + 2; b[1] = i[1] - T.o[1] + 2; b[2] = (D == 3) ? i[2] - T.o[2] + 2 : 0;
@@ -382,7 +370,7 @@ __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D
         }
     }
     // the true old cell (needed by the global-path deposit only)
-    const int iold[3] = { INNER ? T.o[0] - 2 + b[0] : i[0], INNER ? T.o[1] - 2 + b[1] : i[1], INNER ? ((D == 3) ? T.o[2] - 2 + b[2] : 0) : i[2] };
+    const int iold[3] = { i[0], i[1], i[2] };
     if (!local) {
         if (PAIR) stray_step<D>(A, p, sp);         // pair launch: the stray list does not record the species
         else defer_stray(A, p, [&] { stray_step<D>(A, p); });
@@ -402,7 +390,6 @@ __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D
     for (int a = 0; a < D; ++a) {
         float x = d[a] + (u[a] * ig) * A.cdt[a];
         split_offset(x, di[a], d[a]);
-        if (INNER) continue;
         int in = i[a] + di[a];
         const int wrapN = (ALLPER || g.bc[a] == ENT_PERIODIC) ? g.N[a] : 0;
         in += (in < 0) ? wrapN : 0;
@@ -410,8 +397,7 @@ __device__ __forceinline__ int tile_particle(const TiledArgs &A, const TileCtx<D
         if (!ALLPER) { if (in < 0) { alive = false; in = 0; } if (in >= g.N[a]) { alive = false; in = g.N[a] - 1; } }
         i[a] = in;
     }
-    if (INNER) cell += di[0] + g.N[0] * (di[1] + ((D == 3) ? g.N[1] * di[2] : 0));
-    else cell = (D == 2) ? i[0] + g.N[0] * i[1] : i[0] + g.N[0] * (i[1] + g.N[1] * i[2]);
+    cell = (D == 2) ? i[0] + g.N[0] * i[1] : i[0] + g.N[0] * (i[1] + g.N[1] * i[2]);
     if (!alive) return 2;
     bool bad = false;
 #pragma unroll
@@ -448,13 +434,6 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
     TileCtx<D> T;
     T.sF = sF; T.sJ = sJ;
     T.o[0] = t0 * TX; T.o[1] = t1 * TY; T.o[2] = t2 * TZ;
-    bool inner = ALLPER;
-    {
-        const int TT[3] = { TX, TY, TZ };
-#pragma unroll
-        for (int a = 0; a < D; ++a) inner &= T.o[a] >= 2 && T.o[a] + TT[a] + 2 <= g.N[a];
-    }
-    T.corner = (T.o[0] - 2) + g.N[0] * ((T.o[1] - 2) + ((D == 3) ? g.N[1] * (T.o[2] - 2) : 0));
     T.sx[0] = g.dx[0]; T.sx[1] = g.dx[1]; T.sx[2] = g.dx[2];
 
     if (tid == 0) {
@@ -530,8 +509,7 @@ step_tiled_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__
         }
         if (!waited) { mbar_wait(&bar, 0); waited = true; }
         if (!live) continue;
-        const int code = inner ? tile_particle<D, TX, TY, TZ, ALLPER, true, PAIR>(A, T, p, cell, d, u, wgt, q, eps, sp)
-                               : tile_particle<D, TX, TY, TZ, ALLPER, false, PAIR>(A, T, p, cell, d, u, wgt, q, eps, sp);
+        const int code = tile_particle<D, TX, TY, TZ, ALLPER, PAIR>(A, T, p, cell, d, u, wgt, q, eps, sp);
         if (code & 1) continue;
         P.cell[p] = cell;
         P.d[0][p] = d[0]; P.d[1][p] = d[1]; if (D == 3) P.d[2][p] = d[2];
